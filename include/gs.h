@@ -47,9 +47,10 @@ typedef enum {
   GS_E_ORDER = -2,    /* call sequence violated (e.g. gs_rasterize_bwd before gs_rasterize_fwd) */
   GS_E_CUDA = -3,     /* a CUDA runtime call failed; text in gs_last_error */
   GS_E_NOMEM = -4,    /* growing the scratch failed */
-  GS_E_OVERFLOW = -5  /* the tile-instance capacity was exceeded by an EARLIER asynchronous iteration: its outputs are
-                         invalid (image = background, gradients = 0).  The context has grown; re-issue from
-                         gs_preprocess. */
+  GS_E_OVERFLOW = -5  /* the tile-instance capacity was exceeded by an asynchronous iteration: that iteration's outputs
+                         are invalid (image = background, gradients = 0).  Reported once, by the first of
+                         gs_preprocess / gs_bin_tiles / gs_poll / gs_get_counts to notice; the context has already
+                         grown when it is returned: re-issue the iteration from gs_preprocess. */
 } gs_status;
 
 /* Pinhole camera + world-to-camera pose, p_c = R p_w + t.  HOST struct. */
@@ -134,6 +135,19 @@ GS_API int gs_get_features(gs_ctx* ctx, void* stream, double* mean2d, float* con
                     uint32_t* depth_key, int32_t* rect);
 /* Non-blocking: GS_E_OVERFLOW if an earlier asynchronous iteration overflowed the instance capacity, else GS_OK. */
 GS_API int gs_poll(gs_ctx* ctx);
+
+/* Stage timing.  gs_profile_enable(ctx, 1) makes the five calls record CUDA events on their stream around each kernel
+ * group; gs_profile_read waits for the last gs_pose_grad and returns the device time in milliseconds of the
+ * GS_NUM_STAGES groups of the last iteration: preprocess, scan+duplicate, radix sort, tile ranges, raster forward,
+ * raster backward (pixel part), per-Gaussian backward, pose gradient.  HOST float[GS_NUM_STAGES]. */
+#define GS_NUM_STAGES 8
+GS_API int gs_profile_enable(gs_ctx* ctx, int on);
+GS_API int gs_profile_read(gs_ctx* ctx, float* ms);
+/* Number of CUDA kernels this context has launched so far (HOST counter). */
+GS_API int gs_get_launch_count(gs_ctx* ctx, uint64_t* n);
+/* Workload of the last forward (SYNCHRONISES): HOST uint64[4] = { evaluated (pixel, Gaussian) pairs with per-pixel
+ * exit, blended pairs, sum over pixels of the last blended list position, sum over tiles of list length * pixels }. */
+GS_API int gs_get_workload(gs_ctx* ctx, void* stream, uint64_t* out);
 
 /* ---- auxiliary kernels outside the five-call contract (losses of configs 2 and 4, on-device pose step) ---------- */
 /* grad[i] = weight * sign(pred[i] - target[i])   (d/dpred of weight * |pred - target|; sign(0) = 0) */

@@ -21,7 +21,9 @@ STATUS = {0: "GS_OK", -1: "GS_E_INVALID", -2: "GS_E_ORDER", -3: "GS_E_CUDA", -4:
 
 EXPORTS = ["gs_create", "gs_destroy", "gs_last_error", "gs_preprocess", "gs_bin_tiles", "gs_rasterize_fwd",
            "gs_rasterize_bwd", "gs_pose_grad", "gs_get_counts", "gs_get_binning", "gs_get_features", "gs_poll",
-           "gs_aux_l1_grad", "gs_aux_pose_step", "gs_fwd_bwd_host"]
+           "gs_aux_l1_grad", "gs_aux_pose_step", "gs_fwd_bwd_host", "gs_profile_enable", "gs_profile_read",
+           "gs_get_launch_count", "gs_get_workload"]
+STAGES = ["preprocess", "scan_dup", "radix_sort", "tile_ranges", "raster_fwd", "raster_bwd", "gauss_bwd", "pose_grad"]
 
 
 class GsError(RuntimeError):
@@ -60,6 +62,10 @@ def load_library():
     lib.gs_poll.argtypes = [vp]
     lib.gs_aux_l1_grad.argtypes = [vp, i64, vp, vp, f, vp]
     lib.gs_aux_pose_step.argtypes = [vp, vp, vp, f]
+    lib.gs_profile_enable.argtypes = [vp, C.c_int]
+    lib.gs_profile_read.argtypes = [vp, C.POINTER(f * 8)]
+    lib.gs_get_launch_count.argtypes = [vp, C.POINTER(C.c_uint64)]
+    lib.gs_get_workload.argtypes = [vp, vp, C.POINTER(C.c_uint64 * 4)]
     lib.gs_fwd_bwd_host.argtypes = [vp, vp, i64, C.c_int, vp, vp, vp, vp, vp, C.POINTER(gs_camera), C.POINTER(f * 3)] + [vp] * 11
     for name in EXPORTS:
         if name != "gs_last_error":
@@ -204,6 +210,24 @@ class Context:
 
     def gs_poll(self):
         self._check(self.lib.gs_poll(self._h))
+
+    def gs_profile_enable(self, on: bool):
+        self._check(self.lib.gs_profile_enable(self._h, int(bool(on))))
+
+    def gs_profile_read(self) -> dict:
+        ms = (C.c_float * 8)()
+        self._check(self.lib.gs_profile_read(self._h, C.byref(ms)))
+        return {k: float(ms[i]) for i, k in enumerate(STAGES)}
+
+    def gs_get_launch_count(self) -> int:
+        n = C.c_uint64(0)
+        self._check(self.lib.gs_get_launch_count(self._h, C.byref(n)))
+        return int(n.value)
+
+    def gs_get_workload(self, stream=None) -> dict:
+        w = (C.c_uint64 * 4)()
+        self._check(self.lib.gs_get_workload(self._h, _stream(stream), C.byref(w)))
+        return dict(evaluated=int(w[0]), blended=int(w[1]), last_pos_sum=int(w[2]), list_len_x_pixels=int(w[3]))
 
     # -- host-buffer path (numpy arrays in / out; copies inside) ---------------------------------------------------
     def gs_fwd_bwd_host(self, scene_arrays, sh_degree, cam, bg, d_rgb, d_depth, out, stream=None):

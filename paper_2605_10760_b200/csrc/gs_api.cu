@@ -152,6 +152,7 @@ int gs_destroy(gs_ctx* ctx) {
   cudaFree(ctx->ranges); cudaFree(ctx->final_T); cudaFree(ctx->n_contrib);
   cudaFree(ctx->pose_acc); cudaFree(ctx->counts); cudaFree(ctx->hb);
   if (ctx->mailbox) cudaFreeHost(ctx->mailbox);
+  if (ctx->ev_made) for (int k = 0; k < 13; ++k) cudaEventDestroy(ctx->ev[k]);
   cudaGetLastError();
   delete ctx;
   return GS_OK;
@@ -161,8 +162,7 @@ const char* gs_last_error(const gs_ctx* ctx) { return ctx ? ctx->err : "null con
 
 int gs_poll(gs_ctx* ctx) {
   if (!ctx) return GS_E_INVALID;
-  const Counts mb = read_mailbox(ctx);
-  if (mb.overflow || ctx->overflow_pending) return fail(ctx, GS_E_OVERFLOW, "tile-instance capacity exceeded in an earlier iteration");
+  if (handle_overflow(ctx)) return fail(ctx, GS_E_OVERFLOW, "tile-instance capacity exceeded in an earlier iteration; scratch has grown, re-issue");
   return GS_OK;
 }
 
@@ -177,10 +177,7 @@ int gs_preprocess(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, const flo
   if (((uintptr_t)quats & 15) != 0) return fail(ctx, GS_E_INVALID, "gs_preprocess: quats must be 16-byte aligned");
   cudaStream_t s = (cudaStream_t)stream;
   GS_CUDA(cudaSetDevice(ctx->device));
-  if (ctx->overflow_pending) {
-    ctx->overflow_pending = false;
-    return fail(ctx, GS_E_OVERFLOW, "tile-instance capacity exceeded in an earlier iteration; scratch has grown, re-issue");
-  }
+  if (handle_overflow(ctx)) return fail(ctx, GS_E_OVERFLOW, "tile-instance capacity exceeded in an earlier iteration; scratch has grown, re-issue");
   int rc;
   if ((rc = ensure_gaussian_capacity(ctx, N)) != GS_OK) return rc;
   DevCam& c = ctx->cam;
@@ -193,8 +190,10 @@ int gs_preprocess(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, const flo
   ctx->N = N; ctx->sh_degree = sh_degree;
   ctx->means = means; ctx->scales = scales; ctx->quats = quats; ctx->opacities = opacities; ctx->sh = sh;
   ctx->seq++;
+  GS_PROF(0, s);
   GS_CUDA(cudaMemsetAsync(ctx->counts, 0, sizeof(Counts), s));
   if ((rc = launch_preprocess(ctx, s)) != GS_OK) return rc;
+  GS_PROF(1, s);
   ctx->stage = 1;
   ctx->pose_acc_valid = false;
   return GS_OK;
@@ -207,10 +206,6 @@ int gs_bin_tiles(gs_ctx* ctx, void* stream) {
   int rc = launch_binning(ctx, (cudaStream_t)stream);
   if (rc != GS_OK) return rc;
   ctx->stage = 2;
-  if (ctx->overflow_pending) {
-    ctx->overflow_pending = false;
-    return fail(ctx, GS_E_OVERFLOW, "tile-instance capacity exceeded in an earlier iteration; scratch has grown, re-issue");
-  }
   return GS_OK;
 }
 
@@ -219,8 +214,10 @@ int gs_rasterize_fwd(gs_ctx* ctx, void* stream, const float* bg, float* rgb, flo
   if (ctx->stage < 2) return fail(ctx, GS_E_ORDER, "gs_rasterize_fwd before gs_bin_tiles");
   GS_CUDA(cudaSetDevice(ctx->device));
   for (int k = 0; k < 3; ++k) ctx->bg[k] = bg ? bg[k] : 0.f;
+  GS_PROF(6, (cudaStream_t)stream);
   int rc = launch_raster_fwd(ctx, (cudaStream_t)stream, rgb, depth, alpha);
   if (rc != GS_OK) return rc;
+  GS_PROF(7, (cudaStream_t)stream);
   ctx->stage = 3;
   return GS_OK;
 }
@@ -239,11 +236,14 @@ int gs_rasterize_bwd(gs_ctx* ctx, void* stream, const float* d_rgb, const float*
   if (ctx->g2d_dirty && ctx->N > 0) GS_CUDA(cudaMemsetAsync(ctx->g2d, 0, (size_t)ctx->N * kG2D * sizeof(float), s));
   ctx->g2d_dirty = true;
   ctx->pose_acc_valid = false;
+  GS_PROF(8, s);
   int rc = launch_raster_bwd(ctx, s, d_rgb, d_depth, d_alpha);
   if (rc != GS_OK) return rc;
+  GS_PROF(9, s);
   if (write) {
     if ((rc = launch_gauss_bwd(ctx, s, flags, g_means, g_scales, g_quats, g_opacities, g_sh)) != GS_OK) return rc;
   }
+  GS_PROF(10, s);
   ctx->stage = 4;
   return GS_OK;
 }
@@ -255,10 +255,13 @@ int gs_pose_grad(gs_ctx* ctx, void* stream, uint32_t flags, float* g_twist) {
   cudaStream_t s = (cudaStream_t)stream;
   GS_CUDA(cudaSetDevice(ctx->device));
   int rc;
+  GS_PROF(11, s);
   if (!ctx->pose_acc_valid) {
     if ((rc = launch_gauss_bwd(ctx, s, GS_POSE_ONLY, nullptr, nullptr, nullptr, nullptr, nullptr)) != GS_OK) return rc;
   }
-  return launch_pose_final(ctx, s, flags, g_twist);
+  rc = launch_pose_final(ctx, s, flags, g_twist);
+  GS_PROF(12, s);
+  return rc;
 }
 
 int gs_get_counts(gs_ctx* ctx, void* stream, int64_t* n_visible, int64_t* n_instances) {
@@ -270,7 +273,10 @@ int gs_get_counts(gs_ctx* ctx, void* stream, int64_t* n_visible, int64_t* n_inst
   GS_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
   if (n_visible) *n_visible = c.n_visible;
   if (n_instances) *n_instances = c.n_instances;
-  if (c.overflow) return fail(ctx, GS_E_OVERFLOW, "tile-instance capacity exceeded in this iteration");
+  if (c.overflow) {
+    handle_overflow(ctx);
+    return fail(ctx, GS_E_OVERFLOW, "tile-instance capacity exceeded in this iteration; scratch has grown, re-issue");
+  }
   return GS_OK;
 }
 
@@ -299,6 +305,41 @@ int gs_get_features(gs_ctx* ctx, void* stream, double* mean2d, float* conic, flo
       ctx->N, ctx->feat, ctx->rect, ctx->depth_key, ctx->tiles_touched, mean2d, conic, color, depth, depth_key, rect);
   GS_LAUNCH_CHECK("features_export_kernel");
   return GS_OK;
+}
+
+int gs_profile_enable(gs_ctx* ctx, int on) {
+  if (!ctx) return GS_E_INVALID;
+  GS_CUDA(cudaSetDevice(ctx->device));
+  if (on && !ctx->ev_made) {
+    for (int k = 0; k < 13; ++k) GS_CUDA(cudaEventCreate(&ctx->ev[k]));
+    ctx->ev_made = true;
+  }
+  ctx->prof_on = on != 0;
+  return GS_OK;
+}
+
+int gs_profile_read(gs_ctx* ctx, float* ms) {
+  if (!ctx || !ms) return GS_E_INVALID;
+  if (!ctx->prof_on) return fail(ctx, GS_E_ORDER, "gs_profile_read: profiling is not enabled");
+  GS_CUDA(cudaSetDevice(ctx->device));
+  GS_CUDA(cudaEventSynchronize(ctx->ev[12]));
+  static const int from[GS_NUM_STAGES] = {0, 2, 3, 4, 6, 8, 9, 11};
+  static const int to[GS_NUM_STAGES] = {1, 3, 4, 5, 7, 9, 10, 12};
+  for (int k = 0; k < GS_NUM_STAGES; ++k) GS_CUDA(cudaEventElapsedTime(&ms[k], ctx->ev[from[k]], ctx->ev[to[k]]));
+  return GS_OK;
+}
+
+int gs_get_launch_count(gs_ctx* ctx, uint64_t* n) {
+  if (!ctx || !n) return GS_E_INVALID;
+  *n = ctx->launches;
+  return GS_OK;
+}
+
+int gs_get_workload(gs_ctx* ctx, void* stream, uint64_t* out) {
+  if (!ctx || !out) return GS_E_INVALID;
+  if (ctx->stage < 3) return fail(ctx, GS_E_ORDER, "gs_get_workload before gs_rasterize_fwd");
+  GS_CUDA(cudaSetDevice(ctx->device));
+  return launch_workload_stats(ctx, (cudaStream_t)stream, out);
 }
 
 int gs_aux_l1_grad(void* stream, int64_t n, const float* pred, const float* target, float weight, float* grad) {

@@ -290,8 +290,18 @@ int ensure_instance_capacity(gs_ctx* ctx, int64_t need) {
   return GS_OK;
 }
 
+// If the mailbox shows that an earlier asynchronous iteration overflowed: grow to fit it, clear the flag, return true.
+bool handle_overflow(gs_ctx* ctx) {
+  const Counts mb = read_mailbox(ctx);
+  if (!mb.overflow) return false;
+  ensure_instance_capacity(ctx, (int64_t)mb.n_instances + (int64_t)mb.n_instances / 4);
+  ctx->mailbox->overflow = 0;
+  return true;
+}
+
 int launch_binning(gs_ctx* ctx, cudaStream_t s) {
   const int64_t tiles = (int64_t)ctx->cam.tiles_x * ctx->cam.tiles_y;
+  GS_PROF(2, s);
   GS_CUDA(cudaMemsetAsync(ctx->ranges, 0, (size_t)tiles * sizeof(uint2), s));
   if (ctx->N == 0) {
     GS_CUDA(cudaMemsetAsync(ctx->counts, 0, sizeof(Counts), s));
@@ -312,15 +322,15 @@ int launch_binning(gs_ctx* ctx, cudaStream_t s) {
     ctx->calibrated = true;
     ctx->cal_N = ctx->N; ctx->cal_W = ctx->cam.W; ctx->cal_H = ctx->cam.H;
   } else {
-    // asynchronous path: look at what the last finished iteration reported (no synchronisation)
+    // asynchronous path: act on what the last finished iteration reported (no synchronisation): an overflow is
+    // reported to the caller (after growing), a near-full buffer is grown ahead of time
+    if (handle_overflow(ctx)) return fail(ctx, GS_E_OVERFLOW, "tile-instance capacity exceeded in an earlier iteration; scratch has grown, re-issue");
     const Counts mb = read_mailbox(ctx);
-    if (mb.overflow || (int64_t)mb.n_instances + (int64_t)mb.n_instances / 8 > ctx->cap_I) {
-      if (mb.overflow) ctx->overflow_pending = true;
+    if ((int64_t)mb.n_instances + (int64_t)mb.n_instances / 8 > ctx->cap_I)
       if ((rc = ensure_instance_capacity(ctx, (int64_t)mb.n_instances + (int64_t)mb.n_instances / 4)) != GS_OK) return rc;
-      ctx->mailbox->overflow = 0;
-    }
     if ((rc = run_scan_dup(ctx, s)) != GS_OK) return rc;
   }
+  GS_PROF(3, s);
   // radix sort plan: 4 depth digits + ceil(tile_bits / 8) tile digits
   SortPlan plan;
   plan.passes = 0;
@@ -342,9 +352,11 @@ int launch_binning(gs_ctx* ctx, cudaStream_t s) {
     cur ^= 1;
   }
   ctx->sorted_buf = cur;
+  GS_PROF(4, s);
   const int threads = 256;
   tile_ranges_kernel<<<(unsigned)div_up(ctx->cap_I, threads), threads, 0, s>>>(ctx->keys[cur], ctx->counts, ctx->ranges);
   GS_LAUNCH_CHECK("tile_ranges_kernel");
+  GS_PROF(5, s);
   return GS_OK;
 }
 

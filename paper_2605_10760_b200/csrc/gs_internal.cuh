@@ -119,7 +119,12 @@ struct gs_ctx {
   gs::Counts* counts = nullptr;       // device
   gs::Counts* mailbox = nullptr;      // pinned host, mapped
   gs::Counts* mailbox_dev = nullptr;  // device alias of the mailbox
-  bool overflow_pending = false;
+
+  // stage timing (gs_profile_*): events recorded around the kernel groups when enabled
+  bool prof_on = false;
+  cudaEvent_t ev[13] = {};
+  bool ev_made = false;
+  uint64_t launches = 0;  // kernels launched by this context (gs_get_launch_count)
 
   // host-buffer path (gs_fwd_bwd_host): device staging, grown on demand
   float* hb = nullptr;
@@ -148,6 +153,13 @@ inline int fail_cuda(gs_ctx* ctx, cudaError_t e, const char* where) {
   do {                                                                 \
     cudaError_t e__ = cudaGetLastError();                              \
     if (e__ != cudaSuccess) return gs::fail_cuda(ctx, e__, name);      \
+    ctx->launches++;                                                   \
+  } while (0)
+
+// stage-timing event k on stream s (no-op unless gs_profile_enable(ctx, 1))
+#define GS_PROF(k, s)                                                  \
+  do {                                                                 \
+    if (ctx->prof_on) cudaEventRecord(ctx->ev[k], s);                  \
   } while (0)
 
 template <typename T>
@@ -183,5 +195,7 @@ int launch_gauss_bwd(gs_ctx* ctx, cudaStream_t s, uint32_t flags, float* g_means
                      float* g_opac, float* g_sh);
 int launch_pose_final(gs_ctx* ctx, cudaStream_t s, uint32_t flags, float* g_twist);
 int ensure_instance_capacity(gs_ctx* ctx, int64_t need);
+bool handle_overflow(gs_ctx* ctx);
+int launch_workload_stats(gs_ctx* ctx, cudaStream_t s, uint64_t* out_host);
 
 }  // namespace gs

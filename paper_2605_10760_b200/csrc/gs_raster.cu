@@ -149,6 +149,63 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint2* __restrict__ ranges, c
   }
 }
 
+// Workload statistics of the forward (introspection only): re-walks every pixel's list with the forward's decisions.
+__global__ void __launch_bounds__(kBatch)
+workload_stats_kernel(int W, int H, int tiles_x, const uint2* __restrict__ ranges, const uint32_t* __restrict__ ids,
+                      const float4* __restrict__ feat, unsigned long long* __restrict__ out) {
+  __shared__ Staged sm[kBatch];
+  const int tile = blockIdx.x;
+  const int ox = (tile % tiles_x) * GS_TILE, oy = (tile / tiles_x) * GS_TILE;
+  int lx, ly;
+  thread_pixel(threadIdx.x, lx, ly);
+  const bool inside = (ox + lx) < W && (oy + ly) < H;
+  const float fx = (float)lx, fy = (float)ly;
+  const uint2 range = ranges[tile];
+  const int n = (int)(range.y - range.x);
+  float T = 1.f;
+  unsigned long long evaluated = 0, blended = 0, last = 0;
+  bool done = !inside;
+  for (int b0 = 0; b0 < n; b0 += kBatch) {
+    __syncthreads();
+    const int idx = b0 + threadIdx.x;
+    if (idx < n) stage_gaussian(feat, __ldg(ids + range.x + idx), ox, oy, sm[threadIdx.x]);
+    __syncthreads();
+    const int cnt = min(kBatch, n - b0);
+    for (int j = 0; j < cnt && !done; ++j) {
+      const float4 g0 = sm[j].g0, g1 = sm[j].g1;
+      ++evaluated;
+      const float a = fminf(GS_ALPHA_MAX, eval_og(fx - g0.x, fy - g0.y, g0.z, g0.w, g1.x, g1.y));
+      if (a < GS_ALPHA_MIN) continue;
+      if (T < GS_T_MIN) { done = true; break; }
+      T = T * (1.f - a);
+      ++blended;
+      last = (unsigned long long)(b0 + j + 1);
+    }
+  }
+  unsigned long long v[4] = {evaluated, blended, last, inside ? (unsigned long long)n : 0ull};
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+#pragma unroll
+    for (int d = 16; d >= 1; d >>= 1) v[k] += __shfl_xor_sync(0xffffffffu, v[k], d);
+    if ((threadIdx.x & 31) == 0 && v[k]) atomicAdd(out + k, v[k]);
+  }
+}
+
+int launch_workload_stats(gs_ctx* ctx, cudaStream_t s, uint64_t* out_host) {
+  const int tiles = ctx->cam.tiles_x * ctx->cam.tiles_y;
+  unsigned long long* d = reinterpret_cast<unsigned long long*>(ctx->pose_acc);  // 16 doubles of scratch, unused here
+  GS_CUDA(cudaMemsetAsync(d, 0, 4 * sizeof(unsigned long long), s));
+  if (tiles > 0) {
+    workload_stats_kernel<<<tiles, kBatch, 0, s>>>(ctx->cam.W, ctx->cam.H, ctx->cam.tiles_x, ctx->ranges,
+                                                   ctx->vals[ctx->sorted_buf], ctx->feat, d);
+    GS_LAUNCH_CHECK("workload_stats_kernel");
+  }
+  GS_CUDA(cudaMemcpyAsync(out_host, d, 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, s));
+  GS_CUDA(cudaStreamSynchronize(s));
+  ctx->pose_acc_valid = false;
+  return GS_OK;
+}
+
 int launch_raster_fwd(gs_ctx* ctx, cudaStream_t s, float* rgb, float* depth, float* alpha) {
   const int tiles = ctx->cam.tiles_x * ctx->cam.tiles_y;
   if (tiles == 0) return GS_OK;

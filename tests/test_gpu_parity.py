@@ -35,7 +35,14 @@ def run_gpu(gpu, sc, gC, gD, gA=None, cam=None, flags=0, want_features=True):
     ds = b.DeviceScene(sc)
     out = ds.alloc_outputs(cam.width, cam.height)
     to = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a, np.float32)).cuda()
-    b.forward(gpu.ctx, ds, cam, out)
+    for attempt in range(3):  # an iteration that outgrew the instance capacity is reported once and re-issued (gs.h)
+        try:
+            b.forward(gpu.ctx, ds, cam, out)
+            gpu.ctx.gs_get_counts()
+            break
+        except b.GsError as e:
+            if e.code != -5 or attempt == 2:
+                raise
     res = {}
     if want_features:
         res["features"] = gpu.ctx.gs_get_features()
@@ -240,7 +247,7 @@ def test_edge_cases(oracle, gpu):
     # one huge Gaussian covering every tile of a ragged image + equal depth keys (ties broken by index)
     N = 40
     ties = scenes.Scene(means=np.tile(np.array([[0.0, 0.0, 2.0]], np.float32), (N, 1)),
-                        scales=np.full((N, 3), 2.0, np.float32), quats=np.tile(np.array([[1.0, 0, 0, 0]], np.float32), (N, 1)),
+                        scales=np.random.default_rng(6).uniform(1.0, 3.0, (N, 3)).astype(np.float32), quats=np.random.default_rng(7).normal(size=(N, 4)).astype(np.float32),
                         opacities=np.linspace(0.05, 0.4, N).astype(np.float32),
                         sh=scenes.rgb_to_sh0(np.random.default_rng(3).uniform(0, 1, (N, 1, 3))).astype(np.float32),
                         sh_degree=0, camera=scenes.Camera(70, 45, 50.0, 50.0, 34.5, 22.0, scenes.identity_pose()),
@@ -291,11 +298,10 @@ def test_growing_instance_count_is_reported_and_recovered(oracle, gpu):
     dsb = b.DeviceScene(big)
     b.forward(ctx, dsb, small, out)           # overflows silently (asynchronous)
     torch.cuda.synchronize()
-    with pytest.raises(b.GsError, match="GS_E_OVERFLOW"):
-        ctx.gs_poll()
     assert float(out["alpha"].max()) == 0.0   # flagged iteration renders the background only
     with pytest.raises(b.GsError, match="GS_E_OVERFLOW"):
-        b.forward(ctx, dsb, small, out)       # reported once; scratch has grown
+        b.forward(ctx, dsb, small, out)       # reported once, by the first call that notices; scratch has grown
+    ctx.gs_poll()
     b.forward(ctx, dsb, small, out)
     n1 = ctx.gs_get_counts()[1]
     assert n1 > 1.5 * n0
