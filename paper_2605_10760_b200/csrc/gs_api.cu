@@ -2,6 +2,7 @@
 // auxiliary kernels and the host-buffer convenience path.  Argument marshalling and launches only.
 #include <math.h>
 #include <new>
+#include <stdlib.h>
 #include <string.h>
 
 #include "gs_internal.cuh"
@@ -23,8 +24,9 @@ __global__ void features_export_kernel(int64_t N, const float4* __restrict__ fea
   if (vis) { f0 = feat[3 * i]; f1 = feat[3 * i + 1]; f2 = feat[3 * i + 2]; r = rect[i]; dk = depth_key[i]; }
   const double ln2 = 0.6931471805599453;
   if (mean2d) {
-    mean2d[2 * i] = vis ? (double)__float_as_int(f0.z) + (double)f0.x : 0.0;
-    mean2d[2 * i + 1] = vis ? (double)__float_as_int(f0.w) + (double)f0.y : 0.0;
+    const int pk = __float_as_int(f0.z);
+    mean2d[2 * i] = vis ? (double)((pk << 16) >> 16) + (double)f0.x : 0.0;
+    mean2d[2 * i + 1] = vis ? (double)(pk >> 16) + (double)f0.y : 0.0;
   }
   if (conic) {
     conic[3 * i] = (float)(-2.0 * ln2 * (double)f1.x);
@@ -102,6 +104,7 @@ static int ensure_image_capacity(gs_ctx* ctx, int64_t tiles, int64_t pix) {
   if (tiles > ctx->cap_tiles) {
     GS_CUDA(cudaDeviceSynchronize());
     if ((rc = grow(ctx, ctx->ranges, tiles)) != GS_OK) return rc;
+    if ((rc = grow(ctx, ctx->tile_order, tiles)) != GS_OK) return rc;
     ctx->cap_tiles = tiles;
   }
   if (pix > ctx->cap_pix) {
@@ -125,6 +128,8 @@ int gs_create(gs_ctx** out, int device) {
   gs_ctx* ctx = new (std::nothrow) gs_ctx();
   if (!ctx) return GS_E_NOMEM;
   ctx->device = device;
+  if (const char* e = getenv("GS_RASTER_FWD")) ctx->shape_fwd = atoi(e);
+  if (const char* e = getenv("GS_RASTER_BWD")) ctx->shape_bwd = atoi(e);
   bool ok = cudaSetDevice(device) == cudaSuccess;
   ok = ok && cudaMalloc((void**)&ctx->counts, sizeof(Counts)) == cudaSuccess;
   ok = ok && cudaMemset(ctx->counts, 0, sizeof(Counts)) == cudaSuccess;
@@ -149,7 +154,7 @@ int gs_destroy(gs_ctx* ctx) {
   cudaFree(ctx->g2d); cudaFree(ctx->scan_status);
   for (int b = 0; b < 2; ++b) { cudaFree(ctx->keys[b]); cudaFree(ctx->vals[b]); }
   cudaFree(ctx->sort_hist); cudaFree(ctx->sort_status); cudaFree(ctx->sort_ticket);
-  cudaFree(ctx->ranges); cudaFree(ctx->final_T); cudaFree(ctx->n_contrib);
+  cudaFree(ctx->ranges); cudaFree(ctx->tile_order); cudaFree(ctx->final_T); cudaFree(ctx->n_contrib);
   cudaFree(ctx->pose_acc); cudaFree(ctx->counts); cudaFree(ctx->hb);
   if (ctx->mailbox) cudaFreeHost(ctx->mailbox);
   if (ctx->ev_made) for (int k = 0; k < 13; ++k) cudaEventDestroy(ctx->ev[k]);

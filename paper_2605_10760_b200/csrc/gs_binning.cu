@@ -259,6 +259,40 @@ __global__ void tile_ranges_kernel(const uint64_t* __restrict__ keys, const Coun
   if (k == (int64_t)I - 1 || (uint32_t)(keys[k + 1] >> 32) != t) ranges[t].y = (uint32_t)(k + 1);
 }
 
+// Tile ids by descending list length (counting sort on length / 8, 1024 buckets; order inside a bucket is arbitrary):
+// the compositing kernels launch their regions in this order, so that the longest lists start first (LPT scheduling).
+__global__ void __launch_bounds__(1024)
+tile_order_kernel(int tiles, const uint2* __restrict__ ranges, uint32_t* __restrict__ order) {
+  __shared__ uint32_t hist[1024];
+  __shared__ uint32_t wsum[32];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  hist[tid] = 0;
+  __syncthreads();
+  for (int t = tid; t < tiles; t += 1024) {
+    const uint2 r = ranges[t];
+    atomicAdd(&hist[1023 - min((r.y - r.x) >> 3, 1023u)], 1u);
+  }
+  __syncthreads();
+  const uint32_t h = hist[tid];
+  uint32_t incl = h;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const uint32_t v = __shfl_up_sync(0xffffffffu, incl, d);
+    if (lane >= d) incl += v;
+  }
+  if (lane == 31) wsum[warp] = incl;
+  __syncthreads();
+  uint32_t base = incl - h;
+  for (int w = 0; w < warp; ++w) base += wsum[w];
+  __syncthreads();
+  hist[tid] = base;  // bucket cursor
+  __syncthreads();
+  for (int t = tid; t < tiles; t += 1024) {
+    const uint2 r = ranges[t];
+    order[atomicAdd(&hist[1023 - min((r.y - r.x) >> 3, 1023u)], 1u)] = (uint32_t)t;
+  }
+}
+
 static int run_scan_dup(gs_ctx* ctx, cudaStream_t s) {
   const int64_t nchunks = div_up(ctx->N, kScanChunk);
   // reset: counts->{n_instances,overflow}, tickets, scan status (n_visible was produced by gs_preprocess: keep it)
@@ -305,6 +339,8 @@ int launch_binning(gs_ctx* ctx, cudaStream_t s) {
   GS_CUDA(cudaMemsetAsync(ctx->ranges, 0, (size_t)tiles * sizeof(uint2), s));
   if (ctx->N == 0) {
     GS_CUDA(cudaMemsetAsync(ctx->counts, 0, sizeof(Counts), s));
+    tile_order_kernel<<<1, 1024, 0, s>>>((int)tiles, ctx->ranges, ctx->tile_order);
+    GS_LAUNCH_CHECK("tile_order_kernel");
     return GS_OK;
   }
   const bool same_shape = ctx->calibrated && ctx->cal_N == ctx->N && ctx->cal_W == ctx->cam.W && ctx->cal_H == ctx->cam.H;
@@ -356,6 +392,8 @@ int launch_binning(gs_ctx* ctx, cudaStream_t s) {
   const int threads = 256;
   tile_ranges_kernel<<<(unsigned)div_up(ctx->cap_I, threads), threads, 0, s>>>(ctx->keys[cur], ctx->counts, ctx->ranges);
   GS_LAUNCH_CHECK("tile_ranges_kernel");
+  tile_order_kernel<<<1, 1024, 0, s>>>((int)tiles, ctx->ranges, ctx->tile_order);
+  GS_LAUNCH_CHECK("tile_order_kernel");
   GS_PROF(5, s);
   return GS_OK;
 }

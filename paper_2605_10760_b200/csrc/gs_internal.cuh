@@ -32,7 +32,8 @@ __device__ __forceinline__ void load_pose(const DevCam& cam, float* T) {
 
 // ---------------------------------------------------------------------------------------------------------------
 // Per-Gaussian feature record written by gs_preprocess and gathered by the rasteriser: 3 x float4 = 48 B.
-//   f0 = { mfx, mfy, as_float(mix), as_float(miy) }  2-D mean = integer pixel (mix,miy) + fraction in [-0.5,0.5]
+//   f0 = { mfx, mfy, bits(miy << 16 | mix & 0xffff), thr }  2-D mean = integer pixel (mix,miy) + fraction in [-0.5,0.5];
+//                               thr = -log2(255 opacity): alpha >= 1/255  <=>  power2 >= thr
 //   f1 = { A, B, C, opacity }   power2 = A dx^2 + B dx dy + C dy^2  (conic pre-scaled: A = -0.5 log2(e) a, B = -log2(e) b,
 //                               C = -0.5 log2(e) c), alpha = min(0.99, opacity * 2^power2)
 //   f2 = { r, g, b, z_c }
@@ -119,6 +120,10 @@ struct gs_ctx {
   gs::Counts* counts = nullptr;       // device
   gs::Counts* mailbox = nullptr;      // pinned host, mapped
   gs::Counts* mailbox_dev = nullptr;  // device alias of the mailbox
+
+  // region shape of the compositing kernels; tuning knobs GS_RASTER_FWD / GS_RASTER_BWD read by gs_create.
+  int shape_fwd = 11, shape_bwd = 11;  // "NXNY": region per warp = (8 NX) x (4 NY) pixels
+  uint32_t* tile_order = nullptr;      // [tiles] tile ids by descending list length (longest lists are scheduled first)
 
   // stage timing (gs_profile_*): events recorded around the kernel groups when enabled
   bool prof_on = false;

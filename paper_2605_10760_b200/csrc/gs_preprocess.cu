@@ -58,13 +58,14 @@ preprocess_kernel(int64_t N, const float* __restrict__ means, const float* __res
           col[2] = fmaf(B[k], __ldg(c + 3 * k + 2), col[2]);
         }
       }
-      // mean = integer pixel + fraction
-      const double rmx = fmin(fmax(rint(P.mx), -1073741824.0), 1073741824.0);
-      const double rmy = fmin(fmax(rint(P.my), -1073741824.0), 1073741824.0);
+      // mean = integer pixel (two int16, clamped: a centre that far off-screen needs no sub-pixel precision) + fraction
+      const double rmx = fmin(fmax(rint(P.mx), -32000.0), 32000.0);
+      const double rmy = fmin(fmax(rint(P.my), -32000.0), 32000.0);
       const double kl = 1.4426950408889634;  // log2(e)
       float4 f0, f1, f2;
       f0.x = (float)(P.mx - rmx); f0.y = (float)(P.my - rmy);
-      f0.z = __int_as_float((int)rmx); f0.w = __int_as_float((int)rmy);
+      f0.z = __int_as_float(((int)rmy << 16) | ((int)rmx & 0xffff));
+      f0.w = (float)(-log2(255.0 * (double)o));  // alpha >= 1/255  <=>  power2 >= thr
       f1.x = (float)(-0.5 * kl * P.a); f1.y = (float)(-kl * P.b); f1.z = (float)(-0.5 * kl * P.c); f1.w = o;
       f2.x = fmaxf(col[0] + 0.5f, 0.f); f2.y = fmaxf(col[1] + 0.5f, 0.f); f2.z = fmaxf(col[2] + 0.5f, 0.f);
       f2.w = (float)P.z;

@@ -1,228 +1,440 @@
-// gs_raster.cu -- steps a6 (front-to-back compositing) and a8 (back-to-front per-pixel backward with warp-level
-// reduction before global atomics).  One CTA per 16x16 tile, one thread per pixel, Gaussians staged through shared
-// memory in batches of 256.  ALU/MUFU-bound.
+// gs_raster.cu -- steps a6 (front-to-back compositing) and a8 (back-to-front per-pixel backward, reduced at warp
+// level before global atomics).
+//
+// v2 design (evidence: profiles/r1_v1_baseline.md -- the one-pixel-per-thread kernels were bound by the LSU pipe:
+// shuffles of the 10-value reduction and broadcast LDS of the Gaussian records):
+//   * one WARP per tile region, 2 x NY interleaved pixels per lane (NY = 4: the whole 16x16 tile, NY = 2: half of it);
+//     the Gaussian record is read from shared memory once per (region, Gaussian) instead of once per 32 pixels and
+//     the conic products are shared across the lane's rows / columns;
+//   * warps are autonomous (single-warp CTAs): no __syncthreads, early exit per region, hardware CTA scheduling
+//     balances the very uneven tile lists;
+//   * Gaussian records are gathered by cp.async (LDGSTS) into a double-buffered warp-private staging area, one batch
+//     ahead of the compute, the sorted ids two batches ahead;
+//   * phase 1 of every batch: lane g tests Gaussian g against the region (exact maximum of the concave power over the
+//     region rectangle) -- Gaussians whose ellipse misses the region never reach the pixel loop;
+//   * phase 2: the surviving Gaussians are taken FOUR at a time: 4 x NS powers evaluated together (ILP; the serial
+//     latency per list entry is what bounds the longest tiles), one REDUX.OR over the packed slot masks;
+//   * the alpha >= 1/255 test is taken in the power domain (power2 >= thr), so rejected pairs cost no MUFU;
+//   * backward: the 10 per-Gaussian sums are accumulated over the lane's pixels first, then ONE 16-slot butterfly
+//     reduce-scatter (16 SHFL) per (region, Gaussian) and one coalesced 10-lane RED.
 #include "gs_internal.cuh"
 #include "gs_raster.cuh"
 
 namespace gs {
 
-__global__ void __launch_bounds__(kBatch)
-raster_fwd_kernel(int W, int H, int tiles_x, const uint2* __restrict__ ranges, const uint32_t* __restrict__ ids,
+constexpr unsigned kFull = 0xffffffffu;
+constexpr int kGroup = 4;                    // Gaussians evaluated together in phase 2
+constexpr int kSlotsRec = kWarpBatch + 1;    // staged records per buffer: 32 + one never-contributing dummy
+
+// Maximum of power2 over the continuous rectangle [0,xmax] x [0,ymax] (region-local), exact for the concave quadratic:
+// 0 if the centre is inside, else the largest of the four clamped edge maxima.
+__device__ __forceinline__ float region_max_power(const GaussReg& g, float xmax, float ymax) {
+  const float x0 = -g.mx, x1 = xmax - g.mx, y0 = -g.my, y1 = ymax - g.my;  // rectangle in centre-relative coordinates
+  if (x0 <= 0.f && x1 >= 0.f && y0 <= 0.f && y1 >= 0.f) return 0.f;
+  const float i2C = __frcp_rn(2.f * g.C), i2A = __frcp_rn(2.f * g.A);
+  float best = -INFINITY;
+#pragma unroll
+  for (int e = 0; e < 2; ++e) {
+    const float dxe = e ? x1 : x0;
+    const float dys = fminf(fmaxf(-g.B * dxe * i2C, y0), y1);
+    best = fmaxf(best, g.A * dxe * dxe + g.B * dxe * dys + g.C * dys * dys);
+    const float dye = e ? y1 : y0;
+    const float dxs = fminf(fmaxf(-g.B * dye * i2A, x0), x1);
+    best = fmaxf(best, g.A * dxs * dxs + g.B * dxs * dye + g.C * dye * dye);
+  }
+  return best;
+}
+
+__device__ __forceinline__ void write_dummy(float4* rec) {
+  rec[0] = make_float4(0.f, 0.f, 0.f, INFINITY);  // thr = +inf: never passes
+  rec[1] = make_float4(0.f, 0.f, 0.f, 0.f);
+  rec[2] = make_float4(0.f, 0.f, 0.f, 0.f);
+}
+
+template <int NX, int NY, bool STATS>
+__global__ void __launch_bounds__(32)
+raster_fwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order, const uint2* __restrict__ ranges, const uint32_t* __restrict__ ids,
                   const float4* __restrict__ feat, float bg0, float bg1, float bg2, float* __restrict__ rgb,
                   float* __restrict__ depth, float* __restrict__ alpha_out, float* __restrict__ final_T,
-                  uint32_t* __restrict__ n_contrib) {
-  __shared__ Staged sm[kBatch];
-  const int tile = blockIdx.x;
-  const int ox = (tile % tiles_x) * GS_TILE, oy = (tile / tiles_x) * GS_TILE;
-  int lx, ly;
-  thread_pixel(threadIdx.x, lx, ly);
-  const int px = ox + lx, py = oy + ly;
-  const bool inside = px < W && py < H;
-  const float fx = (float)lx, fy = (float)ly;
+                  uint32_t* __restrict__ n_contrib, unsigned long long* __restrict__ stats) {
+  constexpr int NS = NX * NY, RX = 2 / NX, RPT = RX * (4 / NY);  // slots per lane, regions per tile
+  __shared__ __align__(16) float4 s_feat[2][kSlotsRec * 3];
+  const int lane = threadIdx.x;
+  const int tile = (int)__ldg(order + blockIdx.x / RPT), sub = blockIdx.x % RPT;
+  const int ox = (tile % tiles_x) * GS_TILE + (sub % RX) * (8 * NX), oy = (tile / tiles_x) * GS_TILE + (sub / RX) * (4 * NY);
+  const int lx = lane & 7, ly = lane >> 3;
+  const float fx0 = (float)lx, fy0 = (float)ly;
+  unsigned alive = 0;
+#pragma unroll
+  for (int k = 0; k < NS; ++k)
+    if (ox + lx + 8 * (k % NX) < W && oy + ly + 4 * (k / NX) < H) alive |= 1u << k;
+  const unsigned inside = alive;
   const uint2 range = ranges[tile];
   const int n = (int)(range.y - range.x);
-  float T = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f, D = 0.f;
-  uint32_t last = 0;
-  bool done = !inside;
-  for (int b0 = 0; b0 < n; b0 += kBatch) {
-    if (__syncthreads_and(done)) break;
-    const int idx = b0 + threadIdx.x;
-    if (idx < n) stage_gaussian(feat, __ldg(ids + range.x + idx), ox, oy, sm[threadIdx.x]);
-    __syncthreads();
-    if (__all_sync(0xffffffffu, done)) continue;
-    const int cnt = min(kBatch, n - b0);
-    for (int j = 0; j < cnt && !done; ++j) {
-      const float4 g0 = sm[j].g0, g1 = sm[j].g1;
-      const float dx = fx - g0.x, dy = fy - g0.y;
-      const float og = eval_og(dx, dy, g0.z, g0.w, g1.x, g1.y);
-      const float a = fminf(GS_ALPHA_MAX, og);
-      if (a < GS_ALPHA_MIN) continue;
-      if (T < GS_T_MIN) { done = true; break; }
-      const float4 g2 = sm[j].g2;
-      const float w = a * T;
-      C0 = fmaf(g1.z, w, C0);
-      C1 = fmaf(g1.w, w, C1);
-      C2 = fmaf(g2.x, w, C2);
-      D = fmaf(g2.y, w, D);
-      T = T * (1.f - a);
-      last = (uint32_t)(b0 + j + 1);
+  const int nb = (n + kWarpBatch - 1) / kWarpBatch;
+  float T[NS], C0[NS], C1[NS], C2[NS], D[NS];
+  uint32_t last[NS];
+#pragma unroll
+  for (int k = 0; k < NS; ++k) { T[k] = 1.f; C0[k] = C1[k] = C2[k] = D[k] = 0.f; last[k] = 0; }
+  unsigned long long n_eval = 0, n_blend = 0;
+  if (lane < 2) write_dummy(&s_feat[lane][kWarpBatch * 3]);
+
+  auto issue = [&](int b, uint32_t id) {
+    if (b * kWarpBatch + lane < n) {
+      const float4* src = feat + 3 * (size_t)id;
+      float4* dst = &s_feat[b & 1][lane * 3];
+      cp_async16(dst, src); cp_async16(dst + 1, src + 1); cp_async16(dst + 2, src + 2);
+    }
+    cp_async_commit();
+  };
+  uint32_t id_next = 0;
+  if (nb > 0) {
+    issue(0, lane < n ? __ldg(ids + range.x + lane) : 0u);
+    if (nb > 1) id_next = (kWarpBatch + lane < n) ? __ldg(ids + range.x + kWarpBatch + lane) : 0u;
+  }
+  bool stop = !__any_sync(kFull, alive != 0);
+  for (int b = 0; b < nb && !stop; ++b) {
+    if (b + 1 < nb) {
+      issue(b + 1, id_next);
+      const int i2 = (b + 2) * kWarpBatch + lane;
+      if (b + 2 < nb) id_next = (i2 < n) ? __ldg(ids + range.x + i2) : 0u;
+      cp_async_wait<1>();
+    } else {
+      cp_async_wait<0>();
+    }
+    __syncwarp();
+    const int cnt = min(kWarpBatch, n - b * kWarpBatch);
+    const float4* sf = s_feat[b & 1];
+    // phase 1: which Gaussians of the batch can reach this region at all?
+    bool relevant = false;
+    if (lane < cnt) {
+      GaussReg g;
+      decode_gauss(sf[3 * lane], sf[3 * lane + 1], ox, oy, g);
+      relevant = region_max_power(g, (float)(8 * NX - 1), (float)(4 * NY - 1)) >= g.thr - 1e-3f;
+    }
+    unsigned rel = __ballot_sync(kFull, relevant);
+    // phase 2: front to back, four list entries at a time
+    while (rel) {
+      int jj[kGroup];
+#pragma unroll
+      for (int q = 0; q < kGroup; ++q) {
+        jj[q] = rel ? (__ffs(rel) - 1) : kWarpBatch;  // kWarpBatch = the dummy record
+        rel &= rel - 1;
+      }
+      GaussReg g[kGroup];
+      float dx[kGroup][NX], dy[kGroup][NY], p[kGroup][NS];
+      unsigned m = 0;
+#pragma unroll
+      for (int q = 0; q < kGroup; ++q) {
+        decode_gauss(sf[3 * jj[q]], sf[3 * jj[q] + 1], ox, oy, g[q]);
+        eval_power<NX, NY>(g[q], fx0, fy0, dx[q], dy[q], p[q]);
+#pragma unroll
+        for (int k = 0; k < NS; ++k) m |= (p[q][k] >= g[q].thr) ? (1u << (q * NS + k)) : 0u;
+      }
+      if (STATS) {
+#pragma unroll
+        for (int q = 0; q < kGroup; ++q) n_eval += (jj[q] < kWarpBatch) ? __popc(alive) : 0;
+      }
+      constexpr unsigned kRep = 1u | (1u << NS) | (1u << (2 * NS)) | (1u << (3 * NS));  // replicate the slot mask over the group
+      const unsigned any = __reduce_or_sync(kFull, m & (alive * kRep));
+      if (any == 0) continue;
+#pragma unroll
+      for (int q = 0; q < kGroup; ++q) {
+        if (((any >> (q * NS)) & ((1u << NS) - 1)) == 0) continue;
+        const float4 f2 = sf[3 * jj[q] + 2];
+        const unsigned mq = (m >> (q * NS)) & alive;
+#pragma unroll
+        for (int k = 0; k < NS; ++k) {
+          if (any & (1u << (q * NS + k))) {
+            if (mq & (1u << k)) {
+              const float a = fminf(GS_ALPHA_MAX, __fmul_rn(g[q].o, ex2_approx(p[q][k])));
+              if (T[k] < GS_T_MIN) {
+                alive &= ~(1u << k);
+              } else {
+                const float w = a * T[k];
+                C0[k] = fmaf(f2.x, w, C0[k]);
+                C1[k] = fmaf(f2.y, w, C1[k]);
+                C2[k] = fmaf(f2.z, w, C2[k]);
+                D[k] = fmaf(f2.w, w, D[k]);
+                T[k] = T[k] * (1.f - a);
+                last[k] = (uint32_t)(b * kWarpBatch + jj[q] + 1);
+                if (STATS) ++n_blend;
+              }
+            }
+          }
+        }
+      }
+      if (!__any_sync(kFull, alive != 0)) { stop = true; break; }
+    }
+    __syncwarp();
+  }
+  cp_async_wait<0>();
+  const size_t HW = (size_t)W * H;
+#pragma unroll
+  for (int k = 0; k < NS; ++k) {
+    if (inside & (1u << k)) {
+      const size_t p = (size_t)(oy + ly + 4 * (k / NX)) * W + (ox + lx + 8 * (k % NX));
+      if (!STATS) {
+        if (rgb) {
+          rgb[p] = fmaf(T[k], bg0, C0[k]);
+          rgb[HW + p] = fmaf(T[k], bg1, C1[k]);
+          rgb[2 * HW + p] = fmaf(T[k], bg2, C2[k]);
+        }
+        if (depth) depth[p] = D[k];
+        if (alpha_out) alpha_out[p] = 1.f - T[k];
+        final_T[p] = T[k];
+        n_contrib[p] = last[k];
+      }
     }
   }
-  if (inside) {
-    const size_t p = (size_t)py * W + px, HW = (size_t)W * H;
-    if (rgb) {
-      rgb[p] = fmaf(T, bg0, C0);
-      rgb[HW + p] = fmaf(T, bg1, C1);
-      rgb[2 * HW + p] = fmaf(T, bg2, C2);
+  if (STATS) {
+    unsigned long long v[4] = {n_eval, n_blend, 0ull, (unsigned long long)n * __popc(inside)};
+#pragma unroll
+    for (int k = 0; k < NS; ++k) v[2] += (inside & (1u << k)) ? last[k] : 0u;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+#pragma unroll
+      for (int d = 16; d >= 1; d >>= 1) v[q] += __shfl_xor_sync(kFull, v[q], d);
+      if (lane == 0 && v[q]) atomicAdd(stats + q, v[q]);
     }
-    if (depth) depth[p] = D;
-    if (alpha_out) alpha_out[p] = 1.f - T;
-    final_T[p] = T;
-    n_contrib[p] = last;
   }
 }
 
-__global__ void __launch_bounds__(kBatch)
-raster_bwd_kernel(int W, int H, int tiles_x, const uint2* __restrict__ ranges, const uint32_t* __restrict__ ids,
+// 16-slot butterfly reduce-scatter over the warp: on return lane l holds the warp total of slot l >> 1.
+__device__ __forceinline__ float reduce_scatter16(float (&v)[16], int lane) {
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const bool up = lane & 16;
+    const float send = up ? v[i] : v[i + 8], keep = up ? v[i + 8] : v[i];
+    v[i] = keep + __shfl_xor_sync(kFull, send, 16);
+  }
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const bool up = lane & 8;
+    const float send = up ? v[i] : v[i + 4], keep = up ? v[i + 4] : v[i];
+    v[i] = keep + __shfl_xor_sync(kFull, send, 8);
+  }
+#pragma unroll
+  for (int i = 0; i < 2; ++i) {
+    const bool up = lane & 4;
+    const float send = up ? v[i] : v[i + 2], keep = up ? v[i + 2] : v[i];
+    v[i] = keep + __shfl_xor_sync(kFull, send, 4);
+  }
+  {
+    const bool up = lane & 2;
+    const float send = up ? v[0] : v[1], keep = up ? v[1] : v[0];
+    v[0] = keep + __shfl_xor_sync(kFull, send, 2);
+  }
+  return v[0] + __shfl_xor_sync(kFull, v[0], 1);
+}
+
+template <int NX, int NY, bool HAS_GA>
+__global__ void __launch_bounds__(32)
+raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order, const uint2* __restrict__ ranges, const uint32_t* __restrict__ ids,
                   const float4* __restrict__ feat, float bg0, float bg1, float bg2, const float* __restrict__ final_T,
                   const uint32_t* __restrict__ n_contrib, const float* __restrict__ d_rgb,
                   const float* __restrict__ d_depth, const float* __restrict__ d_alpha, float* __restrict__ g2d) {
-  __shared__ Staged sm[kBatch];
-  __shared__ uint32_t s_max[kBatch / 32];
-  const int tile = blockIdx.x;
-  const int ox = (tile % tiles_x) * GS_TILE, oy = (tile / tiles_x) * GS_TILE;
-  int lx, ly;
-  thread_pixel(threadIdx.x, lx, ly);
-  const int px = ox + lx, py = oy + ly;
-  const bool inside = px < W && py < H;
-  const float fx = (float)lx, fy = (float)ly;
+  constexpr int NS = NX * NY, RX = 2 / NX, RPT = RX * (4 / NY);  // slots per lane, regions per tile
+  __shared__ __align__(16) float4 s_feat[2][kSlotsRec * 3];
+  __shared__ uint32_t s_id[2][kSlotsRec];
+  const int lane = threadIdx.x;
+  const int tile = (int)__ldg(order + blockIdx.x / RPT), sub = blockIdx.x % RPT;
+  const int ox = (tile % tiles_x) * GS_TILE + (sub % RX) * (8 * NX), oy = (tile / tiles_x) * GS_TILE + (sub / RX) * (4 * NY);
+  const int lx = lane & 7, ly = lane >> 3;
+  const float fx0 = (float)lx, fy0 = (float)ly;
   const uint2 range = ranges[tile];
-  float T = 1.f, gC0 = 0.f, gC1 = 0.f, gC2 = 0.f, gD = 0.f, gA = 0.f;
-  uint32_t last = 0;
-  if (inside) {
-    const size_t p = (size_t)py * W + px, HW = (size_t)W * H;
-    T = final_T[p];
-    last = n_contrib[p];
-    gC0 = d_rgb[p]; gC1 = d_rgb[HW + p]; gC2 = d_rgb[2 * HW + p];
-    if (d_depth) gD = d_depth[p];
-    if (d_alpha) gA = d_alpha[p];
+  float T[NS], S[NS], gC0[NS], gC1[NS], gC2[NS], gD[NS], gA[HAS_GA ? NS : 1];
+  uint32_t last[NS];
+  const size_t HW = (size_t)W * H;
+  uint32_t maxlast = 0;
+#pragma unroll
+  for (int k = 0; k < NS; ++k) {
+    const int X = ox + lx + 8 * (k % NX), Y = oy + ly + 4 * (k / NX);
+    T[k] = 1.f; last[k] = 0; gC0[k] = gC1[k] = gC2[k] = gD[k] = 0.f;
+    if (HAS_GA) gA[k] = 0.f;
+    if (X < W && Y < H) {
+      const size_t p = (size_t)Y * W + X;
+      T[k] = final_T[p];
+      last[k] = n_contrib[p];
+      gC0[k] = d_rgb[p]; gC1[k] = d_rgb[HW + p]; gC2[k] = d_rgb[2 * HW + p];
+      if (d_depth) gD[k] = d_depth[p];
+      if (HAS_GA) gA[k] = d_alpha[p];
+    }
+    S[k] = T[k] * (gC0[k] * bg0 + gC1[k] * bg1 + gC2[k] * bg2);
+    maxlast = max(maxlast, last[k]);
   }
-  float S = T * (gC0 * bg0 + gC1 * bg1 + gC2 * bg2);
-  // deepest blended position in the tile
-  uint32_t m = __reduce_max_sync(0xffffffffu, last);
-  if ((threadIdx.x & 31) == 0) s_max[threadIdx.x >> 5] = m;
-  __syncthreads();
-  uint32_t maxc = 0;
+  maxlast = __reduce_max_sync(kFull, maxlast);  // deepest blended list position of the region
+  const int n = (int)maxlast;
+  const int nb = (n + kWarpBatch - 1) / kWarpBatch;
+  if (lane < 2) { write_dummy(&s_feat[lane][kWarpBatch * 3]); s_id[lane][kWarpBatch] = 0; }
+
+  auto issue = [&](int b, uint32_t id) {
+    if (b * kWarpBatch + lane < n) {
+      const float4* src = feat + 3 * (size_t)id;
+      float4* dst = &s_feat[b & 1][lane * 3];
+      cp_async16(dst, src); cp_async16(dst + 1, src + 1); cp_async16(dst + 2, src + 2);
+      s_id[b & 1][lane] = id;
+    }
+    cp_async_commit();
+  };
+  uint32_t id_next = 0;
+  if (nb > 0) {
+    const int i0 = (nb - 1) * kWarpBatch + lane;
+    issue(nb - 1, i0 < n ? __ldg(ids + range.x + i0) : 0u);
+    if (nb > 1) id_next = __ldg(ids + range.x + (nb - 2) * kWarpBatch + lane);
+  }
+  for (int b = nb - 1; b >= 0; --b) {
+    if (b >= 1) {
+      issue(b - 1, id_next);
+      if (b >= 2) id_next = __ldg(ids + range.x + (b - 2) * kWarpBatch + lane);
+      cp_async_wait<1>();
+    } else {
+      cp_async_wait<0>();
+    }
+    __syncwarp();
+    const int cnt = min(kWarpBatch, n - b * kWarpBatch);
+    const float4* sf = s_feat[b & 1];
+    bool relevant = false;
+    if (lane < cnt) {
+      GaussReg g;
+      decode_gauss(sf[3 * lane], sf[3 * lane + 1], ox, oy, g);
+      relevant = region_max_power(g, (float)(8 * NX - 1), (float)(4 * NY - 1)) >= g.thr - 1e-3f;
+    }
+    unsigned rel = __ballot_sync(kFull, relevant);
+    while (rel) {  // back to front, four list entries at a time
+      int jj[kGroup];
 #pragma unroll
-  for (int w = 0; w < kBatch / 32; ++w) maxc = max(maxc, s_max[w]);
-  const int lane = threadIdx.x & 31;
-  const int rounds = (int)((maxc + kBatch - 1) / kBatch);
-  for (int r = rounds - 1; r >= 0; --r) {
-    const int b0 = r * kBatch;
-    __syncthreads();
-    const int idx = b0 + threadIdx.x;
-    if (idx < (int)maxc) stage_gaussian(feat, __ldg(ids + range.x + idx), ox, oy, sm[threadIdx.x]);
-    __syncthreads();
-    const int cnt = min(kBatch, (int)maxc - b0);
-    for (int j = cnt - 1; j >= 0; --j) {
-      const uint32_t pos = (uint32_t)(b0 + j);
-      const float4 g0 = sm[j].g0, g1 = sm[j].g1;
-      const float dx = fx - g0.x, dy = fy - g0.y;
-      const float og = eval_og(dx, dy, g0.z, g0.w, g1.x, g1.y);
-      const float a = fminf(GS_ALPHA_MAX, og);
-      const bool valid = pos < last && a >= GS_ALPHA_MIN;
-      if (!__any_sync(0xffffffffu, valid)) continue;
-      const float4 g2 = sm[j].g2;
-      float v[10];
+      for (int q = 0; q < kGroup; ++q) {
+        jj[q] = rel ? (31 - __clz(rel)) : kWarpBatch;
+        if (rel) rel &= ~(1u << jj[q]);
+      }
+      GaussReg g[kGroup];
+      float dx[kGroup][NX], dy[kGroup][NY], p[kGroup][NS];
+      unsigned m = 0;
 #pragma unroll
-      for (int k = 0; k < 10; ++k) v[k] = 0.f;
-      if (valid) {
-        const float oma = 1.f - a;
-        T = __fdividef(T, oma);  // transmittance in front of this Gaussian
-        const float w = a * T;
-        const float wi = fmaf(gC0, g1.z, fmaf(gC1, g1.w, fmaf(gC2, g2.x, fmaf(gD, g2.y, gA))));
-        const float dalpha = fmaf(T, wi, -__fdividef(S, oma));
-        S = fmaf(wi, w, S);
-        v[6] = w * gC0; v[7] = w * gC1; v[8] = w * gC2; v[9] = w * gD;
-        if (og <= GS_ALPHA_MAX) {
-          const float gp = a * dalpha;
-          const float A = g0.z, B = g0.w, Cc = g1.x;
-          v[0] = gp * fmaf(2.f * A, dx, B * dy);
-          v[1] = gp * fmaf(2.f * Cc, dy, B * dx);
-          v[2] = gp * dx * dx;
-          v[3] = gp * dx * dy;
-          v[4] = gp * dy * dy;
-          v[5] = gp;
+      for (int q = 0; q < kGroup; ++q) {
+        decode_gauss(sf[3 * jj[q]], sf[3 * jj[q] + 1], ox, oy, g[q]);
+        eval_power<NX, NY>(g[q], fx0, fy0, dx[q], dy[q], p[q]);
+        const uint32_t pos = (uint32_t)(b * kWarpBatch + jj[q]);
+#pragma unroll
+        for (int k = 0; k < NS; ++k) m |= (p[q][k] >= g[q].thr && pos < last[k]) ? (1u << (q * NS + k)) : 0u;
+      }
+      const unsigned any = __reduce_or_sync(kFull, m);
+      if (any == 0) continue;
+#pragma unroll
+      for (int q = 0; q < kGroup; ++q) {
+        if (((any >> (q * NS)) & ((1u << NS) - 1)) == 0) continue;
+        const float4 f2 = sf[3 * jj[q] + 2];
+        const uint32_t id = s_id[b & 1][jj[q]];
+        float tAx[NX], tBx[NX], tCy[NY], tBy[NY];
+#pragma unroll
+        for (int kx = 0; kx < NX; ++kx) { tAx[kx] = 2.f * g[q].A * dx[q][kx]; tBx[kx] = g[q].B * dx[q][kx]; }
+#pragma unroll
+        for (int ky = 0; ky < NY; ++ky) { tCy[ky] = 2.f * g[q].C * dy[q][ky]; tBy[ky] = g[q].B * dy[q][ky]; }
+        float v[16];
+#pragma unroll
+        for (int u = 0; u < 16; ++u) v[u] = 0.f;
+#pragma unroll
+        for (int k = 0; k < NS; ++k) {
+          if (any & (1u << (q * NS + k))) {
+            if (m & (1u << (q * NS + k))) {
+              const int kx = k % NX, ky = k / NX;
+              const float og = __fmul_rn(g[q].o, ex2_approx(p[q][k]));
+              const float a = fminf(GS_ALPHA_MAX, og);
+              const float ioma = __frcp_rn(1.f - a);
+              const float Tk = T[k] * ioma;  // transmittance in front of this Gaussian
+              T[k] = Tk;
+              const float w = a * Tk;
+              float wi = fmaf(gC0[k], f2.x, fmaf(gC1[k], f2.y, fmaf(gC2[k], f2.z, gD[k] * f2.w)));
+              if (HAS_GA) wi += gA[k];
+              const float dalpha = fmaf(Tk, wi, -S[k] * ioma);
+              S[k] = fmaf(wi, w, S[k]);
+              v[6] = fmaf(w, gC0[k], v[6]);
+              v[7] = fmaf(w, gC1[k], v[7]);
+              v[8] = fmaf(w, gC2[k], v[8]);
+              v[9] = fmaf(w, gD[k], v[9]);
+              if (og <= GS_ALPHA_MAX) {
+                const float gp = a * dalpha;
+                v[0] = fmaf(gp, tAx[kx] + tBy[ky], v[0]);
+                v[1] = fmaf(gp, tCy[ky] + tBx[kx], v[1]);
+                v[2] = fmaf(gp * dx[q][kx], dx[q][kx], v[2]);
+                v[3] = fmaf(gp * dx[q][kx], dy[q][ky], v[3]);
+                v[4] = fmaf(gp * dy[q][ky], dy[q][ky], v[4]);
+                v[5] += gp;
+              }
+            }
+          }
         }
-      }
-#pragma unroll
-      for (int k = 0; k < 10; ++k) {
-#pragma unroll
-        for (int d = 16; d >= 1; d >>= 1) v[k] += __shfl_xor_sync(0xffffffffu, v[k], d);
-      }
-      if (lane == 0) {
-        float* g = g2d + (size_t)__float_as_uint(g2.z) * kG2D;
-#pragma unroll
-        for (int k = 0; k < 10; ++k) atomicAdd(g + k, v[k]);
+        const float tot = reduce_scatter16(v, lane);
+        if ((lane & 1) == 0 && lane < 20) atomicAdd(g2d + (size_t)id * kG2D + (lane >> 1), tot);
       }
     }
+    __syncwarp();
   }
+}
+
+template <int NX, int NY>
+static int launch_fwd_t(gs_ctx* ctx, cudaStream_t s, float* rgb, float* depth, float* alpha) {
+  const int units = ctx->cam.tiles_x * ctx->cam.tiles_y * (2 / NX) * (4 / NY);
+  raster_fwd_kernel<NX, NY, false><<<units, 32, 0, s>>>(ctx->cam.W, ctx->cam.H, ctx->cam.tiles_x, ctx->tile_order,
+                                                         ctx->ranges, ctx->vals[ctx->sorted_buf], ctx->feat,
+                                                         ctx->bg[0], ctx->bg[1], ctx->bg[2], rgb, depth, alpha,
+                                                         ctx->final_T, ctx->n_contrib, nullptr);
+  GS_LAUNCH_CHECK("raster_fwd_kernel");
+  return GS_OK;
+}
+
+template <int NX, int NY>
+static int launch_bwd_t(gs_ctx* ctx, cudaStream_t s, const float* d_rgb, const float* d_depth, const float* d_alpha) {
+  const int units = ctx->cam.tiles_x * ctx->cam.tiles_y * (2 / NX) * (4 / NY);
+  if (d_alpha)
+    raster_bwd_kernel<NX, NY, true><<<units, 32, 0, s>>>(ctx->cam.W, ctx->cam.H, ctx->cam.tiles_x, ctx->tile_order,
+                                                          ctx->ranges, ctx->vals[ctx->sorted_buf], ctx->feat,
+                                                          ctx->bg[0], ctx->bg[1], ctx->bg[2], ctx->final_T,
+                                                          ctx->n_contrib, d_rgb, d_depth, d_alpha, ctx->g2d);
+  else
+    raster_bwd_kernel<NX, NY, false><<<units, 32, 0, s>>>(ctx->cam.W, ctx->cam.H, ctx->cam.tiles_x, ctx->tile_order,
+                                                           ctx->ranges, ctx->vals[ctx->sorted_buf], ctx->feat,
+                                                           ctx->bg[0], ctx->bg[1], ctx->bg[2], ctx->final_T,
+                                                           ctx->n_contrib, d_rgb, d_depth, d_alpha, ctx->g2d);
+  GS_LAUNCH_CHECK("raster_bwd_kernel");
+  return GS_OK;
+}
+
+// region shape per warp = (8 NX) x (4 NY) pixels; selectable for tuning (GS_RASTER_FWD / GS_RASTER_BWD = "NXNY")
+#define GS_DISPATCH(shape, F, ...)                      \
+  switch (shape) {                                      \
+    case 11: return F<1, 1>(__VA_ARGS__);               \
+    case 12: return F<1, 2>(__VA_ARGS__);               \
+    case 21: return F<2, 1>(__VA_ARGS__);               \
+    case 22: return F<2, 2>(__VA_ARGS__);               \
+    default: return F<2, 4>(__VA_ARGS__);               \
+  }
+
+int launch_raster_fwd(gs_ctx* ctx, cudaStream_t s, float* rgb, float* depth, float* alpha) {
+  if (ctx->cam.tiles_x * ctx->cam.tiles_y == 0) return GS_OK;
+  GS_DISPATCH(ctx->shape_fwd, launch_fwd_t, ctx, s, rgb, depth, alpha)
+}
+
+int launch_raster_bwd(gs_ctx* ctx, cudaStream_t s, const float* d_rgb, const float* d_depth, const float* d_alpha) {
+  if (ctx->cam.tiles_x * ctx->cam.tiles_y == 0) return GS_OK;
+  GS_DISPATCH(ctx->shape_bwd, launch_bwd_t, ctx, s, d_rgb, d_depth, d_alpha)
 }
 
 // Workload statistics of the forward (introspection only): re-walks every pixel's list with the forward's decisions.
-__global__ void __launch_bounds__(kBatch)
-workload_stats_kernel(int W, int H, int tiles_x, const uint2* __restrict__ ranges, const uint32_t* __restrict__ ids,
-                      const float4* __restrict__ feat, unsigned long long* __restrict__ out) {
-  __shared__ Staged sm[kBatch];
-  const int tile = blockIdx.x;
-  const int ox = (tile % tiles_x) * GS_TILE, oy = (tile / tiles_x) * GS_TILE;
-  int lx, ly;
-  thread_pixel(threadIdx.x, lx, ly);
-  const bool inside = (ox + lx) < W && (oy + ly) < H;
-  const float fx = (float)lx, fy = (float)ly;
-  const uint2 range = ranges[tile];
-  const int n = (int)(range.y - range.x);
-  float T = 1.f;
-  unsigned long long evaluated = 0, blended = 0, last = 0;
-  bool done = !inside;
-  for (int b0 = 0; b0 < n; b0 += kBatch) {
-    __syncthreads();
-    const int idx = b0 + threadIdx.x;
-    if (idx < n) stage_gaussian(feat, __ldg(ids + range.x + idx), ox, oy, sm[threadIdx.x]);
-    __syncthreads();
-    const int cnt = min(kBatch, n - b0);
-    for (int j = 0; j < cnt && !done; ++j) {
-      const float4 g0 = sm[j].g0, g1 = sm[j].g1;
-      ++evaluated;
-      const float a = fminf(GS_ALPHA_MAX, eval_og(fx - g0.x, fy - g0.y, g0.z, g0.w, g1.x, g1.y));
-      if (a < GS_ALPHA_MIN) continue;
-      if (T < GS_T_MIN) { done = true; break; }
-      T = T * (1.f - a);
-      ++blended;
-      last = (unsigned long long)(b0 + j + 1);
-    }
-  }
-  unsigned long long v[4] = {evaluated, blended, last, inside ? (unsigned long long)n : 0ull};
-#pragma unroll
-  for (int k = 0; k < 4; ++k) {
-#pragma unroll
-    for (int d = 16; d >= 1; d >>= 1) v[k] += __shfl_xor_sync(0xffffffffu, v[k], d);
-    if ((threadIdx.x & 31) == 0 && v[k]) atomicAdd(out + k, v[k]);
-  }
-}
-
 int launch_workload_stats(gs_ctx* ctx, cudaStream_t s, uint64_t* out_host) {
   const int tiles = ctx->cam.tiles_x * ctx->cam.tiles_y;
   unsigned long long* d = reinterpret_cast<unsigned long long*>(ctx->pose_acc);  // 16 doubles of scratch, unused here
   GS_CUDA(cudaMemsetAsync(d, 0, 4 * sizeof(unsigned long long), s));
   if (tiles > 0) {
-    workload_stats_kernel<<<tiles, kBatch, 0, s>>>(ctx->cam.W, ctx->cam.H, ctx->cam.tiles_x, ctx->ranges,
-                                                   ctx->vals[ctx->sorted_buf], ctx->feat, d);
-    GS_LAUNCH_CHECK("workload_stats_kernel");
+    raster_fwd_kernel<2, 4, true><<<tiles, 32, 0, s>>>(ctx->cam.W, ctx->cam.H, ctx->cam.tiles_x, ctx->tile_order,
+                                                        ctx->ranges, ctx->vals[ctx->sorted_buf], ctx->feat, 0.f, 0.f,
+                                                        0.f, nullptr, nullptr, nullptr, nullptr, nullptr, d);
+    GS_LAUNCH_CHECK("raster_fwd_kernel<stats>");
   }
   GS_CUDA(cudaMemcpyAsync(out_host, d, 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, s));
   GS_CUDA(cudaStreamSynchronize(s));
   ctx->pose_acc_valid = false;
-  return GS_OK;
-}
-
-int launch_raster_fwd(gs_ctx* ctx, cudaStream_t s, float* rgb, float* depth, float* alpha) {
-  const int tiles = ctx->cam.tiles_x * ctx->cam.tiles_y;
-  if (tiles == 0) return GS_OK;
-  raster_fwd_kernel<<<tiles, kBatch, 0, s>>>(ctx->cam.W, ctx->cam.H, ctx->cam.tiles_x, ctx->ranges,
-                                             ctx->vals[ctx->sorted_buf], ctx->feat, ctx->bg[0], ctx->bg[1], ctx->bg[2],
-                                             rgb, depth, alpha, ctx->final_T, ctx->n_contrib);
-  GS_LAUNCH_CHECK("raster_fwd_kernel");
-  return GS_OK;
-}
-
-int launch_raster_bwd(gs_ctx* ctx, cudaStream_t s, const float* d_rgb, const float* d_depth, const float* d_alpha) {
-  const int tiles = ctx->cam.tiles_x * ctx->cam.tiles_y;
-  if (tiles == 0) return GS_OK;
-  raster_bwd_kernel<<<tiles, kBatch, 0, s>>>(ctx->cam.W, ctx->cam.H, ctx->cam.tiles_x, ctx->ranges,
-                                             ctx->vals[ctx->sorted_buf], ctx->feat, ctx->bg[0], ctx->bg[1], ctx->bg[2],
-                                             ctx->final_T, ctx->n_contrib, d_rgb, d_depth, d_alpha, ctx->g2d);
-  GS_LAUNCH_CHECK("raster_bwd_kernel");
   return GS_OK;
 }
 

@@ -1,19 +1,14 @@
-// gs_raster.cuh -- pieces shared by the forward and backward compositing kernels.  The alpha evaluation MUST be the
-// same instruction sequence in both (the backward re-takes the forward's alpha >= 1/255 decisions), so it is written
-// with explicit rounding intrinsics that the compiler cannot re-associate or contract differently per kernel.
+// gs_raster.cuh -- pieces shared by the forward and backward compositing kernels (v2: one warp per tile region,
+// several interleaved pixels per lane).  The power evaluation MUST be the same instruction sequence in both kernels
+// (the backward re-takes the forward's alpha >= 1/255 decisions), so it is written with explicit rounding intrinsics
+// that the compiler cannot contract or re-associate differently per kernel.
 #pragma once
 
 #include "gs_internal.cuh"
 
 namespace gs {
 
-constexpr int kBatch = 256;  // Gaussians staged in shared memory per round (= threads per tile CTA)
-
-// Staged Gaussian, tile-local: 3 x float4 (broadcast LDS.128 in the inner loop)
-//   g0 = { mx_local, my_local, A, B }   g1 = { C, opacity, r, g }   g2 = { b, z, id (bits), - }
-struct Staged {
-  float4 g0, g1, g2;
-};
+constexpr int kWarpBatch = 32;  // Gaussians staged per round by one warp (one per lane)
 
 __device__ __forceinline__ float ex2_approx(float x) {
   float y;
@@ -21,34 +16,56 @@ __device__ __forceinline__ float ex2_approx(float x) {
   return y;
 }
 
-// power2 = A dx^2 + B dx dy + C dy^2 (log2 units, <= 0 up to rounding); returns opacity * 2^power2 (unclamped).
-__device__ __forceinline__ float eval_og(float dx, float dy, float A, float B, float C, float o) {
-  const float t = __fmaf_rn(A, dx, __fmul_rn(B, dy));
-  float p = __fmul_rn(t, dx);
-  p = __fmaf_rn(__fmul_rn(C, dy), dy, p);
-  return __fmul_rn(o, ex2_approx(p));
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
+  const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() {
+  asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
 }
 
-// Gathers Gaussian `id` and converts its mean to coordinates local to the tile origin (ox, oy): the integer part of the
-// mean minus the origin is exact, the fraction is added in fp32 (absolute pixel coordinates
-// in fp32 would cost ~6e-5 px at x ~ 1000).
-__device__ __forceinline__ void stage_gaussian(const float4* __restrict__ feat, uint32_t id, int ox, int oy,
-                                               Staged& s) {
-  const float4 f0 = __ldg(feat + 3 * (size_t)id);
-  const float4 f1 = __ldg(feat + 3 * (size_t)id + 1);
-  const float4 f2 = __ldg(feat + 3 * (size_t)id + 2);
-  const float mx = (float)(__float_as_int(f0.z) - ox) + f0.x;
-  const float my = (float)(__float_as_int(f0.w) - oy) + f0.y;
-  s.g0 = make_float4(mx, my, f1.x, f1.y);
-  s.g1 = make_float4(f1.z, f1.w, f2.x, f2.y);
-  s.g2 = make_float4(f2.z, f2.w, __uint_as_float(id), 0.f);
+// Pixel slots of a lane.  Lanes form an 8 (x) by 4 (y) grid; slot (kx, ky) of lane (lx, ly) is the pixel
+// (lx + 8 kx, ly + 4 ky) of the warp's region, kx < NX, ky < NY: the region is (8 NX) x (4 NY) pixels and a lane's
+// pixels are INTERLEAVED over it, so that the footprint of one Gaussian falls on few slots of many lanes (SIMT
+// efficiency) rather than on all slots of few lanes.  Slot index k = ky * NX + kx.
+
+// One staged Gaussian, decoded for a region with origin (ox, oy).
+struct GaussReg {
+  float mx, my;       // mean, region-local
+  float A, B, C, o;   // pre-scaled conic, opacity
+  float thr;          // power threshold: alpha >= 1/255 <=> power2 >= thr
+};
+
+__device__ __forceinline__ void decode_gauss(const float4& f0, const float4& f1, int ox, int oy, GaussReg& g) {
+  const int pk = __float_as_int(f0.z);
+  g.mx = (float)(((pk << 16) >> 16) - ox) + f0.x;  // integer part minus origin is exact; fraction added in fp32
+  g.my = (float)((pk >> 16) - oy) + f0.y;
+  g.A = f1.x; g.B = f1.y; g.C = f1.z; g.o = f1.w;
+  g.thr = f0.w;
 }
 
-// Thread -> pixel mapping inside a 16x16 tile: a warp covers an 8x4 patch (less early-exit waste than 16x2).
-__device__ __forceinline__ void thread_pixel(int tid, int& lx, int& ly) {
-  const int warp = tid >> 5, lane = tid & 31;
-  lx = (warp & 1) * 8 + (lane & 7);
-  ly = (warp >> 1) * 4 + (lane >> 3);
+// power2 of every slot: p[ky*NX+kx] = A dx^2 + B dx dy + C dy^2 with the products shared across rows / columns.
+template <int NX, int NY>
+__device__ __forceinline__ void eval_power(const GaussReg& g, float fx0, float fy0, float (&dx)[NX], float (&dy)[NY],
+                                           float (&p)[NX * NY]) {
+  float ax[NX], bx[NX], cy[NY];
+#pragma unroll
+  for (int kx = 0; kx < NX; ++kx) {
+    dx[kx] = __fsub_rn(fx0 + 8.f * kx, g.mx);
+    ax[kx] = __fmul_rn(__fmul_rn(g.A, dx[kx]), dx[kx]);
+    bx[kx] = __fmul_rn(g.B, dx[kx]);
+  }
+#pragma unroll
+  for (int ky = 0; ky < NY; ++ky) {
+    dy[ky] = __fsub_rn(fy0 + 4.f * ky, g.my);
+    cy[ky] = __fmul_rn(__fmul_rn(g.C, dy[ky]), dy[ky]);
+  }
+#pragma unroll
+  for (int ky = 0; ky < NY; ++ky)
+#pragma unroll
+    for (int kx = 0; kx < NX; ++kx) p[ky * NX + kx] = __fmaf_rn(bx[kx], dy[ky], __fadd_rn(ax[kx], cy[ky]));
 }
 
 }  // namespace gs
