@@ -92,9 +92,6 @@ static int ensure_gaussian_capacity(gs_ctx* ctx, int64_t N) {
   if ((rc = grow(ctx, ctx->g2d, cap * kG2D)) != GS_OK) return rc;
   GS_CUDA(cudaMemset(ctx->g2d, 0, (size_t)cap * kG2D * sizeof(float)));
   ctx->g2d_dirty = false;
-  const int64_t chunks = div_up(cap, kScanChunk) + 1;
-  if ((rc = grow(ctx, ctx->scan_status, chunks)) != GS_OK) return rc;
-  ctx->cap_scan_chunks = chunks;
   ctx->cap_N = cap;
   return GS_OK;
 }
@@ -105,6 +102,8 @@ static int ensure_image_capacity(gs_ctx* ctx, int64_t tiles, int64_t pix) {
     GS_CUDA(cudaDeviceSynchronize());
     if ((rc = grow(ctx, ctx->ranges, tiles)) != GS_OK) return rc;
     if ((rc = grow(ctx, ctx->tile_order, tiles)) != GS_OK) return rc;
+    if ((rc = grow(ctx, ctx->tile_count, tiles * kCtrStride)) != GS_OK) return rc;
+    if ((rc = grow(ctx, ctx->tile_cursor, tiles * kCtrStride)) != GS_OK) return rc;
     ctx->cap_tiles = tiles;
   }
   if (pix > ctx->cap_pix) {
@@ -134,8 +133,6 @@ int gs_create(gs_ctx** out, int device) {
   ok = ok && cudaMalloc((void**)&ctx->counts, sizeof(Counts)) == cudaSuccess;
   ok = ok && cudaMemset(ctx->counts, 0, sizeof(Counts)) == cudaSuccess;
   ok = ok && cudaMalloc((void**)&ctx->pose_acc, 16 * sizeof(double)) == cudaSuccess;
-  ok = ok && cudaMalloc((void**)&ctx->sort_hist, kMaxPasses * kRadix * sizeof(uint32_t)) == cudaSuccess;
-  ok = ok && cudaMalloc((void**)&ctx->sort_ticket, (kMaxPasses + 2) * sizeof(uint32_t)) == cudaSuccess;
   ok = ok && cudaHostAlloc((void**)&ctx->mailbox, sizeof(Counts), cudaHostAllocMapped) == cudaSuccess;
   if (ok) {
     memset(ctx->mailbox, 0, sizeof(Counts));
@@ -151,9 +148,9 @@ int gs_destroy(gs_ctx* ctx) {
   cudaSetDevice(ctx->device);
   cudaDeviceSynchronize();
   cudaFree(ctx->feat); cudaFree(ctx->rect); cudaFree(ctx->depth_key); cudaFree(ctx->tiles_touched);
-  cudaFree(ctx->g2d); cudaFree(ctx->scan_status);
+  cudaFree(ctx->g2d);
   for (int b = 0; b < 2; ++b) { cudaFree(ctx->keys[b]); cudaFree(ctx->vals[b]); }
-  cudaFree(ctx->sort_hist); cudaFree(ctx->sort_status); cudaFree(ctx->sort_ticket);
+  cudaFree(ctx->tile_count); cudaFree(ctx->tile_cursor);
   cudaFree(ctx->ranges); cudaFree(ctx->tile_order); cudaFree(ctx->final_T); cudaFree(ctx->n_contrib);
   cudaFree(ctx->pose_acc); cudaFree(ctx->counts); cudaFree(ctx->hb);
   if (ctx->mailbox) cudaFreeHost(ctx->mailbox);
@@ -197,6 +194,7 @@ int gs_preprocess(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, const flo
   ctx->seq++;
   GS_PROF(0, s);
   GS_CUDA(cudaMemsetAsync(ctx->counts, 0, sizeof(Counts), s));
+  GS_CUDA(cudaMemsetAsync(ctx->tile_count, 0, (size_t)c.tiles_x * c.tiles_y * kCtrStride * sizeof(uint32_t), s));
   if ((rc = launch_preprocess(ctx, s)) != GS_OK) return rc;
   GS_PROF(1, s);
   ctx->stage = 1;
@@ -293,7 +291,9 @@ int gs_get_binning(gs_ctx* ctx, void* stream, uint64_t* keys_sorted, uint32_t* i
   int64_t I = 0;
   int rc = gs_get_counts(ctx, stream, nullptr, &I);
   if (rc != GS_OK) return rc;
-  if (keys_sorted && I) GS_CUDA(cudaMemcpyAsync(keys_sorted, ctx->keys[ctx->sorted_buf], (size_t)I * 8, cudaMemcpyDeviceToDevice, s));
+  if (keys_sorted && I) {
+    if ((rc = export_sorted_keys(ctx, s, keys_sorted)) != GS_OK) return rc;
+  }
   if (ids_sorted && I) GS_CUDA(cudaMemcpyAsync(ids_sorted, ctx->vals[ctx->sorted_buf], (size_t)I * 4, cudaMemcpyDeviceToDevice, s));
   if (tile_ranges)
     GS_CUDA(cudaMemcpyAsync(tile_ranges, ctx->ranges, (size_t)ctx->cam.tiles_x * ctx->cam.tiles_y * 8, cudaMemcpyDeviceToDevice, s));

@@ -46,24 +46,17 @@ constexpr int kFeatVec = 3;
 // with gp = alpha * dL/dalpha on unclamped contributions and w = alpha T.
 constexpr int kG2D = 12;
 
+constexpr int kCtrStride = 32;  // per-tile counters are one per 128-byte line (gs_binning.cu)
+
 // Device counters (one per context) + pinned-host mirror ("mailbox") the host may poll without synchronising.
 struct Counts {
   uint32_t n_visible;
   uint32_t n_instances;  // total tile instances of the last scan (even if it overflowed)
   uint32_t overflow;     // 1 if n_instances > capacity: nothing was emitted and downstream kernels see 0 instances
   uint32_t seq;          // iteration number of the writer
+  uint32_t n_large;      // number of tiles whose list is longer than the small-sort capacity
 };
 
-constexpr int kRadixBits = 8;
-constexpr int kRadix = 1 << kRadixBits;
-constexpr int kSortThreads = 256;
-constexpr int kSortKPT = 8;                       // keys per thread
-constexpr int kSortChunk = kSortThreads * kSortKPT;  // keys per block
-constexpr int kMaxPasses = 8;
-
-constexpr int kScanThreads = 256;
-constexpr int kScanIPT = 4;
-constexpr int kScanChunk = kScanThreads * kScanIPT;
 
 }  // namespace gs
 
@@ -91,25 +84,22 @@ struct gs_ctx {
   uint32_t* tiles_touched = nullptr;  // [N]
   float* g2d = nullptr;             // [N,12]; kept all-zero between iterations (the consumer clears what it reads)
   bool g2d_dirty = false;
-  uint64_t* scan_status = nullptr;  // [cap scan chunks]
-  int64_t cap_scan_chunks = 0;
 
   // per-instance scratch (capacity cap_I)
   int64_t cap_I = 0;
   bool calibrated = false;
   int64_t cal_N = -1;
   int32_t cal_W = -1, cal_H = -1;
-  uint64_t* keys[2] = {nullptr, nullptr};
-  uint32_t* vals[2] = {nullptr, nullptr};
+  uint64_t* keys[2] = {nullptr, nullptr};  // [0]: (depth bits << 32 | id) bucketed by tile, sorted in place
+  uint32_t* vals[2] = {nullptr, nullptr};  // [0]: sorted Gaussian ids (what the compositing kernels read)
   int sorted_buf = 0;
-  uint32_t* sort_hist = nullptr;    // [kMaxPasses, 256] global digit histograms -> exclusive bases
-  uint32_t* sort_status = nullptr;  // [kMaxPasses, chunks, 256] decoupled look-back words
-  uint32_t* sort_ticket = nullptr;  // [kMaxPasses + 2] dynamic chunk ids
-  int64_t cap_sort_chunks = 0;
+  bool sort_attr_set = false;
 
   // per-tile / per-pixel scratch
   int64_t cap_tiles = 0, cap_pix = 0;
   uint2* ranges = nullptr;          // [tiles]
+  uint32_t* tile_count = nullptr;   // [tiles] instances per tile (atomics in gs_preprocess)
+  uint32_t* tile_cursor = nullptr;  // [tiles] write cursors of the duplication
   float* final_T = nullptr;         // [H*W]
   uint32_t* n_contrib = nullptr;    // [H*W]
 
@@ -188,6 +178,7 @@ inline Counts read_mailbox(const gs_ctx* ctx) {
   const volatile Counts* m = ctx->mailbox;
   Counts c;
   c.n_visible = m->n_visible; c.n_instances = m->n_instances; c.overflow = m->overflow; c.seq = m->seq;
+  c.n_large = 0;
   return c;
 }
 
@@ -201,6 +192,7 @@ int launch_gauss_bwd(gs_ctx* ctx, cudaStream_t s, uint32_t flags, float* g_means
 int launch_pose_final(gs_ctx* ctx, cudaStream_t s, uint32_t flags, float* g_twist);
 int ensure_instance_capacity(gs_ctx* ctx, int64_t need);
 bool handle_overflow(gs_ctx* ctx);
+int export_sorted_keys(gs_ctx* ctx, cudaStream_t s, uint64_t* out);
 int launch_workload_stats(gs_ctx* ctx, cudaStream_t s, uint64_t* out_host);
 
 }  // namespace gs

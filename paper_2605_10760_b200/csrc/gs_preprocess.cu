@@ -11,7 +11,8 @@ __global__ void __launch_bounds__(256)
 preprocess_kernel(int64_t N, const float* __restrict__ means, const float* __restrict__ scales,
                   const float* __restrict__ quats, const float* __restrict__ opacities, const float* __restrict__ sh,
                   DevCam cam, float4* __restrict__ feat, ushort4* __restrict__ rect, uint32_t* __restrict__ depth_key,
-                  uint32_t* __restrict__ tiles_touched, Counts* __restrict__ counts) {
+                  uint32_t* __restrict__ tiles_touched, uint32_t* __restrict__ tile_count,
+                  Counts* __restrict__ counts) {
   constexpr int K = (DEG + 1) * (DEG + 1);
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   float T[12];
@@ -73,6 +74,8 @@ preprocess_kernel(int64_t N, const float* __restrict__ means, const float* __res
       rect[i] = make_ushort4((unsigned short)tx0, (unsigned short)ty0, (unsigned short)tx1, (unsigned short)ty1);
       depth_key[i] = __float_as_uint(depth_key_f32(T, mu0, mu1, mu2));
       tiles_touched[i] = (uint32_t)((tx1 - tx0) * (ty1 - ty0));
+      for (int ty = ty0; ty < ty1; ++ty)  // MSD digit histogram of the binning sort (gs_binning.cu)
+        for (int tx = tx0; tx < tx1; ++tx) atomicAdd(&tile_count[(size_t)(ty * cam.tiles_x + tx) * kCtrStride], 1u);
     } else {
       tiles_touched[i] = 0u;
     }
@@ -89,7 +92,7 @@ int launch_preprocess(gs_ctx* ctx, cudaStream_t s) {
 #define GS_PRE(D)                                                                                                    \
   preprocess_kernel<D><<<blocks, threads, 0, s>>>(N, ctx->means, ctx->scales, ctx->quats, ctx->opacities, ctx->sh,  \
                                                    ctx->cam, ctx->feat, ctx->rect, ctx->depth_key,                  \
-                                                   ctx->tiles_touched, ctx->counts)
+                                                   ctx->tiles_touched, ctx->tile_count, ctx->counts)
   switch (ctx->sh_degree) {
     case 0: GS_PRE(0); break;
     case 1: GS_PRE(1); break;
