@@ -241,8 +241,8 @@ def run_ours(args):
     else:
         N, K3 = scs[0].N, 3 * (scs[0].sh_degree + 1) ** 2
         V, I = mean("visible"), mean("instances")
-        by = {"preprocess": 44 * N + 4 * K3 * V + 64 * V + 4 * N, "scan_dup": 4 * N + 12 * V + 12 * I,
-              "radix_sort": (8 + 24 * 6) * I, "tile_ranges": 8 * I,
+        by = {"preprocess": 44 * N + 4 * K3 * V + 64 * V + 4 * N, "tile_scan": 16.0 * (W // 16 + 1) * (H // 16 + 1),
+              "emit": 4 * N + 12 * V + 8 * I, "tile_sort": 20 * I,
               "gauss_bwd": (44 + 4 * K3) * V + 96 * V + (44 + 4 * K3) * N, "pose_grad": 120.0}[dominant]
         roof = {"kernel": dominant, "bound": "hbm", "achieved": by / (stage_ms[dominant] * 1e-3) / 1e9,
                 "peak": hbm_peak, "unit": "GB/s"}
@@ -255,7 +255,7 @@ def run_ours(args):
     # whole-iteration HBM figure (BASELINE.json "% HBM roofline"): algorithmic bytes of all stages / step time
     N, K3 = scs[0].N, 3 * (scs[0].sh_degree + 1) ** 2
     V, I, P = mean("visible"), mean("instances"), W * H
-    bytes_iter = (44 * N + 4 * K3 * V + 64 * V + 4 * N) + (4 * N + 12 * V + 12 * I) + 24 * I + 8 * I + \
+    bytes_iter = (44 * N + 4 * K3 * V + 64 * V + 4 * N) + (4 * N + 12 * V + 8 * I) + 20 * I + \
                  (4 * I + 48 * V + 24 * P) + (4 * I + 48 * V + 28 * P + 96 * V) + ((44 + 4 * K3) * V + (44 + 4 * K3) * N)
     hbm_frac_iter = bytes_iter / (ms_total / K * 1e-3) / 1e9 / hbm_peak
 

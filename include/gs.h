@@ -138,7 +138,7 @@ GS_API int gs_poll(gs_ctx* ctx);
 
 /* Stage timing.  gs_profile_enable(ctx, 1) makes the five calls record CUDA events on their stream around each kernel
  * group; gs_profile_read waits for the last gs_pose_grad and returns the device time in milliseconds of the
- * GS_NUM_STAGES groups of the last iteration: preprocess, scan+duplicate, radix sort, tile ranges, raster forward,
+ * GS_NUM_STAGES groups of the last iteration: preprocess, tile scan, duplication (emit), per-tile sort, raster forward,
  * raster backward (pixel part), per-Gaussian backward, pose gradient.  HOST float[GS_NUM_STAGES]. */
 #define GS_NUM_STAGES 8
 GS_API int gs_profile_enable(gs_ctx* ctx, int on);

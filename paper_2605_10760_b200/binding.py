@@ -23,7 +23,7 @@ EXPORTS = ["gs_create", "gs_destroy", "gs_last_error", "gs_preprocess", "gs_bin_
            "gs_rasterize_bwd", "gs_pose_grad", "gs_get_counts", "gs_get_binning", "gs_get_features", "gs_poll",
            "gs_aux_l1_grad", "gs_aux_pose_step", "gs_fwd_bwd_host", "gs_profile_enable", "gs_profile_read",
            "gs_get_launch_count", "gs_get_workload"]
-STAGES = ["preprocess", "scan_dup", "radix_sort", "tile_ranges", "raster_fwd", "raster_bwd", "gauss_bwd", "pose_grad"]
+STAGES = ["preprocess", "tile_scan", "emit", "tile_sort", "raster_fwd", "raster_bwd", "gauss_bwd", "pose_grad"]
 
 
 class GsError(RuntimeError):

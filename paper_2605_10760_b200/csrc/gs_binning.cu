@@ -18,6 +18,7 @@ namespace gs {
 
 constexpr int kSmallSort = 1031;   // buckets up to this size (a whole length/8 class of the tile order): 128-thread CTA, static smem
 constexpr int kLargeSort = 8192;
+constexpr int kScanCache = 8192;   // tile counts cached in shared memory by the scan kernel (all of them up to ~2 Mpix)
 // tile_count / tile_cursor are strided by 32 words: one counter per 128-byte line, so that the atomics of different
 // tiles are served by different L2 lines (3225 adjacent counters would share ~100 lines and serialise there)   // up to this size: 512-thread CTA, 64 KB dynamic shared memory; beyond: global memory
 
@@ -31,14 +32,16 @@ tile_scan_kernel(int tiles, const uint32_t* __restrict__ tile_count, uint32_t* _
   __shared__ uint32_t hist[1024];
   __shared__ uint32_t wsum[32];
   __shared__ uint32_t s_carry, s_large;
+  __shared__ uint32_t s_cnt[kScanCache];  // the counts, fetched once with all loads in flight together
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  for (int t = tid; t < min(tiles, kScanCache); t += 1024) s_cnt[t] = tile_count[(size_t)t * kCtrStride];
   hist[tid] = 0;
   if (tid == 0) { s_carry = 0; s_large = 0; }
   __syncthreads();
   // exclusive scan of the counts, 1024 tiles per round
   for (int base = 0; base < tiles; base += 1024) {
     const int t = base + tid;
-    const uint32_t c = t < tiles ? tile_count[(size_t)t * kCtrStride] : 0u;
+    const uint32_t c = t < tiles ? (t < kScanCache ? s_cnt[t] : tile_count[(size_t)t * kCtrStride]) : 0u;
     uint32_t incl = c;
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {
@@ -91,23 +94,26 @@ tile_scan_kernel(int tiles, const uint32_t* __restrict__ tile_count, uint32_t* _
   hist[tid] = bbase;
   __syncthreads();
   for (int t = tid; t < tiles; t += 1024)
-    order[atomicAdd(&hist[1023 - min(tile_count[(size_t)t * kCtrStride] >> 3, 1023u)], 1u)] = (uint32_t)t;
+    order[atomicAdd(&hist[1023 - min((t < kScanCache ? s_cnt[t] : tile_count[(size_t)t * kCtrStride]) >> 3, 1023u)], 1u)] = (uint32_t)t;
 }
 
 // ---------------------------------------------------------------------------------------------------------------
 // a3: duplication.  One thread per Gaussian; (depth bits << 32 | index) goes to the bucket of every tile of the rect.
 // ---------------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
-emit_kernel(int64_t N, const uint32_t* __restrict__ tiles_touched, const ushort4* __restrict__ rect,
+emit_kernel(const uint32_t* __restrict__ vis_ids, const uint32_t* __restrict__ tiles_touched, const ushort4* __restrict__ rect,
             const uint32_t* __restrict__ depth_key, int tiles_x, uint32_t* __restrict__ tile_cursor,
             const Counts* __restrict__ counts, uint64_t* __restrict__ keys) {
   // Warp-cooperative: the instances of the warp's 32 Gaussians form one work list (prefix sum of the per-lane counts);
   // every round the 32 lanes take 32 consecutive work items, whatever Gaussian they belong to, so a Gaussian covering
   // hundreds of tiles is emitted by the whole warp and 32 independent atomics are in flight per round.
-  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const int lane = threadIdx.x & 31;
   if (counts->overflow) return;
-  uint32_t n = (i < N) ? tiles_touched[i] : 0u;
+  const uint32_t V = counts->n_visible;
+  if (k - lane >= V) return;  // whole warp beyond the compacted list
+  const uint32_t i = (k < V) ? vis_ids[k] : 0u;
+  uint32_t n = (k < V) ? tiles_touched[i] : 0u;
   ushort4 r = make_ushort4(0, 0, 0, 0);
   uint64_t key = 0;
   if (n) {
@@ -292,7 +298,7 @@ int launch_binning(gs_ctx* ctx, cudaStream_t s) {
   }
   GS_PROF(3, s);
   if (ctx->N > 0) {
-    emit_kernel<<<(unsigned)div_up(ctx->N, 256), 256, 0, s>>>(ctx->N, ctx->tiles_touched, ctx->rect, ctx->depth_key,
+    emit_kernel<<<(unsigned)div_up(ctx->N, 256), 256, 0, s>>>(ctx->vis_ids, ctx->tiles_touched, ctx->rect, ctx->depth_key,
                                                               ctx->cam.tiles_x, ctx->tile_cursor, ctx->counts,
                                                               ctx->keys[0]);
     GS_LAUNCH_CHECK("emit_kernel");

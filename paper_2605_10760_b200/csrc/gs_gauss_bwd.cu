@@ -17,17 +17,23 @@ template <int DEG, bool WRITE>
 __global__ void __launch_bounds__(128)
 gauss_bwd_kernel(int64_t N, const float* __restrict__ means, const float* __restrict__ scales,
                  const float* __restrict__ quats, const float* __restrict__ opacities, const float* __restrict__ sh,
-                 DevCam cam, const uint32_t* __restrict__ tiles_touched, float* __restrict__ g2d, bool accumulate,
+                 DevCam cam, const uint32_t* __restrict__ vis_ids, const Counts* __restrict__ counts,
+                 float* __restrict__ g2d, bool accumulate,
                  float* __restrict__ g_means, float* __restrict__ g_scales, float* __restrict__ g_quats,
                  float* __restrict__ g_opac, float* __restrict__ g_sh, double* __restrict__ pose_acc) {
   constexpr int K = (DEG + 1) * (DEG + 1);
-  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  // one thread per VISIBLE Gaussian (compacted list of gs_preprocess); culled Gaussians were zero-filled by memset
+  const int64_t kk = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const uint32_t V = counts->n_visible;
+  if ((int64_t)blockIdx.x * blockDim.x >= (int64_t)V) return;
+  const bool vis = kk < (int64_t)V;
+  const int64_t i = vis ? (int64_t)vis_ids[kk] : 0;
+  (void)N;
   float T[12];
   load_pose(cam, T);
   double acc[15];
 #pragma unroll
   for (int k = 0; k < 15; ++k) acc[k] = 0.0;
-  const bool vis = i < N && tiles_touched[i] > 0;
   if (vis) {
     float4* gp4 = reinterpret_cast<float4*>(g2d + (size_t)i * kG2D);
     const float4 ga = gp4[0], gb = gp4[1], gc = gp4[2];
@@ -182,20 +188,6 @@ gauss_bwd_kernel(int64_t N, const float* __restrict__ means, const float* __rest
       acc[9 + c] = P.J11 * gT[3 + c] + gpc[1] * mud[c];
       acc[12 + c] = P.J02 * gT[c] + P.J12 * gT[3 + c] + gpc[2] * mud[c];
     }
-  } else if (WRITE && i < N && !accumulate) {
-    constexpr int K3 = 3 * K;
-#pragma unroll
-    for (int k = 0; k < 3; ++k) { g_means[3 * i + k] = 0.f; g_scales[3 * i + k] = 0.f; }
-    *reinterpret_cast<float4*>(g_quats + 4 * i) = make_float4(0.f, 0.f, 0.f, 0.f);
-    g_opac[i] = 0.f;
-    float* gsh = g_sh + (int64_t)K3 * i;
-    if constexpr (K3 % 4 == 0) {
-#pragma unroll
-      for (int v = 0; v < K3 / 4; ++v) reinterpret_cast<float4*>(gsh)[v] = make_float4(0.f, 0.f, 0.f, 0.f);
-    } else {
-#pragma unroll
-      for (int k = 0; k < K3; ++k) gsh[k] = 0.f;
-    }
   }
   // block reduction of the 15 pose partials (fp64), one atomic set per block
   __shared__ double s_acc[4][15];
@@ -251,11 +243,19 @@ int launch_gauss_bwd(gs_ctx* ctx, cudaStream_t s, uint32_t flags, float* g_means
   if (ctx->N == 0) return GS_OK;
   const bool write = !(flags & GS_POSE_ONLY);
   const bool accum = (flags & GS_ACCUMULATE) != 0;
+  if (write && !accum) {  // dense outputs: exact zeros for the culled Gaussians, the visible ones are overwritten below
+    const size_t f = sizeof(float), Nn = (size_t)ctx->N, K3 = 3 * (size_t)(ctx->sh_degree + 1) * (ctx->sh_degree + 1);
+    GS_CUDA(cudaMemsetAsync(g_means, 0, Nn * 3 * f, s));
+    GS_CUDA(cudaMemsetAsync(g_scales, 0, Nn * 3 * f, s));
+    GS_CUDA(cudaMemsetAsync(g_quats, 0, Nn * 4 * f, s));
+    GS_CUDA(cudaMemsetAsync(g_opac, 0, Nn * f, s));
+    GS_CUDA(cudaMemsetAsync(g_sh, 0, Nn * K3 * f, s));
+  }
   const int threads = 128;
   const unsigned blocks = (unsigned)div_up(ctx->N, threads);
 #define GS_GB(D, Wr)                                                                                                 \
   gauss_bwd_kernel<D, Wr><<<blocks, threads, 0, s>>>(ctx->N, ctx->means, ctx->scales, ctx->quats, ctx->opacities,   \
-                                                      ctx->sh, ctx->cam, ctx->tiles_touched, ctx->g2d, accum,       \
+                                                      ctx->sh, ctx->cam, ctx->vis_ids, ctx->counts, ctx->g2d, accum, \
                                                       g_means, g_scales, g_quats, g_opac, g_sh, ctx->pose_acc)
   if (write) {
     switch (ctx->sh_degree) {

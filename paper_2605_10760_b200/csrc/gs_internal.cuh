@@ -82,6 +82,7 @@ struct gs_ctx {
   ushort4* rect = nullptr;          // [N] tile rect tx0,ty0,tx1,ty1
   uint32_t* depth_key = nullptr;    // [N]
   uint32_t* tiles_touched = nullptr;  // [N]
+  uint32_t* vis_ids = nullptr;        // [N] indices of the visible Gaussians, compacted (arbitrary order)
   float* g2d = nullptr;             // [N,12]; kept all-zero between iterations (the consumer clears what it reads)
   bool g2d_dirty = false;
 

@@ -12,7 +12,7 @@ preprocess_kernel(int64_t N, const float* __restrict__ means, const float* __res
                   const float* __restrict__ quats, const float* __restrict__ opacities, const float* __restrict__ sh,
                   DevCam cam, float4* __restrict__ feat, ushort4* __restrict__ rect, uint32_t* __restrict__ depth_key,
                   uint32_t* __restrict__ tiles_touched, uint32_t* __restrict__ tile_count,
-                  Counts* __restrict__ counts) {
+                  uint32_t* __restrict__ vis_ids, Counts* __restrict__ counts) {
   constexpr int K = (DEG + 1) * (DEG + 1);
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   float T[12];
@@ -80,8 +80,15 @@ preprocess_kernel(int64_t N, const float* __restrict__ means, const float* __res
       tiles_touched[i] = 0u;
     }
   }
+  // compacted list of visible Gaussians (arbitrary order): the per-Gaussian kernels downstream run on it
   const unsigned ball = __ballot_sync(0xffffffffu, vis);
-  if ((threadIdx.x & 31) == 0 && ball) atomicAdd(&counts->n_visible, (uint32_t)__popc(ball));
+  if (ball) {
+    const int lane = threadIdx.x & 31;
+    uint32_t base = 0;
+    if (lane == 0) base = atomicAdd(&counts->n_visible, (uint32_t)__popc(ball));
+    base = __shfl_sync(0xffffffffu, base, 0);
+    if (vis) vis_ids[base + __popc(ball & ((1u << lane) - 1))] = (uint32_t)i;
+  }
 }
 
 int launch_preprocess(gs_ctx* ctx, cudaStream_t s) {
@@ -92,7 +99,7 @@ int launch_preprocess(gs_ctx* ctx, cudaStream_t s) {
 #define GS_PRE(D)                                                                                                    \
   preprocess_kernel<D><<<blocks, threads, 0, s>>>(N, ctx->means, ctx->scales, ctx->quats, ctx->opacities, ctx->sh,  \
                                                    ctx->cam, ctx->feat, ctx->rect, ctx->depth_key,                  \
-                                                   ctx->tiles_touched, ctx->tile_count, ctx->counts)
+                                                   ctx->tiles_touched, ctx->tile_count, ctx->vis_ids, ctx->counts)
   switch (ctx->sh_degree) {
     case 0: GS_PRE(0); break;
     case 1: GS_PRE(1); break;
