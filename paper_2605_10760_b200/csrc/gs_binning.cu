@@ -104,21 +104,24 @@ __global__ void __launch_bounds__(256)
 emit_kernel(const uint32_t* __restrict__ vis_ids, const uint32_t* __restrict__ tiles_touched, const ushort4* __restrict__ rect,
             const uint32_t* __restrict__ depth_key, int tiles_x, uint32_t* __restrict__ tile_cursor,
             const Counts* __restrict__ counts, uint64_t* __restrict__ keys) {
-  // Warp-cooperative: the instances of the warp's 32 Gaussians form one work list (prefix sum of the per-lane counts);
-  // every round the 32 lanes take 32 consecutive work items, whatever Gaussian they belong to, so a Gaussian covering
-  // hundreds of tiles is emitted by the whole warp and 32 independent atomics are in flight per round.
-  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  const int lane = threadIdx.x & 31;
+  // Block-cooperative: the instances of the block's 256 Gaussians form one work list (prefix sum of the per-Gaussian
+  // tile counts); every round the 256 threads take 256 consecutive work items, whatever Gaussian they belong to, so a
+  // Gaussian covering hundreds of tiles is emitted by the whole block; four independent atomics per thread are put in
+  // flight before their results are used.
+  __shared__ uint32_t s_excl[257], s_w[256], s_xy[256], s_ws[8];
+  __shared__ uint64_t s_key[256];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   if (counts->overflow) return;
   const uint32_t V = counts->n_visible;
-  if (k - lane >= V) return;  // whole warp beyond the compacted list
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + tid;
+  if ((int64_t)blockIdx.x * blockDim.x >= (int64_t)V) return;
   const uint32_t i = (k < V) ? vis_ids[k] : 0u;
-  uint32_t n = (k < V) ? tiles_touched[i] : 0u;
-  ushort4 r = make_ushort4(0, 0, 0, 0);
+  const uint32_t n = (k < V) ? tiles_touched[i] : 0u;
+  ushort4 r = make_ushort4(0, 0, 1, 0);
   uint64_t key = 0;
   if (n) {
     r = rect[i];
-    key = ((uint64_t)depth_key[i] << 32) | (uint64_t)(uint32_t)i;
+    key = ((uint64_t)depth_key[i] << 32) | (uint64_t)i;
   }
   uint32_t incl = n;
 #pragma unroll
@@ -126,29 +129,42 @@ emit_kernel(const uint32_t* __restrict__ vis_ids, const uint32_t* __restrict__ t
     const uint32_t v = __shfl_up_sync(0xffffffffu, incl, d);
     if (lane >= d) incl += v;
   }
-  const uint32_t total = __shfl_sync(0xffffffffu, incl, 31);
-  const uint32_t excl = incl - n;
-  const uint32_t w = (uint32_t)(r.z - r.x);
-  for (uint32_t base = 0; base < total; base += 32) {
-    const uint32_t item = base + lane;
-    // owner = last lane whose exclusive prefix is <= item (binary search over the lanes' prefixes)
-    int owner = 0;
+  if (lane == 31) s_ws[warp] = incl;
+  __syncthreads();
+  uint32_t wb = 0;
 #pragma unroll
-    for (int step = 16; step >= 1; step >>= 1) {
-      const uint32_t e = __shfl_sync(0xffffffffu, excl, owner + step);
-      if (e <= item) owner += step;
+  for (int q = 0; q < 8; ++q) wb += (q < warp) ? s_ws[q] : 0u;
+  s_excl[tid] = wb + incl - n;
+  s_w[tid] = (uint32_t)(r.z - r.x);
+  s_xy[tid] = (uint32_t)r.x | ((uint32_t)r.y << 16);
+  s_key[tid] = key;
+  if (tid == 255) s_excl[256] = wb + incl;
+  __syncthreads();
+  const uint32_t total = s_excl[256];
+  for (uint32_t base = 0; base < total; base += 1024) {
+    uint32_t* cur[4];
+    uint64_t kk[4];
+    uint32_t pos[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const uint32_t item = base + u * 256 + tid;
+      cur[u] = nullptr;
+      if (item < total) {
+        int owner = 0;  // last Gaussian of the block whose exclusive prefix is <= item
+#pragma unroll
+        for (int step = 128; step >= 1; step >>= 1)
+          if (s_excl[owner + step] <= item) owner += step;
+        const uint32_t local = item - s_excl[owner], w = s_w[owner], xy = s_xy[owner];
+        const uint32_t ty = (xy >> 16) + local / w, tx = (xy & 0xffffu) + local % w;
+        cur[u] = &tile_cursor[(size_t)(ty * tiles_x + tx) * kCtrStride];
+        kk[u] = s_key[owner];
+      }
     }
-    const uint32_t o_excl = __shfl_sync(0xffffffffu, excl, owner);
-    const uint32_t o_w = __shfl_sync(0xffffffffu, w, owner);
-    const uint32_t o_x0 = __shfl_sync(0xffffffffu, (uint32_t)r.x, owner);
-    const uint32_t o_y0 = __shfl_sync(0xffffffffu, (uint32_t)r.y, owner);
-    const uint64_t o_key = __shfl_sync(0xffffffffu, key, owner);
-    if (item < total) {
-      const uint32_t local = item - o_excl;
-      const uint32_t ty = o_y0 + local / o_w, tx = o_x0 + local % o_w;
-      const uint32_t pos = atomicAdd(&tile_cursor[(size_t)(ty * tiles_x + tx) * kCtrStride], 1u);
-      keys[pos] = o_key;
-    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) pos[u] = cur[u] ? atomicAdd(cur[u], 1u) : 0u;
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+      if (cur[u]) keys[pos[u]] = kk[u];
   }
 }
 

@@ -243,14 +243,11 @@ int launch_gauss_bwd(gs_ctx* ctx, cudaStream_t s, uint32_t flags, float* g_means
   if (ctx->N == 0) return GS_OK;
   const bool write = !(flags & GS_POSE_ONLY);
   const bool accum = (flags & GS_ACCUMULATE) != 0;
-  if (write && !accum) {  // dense outputs: exact zeros for the culled Gaussians, the visible ones are overwritten below
-    const size_t f = sizeof(float), Nn = (size_t)ctx->N, K3 = 3 * (size_t)(ctx->sh_degree + 1) * (ctx->sh_degree + 1);
-    GS_CUDA(cudaMemsetAsync(g_means, 0, Nn * 3 * f, s));
-    GS_CUDA(cudaMemsetAsync(g_scales, 0, Nn * 3 * f, s));
-    GS_CUDA(cudaMemsetAsync(g_quats, 0, Nn * 4 * f, s));
-    GS_CUDA(cudaMemsetAsync(g_opac, 0, Nn * f, s));
-    GS_CUDA(cudaMemsetAsync(g_sh, 0, Nn * K3 * f, s));
+  if (write && !accum && !ctx->zero_filled) {
+    int rc = launch_zero_fill(ctx, s, g_means, g_scales, g_quats, g_opac, g_sh);
+    if (rc != GS_OK) return rc;
   }
+  ctx->zero_filled = false;
   const int threads = 128;
   const unsigned blocks = (unsigned)div_up(ctx->N, threads);
 #define GS_GB(D, Wr)                                                                                                 \
@@ -274,6 +271,19 @@ int launch_gauss_bwd(gs_ctx* ctx, cudaStream_t s, uint32_t flags, float* g_means
   }
 #undef GS_GB
   GS_LAUNCH_CHECK("gauss_bwd_kernel");
+  return GS_OK;
+}
+
+// Dense outputs: exact zeros for the culled Gaussians (the visible ones are overwritten by gauss_bwd_kernel).
+int launch_zero_fill(gs_ctx* ctx, cudaStream_t s, float* g_means, float* g_scales, float* g_quats, float* g_opac,
+                     float* g_sh) {
+  const size_t f = sizeof(float), Nn = (size_t)ctx->N, K3 = 3 * (size_t)(ctx->sh_degree + 1) * (ctx->sh_degree + 1);
+  if (Nn == 0) return GS_OK;
+  GS_CUDA(cudaMemsetAsync(g_sh, 0, Nn * K3 * f, s));
+  GS_CUDA(cudaMemsetAsync(g_means, 0, Nn * 3 * f, s));
+  GS_CUDA(cudaMemsetAsync(g_scales, 0, Nn * 3 * f, s));
+  GS_CUDA(cudaMemsetAsync(g_quats, 0, Nn * 4 * f, s));
+  GS_CUDA(cudaMemsetAsync(g_opac, 0, Nn * f, s));
   return GS_OK;
 }
 

@@ -116,6 +116,11 @@ struct gs_ctx {
   int shape_fwd = 11, shape_bwd = 11;  // "NXNY": region per warp = (8 NX) x (4 NY) pixels
   uint32_t* tile_order = nullptr;      // [tiles] tile ids by descending list length (longest lists are scheduled first)
 
+  // side stream: the zero fill of the dense gradient arrays overlaps the (ALU-bound) pixel backward
+  cudaStream_t side_stream = nullptr;
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+  bool zero_filled = false;  // set by gs_rasterize_bwd when the fill was issued on the side stream
+
   // stage timing (gs_profile_*): events recorded around the kernel groups when enabled
   bool prof_on = false;
   cudaEvent_t ev[13] = {};
@@ -190,6 +195,7 @@ int launch_raster_fwd(gs_ctx* ctx, cudaStream_t s, float* rgb, float* depth, flo
 int launch_raster_bwd(gs_ctx* ctx, cudaStream_t s, const float* d_rgb, const float* d_depth, const float* d_alpha);
 int launch_gauss_bwd(gs_ctx* ctx, cudaStream_t s, uint32_t flags, float* g_means, float* g_scales, float* g_quats,
                      float* g_opac, float* g_sh);
+int launch_zero_fill(gs_ctx* ctx, cudaStream_t s, float* g_means, float* g_scales, float* g_quats, float* g_opac, float* g_sh);
 int launch_pose_final(gs_ctx* ctx, cudaStream_t s, uint32_t flags, float* g_twist);
 int ensure_instance_capacity(gs_ctx* ctx, int64_t need);
 bool handle_overflow(gs_ctx* ctx);
