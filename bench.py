@@ -135,6 +135,21 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def max_over_ranks(ms_local: float, dist, device) -> float:
+    """Device time of the job = the slowest rank's (replicas only: no data-path collective)."""
+    if dist is None:
+        return float(ms_local)
+    import torch
+    t = torch.tensor([ms_local], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def replica_throughput(world: int, steps: int, ms_total: float) -> float:
+    """Whole-job iterations/s: every rank ran `steps` steps of its own replica in `ms_total` (max over ranks)."""
+    return world * steps / (ms_total / 1e3)
+
+
 def run_ours(args):
     import torch
     from paper_2605_10760_b200 import binding as B
@@ -204,11 +219,8 @@ def run_ours(args):
     ms_total = e0.elapsed_time(e1)
     ctx.gs_poll()
     launches = ctx.gs_get_launch_count() - l0
-    if dist is not None:
-        t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
-    value = world * K / (ms_total / 1e3)
+    ms_total = max_over_ranks(ms_total, dist, dev)
+    value = replica_throughput(world, K, ms_total)
 
     # ---- per-stage device times (second loop, stage events on; same steps) ----
     ctx.gs_profile_enable(True)
