@@ -179,7 +179,7 @@ int gs_preprocess(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, const flo
                   const float* quats, const float* opacities, const float* sh, const gs_camera* cam,
                   const float* T_cw_dev) {
   if (!ctx) return GS_E_INVALID;
-  if (N < 0 || N >= (1ll << 31) || sh_degree < 0 || sh_degree > 3 || !cam) return fail(ctx, GS_E_INVALID, "gs_preprocess: bad N, sh_degree or camera");
+  if (N < 0 || N >= (1ll << 27) || sh_degree < 0 || sh_degree > 3 || !cam) return fail(ctx, GS_E_INVALID, "gs_preprocess: bad N, sh_degree or camera");
   if (N > 0 && (!means || !scales || !quats || !opacities || !sh)) return fail(ctx, GS_E_INVALID, "gs_preprocess: null parameter array");
   if (cam->width <= 0 || cam->height <= 0 || cam->width > 65535 * GS_TILE || cam->height > 65535 * GS_TILE)
     return fail(ctx, GS_E_INVALID, "gs_preprocess: bad image size");

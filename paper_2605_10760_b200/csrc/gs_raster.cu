@@ -24,7 +24,6 @@ namespace gs {
 
 constexpr unsigned kFull = 0xffffffffu;
 constexpr int kGroup = 4;                    // Gaussians evaluated together in phase 2
-constexpr int kSlotsRec = kWarpBatch + 1;    // staged records per buffer: 32 + one never-contributing dummy
 
 // Maximum of power2 over the continuous rectangle [0,xmax] x [0,ymax] (region-local), exact for the concave quadratic:
 // 0 if the centre is inside, else the largest of the four clamped edge maxima.
@@ -45,12 +44,6 @@ __device__ __forceinline__ float region_max_power(const GaussReg& g, float xmax,
   return best;
 }
 
-__device__ __forceinline__ void write_dummy(float4* rec) {
-  rec[0] = make_float4(0.f, 0.f, 0.f, INFINITY);  // thr = +inf: never passes
-  rec[1] = make_float4(0.f, 0.f, 0.f, 0.f);
-  rec[2] = make_float4(0.f, 0.f, 0.f, 0.f);
-}
-
 template <int NX, int NY, bool STATS>
 __global__ void __launch_bounds__(32)
 raster_fwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order, const uint2* __restrict__ ranges, const uint32_t* __restrict__ ids,
@@ -58,7 +51,8 @@ raster_fwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
                   float* __restrict__ depth, float* __restrict__ alpha_out, float* __restrict__ final_T,
                   uint32_t* __restrict__ n_contrib, unsigned long long* __restrict__ stats) {
   constexpr int NS = NX * NY, RX = 2 / NX, RPT = RX * (4 / NY);  // slots per lane, regions per tile
-  __shared__ __align__(16) float4 s_feat[2][kSlotsRec * 3];
+  __shared__ __align__(16) float4 s_feat[2][kWarpBatch * 3];          // raw records, double-buffered (cp.async)
+  __shared__ __align__(16) float4 s_rel[(kWarpBatch + kGroup) * 3];    // decoded records of the relevant Gaussians
   const int lane = threadIdx.x;
   const int tile = (int)__ldg(order + blockIdx.x / RPT), sub = blockIdx.x % RPT;
   const int ox = (tile % tiles_x) * GS_TILE + (sub % RX) * (8 * NX), oy = (tile / tiles_x) * GS_TILE + (sub / RX) * (4 * NY);
@@ -77,7 +71,6 @@ raster_fwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
 #pragma unroll
   for (int k = 0; k < NS; ++k) { T[k] = 1.f; C0[k] = C1[k] = C2[k] = D[k] = 0.f; last[k] = 0; }
   unsigned long long n_eval = 0, n_blend = 0;
-  if (lane < 2) write_dummy(&s_feat[lane][kWarpBatch * 3]);
 
   auto issue = [&](int b, uint32_t id) {
     if (b * kWarpBatch + lane < n) {
@@ -105,35 +98,47 @@ raster_fwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
     __syncwarp();
     const int cnt = min(kWarpBatch, n - b * kWarpBatch);
     const float4* sf = s_feat[b & 1];
-    // phase 1: which Gaussians of the batch can reach this region at all?
+    // phase 1: which Gaussians of the batch can reach this region at all?  Lane g decodes Gaussian g once (region-local
+    // mean) and, if relevant, appends the decoded record to the compact list s_rel in list order.
     bool relevant = false;
+    float4 c0 = make_float4(0.f, 0.f, 0.f, 0.f), c1 = c0;
     if (lane < cnt) {
       GaussReg g;
       decode_gauss(sf[3 * lane], sf[3 * lane + 1], ox, oy, g);
       relevant = region_max_power(g, (float)(8 * NX - 1), (float)(4 * NY - 1)) >= g.thr - 1e-3f;
+      c0 = make_float4(g.mx, g.my, g.A, g.B);
+      c1 = make_float4(g.C, g.o, g.thr, __int_as_float(lane));
     }
-    unsigned rel = __ballot_sync(kFull, relevant);
+    const unsigned rel = __ballot_sync(kFull, relevant);
+    const int nrel = __popc(rel);
+    if (relevant) {
+      const int r = __popc(rel & ((1u << lane) - 1u));
+      s_rel[3 * r] = c0; s_rel[3 * r + 1] = c1; s_rel[3 * r + 2] = sf[3 * lane + 2];
+    }
+    if (lane < kGroup) {  // padding records never pass: p >= NaN is false
+      s_rel[3 * (nrel + lane)] = make_float4(0.f, 0.f, 0.f, 0.f);
+      s_rel[3 * (nrel + lane) + 1] = make_float4(0.f, 0.f, __int_as_float(0x7fc00000), 0.f);
+    }
+    __syncwarp();
     // phase 2: front to back, four list entries at a time
-    while (rel) {
+    for (int r0 = 0; r0 < nrel; r0 += kGroup) {
       int jj[kGroup];
-#pragma unroll
-      for (int q = 0; q < kGroup; ++q) {
-        jj[q] = rel ? (__ffs(rel) - 1) : kWarpBatch;  // kWarpBatch = the dummy record
-        rel &= rel - 1;
-      }
       GaussReg g[kGroup];
       float dx[kGroup][NX], dy[kGroup][NY], p[kGroup][NS];
       unsigned m = 0;
 #pragma unroll
       for (int q = 0; q < kGroup; ++q) {
-        decode_gauss(sf[3 * jj[q]], sf[3 * jj[q] + 1], ox, oy, g[q]);
+        const float4 a0 = s_rel[3 * (r0 + q)], a1 = s_rel[3 * (r0 + q) + 1];
+        g[q].mx = a0.x; g[q].my = a0.y; g[q].A = a0.z; g[q].B = a0.w;
+        g[q].C = a1.x; g[q].o = a1.y; g[q].thr = a1.z;
+        jj[q] = __float_as_int(a1.w);
         eval_power<NX, NY>(g[q], fx0, fy0, dx[q], dy[q], p[q]);
 #pragma unroll
         for (int k = 0; k < NS; ++k) m |= (p[q][k] >= g[q].thr) ? (1u << (q * NS + k)) : 0u;
       }
       if (STATS) {
 #pragma unroll
-        for (int q = 0; q < kGroup; ++q) n_eval += (jj[q] < kWarpBatch) ? __popc(alive) : 0;
+        for (int q = 0; q < kGroup; ++q) n_eval += (r0 + q < nrel) ? __popc(alive) : 0;
       }
       constexpr unsigned kRep = 1u | (1u << NS) | (1u << (2 * NS)) | (1u << (3 * NS));  // replicate the slot mask over the group
       const unsigned any = __reduce_or_sync(kFull, m & (alive * kRep));
@@ -141,7 +146,7 @@ raster_fwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
 #pragma unroll
       for (int q = 0; q < kGroup; ++q) {
         if (((any >> (q * NS)) & ((1u << NS) - 1)) == 0) continue;
-        const float4 f2 = sf[3 * jj[q] + 2];
+        const float4 f2 = s_rel[3 * (r0 + q) + 2];
         const unsigned mq = (m >> (q * NS)) & alive;
 #pragma unroll
         for (int k = 0; k < NS; ++k) {
@@ -235,8 +240,9 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
                   const uint32_t* __restrict__ n_contrib, const float* __restrict__ d_rgb,
                   const float* __restrict__ d_depth, const float* __restrict__ d_alpha, float* __restrict__ g2d) {
   constexpr int NS = NX * NY, RX = 2 / NX, RPT = RX * (4 / NY);  // slots per lane, regions per tile
-  __shared__ __align__(16) float4 s_feat[2][kSlotsRec * 3];
-  __shared__ uint32_t s_id[2][kSlotsRec];
+  __shared__ __align__(16) float4 s_feat[2][kWarpBatch * 3];
+  __shared__ __align__(16) float4 s_rel[(kWarpBatch + kGroup) * 3];
+  __shared__ uint32_t s_id[2][kWarpBatch];
   const int lane = threadIdx.x;
   const int tile = (int)__ldg(order + blockIdx.x / RPT), sub = blockIdx.x % RPT;
   const int ox = (tile % tiles_x) * GS_TILE + (sub % RX) * (8 * NX), oy = (tile / tiles_x) * GS_TILE + (sub / RX) * (4 * NY);
@@ -266,7 +272,6 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
   maxlast = __reduce_max_sync(kFull, maxlast);  // deepest blended list position of the region
   const int n = (int)maxlast;
   const int nb = (n + kWarpBatch - 1) / kWarpBatch;
-  if (lane < 2) { write_dummy(&s_feat[lane][kWarpBatch * 3]); s_id[lane][kWarpBatch] = 0; }
 
   auto issue = [&](int b, uint32_t id) {
     if (b * kWarpBatch + lane < n) {
@@ -294,28 +299,41 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
     __syncwarp();
     const int cnt = min(kWarpBatch, n - b * kWarpBatch);
     const float4* sf = s_feat[b & 1];
+    // phase 1 (see the forward): decoded records of the relevant Gaussians, compacted in REVERSE list order; the
+    // fourth word of the second vector carries (Gaussian id << 5 | position in the batch)
     bool relevant = false;
+    float4 c0 = make_float4(0.f, 0.f, 0.f, 0.f), c1 = c0;
     if (lane < cnt) {
       GaussReg g;
       decode_gauss(sf[3 * lane], sf[3 * lane + 1], ox, oy, g);
       relevant = region_max_power(g, (float)(8 * NX - 1), (float)(4 * NY - 1)) >= g.thr - 1e-3f;
+      c0 = make_float4(g.mx, g.my, g.A, g.B);
+      c1 = make_float4(g.C, g.o, g.thr, __uint_as_float((s_id[b & 1][lane] << 5) | (uint32_t)lane));
     }
-    unsigned rel = __ballot_sync(kFull, relevant);
-    while (rel) {  // back to front, four list entries at a time
-      int jj[kGroup];
-#pragma unroll
-      for (int q = 0; q < kGroup; ++q) {
-        jj[q] = rel ? (31 - __clz(rel)) : kWarpBatch;
-        if (rel) rel &= ~(1u << jj[q]);
-      }
+    const unsigned rel = __ballot_sync(kFull, relevant);
+    const int nrel = __popc(rel);
+    if (relevant) {
+      const int r = nrel - 1 - __popc(rel & ((1u << lane) - 1u));
+      s_rel[3 * r] = c0; s_rel[3 * r + 1] = c1; s_rel[3 * r + 2] = sf[3 * lane + 2];
+    }
+    if (lane < kGroup) {  // padding records never pass: p >= NaN is false
+      s_rel[3 * (nrel + lane)] = make_float4(0.f, 0.f, 0.f, 0.f);
+      s_rel[3 * (nrel + lane) + 1] = make_float4(0.f, 0.f, __int_as_float(0x7fc00000), 0.f);
+    }
+    __syncwarp();
+    for (int r0 = 0; r0 < nrel; r0 += kGroup) {  // back to front, four list entries at a time
+      uint32_t tag[kGroup];
       GaussReg g[kGroup];
       float dx[kGroup][NX], dy[kGroup][NY], p[kGroup][NS];
       unsigned m = 0;
 #pragma unroll
       for (int q = 0; q < kGroup; ++q) {
-        decode_gauss(sf[3 * jj[q]], sf[3 * jj[q] + 1], ox, oy, g[q]);
+        const float4 a0 = s_rel[3 * (r0 + q)], a1 = s_rel[3 * (r0 + q) + 1];
+        g[q].mx = a0.x; g[q].my = a0.y; g[q].A = a0.z; g[q].B = a0.w;
+        g[q].C = a1.x; g[q].o = a1.y; g[q].thr = a1.z;
+        tag[q] = __float_as_uint(a1.w);
         eval_power<NX, NY>(g[q], fx0, fy0, dx[q], dy[q], p[q]);
-        const uint32_t pos = (uint32_t)(b * kWarpBatch + jj[q]);
+        const uint32_t pos = (uint32_t)(b * kWarpBatch) + (tag[q] & 31u);
 #pragma unroll
         for (int k = 0; k < NS; ++k) m |= (p[q][k] >= g[q].thr && pos < last[k]) ? (1u << (q * NS + k)) : 0u;
       }
@@ -324,8 +342,8 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
 #pragma unroll
       for (int q = 0; q < kGroup; ++q) {
         if (((any >> (q * NS)) & ((1u << NS) - 1)) == 0) continue;
-        const float4 f2 = sf[3 * jj[q] + 2];
-        const uint32_t id = s_id[b & 1][jj[q]];
+        const float4 f2 = s_rel[3 * (r0 + q) + 2];
+        const uint32_t id = tag[q] >> 5;
         float tAx[NX], tBx[NX], tCy[NY], tBy[NY];
 #pragma unroll
         for (int kx = 0; kx < NX; ++kx) { tAx[kx] = 2.f * g[q].A * dx[q][kx]; tBx[kx] = g[q].B * dx[q][kx]; }
