@@ -129,7 +129,6 @@ int gs_create(gs_ctx** out, int device) {
   if (!ctx) return GS_E_NOMEM;
   ctx->device = device;
   if (const char* e = getenv("GS_RASTER_FWD")) ctx->shape_fwd = atoi(e);
-  if (const char* e = getenv("GS_RASTER_BWD")) ctx->shape_bwd = atoi(e);
   bool ok = cudaSetDevice(device) == cudaSuccess;
   ok = ok && cudaMalloc((void**)&ctx->counts, sizeof(Counts)) == cudaSuccess;
   ok = ok && cudaMemset(ctx->counts, 0, sizeof(Counts)) == cudaSuccess;

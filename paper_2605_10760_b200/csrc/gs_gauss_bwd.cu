@@ -46,8 +46,8 @@ gauss_bwd_kernel(int64_t N, const float* __restrict__ means, const float* __rest
     ProjD P;
     project_gaussian(cam, T, mu0, mu1, mu2, s0, s1, s2, q.x, q.y, q.z, q.w, o, P);
     const double W[9] = {T[0], T[1], T[2], T[4], T[5], T[6], T[8], T[9], T[10]};
-    const double ln2 = 0.6931471805599453;
-    const double g_mx = -ln2 * (double)ga.x, g_my = -ln2 * (double)ga.y;
+    // ga.x, ga.y = sum gp dx, sum gp dy (moments about the mean); d power / d mean = -(Q d), ln2 * log2(e) = 1
+    const double g_mx = P.a * (double)ga.x + P.b * (double)ga.y, g_my = P.b * (double)ga.x + P.c * (double)ga.y;
     const double g_a = -0.5 * (double)ga.z, g_b = -(double)ga.w, g_c = -0.5 * (double)gb.x;
     const double g_o = (double)gb.y / (double)o;
     const float gcol[3] = {gb.z, gb.w, gc.x};

@@ -41,7 +41,7 @@ __device__ __forceinline__ void load_pose(const DevCam& cam, float* T) {
 constexpr int kFeatVec = 3;
 
 // 2-D gradient record accumulated by the pixel backward (global atomics), 12 floats = 48 B per Gaussian:
-//   [0] sum gp (2A dx + B dy)   [1] sum gp (B dx + 2C dy)   [2] sum gp dx^2   [3] sum gp dx dy   [4] sum gp dy^2
+//   [0] sum gp dx               [1] sum gp dy               [2] sum gp dx^2   [3] sum gp dx dy   [4] sum gp dy^2
 //   [5] sum gp                  [6..8] sum w gC             [9] sum w gD      [10],[11] unused
 // with gp = alpha * dL/dalpha on unclamped contributions and w = alpha T.
 constexpr int kG2D = 12;
@@ -113,7 +113,7 @@ struct gs_ctx {
   gs::Counts* mailbox_dev = nullptr;  // device alias of the mailbox
 
   // region shape of the compositing kernels; tuning knobs GS_RASTER_FWD / GS_RASTER_BWD read by gs_create.
-  int shape_fwd = 11, shape_bwd = 11;  // "NXNY": region per warp = (8 NX) x (4 NY) pixels
+  int shape_fwd = 11;  // forward "NXNY": region per warp = (8 NX) x (4 NY) pixels (the backward is fixed at 8 x 4)
   uint32_t* tile_order = nullptr;      // [tiles] tile ids by descending list length (longest lists are scheduled first)
 
   // side stream: the zero fill of the dense gradient arrays overlaps the (ALU-bound) pixel backward

@@ -22,28 +22,6 @@
 
 namespace gs {
 
-constexpr unsigned kFull = 0xffffffffu;
-constexpr int kGroup = 4;                    // Gaussians evaluated together in phase 2
-
-// Maximum of power2 over the continuous rectangle [0,xmax] x [0,ymax] (region-local), exact for the concave quadratic:
-// 0 if the centre is inside, else the largest of the four clamped edge maxima.
-__device__ __forceinline__ float region_max_power(const GaussReg& g, float xmax, float ymax) {
-  const float x0 = -g.mx, x1 = xmax - g.mx, y0 = -g.my, y1 = ymax - g.my;  // rectangle in centre-relative coordinates
-  if (x0 <= 0.f && x1 >= 0.f && y0 <= 0.f && y1 >= 0.f) return 0.f;
-  const float i2C = __frcp_rn(2.f * g.C), i2A = __frcp_rn(2.f * g.A);
-  float best = -INFINITY;
-#pragma unroll
-  for (int e = 0; e < 2; ++e) {
-    const float dxe = e ? x1 : x0;
-    const float dys = fminf(fmaxf(-g.B * dxe * i2C, y0), y1);
-    best = fmaxf(best, g.A * dxe * dxe + g.B * dxe * dys + g.C * dys * dys);
-    const float dye = e ? y1 : y0;
-    const float dxs = fminf(fmaxf(-g.B * dye * i2A, x0), x1);
-    best = fmaxf(best, g.A * dxs * dxs + g.B * dxs * dye + g.C * dye * dye);
-  }
-  return best;
-}
-
 template <int NX, int NY, bool STATS>
 __global__ void __launch_bounds__(32)
 raster_fwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order, const uint2* __restrict__ ranges, const uint32_t* __restrict__ ids,
@@ -205,192 +183,6 @@ raster_fwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
   }
 }
 
-// 16-slot butterfly reduce-scatter over the warp: on return lane l holds the warp total of slot l >> 1.
-__device__ __forceinline__ float reduce_scatter16(float (&v)[16], int lane) {
-#pragma unroll
-  for (int i = 0; i < 8; ++i) {
-    const bool up = lane & 16;
-    const float send = up ? v[i] : v[i + 8], keep = up ? v[i + 8] : v[i];
-    v[i] = keep + __shfl_xor_sync(kFull, send, 16);
-  }
-#pragma unroll
-  for (int i = 0; i < 4; ++i) {
-    const bool up = lane & 8;
-    const float send = up ? v[i] : v[i + 4], keep = up ? v[i + 4] : v[i];
-    v[i] = keep + __shfl_xor_sync(kFull, send, 8);
-  }
-#pragma unroll
-  for (int i = 0; i < 2; ++i) {
-    const bool up = lane & 4;
-    const float send = up ? v[i] : v[i + 2], keep = up ? v[i + 2] : v[i];
-    v[i] = keep + __shfl_xor_sync(kFull, send, 4);
-  }
-  {
-    const bool up = lane & 2;
-    const float send = up ? v[0] : v[1], keep = up ? v[1] : v[0];
-    v[0] = keep + __shfl_xor_sync(kFull, send, 2);
-  }
-  return v[0] + __shfl_xor_sync(kFull, v[0], 1);
-}
-
-template <int NX, int NY, bool HAS_GA>
-__global__ void __launch_bounds__(32)
-raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order, const uint2* __restrict__ ranges, const uint32_t* __restrict__ ids,
-                  const float4* __restrict__ feat, float bg0, float bg1, float bg2, const float* __restrict__ final_T,
-                  const uint32_t* __restrict__ n_contrib, const float* __restrict__ d_rgb,
-                  const float* __restrict__ d_depth, const float* __restrict__ d_alpha, float* __restrict__ g2d) {
-  constexpr int NS = NX * NY, RX = 2 / NX, RPT = RX * (4 / NY);  // slots per lane, regions per tile
-  __shared__ __align__(16) float4 s_feat[2][kWarpBatch * 3];
-  __shared__ __align__(16) float4 s_rel[(kWarpBatch + kGroup) * 3];
-  __shared__ uint32_t s_id[2][kWarpBatch];
-  const int lane = threadIdx.x;
-  const int tile = (int)__ldg(order + blockIdx.x / RPT), sub = blockIdx.x % RPT;
-  const int ox = (tile % tiles_x) * GS_TILE + (sub % RX) * (8 * NX), oy = (tile / tiles_x) * GS_TILE + (sub / RX) * (4 * NY);
-  const int lx = lane & 7, ly = lane >> 3;
-  const float fx0 = (float)lx, fy0 = (float)ly;
-  const uint2 range = ranges[tile];
-  float T[NS], S[NS], gC0[NS], gC1[NS], gC2[NS], gD[NS], gA[HAS_GA ? NS : 1];
-  uint32_t last[NS];
-  const size_t HW = (size_t)W * H;
-  uint32_t maxlast = 0;
-#pragma unroll
-  for (int k = 0; k < NS; ++k) {
-    const int X = ox + lx + 8 * (k % NX), Y = oy + ly + 4 * (k / NX);
-    T[k] = 1.f; last[k] = 0; gC0[k] = gC1[k] = gC2[k] = gD[k] = 0.f;
-    if (HAS_GA) gA[k] = 0.f;
-    if (X < W && Y < H) {
-      const size_t p = (size_t)Y * W + X;
-      T[k] = final_T[p];
-      last[k] = n_contrib[p];
-      gC0[k] = d_rgb[p]; gC1[k] = d_rgb[HW + p]; gC2[k] = d_rgb[2 * HW + p];
-      if (d_depth) gD[k] = d_depth[p];
-      if (HAS_GA) gA[k] = d_alpha[p];
-    }
-    S[k] = T[k] * (gC0[k] * bg0 + gC1[k] * bg1 + gC2[k] * bg2);
-    maxlast = max(maxlast, last[k]);
-  }
-  maxlast = __reduce_max_sync(kFull, maxlast);  // deepest blended list position of the region
-  const int n = (int)maxlast;
-  const int nb = (n + kWarpBatch - 1) / kWarpBatch;
-
-  auto issue = [&](int b, uint32_t id) {
-    if (b * kWarpBatch + lane < n) {
-      const float4* src = feat + 3 * (size_t)id;
-      float4* dst = &s_feat[b & 1][lane * 3];
-      cp_async16(dst, src); cp_async16(dst + 1, src + 1); cp_async16(dst + 2, src + 2);
-      s_id[b & 1][lane] = id;
-    }
-    cp_async_commit();
-  };
-  uint32_t id_next = 0;
-  if (nb > 0) {
-    const int i0 = (nb - 1) * kWarpBatch + lane;
-    issue(nb - 1, i0 < n ? __ldg(ids + range.x + i0) : 0u);
-    if (nb > 1) id_next = __ldg(ids + range.x + (nb - 2) * kWarpBatch + lane);
-  }
-  for (int b = nb - 1; b >= 0; --b) {
-    if (b >= 1) {
-      issue(b - 1, id_next);
-      if (b >= 2) id_next = __ldg(ids + range.x + (b - 2) * kWarpBatch + lane);
-      cp_async_wait<1>();
-    } else {
-      cp_async_wait<0>();
-    }
-    __syncwarp();
-    const int cnt = min(kWarpBatch, n - b * kWarpBatch);
-    const float4* sf = s_feat[b & 1];
-    // phase 1 (see the forward): decoded records of the relevant Gaussians, compacted in REVERSE list order; the
-    // fourth word of the second vector carries (Gaussian id << 5 | position in the batch)
-    bool relevant = false;
-    float4 c0 = make_float4(0.f, 0.f, 0.f, 0.f), c1 = c0;
-    if (lane < cnt) {
-      GaussReg g;
-      decode_gauss(sf[3 * lane], sf[3 * lane + 1], ox, oy, g);
-      relevant = region_max_power(g, (float)(8 * NX - 1), (float)(4 * NY - 1)) >= g.thr - 1e-3f;
-      c0 = make_float4(g.mx, g.my, g.A, g.B);
-      c1 = make_float4(g.C, g.o, g.thr, __uint_as_float((s_id[b & 1][lane] << 5) | (uint32_t)lane));
-    }
-    const unsigned rel = __ballot_sync(kFull, relevant);
-    const int nrel = __popc(rel);
-    if (relevant) {
-      const int r = nrel - 1 - __popc(rel & ((1u << lane) - 1u));
-      s_rel[3 * r] = c0; s_rel[3 * r + 1] = c1; s_rel[3 * r + 2] = sf[3 * lane + 2];
-    }
-    if (lane < kGroup) {  // padding records never pass: p >= NaN is false
-      s_rel[3 * (nrel + lane)] = make_float4(0.f, 0.f, 0.f, 0.f);
-      s_rel[3 * (nrel + lane) + 1] = make_float4(0.f, 0.f, __int_as_float(0x7fc00000), 0.f);
-    }
-    __syncwarp();
-    for (int r0 = 0; r0 < nrel; r0 += kGroup) {  // back to front, four list entries at a time
-      uint32_t tag[kGroup];
-      GaussReg g[kGroup];
-      float dx[kGroup][NX], dy[kGroup][NY], p[kGroup][NS];
-      unsigned m = 0;
-#pragma unroll
-      for (int q = 0; q < kGroup; ++q) {
-        const float4 a0 = s_rel[3 * (r0 + q)], a1 = s_rel[3 * (r0 + q) + 1];
-        g[q].mx = a0.x; g[q].my = a0.y; g[q].A = a0.z; g[q].B = a0.w;
-        g[q].C = a1.x; g[q].o = a1.y; g[q].thr = a1.z;
-        tag[q] = __float_as_uint(a1.w);
-        eval_power<NX, NY>(g[q], fx0, fy0, dx[q], dy[q], p[q]);
-        const uint32_t pos = (uint32_t)(b * kWarpBatch) + (tag[q] & 31u);
-#pragma unroll
-        for (int k = 0; k < NS; ++k) m |= (p[q][k] >= g[q].thr && pos < last[k]) ? (1u << (q * NS + k)) : 0u;
-      }
-      const unsigned any = __reduce_or_sync(kFull, m);
-      if (any == 0) continue;
-#pragma unroll
-      for (int q = 0; q < kGroup; ++q) {
-        if (((any >> (q * NS)) & ((1u << NS) - 1)) == 0) continue;
-        const float4 f2 = s_rel[3 * (r0 + q) + 2];
-        const uint32_t id = tag[q] >> 5;
-        float tAx[NX], tBx[NX], tCy[NY], tBy[NY];
-#pragma unroll
-        for (int kx = 0; kx < NX; ++kx) { tAx[kx] = 2.f * g[q].A * dx[q][kx]; tBx[kx] = g[q].B * dx[q][kx]; }
-#pragma unroll
-        for (int ky = 0; ky < NY; ++ky) { tCy[ky] = 2.f * g[q].C * dy[q][ky]; tBy[ky] = g[q].B * dy[q][ky]; }
-        float v[16];
-#pragma unroll
-        for (int u = 0; u < 16; ++u) v[u] = 0.f;
-#pragma unroll
-        for (int k = 0; k < NS; ++k) {
-          if (any & (1u << (q * NS + k))) {
-            if (m & (1u << (q * NS + k))) {
-              const int kx = k % NX, ky = k / NX;
-              const float og = __fmul_rn(g[q].o, ex2_approx(p[q][k]));
-              const float a = fminf(GS_ALPHA_MAX, og);
-              const float ioma = __frcp_rn(1.f - a);
-              const float Tk = T[k] * ioma;  // transmittance in front of this Gaussian
-              T[k] = Tk;
-              const float w = a * Tk;
-              float wi = fmaf(gC0[k], f2.x, fmaf(gC1[k], f2.y, fmaf(gC2[k], f2.z, gD[k] * f2.w)));
-              if (HAS_GA) wi += gA[k];
-              const float dalpha = fmaf(Tk, wi, -S[k] * ioma);
-              S[k] = fmaf(wi, w, S[k]);
-              v[6] = fmaf(w, gC0[k], v[6]);
-              v[7] = fmaf(w, gC1[k], v[7]);
-              v[8] = fmaf(w, gC2[k], v[8]);
-              v[9] = fmaf(w, gD[k], v[9]);
-              if (og <= GS_ALPHA_MAX) {
-                const float gp = a * dalpha;
-                v[0] = fmaf(gp, tAx[kx] + tBy[ky], v[0]);
-                v[1] = fmaf(gp, tCy[ky] + tBx[kx], v[1]);
-                v[2] = fmaf(gp * dx[q][kx], dx[q][kx], v[2]);
-                v[3] = fmaf(gp * dx[q][kx], dy[q][ky], v[3]);
-                v[4] = fmaf(gp * dy[q][ky], dy[q][ky], v[4]);
-                v[5] += gp;
-              }
-            }
-          }
-        }
-        const float tot = reduce_scatter16(v, lane);
-        if ((lane & 1) == 0 && lane < 20) atomicAdd(g2d + (size_t)id * kG2D + (lane >> 1), tot);
-      }
-    }
-    __syncwarp();
-  }
-}
-
 template <int NX, int NY>
 static int launch_fwd_t(gs_ctx* ctx, cudaStream_t s, float* rgb, float* depth, float* alpha) {
   const int units = ctx->cam.tiles_x * ctx->cam.tiles_y * (2 / NX) * (4 / NY);
@@ -399,23 +191,6 @@ static int launch_fwd_t(gs_ctx* ctx, cudaStream_t s, float* rgb, float* depth, f
                                                          ctx->bg[0], ctx->bg[1], ctx->bg[2], rgb, depth, alpha,
                                                          ctx->final_T, ctx->n_contrib, nullptr);
   GS_LAUNCH_CHECK("raster_fwd_kernel");
-  return GS_OK;
-}
-
-template <int NX, int NY>
-static int launch_bwd_t(gs_ctx* ctx, cudaStream_t s, const float* d_rgb, const float* d_depth, const float* d_alpha) {
-  const int units = ctx->cam.tiles_x * ctx->cam.tiles_y * (2 / NX) * (4 / NY);
-  if (d_alpha)
-    raster_bwd_kernel<NX, NY, true><<<units, 32, 0, s>>>(ctx->cam.W, ctx->cam.H, ctx->cam.tiles_x, ctx->tile_order,
-                                                          ctx->ranges, ctx->vals[ctx->sorted_buf], ctx->feat,
-                                                          ctx->bg[0], ctx->bg[1], ctx->bg[2], ctx->final_T,
-                                                          ctx->n_contrib, d_rgb, d_depth, d_alpha, ctx->g2d);
-  else
-    raster_bwd_kernel<NX, NY, false><<<units, 32, 0, s>>>(ctx->cam.W, ctx->cam.H, ctx->cam.tiles_x, ctx->tile_order,
-                                                           ctx->ranges, ctx->vals[ctx->sorted_buf], ctx->feat,
-                                                           ctx->bg[0], ctx->bg[1], ctx->bg[2], ctx->final_T,
-                                                           ctx->n_contrib, d_rgb, d_depth, d_alpha, ctx->g2d);
-  GS_LAUNCH_CHECK("raster_bwd_kernel");
   return GS_OK;
 }
 
@@ -432,11 +207,6 @@ static int launch_bwd_t(gs_ctx* ctx, cudaStream_t s, const float* d_rgb, const f
 int launch_raster_fwd(gs_ctx* ctx, cudaStream_t s, float* rgb, float* depth, float* alpha) {
   if (ctx->cam.tiles_x * ctx->cam.tiles_y == 0) return GS_OK;
   GS_DISPATCH(ctx->shape_fwd, launch_fwd_t, ctx, s, rgb, depth, alpha)
-}
-
-int launch_raster_bwd(gs_ctx* ctx, cudaStream_t s, const float* d_rgb, const float* d_depth, const float* d_alpha) {
-  if (ctx->cam.tiles_x * ctx->cam.tiles_y == 0) return GS_OK;
-  GS_DISPATCH(ctx->shape_bwd, launch_bwd_t, ctx, s, d_rgb, d_depth, d_alpha)
 }
 
 // Workload statistics of the forward (introspection only): re-walks every pixel's list with the forward's decisions.

@@ -68,4 +68,32 @@ __device__ __forceinline__ void eval_power(const GaussReg& g, float fx0, float f
     for (int kx = 0; kx < NX; ++kx) p[ky * NX + kx] = __fmaf_rn(bx[kx], dy[ky], __fadd_rn(ax[kx], cy[ky]));
 }
 
+__device__ __forceinline__ float rcp_approx(float x) {
+  float y;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+
+constexpr unsigned kFull = 0xffffffffu;
+constexpr int kGroup = 4;                    // Gaussians evaluated together in phase 2
+
+// Maximum of power2 over the continuous rectangle [0,xmax] x [0,ymax] (region-local), exact for the concave quadratic:
+// 0 if the centre is inside, else the largest of the four clamped edge maxima.
+__device__ __forceinline__ float region_max_power(const GaussReg& g, float xmax, float ymax) {
+  const float x0 = -g.mx, x1 = xmax - g.mx, y0 = -g.my, y1 = ymax - g.my;  // rectangle in centre-relative coordinates
+  if (x0 <= 0.f && x1 >= 0.f && y0 <= 0.f && y1 >= 0.f) return 0.f;
+  const float i2C = rcp_approx(2.f * g.C), i2A = rcp_approx(2.f * g.A);  // the test has 1e-3 of slack
+  float best = -INFINITY;
+#pragma unroll
+  for (int e = 0; e < 2; ++e) {
+    const float dxe = e ? x1 : x0;
+    const float dys = fminf(fmaxf(-g.B * dxe * i2C, y0), y1);
+    best = fmaxf(best, g.A * dxe * dxe + g.B * dxe * dys + g.C * dys * dys);
+    const float dye = e ? y1 : y0;
+    const float dxs = fminf(fmaxf(-g.B * dye * i2A, x0), x1);
+    best = fmaxf(best, g.A * dxs * dxs + g.B * dxs * dye + g.C * dye * dye);
+  }
+  return best;
+}
+
 }  // namespace gs

@@ -1,0 +1,240 @@
+// gs_raster_bwd.cu -- step a8: back-to-front per-pixel backward of the compositing, reduced per (region, Gaussian)
+// before global atomics.
+//
+// v4 design (evidence: profiles/r1_v3_regions.md -- one warp per 8x4-pixel region, one pixel per lane; the register
+// butterfly that reduced the 10 per-Gaussian sums over the lanes was 42 % of the instructions, and parking the 10
+// values per lane in shared memory instead made the kernel LSU-bound: 20 wavefronts per (region, Gaussian)):
+//   * PIXEL phase (lane = pixel): walks the region's list back to front exactly like the forward walks it front to
+//     back (cp.async staging, phase-1 rectangle culling, groups of four), rebuilds T, and for every Gaussian that
+//     reaches at least one pixel hands over just TWO numbers per lane -- gp = alpha dL/dalpha (0 where clamped or not
+//     blended) and w = alpha T -- with one STS.64 into a [slot][pixel] table;
+//   * GAUSSIAN phase (lane = Gaussian slot x half of the region), run when 16 slots are full: every lane walks 16
+//     pixels of ITS Gaussian, re-forms dx, dy from the slot's mean and accumulates the 10 sums (moments of gp about the
+//     mean; w-weighted upstream colour / depth gradients) in registers -- no cross-lane reduction except one SHFL per
+//     sum to join the two halves -- and the 16 x 10 totals leave through shared memory as coalesced RED.ADD.F32.
+//   ~15 instructions and ~5 shared-memory wavefronts per (region, Gaussian) for the whole reduction.
+#include "gs_internal.cuh"
+#include "gs_raster.cuh"
+
+namespace gs {
+
+constexpr int kSlots = 16;     // Gaussians per flush of the Gaussian phase
+constexpr int kPairRow = 33;   // float2 per slot row (32 pixels + 1: conflict-free transposed LDS.64)
+constexpr int kOutVals = 10;   // sums per Gaussian (gs_internal.cuh kG2D, first 10)
+
+// Gaussian phase.  SPLIT = 2: lane = (slot = lane & 15, half = lane >> 4), 2 pixel rows per lane;
+//                  SPLIT = 4: lane = (slot = lane & 7, quarter = lane >> 3), 1 pixel row per lane (tail flush, <= 8 slots).
+template <int SPLIT>
+__device__ __forceinline__ void gaussian_phase(const float2* s_pair, const float4* s_slot, const float4* s_pix,
+                                               float* s_out, int nslot, int lane, float* __restrict__ g2d) {
+  constexpr int LS = 32 / SPLIT, R = 4 / SPLIT;  // slots per pass, pixel rows per lane
+  __syncwarp();
+  const int slot = lane & (LS - 1), part = lane / LS;
+  const float4 sl = s_slot[slot];
+  float dxs[8], dys[R];
+#pragma unroll
+  for (int c = 0; c < 8; ++c) dxs[c] = (float)c - sl.x;
+#pragma unroll
+  for (int r = 0; r < R; ++r) dys[r] = (float)(part * R + r) - sl.y;
+  const float2* pr = s_pair + slot * kPairRow + part * (R * 8);
+  const float4* px = s_pix + part * (R * 8);
+  float acc[kOutVals];
+#pragma unroll
+  for (int u = 0; u < kOutVals; ++u) acc[u] = 0.f;
+#pragma unroll
+  for (int r = 0; r < R; ++r) {
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+      const float2 pw = pr[r * 8 + c];  // gp, w of (this Gaussian, pixel)
+      const float4 gu = px[r * 8 + c];  // upstream dL/dRGB, dL/dDepth of the pixel
+      const float gx = pw.x * dxs[c], gy = pw.x * dys[r];
+      acc[0] += gx;
+      acc[1] += gy;
+      acc[2] = fmaf(gx, dxs[c], acc[2]);
+      acc[3] = fmaf(gx, dys[r], acc[3]);
+      acc[4] = fmaf(gy, dys[r], acc[4]);
+      acc[5] += pw.x;
+      acc[6] = fmaf(pw.y, gu.x, acc[6]);
+      acc[7] = fmaf(pw.y, gu.y, acc[7]);
+      acc[8] = fmaf(pw.y, gu.z, acc[8]);
+      acc[9] = fmaf(pw.y, gu.w, acc[9]);
+    }
+  }
+#pragma unroll
+  for (int u = 0; u < kOutVals; ++u) {
+    acc[u] += __shfl_xor_sync(kFull, acc[u], 16);
+    if (SPLIT == 4) acc[u] += __shfl_xor_sync(kFull, acc[u], 8);
+  }
+  if (part == 0) {
+#pragma unroll
+    for (int u = 0; u < kOutVals; ++u) s_out[slot * kOutVals + u] = acc[u];
+  }
+  __syncwarp();
+  // coalesced RED: consecutive lanes carry consecutive values of consecutive slots
+  const int total = nslot * kOutVals;
+#pragma unroll
+  for (int t = 0; t < (LS * kOutVals + 31) / 32; ++t) {
+    const int idx = t * 32 + lane;
+    if (idx < total) {
+      const int sl_i = idx / kOutVals, val = idx - sl_i * kOutVals;
+      const uint32_t id = __float_as_uint(s_slot[sl_i].z);
+      atomicAdd(g2d + (size_t)id * kG2D + val, s_out[idx]);
+    }
+  }
+  __syncwarp();
+}
+
+template <bool HAS_GA>
+__global__ void __launch_bounds__(32)
+raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order, const uint2* __restrict__ ranges,
+                  const uint32_t* __restrict__ ids, const float4* __restrict__ feat, float bg0, float bg1, float bg2,
+                  const float* __restrict__ final_T, const uint32_t* __restrict__ n_contrib,
+                  const float* __restrict__ d_rgb, const float* __restrict__ d_depth, const float* __restrict__ d_alpha,
+                  float* __restrict__ g2d) {
+  constexpr int RPT = 8;  // 8x4-pixel regions per 16x16 tile
+  __shared__ __align__(16) float4 s_feat[2][kWarpBatch * 3];
+  __shared__ __align__(16) float4 s_rel[(kWarpBatch + kGroup) * 3];
+  __shared__ uint32_t s_id[2][kWarpBatch];
+  __shared__ __align__(16) float2 s_pair[kSlots * kPairRow];
+  __shared__ __align__(16) float4 s_slot[kSlots];
+  __shared__ __align__(16) float4 s_pix[32];
+  __shared__ __align__(16) float s_out[kSlots * kOutVals];
+  const int lane = threadIdx.x;
+  const int tile = (int)__ldg(order + blockIdx.x / RPT), sub = blockIdx.x % RPT;
+  const int ox = (tile % tiles_x) * GS_TILE + (sub % 2) * 8, oy = (tile / tiles_x) * GS_TILE + (sub / 2) * 4;
+  const int lx = lane & 7, ly = lane >> 3;
+  const float fx0 = (float)lx, fy0 = (float)ly;
+  const uint2 range = ranges[tile];
+  const size_t HW = (size_t)W * H;
+  float T = 1.f, gC0 = 0.f, gC1 = 0.f, gC2 = 0.f, gD = 0.f, gA = 0.f;
+  uint32_t last = 0;
+  {
+    const int X = ox + lx, Y = oy + ly;
+    if (X < W && Y < H) {
+      const size_t p = (size_t)Y * W + X;
+      T = final_T[p];
+      last = n_contrib[p];
+      gC0 = d_rgb[p]; gC1 = d_rgb[HW + p]; gC2 = d_rgb[2 * HW + p];
+      if (d_depth) gD = d_depth[p];
+      if (HAS_GA) gA = d_alpha[p];
+    }
+  }
+  s_pix[lane] = make_float4(gC0, gC1, gC2, gD);
+  float S = T * (gC0 * bg0 + gC1 * bg1 + gC2 * bg2);
+  const int n = (int)__reduce_max_sync(kFull, last);  // deepest blended list position of the region
+  const int nb = (n + kWarpBatch - 1) / kWarpBatch;
+  int nslot = 0;
+
+  auto issue = [&](int b, uint32_t id) {
+    if (b * kWarpBatch + lane < n) {
+      const float4* src = feat + 3 * (size_t)id;
+      float4* dst = &s_feat[b & 1][lane * 3];
+      cp_async16(dst, src); cp_async16(dst + 1, src + 1); cp_async16(dst + 2, src + 2);
+      s_id[b & 1][lane] = id;
+    }
+    cp_async_commit();
+  };
+  uint32_t id_next = 0;
+  if (nb > 0) {
+    const int i0 = (nb - 1) * kWarpBatch + lane;
+    issue(nb - 1, i0 < n ? __ldg(ids + range.x + i0) : 0u);
+    if (nb > 1) id_next = __ldg(ids + range.x + (nb - 2) * kWarpBatch + lane);
+  }
+  for (int b = nb - 1; b >= 0; --b) {
+    if (b >= 1) {
+      issue(b - 1, id_next);
+      if (b >= 2) id_next = __ldg(ids + range.x + (b - 2) * kWarpBatch + lane);
+      cp_async_wait<1>();
+    } else {
+      cp_async_wait<0>();
+    }
+    __syncwarp();
+    const int cnt = min(kWarpBatch, n - b * kWarpBatch);
+    const float4* sf = s_feat[b & 1];
+    // phase 1 (see the forward): decoded records of the relevant Gaussians, compacted in REVERSE list order; the
+    // fourth word of the second vector carries (Gaussian id << 5 | position in the batch)
+    bool relevant = false;
+    float4 c0 = make_float4(0.f, 0.f, 0.f, 0.f), c1 = c0;
+    if (lane < cnt) {
+      GaussReg g;
+      decode_gauss(sf[3 * lane], sf[3 * lane + 1], ox, oy, g);
+      relevant = region_max_power(g, 7.f, 3.f) >= g.thr - 1e-3f;
+      c0 = make_float4(g.mx, g.my, g.A, g.B);
+      c1 = make_float4(g.C, g.o, g.thr, __uint_as_float((s_id[b & 1][lane] << 5) | (uint32_t)lane));
+    }
+    const unsigned rel = __ballot_sync(kFull, relevant);
+    const int nrel = __popc(rel);
+    if (relevant) {
+      const int r = nrel - 1 - __popc(rel & ((1u << lane) - 1u));
+      s_rel[3 * r] = c0; s_rel[3 * r + 1] = c1; s_rel[3 * r + 2] = sf[3 * lane + 2];
+    }
+    if (lane < kGroup) {  // padding records never pass: p >= NaN is false
+      s_rel[3 * (nrel + lane)] = make_float4(0.f, 0.f, 0.f, 0.f);
+      s_rel[3 * (nrel + lane) + 1] = make_float4(0.f, 0.f, __int_as_float(0x7fc00000), 0.f);
+    }
+    __syncwarp();
+    for (int r0 = 0; r0 < nrel; r0 += kGroup) {  // back to front, four list entries at a time
+      uint32_t tag[kGroup];
+      GaussReg g[kGroup];
+      float p[kGroup];
+      unsigned m = 0;
+#pragma unroll
+      for (int q = 0; q < kGroup; ++q) {
+        const float4 a0 = s_rel[3 * (r0 + q)], a1 = s_rel[3 * (r0 + q) + 1];
+        g[q].mx = a0.x; g[q].my = a0.y; g[q].A = a0.z; g[q].B = a0.w;
+        g[q].C = a1.x; g[q].o = a1.y; g[q].thr = a1.z;
+        tag[q] = __float_as_uint(a1.w);
+        float dx[1], dy[1], pp[1];
+        eval_power<1, 1>(g[q], fx0, fy0, dx, dy, pp);
+        p[q] = pp[0];
+        const uint32_t pos = (uint32_t)(b * kWarpBatch) + (tag[q] & 31u);
+        m |= (p[q] >= g[q].thr && pos < last) ? (1u << q) : 0u;
+      }
+      const unsigned any = __reduce_or_sync(kFull, m);
+      if (any == 0) continue;
+#pragma unroll
+      for (int q = 0; q < kGroup; ++q) {
+        if (((any >> q) & 1u) == 0) continue;
+        float gp = 0.f, w = 0.f;
+        if (m & (1u << q)) {
+          const float4 f2 = s_rel[3 * (r0 + q) + 2];
+          const float og = __fmul_rn(g[q].o, ex2_approx(p[q]));
+          const float a = fminf(GS_ALPHA_MAX, og);
+          const float ioma = rcp_approx(1.f - a);
+          T *= ioma;  // transmittance in front of this Gaussian
+          w = a * T;
+          float wi = fmaf(gC0, f2.x, fmaf(gC1, f2.y, fmaf(gC2, f2.z, gD * f2.w)));
+          if (HAS_GA) wi += gA;
+          const float dalpha = fmaf(T, wi, -S * ioma);
+          S = fmaf(wi, w, S);
+          gp = (og <= GS_ALPHA_MAX) ? a * dalpha : 0.f;  // no gradient through the clamp (Q2)
+        }
+        s_pair[nslot * kPairRow + lane] = make_float2(gp, w);
+        if (lane == 0) s_slot[nslot] = make_float4(g[q].mx, g[q].my, __uint_as_float(tag[q] >> 5), 0.f);
+        if (++nslot == kSlots) {
+          gaussian_phase<2>(s_pair, s_slot, s_pix, s_out, kSlots, lane, g2d);
+          nslot = 0;
+        }
+      }
+    }
+    __syncwarp();
+  }
+  if (nslot > 8) gaussian_phase<2>(s_pair, s_slot, s_pix, s_out, nslot, lane, g2d);
+  else if (nslot > 0) gaussian_phase<4>(s_pair, s_slot, s_pix, s_out, nslot, lane, g2d);
+}
+
+int launch_raster_bwd(gs_ctx* ctx, cudaStream_t s, const float* d_rgb, const float* d_depth, const float* d_alpha) {
+  const int units = ctx->cam.tiles_x * ctx->cam.tiles_y * 8;
+  if (units == 0) return GS_OK;
+#define GS_BWD(GA)                                                                                                  \
+  raster_bwd_kernel<GA><<<units, 32, 0, s>>>(ctx->cam.W, ctx->cam.H, ctx->cam.tiles_x, ctx->tile_order, ctx->ranges, \
+                                             ctx->vals[ctx->sorted_buf], ctx->feat, ctx->bg[0], ctx->bg[1],         \
+                                             ctx->bg[2], ctx->final_T, ctx->n_contrib, d_rgb, d_depth, d_alpha,     \
+                                             ctx->g2d)
+  if (d_alpha) GS_BWD(true); else GS_BWD(false);
+#undef GS_BWD
+  GS_LAUNCH_CHECK("raster_bwd_kernel");
+  return GS_OK;
+}
+
+}  // namespace gs
