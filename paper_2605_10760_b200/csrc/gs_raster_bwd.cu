@@ -18,6 +18,9 @@
 
 namespace gs {
 
+#ifndef GS_BWD_MIN_BLOCKS
+#define GS_BWD_MIN_BLOCKS 22
+#endif
 constexpr int kSlots = 16;     // Gaussians per flush of the Gaussian phase
 constexpr int kPairRow = 33;   // float2 per slot row (32 pixels + 1: conflict-free transposed LDS.64)
 constexpr int kOutVals = 10;   // sums per Gaussian (gs_internal.cuh kG2D, first 10)
@@ -25,17 +28,19 @@ constexpr int kOutVals = 10;   // sums per Gaussian (gs_internal.cuh kG2D, first
 // Gaussian phase.  SPLIT = 2: lane = (slot = lane & 15, half = lane >> 4), 2 pixel rows per lane;
 //                  SPLIT = 4: lane = (slot = lane & 7, quarter = lane >> 3), 1 pixel row per lane (tail flush, <= 8 slots).
 template <int SPLIT>
-__device__ __forceinline__ void gaussian_phase(const float2* s_pair, const float4* s_slot, const float4* s_pix,
-                                               float* s_out, int nslot, int lane, float* __restrict__ g2d) {
+__device__ __forceinline__ void gaussian_phase(float2* s_pair, const float4* s_pix, int nslot, int lane, float slot_mx,
+                                               float slot_my, uint32_t slot_id, float* __restrict__ g2d) {
   constexpr int LS = 32 / SPLIT, R = 4 / SPLIT;  // slots per pass, pixel rows per lane
   __syncwarp();
   const int slot = lane & (LS - 1), part = lane / LS;
-  const float4 sl = s_slot[slot];
+  // the slot records live in registers: lane s (and lane s + 16) holds the record of slot s
+  const float mx = SPLIT == 2 ? slot_mx : __shfl_sync(kFull, slot_mx, slot);
+  const float my = SPLIT == 2 ? slot_my : __shfl_sync(kFull, slot_my, slot);
   float dxs[8], dys[R];
 #pragma unroll
-  for (int c = 0; c < 8; ++c) dxs[c] = (float)c - sl.x;
+  for (int c = 0; c < 8; ++c) dxs[c] = (float)c - mx;
 #pragma unroll
-  for (int r = 0; r < R; ++r) dys[r] = (float)(part * R + r) - sl.y;
+  for (int r = 0; r < R; ++r) dys[r] = (float)(part * R + r) - my;
   const float2* pr = s_pair + slot * kPairRow + part * (R * 8);
   const float4* px = s_pix + part * (R * 8);
   float acc[kOutVals];
@@ -65,27 +70,27 @@ __device__ __forceinline__ void gaussian_phase(const float2* s_pair, const float
     acc[u] += __shfl_xor_sync(kFull, acc[u], 16);
     if (SPLIT == 4) acc[u] += __shfl_xor_sync(kFull, acc[u], 8);
   }
+  // the totals leave through shared memory (the pair table is consumed: the shuffles above converged the warp) so that
+  // consecutive lanes carry consecutive values of consecutive slots: coalesced RED
+  float* s_out = reinterpret_cast<float*>(s_pair);
   if (part == 0) {
 #pragma unroll
     for (int u = 0; u < kOutVals; ++u) s_out[slot * kOutVals + u] = acc[u];
   }
   __syncwarp();
-  // coalesced RED: consecutive lanes carry consecutive values of consecutive slots
   const int total = nslot * kOutVals;
 #pragma unroll
   for (int t = 0; t < (LS * kOutVals + 31) / 32; ++t) {
     const int idx = t * 32 + lane;
-    if (idx < total) {
-      const int sl_i = idx / kOutVals, val = idx - sl_i * kOutVals;
-      const uint32_t id = __float_as_uint(s_slot[sl_i].z);
-      atomicAdd(g2d + (size_t)id * kG2D + val, s_out[idx]);
-    }
+    const int sl_i = min(idx / kOutVals, LS - 1), val = idx - sl_i * kOutVals;
+    const uint32_t id = __shfl_sync(kFull, slot_id, sl_i);
+    if (idx < total) atomicAdd(g2d + (size_t)id * kG2D + val, s_out[idx]);
   }
   __syncwarp();
 }
 
 template <bool HAS_GA>
-__global__ void __launch_bounds__(32)
+__global__ void __launch_bounds__(32, GS_BWD_MIN_BLOCKS)
 raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order, const uint2* __restrict__ ranges,
                   const uint32_t* __restrict__ ids, const float4* __restrict__ feat, float bg0, float bg1, float bg2,
                   const float* __restrict__ final_T, const uint32_t* __restrict__ n_contrib,
@@ -94,11 +99,8 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
   constexpr int RPT = 8;  // 8x4-pixel regions per 16x16 tile
   __shared__ __align__(16) float4 s_feat[2][kWarpBatch * 3];
   __shared__ __align__(16) float4 s_rel[(kWarpBatch + kGroup) * 3];
-  __shared__ uint32_t s_id[2][kWarpBatch];
   __shared__ __align__(16) float2 s_pair[kSlots * kPairRow];
-  __shared__ __align__(16) float4 s_slot[kSlots];
   __shared__ __align__(16) float4 s_pix[32];
-  __shared__ __align__(16) float s_out[kSlots * kOutVals];
   const int lane = threadIdx.x;
   const int tile = (int)__ldg(order + blockIdx.x / RPT), sub = blockIdx.x % RPT;
   const int ox = (tile % tiles_x) * GS_TILE + (sub % 2) * 8, oy = (tile / tiles_x) * GS_TILE + (sub / 2) * 4;
@@ -124,25 +126,30 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
   const int n = (int)__reduce_max_sync(kFull, last);  // deepest blended list position of the region
   const int nb = (n + kWarpBatch - 1) / kWarpBatch;
   int nslot = 0;
+  float2* pair_ptr = s_pair + lane;     // where this lane's (gp, w) of the next slot goes
+  float slot_mx = 0.f, slot_my = 0.f;  // record of slot (lane & 15), kept in registers
+  uint32_t slot_id = 0;
 
   auto issue = [&](int b, uint32_t id) {
     if (b * kWarpBatch + lane < n) {
       const float4* src = feat + 3 * (size_t)id;
       float4* dst = &s_feat[b & 1][lane * 3];
       cp_async16(dst, src); cp_async16(dst + 1, src + 1); cp_async16(dst + 2, src + 2);
-      s_id[b & 1][lane] = id;
     }
     cp_async_commit();
   };
-  uint32_t id_next = 0;
+  uint32_t id_cur = 0, id_staged = 0, id_next = 0;  // ids of this lane's entry in batches b, b - 1, b - 2
   if (nb > 0) {
     const int i0 = (nb - 1) * kWarpBatch + lane;
-    issue(nb - 1, i0 < n ? __ldg(ids + range.x + i0) : 0u);
+    id_staged = i0 < n ? __ldg(ids + range.x + i0) : 0u;
+    issue(nb - 1, id_staged);
     if (nb > 1) id_next = __ldg(ids + range.x + (nb - 2) * kWarpBatch + lane);
   }
   for (int b = nb - 1; b >= 0; --b) {
+    id_cur = id_staged;
     if (b >= 1) {
       issue(b - 1, id_next);
+      id_staged = id_next;
       if (b >= 2) id_next = __ldg(ids + range.x + (b - 2) * kWarpBatch + lane);
       cp_async_wait<1>();
     } else {
@@ -150,6 +157,7 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
     }
     __syncwarp();
     const int cnt = min(kWarpBatch, n - b * kWarpBatch);
+    const int lastb = (int)last - b * kWarpBatch;  // entries of this batch at positions < lastb were blended by this pixel
     const float4* sf = s_feat[b & 1];
     // phase 1 (see the forward): decoded records of the relevant Gaussians, compacted in REVERSE list order; the
     // fourth word of the second vector carries (Gaussian id << 5 | position in the batch)
@@ -160,7 +168,7 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
       decode_gauss(sf[3 * lane], sf[3 * lane + 1], ox, oy, g);
       relevant = region_max_power(g, 7.f, 3.f) >= g.thr - 1e-3f;
       c0 = make_float4(g.mx, g.my, g.A, g.B);
-      c1 = make_float4(g.C, g.o, g.thr, __uint_as_float((s_id[b & 1][lane] << 5) | (uint32_t)lane));
+      c1 = make_float4(g.C, g.o, g.thr, __uint_as_float((id_cur << 5) | (uint32_t)lane));
     }
     const unsigned rel = __ballot_sync(kFull, relevant);
     const int nrel = __popc(rel);
@@ -187,8 +195,7 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
         float dx[1], dy[1], pp[1];
         eval_power<1, 1>(g[q], fx0, fy0, dx, dy, pp);
         p[q] = pp[0];
-        const uint32_t pos = (uint32_t)(b * kWarpBatch) + (tag[q] & 31u);
-        m |= (p[q] >= g[q].thr && pos < last) ? (1u << q) : 0u;
+        m |= (p[q] >= g[q].thr && (int)(tag[q] & 31u) < lastb) ? (1u << q) : 0u;
       }
       const unsigned any = __reduce_or_sync(kFull, m);
       if (any == 0) continue;
@@ -209,18 +216,20 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
           S = fmaf(wi, w, S);
           gp = (og <= GS_ALPHA_MAX) ? a * dalpha : 0.f;  // no gradient through the clamp (Q2)
         }
-        s_pair[nslot * kPairRow + lane] = make_float2(gp, w);
-        if (lane == 0) s_slot[nslot] = make_float4(g[q].mx, g[q].my, __uint_as_float(tag[q] >> 5), 0.f);
+        *pair_ptr = make_float2(gp, w);
+        pair_ptr += kPairRow;
+        if ((lane & (kSlots - 1)) == nslot) { slot_mx = g[q].mx; slot_my = g[q].my; slot_id = tag[q] >> 5; }
         if (++nslot == kSlots) {
-          gaussian_phase<2>(s_pair, s_slot, s_pix, s_out, kSlots, lane, g2d);
+          gaussian_phase<2>(s_pair, s_pix, kSlots, lane, slot_mx, slot_my, slot_id, g2d);
           nslot = 0;
+          pair_ptr = s_pair + lane;
         }
       }
     }
     __syncwarp();
   }
-  if (nslot > 8) gaussian_phase<2>(s_pair, s_slot, s_pix, s_out, nslot, lane, g2d);
-  else if (nslot > 0) gaussian_phase<4>(s_pair, s_slot, s_pix, s_out, nslot, lane, g2d);
+  if (nslot > 8) gaussian_phase<2>(s_pair, s_pix, nslot, lane, slot_mx, slot_my, slot_id, g2d);
+  else if (nslot > 0) gaussian_phase<4>(s_pair, s_pix, nslot, lane, slot_mx, slot_my, slot_id, g2d);
 }
 
 int launch_raster_bwd(gs_ctx* ctx, cudaStream_t s, const float* d_rgb, const float* d_depth, const float* d_alpha) {
