@@ -137,6 +137,8 @@ int gs_create(gs_ctx** out, int device) {
   ok = ok && cudaStreamCreateWithFlags(&ctx->side_stream, cudaStreamNonBlocking) == cudaSuccess;
   ok = ok && cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming) == cudaSuccess;
   ok = ok && cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming) == cudaSuccess;
+  ok = ok && cudaEventCreateWithFlags(&ctx->ev_fork2, cudaEventDisableTiming) == cudaSuccess;
+  ok = ok && cudaEventCreateWithFlags(&ctx->ev_join2, cudaEventDisableTiming) == cudaSuccess;
   if (ok) {
     memset(ctx->mailbox, 0, sizeof(Counts));
     ok = cudaHostGetDevicePointer((void**)&ctx->mailbox_dev, ctx->mailbox, 0) == cudaSuccess;
@@ -160,6 +162,8 @@ int gs_destroy(gs_ctx* ctx) {
   if (ctx->side_stream) cudaStreamDestroy(ctx->side_stream);
   if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
   if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
+  if (ctx->ev_fork2) cudaEventDestroy(ctx->ev_fork2);
+  if (ctx->ev_join2) cudaEventDestroy(ctx->ev_join2);
   if (ctx->ev_made) for (int k = 0; k < 13; ++k) cudaEventDestroy(ctx->ev[k]);
   cudaGetLastError();
   delete ctx;

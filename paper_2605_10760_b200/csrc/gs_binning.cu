@@ -16,7 +16,8 @@
 
 namespace gs {
 
-constexpr int kSmallSort = 1031;   // buckets up to this size (a whole length/8 class of the tile order): 128-thread CTA, static smem
+constexpr int kSmallSortMax = 255;  // buckets up to this size are sorted by one warp (whole length/8 classes of the tile order)
+constexpr int kMidSortMax = 1023;   // buckets up to this size are sorted by one CTA of 4 warps; beyond: the large kernel
 constexpr int kLargeSort = 8192;
 constexpr int kScanCache = 8192;   // tile counts cached in shared memory by the scan kernel (all of them up to ~2 Mpix)
 // tile_count / tile_cursor are strided by 32 words: one counter per 128-byte line, so that the atomics of different
@@ -31,12 +32,12 @@ tile_scan_kernel(int tiles, const uint32_t* __restrict__ tile_count, uint32_t* _
                  Counts* mailbox, uint32_t seq) {
   __shared__ uint32_t hist[1024];
   __shared__ uint32_t wsum[32];
-  __shared__ uint32_t s_carry, s_large;
+  __shared__ uint32_t s_carry, s_large, s_mid;
   __shared__ uint32_t s_cnt[kScanCache];  // the counts, fetched once with all loads in flight together
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   for (int t = tid; t < min(tiles, kScanCache); t += 1024) s_cnt[t] = tile_count[(size_t)t * kCtrStride];
   hist[tid] = 0;
-  if (tid == 0) { s_carry = 0; s_large = 0; }
+  if (tid == 0) { s_carry = 0; s_large = 0; s_mid = 0; }
   __syncthreads();
   // exclusive scan of the counts, 1024 tiles per round
   for (int base = 0; base < tiles; base += 1024) {
@@ -56,7 +57,8 @@ tile_scan_kernel(int tiles, const uint32_t* __restrict__ tile_count, uint32_t* _
       tile_cursor[(size_t)t * kCtrStride] = off;
       ranges[t] = c ? make_uint2(off, off + c) : make_uint2(0u, 0u);  // cleared below if the iteration overflows
       atomicAdd(&hist[1023 - min(c >> 3, 1023u)], 1u);
-      if (c > (uint32_t)kSmallSort) atomicAdd(&s_large, 1u);
+      if (c > (uint32_t)kMidSortMax) atomicAdd(&s_large, 1u);
+      if (c > (uint32_t)kSmallSortMax) atomicAdd(&s_mid, 1u);
     }
     __syncthreads();
     if (tid == 1023) s_carry = off + c;
@@ -68,6 +70,7 @@ tile_scan_kernel(int tiles, const uint32_t* __restrict__ tile_count, uint32_t* _
     counts->n_instances = I;
     counts->overflow = ovf ? 1u : 0u;
     counts->n_large = s_large;
+    counts->n_mid = s_mid;
     counts->seq = seq;
     mailbox->n_instances = I;
     mailbox->overflow = ovf ? 1u : 0u;
@@ -201,42 +204,147 @@ __device__ __forceinline__ void bitonic_sort(uint64_t* s, int n, int tid, int nt
   }
 }
 
-// LARGE = false: buckets with n <= kSmallSort, static shared memory, 128 threads.
-// LARGE = true : the blockIdx.x-th longest bucket if n > kSmallSort; dynamic shared memory up to kLargeSort keys, the
-//                same network in place in global memory beyond (slow; degenerate scenes only).
-template <bool LARGE>
-__global__ void __launch_bounds__(LARGE ? 512 : 128)
-tile_sort_kernel(const uint32_t* __restrict__ order, const uint2* __restrict__ ranges,
-                 const Counts* __restrict__ counts, uint64_t* __restrict__ keys, uint32_t* __restrict__ ids) {
+// ---------------------------------------------------------------------------------------------------------------
+// Register-resident bitonic network (evidence: profiles/r1_v3_regions.md -- a shared-memory network with one
+// __syncthreads per level took 38.6 + 21.8 us).  A bucket of up to 32 * E * NW keys is held by NW warps, E consecutive
+// keys per thread: strides below E are in-register compare-exchanges, strides E .. 16 E are SHFL.XOR exchanges, and
+// only strides >= 32 E (none for NW = 1) go through shared memory with a barrier.  Normalised network: every
+// comparator is ascending; the first step of a K-merge pairs i with its mirror i ^ (K - 1), the other steps i with
+// i ^ j.  The (K, j) loops are run-time loops around unrolled per-stride bodies (fully unrolled, the network is
+// ~160 KB of straight-line code and runs at the instruction-fetch rate).  Padding keys are +inf.
+// ---------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void cmp_swap(uint64_t& a, uint64_t& b) {
+  const bool sw = a > b;
+  const uint64_t lo = sw ? b : a, hi = sw ? a : b;
+  a = lo; b = hi;
+}
+
+// in-register comparators between e and e ^ X for every e whose bit B is clear (X = B: half-cleaner, X = 2B - 1: mirror)
+template <int E, int B, bool MIRROR>
+__device__ __forceinline__ void reg_step(uint64_t (&k)[E]) {
+  constexpr int X = MIRROR ? 2 * B - 1 : B;
+#pragma unroll
+  for (int e = 0; e < E; ++e)
+    if ((e & B) == 0) cmp_swap(k[e], k[e ^ X]);
+}
+
+template <int E, bool MIRROR>
+__device__ __forceinline__ void reg_step_dyn(uint64_t (&k)[E], int B) {
+  if (E > 1 && B == 1) reg_step<E, 1, MIRROR>(k);
+  if (E > 2 && B == 2) reg_step<E, (E > 2 ? 2 : 1), MIRROR>(k);
+  if (E > 4 && B == 4) reg_step<E, (E > 4 ? 4 : 1), MIRROR>(k);
+  if (E > 8 && B == 8) reg_step<E, (E > 8 ? 8 : 1), MIRROR>(k);
+}
+
+// cross-lane step: partner lane = lane ^ d; `lower` threads keep the minima
+template <int E, bool MIRROR>
+__device__ __forceinline__ void lane_step(uint64_t (&k)[E], int d, bool lower) {
+  uint64_t o[E];
+#pragma unroll
+  for (int e = 0; e < E; ++e) o[e] = __shfl_xor_sync(0xffffffffu, k[MIRROR ? E - 1 - e : e], d);
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const bool take = (o[e] < k[e]) == lower;
+    k[e] = take ? o[e] : k[e];
+  }
+}
+
+// cross-warp step through shared memory, layout s[e * T + tid] (conflict-free for the store and the partner load)
+template <int E, int T, bool MIRROR>
+__device__ __forceinline__ void smem_step(uint64_t (&k)[E], uint64_t* s, int tid, int x, bool lower) {
+#pragma unroll
+  for (int e = 0; e < E; ++e) s[e * T + tid] = k[e];
+  __syncthreads();
+  const int pt = tid ^ x;
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const uint64_t o = s[(MIRROR ? E - 1 - e : e) * T + pt];
+    const bool take = (o < k[e]) == lower;
+    k[e] = take ? o : k[e];
+  }
+  __syncthreads();
+}
+
+template <int E, int NW>
+__device__ __forceinline__ void bucket_sort(uint64_t* __restrict__ g, uint32_t* __restrict__ ids, int n, uint64_t* s, int tid) {
+  constexpr int T = 32 * NW;
+  uint64_t k[E];
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const int i = tid * E + e;
+    k[e] = i < n ? g[i] : ~0ull;
+  }
+  int P = 64;
+  while (P < n) P <<= 1;  // merges beyond the first power of two >= n would only move padding
+#pragma unroll 1
+  for (int K = 2; K <= P; K <<= 1) {
+    if (K <= E) reg_step_dyn<E, true>(k, K >> 1);
+    else if (NW == 1 || K <= 32 * E) lane_step<E, true>(k, K / E - 1, (tid & (K / (2 * E))) == 0);
+    else smem_step<E, T, true>(k, s, tid, K / E - 1, (tid & (K / (2 * E))) == 0);
+#pragma unroll 1
+    for (int j = K >> 2; j >= 1; j >>= 1) {
+      if (NW > 1 && j >= 32 * E) smem_step<E, T, false>(k, s, tid, j / E, (tid & (j / E)) == 0);
+      else if (j >= E) lane_step<E, false>(k, j / E, (tid & (j / E)) == 0);
+      else reg_step_dyn<E, false>(k, j);
+    }
+  }
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const int i = tid * E + e;
+    if (i < n) { g[i] = k[e]; ids[i] = (uint32_t)k[e]; }
+  }
+}
+
+// Buckets of 1024 .. kLargeSort keys (the first n_large entries of `order`): one CTA of 512 threads per bucket, 16 keys
+// per thread; beyond kLargeSort the shared-memory-free network above runs in place in global memory (slow; degenerate
+// scenes only).
+__global__ void __launch_bounds__(512)
+tile_sort_large_kernel(const uint32_t* __restrict__ order, const uint2* __restrict__ ranges,
+                       const Counts* __restrict__ counts, uint64_t* __restrict__ keys, uint32_t* __restrict__ ids) {
   extern __shared__ uint64_t s_dyn[];
-  __shared__ uint64_t s_small[LARGE ? 1 : kSmallSort + 1];
   const int tid = threadIdx.x, nth = blockDim.x;
-  const int first = blockIdx.x, stride = LARGE ? gridDim.x : 1 << 30;
-  const int limit = LARGE ? (int)counts->n_large : (int)blockIdx.x + 1;  // the large tiles come first in `order`
-  for (int b = first; b < limit; b += stride) {
+  const int limit = (int)counts->n_large;
+  for (int b = blockIdx.x; b < limit; b += gridDim.x) {
     const int tile = (int)order[b];
     const uint2 r = ranges[tile];
     const int n = (int)(r.y - r.x);
-    if (LARGE ? (n <= kSmallSort) : (n > kSmallSort)) continue;
-    if (n == 0) continue;
+    if (n <= kMidSortMax) continue;
     uint64_t* g = keys + r.x;
-    if (LARGE && n > kLargeSort) {
+    if (n > kLargeSort) {
       bitonic_sort(g, n, tid, nth);  // __syncthreads orders the CTA's own global writes
       for (int t = tid; t < n; t += nth) ids[r.x + t] = (uint32_t)g[t];
       __syncthreads();
       continue;
     }
-    uint64_t* s = LARGE ? s_dyn : s_small;
-    for (int t = tid; t < n; t += nth) s[t] = g[t];
-    __syncthreads();
-    bitonic_sort(s, n, tid, nth);
-    for (int t = tid; t < n; t += nth) {
-      const uint64_t k = s[t];
-      g[t] = k;
-      ids[r.x + t] = (uint32_t)k;
-    }
+    if (n <= 2048) bucket_sort<4, 16>(g, ids + r.x, n, s_dyn, tid);
+    else bucket_sort<16, 16>(g, ids + r.x, n, s_dyn, tid);
     __syncthreads();
   }
+}
+
+// Buckets up to kMidSortMax keys.  CTAs of 4 warps: the first n_mid entries of `order` (256 .. 1023 keys; those of the
+// large kernel are skipped) take a whole CTA each, 8 keys per thread; the remaining buckets (< 256 keys) take one warp
+// each, four buckets per CTA, no barrier at all.
+__global__ void __launch_bounds__(128)
+tile_sort_kernel(int tiles, const uint32_t* __restrict__ order, const uint2* __restrict__ ranges,
+                 const Counts* __restrict__ counts, uint64_t* __restrict__ keys, uint32_t* __restrict__ ids) {
+  __shared__ uint64_t s_x[1024];
+  const int tid = threadIdx.x;
+  const int n_mid = (int)counts->n_mid;
+  if ((int)blockIdx.x < n_mid) {
+    const uint2 r = ranges[order[blockIdx.x]];
+    const int n = (int)(r.y - r.x);
+    if (n > kMidSortMax) return;
+    bucket_sort<8, 4>(keys + r.x, ids + r.x, n, s_x, tid);
+    return;
+  }
+  const int idx = n_mid + ((int)blockIdx.x - n_mid) * 4 + (tid >> 5);
+  if (idx >= tiles) return;
+  const uint2 r = ranges[order[idx]];
+  const int n = (int)(r.y - r.x), lane = tid & 31;
+  if (n == 0) return;
+  if (n <= 64) bucket_sort<2, 1>(keys + r.x, ids + r.x, n, nullptr, lane);
+  else bucket_sort<8, 1>(keys + r.x, ids + r.x, n, nullptr, lane);
 }
 
 // export for gs_get_binning: keys_sorted[k] = tile << 32 | depth bits
@@ -322,16 +430,24 @@ int launch_binning(gs_ctx* ctx, cudaStream_t s) {
   GS_PROF(4, s);
   if (ctx->N > 0 && tiles > 0) {
     if (!ctx->sort_attr_set) {
-      GS_CUDA(cudaFuncSetAttribute(tile_sort_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+      GS_CUDA(cudaFuncSetAttribute(tile_sort_large_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                    kLargeSort * (int)sizeof(uint64_t)));
       ctx->sort_attr_set = true;
     }
-    tile_sort_kernel<true><<<min(tiles, 296), 512, kLargeSort * sizeof(uint64_t), s>>>(ctx->tile_order, ctx->ranges, ctx->counts,
-                                                                            ctx->keys[0], ctx->vals[0]);
-    GS_LAUNCH_CHECK("tile_sort_kernel<large>");
-    tile_sort_kernel<false><<<tiles, 128, 0, s>>>(ctx->tile_order, ctx->ranges, ctx->counts, ctx->keys[0],
-                                                  ctx->vals[0]);
-    GS_LAUNCH_CHECK("tile_sort_kernel<small>");
+    // the few long buckets (block-wide network) sort on the side stream while the warp kernel sorts the rest
+    const bool fork = ctx->side_stream != nullptr;
+    cudaStream_t sl = fork ? ctx->side_stream : s;
+    if (fork) {
+      GS_CUDA(cudaEventRecord(ctx->ev_fork2, s));
+      GS_CUDA(cudaStreamWaitEvent(sl, ctx->ev_fork2, 0));
+    }
+    tile_sort_large_kernel<<<min(tiles, 296), 512, kLargeSort * sizeof(uint64_t), sl>>>(ctx->tile_order, ctx->ranges, ctx->counts,
+                                                                                        ctx->keys[0], ctx->vals[0]);
+    GS_LAUNCH_CHECK("tile_sort_large_kernel");
+    if (fork) GS_CUDA(cudaEventRecord(ctx->ev_join2, sl));
+    tile_sort_kernel<<<tiles, 128, 0, s>>>(tiles, ctx->tile_order, ctx->ranges, ctx->counts, ctx->keys[0], ctx->vals[0]);
+    GS_LAUNCH_CHECK("tile_sort_kernel");
+    if (fork) GS_CUDA(cudaStreamWaitEvent(s, ctx->ev_join2, 0));
   }
   ctx->sorted_buf = 0;
   GS_PROF(5, s);

@@ -54,7 +54,8 @@ struct Counts {
   uint32_t n_instances;  // total tile instances of the last scan (even if it overflowed)
   uint32_t overflow;     // 1 if n_instances > capacity: nothing was emitted and downstream kernels see 0 instances
   uint32_t seq;          // iteration number of the writer
-  uint32_t n_large;      // number of tiles whose list is longer than the small-sort capacity
+  uint32_t n_large;      // number of tiles whose list is longer than one 4-warp CTA sorts in registers (> 1023)
+  uint32_t n_mid;        // number of tiles whose list is longer than one warp sorts in registers (> 255; includes n_large)
 };
 
 
@@ -118,7 +119,7 @@ struct gs_ctx {
 
   // side stream: the zero fill of the dense gradient arrays overlaps the (ALU-bound) pixel backward
   cudaStream_t side_stream = nullptr;
-  cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_fork2 = nullptr, ev_join2 = nullptr;
   bool zero_filled = false;  // set by gs_rasterize_bwd when the fill was issued on the side stream
 
   // stage timing (gs_profile_*): events recorded around the kernel groups when enabled
@@ -184,7 +185,7 @@ inline Counts read_mailbox(const gs_ctx* ctx) {
   const volatile Counts* m = ctx->mailbox;
   Counts c;
   c.n_visible = m->n_visible; c.n_instances = m->n_instances; c.overflow = m->overflow; c.seq = m->seq;
-  c.n_large = 0;
+  c.n_large = 0; c.n_mid = 0;
   return c;
 }
 
