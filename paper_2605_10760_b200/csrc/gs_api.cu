@@ -90,6 +90,7 @@ static int ensure_gaussian_capacity(gs_ctx* ctx, int64_t N) {
   if ((rc = grow(ctx, ctx->depth_key, cap)) != GS_OK) return rc;
   if ((rc = grow(ctx, ctx->tiles_touched, cap + 4)) != GS_OK) return rc;
   if ((rc = grow(ctx, ctx->vis_ids, cap)) != GS_OK) return rc;
+  if ((rc = grow(ctx, ctx->vis_rec, cap)) != GS_OK) return rc;
   if ((rc = grow(ctx, ctx->g2d, cap * kG2D)) != GS_OK) return rc;
   GS_CUDA(cudaMemset(ctx->g2d, 0, (size_t)cap * kG2D * sizeof(float)));
   ctx->g2d_dirty = false;
@@ -152,10 +153,10 @@ int gs_destroy(gs_ctx* ctx) {
   if (!ctx) return GS_E_INVALID;
   cudaSetDevice(ctx->device);
   cudaDeviceSynchronize();
-  cudaFree(ctx->feat); cudaFree(ctx->rect); cudaFree(ctx->depth_key); cudaFree(ctx->tiles_touched); cudaFree(ctx->vis_ids);
+  cudaFree(ctx->feat); cudaFree(ctx->rect); cudaFree(ctx->depth_key); cudaFree(ctx->tiles_touched); cudaFree(ctx->vis_ids); cudaFree(ctx->vis_rec);
   cudaFree(ctx->g2d);
   for (int b = 0; b < 2; ++b) { cudaFree(ctx->keys[b]); cudaFree(ctx->vals[b]); }
-  cudaFree(ctx->tile_count); cudaFree(ctx->tile_cursor);
+  cudaFree(ctx->tile_count); cudaFree(ctx->tile_cursor); cudaFree(ctx->scan_ws);
   cudaFree(ctx->ranges); cudaFree(ctx->tile_order); cudaFree(ctx->final_T); cudaFree(ctx->n_contrib);
   cudaFree(ctx->pose_acc); cudaFree(ctx->counts); cudaFree(ctx->hb);
   if (ctx->mailbox) cudaFreeHost(ctx->mailbox);

@@ -19,143 +19,212 @@ namespace gs {
 constexpr int kSmallSortMax = 255;  // buckets up to this size are sorted by one warp (whole length/8 classes of the tile order)
 constexpr int kMidSortMax = 1023;   // buckets up to this size are sorted by one CTA of 4 warps; beyond: the large kernel
 constexpr int kLargeSort = 8192;
-constexpr int kScanCache = 8192;   // tile counts cached in shared memory by the scan kernel (all of them up to ~2 Mpix)
 // tile_count / tile_cursor are strided by 32 words: one counter per 128-byte line, so that the atomics of different
 // tiles are served by different L2 lines (3225 adjacent counters would share ~100 lines and serialise there)   // up to this size: 512-thread CTA, 64 KB dynamic shared memory; beyond: global memory
 
 // ---------------------------------------------------------------------------------------------------------------
 // a2 + a5: prefix sum over the tile counts, ranges, totals, overflow flag, LPT tile order.  One CTA of 1024 threads.
 // ---------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(1024)
-tile_scan_kernel(int tiles, const uint32_t* __restrict__ tile_count, uint32_t* __restrict__ tile_cursor,
-                 uint2* __restrict__ ranges, uint32_t* __restrict__ order, int64_t capacity, Counts* counts,
-                 Counts* mailbox, uint32_t seq) {
-  __shared__ uint32_t hist[1024];
-  __shared__ uint32_t wsum[32];
-  __shared__ uint32_t s_carry, s_large, s_mid;
-  __shared__ uint32_t s_cnt[kScanCache];  // the counts, fetched once with all loads in flight together
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  for (int t = tid; t < min(tiles, kScanCache); t += 1024) s_cnt[t] = tile_count[(size_t)t * kCtrStride];
-  hist[tid] = 0;
-  if (tid == 0) { s_carry = 0; s_large = 0; s_mid = 0; }
-  __syncthreads();
-  // exclusive scan of the counts, 1024 tiles per round
-  for (int base = 0; base < tiles; base += 1024) {
-    const int t = base + tid;
-    const uint32_t c = t < tiles ? (t < kScanCache ? s_cnt[t] : tile_count[(size_t)t * kCtrStride]) : 0u;
-    uint32_t incl = c;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-      const uint32_t v = __shfl_up_sync(0xffffffffu, incl, d);
-      if (lane >= d) incl += v;
-    }
-    if (lane == 31) wsum[warp] = incl;
-    __syncthreads();
-    uint32_t off = s_carry + incl - c;
-    for (int w = 0; w < warp; ++w) off += wsum[w];
-    if (t < tiles) {
-      tile_cursor[(size_t)t * kCtrStride] = off;
-      ranges[t] = c ? make_uint2(off, off + c) : make_uint2(0u, 0u);  // cleared below if the iteration overflows
-      atomicAdd(&hist[1023 - min(c >> 3, 1023u)], 1u);
-      if (c > (uint32_t)kMidSortMax) atomicAdd(&s_large, 1u);
-      if (c > (uint32_t)kSmallSortMax) atomicAdd(&s_mid, 1u);
-    }
-    __syncthreads();
-    if (tid == 1023) s_carry = off + c;
-    __syncthreads();
-  }
-  const uint32_t I = s_carry;
-  const bool ovf = (int64_t)I > capacity;
-  if (tid == 0) {
-    counts->n_instances = I;
-    counts->overflow = ovf ? 1u : 0u;
-    counts->n_large = s_large;
-    counts->n_mid = s_mid;
-    counts->seq = seq;
-    mailbox->n_instances = I;
-    mailbox->overflow = ovf ? 1u : 0u;
-    mailbox->n_visible = counts->n_visible;
-    __threadfence_system();
-    mailbox->seq = seq;
-  }
-  if (ovf)
-    for (int t = tid; t < tiles; t += 1024) ranges[t] = make_uint2(0u, 0u);  // the flagged iteration renders nothing
-  // tile ids by descending list length (counting sort on length / 8; order inside a bucket is arbitrary)
-  const uint32_t h = hist[tid];
-  uint32_t incl = h;
+// Multi-CTA single-pass scan.  (Measured with clock64 on the one-CTA versions: ~20 k cycles whatever the algorithm --
+// shared-memory atomics, L2 atomics or none -- because the 3225 strided counter loads and the ~3 x 3225 scattered
+// stores of ONE SM retire about one sector per cycle.)  CTA b owns the tiles [b * TPC, (b + 1) * TPC), IT consecutive
+// tiles per thread.  The block scan carries 9 words per thread: the instance count and 16 length-class counters packed
+// as 16-bit fields, so one scan yields the per-tile ranges AND a stable counting sort of the tiles by length class
+// (= the tile order); no atomics.  Every CTA publishes its 17 unpacked totals with an epoch flag and reads those of
+// all the others (at most 128 CTAs, all co-resident), i.e. one L2 round trip instead of a second kernel.
+constexpr int kScanT = 256;      // threads per CTA
+constexpr int kScanWords = 9;    // [0] instances, [1..8] 16 class counters, two per word
+constexpr int kScanCls = 16;
+constexpr int kScanAgg = 1 + kScanCls;
+constexpr int kScanMaxCta = 128;
+
+// length class, longest first: 0: >= 1024, then half-octave steps 768, 512, 384, 256, ..., 12, 8; 15: < 8.
+// Class 0 holds exactly the tiles beyond kMidSortMax, classes 0..4 those beyond kSmallSortMax.
+__device__ __forceinline__ int length_class(uint32_t c) {
+  if (c < 8u) return 15;
+  const int e = 31 - __clz((int)c);
+  const int q = 2 * e + (int)((c >> (e - 1)) & 1u);
+  return max(20 - q, 0);
+}
+
+struct ScanVec { uint32_t w[kScanWords]; };
+
+__device__ __forceinline__ ScanVec block_excl_scan_vec(const ScanVec& v, uint32_t (*wsum)[kScanWords], int lane, int warp,
+                                                       ScanVec& total) {
+  constexpr int NW = kScanT / 32;
+  ScanVec incl = v;
 #pragma unroll
   for (int d = 1; d < 32; d <<= 1) {
-    const uint32_t v = __shfl_up_sync(0xffffffffu, incl, d);
-    if (lane >= d) incl += v;
+#pragma unroll
+    for (int k = 0; k < kScanWords; ++k) {
+      const uint32_t u = __shfl_up_sync(0xffffffffu, incl.w[k], d);
+      if (lane >= d) incl.w[k] += u;
+    }
+  }
+  if (lane == 31) {
+#pragma unroll
+    for (int k = 0; k < kScanWords; ++k) wsum[warp][k] = incl.w[k];
   }
   __syncthreads();
-  if (lane == 31) wsum[warp] = incl;
+  ScanVec r;
+#pragma unroll
+  for (int k = 0; k < kScanWords; ++k) {
+    uint32_t before = 0, all = 0;
+#pragma unroll
+    for (int w = 0; w < NW; ++w) {
+      const uint32_t x = wsum[w][k];
+      before += (w < warp) ? x : 0u;
+      all += x;
+    }
+    r.w[k] = before + incl.w[k] - v.w[k];
+    total.w[k] = all;
+  }
+  return r;
+}
+
+template <int IT>
+__global__ void __launch_bounds__(kScanT)
+tile_scan_kernel(int tiles, const uint32_t* __restrict__ tile_count, uint32_t* __restrict__ tile_cursor,
+                 uint2* __restrict__ ranges, uint32_t* __restrict__ order, uint32_t* agg, uint32_t* flags,
+                 uint32_t epoch, int64_t capacity, Counts* counts, Counts* mailbox, uint32_t seq) {
+  __shared__ uint32_t wsum[kScanT / 32][kScanWords];
+  __shared__ uint32_t s_pre[kScanAgg], s_tot[kScanAgg], s_base[kScanCls];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int b = blockIdx.x, nb = gridDim.x;
+  const int t0 = (b * kScanT + tid) * IT;
+  if (tid < kScanAgg) { s_pre[tid] = 0; s_tot[tid] = 0; }
+  uint32_t c[IT];
+  int cls[IT];
+  ScanVec v, total;
+#pragma unroll
+  for (int k = 0; k < kScanWords; ++k) v.w[k] = 0;
+#pragma unroll
+  for (int u = 0; u < IT; ++u) c[u] = (t0 + u < tiles) ? __ldg(tile_count + (size_t)(t0 + u) * kCtrStride) : 0u;
+#pragma unroll
+  for (int u = 0; u < IT; ++u) {
+    cls[u] = length_class(c[u]);
+    if (t0 + u < tiles) {
+      v.w[0] += c[u];
+#pragma unroll
+      for (int w = 0; w < 8; ++w) v.w[1 + w] += ((cls[u] >> 1) == w) ? (1u << ((cls[u] & 1) * 16)) : 0u;
+    }
+  }
+  ScanVec pref = block_excl_scan_vec(v, wsum, lane, warp, total);
+  // publish this CTA's totals, then gather everybody's
+  if (tid < kScanAgg) {
+    const uint32_t x = tid == 0 ? total.w[0] : (total.w[1 + ((tid - 1) >> 1)] >> (((tid - 1) & 1) * 16)) & 0xffffu;
+    __stcg(agg + b * kScanAgg + tid, x);
+    __threadfence();
+  }
   __syncthreads();
-  uint32_t bbase = incl - h;
-  for (int w = 0; w < warp; ++w) bbase += wsum[w];
+  if (tid == 0) { __threadfence(); *reinterpret_cast<volatile uint32_t*>(flags + b) = epoch; }
+  for (int i = tid; i < nb * kScanAgg; i += kScanT) {
+    const int j = i / kScanAgg, k = i - j * kScanAgg;
+    while (*reinterpret_cast<volatile uint32_t*>(flags + j) != epoch) {}
+    __threadfence();
+    const uint32_t x = __ldcg(agg + j * kScanAgg + k);
+    if (x) {
+      atomicAdd(&s_tot[k], x);
+      if (j < b) atomicAdd(&s_pre[k], x);
+    }
+  }
   __syncthreads();
-  hist[tid] = bbase;
+  const uint32_t I = s_tot[0];
+  const bool ovf = (int64_t)I > capacity;
+  if (tid == 0) {
+    uint32_t bb = 0, nl = 0, nm = 0;
+    for (int k = 0; k < kScanCls; ++k) {
+      s_base[k] = bb + s_pre[1 + k];
+      bb += s_tot[1 + k];
+      if (k == 0) nl = bb;
+      if (k == 4) nm = bb;
+    }
+    if (b == 0) {
+      counts->n_instances = I;
+      counts->overflow = ovf ? 1u : 0u;
+      counts->n_large = nl;
+      counts->n_mid = nm;
+      counts->seq = seq;
+      // one 16-byte store to the mapped host mailbox {n_visible, n_instances, overflow, seq}: a single posted write,
+      // so no system-scope fence is needed to order the fields
+      *reinterpret_cast<uint4*>(mailbox) = make_uint4(counts->n_visible, I, ovf ? 1u : 0u, seq);
+    }
+  }
   __syncthreads();
-  for (int t = tid; t < tiles; t += 1024)
-    order[atomicAdd(&hist[1023 - min((t < kScanCache ? s_cnt[t] : tile_count[(size_t)t * kCtrStride]) >> 3, 1023u)], 1u)] = (uint32_t)t;
+  uint32_t off = s_pre[0] + pref.w[0];
+#pragma unroll
+  for (int u = 0; u < IT; ++u) {
+    if (t0 + u < tiles) {
+      tile_cursor[(size_t)(t0 + u) * kCtrStride] = off;
+      // an iteration that overflows the instance capacity renders nothing
+      ranges[t0 + u] = (c[u] && !ovf) ? make_uint2(off, off + c[u]) : make_uint2(0u, 0u);
+      off += c[u];
+      // tile ids by descending length class: class base + tiles of the class in earlier CTAs / threads / own tiles
+      const int k = cls[u];
+      uint32_t word = 0;
+#pragma unroll
+      for (int w = 0; w < 8; ++w) {
+        const bool hit = (k >> 1) == w;
+        word = hit ? pref.w[1 + w] : word;
+        pref.w[1 + w] += hit ? (1u << ((k & 1) * 16)) : 0u;
+      }
+      order[s_base[k] + ((word >> ((k & 1) * 16)) & 0xffffu)] = (uint32_t)(t0 + u);
+    }
+  }
 }
 
 // ---------------------------------------------------------------------------------------------------------------
 // a3: duplication.  One thread per Gaussian; (depth bits << 32 | index) goes to the bucket of every tile of the rect.
 // ---------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256)
-emit_kernel(const uint32_t* __restrict__ vis_ids, const uint32_t* __restrict__ tiles_touched, const ushort4* __restrict__ rect,
-            const uint32_t* __restrict__ depth_key, int tiles_x, uint32_t* __restrict__ tile_cursor,
+constexpr int kEmitG = 32;    // visible Gaussians per CTA
+constexpr int kEmitT = 128;   // threads per CTA
+
+__global__ void __launch_bounds__(kEmitT)
+emit_kernel(const uint4* __restrict__ vis_rec, int tiles_x, uint32_t* __restrict__ tile_cursor,
             const Counts* __restrict__ counts, uint64_t* __restrict__ keys) {
-  // Block-cooperative: the instances of the block's 256 Gaussians form one work list (prefix sum of the per-Gaussian
-  // tile counts); every round the 256 threads take 256 consecutive work items, whatever Gaussian they belong to, so a
-  // Gaussian covering hundreds of tiles is emitted by the whole block; four independent atomics per thread are put in
-  // flight before their results are used.
-  __shared__ uint32_t s_excl[257], s_w[256], s_xy[256], s_ws[8];
-  __shared__ uint64_t s_key[256];
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  if (counts->overflow) return;
+  // Block-cooperative: the instances of the CTA's 32 Gaussians form one work list (prefix sum of the per-Gaussian tile
+  // counts); every round the 128 threads take consecutive work items, whatever Gaussian they belong to, so a Gaussian
+  // covering hundreds of tiles is emitted by the whole CTA; four independent atomics per thread are put in flight
+  // before their results are used.  Small CTAs (many of them, few Gaussians each): the kernel is a chain of dependent
+  // round trips (record -> cursor atomic -> key store), so what matters is how many chains are in flight per SM.
+  __shared__ uint32_t s_excl[kEmitG + 1], s_w[kEmitG], s_xy[kEmitG];
+  __shared__ uint64_t s_key[kEmitG];
+  const int tid = threadIdx.x;
   const uint32_t V = counts->n_visible;
-  const int64_t k = (int64_t)blockIdx.x * blockDim.x + tid;
-  if ((int64_t)blockIdx.x * blockDim.x >= (int64_t)V) return;
-  const uint32_t i = (k < V) ? vis_ids[k] : 0u;
-  const uint32_t n = (k < V) ? tiles_touched[i] : 0u;
-  ushort4 r = make_ushort4(0, 0, 1, 0);
-  uint64_t key = 0;
-  if (n) {
-    r = rect[i];
-    key = ((uint64_t)depth_key[i] << 32) | (uint64_t)i;
-  }
-  uint32_t incl = n;
+  const uint32_t k0 = blockIdx.x * kEmitG;
+  if (k0 >= V || counts->overflow) return;
+  if (tid < 32) {
+    const uint32_t k = k0 + tid;
+    uint4 rec = make_uint4(0u, 0u, 0u, 0u);
+    if (k < V) rec = __ldg(vis_rec + k);
+    const uint32_t w = (rec.y & 0xffffu) - (rec.x & 0xffffu), h = (rec.y >> 16) - (rec.x >> 16);
+    const uint32_t n = w * h;
+    uint32_t incl = n;
 #pragma unroll
-  for (int d = 1; d < 32; d <<= 1) {
-    const uint32_t v = __shfl_up_sync(0xffffffffu, incl, d);
-    if (lane >= d) incl += v;
+    for (int d = 1; d < 32; d <<= 1) {
+      const uint32_t v = __shfl_up_sync(0xffffffffu, incl, d);
+      if (tid >= d) incl += v;
+    }
+    s_excl[tid] = incl - n;
+    s_w[tid] = max(w, 1u);
+    s_xy[tid] = rec.x;
+    s_key[tid] = ((uint64_t)rec.z << 32) | (uint64_t)rec.w;
+    if (tid == 31) s_excl[32] = incl;
   }
-  if (lane == 31) s_ws[warp] = incl;
   __syncthreads();
-  uint32_t wb = 0;
-#pragma unroll
-  for (int q = 0; q < 8; ++q) wb += (q < warp) ? s_ws[q] : 0u;
-  s_excl[tid] = wb + incl - n;
-  s_w[tid] = (uint32_t)(r.z - r.x);
-  s_xy[tid] = (uint32_t)r.x | ((uint32_t)r.y << 16);
-  s_key[tid] = key;
-  if (tid == 255) s_excl[256] = wb + incl;
-  __syncthreads();
-  const uint32_t total = s_excl[256];
-  for (uint32_t base = 0; base < total; base += 1024) {
+  const uint32_t total = s_excl[kEmitG];
+  for (uint32_t base = 0; base < total; base += kEmitT * 4) {
     uint32_t* cur[4];
     uint64_t kk[4];
     uint32_t pos[4];
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
-      const uint32_t item = base + u * 256 + tid;
+      const uint32_t item = base + u * kEmitT + tid;
       cur[u] = nullptr;
       if (item < total) {
-        int owner = 0;  // last Gaussian of the block whose exclusive prefix is <= item
+        int owner = 0;  // last Gaussian of the CTA whose exclusive prefix is <= item
 #pragma unroll
-        for (int step = 128; step >= 1; step >>= 1)
+        for (int step = kEmitG / 2; step >= 1; step >>= 1)
           if (s_excl[owner + step] <= item) owner += step;
         const uint32_t local = item - s_excl[owner], w = s_w[owner], xy = s_xy[owner];
         const uint32_t ty = (xy >> 16) + local / w, tx = (xy & 0xffffu) + local % w;
@@ -387,8 +456,24 @@ bool handle_overflow(gs_ctx* ctx) {
 
 static int run_tile_scan(gs_ctx* ctx, cudaStream_t s) {
   const int tiles = ctx->cam.tiles_x * ctx->cam.tiles_y;
-  tile_scan_kernel<<<1, 1024, 0, s>>>(tiles, ctx->tile_count, ctx->tile_cursor, ctx->ranges, ctx->tile_order,
-                                      ctx->cap_I, ctx->counts, ctx->mailbox_dev, ctx->seq);
+  if (tiles == 0) return GS_OK;
+  if (!ctx->scan_ws) {
+    GS_CUDA(cudaMalloc((void**)&ctx->scan_ws, (size_t)kScanMaxCta * (kScanAgg + 1) * sizeof(uint32_t)));
+    GS_CUDA(cudaMemset(ctx->scan_ws, 0, (size_t)kScanMaxCta * (kScanAgg + 1) * sizeof(uint32_t)));
+  }
+  uint32_t* agg = ctx->scan_ws;
+  uint32_t* flags = ctx->scan_ws + kScanMaxCta * kScanAgg;
+  const uint32_t epoch = ++ctx->scan_epoch;
+  const int nb1 = (int)div_up(tiles, kScanT);
+  if (nb1 <= kScanMaxCta) {
+    tile_scan_kernel<1><<<nb1, kScanT, 0, s>>>(tiles, ctx->tile_count, ctx->tile_cursor, ctx->ranges, ctx->tile_order, agg,
+                                               flags, epoch, ctx->cap_I, ctx->counts, ctx->mailbox_dev, ctx->seq);
+  } else {
+    const int nb8 = (int)div_up(tiles, kScanT * 8);
+    if (nb8 > kScanMaxCta) return fail(ctx, GS_E_INVALID, "gs_bin_tiles: more than 262144 tiles");
+    tile_scan_kernel<8><<<nb8, kScanT, 0, s>>>(tiles, ctx->tile_count, ctx->tile_cursor, ctx->ranges, ctx->tile_order, agg,
+                                               flags, epoch, ctx->cap_I, ctx->counts, ctx->mailbox_dev, ctx->seq);
+  }
   GS_LAUNCH_CHECK("tile_scan_kernel");
   return GS_OK;
 }
@@ -422,9 +507,8 @@ int launch_binning(gs_ctx* ctx, cudaStream_t s) {
   }
   GS_PROF(3, s);
   if (ctx->N > 0) {
-    emit_kernel<<<(unsigned)div_up(ctx->N, 256), 256, 0, s>>>(ctx->vis_ids, ctx->tiles_touched, ctx->rect, ctx->depth_key,
-                                                              ctx->cam.tiles_x, ctx->tile_cursor, ctx->counts,
-                                                              ctx->keys[0]);
+    emit_kernel<<<(unsigned)div_up(ctx->N, kEmitG), kEmitT, 0, s>>>(ctx->vis_rec, ctx->cam.tiles_x, ctx->tile_cursor,
+                                                                    ctx->counts, ctx->keys[0]);
     GS_LAUNCH_CHECK("emit_kernel");
   }
   GS_PROF(4, s);

@@ -49,7 +49,7 @@ constexpr int kG2D = 12;
 constexpr int kCtrStride = 32;  // per-tile counters are one per 128-byte line (gs_binning.cu)
 
 // Device counters (one per context) + pinned-host mirror ("mailbox") the host may poll without synchronising.
-struct Counts {
+struct alignas(16) Counts {
   uint32_t n_visible;
   uint32_t n_instances;  // total tile instances of the last scan (even if it overflowed)
   uint32_t overflow;     // 1 if n_instances > capacity: nothing was emitted and downstream kernels see 0 instances
@@ -84,6 +84,7 @@ struct gs_ctx {
   uint32_t* depth_key = nullptr;    // [N]
   uint32_t* tiles_touched = nullptr;  // [N]
   uint32_t* vis_ids = nullptr;        // [N] indices of the visible Gaussians, compacted (arbitrary order)
+  uint4* vis_rec = nullptr;           // [N] same order: {tx0 | ty0 << 16, tx1 | ty1 << 16, depth key, index}
   float* g2d = nullptr;             // [N,12]; kept all-zero between iterations (the consumer clears what it reads)
   bool g2d_dirty = false;
 
@@ -102,6 +103,8 @@ struct gs_ctx {
   uint2* ranges = nullptr;          // [tiles]
   uint32_t* tile_count = nullptr;   // [tiles] instances per tile (atomics in gs_preprocess)
   uint32_t* tile_cursor = nullptr;  // [tiles] write cursors of the duplication
+  uint32_t* scan_ws = nullptr;      // tile scan: per-CTA totals [128][17] + epoch flags [128]
+  uint32_t scan_epoch = 0;
   float* final_T = nullptr;         // [H*W]
   uint32_t* n_contrib = nullptr;    // [H*W]
 
@@ -182,9 +185,14 @@ inline int64_t div_up(int64_t a, int64_t b) { return (a + b - 1) / b; }
 
 // Non-blocking read of the pinned-host mailbox the device writes.
 inline Counts read_mailbox(const gs_ctx* ctx) {
+  // the device writes the first four words with one 16-byte store; re-read until the sequence word is stable
   const volatile Counts* m = ctx->mailbox;
   Counts c;
-  c.n_visible = m->n_visible; c.n_instances = m->n_instances; c.overflow = m->overflow; c.seq = m->seq;
+  for (int attempt = 0; attempt < 4; ++attempt) {
+    c.seq = m->seq;
+    c.n_visible = m->n_visible; c.n_instances = m->n_instances; c.overflow = m->overflow;
+    if (m->seq == c.seq) break;
+  }
   c.n_large = 0; c.n_mid = 0;
   return c;
 }

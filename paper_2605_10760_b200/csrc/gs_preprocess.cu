@@ -12,12 +12,13 @@ preprocess_kernel(int64_t N, const float* __restrict__ means, const float* __res
                   const float* __restrict__ quats, const float* __restrict__ opacities, const float* __restrict__ sh,
                   DevCam cam, float4* __restrict__ feat, ushort4* __restrict__ rect, uint32_t* __restrict__ depth_key,
                   uint32_t* __restrict__ tiles_touched, uint32_t* __restrict__ tile_count,
-                  uint32_t* __restrict__ vis_ids, Counts* __restrict__ counts) {
+                  uint32_t* __restrict__ vis_ids, uint4* __restrict__ vis_rec, Counts* __restrict__ counts) {
   constexpr int K = (DEG + 1) * (DEG + 1);
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   float T[12];
   load_pose(cam, T);
   bool vis = false;
+  uint4 rec = make_uint4(0u, 0u, 0u, 0u);  // what the duplication needs: packed tile rect, depth key, index
   if (i < N) {
     const float mu0 = means[3 * i], mu1 = means[3 * i + 1], mu2 = means[3 * i + 2];
     const float o = opacities[i];
@@ -72,7 +73,9 @@ preprocess_kernel(int64_t N, const float* __restrict__ means, const float* __res
       f2.w = (float)P.z;
       feat[3 * i] = f0; feat[3 * i + 1] = f1; feat[3 * i + 2] = f2;
       rect[i] = make_ushort4((unsigned short)tx0, (unsigned short)ty0, (unsigned short)tx1, (unsigned short)ty1);
-      depth_key[i] = __float_as_uint(depth_key_f32(T, mu0, mu1, mu2));
+      const uint32_t dk = __float_as_uint(depth_key_f32(T, mu0, mu1, mu2));
+      depth_key[i] = dk;
+      rec = make_uint4((uint32_t)tx0 | ((uint32_t)ty0 << 16), (uint32_t)tx1 | ((uint32_t)ty1 << 16), dk, (uint32_t)i);
       tiles_touched[i] = (uint32_t)((tx1 - tx0) * (ty1 - ty0));
       for (int ty = ty0; ty < ty1; ++ty)  // MSD digit histogram of the binning sort (gs_binning.cu)
         for (int tx = tx0; tx < tx1; ++tx) atomicAdd(&tile_count[(size_t)(ty * cam.tiles_x + tx) * kCtrStride], 1u);
@@ -87,7 +90,11 @@ preprocess_kernel(int64_t N, const float* __restrict__ means, const float* __res
     uint32_t base = 0;
     if (lane == 0) base = atomicAdd(&counts->n_visible, (uint32_t)__popc(ball));
     base = __shfl_sync(0xffffffffu, base, 0);
-    if (vis) vis_ids[base + __popc(ball & ((1u << lane) - 1))] = (uint32_t)i;
+    if (vis) {
+      const uint32_t slot = base + __popc(ball & ((1u << lane) - 1));
+      vis_ids[slot] = (uint32_t)i;
+      vis_rec[slot] = rec;
+    }
   }
 }
 
@@ -99,7 +106,7 @@ int launch_preprocess(gs_ctx* ctx, cudaStream_t s) {
 #define GS_PRE(D)                                                                                                    \
   preprocess_kernel<D><<<blocks, threads, 0, s>>>(N, ctx->means, ctx->scales, ctx->quats, ctx->opacities, ctx->sh,  \
                                                    ctx->cam, ctx->feat, ctx->rect, ctx->depth_key,                  \
-                                                   ctx->tiles_touched, ctx->tile_count, ctx->vis_ids, ctx->counts)
+                                                   ctx->tiles_touched, ctx->tile_count, ctx->vis_ids, ctx->vis_rec, ctx->counts)
   switch (ctx->sh_degree) {
     case 0: GS_PRE(0); break;
     case 1: GS_PRE(1); break;
