@@ -7,6 +7,12 @@
 
 namespace gs {
 
+// scalar type of the per-Gaussian chain: fp32 (the gradient tolerance is 1e-3 relative L2; the forward projection in
+// gs_preprocess stays fp64).  The pose partial sums are reduced in fp32 inside a warp and in fp64 beyond.
+using R = float;
+__device__ __forceinline__ float gs_rsqrt(float x) { return rsqrtf(x); }
+__device__ __forceinline__ double gs_rsqrt(double x) { return rsqrt(x); }
+
 template <typename T>
 __device__ __forceinline__ void store_or_add(T* p, T v, bool accumulate) {
   *p = accumulate ? (*p + v) : v;
@@ -31,9 +37,9 @@ gauss_bwd_kernel(int64_t N, const float* __restrict__ means, const float* __rest
   (void)N;
   float T[12];
   load_pose(cam, T);
-  double acc[15];
+  R acc[15];
 #pragma unroll
-  for (int k = 0; k < 15; ++k) acc[k] = 0.0;
+  for (int k = 0; k < 15; ++k) acc[k] = (R)0;
   if (vis) {
     float4* gp4 = reinterpret_cast<float4*>(g2d + (size_t)i * kG2D);
     const float4 ga = gp4[0], gb = gp4[1], gc = gp4[2];
@@ -43,31 +49,31 @@ gauss_bwd_kernel(int64_t N, const float* __restrict__ means, const float* __rest
     const float s0 = scales[3 * i], s1 = scales[3 * i + 1], s2 = scales[3 * i + 2];
     const float4 q = *reinterpret_cast<const float4*>(quats + 4 * i);
     const float o = opacities[i];
-    ProjD P;
-    project_gaussian(cam, T, mu0, mu1, mu2, s0, s1, s2, q.x, q.y, q.z, q.w, o, P);
-    const double W[9] = {T[0], T[1], T[2], T[4], T[5], T[6], T[8], T[9], T[10]};
+    Proj<R> P;
+    project_gaussian<R>(cam, T, mu0, mu1, mu2, s0, s1, s2, q.x, q.y, q.z, q.w, o, P);
+    const R W[9] = {T[0], T[1], T[2], T[4], T[5], T[6], T[8], T[9], T[10]};
     // ga.x, ga.y = sum gp dx, sum gp dy (moments about the mean); d power / d mean = -(Q d), ln2 * log2(e) = 1
-    const double g_mx = P.a * (double)ga.x + P.b * (double)ga.y, g_my = P.b * (double)ga.x + P.c * (double)ga.y;
-    const double g_a = -0.5 * (double)ga.z, g_b = -(double)ga.w, g_c = -0.5 * (double)gb.x;
-    const double g_o = (double)gb.y / (double)o;
+    const R g_mx = P.a * (R)ga.x + P.b * (R)ga.y, g_my = P.b * (R)ga.x + P.c * (R)ga.y;
+    const R g_a = -(R)0.5 * (R)ga.z, g_b = -(R)ga.w, g_c = -(R)0.5 * (R)gb.x;
+    const R g_o = (R)gb.y / (R)o;
     const float gcol[3] = {gb.z, gb.w, gc.x};
-    const double g_z = gc.y;
+    const R g_z = gc.y;
     // conic -> Sigma': gS = -Q gQ Q
-    const double q00 = P.a, q01 = P.b, q11 = P.c;
-    const double h = 0.5 * g_b;
-    const double t00 = q00 * g_a + q01 * h, t01 = q00 * h + q01 * g_c;
-    const double t10 = q01 * g_a + q11 * h, t11 = q01 * h + q11 * g_c;
-    const double gS00 = -(t00 * q00 + t01 * q01), gS01 = -(t00 * q01 + t01 * q11);
-    const double gS10 = -(t10 * q00 + t11 * q01), gS11 = -(t10 * q01 + t11 * q11);
+    const R q00 = P.a, q01 = P.b, q11 = P.c;
+    const R h = (R)0.5 * g_b;
+    const R t00 = q00 * g_a + q01 * h, t01 = q00 * h + q01 * g_c;
+    const R t10 = q01 * g_a + q11 * h, t11 = q01 * h + q11 * g_c;
+    const R gS00 = -(t00 * q00 + t01 * q01), gS01 = -(t00 * q01 + t01 * q11);
+    const R gS10 = -(t10 * q00 + t11 * q01), gS11 = -(t10 * q01 + t11 * q11);
     // gM = 2 gS M
-    double gM[6];
+    R gM[6];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-      gM[c] = 2.0 * (gS00 * P.M[c] + gS01 * P.M[3 + c]);
-      gM[3 + c] = 2.0 * (gS10 * P.M[c] + gS11 * P.M[3 + c]);
+      gM[c] = (R)2.0 * (gS00 * P.M[c] + gS01 * P.M[3 + c]);
+      gM[3 + c] = (R)2.0 * (gS10 * P.M[c] + gS11 * P.M[3 + c]);
     }
     // gT = gM M3^T ; gM3 = Tm^T gM
-    double gT[6], gM3[9];
+    R gT[6], gM3[9];
 #pragma unroll
     for (int r = 0; r < 2; ++r)
 #pragma unroll
@@ -78,43 +84,43 @@ gauss_bwd_kernel(int64_t N, const float* __restrict__ means, const float* __rest
 #pragma unroll
       for (int c = 0; c < 3; ++c) gM3[3 * r + c] = P.Tm[r] * gM[c] + P.Tm[3 + r] * gM[3 + c];
     // M3 = R diag(s)
-    const double sd[3] = {s0, s1, s2};
-    double gs_[3], gR[9];
+    const R sd[3] = {s0, s1, s2};
+    R gs_[3], gR[9];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-      gs_[c] = P.R[c] * gM3[c] + P.R[3 + c] * gM3[3 + c] + P.R[6 + c] * gM3[6 + c];
+      gs_[c] = P.Rm[c] * gM3[c] + P.Rm[3 + c] * gM3[3 + c] + P.Rm[6 + c] * gM3[6 + c];
 #pragma unroll
       for (int r = 0; r < 3; ++r) gR[3 * r + c] = gM3[3 * r + c] * sd[c];
     }
     // quaternion (w,x,y,z): gr_k = <gR, dR/dr_k>, then through the normalisation
-    const double w = P.r[0], x = P.r[1], y = P.r[2], z = P.r[3];
-    double gr[4];
-    gr[0] = 2.0 * (-z * gR[1] + y * gR[2] + z * gR[3] - x * gR[5] - y * gR[6] + x * gR[7]);
-    gr[1] = 2.0 * (y * gR[1] + z * gR[2] + y * gR[3] - 2.0 * x * gR[4] - w * gR[5] + z * gR[6] + w * gR[7] - 2.0 * x * gR[8]);
-    gr[2] = 2.0 * (-2.0 * y * gR[0] + x * gR[1] + w * gR[2] + x * gR[3] + z * gR[5] - w * gR[6] + z * gR[7] - 2.0 * y * gR[8]);
-    gr[3] = 2.0 * (-2.0 * z * gR[0] - w * gR[1] + x * gR[2] + w * gR[3] - 2.0 * z * gR[4] + y * gR[5] + x * gR[6] + y * gR[7]);
-    const double rd = w * gr[0] + x * gr[1] + y * gr[2] + z * gr[3];
-    const double iqn = 1.0 / P.qn;
-    double gq[4];
+    const R w = P.r[0], x = P.r[1], y = P.r[2], z = P.r[3];
+    R gr[4];
+    gr[0] = (R)2.0 * (-z * gR[1] + y * gR[2] + z * gR[3] - x * gR[5] - y * gR[6] + x * gR[7]);
+    gr[1] = (R)2.0 * (y * gR[1] + z * gR[2] + y * gR[3] - (R)2.0 * x * gR[4] - w * gR[5] + z * gR[6] + w * gR[7] - (R)2.0 * x * gR[8]);
+    gr[2] = (R)2.0 * (-(R)2.0 * y * gR[0] + x * gR[1] + w * gR[2] + x * gR[3] + z * gR[5] - w * gR[6] + z * gR[7] - (R)2.0 * y * gR[8]);
+    gr[3] = (R)2.0 * (-(R)2.0 * z * gR[0] - w * gR[1] + x * gR[2] + w * gR[3] - (R)2.0 * z * gR[4] + y * gR[5] + x * gR[6] + y * gR[7]);
+    const R rd = w * gr[0] + x * gr[1] + y * gr[2] + z * gr[3];
+    const R iqn = (R)1.0 / P.qn;
+    R gq[4];
 #pragma unroll
     for (int k = 0; k < 4; ++k) gq[k] = (gr[k] - P.r[k] * rd) * iqn;
     // T = J W: gJ = gT W^T (only the four non-zero entries of J), gW += J^T gT
-    const double gJ00 = gT[0] * W[0] + gT[1] * W[1] + gT[2] * W[2];
-    const double gJ02 = gT[0] * W[6] + gT[1] * W[7] + gT[2] * W[8];
-    const double gJ11 = gT[3] * W[3] + gT[4] * W[4] + gT[5] * W[5];
-    const double gJ12 = gT[3] * W[6] + gT[4] * W[7] + gT[5] * W[8];
-    const double iz = 1.0 / P.z, iz2 = iz * iz, fx = cam.fx, fy = cam.fy;
-    double gpc[3];
+    const R gJ00 = gT[0] * W[0] + gT[1] * W[1] + gT[2] * W[2];
+    const R gJ02 = gT[0] * W[6] + gT[1] * W[7] + gT[2] * W[8];
+    const R gJ11 = gT[3] * W[3] + gT[4] * W[4] + gT[5] * W[5];
+    const R gJ12 = gT[3] * W[6] + gT[4] * W[7] + gT[5] * W[8];
+    const R iz = (R)1.0 / P.z, iz2 = iz * iz, fx = cam.fx, fy = cam.fy;
+    R gpc[3];
     gpc[0] = g_mx * fx * iz - gJ02 * fx * iz2;
     gpc[1] = g_my * fy * iz - gJ12 * fy * iz2;
     gpc[2] = -g_mx * fx * P.x * iz2 - g_my * fy * P.y * iz2 + g_z - gJ00 * fx * iz2 - gJ11 * fy * iz2 +
-             2.0 * gJ02 * fx * P.x * iz2 * iz + 2.0 * gJ12 * fy * P.y * iz2 * iz;
+             (R)2.0 * gJ02 * fx * P.x * iz2 * iz + (R)2.0 * gJ12 * fy * P.y * iz2 * iz;
     // colour: same fp32 sequence as the forward, so the clamp decision is identical
-    const double ccx = -((double)T[0] * T[3] + (double)T[4] * T[7] + (double)T[8] * T[11]);
-    const double ccy = -((double)T[1] * T[3] + (double)T[5] * T[7] + (double)T[9] * T[11]);
-    const double ccz = -((double)T[2] * T[3] + (double)T[6] * T[7] + (double)T[10] * T[11]);
-    const double vx = (double)mu0 - ccx, vy = (double)mu1 - ccy, vz = (double)mu2 - ccz;
-    const double ivn = rsqrt(vx * vx + vy * vy + vz * vz);
+    const R ccx = -((R)T[0] * T[3] + (R)T[4] * T[7] + (R)T[8] * T[11]);
+    const R ccy = -((R)T[1] * T[3] + (R)T[5] * T[7] + (R)T[9] * T[11]);
+    const R ccz = -((R)T[2] * T[3] + (R)T[6] * T[7] + (R)T[10] * T[11]);
+    const R vx = (R)mu0 - ccx, vy = (R)mu1 - ccy, vz = (R)mu2 - ccz;
+    const R ivn = gs_rsqrt(vx * vx + vy * vy + vz * vz);
     const float nx = (float)(vx * ivn), ny = (float)(vy * ivn), nz = (float)(vz * ivn);
     float B[K];
     sh_basis<DEG>(nx, ny, nz, B);
@@ -145,10 +151,10 @@ gauss_bwd_kernel(int64_t N, const float* __restrict__ means, const float* __rest
     for (int k = 0; k < K; ++k) wk[k] = shv[3 * k] * gcr[0] + shv[3 * k + 1] * gcr[1] + shv[3 * k + 2] * gcr[2];
     float gnx = 0.f, gny = 0.f, gnz = 0.f;
     if (DEG > 0) sh_basis_grad<DEG>(nx, ny, nz, wk, gnx, gny, gnz);
-    const double nd = (double)nx * gnx + (double)ny * gny + (double)nz * gnz;
-    const double gv[3] = {((double)gnx - nx * nd) * ivn, ((double)gny - ny * nd) * ivn, ((double)gnz - nz * nd) * ivn};
+    const R nd = (R)nx * gnx + (R)ny * gny + (R)nz * gnz;
+    const R gv[3] = {((R)gnx - nx * nd) * ivn, ((R)gny - ny * nd) * ivn, ((R)gnz - nz * nd) * ivn};
     if (WRITE) {
-      const double gmu[3] = {W[0] * gpc[0] + W[3] * gpc[1] + W[6] * gpc[2] + gv[0],
+      const R gmu[3] = {W[0] * gpc[0] + W[3] * gpc[1] + W[6] * gpc[2] + gv[0],
                              W[1] * gpc[0] + W[4] * gpc[1] + W[7] * gpc[2] + gv[1],
                              W[2] * gpc[0] + W[5] * gpc[1] + W[8] * gpc[2] + gv[2]};
 #pragma unroll
@@ -181,7 +187,7 @@ gauss_bwd_kernel(int64_t N, const float* __restrict__ means, const float* __rest
     // pose partial sums: sum g_pc, sum g_v, g_W = J^T gT + g_pc mu^T
     acc[0] = gpc[0]; acc[1] = gpc[1]; acc[2] = gpc[2];
     acc[3] = gv[0]; acc[4] = gv[1]; acc[5] = gv[2];
-    const double mud[3] = {mu0, mu1, mu2};
+    const R mud[3] = {mu0, mu1, mu2};
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
       acc[6 + c] = P.J00 * gT[c] + gpc[0] * mud[c];
@@ -189,7 +195,7 @@ gauss_bwd_kernel(int64_t N, const float* __restrict__ means, const float* __rest
       acc[12 + c] = P.J02 * gT[c] + P.J12 * gT[3 + c] + gpc[2] * mud[c];
     }
   }
-  // block reduction of the 15 pose partials (fp64), one atomic set per block
+  // block reduction of the 15 pose partials: fp32 inside the warp, fp64 across warps and blocks, one atomic set per block
   __shared__ double s_acc[4][15];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const bool any = __any_sync(0xffffffffu, vis);
@@ -202,7 +208,7 @@ gauss_bwd_kernel(int64_t N, const float* __restrict__ means, const float* __rest
   }
   if (lane == 0) {
 #pragma unroll
-    for (int k = 0; k < 15; ++k) s_acc[warp][k] = any ? acc[k] : 0.0;
+    for (int k = 0; k < 15; ++k) s_acc[warp][k] = any ? (double)acc[k] : 0.0;
   }
   __syncthreads();
   if (threadIdx.x < 15) {

@@ -24,7 +24,7 @@ preprocess_kernel(int64_t N, const float* __restrict__ means, const float* __res
     const float o = opacities[i];
     ProjD P;
     const float4 q = *reinterpret_cast<const float4*>(quats + 4 * i);
-    vis = project_gaussian(cam, T, mu0, mu1, mu2, scales[3 * i], scales[3 * i + 1], scales[3 * i + 2], q.x, q.y, q.z,
+    vis = project_gaussian<double>(cam, T, mu0, mu1, mu2, scales[3 * i], scales[3 * i + 1], scales[3 * i + 2], q.x, q.y, q.z,
                            q.w, o, P);
     int tx0 = 0, ty0 = 0, tx1 = 0, ty1 = 0;
     if (vis) vis = tile_rect(cam, P, o, tx0, ty0, tx1, ty1);

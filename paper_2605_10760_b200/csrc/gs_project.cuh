@@ -8,53 +8,60 @@
 
 namespace gs {
 
-struct ProjD {
-  double x, y, z;        // camera-space centre
-  double r[4], qn;       // unit quaternion, |q|
-  double R[9], M3[9];    // R(r), M3 = R diag(s)
-  double J00, J02, J11, J12;
-  double Tm[6], M[6];    // T = J W, M = T M3
-  double cxx, cxy, cyy;  // Sigma' (dilated)
-  double a, b, c;        // conic
-  double mx, my;
+// R = double in gs_preprocess (the 2-D mean and the conic feed the 1e-5 image tolerance), float in the per-Gaussian
+// backward (1e-3 gradient tolerance; fp32 halves the registers and the latency of the chain).
+template <typename R>
+struct Proj {
+  R x, y, z;        // camera-space centre
+  R r[4], qn;       // unit quaternion, |q|
+  R Rm[9], M3[9];   // R(r), M3 = R diag(s)
+  R J00, J02, J11, J12;
+  R Tm[6], M[6];    // T = J W, M = T M3
+  R cxx, cxy, cyy;  // Sigma' (dilated)
+  R a, b, c;        // conic
+  R mx, my;
 };
+using ProjD = Proj<double>;
 
 // Canonical fp32 depth key: bit pattern of fmaf(W20, mx, fmaf(W21, my, fmaf(W22, mz, tz)))  (Q13).
 __device__ __forceinline__ float depth_key_f32(const float* T, float mx, float my, float mz) {
   return __fmaf_rn(T[8], mx, __fmaf_rn(T[9], my, __fmaf_rn(T[10], mz, T[11])));
 }
 
-__device__ __forceinline__ void quat_rotation(const double* r, double* R) {
-  const double w = r[0], x = r[1], y = r[2], z = r[3];
-  R[0] = 1.0 - 2.0 * (y * y + z * z); R[1] = 2.0 * (x * y - w * z);       R[2] = 2.0 * (x * z + w * y);
-  R[3] = 2.0 * (x * y + w * z);       R[4] = 1.0 - 2.0 * (x * x + z * z); R[5] = 2.0 * (y * z - w * x);
-  R[6] = 2.0 * (x * z - w * y);       R[7] = 2.0 * (y * z + w * x);       R[8] = 1.0 - 2.0 * (x * x + y * y);
+template <typename R>
+__device__ __forceinline__ void quat_rotation(const R* r, R* Rm) {
+  const R w = r[0], x = r[1], y = r[2], z = r[3];
+  const R one = (R)1, two = (R)2;
+  Rm[0] = one - two * (y * y + z * z); Rm[1] = two * (x * y - w * z);       Rm[2] = two * (x * z + w * y);
+  Rm[3] = two * (x * y + w * z);       Rm[4] = one - two * (x * x + z * z); Rm[5] = two * (y * z - w * x);
+  Rm[6] = two * (x * z - w * y);       Rm[7] = two * (y * z + w * x);       Rm[8] = one - two * (x * x + y * y);
 }
 
 // Returns false when the Gaussian is culled before any covariance work (behind the near plane, opacity < 1/255) or
 // its projection is degenerate / non-finite.
+template <typename R>
 __device__ __forceinline__ bool project_gaussian(const DevCam& cam, const float* T, float mu0, float mu1, float mu2,
                                                  float s0, float s1, float s2, float q0, float q1, float q2, float q3,
-                                                 float opacity, ProjD& P) {
-  const double W[9] = {T[0], T[1], T[2], T[4], T[5], T[6], T[8], T[9], T[10]};
-  const double m0 = mu0, m1 = mu1, m2 = mu2;
-  P.x = W[0] * m0 + W[1] * m1 + W[2] * m2 + (double)T[3];
-  P.y = W[3] * m0 + W[4] * m1 + W[5] * m2 + (double)T[7];
-  P.z = W[6] * m0 + W[7] * m1 + W[8] * m2 + (double)T[11];
-  if (!(P.z > (double)cam.near_z)) return false;
+                                                 float opacity, Proj<R>& P) {
+  const R W[9] = {(R)T[0], (R)T[1], (R)T[2], (R)T[4], (R)T[5], (R)T[6], (R)T[8], (R)T[9], (R)T[10]};
+  const R m0 = mu0, m1 = mu1, m2 = mu2;
+  P.x = W[0] * m0 + W[1] * m1 + W[2] * m2 + (R)T[3];
+  P.y = W[3] * m0 + W[4] * m1 + W[5] * m2 + (R)T[7];
+  P.z = W[6] * m0 + W[7] * m1 + W[8] * m2 + (R)T[11];
+  if (!(P.z > (R)cam.near_z)) return false;
   if ((double)opacity < 1.0 / 255.0) return false;
-  const double q[4] = {q0, q1, q2, q3};
+  const R q[4] = {(R)q0, (R)q1, (R)q2, (R)q3};
   P.qn = sqrt(q[0] * q[0] + q[1] * q[1] + q[2] * q[2] + q[3] * q[3]);
-  const double iq = 1.0 / P.qn;
+  const R iq = (R)1 / P.qn;
 #pragma unroll
   for (int k = 0; k < 4; ++k) P.r[k] = q[k] * iq;
-  quat_rotation(P.r, P.R);
-  const double s[3] = {s0, s1, s2};
+  quat_rotation<R>(P.r, P.Rm);
+  const R s[3] = {(R)s0, (R)s1, (R)s2};
 #pragma unroll
   for (int r = 0; r < 3; ++r)
 #pragma unroll
-    for (int c = 0; c < 3; ++c) P.M3[3 * r + c] = P.R[3 * r + c] * s[c];
-  const double iz = 1.0 / P.z, fx = cam.fx, fy = cam.fy;
+    for (int c = 0; c < 3; ++c) P.M3[3 * r + c] = P.Rm[3 * r + c] * s[c];
+  const R iz = (R)1 / P.z, fx = cam.fx, fy = cam.fy;
   P.J00 = fx * iz; P.J02 = -fx * P.x * iz * iz;
   P.J11 = fy * iz; P.J12 = -fy * P.y * iz * iz;
 #pragma unroll
@@ -67,15 +74,15 @@ __device__ __forceinline__ bool project_gaussian(const DevCam& cam, const float*
 #pragma unroll
     for (int c = 0; c < 3; ++c)
       P.M[3 * r + c] = P.Tm[3 * r] * P.M3[c] + P.Tm[3 * r + 1] * P.M3[3 + c] + P.Tm[3 * r + 2] * P.M3[6 + c];
-  P.cxx = P.M[0] * P.M[0] + P.M[1] * P.M[1] + P.M[2] * P.M[2] + (double)GS_DILATION;
+  P.cxx = P.M[0] * P.M[0] + P.M[1] * P.M[1] + P.M[2] * P.M[2] + (R)GS_DILATION;
   P.cxy = P.M[0] * P.M[3] + P.M[1] * P.M[4] + P.M[2] * P.M[5];
-  P.cyy = P.M[3] * P.M[3] + P.M[4] * P.M[4] + P.M[5] * P.M[5] + (double)GS_DILATION;
-  const double det = P.cxx * P.cyy - P.cxy * P.cxy;
-  if (!(det > 0.0) || !isfinite(det)) return false;
-  const double idet = 1.0 / det;
+  P.cyy = P.M[3] * P.M[3] + P.M[4] * P.M[4] + P.M[5] * P.M[5] + (R)GS_DILATION;
+  const R det = P.cxx * P.cyy - P.cxy * P.cxy;
+  if (!(det > (R)0) || !isfinite(det)) return false;
+  const R idet = (R)1 / det;
   P.a = P.cyy * idet; P.b = -P.cxy * idet; P.c = P.cxx * idet;
-  P.mx = fx * P.x * iz + (double)cam.cx;
-  P.my = fy * P.y * iz + (double)cam.cy;
+  P.mx = fx * P.x * iz + (R)cam.cx;
+  P.my = fy * P.y * iz + (R)cam.cy;
   if (!isfinite(P.mx) || !isfinite(P.my)) return false;
   return true;
 }
