@@ -117,7 +117,7 @@ struct gs_ctx {
   gs::Counts* mailbox_dev = nullptr;  // device alias of the mailbox
 
   // region shape of the compositing kernels; tuning knobs GS_RASTER_FWD / GS_RASTER_BWD read by gs_create.
-  int shape_fwd = 11;  // forward "NXNY": region per warp = (8 NX) x (4 NY) pixels (the backward is fixed at 8 x 4)
+  int shape_fwd = 0;  // 0: the branch-free 8 x 4 kernel; else the generic forward "NXNY": region per warp = (8 NX) x (4 NY) pixels (the backward is fixed at 8 x 4)
   uint32_t* tile_order = nullptr;      // [tiles] tile ids by descending list length (longest lists are scheduled first)
 
   // side stream: the zero fill of the dense gradient arrays overlaps the (ALU-bound) pixel backward

@@ -183,6 +183,128 @@ raster_fwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Forward, 8x4-pixel regions, one pixel per lane (the default).  Evidence: profiles/r1_v3_regions.md -- the generic
+// kernel above spent 57 warp instructions per relevant (region, Gaussian) entry, a third of them on the mask / vote /
+// branch bookkeeping of its groups of four.  Here phase 2 is branch-free: every relevant entry is evaluated and blended
+// under a per-lane predicate (alpha_eff = 0 where the pixel is not hit), four entries unrolled for ILP, one vote per
+// four entries for the early exit.  ~26 instructions per entry.
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(32)
+raster_fwd84_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order, const uint2* __restrict__ ranges,
+                    const uint32_t* __restrict__ ids, const float4* __restrict__ feat, float bg0, float bg1, float bg2,
+                    float* __restrict__ rgb, float* __restrict__ depth, float* __restrict__ alpha_out,
+                    float* __restrict__ final_T, uint32_t* __restrict__ n_contrib) {
+  __shared__ __align__(16) float4 s_feat[2][kWarpBatch * 3];          // raw records, double-buffered (cp.async)
+  __shared__ __align__(16) float4 s_rel[(kWarpBatch + kGroup) * 3];    // decoded records of the relevant Gaussians
+  const int lane = threadIdx.x;
+  const int tile = (int)__ldg(order + blockIdx.x / 8), sub = blockIdx.x % 8;
+  const int ox = (tile % tiles_x) * GS_TILE + (sub % 2) * 8, oy = (tile / tiles_x) * GS_TILE + (sub / 2) * 4;
+  const int lx = lane & 7, ly = lane >> 3;
+  const float fx0 = (float)lx, fy0 = (float)ly;
+  const bool inside = ox + lx < W && oy + ly < H;
+  const uint2 range = ranges[tile];
+  const int n = (int)(range.y - range.x);
+  const int nb = (n + kWarpBatch - 1) / kWarpBatch;
+  // T starts at 0 for a lane outside the image, so such a lane never blends (and writes nothing)
+  float T = inside ? 1.f : 0.f, C0 = 0.f, C1 = 0.f, C2 = 0.f, D = 0.f;
+  uint32_t last = 0;
+
+  auto issue = [&](int b, uint32_t id) {
+    if (b * kWarpBatch + lane < n) {
+      const float4* src = feat + 3 * (size_t)id;
+      float4* dst = &s_feat[b & 1][lane * 3];
+      cp_async16(dst, src); cp_async16(dst + 1, src + 1); cp_async16(dst + 2, src + 2);
+    }
+    cp_async_commit();
+  };
+  uint32_t id_next = 0;
+  if (nb > 0) {
+    issue(0, lane < n ? __ldg(ids + range.x + lane) : 0u);
+    if (nb > 1) id_next = (kWarpBatch + lane < n) ? __ldg(ids + range.x + kWarpBatch + lane) : 0u;
+  }
+  bool stop = !__any_sync(kFull, inside);
+  for (int b = 0; b < nb && !stop; ++b) {
+    if (b + 1 < nb) {
+      issue(b + 1, id_next);
+      const int i2 = (b + 2) * kWarpBatch + lane;
+      if (b + 2 < nb) id_next = (i2 < n) ? __ldg(ids + range.x + i2) : 0u;
+      cp_async_wait<1>();
+    } else {
+      cp_async_wait<0>();
+    }
+    __syncwarp();
+    const int cnt = min(kWarpBatch, n - b * kWarpBatch);
+    const float4* sf = s_feat[b & 1];
+    // phase 1: lane g decodes Gaussian g once (region-local mean) and, if its ellipse can reach the region, appends
+    // the decoded record to the compact list s_rel in list order; the last word is the list position + 1
+    bool relevant = false;
+    float4 c0 = make_float4(0.f, 0.f, 0.f, 0.f), c1 = c0;
+    if (lane < cnt) {
+      GaussReg g;
+      decode_gauss(sf[3 * lane], sf[3 * lane + 1], ox, oy, g);
+      relevant = region_max_power(g, 7.f, 3.f) >= g.thr - 1e-3f;
+      c0 = make_float4(g.mx, g.my, g.A, g.B);
+      c1 = make_float4(g.C, g.o, g.thr, __int_as_float(b * kWarpBatch + lane + 1));
+    }
+    const unsigned rel = __ballot_sync(kFull, relevant);
+    const int nrel = __popc(rel);
+    if (relevant) {
+      const int r = __popc(rel & ((1u << lane) - 1u));
+      s_rel[3 * r] = c0; s_rel[3 * r + 1] = c1; s_rel[3 * r + 2] = sf[3 * lane + 2];
+    }
+    if (lane < kGroup) {  // padding records never pass: p >= NaN is false
+      s_rel[3 * (nrel + lane)] = make_float4(0.f, 0.f, 0.f, 0.f);
+      s_rel[3 * (nrel + lane) + 1] = make_float4(0.f, 0.f, __int_as_float(0x7fc00000), 0.f);
+      s_rel[3 * (nrel + lane) + 2] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    __syncwarp();
+    // phase 2: front to back, branch-free
+    for (int r0 = 0; r0 < nrel; r0 += kGroup) {
+#pragma unroll
+      for (int q = 0; q < kGroup; ++q) {
+        const float4 a0 = s_rel[3 * (r0 + q)], a1 = s_rel[3 * (r0 + q) + 1], f2 = s_rel[3 * (r0 + q) + 2];
+        float dx, dy;
+        const float p = eval_power1(a0.x, a0.y, a0.z, a0.w, a1.x, fx0, fy0, dx, dy);
+        const bool hit = (p >= a1.z) && (T >= GS_T_MIN);   // alpha >= 1/255 and the pixel has not terminated
+        const float a = hit ? fminf(GS_ALPHA_MAX, __fmul_rn(a1.y, ex2_approx(p))) : 0.f;
+        const float w = a * T;
+        C0 = fmaf(f2.x, w, C0);
+        C1 = fmaf(f2.y, w, C1);
+        C2 = fmaf(f2.z, w, C2);
+        D = fmaf(f2.w, w, D);
+        T = T * (1.f - a);
+        last = hit ? __float_as_uint(a1.w) : last;
+      }
+      if (!__any_sync(kFull, T >= GS_T_MIN)) { stop = true; break; }
+    }
+    __syncwarp();
+  }
+  cp_async_wait<0>();
+  if (inside) {
+    const size_t HW = (size_t)W * H;
+    const size_t p = (size_t)(oy + ly) * W + (ox + lx);
+    if (rgb) {
+      rgb[p] = fmaf(T, bg0, C0);
+      rgb[HW + p] = fmaf(T, bg1, C1);
+      rgb[2 * HW + p] = fmaf(T, bg2, C2);
+    }
+    if (depth) depth[p] = D;
+    if (alpha_out) alpha_out[p] = 1.f - T;
+    final_T[p] = T;
+    n_contrib[p] = last;
+  }
+}
+
+static int launch_fwd84(gs_ctx* ctx, cudaStream_t s, float* rgb, float* depth, float* alpha) {
+  const int units = ctx->cam.tiles_x * ctx->cam.tiles_y * 8;
+  raster_fwd84_kernel<<<units, 32, 0, s>>>(ctx->cam.W, ctx->cam.H, ctx->cam.tiles_x, ctx->tile_order, ctx->ranges,
+                                           ctx->vals[ctx->sorted_buf], ctx->feat, ctx->bg[0], ctx->bg[1], ctx->bg[2],
+                                           rgb, depth, alpha, ctx->final_T, ctx->n_contrib);
+  GS_LAUNCH_CHECK("raster_fwd84_kernel");
+  return GS_OK;
+}
+
 template <int NX, int NY>
 static int launch_fwd_t(gs_ctx* ctx, cudaStream_t s, float* rgb, float* depth, float* alpha) {
   const int units = ctx->cam.tiles_x * ctx->cam.tiles_y * (2 / NX) * (4 / NY);
@@ -206,6 +328,7 @@ static int launch_fwd_t(gs_ctx* ctx, cudaStream_t s, float* rgb, float* depth, f
 
 int launch_raster_fwd(gs_ctx* ctx, cudaStream_t s, float* rgb, float* depth, float* alpha) {
   if (ctx->cam.tiles_x * ctx->cam.tiles_y == 0) return GS_OK;
+  if (ctx->shape_fwd == 0) return launch_fwd84(ctx, s, rgb, depth, alpha);
   GS_DISPATCH(ctx->shape_fwd, launch_fwd_t, ctx, s, rgb, depth, alpha)
 }
 

@@ -46,16 +46,16 @@ __device__ __forceinline__ void decode_gauss(const float4& f0, const float4& f1,
   g.thr = f0.w;
 }
 
-// power2 of every slot: p[ky*NX+kx] = A dx^2 + B dx dy + C dy^2 with the products shared across rows / columns.
+// power2 of every slot: p[ky*NX+kx] = dx (A dx + B dy) + C dy^2, with the products shared across rows / columns.
+// Explicit rounding intrinsics: the sequence is the same in every kernel that includes this header.
 template <int NX, int NY>
 __device__ __forceinline__ void eval_power(const GaussReg& g, float fx0, float fy0, float (&dx)[NX], float (&dy)[NY],
                                            float (&p)[NX * NY]) {
-  float ax[NX], bx[NX], cy[NY];
+  float ax[NX], cy[NY];
 #pragma unroll
   for (int kx = 0; kx < NX; ++kx) {
     dx[kx] = __fsub_rn(fx0 + 8.f * kx, g.mx);
-    ax[kx] = __fmul_rn(__fmul_rn(g.A, dx[kx]), dx[kx]);
-    bx[kx] = __fmul_rn(g.B, dx[kx]);
+    ax[kx] = __fmul_rn(g.A, dx[kx]);
   }
 #pragma unroll
   for (int ky = 0; ky < NY; ++ky) {
@@ -65,7 +65,16 @@ __device__ __forceinline__ void eval_power(const GaussReg& g, float fx0, float f
 #pragma unroll
   for (int ky = 0; ky < NY; ++ky)
 #pragma unroll
-    for (int kx = 0; kx < NX; ++kx) p[ky * NX + kx] = __fmaf_rn(bx[kx], dy[ky], __fadd_rn(ax[kx], cy[ky]));
+    for (int kx = 0; kx < NX; ++kx)
+      p[ky * NX + kx] = __fmaf_rn(dx[kx], __fmaf_rn(g.B, dy[ky], ax[kx]), cy[ky]);
+}
+
+// the same sequence for one pixel per lane (8x4 regions)
+__device__ __forceinline__ float eval_power1(float mx, float my, float A, float B, float C, float fx0, float fy0,
+                                             float& dx, float& dy) {
+  dx = __fsub_rn(fx0, mx);
+  dy = __fsub_rn(fy0, my);
+  return __fmaf_rn(dx, __fmaf_rn(B, dy, __fmul_rn(A, dx)), __fmul_rn(__fmul_rn(C, dy), dy));
 }
 
 __device__ __forceinline__ float rcp_approx(float x) {
