@@ -81,7 +81,7 @@ GS_API int gs_destroy(gs_ctx* ctx);
 GS_API const char* gs_last_error(const gs_ctx* ctx);
 
 /* Step a1 -- EWA projection, conic, screen extent, colour (oracle reading C1 steps 1-6, 8).
- *   N            number of Gaussians (0 <= N < 2^27)
+ *   N            number of Gaussians (0 <= N < 2^24: sorted list entries carry index << 8 | region mask)
  *   sh_degree    0..3; K = (sh_degree+1)^2 coefficients per channel
  *   means        [N,3]  world-space centres mu
  *   scales       [N,3]  ACTIVATED scales s > 0  (Sigma = R diag(s)^2 R^T)

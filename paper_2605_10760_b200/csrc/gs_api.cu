@@ -183,7 +183,7 @@ int gs_preprocess(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, const flo
                   const float* quats, const float* opacities, const float* sh, const gs_camera* cam,
                   const float* T_cw_dev) {
   if (!ctx) return GS_E_INVALID;
-  if (N < 0 || N >= (1ll << 27) || sh_degree < 0 || sh_degree > 3 || !cam) return fail(ctx, GS_E_INVALID, "gs_preprocess: bad N, sh_degree or camera");
+  if (N < 0 || N >= (1ll << 24) || sh_degree < 0 || sh_degree > 3 || !cam) return fail(ctx, GS_E_INVALID, "gs_preprocess: bad N, sh_degree or camera");
   if (N > 0 && (!means || !scales || !quats || !opacities || !sh)) return fail(ctx, GS_E_INVALID, "gs_preprocess: null parameter array");
   if (cam->width <= 0 || cam->height <= 0 || cam->width > 65535 * GS_TILE || cam->height > 65535 * GS_TILE)
     return fail(ctx, GS_E_INVALID, "gs_preprocess: bad image size");
@@ -317,7 +317,9 @@ int gs_get_binning(gs_ctx* ctx, void* stream, uint64_t* keys_sorted, uint32_t* i
   if (keys_sorted && I) {
     if ((rc = export_sorted_keys(ctx, s, keys_sorted)) != GS_OK) return rc;
   }
-  if (ids_sorted && I) GS_CUDA(cudaMemcpyAsync(ids_sorted, ctx->vals[ctx->sorted_buf], (size_t)I * 4, cudaMemcpyDeviceToDevice, s));
+  if (ids_sorted && I) {
+    if ((rc = export_sorted_ids(ctx, s, I, ids_sorted)) != GS_OK) return rc;
+  }
   if (tile_ranges)
     GS_CUDA(cudaMemcpyAsync(tile_ranges, ctx->ranges, (size_t)ctx->cam.tiles_x * ctx->cam.tiles_y * 8, cudaMemcpyDeviceToDevice, s));
   return GS_OK;

@@ -13,6 +13,7 @@
 //      whatever the arrival order was.  Buckets beyond the shared-memory capacity are sorted in global memory.
 // Integer work only.  Bytes: 8 I (emit) + 8 I (sort read) + 12 I (sorted keys + ids) vs (8 + 24 * 6) I before.
 #include "gs_internal.cuh"
+#include "gs_raster.cuh"
 
 namespace gs {
 
@@ -179,16 +180,33 @@ tile_scan_kernel(int tiles, const uint32_t* __restrict__ tile_count, uint32_t* _
 constexpr int kEmitG = 32;    // visible Gaussians per CTA
 constexpr int kEmitT = 128;   // threads per CTA
 
+// Which of the eight 8x4-pixel regions of tile (tx, ty) can the ellipse {alpha >= 1/255} of this Gaussian reach?  The
+// test is the one the compositing kernels used to repeat per (region, batch) in their phase 1 (exact maximum of the
+// concave power over the region rectangle, gs_raster.cuh), done ONCE per instance here: profiles/r1_v4 -- phase 1 was
+// 27 % of the forward's instructions and its staging of never-relevant records 2/3 of the cp.async traffic.
+__device__ __forceinline__ uint32_t region_mask(const float4& f0, const float4& f1, int tx, int ty) {
+  uint32_t m = 0;
+#pragma unroll
+  for (int sub = 0; sub < 8; ++sub) {
+    GaussReg g;
+    decode_gauss(f0, f1, tx * GS_TILE + (sub % 2) * 8, ty * GS_TILE + (sub / 2) * 4, g);
+    m |= (region_max_power(g, 7.f, 3.f) >= g.thr - 1e-3f) ? (1u << sub) : 0u;
+  }
+  return m;
+}
+
 __global__ void __launch_bounds__(kEmitT)
-emit_kernel(const uint4* __restrict__ vis_rec, int tiles_x, uint32_t* __restrict__ tile_cursor,
-            const Counts* __restrict__ counts, uint64_t* __restrict__ keys) {
+emit_kernel(const uint4* __restrict__ vis_rec, const float4* __restrict__ feat, int tiles_x,
+            uint32_t* __restrict__ tile_cursor, const Counts* __restrict__ counts, uint64_t* __restrict__ keys) {
   // Block-cooperative: the instances of the CTA's 32 Gaussians form one work list (prefix sum of the per-Gaussian tile
   // counts); every round the 128 threads take consecutive work items, whatever Gaussian they belong to, so a Gaussian
   // covering hundreds of tiles is emitted by the whole CTA; four independent atomics per thread are put in flight
   // before their results are used.  Small CTAs (many of them, few Gaussians each): the kernel is a chain of dependent
   // round trips (record -> cursor atomic -> key store), so what matters is how many chains are in flight per SM.
+  // key = depth bits << 32 | index << 8 | region mask (the mask is a function of (index, tile): the order is unchanged)
   __shared__ uint32_t s_excl[kEmitG + 1], s_w[kEmitG], s_xy[kEmitG];
   __shared__ uint64_t s_key[kEmitG];
+  __shared__ float4 s_f0[kEmitG], s_f1[kEmitG];
   const int tid = threadIdx.x;
   const uint32_t V = counts->n_visible;
   const uint32_t k0 = blockIdx.x * kEmitG;
@@ -196,7 +214,11 @@ emit_kernel(const uint4* __restrict__ vis_rec, int tiles_x, uint32_t* __restrict
   if (tid < 32) {
     const uint32_t k = k0 + tid;
     uint4 rec = make_uint4(0u, 0u, 0u, 0u);
-    if (k < V) rec = __ldg(vis_rec + k);
+    if (k < V) {
+      rec = __ldg(vis_rec + k);
+      s_f0[tid] = __ldg(feat + 3 * (size_t)rec.w);
+      s_f1[tid] = __ldg(feat + 3 * (size_t)rec.w + 1);
+    }
     const uint32_t w = (rec.y & 0xffffu) - (rec.x & 0xffffu), h = (rec.y >> 16) - (rec.x >> 16);
     const uint32_t n = w * h;
     uint32_t incl = n;
@@ -208,7 +230,7 @@ emit_kernel(const uint4* __restrict__ vis_rec, int tiles_x, uint32_t* __restrict
     s_excl[tid] = incl - n;
     s_w[tid] = max(w, 1u);
     s_xy[tid] = rec.x;
-    s_key[tid] = ((uint64_t)rec.z << 32) | (uint64_t)rec.w;
+    s_key[tid] = ((uint64_t)rec.z << 32) | ((uint64_t)rec.w << 8);
     if (tid == 31) s_excl[32] = incl;
   }
   __syncthreads();
@@ -229,7 +251,7 @@ emit_kernel(const uint4* __restrict__ vis_rec, int tiles_x, uint32_t* __restrict
         const uint32_t local = item - s_excl[owner], w = s_w[owner], xy = s_xy[owner];
         const uint32_t ty = (xy >> 16) + local / w, tx = (xy & 0xffffu) + local % w;
         cur[u] = &tile_cursor[(size_t)(ty * tiles_x + tx) * kCtrStride];
-        kk[u] = s_key[owner];
+        kk[u] = s_key[owner] | (uint64_t)region_mask(s_f0[owner], s_f1[owner], (int)tx, (int)ty);
       }
     }
 #pragma unroll
@@ -425,6 +447,18 @@ __global__ void export_keys_kernel(int tiles, const uint2* __restrict__ ranges, 
   for (uint32_t k = r.x + threadIdx.x; k < r.y; k += blockDim.x) out[k] = ((uint64_t)tile << 32) | (keys[k] >> 32);
 }
 
+__global__ void export_ids_kernel(int64_t I, const uint32_t* __restrict__ vals, uint32_t* __restrict__ out) {
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k < I) out[k] = vals[k] >> 8;  // strip the region mask
+}
+
+int export_sorted_ids(gs_ctx* ctx, cudaStream_t s, int64_t I, uint32_t* out) {
+  if (I <= 0) return GS_OK;
+  export_ids_kernel<<<(unsigned)div_up(I, 256), 256, 0, s>>>(I, ctx->vals[ctx->sorted_buf], out);
+  GS_LAUNCH_CHECK("export_ids_kernel");
+  return GS_OK;
+}
+
 int export_sorted_keys(gs_ctx* ctx, cudaStream_t s, uint64_t* out) {
   const int tiles = ctx->cam.tiles_x * ctx->cam.tiles_y;
   if (tiles == 0) return GS_OK;
@@ -507,8 +541,8 @@ int launch_binning(gs_ctx* ctx, cudaStream_t s) {
   }
   GS_PROF(3, s);
   if (ctx->N > 0) {
-    emit_kernel<<<(unsigned)div_up(ctx->N, kEmitG), kEmitT, 0, s>>>(ctx->vis_rec, ctx->cam.tiles_x, ctx->tile_cursor,
-                                                                    ctx->counts, ctx->keys[0]);
+    emit_kernel<<<(unsigned)div_up(ctx->N, kEmitG), kEmitT, 0, s>>>(ctx->vis_rec, ctx->feat, ctx->cam.tiles_x,
+                                                                    ctx->tile_cursor, ctx->counts, ctx->keys[0]);
     GS_LAUNCH_CHECK("emit_kernel");
   }
   GS_PROF(4, s);

@@ -94,7 +94,7 @@ struct gs_ctx {
   int64_t cal_N = -1;
   int32_t cal_W = -1, cal_H = -1;
   uint64_t* keys[2] = {nullptr, nullptr};  // [0]: (depth bits << 32 | id) bucketed by tile, sorted in place
-  uint32_t* vals[2] = {nullptr, nullptr};  // [0]: sorted Gaussian ids (what the compositing kernels read)
+  uint32_t* vals[2] = {nullptr, nullptr};  // [0]: sorted (Gaussian id << 8 | region mask): what the compositing kernels read
   int sorted_buf = 0;
   bool sort_attr_set = false;
 
@@ -209,6 +209,7 @@ int launch_pose_final(gs_ctx* ctx, cudaStream_t s, uint32_t flags, float* g_twis
 int ensure_instance_capacity(gs_ctx* ctx, int64_t need);
 bool handle_overflow(gs_ctx* ctx);
 int export_sorted_keys(gs_ctx* ctx, cudaStream_t s, uint64_t* out);
+int export_sorted_ids(gs_ctx* ctx, cudaStream_t s, int64_t I, uint32_t* out);
 int launch_workload_stats(gs_ctx* ctx, cudaStream_t s, uint64_t* out_host);
 
 }  // namespace gs

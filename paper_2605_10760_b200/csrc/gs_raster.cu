@@ -52,7 +52,7 @@ raster_fwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
 
   auto issue = [&](int b, uint32_t id) {
     if (b * kWarpBatch + lane < n) {
-      const float4* src = feat + 3 * (size_t)id;
+      const float4* src = feat + 3 * (size_t)(id >> 8);  // list entries are index << 8 | region mask
       float4* dst = &s_feat[b & 1][lane * 3];
       cp_async16(dst, src); cp_async16(dst + 1, src + 1); cp_async16(dst + 2, src + 2);
     }
@@ -195,8 +195,9 @@ raster_fwd84_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ orde
                     const uint32_t* __restrict__ ids, const float4* __restrict__ feat, float bg0, float bg1, float bg2,
                     float* __restrict__ rgb, float* __restrict__ depth, float* __restrict__ alpha_out,
                     float* __restrict__ final_T, uint32_t* __restrict__ n_contrib) {
-  __shared__ __align__(16) float4 s_feat[2][kWarpBatch * 3];          // raw records, double-buffered (cp.async)
-  __shared__ __align__(16) float4 s_rel[(kWarpBatch + kGroup) * 3];    // decoded records of the relevant Gaussians
+  __shared__ __align__(16) float4 s_feat[2][kWarpBatch * 3];          // raw records of the relevant entries (cp.async)
+  __shared__ uint32_t s_pos[2][kWarpBatch];                            // their list positions + 1
+  __shared__ __align__(16) float4 s_rel[(kWarpBatch + kGroup) * 3];    // decoded records
   const int lane = threadIdx.x;
   const int tile = (int)__ldg(order + blockIdx.x / 8), sub = blockIdx.x % 8;
   const int ox = (tile % tiles_x) * GS_TILE + (sub % 2) * 8, oy = (tile / tiles_x) * GS_TILE + (sub / 2) * 4;
@@ -210,53 +211,58 @@ raster_fwd84_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ orde
   float T = inside ? 1.f : 0.f, C0 = 0.f, C1 = 0.f, C2 = 0.f, D = 0.f;
   uint32_t last = 0;
 
-  auto issue = [&](int b, uint32_t id) {
-    if (b * kWarpBatch + lane < n) {
-      const float4* src = feat + 3 * (size_t)id;
-      float4* dst = &s_feat[b & 1][lane * 3];
+  // phase 1: the list entries are (index << 8 | region mask) -- gs_bin_tiles already decided which regions of the tile
+  // a Gaussian can reach.  Lane g looks at entry g of the batch; the relevant ones are compacted (ballot rank) and only
+  // their records are staged, one batch ahead.
+  auto issue = [&](int b, uint32_t v) -> int {
+    const bool relevant = (b * kWarpBatch + lane < n) && ((v >> sub) & 1u);
+    const unsigned rel = __ballot_sync(kFull, relevant);
+    if (relevant) {
+      const int r = __popc(rel & ((1u << lane) - 1u));
+      const float4* src = feat + 3 * (size_t)(v >> 8);
+      float4* dst = &s_feat[b & 1][r * 3];
       cp_async16(dst, src); cp_async16(dst + 1, src + 1); cp_async16(dst + 2, src + 2);
+      s_pos[b & 1][r] = (uint32_t)(b * kWarpBatch + lane + 1);
     }
     cp_async_commit();
+    return __popc(rel);
   };
-  uint32_t id_next = 0;
+  uint32_t v_next = 0;
+  int nrel = 0, nrel_next = 0;
   if (nb > 0) {
-    issue(0, lane < n ? __ldg(ids + range.x + lane) : 0u);
-    if (nb > 1) id_next = (kWarpBatch + lane < n) ? __ldg(ids + range.x + kWarpBatch + lane) : 0u;
+    nrel_next = issue(0, lane < n ? __ldg(ids + range.x + lane) : 0u);
+    if (nb > 1) v_next = (kWarpBatch + lane < n) ? __ldg(ids + range.x + kWarpBatch + lane) : 0u;
   }
   bool stop = !__any_sync(kFull, inside);
   for (int b = 0; b < nb && !stop; ++b) {
+    nrel = nrel_next;
     if (b + 1 < nb) {
-      issue(b + 1, id_next);
+      nrel_next = issue(b + 1, v_next);
       const int i2 = (b + 2) * kWarpBatch + lane;
-      if (b + 2 < nb) id_next = (i2 < n) ? __ldg(ids + range.x + i2) : 0u;
+      if (b + 2 < nb) v_next = (i2 < n) ? __ldg(ids + range.x + i2) : 0u;
       cp_async_wait<1>();
     } else {
       cp_async_wait<0>();
     }
     __syncwarp();
-    const int cnt = min(kWarpBatch, n - b * kWarpBatch);
+    if (nrel == 0) continue;
     const float4* sf = s_feat[b & 1];
-    // phase 1: lane g decodes Gaussian g once (region-local mean) and, if its ellipse can reach the region, appends
-    // the decoded record to the compact list s_rel in list order; the last word is the list position + 1
-    bool relevant = false;
-    float4 c0 = make_float4(0.f, 0.f, 0.f, 0.f), c1 = c0;
-    if (lane < cnt) {
+    if (lane < nrel) {  // decode once per (region, Gaussian): region-local mean
       GaussReg g;
       decode_gauss(sf[3 * lane], sf[3 * lane + 1], ox, oy, g);
-      relevant = region_max_power(g, 7.f, 3.f) >= g.thr - 1e-3f;
-      c0 = make_float4(g.mx, g.my, g.A, g.B);
-      c1 = make_float4(g.C, g.o, g.thr, __int_as_float(b * kWarpBatch + lane + 1));
+      s_rel[3 * lane] = make_float4(g.mx, g.my, g.A, g.B);
+      s_rel[3 * lane + 1] = make_float4(g.C, g.o, g.thr, __uint_as_float(s_pos[b & 1][lane]));
+      s_rel[3 * lane + 2] = sf[3 * lane + 2];
+    } else if (lane < nrel + kGroup) {  // padding records never pass: p >= NaN is false
+      s_rel[3 * lane] = make_float4(0.f, 0.f, 0.f, 0.f);
+      s_rel[3 * lane + 1] = make_float4(0.f, 0.f, __int_as_float(0x7fc00000), 0.f);
+      s_rel[3 * lane + 2] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
-    const unsigned rel = __ballot_sync(kFull, relevant);
-    const int nrel = __popc(rel);
-    if (relevant) {
-      const int r = __popc(rel & ((1u << lane) - 1u));
-      s_rel[3 * r] = c0; s_rel[3 * r + 1] = c1; s_rel[3 * r + 2] = sf[3 * lane + 2];
-    }
-    if (lane < kGroup) {  // padding records never pass: p >= NaN is false
-      s_rel[3 * (nrel + lane)] = make_float4(0.f, 0.f, 0.f, 0.f);
-      s_rel[3 * (nrel + lane) + 1] = make_float4(0.f, 0.f, __int_as_float(0x7fc00000), 0.f);
-      s_rel[3 * (nrel + lane) + 2] = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (nrel + kGroup > kWarpBatch && lane < nrel + kGroup - kWarpBatch) {
+      const int r = kWarpBatch + lane;
+      s_rel[3 * r] = make_float4(0.f, 0.f, 0.f, 0.f);
+      s_rel[3 * r + 1] = make_float4(0.f, 0.f, __int_as_float(0x7fc00000), 0.f);
+      s_rel[3 * r + 2] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
     __syncwarp();
     // phase 2: front to back, branch-free

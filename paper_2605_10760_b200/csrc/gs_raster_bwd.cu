@@ -99,6 +99,7 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
   constexpr int RPT = 8;  // 8x4-pixel regions per 16x16 tile
   __shared__ __align__(16) float4 s_feat[2][kWarpBatch * 3];
   __shared__ __align__(16) float4 s_rel[(kWarpBatch + kGroup) * 3];
+  __shared__ uint32_t s_tag[2][kWarpBatch];
   __shared__ __align__(16) float2 s_pair[kSlots * kPairRow];
   __shared__ __align__(16) float4 s_pix[32];
   const int lane = threadIdx.x;
@@ -130,55 +131,57 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
   float slot_mx = 0.f, slot_my = 0.f;  // record of slot (lane & 15), kept in registers
   uint32_t slot_id = 0;
 
-  auto issue = [&](int b, uint32_t id) {
-    if (b * kWarpBatch + lane < n) {
-      const float4* src = feat + 3 * (size_t)id;
-      float4* dst = &s_feat[b & 1][lane * 3];
+  // phase 1: the list entries are (index << 8 | region mask) -- gs_bin_tiles already decided which regions of the tile
+  // a Gaussian can reach.  Lane g looks at entry g of the batch; the relevant ones are compacted in REVERSE list order
+  // (ballot rank) and only their records are staged, one batch ahead; tag = index << 5 | position in the batch.
+  auto issue = [&](int b, uint32_t v) -> int {
+    const bool relevant = (b * kWarpBatch + lane < n) && ((v >> sub) & 1u);
+    const unsigned rel = __ballot_sync(kFull, relevant);
+    const int cnt = __popc(rel);
+    if (relevant) {
+      const int r = cnt - 1 - __popc(rel & ((1u << lane) - 1u));
+      const float4* src = feat + 3 * (size_t)(v >> 8);
+      float4* dst = &s_feat[b & 1][r * 3];
       cp_async16(dst, src); cp_async16(dst + 1, src + 1); cp_async16(dst + 2, src + 2);
+      s_tag[b & 1][r] = ((v >> 8) << 5) | (uint32_t)lane;
     }
     cp_async_commit();
+    return cnt;
   };
-  uint32_t id_cur = 0, id_staged = 0, id_next = 0;  // ids of this lane's entry in batches b, b - 1, b - 2
+  uint32_t v_next = 0;
+  int nrel = 0, nrel_next = 0;
   if (nb > 0) {
     const int i0 = (nb - 1) * kWarpBatch + lane;
-    id_staged = i0 < n ? __ldg(ids + range.x + i0) : 0u;
-    issue(nb - 1, id_staged);
-    if (nb > 1) id_next = __ldg(ids + range.x + (nb - 2) * kWarpBatch + lane);
+    nrel_next = issue(nb - 1, i0 < n ? __ldg(ids + range.x + i0) : 0u);
+    if (nb > 1) v_next = __ldg(ids + range.x + (nb - 2) * kWarpBatch + lane);
   }
   for (int b = nb - 1; b >= 0; --b) {
-    id_cur = id_staged;
+    nrel = nrel_next;
     if (b >= 1) {
-      issue(b - 1, id_next);
-      id_staged = id_next;
-      if (b >= 2) id_next = __ldg(ids + range.x + (b - 2) * kWarpBatch + lane);
+      nrel_next = issue(b - 1, v_next);
+      if (b >= 2) v_next = __ldg(ids + range.x + (b - 2) * kWarpBatch + lane);
       cp_async_wait<1>();
     } else {
       cp_async_wait<0>();
     }
     __syncwarp();
-    const int cnt = min(kWarpBatch, n - b * kWarpBatch);
+    if (nrel == 0) continue;
     const int lastb = (int)last - b * kWarpBatch;  // entries of this batch at positions < lastb were blended by this pixel
     const float4* sf = s_feat[b & 1];
-    // phase 1 (see the forward): decoded records of the relevant Gaussians, compacted in REVERSE list order; the
-    // fourth word of the second vector carries (Gaussian id << 5 | position in the batch)
-    bool relevant = false;
-    float4 c0 = make_float4(0.f, 0.f, 0.f, 0.f), c1 = c0;
-    if (lane < cnt) {
+    if (lane < nrel) {  // decode once per (region, Gaussian): region-local mean
       GaussReg g;
       decode_gauss(sf[3 * lane], sf[3 * lane + 1], ox, oy, g);
-      relevant = region_max_power(g, 7.f, 3.f) >= g.thr - 1e-3f;
-      c0 = make_float4(g.mx, g.my, g.A, g.B);
-      c1 = make_float4(g.C, g.o, g.thr, __uint_as_float((id_cur << 5) | (uint32_t)lane));
+      s_rel[3 * lane] = make_float4(g.mx, g.my, g.A, g.B);
+      s_rel[3 * lane + 1] = make_float4(g.C, g.o, g.thr, __uint_as_float(s_tag[b & 1][lane]));
+      s_rel[3 * lane + 2] = sf[3 * lane + 2];
+    } else if (lane < nrel + kGroup) {  // padding records never pass: p >= NaN is false
+      s_rel[3 * lane] = make_float4(0.f, 0.f, 0.f, 0.f);
+      s_rel[3 * lane + 1] = make_float4(0.f, 0.f, __int_as_float(0x7fc00000), 0.f);
     }
-    const unsigned rel = __ballot_sync(kFull, relevant);
-    const int nrel = __popc(rel);
-    if (relevant) {
-      const int r = nrel - 1 - __popc(rel & ((1u << lane) - 1u));
-      s_rel[3 * r] = c0; s_rel[3 * r + 1] = c1; s_rel[3 * r + 2] = sf[3 * lane + 2];
-    }
-    if (lane < kGroup) {  // padding records never pass: p >= NaN is false
-      s_rel[3 * (nrel + lane)] = make_float4(0.f, 0.f, 0.f, 0.f);
-      s_rel[3 * (nrel + lane) + 1] = make_float4(0.f, 0.f, __int_as_float(0x7fc00000), 0.f);
+    if (nrel + kGroup > kWarpBatch && lane < nrel + kGroup - kWarpBatch) {
+      const int r = kWarpBatch + lane;
+      s_rel[3 * r] = make_float4(0.f, 0.f, 0.f, 0.f);
+      s_rel[3 * r + 1] = make_float4(0.f, 0.f, __int_as_float(0x7fc00000), 0.f);
     }
     __syncwarp();
     for (int r0 = 0; r0 < nrel; r0 += kGroup) {  // back to front, four list entries at a time
