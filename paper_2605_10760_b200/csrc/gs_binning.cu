@@ -185,12 +185,28 @@ constexpr int kEmitT = 128;   // threads per CTA
 // concave power over the region rectangle, gs_raster.cuh), done ONCE per instance here: profiles/r1_v4 -- phase 1 was
 // 27 % of the forward's instructions and its staging of never-relevant records 2/3 of the cp.async traffic.
 __device__ __forceinline__ uint32_t region_mask(const float4& f0, const float4& f1, int tx, int ty) {
+  GaussReg g;  // decoded once, relative to the tile origin; the reciprocals are shared by the eight rectangles
+  decode_gauss(f0, f1, tx * GS_TILE, ty * GS_TILE, g);
+  const float nbc = -g.B * rcp_approx(2.f * g.C), nba = -g.B * rcp_approx(2.f * g.A);
+  const float thr = g.thr - 1e-3f;
   uint32_t m = 0;
 #pragma unroll
   for (int sub = 0; sub < 8; ++sub) {
-    GaussReg g;
-    decode_gauss(f0, f1, tx * GS_TILE + (sub % 2) * 8, ty * GS_TILE + (sub / 2) * 4, g);
-    m |= (region_max_power(g, 7.f, 3.f) >= g.thr - 1e-3f) ? (1u << sub) : 0u;
+    const float x0 = (float)((sub % 2) * 8) - g.mx, x1 = x0 + 7.f, y0 = (float)((sub / 2) * 4) - g.my, y1 = y0 + 3.f;
+    float best = 0.f;
+    if (!(x0 <= 0.f && x1 >= 0.f && y0 <= 0.f && y1 >= 0.f)) {
+      best = -INFINITY;
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        const float dxe = e ? x1 : x0;
+        const float dys = fminf(fmaxf(nbc * dxe, y0), y1);
+        best = fmaxf(best, g.A * dxe * dxe + g.B * dxe * dys + g.C * dys * dys);
+        const float dye = e ? y1 : y0;
+        const float dxs = fminf(fmaxf(nba * dye, x0), x1);
+        best = fmaxf(best, g.A * dxs * dxs + g.B * dxs * dye + g.C * dye * dye);
+      }
+    }
+    m |= (best >= thr) ? (1u << sub) : 0u;
   }
   return m;
 }
