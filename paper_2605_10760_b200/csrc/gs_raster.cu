@@ -195,9 +195,8 @@ raster_fwd84_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ orde
                     const uint32_t* __restrict__ ids, const float4* __restrict__ feat, float bg0, float bg1, float bg2,
                     float* __restrict__ rgb, float* __restrict__ depth, float* __restrict__ alpha_out,
                     float* __restrict__ final_T, uint32_t* __restrict__ n_contrib) {
-  __shared__ __align__(16) float4 s_feat[2][kWarpBatch * 3];          // raw records of the relevant entries (cp.async)
-  __shared__ uint32_t s_pos[2][kWarpBatch];                            // their list positions + 1
-  __shared__ __align__(16) float4 s_rel[(kWarpBatch + kGroup) * 3];    // decoded records
+  __shared__ __align__(16) float4 s_feat[2][(kWarpBatch + kGroup) * 3];  // records of the relevant entries (cp.async),
+  __shared__ uint32_t s_pos[2][kWarpBatch];                               // decoded in place; their list positions + 1
   const int lane = threadIdx.x;
   const int tile = (int)__ldg(order + blockIdx.x / 8), sub = blockIdx.x % 8;
   const int ox = (tile % tiles_x) * GS_TILE + (sub % 2) * 8, oy = (tile / tiles_x) * GS_TILE + (sub / 2) * 4;
@@ -246,30 +245,24 @@ raster_fwd84_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ orde
     }
     __syncwarp();
     if (nrel == 0) continue;
-    const float4* sf = s_feat[b & 1];
-    if (lane < nrel) {  // decode once per (region, Gaussian): region-local mean
+    float4* sf = s_feat[b & 1];
+    if (lane < nrel) {  // decode once per (region, Gaussian), in place: region-local mean
       GaussReg g;
       decode_gauss(sf[3 * lane], sf[3 * lane + 1], ox, oy, g);
-      s_rel[3 * lane] = make_float4(g.mx, g.my, g.A, g.B);
-      s_rel[3 * lane + 1] = make_float4(g.C, g.o, g.thr, __uint_as_float(s_pos[b & 1][lane]));
-      s_rel[3 * lane + 2] = sf[3 * lane + 2];
-    } else if (lane < nrel + kGroup) {  // padding records never pass: p >= NaN is false
-      s_rel[3 * lane] = make_float4(0.f, 0.f, 0.f, 0.f);
-      s_rel[3 * lane + 1] = make_float4(0.f, 0.f, __int_as_float(0x7fc00000), 0.f);
-      s_rel[3 * lane + 2] = make_float4(0.f, 0.f, 0.f, 0.f);
+      sf[3 * lane] = make_float4(g.mx, g.my, g.A, g.B);
+      sf[3 * lane + 1] = make_float4(g.C, g.o, g.thr, __uint_as_float(s_pos[b & 1][lane]));
     }
-    if (nrel + kGroup > kWarpBatch && lane < nrel + kGroup - kWarpBatch) {
-      const int r = kWarpBatch + lane;
-      s_rel[3 * r] = make_float4(0.f, 0.f, 0.f, 0.f);
-      s_rel[3 * r + 1] = make_float4(0.f, 0.f, __int_as_float(0x7fc00000), 0.f);
-      s_rel[3 * r + 2] = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (lane < kGroup) {  // padding records never pass: p >= NaN is false
+      sf[3 * (nrel + lane)] = make_float4(0.f, 0.f, 0.f, 0.f);
+      sf[3 * (nrel + lane) + 1] = make_float4(0.f, 0.f, __int_as_float(0x7fc00000), 0.f);
+      sf[3 * (nrel + lane) + 2] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
     __syncwarp();
     // phase 2: front to back, branch-free
     for (int r0 = 0; r0 < nrel; r0 += kGroup) {
 #pragma unroll
       for (int q = 0; q < kGroup; ++q) {
-        const float4 a0 = s_rel[3 * (r0 + q)], a1 = s_rel[3 * (r0 + q) + 1], f2 = s_rel[3 * (r0 + q) + 2];
+        const float4 a0 = sf[3 * (r0 + q)], a1 = sf[3 * (r0 + q) + 1], f2 = sf[3 * (r0 + q) + 2];
         float dx, dy;
         const float p = eval_power1(a0.x, a0.y, a0.z, a0.w, a1.x, fx0, fy0, dx, dy);
         const bool hit = (p >= a1.z) && (T >= GS_T_MIN);   // alpha >= 1/255 and the pixel has not terminated

@@ -97,8 +97,7 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
                   const float* __restrict__ d_rgb, const float* __restrict__ d_depth, const float* __restrict__ d_alpha,
                   float* __restrict__ g2d) {
   constexpr int RPT = 8;  // 8x4-pixel regions per 16x16 tile
-  __shared__ __align__(16) float4 s_feat[2][kWarpBatch * 3];
-  __shared__ __align__(16) float4 s_rel[(kWarpBatch + kGroup) * 3];
+  __shared__ __align__(16) float4 s_feat[2][(kWarpBatch + kGroup) * 3];  // records of the relevant entries, decoded in place
   __shared__ uint32_t s_tag[2][kWarpBatch];
   __shared__ __align__(16) float2 s_pair[kSlots * kPairRow];
   __shared__ __align__(16) float4 s_pix[32];
@@ -167,21 +166,16 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
     __syncwarp();
     if (nrel == 0) continue;
     const int lastb = (int)last - b * kWarpBatch;  // entries of this batch at positions < lastb were blended by this pixel
-    const float4* sf = s_feat[b & 1];
-    if (lane < nrel) {  // decode once per (region, Gaussian): region-local mean
+    float4* sf = s_feat[b & 1];
+    if (lane < nrel) {  // decode once per (region, Gaussian), in place: region-local mean
       GaussReg g;
       decode_gauss(sf[3 * lane], sf[3 * lane + 1], ox, oy, g);
-      s_rel[3 * lane] = make_float4(g.mx, g.my, g.A, g.B);
-      s_rel[3 * lane + 1] = make_float4(g.C, g.o, g.thr, __uint_as_float(s_tag[b & 1][lane]));
-      s_rel[3 * lane + 2] = sf[3 * lane + 2];
-    } else if (lane < nrel + kGroup) {  // padding records never pass: p >= NaN is false
-      s_rel[3 * lane] = make_float4(0.f, 0.f, 0.f, 0.f);
-      s_rel[3 * lane + 1] = make_float4(0.f, 0.f, __int_as_float(0x7fc00000), 0.f);
+      sf[3 * lane] = make_float4(g.mx, g.my, g.A, g.B);
+      sf[3 * lane + 1] = make_float4(g.C, g.o, g.thr, __uint_as_float(s_tag[b & 1][lane]));
     }
-    if (nrel + kGroup > kWarpBatch && lane < nrel + kGroup - kWarpBatch) {
-      const int r = kWarpBatch + lane;
-      s_rel[3 * r] = make_float4(0.f, 0.f, 0.f, 0.f);
-      s_rel[3 * r + 1] = make_float4(0.f, 0.f, __int_as_float(0x7fc00000), 0.f);
+    if (lane < kGroup) {  // padding records never pass: p >= NaN is false
+      sf[3 * (nrel + lane)] = make_float4(0.f, 0.f, 0.f, 0.f);
+      sf[3 * (nrel + lane) + 1] = make_float4(0.f, 0.f, __int_as_float(0x7fc00000), 0.f);
     }
     __syncwarp();
     for (int r0 = 0; r0 < nrel; r0 += kGroup) {  // back to front, four list entries at a time
@@ -191,7 +185,7 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
       unsigned m = 0;
 #pragma unroll
       for (int q = 0; q < kGroup; ++q) {
-        const float4 a0 = s_rel[3 * (r0 + q)], a1 = s_rel[3 * (r0 + q) + 1];
+        const float4 a0 = sf[3 * (r0 + q)], a1 = sf[3 * (r0 + q) + 1];
         g[q].mx = a0.x; g[q].my = a0.y; g[q].A = a0.z; g[q].B = a0.w;
         g[q].C = a1.x; g[q].o = a1.y; g[q].thr = a1.z;
         tag[q] = __float_as_uint(a1.w);
@@ -207,7 +201,7 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
         if (((any >> q) & 1u) == 0) continue;
         float gp = 0.f, w = 0.f;
         if (m & (1u << q)) {
-          const float4 f2 = s_rel[3 * (r0 + q) + 2];
+          const float4 f2 = sf[3 * (r0 + q) + 2];
           const float og = __fmul_rn(g[q].o, ex2_approx(p[q]));
           const float a = fminf(GS_ALPHA_MAX, og);
           const float ioma = rcp_approx(1.f - a);
