@@ -179,30 +179,27 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
     }
     __syncwarp();
     for (int r0 = 0; r0 < nrel; r0 += kGroup) {  // back to front, four list entries at a time
-      uint32_t tag[kGroup];
-      GaussReg g[kGroup];
+      float4 a0[kGroup], a1[kGroup];
       float p[kGroup];
-      unsigned m = 0;
+      bool hit[kGroup];
+      unsigned bal[kGroup];
 #pragma unroll
       for (int q = 0; q < kGroup; ++q) {
-        const float4 a0 = sf[3 * (r0 + q)], a1 = sf[3 * (r0 + q) + 1];
-        g[q].mx = a0.x; g[q].my = a0.y; g[q].A = a0.z; g[q].B = a0.w;
-        g[q].C = a1.x; g[q].o = a1.y; g[q].thr = a1.z;
-        tag[q] = __float_as_uint(a1.w);
-        float dx[1], dy[1], pp[1];
-        eval_power<1, 1>(g[q], fx0, fy0, dx, dy, pp);
-        p[q] = pp[0];
-        m |= (p[q] >= g[q].thr && (int)(tag[q] & 31u) < lastb) ? (1u << q) : 0u;
+        a0[q] = sf[3 * (r0 + q)];      // mx, my, A, B
+        a1[q] = sf[3 * (r0 + q) + 1];  // C, opacity, thr, tag
+        float dx, dy;
+        p[q] = eval_power1(a0[q].x, a0[q].y, a0[q].z, a0[q].w, a1[q].x, fx0, fy0, dx, dy);
+        // blended by the forward: alpha >= 1/255 and in front of the pixel's last contributor
+        hit[q] = p[q] >= a1[q].z && (int)(__float_as_uint(a1[q].w) & 31u) < lastb;
+        bal[q] = __ballot_sync(kFull, hit[q]);
       }
-      const unsigned any = __reduce_or_sync(kFull, m);
-      if (any == 0) continue;
 #pragma unroll
       for (int q = 0; q < kGroup; ++q) {
-        if (((any >> q) & 1u) == 0) continue;
+        if (bal[q] == 0) continue;  // the Gaussian reaches no pixel of the region
         float gp = 0.f, w = 0.f;
-        if (m & (1u << q)) {
+        if (hit[q]) {
           const float4 f2 = sf[3 * (r0 + q) + 2];
-          const float og = __fmul_rn(g[q].o, ex2_approx(p[q]));
+          const float og = __fmul_rn(a1[q].y, ex2_approx(p[q]));
           const float a = fminf(GS_ALPHA_MAX, og);
           const float ioma = rcp_approx(1.f - a);
           T *= ioma;  // transmittance in front of this Gaussian
@@ -215,7 +212,9 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
         }
         *pair_ptr = make_float2(gp, w);
         pair_ptr += kPairRow;
-        if ((lane & (kSlots - 1)) == nslot) { slot_mx = g[q].mx; slot_my = g[q].my; slot_id = tag[q] >> 5; }
+        if ((lane & (kSlots - 1)) == nslot) {
+          slot_mx = a0[q].x; slot_my = a0[q].y; slot_id = __float_as_uint(a1[q].w) >> 5;
+        }
         if (++nslot == kSlots) {
           gaussian_phase<2>(s_pair, s_pix, kSlots, lane, slot_mx, slot_my, slot_id, g2d);
           nslot = 0;
