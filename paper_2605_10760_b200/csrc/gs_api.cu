@@ -98,13 +98,30 @@ static int ensure_gaussian_capacity(gs_ctx* ctx, int64_t N) {
   return GS_OK;
 }
 
+// One allocation holds everything gs_preprocess must zero at the start of an iteration, so that it is ONE memset:
+// [Counts, 128 B][pose accumulators, 16 doubles][per-tile instance counters, one per 128-byte line].
+static int alloc_header(gs_ctx* ctx, int64_t tiles) {
+  if (ctx->hdr) cudaFree(ctx->hdr);
+  ctx->hdr = nullptr;
+  const size_t bytes = kHdrBytes + (size_t)tiles * kCtrStride * sizeof(uint32_t);
+  if (cudaMalloc((void**)&ctx->hdr, bytes) != cudaSuccess || cudaMemset(ctx->hdr, 0, bytes) != cudaSuccess) {
+    cudaGetLastError();
+    ctx->hdr = nullptr;
+    return fail(ctx, GS_E_NOMEM, "cudaMalloc failed while growing scratch");
+  }
+  ctx->counts = reinterpret_cast<Counts*>(ctx->hdr);
+  ctx->pose_acc = reinterpret_cast<double*>(ctx->hdr + 128);
+  ctx->tile_count = reinterpret_cast<uint32_t*>(ctx->hdr + kHdrBytes);
+  return GS_OK;
+}
+
 static int ensure_image_capacity(gs_ctx* ctx, int64_t tiles, int64_t pix) {
   int rc;
   if (tiles > ctx->cap_tiles) {
     GS_CUDA(cudaDeviceSynchronize());
     if ((rc = grow(ctx, ctx->ranges, tiles)) != GS_OK) return rc;
     if ((rc = grow(ctx, ctx->tile_order, tiles)) != GS_OK) return rc;
-    if ((rc = grow(ctx, ctx->tile_count, tiles * kCtrStride)) != GS_OK) return rc;
+    if ((rc = alloc_header(ctx, tiles)) != GS_OK) return rc;
     if ((rc = grow(ctx, ctx->tile_cursor, tiles * kCtrStride)) != GS_OK) return rc;
     ctx->cap_tiles = tiles;
   }
@@ -131,9 +148,7 @@ int gs_create(gs_ctx** out, int device) {
   ctx->device = device;
   if (const char* e = getenv("GS_RASTER_FWD")) ctx->shape_fwd = atoi(e);
   bool ok = cudaSetDevice(device) == cudaSuccess;
-  ok = ok && cudaMalloc((void**)&ctx->counts, sizeof(Counts)) == cudaSuccess;
-  ok = ok && cudaMemset(ctx->counts, 0, sizeof(Counts)) == cudaSuccess;
-  ok = ok && cudaMalloc((void**)&ctx->pose_acc, 16 * sizeof(double)) == cudaSuccess;
+  ok = ok && alloc_header(ctx, 0) == GS_OK;
   ok = ok && cudaHostAlloc((void**)&ctx->mailbox, sizeof(Counts), cudaHostAllocMapped) == cudaSuccess;
   ok = ok && cudaStreamCreateWithFlags(&ctx->side_stream, cudaStreamNonBlocking) == cudaSuccess;
   ok = ok && cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming) == cudaSuccess;
@@ -156,9 +171,9 @@ int gs_destroy(gs_ctx* ctx) {
   cudaFree(ctx->feat); cudaFree(ctx->rect); cudaFree(ctx->depth_key); cudaFree(ctx->tiles_touched); cudaFree(ctx->vis_ids); cudaFree(ctx->vis_rec);
   cudaFree(ctx->g2d);
   for (int b = 0; b < 2; ++b) { cudaFree(ctx->keys[b]); cudaFree(ctx->vals[b]); }
-  cudaFree(ctx->tile_count); cudaFree(ctx->tile_cursor); cudaFree(ctx->scan_ws);
+  cudaFree(ctx->hdr); cudaFree(ctx->tile_cursor); cudaFree(ctx->scan_ws);
   cudaFree(ctx->ranges); cudaFree(ctx->tile_order); cudaFree(ctx->final_T); cudaFree(ctx->n_contrib);
-  cudaFree(ctx->pose_acc); cudaFree(ctx->counts); cudaFree(ctx->hb);
+  cudaFree(ctx->hb);
   if (ctx->mailbox) cudaFreeHost(ctx->mailbox);
   if (ctx->side_stream) cudaStreamDestroy(ctx->side_stream);
   if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
@@ -204,8 +219,9 @@ int gs_preprocess(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, const flo
   ctx->means = means; ctx->scales = scales; ctx->quats = quats; ctx->opacities = opacities; ctx->sh = sh;
   ctx->seq++;
   GS_PROF(0, s);
-  GS_CUDA(cudaMemsetAsync(ctx->counts, 0, sizeof(Counts), s));
-  GS_CUDA(cudaMemsetAsync(ctx->tile_count, 0, (size_t)c.tiles_x * c.tiles_y * kCtrStride * sizeof(uint32_t), s));
+  // counters, pose accumulators and per-tile instance counters: one memset (alloc_header)
+  GS_CUDA(cudaMemsetAsync(ctx->hdr, 0, kHdrBytes + (size_t)c.tiles_x * c.tiles_y * kCtrStride * sizeof(uint32_t), s));
+  ctx->pose_acc_clean = true;
   if ((rc = launch_preprocess(ctx, s)) != GS_OK) return rc;
   GS_PROF(1, s);
   ctx->stage = 1;

@@ -243,7 +243,8 @@ __global__ void pose_final_kernel(DevCam cam, const double* __restrict__ pose_ac
 
 int launch_gauss_bwd(gs_ctx* ctx, cudaStream_t s, uint32_t flags, float* g_means, float* g_scales, float* g_quats,
                      float* g_opac, float* g_sh) {
-  GS_CUDA(cudaMemsetAsync(ctx->pose_acc, 0, 15 * sizeof(double), s));
+  if (!ctx->pose_acc_clean) GS_CUDA(cudaMemsetAsync(ctx->pose_acc, 0, 15 * sizeof(double), s));
+  ctx->pose_acc_clean = false;
   ctx->pose_acc_valid = true;
   ctx->g2d_dirty = false;
   if (ctx->N == 0) return GS_OK;

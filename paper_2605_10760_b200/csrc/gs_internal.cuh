@@ -46,6 +46,7 @@ constexpr int kFeatVec = 3;
 // with gp = alpha * dL/dalpha on unclamped contributions and w = alpha T.
 constexpr int kG2D = 12;
 
+constexpr int kHdrBytes = 256;  // Counts (128 B) + 16 pose accumulators, in front of the per-tile counters (gs_api.cu)
 constexpr int kCtrStride = 32;  // per-tile counters are one per 128-byte line (gs_binning.cu)
 
 // Device counters (one per context) + pinned-host mirror ("mailbox") the host may poll without synchronising.
@@ -111,6 +112,8 @@ struct gs_ctx {
   // pose-gradient accumulators: 15 doubles: sum g_pc (3), sum g_v (3), g_W (9)
   double* pose_acc = nullptr;
   bool pose_acc_valid = false;
+  bool pose_acc_clean = false;  // zeroed by gs_preprocess and not yet accumulated into
+  char* hdr = nullptr;          // one allocation: counts, pose_acc, tile_count (zeroed by one memset per iteration)
 
   gs::Counts* counts = nullptr;       // device
   gs::Counts* mailbox = nullptr;      // pinned host, mapped

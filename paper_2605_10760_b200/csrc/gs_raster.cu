@@ -345,6 +345,7 @@ int launch_workload_stats(gs_ctx* ctx, cudaStream_t s, uint64_t* out_host) {
   GS_CUDA(cudaMemcpyAsync(out_host, d, 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, s));
   GS_CUDA(cudaStreamSynchronize(s));
   ctx->pose_acc_valid = false;
+  ctx->pose_acc_clean = false;
   return GS_OK;
 }
 
