@@ -13,7 +13,8 @@ namespace gs {
 
 __global__ void features_export_kernel(int64_t N, const float4* __restrict__ feat, const ushort4* __restrict__ rect,
                                        const uint32_t* __restrict__ depth_key,
-                                       const uint32_t* __restrict__ tiles_touched, double* mean2d, float* conic,
+                                       const uint32_t* __restrict__ tiles_touched,
+                                       const uint32_t* __restrict__ slot_of, double* mean2d, float* conic,
                                        float* color, float* depth, uint32_t* dkey, int32_t* rect_out) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= N) return;
@@ -21,7 +22,10 @@ __global__ void features_export_kernel(int64_t N, const float4* __restrict__ fea
   float4 f0 = make_float4(0, 0, 0, 0), f1 = f0, f2 = f0;
   ushort4 r = make_ushort4(0, 0, 0, 0);
   uint32_t dk = 0;
-  if (vis) { f0 = feat[3 * i]; f1 = feat[3 * i + 1]; f2 = feat[3 * i + 2]; r = rect[i]; dk = depth_key[i]; }
+  if (vis) {
+    const size_t k = slot_of[i];  // the feature records are stored by visible slot
+    f0 = feat[3 * k]; f1 = feat[3 * k + 1]; f2 = feat[3 * k + 2]; r = rect[i]; dk = depth_key[i];
+  }
   const double ln2 = 0.6931471805599453;
   if (mean2d) {
     const int pk = __float_as_int(f0.z);
@@ -91,6 +95,8 @@ static int ensure_gaussian_capacity(gs_ctx* ctx, int64_t N) {
   if ((rc = grow(ctx, ctx->tiles_touched, cap + 4)) != GS_OK) return rc;
   if ((rc = grow(ctx, ctx->vis_ids, cap)) != GS_OK) return rc;
   if ((rc = grow(ctx, ctx->vis_rec, cap)) != GS_OK) return rc;
+  if ((rc = grow(ctx, ctx->vis_par, 3 * cap)) != GS_OK) return rc;
+  if ((rc = grow(ctx, ctx->slot_of, cap)) != GS_OK) return rc;
   if ((rc = grow(ctx, ctx->g2d, cap * kG2D)) != GS_OK) return rc;
   GS_CUDA(cudaMemset(ctx->g2d, 0, (size_t)cap * kG2D * sizeof(float)));
   ctx->g2d_dirty = false;
@@ -168,7 +174,7 @@ int gs_destroy(gs_ctx* ctx) {
   if (!ctx) return GS_E_INVALID;
   cudaSetDevice(ctx->device);
   cudaDeviceSynchronize();
-  cudaFree(ctx->feat); cudaFree(ctx->rect); cudaFree(ctx->depth_key); cudaFree(ctx->tiles_touched); cudaFree(ctx->vis_ids); cudaFree(ctx->vis_rec);
+  cudaFree(ctx->feat); cudaFree(ctx->rect); cudaFree(ctx->depth_key); cudaFree(ctx->tiles_touched); cudaFree(ctx->vis_ids); cudaFree(ctx->vis_rec); cudaFree(ctx->vis_par); cudaFree(ctx->slot_of);
   cudaFree(ctx->g2d);
   for (int b = 0; b < 2; ++b) { cudaFree(ctx->keys[b]); cudaFree(ctx->vals[b]); }
   cudaFree(ctx->hdr); cudaFree(ctx->tile_cursor); cudaFree(ctx->scan_ws);
@@ -348,7 +354,8 @@ int gs_get_features(gs_ctx* ctx, void* stream, double* mean2d, float* conic, flo
   GS_CUDA(cudaSetDevice(ctx->device));
   if (ctx->N == 0) return GS_OK;
   features_export_kernel<<<(unsigned)div_up(ctx->N, 256), 256, 0, (cudaStream_t)stream>>>(
-      ctx->N, ctx->feat, ctx->rect, ctx->depth_key, ctx->tiles_touched, mean2d, conic, color, depth, depth_key, rect);
+      ctx->N, ctx->feat, ctx->rect, ctx->depth_key, ctx->tiles_touched, ctx->slot_of, mean2d, conic, color, depth, depth_key,
+      rect);
   GS_LAUNCH_CHECK("features_export_kernel");
   return GS_OK;
 }

@@ -232,8 +232,8 @@ emit_kernel(const uint4* __restrict__ vis_rec, const float4* __restrict__ feat, 
     uint4 rec = make_uint4(0u, 0u, 0u, 0u);
     if (k < V) {
       rec = __ldg(vis_rec + k);
-      s_f0[tid] = __ldg(feat + 3 * (size_t)rec.w);
-      s_f1[tid] = __ldg(feat + 3 * (size_t)rec.w + 1);
+      s_f0[tid] = __ldg(feat + 3 * (size_t)k);  // the feature records are stored by visible slot
+      s_f1[tid] = __ldg(feat + 3 * (size_t)k + 1);
     }
     const uint32_t w = (rec.y & 0xffffu) - (rec.x & 0xffffu), h = (rec.y >> 16) - (rec.x >> 16);
     const uint32_t n = w * h;
@@ -372,8 +372,15 @@ __device__ __forceinline__ void smem_step(uint64_t (&k)[E], uint64_t* s, int tid
   __syncthreads();
 }
 
+// what the compositing kernels read: (visible slot << 8 | region mask) for a sorted key (.. | index << 8 | mask)
+__device__ __forceinline__ uint32_t list_entry(uint64_t key, const uint32_t* __restrict__ slot_of) {
+  const uint32_t lo = (uint32_t)key;
+  return (__ldg(slot_of + (lo >> 8)) << 8) | (lo & 0xffu);
+}
+
 template <int E, int NW>
-__device__ __forceinline__ void bucket_sort(uint64_t* __restrict__ g, uint32_t* __restrict__ ids, int n, uint64_t* s, int tid) {
+__device__ __forceinline__ void bucket_sort(uint64_t* __restrict__ g, uint32_t* __restrict__ ids, int n, uint64_t* s, int tid,
+                                            const uint32_t* __restrict__ slot_of) {
   constexpr int T = 32 * NW;
   uint64_t k[E];
 #pragma unroll
@@ -398,7 +405,7 @@ __device__ __forceinline__ void bucket_sort(uint64_t* __restrict__ g, uint32_t* 
 #pragma unroll
   for (int e = 0; e < E; ++e) {
     const int i = tid * E + e;
-    if (i < n) { g[i] = k[e]; ids[i] = (uint32_t)k[e]; }
+    if (i < n) { g[i] = k[e]; ids[i] = list_entry(k[e], slot_of); }
   }
 }
 
@@ -407,7 +414,8 @@ __device__ __forceinline__ void bucket_sort(uint64_t* __restrict__ g, uint32_t* 
 // scenes only).
 __global__ void __launch_bounds__(512)
 tile_sort_large_kernel(const uint32_t* __restrict__ order, const uint2* __restrict__ ranges,
-                       const Counts* __restrict__ counts, uint64_t* __restrict__ keys, uint32_t* __restrict__ ids) {
+                       const Counts* __restrict__ counts, uint64_t* __restrict__ keys, uint32_t* __restrict__ ids,
+                       const uint32_t* __restrict__ slot_of) {
   extern __shared__ uint64_t s_dyn[];
   const int tid = threadIdx.x, nth = blockDim.x;
   const int limit = (int)counts->n_large;
@@ -419,12 +427,12 @@ tile_sort_large_kernel(const uint32_t* __restrict__ order, const uint2* __restri
     uint64_t* g = keys + r.x;
     if (n > kLargeSort) {
       bitonic_sort(g, n, tid, nth);  // __syncthreads orders the CTA's own global writes
-      for (int t = tid; t < n; t += nth) ids[r.x + t] = (uint32_t)g[t];
+      for (int t = tid; t < n; t += nth) ids[r.x + t] = list_entry(g[t], slot_of);
       __syncthreads();
       continue;
     }
-    if (n <= 2048) bucket_sort<4, 16>(g, ids + r.x, n, s_dyn, tid);
-    else bucket_sort<16, 16>(g, ids + r.x, n, s_dyn, tid);
+    if (n <= 2048) bucket_sort<4, 16>(g, ids + r.x, n, s_dyn, tid, slot_of);
+    else bucket_sort<16, 16>(g, ids + r.x, n, s_dyn, tid, slot_of);
     __syncthreads();
   }
 }
@@ -434,7 +442,8 @@ tile_sort_large_kernel(const uint32_t* __restrict__ order, const uint2* __restri
 // each, four buckets per CTA, no barrier at all.
 __global__ void __launch_bounds__(128)
 tile_sort_kernel(int tiles, const uint32_t* __restrict__ order, const uint2* __restrict__ ranges,
-                 const Counts* __restrict__ counts, uint64_t* __restrict__ keys, uint32_t* __restrict__ ids) {
+                 const Counts* __restrict__ counts, uint64_t* __restrict__ keys, uint32_t* __restrict__ ids,
+                 const uint32_t* __restrict__ slot_of) {
   __shared__ uint64_t s_x[1024];
   const int tid = threadIdx.x;
   const int n_mid = (int)counts->n_mid;
@@ -442,7 +451,7 @@ tile_sort_kernel(int tiles, const uint32_t* __restrict__ order, const uint2* __r
     const uint2 r = ranges[order[blockIdx.x]];
     const int n = (int)(r.y - r.x);
     if (n > kMidSortMax) return;
-    bucket_sort<8, 4>(keys + r.x, ids + r.x, n, s_x, tid);
+    bucket_sort<8, 4>(keys + r.x, ids + r.x, n, s_x, tid, slot_of);
     return;
   }
   const int idx = n_mid + ((int)blockIdx.x - n_mid) * 4 + (tid >> 5);
@@ -450,8 +459,8 @@ tile_sort_kernel(int tiles, const uint32_t* __restrict__ order, const uint2* __r
   const uint2 r = ranges[order[idx]];
   const int n = (int)(r.y - r.x), lane = tid & 31;
   if (n == 0) return;
-  if (n <= 64) bucket_sort<2, 1>(keys + r.x, ids + r.x, n, nullptr, lane);
-  else bucket_sort<8, 1>(keys + r.x, ids + r.x, n, nullptr, lane);
+  if (n <= 64) bucket_sort<2, 1>(keys + r.x, ids + r.x, n, nullptr, lane, slot_of);
+  else bucket_sort<8, 1>(keys + r.x, ids + r.x, n, nullptr, lane, slot_of);
 }
 
 // export for gs_get_binning: keys_sorted[k] = tile << 32 | depth bits
@@ -463,14 +472,15 @@ __global__ void export_keys_kernel(int tiles, const uint2* __restrict__ ranges, 
   for (uint32_t k = r.x + threadIdx.x; k < r.y; k += blockDim.x) out[k] = ((uint64_t)tile << 32) | (keys[k] >> 32);
 }
 
-__global__ void export_ids_kernel(int64_t I, const uint32_t* __restrict__ vals, uint32_t* __restrict__ out) {
+__global__ void export_ids_kernel(int64_t I, const uint32_t* __restrict__ vals, const uint32_t* __restrict__ vis_ids,
+                                  uint32_t* __restrict__ out) {
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (k < I) out[k] = vals[k] >> 8;  // strip the region mask
+  if (k < I) out[k] = vis_ids[vals[k] >> 8];  // strip the region mask, visible slot -> Gaussian index
 }
 
 int export_sorted_ids(gs_ctx* ctx, cudaStream_t s, int64_t I, uint32_t* out) {
   if (I <= 0) return GS_OK;
-  export_ids_kernel<<<(unsigned)div_up(I, 256), 256, 0, s>>>(I, ctx->vals[ctx->sorted_buf], out);
+  export_ids_kernel<<<(unsigned)div_up(I, 256), 256, 0, s>>>(I, ctx->vals[ctx->sorted_buf], ctx->vis_ids, out);
   GS_LAUNCH_CHECK("export_ids_kernel");
   return GS_OK;
 }
@@ -576,10 +586,11 @@ int launch_binning(gs_ctx* ctx, cudaStream_t s) {
       GS_CUDA(cudaStreamWaitEvent(sl, ctx->ev_fork2, 0));
     }
     tile_sort_large_kernel<<<min(tiles, 296), 512, kLargeSort * sizeof(uint64_t), sl>>>(ctx->tile_order, ctx->ranges, ctx->counts,
-                                                                                        ctx->keys[0], ctx->vals[0]);
+                                                                                        ctx->keys[0], ctx->vals[0], ctx->slot_of);
     GS_LAUNCH_CHECK("tile_sort_large_kernel");
     if (fork) GS_CUDA(cudaEventRecord(ctx->ev_join2, sl));
-    tile_sort_kernel<<<tiles, 128, 0, s>>>(tiles, ctx->tile_order, ctx->ranges, ctx->counts, ctx->keys[0], ctx->vals[0]);
+    tile_sort_kernel<<<tiles, 128, 0, s>>>(tiles, ctx->tile_order, ctx->ranges, ctx->counts, ctx->keys[0], ctx->vals[0],
+                                           ctx->slot_of);
     GS_LAUNCH_CHECK("tile_sort_kernel");
     if (fork) GS_CUDA(cudaStreamWaitEvent(s, ctx->ev_join2, 0));
   }

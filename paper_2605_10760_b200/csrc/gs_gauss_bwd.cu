@@ -23,7 +23,8 @@ template <int DEG, bool WRITE>
 __global__ void __launch_bounds__(128)
 gauss_bwd_kernel(int64_t N, const float* __restrict__ means, const float* __restrict__ scales,
                  const float* __restrict__ quats, const float* __restrict__ opacities, const float* __restrict__ sh,
-                 DevCam cam, const uint32_t* __restrict__ vis_ids, const Counts* __restrict__ counts,
+                 DevCam cam, const uint32_t* __restrict__ vis_ids, const float4* __restrict__ vis_par,
+                 const Counts* __restrict__ counts,
                  float* __restrict__ g2d, bool accumulate,
                  float* __restrict__ g_means, float* __restrict__ g_scales, float* __restrict__ g_quats,
                  float* __restrict__ g_opac, float* __restrict__ g_sh, double* __restrict__ pose_acc) {
@@ -41,14 +42,15 @@ gauss_bwd_kernel(int64_t N, const float* __restrict__ means, const float* __rest
 #pragma unroll
   for (int k = 0; k < 15; ++k) acc[k] = (R)0;
   if (vis) {
-    float4* gp4 = reinterpret_cast<float4*>(g2d + (size_t)i * kG2D);
+    // g2d and the parameter copies are stored by visible slot (= this thread's index): sequential streams; only the SH
+    // record and the dense gradient outputs are addressed by the Gaussian index
+    float4* gp4 = reinterpret_cast<float4*>(g2d + (size_t)kk * kG2D);
     const float4 ga = gp4[0], gb = gp4[1], gc = gp4[2];
     const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
     gp4[0] = zero; gp4[1] = zero; gp4[2] = zero;  // keep the accumulator all-zero for the next iteration
-    const float mu0 = means[3 * i], mu1 = means[3 * i + 1], mu2 = means[3 * i + 2];
-    const float s0 = scales[3 * i], s1 = scales[3 * i + 1], s2 = scales[3 * i + 2];
-    const float4 q = *reinterpret_cast<const float4*>(quats + 4 * i);
-    const float o = opacities[i];
+    const float4 pa = __ldg(vis_par + 3 * (size_t)kk), pb = __ldg(vis_par + 3 * (size_t)kk + 1), q = __ldg(vis_par + 3 * (size_t)kk + 2);
+    const float mu0 = pa.x, mu1 = pa.y, mu2 = pa.z, o = pa.w;
+    const float s0 = pb.x, s1 = pb.y, s2 = pb.z;
     Proj<R> P;
     project_gaussian<R>(cam, T, mu0, mu1, mu2, s0, s1, s2, q.x, q.y, q.z, q.w, o, P);
     const R W[9] = {T[0], T[1], T[2], T[4], T[5], T[6], T[8], T[9], T[10]};
@@ -259,7 +261,7 @@ int launch_gauss_bwd(gs_ctx* ctx, cudaStream_t s, uint32_t flags, float* g_means
   const unsigned blocks = (unsigned)div_up(ctx->N, threads);
 #define GS_GB(D, Wr)                                                                                                 \
   gauss_bwd_kernel<D, Wr><<<blocks, threads, 0, s>>>(ctx->N, ctx->means, ctx->scales, ctx->quats, ctx->opacities,   \
-                                                      ctx->sh, ctx->cam, ctx->vis_ids, ctx->counts, ctx->g2d, accum, \
+                                                      ctx->sh, ctx->cam, ctx->vis_ids, ctx->vis_par, ctx->counts, ctx->g2d, accum, \
                                                       g_means, g_scales, g_quats, g_opac, g_sh, ctx->pose_acc)
   if (write) {
     switch (ctx->sh_degree) {

@@ -80,13 +80,15 @@ struct gs_ctx {
 
   // per-Gaussian scratch (capacity cap_N)
   int64_t cap_N = 0;
-  float4* feat = nullptr;           // [N,3]
+  float4* feat = nullptr;           // [N,3], indexed by VISIBLE SLOT
   ushort4* rect = nullptr;          // [N] tile rect tx0,ty0,tx1,ty1
   uint32_t* depth_key = nullptr;    // [N]
   uint32_t* tiles_touched = nullptr;  // [N]
   uint32_t* vis_ids = nullptr;        // [N] indices of the visible Gaussians, compacted (arbitrary order)
   uint4* vis_rec = nullptr;           // [N] same order: {tx0 | ty0 << 16, tx1 | ty1 << 16, depth key, index}
-  float* g2d = nullptr;             // [N,12]; kept all-zero between iterations (the consumer clears what it reads)
+  float4* vis_par = nullptr;          // [N,3] same order: {mu, opacity} {scale, -} {quat}: what gauss_bwd needs again
+  uint32_t* slot_of = nullptr;        // [N] visible slot of Gaussian i (valid where tiles_touched[i] > 0)
+  float* g2d = nullptr;             // [N,12], indexed by visible slot; kept all-zero between iterations (the consumer clears what it reads)
   bool g2d_dirty = false;
 
   // per-instance scratch (capacity cap_I)

@@ -12,13 +12,15 @@ preprocess_kernel(int64_t N, const float* __restrict__ means, const float* __res
                   const float* __restrict__ quats, const float* __restrict__ opacities, const float* __restrict__ sh,
                   DevCam cam, float4* __restrict__ feat, ushort4* __restrict__ rect, uint32_t* __restrict__ depth_key,
                   uint32_t* __restrict__ tiles_touched, uint32_t* __restrict__ tile_count,
-                  uint32_t* __restrict__ vis_ids, uint4* __restrict__ vis_rec, Counts* __restrict__ counts) {
+                  uint32_t* __restrict__ vis_ids, uint4* __restrict__ vis_rec, float4* __restrict__ vis_par,
+                  uint32_t* __restrict__ slot_of, Counts* __restrict__ counts) {
   constexpr int K = (DEG + 1) * (DEG + 1);
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   float T[12];
   load_pose(cam, T);
   bool vis = false;
   uint4 rec = make_uint4(0u, 0u, 0u, 0u);  // what the duplication needs: packed tile rect, depth key, index
+  float4 f0 = make_float4(0.f, 0.f, 0.f, 0.f), f1 = f0, f2 = f0, p0 = f0, p1 = f0, p2 = f0;
   if (i < N) {
     const float mu0 = means[3 * i], mu1 = means[3 * i + 1], mu2 = means[3 * i + 2];
     const float o = opacities[i];
@@ -64,14 +66,16 @@ preprocess_kernel(int64_t N, const float* __restrict__ means, const float* __res
       const double rmx = fmin(fmax(rint(P.mx), -32000.0), 32000.0);
       const double rmy = fmin(fmax(rint(P.my), -32000.0), 32000.0);
       const double kl = 1.4426950408889634;  // log2(e)
-      float4 f0, f1, f2;
       f0.x = (float)(P.mx - rmx); f0.y = (float)(P.my - rmy);
       f0.z = __int_as_float(((int)rmy << 16) | ((int)rmx & 0xffff));
       f0.w = (float)(-log2(255.0 * (double)o));  // alpha >= 1/255  <=>  power2 >= thr
       f1.x = (float)(-0.5 * kl * P.a); f1.y = (float)(-kl * P.b); f1.z = (float)(-0.5 * kl * P.c); f1.w = o;
       f2.x = fmaxf(col[0] + 0.5f, 0.f); f2.y = fmaxf(col[1] + 0.5f, 0.f); f2.z = fmaxf(col[2] + 0.5f, 0.f);
       f2.w = (float)P.z;
-      feat[3 * i] = f0; feat[3 * i + 1] = f1; feat[3 * i + 2] = f2;
+      // the parameters the per-Gaussian backward needs again, kept with the features in VISIBLE-SLOT order (below)
+      p0 = make_float4(mu0, mu1, mu2, o);
+      p1 = make_float4(scales[3 * i], scales[3 * i + 1], scales[3 * i + 2], 0.f);
+      p2 = q;
       rect[i] = make_ushort4((unsigned short)tx0, (unsigned short)ty0, (unsigned short)tx1, (unsigned short)ty1);
       const uint32_t dk = __float_as_uint(depth_key_f32(T, mu0, mu1, mu2));
       depth_key[i] = dk;
@@ -92,8 +96,14 @@ preprocess_kernel(int64_t N, const float* __restrict__ means, const float* __res
     base = __shfl_sync(0xffffffffu, base, 0);
     if (vis) {
       const uint32_t slot = base + __popc(ball & ((1u << lane) - 1));
+      // everything downstream is indexed by the visible slot: the feature records, the parameter copies and the 2-D
+      // gradient accumulators of the visible Gaussians are dense arrays (sequential for the per-Gaussian kernels, a
+      // third of the footprint for the gathers of the compositing kernels)
       vis_ids[slot] = (uint32_t)i;
+      slot_of[i] = slot;
       vis_rec[slot] = rec;
+      feat[3 * (size_t)slot] = f0; feat[3 * (size_t)slot + 1] = f1; feat[3 * (size_t)slot + 2] = f2;
+      vis_par[3 * (size_t)slot] = p0; vis_par[3 * (size_t)slot + 1] = p1; vis_par[3 * (size_t)slot + 2] = p2;
     }
   }
 }
@@ -106,7 +116,7 @@ int launch_preprocess(gs_ctx* ctx, cudaStream_t s) {
 #define GS_PRE(D)                                                                                                    \
   preprocess_kernel<D><<<blocks, threads, 0, s>>>(N, ctx->means, ctx->scales, ctx->quats, ctx->opacities, ctx->sh,  \
                                                    ctx->cam, ctx->feat, ctx->rect, ctx->depth_key,                  \
-                                                   ctx->tiles_touched, ctx->tile_count, ctx->vis_ids, ctx->vis_rec, ctx->counts)
+                                                   ctx->tiles_touched, ctx->tile_count, ctx->vis_ids, ctx->vis_rec, ctx->vis_par, ctx->slot_of, ctx->counts)
   switch (ctx->sh_degree) {
     case 0: GS_PRE(0); break;
     case 1: GS_PRE(1); break;
