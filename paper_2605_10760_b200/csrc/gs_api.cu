@@ -11,8 +11,7 @@ using namespace gs;
 
 namespace gs {
 
-__global__ void features_export_kernel(int64_t N, const float4* __restrict__ feat, const ushort4* __restrict__ rect,
-                                       const uint32_t* __restrict__ depth_key,
+__global__ void features_export_kernel(int64_t N, const float4* __restrict__ feat, const uint4* __restrict__ vis_rec,
                                        const uint32_t* __restrict__ tiles_touched,
                                        const uint32_t* __restrict__ slot_of, double* mean2d, float* conic,
                                        float* color, float* depth, uint32_t* dkey, int32_t* rect_out) {
@@ -24,7 +23,11 @@ __global__ void features_export_kernel(int64_t N, const float4* __restrict__ fea
   uint32_t dk = 0;
   if (vis) {
     const size_t k = slot_of[i];  // the feature records are stored by visible slot
-    f0 = feat[3 * k]; f1 = feat[3 * k + 1]; f2 = feat[3 * k + 2]; r = rect[i]; dk = depth_key[i];
+    f0 = feat[3 * k]; f1 = feat[3 * k + 1]; f2 = feat[3 * k + 2];
+    const uint4 rec = vis_rec[k];  // {tx0 | ty0 << 16, tx1 | ty1 << 16, depth key, index}
+    r = make_ushort4((unsigned short)(rec.x & 0xffffu), (unsigned short)(rec.x >> 16), (unsigned short)(rec.y & 0xffffu),
+                     (unsigned short)(rec.y >> 16));
+    dk = rec.z;
   }
   const double ln2 = 0.6931471805599453;
   if (mean2d) {
@@ -90,8 +93,6 @@ static int ensure_gaussian_capacity(gs_ctx* ctx, int64_t N) {
   const int64_t cap = N + N / 8 + 1024;
   int rc;
   if ((rc = grow(ctx, ctx->feat, 3 * cap)) != GS_OK) return rc;
-  if ((rc = grow(ctx, ctx->rect, cap)) != GS_OK) return rc;
-  if ((rc = grow(ctx, ctx->depth_key, cap)) != GS_OK) return rc;
   if ((rc = grow(ctx, ctx->tiles_touched, cap + 4)) != GS_OK) return rc;
   if ((rc = grow(ctx, ctx->vis_ids, cap)) != GS_OK) return rc;
   if ((rc = grow(ctx, ctx->vis_rec, cap)) != GS_OK) return rc;
@@ -174,7 +175,7 @@ int gs_destroy(gs_ctx* ctx) {
   if (!ctx) return GS_E_INVALID;
   cudaSetDevice(ctx->device);
   cudaDeviceSynchronize();
-  cudaFree(ctx->feat); cudaFree(ctx->rect); cudaFree(ctx->depth_key); cudaFree(ctx->tiles_touched); cudaFree(ctx->vis_ids); cudaFree(ctx->vis_rec); cudaFree(ctx->vis_par); cudaFree(ctx->slot_of);
+  cudaFree(ctx->feat); cudaFree(ctx->tiles_touched); cudaFree(ctx->vis_ids); cudaFree(ctx->vis_rec); cudaFree(ctx->vis_par); cudaFree(ctx->slot_of);
   cudaFree(ctx->g2d);
   for (int b = 0; b < 2; ++b) { cudaFree(ctx->keys[b]); cudaFree(ctx->vals[b]); }
   cudaFree(ctx->hdr); cudaFree(ctx->tile_cursor); cudaFree(ctx->scan_ws);
@@ -354,7 +355,7 @@ int gs_get_features(gs_ctx* ctx, void* stream, double* mean2d, float* conic, flo
   GS_CUDA(cudaSetDevice(ctx->device));
   if (ctx->N == 0) return GS_OK;
   features_export_kernel<<<(unsigned)div_up(ctx->N, 256), 256, 0, (cudaStream_t)stream>>>(
-      ctx->N, ctx->feat, ctx->rect, ctx->depth_key, ctx->tiles_touched, ctx->slot_of, mean2d, conic, color, depth, depth_key,
+      ctx->N, ctx->feat, ctx->vis_rec, ctx->tiles_touched, ctx->slot_of, mean2d, conic, color, depth, depth_key,
       rect);
   GS_LAUNCH_CHECK("features_export_kernel");
   return GS_OK;

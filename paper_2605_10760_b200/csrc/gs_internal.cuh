@@ -81,8 +81,6 @@ struct gs_ctx {
   // per-Gaussian scratch (capacity cap_N)
   int64_t cap_N = 0;
   float4* feat = nullptr;           // [N,3], indexed by VISIBLE SLOT
-  ushort4* rect = nullptr;          // [N] tile rect tx0,ty0,tx1,ty1
-  uint32_t* depth_key = nullptr;    // [N]
   uint32_t* tiles_touched = nullptr;  // [N]
   uint32_t* vis_ids = nullptr;        // [N] indices of the visible Gaussians, compacted (arbitrary order)
   uint4* vis_rec = nullptr;           // [N] same order: {tx0 | ty0 << 16, tx1 | ty1 << 16, depth key, index}

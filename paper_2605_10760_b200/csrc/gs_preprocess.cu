@@ -10,7 +10,7 @@ template <int DEG>
 __global__ void __launch_bounds__(256)
 preprocess_kernel(int64_t N, const float* __restrict__ means, const float* __restrict__ scales,
                   const float* __restrict__ quats, const float* __restrict__ opacities, const float* __restrict__ sh,
-                  DevCam cam, float4* __restrict__ feat, ushort4* __restrict__ rect, uint32_t* __restrict__ depth_key,
+                  DevCam cam, float4* __restrict__ feat,
                   uint32_t* __restrict__ tiles_touched, uint32_t* __restrict__ tile_count,
                   uint32_t* __restrict__ vis_ids, uint4* __restrict__ vis_rec, float4* __restrict__ vis_par,
                   uint32_t* __restrict__ slot_of, Counts* __restrict__ counts) {
@@ -76,9 +76,7 @@ preprocess_kernel(int64_t N, const float* __restrict__ means, const float* __res
       p0 = make_float4(mu0, mu1, mu2, o);
       p1 = make_float4(scales[3 * i], scales[3 * i + 1], scales[3 * i + 2], 0.f);
       p2 = q;
-      rect[i] = make_ushort4((unsigned short)tx0, (unsigned short)ty0, (unsigned short)tx1, (unsigned short)ty1);
       const uint32_t dk = __float_as_uint(depth_key_f32(T, mu0, mu1, mu2));
-      depth_key[i] = dk;
       rec = make_uint4((uint32_t)tx0 | ((uint32_t)ty0 << 16), (uint32_t)tx1 | ((uint32_t)ty1 << 16), dk, (uint32_t)i);
       tiles_touched[i] = (uint32_t)((tx1 - tx0) * (ty1 - ty0));
       for (int ty = ty0; ty < ty1; ++ty)  // MSD digit histogram of the binning sort (gs_binning.cu)
@@ -115,7 +113,7 @@ int launch_preprocess(gs_ctx* ctx, cudaStream_t s) {
   const unsigned blocks = (unsigned)div_up(N, threads);
 #define GS_PRE(D)                                                                                                    \
   preprocess_kernel<D><<<blocks, threads, 0, s>>>(N, ctx->means, ctx->scales, ctx->quats, ctx->opacities, ctx->sh,  \
-                                                   ctx->cam, ctx->feat, ctx->rect, ctx->depth_key,                  \
+                                                   ctx->cam, ctx->feat,                  \
                                                    ctx->tiles_touched, ctx->tile_count, ctx->vis_ids, ctx->vis_rec, ctx->vis_par, ctx->slot_of, ctx->counts)
   switch (ctx->sh_degree) {
     case 0: GS_PRE(0); break;
