@@ -13,97 +13,95 @@ preprocess_kernel(int64_t N, const float* __restrict__ means, const float* __res
                   DevCam cam, float4* __restrict__ feat,
                   uint32_t* __restrict__ tiles_touched, uint32_t* __restrict__ tile_count,
                   uint32_t* __restrict__ vis_ids, uint4* __restrict__ vis_rec, float4* __restrict__ vis_par,
-                  uint32_t* __restrict__ slot_of, Counts* __restrict__ counts) {
+                  uint32_t* __restrict__ slot_of, float* __restrict__ vis_sh, Counts* __restrict__ counts) {
   constexpr int K = (DEG + 1) * (DEG + 1);
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   float T[12];
   load_pose(cam, T);
   bool vis = false;
-  uint4 rec = make_uint4(0u, 0u, 0u, 0u);  // what the duplication needs: packed tile rect, depth key, index
-  float4 f0 = make_float4(0.f, 0.f, 0.f, 0.f), f1 = f0, f2 = f0, p0 = f0, p1 = f0, p2 = f0;
+  float mu0 = 0.f, mu1 = 0.f, mu2 = 0.f, o = 0.f, sc0 = 0.f, sc1 = 0.f, sc2 = 0.f;
+  float4 q = make_float4(0.f, 0.f, 0.f, 0.f);
+  ProjD P;
+  int tx0 = 0, ty0 = 0, tx1 = 0, ty1 = 0;
   if (i < N) {
-    const float mu0 = means[3 * i], mu1 = means[3 * i + 1], mu2 = means[3 * i + 2];
-    const float o = opacities[i];
-    ProjD P;
-    const float4 q = *reinterpret_cast<const float4*>(quats + 4 * i);
-    vis = project_gaussian<double>(cam, T, mu0, mu1, mu2, scales[3 * i], scales[3 * i + 1], scales[3 * i + 2], q.x, q.y, q.z,
-                           q.w, o, P);
-    int tx0 = 0, ty0 = 0, tx1 = 0, ty1 = 0;
+    mu0 = means[3 * i]; mu1 = means[3 * i + 1]; mu2 = means[3 * i + 2];
+    sc0 = scales[3 * i]; sc1 = scales[3 * i + 1]; sc2 = scales[3 * i + 2];
+    o = opacities[i];
+    q = *reinterpret_cast<const float4*>(quats + 4 * i);
+    vis = project_gaussian<double>(cam, T, mu0, mu1, mu2, sc0, sc1, sc2, q.x, q.y, q.z, q.w, o, P);
     if (vis) vis = tile_rect(cam, P, o, tx0, ty0, tx1, ty1);
-    if (vis) {
-      // view direction mu - c_cam, c_cam = -W^T t
-      const double ccx = -((double)T[0] * T[3] + (double)T[4] * T[7] + (double)T[8] * T[11]);
-      const double ccy = -((double)T[1] * T[3] + (double)T[5] * T[7] + (double)T[9] * T[11]);
-      const double ccz = -((double)T[2] * T[3] + (double)T[6] * T[7] + (double)T[10] * T[11]);
-      const double vx = (double)mu0 - ccx, vy = (double)mu1 - ccy, vz = (double)mu2 - ccz;
-      const double ivn = rsqrt(vx * vx + vy * vy + vz * vz);
-      float B[K];
-      sh_basis<DEG>((float)(vx * ivn), (float)(vy * ivn), (float)(vz * ivn), B);
-      const float* c = sh + (int64_t)3 * K * i;
-      float col[3] = {0.f, 0.f, 0.f};
-      if constexpr ((3 * K) % 4 == 0) {
-        float buf[3 * K];
-#pragma unroll
-        for (int v = 0; v < 3 * K / 4; ++v) {
-          const float4 t = __ldg(reinterpret_cast<const float4*>(c) + v);
-          buf[4 * v] = t.x; buf[4 * v + 1] = t.y; buf[4 * v + 2] = t.z; buf[4 * v + 3] = t.w;
-        }
-#pragma unroll
-        for (int k = 0; k < K; ++k) {
-          col[0] = fmaf(B[k], buf[3 * k], col[0]);
-          col[1] = fmaf(B[k], buf[3 * k + 1], col[1]);
-          col[2] = fmaf(B[k], buf[3 * k + 2], col[2]);
-        }
-      } else {
-#pragma unroll
-        for (int k = 0; k < K; ++k) {
-          col[0] = fmaf(B[k], __ldg(c + 3 * k), col[0]);
-          col[1] = fmaf(B[k], __ldg(c + 3 * k + 1), col[1]);
-          col[2] = fmaf(B[k], __ldg(c + 3 * k + 2), col[2]);
-        }
-      }
-      // mean = integer pixel (two int16, clamped: a centre that far off-screen needs no sub-pixel precision) + fraction
-      const double rmx = fmin(fmax(rint(P.mx), -32000.0), 32000.0);
-      const double rmy = fmin(fmax(rint(P.my), -32000.0), 32000.0);
-      const double kl = 1.4426950408889634;  // log2(e)
-      f0.x = (float)(P.mx - rmx); f0.y = (float)(P.my - rmy);
-      f0.z = __int_as_float(((int)rmy << 16) | ((int)rmx & 0xffff));
-      f0.w = (float)(-log2(255.0 * (double)o));  // alpha >= 1/255  <=>  power2 >= thr
-      f1.x = (float)(-0.5 * kl * P.a); f1.y = (float)(-kl * P.b); f1.z = (float)(-0.5 * kl * P.c); f1.w = o;
-      f2.x = fmaxf(col[0] + 0.5f, 0.f); f2.y = fmaxf(col[1] + 0.5f, 0.f); f2.z = fmaxf(col[2] + 0.5f, 0.f);
-      f2.w = (float)P.z;
-      // the parameters the per-Gaussian backward needs again, kept with the features in VISIBLE-SLOT order (below)
-      p0 = make_float4(mu0, mu1, mu2, o);
-      p1 = make_float4(scales[3 * i], scales[3 * i + 1], scales[3 * i + 2], 0.f);
-      p2 = q;
-      const uint32_t dk = __float_as_uint(depth_key_f32(T, mu0, mu1, mu2));
-      rec = make_uint4((uint32_t)tx0 | ((uint32_t)ty0 << 16), (uint32_t)tx1 | ((uint32_t)ty1 << 16), dk, (uint32_t)i);
-      tiles_touched[i] = (uint32_t)((tx1 - tx0) * (ty1 - ty0));
-      for (int ty = ty0; ty < ty1; ++ty)  // MSD digit histogram of the binning sort (gs_binning.cu)
-        for (int tx = tx0; tx < tx1; ++tx) atomicAdd(&tile_count[(size_t)(ty * cam.tiles_x + tx) * kCtrStride], 1u);
-    } else {
-      tiles_touched[i] = 0u;
-    }
+    tiles_touched[i] = vis ? (uint32_t)((tx1 - tx0) * (ty1 - ty0)) : 0u;
   }
-  // compacted list of visible Gaussians (arbitrary order): the per-Gaussian kernels downstream run on it
+  // Compacted list of visible Gaussians (arbitrary order).  Everything downstream is indexed by the visible slot: the
+  // feature records, the parameter / SH copies and the 2-D gradient accumulators of the visible Gaussians are dense
+  // arrays -- sequential streams for the per-Gaussian kernels (their scattered 64-byte DRAM bursts, ~9 per Gaussian,
+  // were what bounded them) and a third of the footprint for the gathers of the compositing kernels.
   const unsigned ball = __ballot_sync(0xffffffffu, vis);
-  if (ball) {
-    const int lane = threadIdx.x & 31;
-    uint32_t base = 0;
-    if (lane == 0) base = atomicAdd(&counts->n_visible, (uint32_t)__popc(ball));
-    base = __shfl_sync(0xffffffffu, base, 0);
-    if (vis) {
-      const uint32_t slot = base + __popc(ball & ((1u << lane) - 1));
-      // everything downstream is indexed by the visible slot: the feature records, the parameter copies and the 2-D
-      // gradient accumulators of the visible Gaussians are dense arrays (sequential for the per-Gaussian kernels, a
-      // third of the footprint for the gathers of the compositing kernels)
-      vis_ids[slot] = (uint32_t)i;
-      slot_of[i] = slot;
-      vis_rec[slot] = rec;
-      feat[3 * (size_t)slot] = f0; feat[3 * (size_t)slot + 1] = f1; feat[3 * (size_t)slot + 2] = f2;
-      vis_par[3 * (size_t)slot] = p0; vis_par[3 * (size_t)slot + 1] = p1; vis_par[3 * (size_t)slot + 2] = p2;
+  if (ball == 0) return;
+  const int lane = threadIdx.x & 31;
+  uint32_t base = 0;
+  if (lane == 0) base = atomicAdd(&counts->n_visible, (uint32_t)__popc(ball));
+  base = __shfl_sync(0xffffffffu, base, 0);
+  if (!vis) return;
+  const size_t slot = base + __popc(ball & ((1u << lane) - 1));
+  // view direction mu - c_cam, c_cam = -W^T t
+  const double ccx = -((double)T[0] * T[3] + (double)T[4] * T[7] + (double)T[8] * T[11]);
+  const double ccy = -((double)T[1] * T[3] + (double)T[5] * T[7] + (double)T[9] * T[11]);
+  const double ccz = -((double)T[2] * T[3] + (double)T[6] * T[7] + (double)T[10] * T[11]);
+  const double vx = (double)mu0 - ccx, vy = (double)mu1 - ccy, vz = (double)mu2 - ccz;
+  const double ivn = rsqrt(vx * vx + vy * vy + vz * vz);
+  float B[K];
+  sh_basis<DEG>((float)(vx * ivn), (float)(vy * ivn), (float)(vz * ivn), B);
+  const float* c = sh + (int64_t)3 * K * i;
+  float* cs = vis_sh + slot * (3 * K);  // slot-ordered copy of the coefficients for the per-Gaussian backward
+  float col[3] = {0.f, 0.f, 0.f};
+  if constexpr ((3 * K) % 4 == 0) {
+    float buf[3 * K];
+#pragma unroll
+    for (int v = 0; v < 3 * K / 4; ++v) {
+      const float4 t = __ldg(reinterpret_cast<const float4*>(c) + v);
+      reinterpret_cast<float4*>(cs)[v] = t;
+      buf[4 * v] = t.x; buf[4 * v + 1] = t.y; buf[4 * v + 2] = t.z; buf[4 * v + 3] = t.w;
+    }
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+      col[0] = fmaf(B[k], buf[3 * k], col[0]);
+      col[1] = fmaf(B[k], buf[3 * k + 1], col[1]);
+      col[2] = fmaf(B[k], buf[3 * k + 2], col[2]);
+    }
+  } else {
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+      const float c0 = __ldg(c + 3 * k), c1 = __ldg(c + 3 * k + 1), c2 = __ldg(c + 3 * k + 2);
+      cs[3 * k] = c0; cs[3 * k + 1] = c1; cs[3 * k + 2] = c2;
+      col[0] = fmaf(B[k], c0, col[0]);
+      col[1] = fmaf(B[k], c1, col[1]);
+      col[2] = fmaf(B[k], c2, col[2]);
     }
   }
+  // mean = integer pixel (two int16, clamped: a centre that far off-screen needs no sub-pixel precision) + fraction
+  const double rmx = fmin(fmax(rint(P.mx), -32000.0), 32000.0);
+  const double rmy = fmin(fmax(rint(P.my), -32000.0), 32000.0);
+  const double kl = 1.4426950408889634;  // log2(e)
+  float4 f0, f1, f2;
+  f0.x = (float)(P.mx - rmx); f0.y = (float)(P.my - rmy);
+  f0.z = __int_as_float(((int)rmy << 16) | ((int)rmx & 0xffff));
+  f0.w = (float)(-log2(255.0 * (double)o));  // alpha >= 1/255  <=>  power2 >= thr
+  f1.x = (float)(-0.5 * kl * P.a); f1.y = (float)(-kl * P.b); f1.z = (float)(-0.5 * kl * P.c); f1.w = o;
+  f2.x = fmaxf(col[0] + 0.5f, 0.f); f2.y = fmaxf(col[1] + 0.5f, 0.f); f2.z = fmaxf(col[2] + 0.5f, 0.f);
+  f2.w = (float)P.z;
+  const uint32_t dk = __float_as_uint(depth_key_f32(T, mu0, mu1, mu2));
+  vis_ids[slot] = (uint32_t)i;
+  slot_of[i] = (uint32_t)slot;
+  // what the duplication needs: packed tile rect, depth key, index
+  vis_rec[slot] = make_uint4((uint32_t)tx0 | ((uint32_t)ty0 << 16), (uint32_t)tx1 | ((uint32_t)ty1 << 16), dk, (uint32_t)i);
+  feat[3 * slot] = f0; feat[3 * slot + 1] = f1; feat[3 * slot + 2] = f2;
+  // the parameters the per-Gaussian backward needs again
+  vis_par[3 * slot] = make_float4(mu0, mu1, mu2, o);
+  vis_par[3 * slot + 1] = make_float4(sc0, sc1, sc2, 0.f);
+  vis_par[3 * slot + 2] = q;
+  for (int ty = ty0; ty < ty1; ++ty)  // MSD digit histogram of the binning sort (gs_binning.cu)
+    for (int tx = tx0; tx < tx1; ++tx) atomicAdd(&tile_count[(size_t)(ty * cam.tiles_x + tx) * kCtrStride], 1u);
 }
 
 int launch_preprocess(gs_ctx* ctx, cudaStream_t s) {
@@ -114,7 +112,7 @@ int launch_preprocess(gs_ctx* ctx, cudaStream_t s) {
 #define GS_PRE(D)                                                                                                    \
   preprocess_kernel<D><<<blocks, threads, 0, s>>>(N, ctx->means, ctx->scales, ctx->quats, ctx->opacities, ctx->sh,  \
                                                    ctx->cam, ctx->feat,                  \
-                                                   ctx->tiles_touched, ctx->tile_count, ctx->vis_ids, ctx->vis_rec, ctx->vis_par, ctx->slot_of, ctx->counts)
+                                                   ctx->tiles_touched, ctx->tile_count, ctx->vis_ids, ctx->vis_rec, ctx->vis_par, ctx->slot_of, ctx->vis_sh, ctx->counts)
   switch (ctx->sh_degree) {
     case 0: GS_PRE(0); break;
     case 1: GS_PRE(1); break;
