@@ -338,6 +338,77 @@ def run_ours(args):
         print(json.dumps(line))
 
 
+def run_extra(args):
+    """Configs 4 (tracking, pose only) and 5 (fused refinement, 8 views accumulated): device-resident throughput and
+    stage times only (the headline line with roofline / e2e / cpu_baseline is the default workload's)."""
+    import torch
+    from paper_2605_10760_b200 import binding as B
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    ctx = B.Context(0)
+    if args.workload == "tracking500k":
+        # BASELINE.json configs[3]: 500k Gaussians frozen, L1 RGB against a render from the perturbed pose; per step:
+        # preprocess (pose read from the device) -> bin -> fwd -> L1 gradient -> bwd (pose only) -> pose gradient ->
+        # on-device normalised pose step; no host synchronisation inside the loop
+        sc = scenes.replica_scene(seed=40, N=500_000)
+        W, H = sc.camera.width, sc.camera.height
+        ds = B.DeviceScene(sc, 0)
+        out = ds.alloc_outputs(W, H)
+        cam_t = sc.camera.copy()
+        cam_t.T_cw = scenes.perturb_pose(sc.camera.T_cw, scenes.tracking_perturbation(40))
+        B.forward(ctx, ds, cam_t, out)
+        torch.cuda.synchronize(); ctx.gs_poll()
+        target = out["rgb"].clone()
+        T_dev = torch.from_numpy(np.ascontiguousarray(sc.camera.T_cw, np.float32).reshape(-1)).to(dev)
+        gC = torch.empty_like(out["rgb"])
+
+        def step(k):
+            B.forward(ctx, ds, sc.camera, out, T_cw_dev=T_dev)
+            B.gs_aux_l1_grad(out["rgb"], target, 1.0 / (3 * W * H), gC)
+            B.backward(ctx, out, gC, None, None, flags=B.GS_POSE_ONLY, pose=True)
+            B.gs_aux_pose_step(T_dev, out["g_twist"], 1e-3)
+        views, label = 1, "tracking500k: BASELINE.json configs[3], 500000 Gaussians, 1200x680, SH3, pose-only, seed 40"
+    else:
+        # BASELINE.json configs[4]: 2M Gaussians (4 Sim(3)-mapped submaps), 8 views per iteration, gradients accumulated
+        sc, cams = scenes.fused_scene(seed=50)
+        W, H = cams[0].width, cams[0].height
+        ds = B.DeviceScene(sc, 0)
+        out = ds.alloc_outputs(W, H)
+        ups = [tuple(torch.from_numpy(a).to(dev) for a in scenes.upstream_gradients(50 + v, W, H)) for v in range(len(cams))]
+
+        def step(k):
+            for v, cam in enumerate(cams):
+                B.forward(ctx, ds, cam, out)
+                B.backward(ctx, out, ups[v][0], ups[v][1], None, flags=(B.GS_ACCUMULATE if v > 0 else 0), pose=False)
+        views, label = len(cams), "fused2m: BASELINE.json configs[4], 2000000 Gaussians, 8 views of 1200x680, SH3, seed 50"
+    k = 0
+    while k < max(args.warmup, 3):
+        try:
+            step(k); torch.cuda.synchronize(); ctx.gs_poll(); k += 1
+        except B.GsError as e:
+            if e.code != -5:
+                raise
+    K = args.steps
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(0) as clk:
+        torch.cuda.synchronize()
+        e0.record()
+        for k in range(K):
+            step(k)
+        e1.record()
+        torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    ctx.gs_poll()
+    nv, ni = ctx.gs_get_counts()
+    value = K / (ms / 1e3)
+    print(json.dumps({"metric": "fwd+bwd rasterize iters/sec", "value": value, "unit": "iter/s", "n_gpus": 1, "steps": K,
+                      "warmup": max(args.warmup, 3), "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak",
+                      "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": {"workload": label},
+                      "views_per_iter": views, "mpix_iter_per_s": value * views * W * H / 1e6, "clocks": clk.summary(),
+                      "last_view": {"visible": nv, "instances": ni}}))
+    ctx.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -349,6 +420,8 @@ def main():
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.workload in ("tracking500k", "fused2m"):
+        run_extra(args)
     else:
         run_ours(args)
 
