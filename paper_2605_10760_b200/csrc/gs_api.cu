@@ -98,7 +98,6 @@ static int ensure_gaussian_capacity(gs_ctx* ctx, int64_t N) {
   if ((rc = grow(ctx, ctx->vis_rec, cap)) != GS_OK) return rc;
   if ((rc = grow(ctx, ctx->vis_par, 3 * cap)) != GS_OK) return rc;
   if ((rc = grow(ctx, ctx->slot_of, cap)) != GS_OK) return rc;
-  if ((rc = grow(ctx, ctx->vis_sh, 48 * cap)) != GS_OK) return rc;
   if ((rc = grow(ctx, ctx->g2d, cap * kG2D)) != GS_OK) return rc;
   GS_CUDA(cudaMemset(ctx->g2d, 0, (size_t)cap * kG2D * sizeof(float)));
   ctx->g2d_dirty = false;
@@ -176,7 +175,7 @@ int gs_destroy(gs_ctx* ctx) {
   if (!ctx) return GS_E_INVALID;
   cudaSetDevice(ctx->device);
   cudaDeviceSynchronize();
-  cudaFree(ctx->feat); cudaFree(ctx->tiles_touched); cudaFree(ctx->vis_ids); cudaFree(ctx->vis_rec); cudaFree(ctx->vis_par); cudaFree(ctx->slot_of); cudaFree(ctx->vis_sh);
+  cudaFree(ctx->feat); cudaFree(ctx->tiles_touched); cudaFree(ctx->vis_ids); cudaFree(ctx->vis_rec); cudaFree(ctx->vis_par); cudaFree(ctx->slot_of);
   cudaFree(ctx->g2d);
   for (int b = 0; b < 2; ++b) { cudaFree(ctx->keys[b]); cudaFree(ctx->vals[b]); }
   cudaFree(ctx->hdr); cudaFree(ctx->tile_cursor); cudaFree(ctx->scan_ws);

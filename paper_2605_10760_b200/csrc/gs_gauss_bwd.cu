@@ -24,7 +24,7 @@ __global__ void __launch_bounds__(128)
 gauss_bwd_kernel(int64_t N, const float* __restrict__ means, const float* __restrict__ scales,
                  const float* __restrict__ quats, const float* __restrict__ opacities, const float* __restrict__ sh,
                  DevCam cam, const uint32_t* __restrict__ vis_ids, const float4* __restrict__ vis_par,
-                 const float* __restrict__ vis_sh, const Counts* __restrict__ counts,
+                 const Counts* __restrict__ counts,
                  float* __restrict__ g2d, bool accumulate,
                  float* __restrict__ g_means, float* __restrict__ g_scales, float* __restrict__ g_quats,
                  float* __restrict__ g_opac, float* __restrict__ g_sh, double* __restrict__ pose_acc) {
@@ -126,7 +126,7 @@ gauss_bwd_kernel(int64_t N, const float* __restrict__ means, const float* __rest
     const float nx = (float)(vx * ivn), ny = (float)(vy * ivn), nz = (float)(vz * ivn);
     float B[K];
     sh_basis<DEG>(nx, ny, nz, B);
-    const float* cf = vis_sh + (size_t)kk * (3 * K);  // slot-ordered copy written by gs_preprocess
+    const float* cf = sh + (int64_t)3 * K * i;
     float col[3] = {0.f, 0.f, 0.f};
     float shv[3 * K];
     if constexpr ((3 * K) % 4 == 0) {
@@ -261,7 +261,7 @@ int launch_gauss_bwd(gs_ctx* ctx, cudaStream_t s, uint32_t flags, float* g_means
   const unsigned blocks = (unsigned)div_up(ctx->N, threads);
 #define GS_GB(D, Wr)                                                                                                 \
   gauss_bwd_kernel<D, Wr><<<blocks, threads, 0, s>>>(ctx->N, ctx->means, ctx->scales, ctx->quats, ctx->opacities,   \
-                                                      ctx->sh, ctx->cam, ctx->vis_ids, ctx->vis_par, ctx->vis_sh, ctx->counts, ctx->g2d, accum, \
+                                                      ctx->sh, ctx->cam, ctx->vis_ids, ctx->vis_par, ctx->counts, ctx->g2d, accum, \
                                                       g_means, g_scales, g_quats, g_opac, g_sh, ctx->pose_acc)
   if (write) {
     switch (ctx->sh_degree) {

@@ -85,7 +85,6 @@ struct gs_ctx {
   uint32_t* vis_ids = nullptr;        // [N] indices of the visible Gaussians, compacted (arbitrary order)
   uint4* vis_rec = nullptr;           // [N] same order: {tx0 | ty0 << 16, tx1 | ty1 << 16, depth key, index}
   float4* vis_par = nullptr;          // [N,3] same order: {mu, opacity} {scale, -} {quat}: what gauss_bwd needs again
-  float* vis_sh = nullptr;            // [N,48] same order: the SH coefficients of the visible Gaussians (3K floats used)
   uint32_t* slot_of = nullptr;        // [N] visible slot of Gaussian i (valid where tiles_touched[i] > 0)
   float* g2d = nullptr;             // [N,12], indexed by visible slot; kept all-zero between iterations (the consumer clears what it reads)
   bool g2d_dirty = false;

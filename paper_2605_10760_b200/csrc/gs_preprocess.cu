@@ -13,7 +13,7 @@ preprocess_kernel(int64_t N, const float* __restrict__ means, const float* __res
                   DevCam cam, float4* __restrict__ feat,
                   uint32_t* __restrict__ tiles_touched, uint32_t* __restrict__ tile_count,
                   uint32_t* __restrict__ vis_ids, uint4* __restrict__ vis_rec, float4* __restrict__ vis_par,
-                  uint32_t* __restrict__ slot_of, float* __restrict__ vis_sh, Counts* __restrict__ counts) {
+                  uint32_t* __restrict__ slot_of, Counts* __restrict__ counts) {
   constexpr int K = (DEG + 1) * (DEG + 1);
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   float T[12];
@@ -33,7 +33,7 @@ preprocess_kernel(int64_t N, const float* __restrict__ means, const float* __res
     tiles_touched[i] = vis ? (uint32_t)((tx1 - tx0) * (ty1 - ty0)) : 0u;
   }
   // Compacted list of visible Gaussians (arbitrary order).  Everything downstream is indexed by the visible slot: the
-  // feature records, the parameter / SH copies and the 2-D gradient accumulators of the visible Gaussians are dense
+  // feature records, the parameter copies and the 2-D gradient accumulators of the visible Gaussians are dense
   // arrays -- sequential streams for the per-Gaussian kernels (their scattered 64-byte DRAM bursts, ~9 per Gaussian,
   // were what bounded them) and a third of the footprint for the gathers of the compositing kernels.
   const unsigned ball = __ballot_sync(0xffffffffu, vis);
@@ -53,14 +53,12 @@ preprocess_kernel(int64_t N, const float* __restrict__ means, const float* __res
   float B[K];
   sh_basis<DEG>((float)(vx * ivn), (float)(vy * ivn), (float)(vz * ivn), B);
   const float* c = sh + (int64_t)3 * K * i;
-  float* cs = vis_sh + slot * (3 * K);  // slot-ordered copy of the coefficients for the per-Gaussian backward
   float col[3] = {0.f, 0.f, 0.f};
   if constexpr ((3 * K) % 4 == 0) {
     float buf[3 * K];
 #pragma unroll
     for (int v = 0; v < 3 * K / 4; ++v) {
       const float4 t = __ldg(reinterpret_cast<const float4*>(c) + v);
-      reinterpret_cast<float4*>(cs)[v] = t;
       buf[4 * v] = t.x; buf[4 * v + 1] = t.y; buf[4 * v + 2] = t.z; buf[4 * v + 3] = t.w;
     }
 #pragma unroll
@@ -73,7 +71,6 @@ preprocess_kernel(int64_t N, const float* __restrict__ means, const float* __res
 #pragma unroll
     for (int k = 0; k < K; ++k) {
       const float c0 = __ldg(c + 3 * k), c1 = __ldg(c + 3 * k + 1), c2 = __ldg(c + 3 * k + 2);
-      cs[3 * k] = c0; cs[3 * k + 1] = c1; cs[3 * k + 2] = c2;
       col[0] = fmaf(B[k], c0, col[0]);
       col[1] = fmaf(B[k], c1, col[1]);
       col[2] = fmaf(B[k], c2, col[2]);
@@ -112,7 +109,7 @@ int launch_preprocess(gs_ctx* ctx, cudaStream_t s) {
 #define GS_PRE(D)                                                                                                    \
   preprocess_kernel<D><<<blocks, threads, 0, s>>>(N, ctx->means, ctx->scales, ctx->quats, ctx->opacities, ctx->sh,  \
                                                    ctx->cam, ctx->feat,                  \
-                                                   ctx->tiles_touched, ctx->tile_count, ctx->vis_ids, ctx->vis_rec, ctx->vis_par, ctx->slot_of, ctx->vis_sh, ctx->counts)
+                                                   ctx->tiles_touched, ctx->tile_count, ctx->vis_ids, ctx->vis_rec, ctx->vis_par, ctx->slot_of, ctx->counts)
   switch (ctx->sh_degree) {
     case 0: GS_PRE(0); break;
     case 1: GS_PRE(1); break;
