@@ -49,9 +49,9 @@ preprocess_kernel(int64_t N, const float* __restrict__ means, const float* __res
   const double ccy = -((double)T[1] * T[3] + (double)T[5] * T[7] + (double)T[9] * T[11]);
   const double ccz = -((double)T[2] * T[3] + (double)T[6] * T[7] + (double)T[10] * T[11]);
   const double vx = (double)mu0 - ccx, vy = (double)mu1 - ccy, vz = (double)mu2 - ccz;
-  const double ivn = rsqrt(vx * vx + vy * vy + vz * vz);
+  const float ivn = rsqrtf((float)(vx * vx + vy * vy + vz * vz));
   float B[K];
-  sh_basis<DEG>((float)(vx * ivn), (float)(vy * ivn), (float)(vz * ivn), B);
+  sh_basis<DEG>((float)vx * ivn, (float)vy * ivn, (float)vz * ivn, B);
   const float* c = sh + (int64_t)3 * K * i;
   float col[3] = {0.f, 0.f, 0.f};
   if constexpr ((3 * K) % 4 == 0) {
@@ -83,7 +83,7 @@ preprocess_kernel(int64_t N, const float* __restrict__ means, const float* __res
   float4 f0, f1, f2;
   f0.x = (float)(P.mx - rmx); f0.y = (float)(P.my - rmy);
   f0.z = __int_as_float(((int)rmy << 16) | ((int)rmx & 0xffff));
-  f0.w = (float)(-log2(255.0 * (double)o));  // alpha >= 1/255  <=>  power2 >= thr
+  f0.w = -log2f(255.f * o);  // alpha >= 1/255  <=>  power2 >= thr
   f1.x = (float)(-0.5 * kl * P.a); f1.y = (float)(-kl * P.b); f1.z = (float)(-0.5 * kl * P.c); f1.w = o;
   f2.x = fmaxf(col[0] + 0.5f, 0.f); f2.y = fmaxf(col[1] + 0.5f, 0.f); f2.z = fmaxf(col[2] + 0.5f, 0.f);
   f2.w = (float)P.z;

@@ -92,12 +92,15 @@ __device__ __forceinline__ bool project_gaussian(const DevCam& cam, const float*
 // (the rendered result is then independent of binning; Q5).  Returns false if no pixel is covered.
 __device__ __forceinline__ bool tile_rect(const DevCam& cam, const ProjD& P, float opacity, int& tx0, int& ty0,
                                           int& tx1, int& ty1) {
-  const double rho = sqrt(2.0 * log(255.0 * (double)opacity));
-  const double hx = rho * sqrt(P.cxx) * (1.0 + 0.0009765625) + 0.0078125;
-  const double hy = rho * sqrt(P.cyy) * (1.0 + 0.0009765625) + 0.0078125;
-  const double Wd = cam.W, Hd = cam.H;
-  const double x0 = fmax(0.0, ceil(P.mx - hx)), x1 = fmin(Wd, floor(P.mx + hx) + 1.0);
-  const double y0 = fmax(0.0, ceil(P.my - hy)), y1 = fmin(Hd, floor(P.my + hy) + 1.0);
+  // fp32 is enough here: its rounding (1e-7 relative, < 1e-4 px) is far inside the outward padding, and the fp64 log and
+  // square roots were a third of the instructions of a visible thread
+  const float rho = sqrtf(2.f * logf(255.f * opacity));
+  const float hx = rho * sqrtf((float)P.cxx) * (1.f + 0.0009765625f) + 0.0078125f;
+  const float hy = rho * sqrtf((float)P.cyy) * (1.f + 0.0009765625f) + 0.0078125f;
+  const float mx = (float)P.mx, my = (float)P.my;
+  const float Wd = (float)cam.W, Hd = (float)cam.H;
+  const float x0 = fmaxf(0.f, ceilf(mx - hx)), x1 = fminf(Wd, floorf(mx + hx) + 1.f);
+  const float y0 = fmaxf(0.f, ceilf(my - hy)), y1 = fminf(Hd, floorf(my + hy) + 1.f);
   if (!(x1 > x0) || !(y1 > y0)) return false;
   const int ix0 = (int)x0, ix1 = (int)x1, iy0 = (int)y0, iy1 = (int)y1;
   tx0 = ix0 / GS_TILE; ty0 = iy0 / GS_TILE;
