@@ -18,7 +18,7 @@
 namespace gs {
 
 constexpr int kSmallSortMax = 255;  // buckets up to this size are sorted by one warp (whole length/8 classes of the tile order)
-constexpr int kMidSortMax = 1023;   // buckets up to this size are sorted by one CTA of 4 warps; beyond: the large kernel
+constexpr int kMidSortMax = 2047;   // buckets up to this size are sorted by one CTA of 4 warps; beyond: the large kernel
 constexpr int kLargeSort = 8192;
 // tile_count / tile_cursor are strided by 32 words: one counter per 128-byte line, so that the atomics of different
 // tiles are served by different L2 lines (3225 adjacent counters would share ~100 lines and serialise there)   // up to this size: 512-thread CTA, 64 KB dynamic shared memory; beyond: global memory
@@ -39,13 +39,13 @@ constexpr int kScanCls = 16;
 constexpr int kScanAgg = 1 + kScanCls;
 constexpr int kScanMaxCta = 128;
 
-// length class, longest first: 0: >= 1024, then half-octave steps 768, 512, 384, 256, ..., 12, 8; 15: < 8.
-// Class 0 holds exactly the tiles beyond kMidSortMax, classes 0..4 those beyond kSmallSortMax.
+// length class, longest first: 0: >= 2048, then half-octave steps 1536, 1024, 768, 512, ..., 24, 16; 15: < 16.
+// Class 0 holds exactly the tiles beyond kMidSortMax, classes 0..6 those beyond kSmallSortMax.
 __device__ __forceinline__ int length_class(uint32_t c) {
-  if (c < 8u) return 15;
+  if (c < 16u) return 15;
   const int e = 31 - __clz((int)c);
   const int q = 2 * e + (int)((c >> (e - 1)) & 1u);
-  return max(20 - q, 0);
+  return max(22 - q, 0);
 }
 
 struct ScanVec { uint32_t w[kScanWords]; };
@@ -138,7 +138,7 @@ tile_scan_kernel(int tiles, const uint32_t* __restrict__ tile_count, uint32_t* _
       s_base[k] = bb + s_pre[1 + k];
       bb += s_tot[1 + k];
       if (k == 0) nl = bb;
-      if (k == 4) nm = bb;
+      if (k == 6) nm = bb;
     }
     if (b == 0) {
       counts->n_instances = I;
@@ -409,7 +409,7 @@ __device__ __forceinline__ void bucket_sort(uint64_t* __restrict__ g, uint32_t* 
   }
 }
 
-// Buckets of 1024 .. kLargeSort keys (the first n_large entries of `order`): one CTA of 512 threads per bucket, 16 keys
+// Buckets of 2048 .. kLargeSort keys (the first n_large entries of `order`): one CTA of 512 threads per bucket, 16 keys
 // per thread; beyond kLargeSort the shared-memory-free network above runs in place in global memory (slow; degenerate
 // scenes only).
 __global__ void __launch_bounds__(512)
@@ -431,27 +431,27 @@ tile_sort_large_kernel(const uint32_t* __restrict__ order, const uint2* __restri
       __syncthreads();
       continue;
     }
-    if (n <= 2048) bucket_sort<4, 16>(g, ids + r.x, n, s_dyn, tid, slot_of);
-    else bucket_sort<16, 16>(g, ids + r.x, n, s_dyn, tid, slot_of);
+    bucket_sort<16, 16>(g, ids + r.x, n, s_dyn, tid, slot_of);
     __syncthreads();
   }
 }
 
-// Buckets up to kMidSortMax keys.  CTAs of 4 warps: the first n_mid entries of `order` (256 .. 1023 keys; those of the
+// Buckets up to kMidSortMax keys.  CTAs of 4 warps: the first n_mid entries of `order` (256 .. 2047 keys; those of the
 // large kernel are skipped) take a whole CTA each, 8 keys per thread; the remaining buckets (< 256 keys) take one warp
 // each, four buckets per CTA, no barrier at all.
 __global__ void __launch_bounds__(128)
 tile_sort_kernel(int tiles, const uint32_t* __restrict__ order, const uint2* __restrict__ ranges,
                  const Counts* __restrict__ counts, uint64_t* __restrict__ keys, uint32_t* __restrict__ ids,
                  const uint32_t* __restrict__ slot_of) {
-  __shared__ uint64_t s_x[1024];
+  __shared__ uint64_t s_x[2048];
   const int tid = threadIdx.x;
   const int n_mid = (int)counts->n_mid;
   if ((int)blockIdx.x < n_mid) {
     const uint2 r = ranges[order[blockIdx.x]];
     const int n = (int)(r.y - r.x);
     if (n > kMidSortMax) return;
-    bucket_sort<8, 4>(keys + r.x, ids + r.x, n, s_x, tid, slot_of);
+    if (n <= 1024) bucket_sort<8, 4>(keys + r.x, ids + r.x, n, s_x, tid, slot_of);
+    else bucket_sort<16, 4>(keys + r.x, ids + r.x, n, s_x, tid, slot_of);
     return;
   }
   const int idx = n_mid + ((int)blockIdx.x - n_mid) * 4 + (tid >> 5);
