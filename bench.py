@@ -38,6 +38,9 @@ SM_COUNT, FP32_LANES, SM_MAX_MHZ = 148, 128, 1965.0
 #       4 colour/depth products (4), clamp test (1), gp (1), 2 mean terms (2 fma + 2 mul + 2 mul = 8), 3 conic terms (6),
 #       = 37; the reduction of the 10 sums over the pixels of the tile is 10 adds per blended pair = 10  -> 47
 FLOP_EVAL, FLOP_BLEND_FWD, FLOP_BLEND_BWD = 12.0, 12.0, 47.0
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the compositing kernels, from the `ncu --set full` capture
+# summarised in profiles/r1_v5_masks.md (scene seed 32); null for the other kernels
+NCU_DRAM_BYTES = {"raster_bwd": 42.19e6 + 0.18e6, "raster_fwd": 14.66e6 + 0.11e6}
 
 
 def load_peaks():
@@ -259,7 +262,8 @@ def run_ours(args):
         roof = {"kernel": dominant, "bound": "hbm", "achieved": by / (stage_ms[dominant] * 1e-3) / 1e9,
                 "peak": hbm_peak, "unit": "GB/s"}
     roof["frac"] = roof["achieved"] / roof["peak"]
-    roof["traffic"] = None
+    roof["traffic"] = NCU_DRAM_BYTES.get(dominant)
+    roof["traffic_unit"] = "bytes of DRAM traffic per launch (ncu, profiles/r1_v5_masks.md)"
     roof["peak_source"] = peak_src if roof["bound"] == "hbm" else \
         f"derived: {SM_COUNT} SMs x {FP32_LANES} FP32 lanes x 2 x {SM_MAX_MHZ:.0f} MHz (DESIGN.md)"
     roof["stage_share"] = stage_ms[dominant] / sum(stage_ms.values())
