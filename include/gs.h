@@ -155,6 +155,22 @@ GS_API int gs_aux_l1_grad(void* stream, int64_t n, const float* pred, const floa
 /* T_cw <- Exp(-step * g / |g|) T_cw on the device (normalised gradient step; no-op if |g| = 0).  T_cw_dev float[12]. */
 GS_API int gs_aux_pose_step(void* stream, float* T_cw_dev, const float* g_twist, float step);
 
+/* ---- mapping-loss terms of Eq. 4 that need no dataset ---------------------------------------- */
+/* alpha L1(I^, I) + beta L1(D^, D) (paper: alpha = 0.95, beta = 0.25).  Reading (Q18): L1(I^, I) = mean over the
+ * 3 H W values of |I^ - I|; L1(D^, D) = (1 / H W) sum over pixels with target_depth > 0 of |D^ - D|; sign(0) = 0.
+ * Inputs: DEVICE float rgb, target_rgb [3,H,W]; depth, target_depth [H,W].  Outputs: DEVICE d_rgb [3,H,W] =
+ * alpha sign(I^ - I) / (3 H W), d_depth [H,W] = beta sign(D^ - D) / (H W) (0 where target_depth <= 0) -- directly the
+ * upstream gradients of gs_rasterize_bwd -- and DEVICE double loss[4] = { L1 rgb, L1 depth, alpha L1 rgb + beta L1 depth,
+ * scratch }.
+ * Asynchronous on `stream`; all arrays caller-owned.  GS_E_INVALID on a null pointer or an empty image. */
+GS_API int gs_loss_map(void* stream, int32_t width, int32_t height, const float* rgb, const float* depth,
+                       const float* target_rgb, const float* target_depth, float alpha, float beta, float* d_rgb,
+                       float* d_depth, double* loss);
+/* lambda_s L_iso = lambda_s sum_i |s_i - mean(s_i)|_1 over the three (activated) scale components (paper: lambda_s =
+ * 10).  DEVICE scales [N,3]; its gradient is ADDED into DEVICE g_scales [N,3] (call after gs_rasterize_bwd);
+ * DEVICE double loss[2]: loss[0] = the weighted loss (loss[1] is scratch). */
+GS_API int gs_loss_iso(void* stream, int64_t N, const float* scales, float lambda_s, float* g_scales, double* loss);
+
 /* ---- host-buffer convenience (bench.py "e2e"): one whole fwd+bwd iteration with HOST arrays -------------------- */
 /* Copies the parameters host->device, runs the five steps with the given upstream gradients (HOST), copies the image
  * and all gradients device->host and synchronises.  Pointers follow the shapes above; outputs may be NULL. */

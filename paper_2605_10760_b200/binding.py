@@ -22,7 +22,7 @@ STATUS = {0: "GS_OK", -1: "GS_E_INVALID", -2: "GS_E_ORDER", -3: "GS_E_CUDA", -4:
 EXPORTS = ["gs_create", "gs_destroy", "gs_last_error", "gs_preprocess", "gs_bin_tiles", "gs_rasterize_fwd",
            "gs_rasterize_bwd", "gs_pose_grad", "gs_get_counts", "gs_get_binning", "gs_get_features", "gs_poll",
            "gs_aux_l1_grad", "gs_aux_pose_step", "gs_fwd_bwd_host", "gs_profile_enable", "gs_profile_read",
-           "gs_get_launch_count", "gs_get_workload"]
+           "gs_get_launch_count", "gs_get_workload", "gs_loss_map", "gs_loss_iso"]
 STAGES = ["preprocess", "tile_scan", "emit", "tile_sort", "raster_fwd", "raster_bwd", "gauss_bwd", "pose_grad"]
 
 
@@ -62,6 +62,8 @@ def load_library():
     lib.gs_poll.argtypes = [vp]
     lib.gs_aux_l1_grad.argtypes = [vp, i64, vp, vp, f, vp]
     lib.gs_aux_pose_step.argtypes = [vp, vp, vp, f]
+    lib.gs_loss_map.argtypes = [vp, C.c_int32, C.c_int32, vp, vp, vp, vp, f, f, vp, vp, vp]
+    lib.gs_loss_iso.argtypes = [vp, i64, vp, f, vp, vp]
     lib.gs_profile_enable.argtypes = [vp, C.c_int]
     lib.gs_profile_read.argtypes = [vp, C.POINTER(f * 8)]
     lib.gs_get_launch_count.argtypes = [vp, C.POINTER(C.c_uint64)]
@@ -254,6 +256,28 @@ def gs_aux_l1_grad(pred, target, weight, grad, stream=None):
                             float(weight), _ptr(grad, torch.float32))
     if rc != 0:
         raise GsError(rc, "gs_aux_l1_grad")
+
+
+def gs_loss_map(rgb, depth, target_rgb, target_depth, alpha, beta, d_rgb, d_depth, loss, stream=None):
+    """Eq. 4 photometric + depth L1 terms: writes the upstream gradients and double loss[4] (device; the last is scratch)."""
+    import torch
+    f32 = torch.float32
+    H, W = depth.shape
+    rc = load_library().gs_loss_map(_stream(stream), int(W), int(H), _ptr(rgb, f32), _ptr(depth, f32), _ptr(target_rgb, f32),
+                                    _ptr(target_depth, f32), float(alpha), float(beta), _ptr(d_rgb, f32), _ptr(d_depth, f32),
+                                    _ptr(loss, torch.float64))
+    if rc != 0:
+        raise GsError(rc, "gs_loss_map")
+
+
+def gs_loss_iso(scales, lambda_s, g_scales, loss, stream=None):
+    """Eq. 4 isotropy regulariser: adds its gradient into g_scales, writes double loss[2] (device)."""
+    import torch
+    f32 = torch.float32
+    rc = load_library().gs_loss_iso(_stream(stream), int(scales.shape[0]), _ptr(scales, f32), float(lambda_s),
+                                    _ptr(g_scales, f32), _ptr(loss, torch.float64))
+    if rc != 0:
+        raise GsError(rc, "gs_loss_iso")
 
 
 def gs_aux_pose_step(T_cw_dev, g_twist, step, stream=None):

@@ -1,0 +1,68 @@
+"""GPU parity of the Eq. 4 loss kernels (gs_loss_map, gs_loss_iso) against oracle/loss.py on the same
+seeded inputs.  Gradients are signs times a constant, so they must match EXACTLY where the oracle's difference is not a
+rounding-level tie; the loss sums are fp32 differences accumulated in fp64: relative 1e-6."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+def _images(seed, H, W):
+    r = np.random.Generator(np.random.PCG64(seed))
+    rgb = r.uniform(0, 1, (3, H, W)).astype(np.float32); trgb = r.uniform(0, 1, (3, H, W)).astype(np.float32)
+    d = r.uniform(0.5, 6, (H, W)).astype(np.float32); td = r.uniform(0.5, 6, (H, W)).astype(np.float32)
+    td[r.uniform(size=(H, W)) < 0.1] = 0.0           # 10 % of the pixels have no target depth
+    rgb[:, 0, :5] = trgb[:, 0, :5]                    # exact matches: sign(0) = 0
+    d[H // 2, :5] = td[H // 2, :5]
+    return rgb, d, trgb, td
+
+
+@pytest.mark.parametrize("shape", [(680, 1200), (33, 47), (1, 1), (16, 16)])   # vector path, ragged (scalar path), tiny
+def test_loss_map_matches_oracle(shape):
+    import torch
+    from oracle import loss as ol
+    from paper_2605_10760_b200 import binding as b
+    H, W = shape
+    rgb, d, trgb, td = _images(7 + H, H, W)
+    lr, ld, gr, gd = ol.l1_terms(rgb, d, trgb, td)
+    total, g_rgb, g_d = ol.map_loss(rgb, d, trgb, td, 0.95, 0.25)
+    t = lambda a: torch.from_numpy(a).cuda()
+    o_rgb = torch.empty(3, H, W, device="cuda"); o_d = torch.empty(H, W, device="cuda")
+    loss = torch.full((4,), -1.0, dtype=torch.float64, device="cuda")
+    b.gs_loss_map(t(rgb), t(d), t(trgb), t(td), 0.95, 0.25, o_rgb, o_d, loss)
+    torch.cuda.synchronize()
+    got = loss.cpu().numpy()
+    assert abs(got[0] - lr) <= 1e-6 * lr + 1e-12 and abs(got[1] - ld) <= 1e-6 * ld + 1e-12
+    assert abs(got[2] - total) <= 1e-6 * total + 1e-12
+    # signs are decided on the same fp32 inputs (the differences are exact in fp64 and correctly rounded in fp32)
+    assert np.array_equal(np.sign(o_rgb.cpu().numpy()), np.sign(g_rgb))
+    assert np.array_equal(np.sign(o_d.cpu().numpy()), np.sign(g_d))
+    assert np.allclose(o_rgb.cpu().numpy(), g_rgb, rtol=2e-7, atol=0) and np.allclose(o_d.cpu().numpy(), g_d, rtol=2e-7, atol=0)
+
+
+def test_loss_iso_matches_oracle_and_accumulates():
+    import torch
+    from oracle import loss as ol
+    from paper_2605_10760_b200 import binding as b
+    r = np.random.Generator(np.random.PCG64(11))
+    N = 100_003
+    s = np.exp(r.normal(-4.5, 0.5, (N, 3))).astype(np.float32)
+    s[:100] = s[:100, :1]                              # isotropic Gaussians: zero loss, zero gradient
+    ref_loss, ref_g = ol.iso_loss(s, 10.0)
+    base = r.normal(size=(N, 3)).astype(np.float32)
+    g = torch.from_numpy(base.copy()).cuda()
+    loss = torch.zeros(2, dtype=torch.float64, device="cuda")
+    b.gs_loss_iso(torch.from_numpy(s).cuda(), 10.0, g, loss)
+    torch.cuda.synchronize()
+    assert abs(float(loss[0]) - ref_loss) <= 1e-5 * ref_loss   # fp32 means of fp32 scales vs fp64
+    got = g.cpu().numpy().astype(np.float64) - base
+    # sign decisions: s_ij - mean can differ between fp32 and fp64 only when |s_ij - mean| is at rounding level
+    margin = np.abs(s.astype(np.float64) - s.astype(np.float64).mean(axis=1, keepdims=True)).min(axis=1)
+    ok = margin > 1e-6 * s.max(axis=1)
+    assert ok.mean() > 0.99
+    assert np.abs(got[ok] - ref_g[ok]).max() < 1e-5
+    assert np.all(got[:100] == 0.0)
+    # N = 0 is a no-op
+    b.gs_loss_iso(torch.zeros(0, 3, device="cuda"), 10.0, torch.zeros(0, 3, device="cuda"), loss)
+    torch.cuda.synchronize()
+    assert float(loss[0]) == 0.0
