@@ -431,7 +431,8 @@ tile_sort_large_kernel(const uint32_t* __restrict__ order, const uint2* __restri
       __syncthreads();
       continue;
     }
-    bucket_sort<16, 16>(g, ids + r.x, n, s_dyn, tid, slot_of);
+    if (n <= 4096) bucket_sort<8, 16>(g, ids + r.x, n, s_dyn, tid, slot_of);
+    else bucket_sort<16, 16>(g, ids + r.x, n, s_dyn, tid, slot_of);
     __syncthreads();
   }
 }
@@ -450,7 +451,9 @@ tile_sort_kernel(int tiles, const uint32_t* __restrict__ order, const uint2* __r
     const uint2 r = ranges[order[blockIdx.x]];
     const int n = (int)(r.y - r.x);
     if (n > kMidSortMax) return;
-    if (n <= 1024) bucket_sort<8, 4>(keys + r.x, ids + r.x, n, s_x, tid, slot_of);
+    // keys per thread matched to the bucket: the network runs over 128 E slots whatever n is
+    if (n <= 512) bucket_sort<4, 4>(keys + r.x, ids + r.x, n, s_x, tid, slot_of);
+    else if (n <= 1024) bucket_sort<8, 4>(keys + r.x, ids + r.x, n, s_x, tid, slot_of);
     else bucket_sort<16, 4>(keys + r.x, ids + r.x, n, s_x, tid, slot_of);
     return;
   }
@@ -460,6 +463,7 @@ tile_sort_kernel(int tiles, const uint32_t* __restrict__ order, const uint2* __r
   const int n = (int)(r.y - r.x), lane = tid & 31;
   if (n == 0) return;
   if (n <= 64) bucket_sort<2, 1>(keys + r.x, ids + r.x, n, nullptr, lane, slot_of);
+  else if (n <= 128) bucket_sort<4, 1>(keys + r.x, ids + r.x, n, nullptr, lane, slot_of);
   else bucket_sort<8, 1>(keys + r.x, ids + r.x, n, nullptr, lane, slot_of);
 }
 
