@@ -171,6 +171,14 @@ GS_API int gs_loss_map(void* stream, int32_t width, int32_t height, const float*
  * DEVICE double loss[2]: loss[0] = the weighted loss (loss[1] is scratch). */
 GS_API int gs_loss_iso(void* stream, int64_t N, const float* scales, float lambda_s, float* g_scales, double* loss);
 
+/* ---- Eq. 19: a submap's Sim(3) correction applied to its Gaussians --------------------------------- */
+/* mu' = s R mu + t, s_i' = s s_i, q' = q_R (x) q (so that Sigma' = s^2 R Sigma R^T); opacity and colour are unchanged
+ * and are not arguments.  s > 0, R row-major float[9] (a rotation), t float[3]: HOST.  means, scales
+ * [N,3], quats [N,4] (16-byte aligned) and the three outputs: DEVICE; an output may alias its input (in place).
+ * Asynchronous on `stream`.  GS_E_INVALID on null pointers, s <= 0 or misaligned quaternions. */
+GS_API int gs_sim3_apply(void* stream, int64_t N, float s, const float* R, const float* t, const float* means,
+                         const float* scales, const float* quats, float* means_out, float* scales_out, float* quats_out);
+
 /* ---- host-buffer convenience (bench.py "e2e"): one whole fwd+bwd iteration with HOST arrays -------------------- */
 /* Copies the parameters host->device, runs the five steps with the given upstream gradients (HOST), copies the image
  * and all gradients device->host and synchronises.  Pointers follow the shapes above; outputs may be NULL. */

@@ -22,7 +22,7 @@ STATUS = {0: "GS_OK", -1: "GS_E_INVALID", -2: "GS_E_ORDER", -3: "GS_E_CUDA", -4:
 EXPORTS = ["gs_create", "gs_destroy", "gs_last_error", "gs_preprocess", "gs_bin_tiles", "gs_rasterize_fwd",
            "gs_rasterize_bwd", "gs_pose_grad", "gs_get_counts", "gs_get_binning", "gs_get_features", "gs_poll",
            "gs_aux_l1_grad", "gs_aux_pose_step", "gs_fwd_bwd_host", "gs_profile_enable", "gs_profile_read",
-           "gs_get_launch_count", "gs_get_workload", "gs_loss_map", "gs_loss_iso"]
+           "gs_get_launch_count", "gs_get_workload", "gs_loss_map", "gs_loss_iso", "gs_sim3_apply"]
 STAGES = ["preprocess", "tile_scan", "emit", "tile_sort", "raster_fwd", "raster_bwd", "gauss_bwd", "pose_grad"]
 
 
@@ -64,6 +64,7 @@ def load_library():
     lib.gs_aux_pose_step.argtypes = [vp, vp, vp, f]
     lib.gs_loss_map.argtypes = [vp, C.c_int32, C.c_int32, vp, vp, vp, vp, f, f, vp, vp, vp]
     lib.gs_loss_iso.argtypes = [vp, i64, vp, f, vp, vp]
+    lib.gs_sim3_apply.argtypes = [vp, i64, f, C.POINTER(f * 9), C.POINTER(f * 3), vp, vp, vp, vp, vp, vp]
     lib.gs_profile_enable.argtypes = [vp, C.c_int]
     lib.gs_profile_read.argtypes = [vp, C.POINTER(f * 8)]
     lib.gs_get_launch_count.argtypes = [vp, C.POINTER(C.c_uint64)]
@@ -278,6 +279,21 @@ def gs_loss_iso(scales, lambda_s, g_scales, loss, stream=None):
                                     _ptr(g_scales, f32), _ptr(loss, torch.float64))
     if rc != 0:
         raise GsError(rc, "gs_loss_iso")
+
+
+def gs_sim3_apply(s, R, t, means, scales, quats, means_out=None, scales_out=None, quats_out=None, stream=None):
+    """Eq. 19: Sim(3) correction (s, R, t) of Gaussians on the device; in place unless outputs are given."""
+    import torch
+    f32 = torch.float32
+    Rm = np.asarray(R, np.float32).reshape(9); tv = np.asarray(t, np.float32).reshape(3)
+    Rc = (C.c_float * 9)(*[float(x) for x in Rm]); tc = (C.c_float * 3)(*[float(x) for x in tv])
+    mo = means if means_out is None else means_out
+    so = scales if scales_out is None else scales_out
+    qo = quats if quats_out is None else quats_out
+    rc = load_library().gs_sim3_apply(_stream(stream), int(means.shape[0]), float(s), Rc, tc, _ptr(means, f32),
+                                      _ptr(scales, f32), _ptr(quats, f32), _ptr(mo, f32), _ptr(so, f32), _ptr(qo, f32))
+    if rc != 0:
+        raise GsError(rc, "gs_sim3_apply")
 
 
 def gs_aux_pose_step(T_cw_dev, g_twist, step, stream=None):
