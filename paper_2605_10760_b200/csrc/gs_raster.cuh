@@ -69,46 +69,6 @@ __device__ __forceinline__ void eval_power(const GaussReg& g, float fx0, float f
       p[ky * NX + kx] = __fmaf_rn(dx[kx], __fmaf_rn(g.B, dy[ky], ax[kx]), cy[ky]);
 }
 
-// Packed fp32 pairs (sm_100 FFMA2 / FMUL2 / FADD2): one issue slot for two independent IEEE-rounded operations
-// (measured: 16 FFMA + 8 IADD per iteration 4.45 ms, 8 FFMA2 + 8 IADD 3.34 ms -- the FMA pipe rate is unchanged, the
-// issue slots halve).  Each component rounds exactly like the scalar instruction.
-typedef unsigned long long f32x2;
-__device__ __forceinline__ f32x2 pack2(float lo, float hi) {
-  f32x2 r;
-  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-  return r;
-}
-__device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi) {
-  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
-}
-__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
-  f32x2 d;
-  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
-  return d;
-}
-__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
-  f32x2 d;
-  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-  return d;
-}
-__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
-  f32x2 d;
-  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-  return d;
-}
-
-// power2 of one pixel for TWO list entries at once; component-wise the same sequence as eval_power1:
-//   dx = fx0 - mx (one rounding, here as fma(-1, mx, fx0)); p = fma(dx, fma(B, dy, A dx), (C dy) dy)
-// m = {mx0, mx1, my0, my1}, ab = {A0, A1, B0, B1}, c2 = {C0, C1}
-__device__ __forceinline__ void eval_power_pair(const float4& m, const float4& ab, f32x2 c2, f32x2 fx2, f32x2 fy2,
-                                                f32x2 neg1, float& p0, float& p1) {
-  const f32x2 dx = fma2(neg1, pack2(m.x, m.y), fx2);
-  const f32x2 dy = fma2(neg1, pack2(m.z, m.w), fy2);
-  const f32x2 u = fma2(pack2(ab.z, ab.w), dy, mul2(pack2(ab.x, ab.y), dx));
-  const f32x2 p = fma2(dx, u, mul2(mul2(c2, dy), dy));
-  unpack2(p, p0, p1);
-}
-
 // the same sequence for one pixel per lane (8x4 regions)
 __device__ __forceinline__ float eval_power1(float mx, float my, float A, float B, float C, float fx0, float fy0,
                                              float& dx, float& dy) {
