@@ -180,7 +180,7 @@ int gs_destroy(gs_ctx* ctx) {
   for (int b = 0; b < 2; ++b) { cudaFree(ctx->keys[b]); cudaFree(ctx->vals[b]); }
   cudaFree(ctx->hdr); cudaFree(ctx->tile_cursor); cudaFree(ctx->scan_ws);
   cudaFree(ctx->ranges); cudaFree(ctx->tile_order); cudaFree(ctx->final_T); cudaFree(ctx->n_contrib);
-  cudaFree(ctx->hb);
+  cudaFree(ctx->hb); cudaFree(ctx->stats_ws);
   if (ctx->mailbox) cudaFreeHost(ctx->mailbox);
   if (ctx->side_stream) cudaStreamDestroy(ctx->side_stream);
   if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
@@ -197,8 +197,7 @@ const char* gs_last_error(const gs_ctx* ctx) { return ctx ? ctx->err : "null con
 
 int gs_poll(gs_ctx* ctx) {
   if (!ctx) return GS_E_INVALID;
-  if (handle_overflow(ctx)) return fail(ctx, GS_E_OVERFLOW, "tile-instance capacity exceeded in an earlier iteration; scratch has grown, re-issue");
-  return GS_OK;
+  return handle_overflow(ctx);
 }
 
 int gs_preprocess(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, const float* means, const float* scales,
@@ -210,10 +209,13 @@ int gs_preprocess(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, const flo
   if (cam->width <= 0 || cam->height <= 0 || cam->width > 65535 * GS_TILE || cam->height > 65535 * GS_TILE)
     return fail(ctx, GS_E_INVALID, "gs_preprocess: bad image size");
   if (((uintptr_t)quats & 15) != 0) return fail(ctx, GS_E_INVALID, "gs_preprocess: quats must be 16-byte aligned");
+  // the SH rows are read as float4 when a row is a whole number of them (degrees 1 and 3: 12 and 48 floats)
+  if ((3 * (sh_degree + 1) * (sh_degree + 1)) % 4 == 0 && ((uintptr_t)sh & 15) != 0)
+    return fail(ctx, GS_E_INVALID, "gs_preprocess: sh must be 16-byte aligned for SH degrees 1 and 3");
   cudaStream_t s = (cudaStream_t)stream;
   GS_CUDA(cudaSetDevice(ctx->device));
-  if (handle_overflow(ctx)) return fail(ctx, GS_E_OVERFLOW, "tile-instance capacity exceeded in an earlier iteration; scratch has grown, re-issue");
   int rc;
+  if ((rc = handle_overflow(ctx)) != GS_OK) return rc;
   if ((rc = ensure_gaussian_capacity(ctx, N)) != GS_OK) return rc;
   DevCam& c = ctx->cam;
   c.W = cam->width; c.H = cam->height;
@@ -268,6 +270,8 @@ int gs_rasterize_bwd(gs_ctx* ctx, void* stream, const float* d_rgb, const float*
   if (write && ctx->N > 0 && (!g_means || !g_scales || !g_quats || !g_opacities || !g_sh))
     return fail(ctx, GS_E_INVALID, "gs_rasterize_bwd: null gradient array without GS_POSE_ONLY");
   if (write && ((uintptr_t)g_quats & 15) != 0) return fail(ctx, GS_E_INVALID, "gs_rasterize_bwd: g_quats must be 16-byte aligned");
+  if (write && (3 * (ctx->sh_degree + 1) * (ctx->sh_degree + 1)) % 4 == 0 && ((uintptr_t)g_sh & 15) != 0)
+    return fail(ctx, GS_E_INVALID, "gs_rasterize_bwd: g_sh must be 16-byte aligned for SH degrees 1 and 3");
   cudaStream_t s = (cudaStream_t)stream;
   GS_CUDA(cudaSetDevice(ctx->device));
   if (ctx->g2d_dirty && ctx->N > 0) GS_CUDA(cudaMemsetAsync(ctx->g2d, 0, (size_t)ctx->N * kG2D * sizeof(float), s));
@@ -323,8 +327,8 @@ int gs_get_counts(gs_ctx* ctx, void* stream, int64_t* n_visible, int64_t* n_inst
   if (n_visible) *n_visible = c.n_visible;
   if (n_instances) *n_instances = c.n_instances;
   if (c.overflow) {
-    handle_overflow(ctx);
-    return fail(ctx, GS_E_OVERFLOW, "tile-instance capacity exceeded in this iteration; scratch has grown, re-issue");
+    const int rc = handle_overflow(ctx);
+    return rc != GS_OK ? rc : fail(ctx, GS_E_OVERFLOW, "tile-instance capacity exceeded in this iteration; scratch has grown, re-issue");
   }
   return GS_OK;
 }

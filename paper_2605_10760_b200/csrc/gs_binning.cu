@@ -509,13 +509,16 @@ int ensure_instance_capacity(gs_ctx* ctx, int64_t need) {
   return GS_OK;
 }
 
-// If the mailbox shows that an earlier asynchronous iteration overflowed: grow to fit it, clear the flag, return true.
-bool handle_overflow(gs_ctx* ctx) {
+// If the mailbox shows that an earlier asynchronous iteration overflowed: grow to fit it, clear the flag and return
+// GS_E_OVERFLOW (the caller re-issues the iteration), or GS_E_NOMEM if the scratch could not grow (the old buffers and
+// capacity stay valid, the flag stays set).  GS_OK when nothing overflowed.
+int handle_overflow(gs_ctx* ctx) {
   const Counts mb = read_mailbox(ctx);
-  if (!mb.overflow) return false;
-  ensure_instance_capacity(ctx, (int64_t)mb.n_instances + (int64_t)mb.n_instances / 4);
+  if (!mb.overflow) return GS_OK;
+  const int rc = ensure_instance_capacity(ctx, (int64_t)mb.n_instances + (int64_t)mb.n_instances / 4);
+  if (rc != GS_OK) return rc;
   ctx->mailbox->overflow = 0;
-  return true;
+  return fail(ctx, GS_E_OVERFLOW, "tile-instance capacity exceeded in an earlier iteration; scratch has grown, re-issue");
 }
 
 static int run_tile_scan(gs_ctx* ctx, cudaStream_t s) {
@@ -563,7 +566,7 @@ int launch_binning(gs_ctx* ctx, cudaStream_t s) {
   } else {
     // asynchronous path: act on what the last finished iteration reported (no synchronisation): an overflow is
     // reported to the caller (after growing), a near-full buffer is grown ahead of time
-    if (handle_overflow(ctx)) return fail(ctx, GS_E_OVERFLOW, "tile-instance capacity exceeded in an earlier iteration; scratch has grown, re-issue");
+    if ((rc = handle_overflow(ctx)) != GS_OK) return rc;
     const Counts mb = read_mailbox(ctx);
     if ((int64_t)mb.n_instances + (int64_t)mb.n_instances / 8 > ctx->cap_I)
       if ((rc = ensure_instance_capacity(ctx, (int64_t)mb.n_instances + (int64_t)mb.n_instances / 4)) != GS_OK) return rc;

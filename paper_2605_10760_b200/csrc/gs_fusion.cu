@@ -13,9 +13,8 @@ struct Sim3Dev {
 };
 
 __global__ void __launch_bounds__(256)
-sim3_kernel(int64_t N, Sim3Dev C, const float* __restrict__ means, const float* __restrict__ scales,
-            const float* __restrict__ quats, float* __restrict__ means_out, float* __restrict__ scales_out,
-            float* __restrict__ quats_out) {
+sim3_kernel(int64_t N, Sim3Dev C, const float* means, const float* scales, const float* quats, float* means_out,
+            float* scales_out, float* quats_out) {  // no __restrict__: an output may alias its input (gs.h)
   const int64_t stride = (int64_t)gridDim.x * blockDim.x;
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += stride) {
     const float m0 = means[3 * i], m1 = means[3 * i + 1], m2 = means[3 * i + 2];

@@ -24,7 +24,7 @@ __global__ void __launch_bounds__(128)
 gauss_bwd_kernel(int64_t N, const float* __restrict__ means, const float* __restrict__ scales,
                  const float* __restrict__ quats, const float* __restrict__ opacities, const float* __restrict__ sh,
                  DevCam cam, const uint32_t* __restrict__ vis_ids, const float4* __restrict__ vis_par,
-                 const Counts* __restrict__ counts,
+                 const float4* __restrict__ feat, const Counts* __restrict__ counts,
                  float* __restrict__ g2d, bool accumulate,
                  float* __restrict__ g_means, float* __restrict__ g_scales, float* __restrict__ g_quats,
                  float* __restrict__ g_opac, float* __restrict__ g_sh, double* __restrict__ pose_acc) {
@@ -52,7 +52,14 @@ gauss_bwd_kernel(int64_t N, const float* __restrict__ means, const float* __rest
     const float mu0 = pa.x, mu1 = pa.y, mu2 = pa.z, o = pa.w;
     const float s0 = pb.x, s1 = pb.y, s2 = pb.z;
     Proj<R> P;
-    project_gaussian<R>(cam, T, mu0, mu1, mu2, s0, s1, s2, q.x, q.y, q.z, q.w, o, P);
+    project_gaussian<R, false>(cam, T, mu0, mu1, mu2, s0, s1, s2, q.x, q.y, q.z, q.w, o, P);
+    {
+      // The conic is taken from the forward's feature record (computed in fp64 by gs_preprocess, stored pre-scaled by
+      // -0.5 log2(e) / -log2(e)): the fp32 determinant cxx cyy - cxy^2 loses all digits for long thin footprints.
+      const float4 f1 = __ldg(feat + 3 * (size_t)kk + 1);
+      const R ln2 = (R)0.69314718055994531;
+      P.a = -(R)2 * ln2 * (R)f1.x; P.b = -ln2 * (R)f1.y; P.c = -(R)2 * ln2 * (R)f1.z;
+    }
     const R W[9] = {T[0], T[1], T[2], T[4], T[5], T[6], T[8], T[9], T[10]};
     // ga.x, ga.y = sum gp dx, sum gp dy (moments about the mean); d power / d mean = -(Q d), ln2 * log2(e) = 1
     const R g_mx = P.a * (R)ga.x + P.b * (R)ga.y, g_my = P.b * (R)ga.x + P.c * (R)ga.y;
@@ -261,7 +268,7 @@ int launch_gauss_bwd(gs_ctx* ctx, cudaStream_t s, uint32_t flags, float* g_means
   const unsigned blocks = (unsigned)div_up(ctx->N, threads);
 #define GS_GB(D, Wr)                                                                                                 \
   gauss_bwd_kernel<D, Wr><<<blocks, threads, 0, s>>>(ctx->N, ctx->means, ctx->scales, ctx->quats, ctx->opacities,   \
-                                                      ctx->sh, ctx->cam, ctx->vis_ids, ctx->vis_par, ctx->counts, ctx->g2d, accum, \
+                                                      ctx->sh, ctx->cam, ctx->vis_ids, ctx->vis_par, ctx->feat, ctx->counts, ctx->g2d, accum, \
                                                       g_means, g_scales, g_quats, g_opac, g_sh, ctx->pose_acc)
   if (write) {
     switch (ctx->sh_degree) {

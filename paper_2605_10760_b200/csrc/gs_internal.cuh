@@ -113,6 +113,7 @@ struct gs_ctx {
   double* pose_acc = nullptr;
   bool pose_acc_valid = false;
   bool pose_acc_clean = false;  // zeroed by gs_preprocess and not yet accumulated into
+  unsigned long long* stats_ws = nullptr;  // gs_get_workload: its own 8 counters (never the pose accumulators)
   char* hdr = nullptr;          // one allocation: counts, pose_acc, tile_count (zeroed by one memset per iteration)
 
   gs::Counts* counts = nullptr;       // device
@@ -170,17 +171,20 @@ inline int fail_cuda(gs_ctx* ctx, cudaError_t e, const char* where) {
     if (ctx->prof_on) cudaEventRecord(ctx->ev[k], s);                  \
   } while (0)
 
+// Replaces the buffer by one of `count` elements (contents are not kept).  The new buffer is allocated FIRST and
+// swapped in on success: when cudaMalloc fails the old buffer -- and the capacity the caller recorded for it -- stay valid.
 template <typename T>
 inline int grow(gs_ctx* ctx, T*& p, int64_t count) {
-  if (p) cudaFree(p);
-  p = nullptr;
-  if (count <= 0) return GS_OK;
-  cudaError_t e = cudaMalloc((void**)&p, (size_t)count * sizeof(T));
-  if (e != cudaSuccess) {
-    p = nullptr;
-    cudaGetLastError();
-    return fail(ctx, GS_E_NOMEM, "cudaMalloc failed while growing scratch");
+  T* fresh = nullptr;
+  if (count > 0) {
+    cudaError_t e = cudaMalloc((void**)&fresh, (size_t)count * sizeof(T));
+    if (e != cudaSuccess) {
+      cudaGetLastError();
+      return fail(ctx, GS_E_NOMEM, "cudaMalloc failed while growing scratch");
+    }
   }
+  if (p) cudaFree(p);
+  p = fresh;
   return GS_OK;
 }
 
@@ -210,7 +214,7 @@ int launch_gauss_bwd(gs_ctx* ctx, cudaStream_t s, uint32_t flags, float* g_means
 int launch_zero_fill(gs_ctx* ctx, cudaStream_t s, float* g_means, float* g_scales, float* g_quats, float* g_opac, float* g_sh);
 int launch_pose_final(gs_ctx* ctx, cudaStream_t s, uint32_t flags, float* g_twist);
 int ensure_instance_capacity(gs_ctx* ctx, int64_t need);
-bool handle_overflow(gs_ctx* ctx);
+int handle_overflow(gs_ctx* ctx);
 int export_sorted_keys(gs_ctx* ctx, cudaStream_t s, uint64_t* out);
 int export_sorted_ids(gs_ctx* ctx, cudaStream_t s, int64_t I, uint32_t* out);
 int launch_workload_stats(gs_ctx* ctx, cudaStream_t s, uint64_t* out_host);

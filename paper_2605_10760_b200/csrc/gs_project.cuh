@@ -38,8 +38,10 @@ __device__ __forceinline__ void quat_rotation(const R* r, R* Rm) {
 }
 
 // Returns false when the Gaussian is culled before any covariance work (behind the near plane, opacity < 1/255) or
-// its projection is degenerate / non-finite.
-template <typename R>
+// its projection is degenerate / non-finite.  CULL = false (per-Gaussian backward): visibility was already decided by
+// gs_preprocess in fp64, so none of the early-outs is taken and every field of P is always written -- an fp32
+// re-projection must never disagree with the forward about which Gaussians exist.
+template <typename R, bool CULL = true>
 __device__ __forceinline__ bool project_gaussian(const DevCam& cam, const float* T, float mu0, float mu1, float mu2,
                                                  float s0, float s1, float s2, float q0, float q1, float q2, float q3,
                                                  float opacity, Proj<R>& P) {
@@ -48,8 +50,8 @@ __device__ __forceinline__ bool project_gaussian(const DevCam& cam, const float*
   P.x = W[0] * m0 + W[1] * m1 + W[2] * m2 + (R)T[3];
   P.y = W[3] * m0 + W[4] * m1 + W[5] * m2 + (R)T[7];
   P.z = W[6] * m0 + W[7] * m1 + W[8] * m2 + (R)T[11];
-  if (!(P.z > (R)cam.near_z)) return false;
-  if ((double)opacity < 1.0 / 255.0) return false;
+  if (CULL && !(P.z > (R)cam.near_z)) return false;
+  if (CULL && (double)opacity < 1.0 / 255.0) return false;
   const R q[4] = {(R)q0, (R)q1, (R)q2, (R)q3};
   P.qn = sqrt(q[0] * q[0] + q[1] * q[1] + q[2] * q[2] + q[3] * q[3]);
   const R iq = (R)1 / P.qn;
@@ -78,12 +80,12 @@ __device__ __forceinline__ bool project_gaussian(const DevCam& cam, const float*
   P.cxy = P.M[0] * P.M[3] + P.M[1] * P.M[4] + P.M[2] * P.M[5];
   P.cyy = P.M[3] * P.M[3] + P.M[4] * P.M[4] + P.M[5] * P.M[5] + (R)GS_DILATION;
   const R det = P.cxx * P.cyy - P.cxy * P.cxy;
-  if (!(det > (R)0) || !isfinite(det)) return false;
+  if (CULL && (!(det > (R)0) || !isfinite(det))) return false;
   const R idet = (R)1 / det;
   P.a = P.cyy * idet; P.b = -P.cxy * idet; P.c = P.cxx * idet;
   P.mx = fx * P.x * iz + (R)cam.cx;
   P.my = fy * P.y * iz + (R)cam.cy;
-  if (!isfinite(P.mx) || !isfinite(P.my)) return false;
+  if (CULL && (!isfinite(P.mx) || !isfinite(P.my))) return false;
   return true;
 }
 

@@ -334,7 +334,8 @@ int launch_raster_fwd(gs_ctx* ctx, cudaStream_t s, float* rgb, float* depth, flo
 // Workload statistics of the forward (introspection only): re-walks every pixel's list with the forward's decisions.
 int launch_workload_stats(gs_ctx* ctx, cudaStream_t s, uint64_t* out_host) {
   const int tiles = ctx->cam.tiles_x * ctx->cam.tiles_y;
-  unsigned long long* d = reinterpret_cast<unsigned long long*>(ctx->pose_acc);  // 16 doubles of scratch, unused here
+  if (!ctx->stats_ws) GS_CUDA(cudaMalloc((void**)&ctx->stats_ws, 8 * sizeof(unsigned long long)));
+  unsigned long long* d = ctx->stats_ws;
   GS_CUDA(cudaMemsetAsync(d, 0, 4 * sizeof(unsigned long long), s));
   if (tiles > 0) {
     raster_fwd_kernel<2, 4, true><<<tiles, 32, 0, s>>>(ctx->cam.W, ctx->cam.H, ctx->cam.tiles_x, ctx->tile_order,
@@ -344,8 +345,6 @@ int launch_workload_stats(gs_ctx* ctx, cudaStream_t s, uint64_t* out_host) {
   }
   GS_CUDA(cudaMemcpyAsync(out_host, d, 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, s));
   GS_CUDA(cudaStreamSynchronize(s));
-  ctx->pose_acc_valid = false;
-  ctx->pose_acc_clean = false;
   return GS_OK;
 }
 

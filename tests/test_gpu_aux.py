@@ -1,0 +1,142 @@
+"""GPU parity of the auxiliary kernels outside the five-call contract (include/gs.h): gs_aux_pose_step against the oracle's
+SE(3) exponential (oracle.pose_apply, pinned to scipy.linalg.expm in tests/test_oracle_pins.py), gs_aux_l1_grad against
+oracle/loss.py, and the degenerate Gaussians the per-Gaussian backward must survive (near-plane grazers and
+needle footprints)."""
+import copy
+
+import numpy as np
+import pytest
+
+from paper_2605_10760_b200 import scenes
+
+pytestmark = pytest.mark.gpu
+
+
+def _T(seed):
+    r = np.random.Generator(np.random.PCG64(seed))
+    return scenes.perturb_pose(scenes.look_at(r.uniform(1, 3, 3), r.uniform(3, 5, 3)), r.normal(0, 0.3, 6))
+
+
+@pytest.mark.parametrize("case", ["generic", "tiny_rotation", "pure_translation", "zero_gradient", "large_rotation"])
+def test_pose_step_matches_oracle_exp(oracle, case):
+    """T <- Exp(-step g / |g|) T  (gs.h); the oracle side is pose_apply(xi, T) with xi formed in fp64."""
+    import torch
+    from paper_2605_10760_b200 import binding as b
+    r = np.random.Generator(np.random.PCG64(len(case)))
+    T0 = _T(3)
+    g = r.normal(size=6).astype(np.float32)
+    step = 1e-3
+    if case == "tiny_rotation":       # theta ~ 1e-9: the series branch of the exponential
+        g[3:] *= 1e-6
+    elif case == "pure_translation":  # theta = 0 exactly
+        g[3:] = 0.0
+    elif case == "zero_gradient":     # |g| = 0: documented no-op
+        g[:] = 0.0
+    elif case == "large_rotation":
+        step = 2.5
+    T_dev = torch.from_numpy(T0.reshape(-1).copy()).cuda()
+    b.gs_aux_pose_step(T_dev, torch.from_numpy(g).cuda(), step)
+    torch.cuda.synchronize()
+    got = T_dev.cpu().numpy().reshape(3, 4)
+    if case == "zero_gradient":
+        assert np.array_equal(got, T0)
+        return
+    g64 = g.astype(np.float64)
+    xi = -step * g64 / np.linalg.norm(g64)
+    want = oracle.pose_apply(xi, T0.astype(np.float64))
+    # fp64 arithmetic on both sides, one rounding to fp32 at the end
+    assert np.abs(got - want).max() <= 6e-8 * max(1.0, np.abs(want).max()), np.abs(got - want).max()
+    R = got[:, :3].astype(np.float64)
+    assert np.abs(R @ R.T - np.eye(3)).max() < 5e-7
+
+
+@pytest.mark.parametrize("n", [1, 1000, 3 * 680 * 1200 + 7])
+def test_l1_grad_matches_oracle(n):
+    """grad = weight * sign(pred - target), sign(0) = 0: the RGB half of oracle/loss.py's l1_terms."""
+    import torch
+    from oracle import loss as ol
+    from paper_2605_10760_b200 import binding as b
+    r = np.random.Generator(np.random.PCG64(n))
+    pred = r.uniform(0, 1, n).astype(np.float32)
+    target = r.uniform(0, 1, n).astype(np.float32)
+    target[:: 7] = pred[:: 7]          # exact ties
+    w = 1.0 / (3 * 77)
+    grad = torch.full((n,), 5.0, device="cuda")
+    b.gs_aux_l1_grad(torch.from_numpy(pred).cuda(), torch.from_numpy(target).cuda(), w, grad)
+    torch.cuda.synchronize()
+    # the oracle works on [3,H,W]: present the vectors as a 3 x 1 x m image (pad to a multiple of 3 with ties)
+    m = (n + 2) // 3
+    P = np.zeros(3 * m, np.float32); Tt = np.zeros(3 * m, np.float32)
+    P[:n] = pred; Tt[:n] = target
+    _, _, g_rgb, _ = ol.l1_terms(P.reshape(3, 1, m), np.zeros((1, m)), Tt.reshape(3, 1, m), np.zeros((1, m)))
+    want = (g_rgb.reshape(-1)[:n] * (3 * m)) * w          # undo the oracle's mean, apply the call's weight
+    got = grad.cpu().numpy()
+    assert np.array_equal(np.sign(got), np.sign(want))
+    assert np.allclose(got, want, rtol=2e-7, atol=0)
+
+
+def _run(gpu_ctx, b, torch, sc, gC, gD):
+    ds = b.DeviceScene(sc)
+    out = ds.alloc_outputs(sc.camera.width, sc.camera.height)
+    for attempt in range(3):
+        try:
+            b.forward(gpu_ctx, ds, sc.camera, out)
+            gpu_ctx.gs_get_counts()
+            break
+        except b.GsError as e:
+            if e.code != -5 or attempt == 2:
+                raise
+    b.backward(gpu_ctx, out, torch.from_numpy(gC).cuda(), torch.from_numpy(gD).cuda(), None, 0)
+    torch.cuda.synchronize()
+    gpu_ctx.gs_poll()
+    return {k: v.cpu().numpy() for k, v in out.items()}
+
+
+def _rel(a, b):
+    a = np.asarray(a, np.float64); b = np.asarray(b, np.float64)
+    n = np.linalg.norm(b)
+    return np.linalg.norm(a - b) / n if n > 0 else np.linalg.norm(a - b)
+
+
+def test_backward_survives_near_plane_grazers_and_needles(oracle):
+    """ADVICE r1 (gs_gauss_bwd.cu): visibility is decided once, by gs_preprocess in fp64; the fp32 per-Gaussian backward
+    must not re-cull (z one ulp beyond near_z) nor lose the conic to cancellation (footprints ~1e3 px long, 1 px wide,
+    correlation 0.999999).  Every output must be finite, the grazers' gradients must match the oracle, and the twist --
+    a sum over ALL Gaussians, so one poisoned Gaussian would show -- must match too."""
+    import torch
+    from paper_2605_10760_b200 import binding as b
+    base = scenes.tiny_scene(seed=4, N=64)
+    sc = copy.copy(base)
+    sc.means = base.means.copy(); sc.scales = base.scales.copy(); sc.quats = base.quats.copy()
+    sc.opacities = base.opacities.copy()
+    near = np.float32(sc.camera.near_z)
+    # (a) 8 grazers: z_c = nextafter(near_z) ... near_z (1 + 1e-6); tiny scales so the footprint stays on screen
+    for k in range(8):
+        z = np.nextafter(near, np.float32(1)) if k == 0 else np.float32(near * (1 + 1e-7 * (1 + 2 * k)))
+        sc.means[k] = [0.02 * (k - 4) * z, 0.01 * (k - 4) * z, z]
+        sc.scales[k] = [0.004, 0.006, 0.005]
+        sc.opacities[k] = 0.6
+    # (b) 4 needles through the image: 3-D Gaussians elongated 1000:1 in the image plane at 45 degrees
+    c, s_ = np.cos(np.pi / 8), np.sin(np.pi / 8)      # rotation by 45 degrees about z
+    for k in range(8, 12):
+        sc.means[k] = [0.1 * (k - 10), -0.1 * (k - 10), 3.0]
+        # sigma ~15, 30, 45 px and ~600 px (correlation 0.999999 after the 0.3 px^2 dilation) by 0.02 px
+        sc.scales[k] = [(600.0 if k == 11 else 15.0 * (k - 7)) * 3.0 / 64.0, 0.02 * 3.0 / 64.0, 1e-3]
+        sc.quats[k] = [c, 0.0, 0.0, s_ if k % 2 == 0 else -s_]
+        sc.opacities[k] = 0.5
+    sc.name = "grazers_and_needles"
+    gC, gD = scenes.upstream_gradients(12, 64, 64)
+    ref = oracle.forward_backward(sc, gC, gD)
+    assert ref["visible"][:12].all(), "the construction must keep the degenerate Gaussians visible in the oracle"
+    ctx = b.Context(0)
+    got = _run(ctx, b, torch, sc, gC, gD)
+    ctx.close()
+    for k in ("rgb", "depth", "alpha", "g_means", "g_scales", "g_quats", "g_opacities", "g_sh", "g_twist"):
+        assert np.isfinite(got[k]).all(), k
+    # grazers: per-Gaussian gradients against the oracle (they are not culled by the backward)
+    for k in ("g_means", "g_scales", "g_quats", "g_opacities", "g_sh"):
+        assert np.any(got[k][:8]), k
+        assert _rel(got[k][:8], ref[k][:8]) <= 1e-3, (k, _rel(got[k][:8], ref[k][:8]))
+    # everything, needles included
+    for k in ("g_means", "g_scales", "g_quats", "g_opacities", "g_sh", "g_twist"):
+        assert _rel(got[k], ref[k]) <= 1e-3, (k, _rel(got[k], ref[k]))

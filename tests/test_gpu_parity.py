@@ -72,7 +72,10 @@ def check_features(oracle, sc, ref, got, cam):
     assert np.array_equal(f["depth_key"][vis_g], ref["z32"].view(np.uint32)[vis_g]), "depth keys differ"
     assert np.abs(f["mean2d"][both] - ref["mean2d"][both]).max() < 1e-6 * max(1.0, np.abs(ref["mean2d"][both]).max() / 1e3) + 4e-8
     assert rel_l2(f["conic"][both], ref["conic"][both]) < 1e-6
-    assert np.abs(f["conic"][both] / ref["conic"][both] - 1)[np.abs(ref["conic"][both]) > 1e-9].max() < 1e-5 or True
+    # per element: two fp32 roundings of an fp64 chain (the off-diagonal entry only where it is not a cancellation residue)
+    co, cg = ref["conic"][both], f["conic"][both].astype(np.float64)
+    live = np.abs(co) > 1e-6 * np.sqrt(co[:, :1] * co[:, 2:3])
+    assert np.abs(cg / co - 1)[live].max() < 1e-5
     assert np.abs(f["color"][both] - ref["color"][both]).max() < 2e-6
     assert np.abs(f["depth"][both] / ref["z"][both] - 1).max() < 1.2e-7
     # rect: oracle-exact  subset of  GPU  subset of  oracle with twice the GPU padding
@@ -89,7 +92,17 @@ def check_features(oracle, sc, ref, got, cam):
     assert (rg[:, 0] >= x0 // 16).all() and (rg[:, 1] >= y0 // 16).all()
     assert (rg[:, 2] <= (x1 - 1) // 16 + 1).all() and (rg[:, 3] <= (y1 - 1) // 16 + 1).all()
     mism = int((ro != rg).any(axis=1).sum())
-    return dict(extra_visible=extra, rect_mismatch=mism, visible=int(vis_o.sum()))
+    nvis = int(vis_o.sum())
+    # Rect agreement is bounded, not just reported.  The tile rects can only differ where an
+    # edge of the exact extent lies within the GPU's outward padding (h 2^-10 + 2^-7 px) of a 16-px tile boundary: for
+    # edge positions uniform modulo the tile that is pad / 16 per edge, four edges per Gaussian (fewer when clipped by
+    # the image).  Allowed: 3x that expectation + 5 sigma + 2.
+    hx0, hy0 = rho * np.sqrt(ref["cov2d"][both, 0]), rho * np.sqrt(ref["cov2d"][both, 2])
+    expected = float(np.sum(2 * ((hx0 + hy0) * 2.0 ** -10 + 2 * 2.0 ** -7) / 16.0))
+    assert mism <= 3 * expected + 5 * np.sqrt(expected) + 2, (mism, expected, nvis)
+    # Gaussians only the GPU keeps: footprints whose exact extent covers no pixel centre but whose padded extent does
+    assert extra <= 1e-2 * nvis + 2, (extra, nvis)
+    return dict(extra_visible=extra, rect_mismatch=mism, visible=nvis)
 
 
 def check_binning(oracle, got, cam):
@@ -128,7 +141,7 @@ def check_grads(ref, got, names=("g_means", "g_scales", "g_quats", "g_opacities"
     return errs
 
 
-def full_check(oracle, gpu, sc, seed, gA=False):
+def full_check(oracle, gpu, sc, seed, gA=False, grad_names=("g_means", "g_scales", "g_quats", "g_opacities", "g_sh", "g_twist")):
     cam = sc.camera
     gC, gD = scenes.upstream_gradients(seed, cam.width, cam.height)
     gAa = scenes.upstream_gradients(seed + 1, cam.width, cam.height)[1] if gA else None
@@ -137,12 +150,13 @@ def full_check(oracle, gpu, sc, seed, gA=False):
     info = check_features(oracle, sc, ref, got, cam)
     info["instances"] = check_binning(oracle, got, cam)
     info["flagged"], info["img_err"] = check_image(ref, got)
-    info["grad_err"] = check_grads(ref, got)
+    info["grad_err"] = check_grads(ref, got, grad_names)
+    info["ref"], info["got"] = ref, got
     # culled Gaussians get exact zeros
     culled = ~((got["features"]["rect"][:, 2] > got["features"]["rect"][:, 0]))
     for k in ("g_means", "g_scales", "g_quats", "g_opacities", "g_sh"):
         assert not np.any(got[k][culled]), k
-    print(sc.name, info)
+    print(sc.name, {k: v for k, v in info.items() if k not in ("ref", "got")})
     return info
 
 
@@ -222,6 +236,46 @@ def test_config5_fused_two_views_accumulate(oracle, gpu):
         assert rel_l2(out[k].cpu().numpy(), acc[k]) <= TOL_GRAD, k
 
 
+def test_config5_fused_full_size_two_views(oracle, gpu):
+    """Config 5 at FULL size (2 M Gaussians = 4 Sim(3)-mapped submaps, 1200x680, SH3), two of the eight views: features,
+    bit-exact binning, image, and the gradients -- including the twist -- accumulated over the views with GS_ACCUMULATE
+    (rendered RGB and depth of G^fused; ~60 blended layers per pixel, lists of 500-750 per tile)."""
+    sc, cams = scenes.fused_scene(seed=50)
+    b, torch = gpu.binding, gpu.torch
+    W, H = cams[0].width, cams[0].height
+    ds = b.DeviceScene(sc)
+    out = ds.alloc_outputs(W, H)
+    names = ("g_means", "g_scales", "g_quats", "g_opacities", "g_sh", "g_twist")
+    acc = None
+    for j, v in enumerate((2, 7)):   # the heaviest view (986 k visible Gaussians) and the one bench.py reports last
+        cam = cams[v]
+        gC, gD = scenes.upstream_gradients(50 + v, W, H)
+        ref = oracle.forward_backward(sc, gC, gD, camera=cam)
+        for attempt in range(3):
+            try:
+                b.forward(gpu.ctx, ds, cam, out)
+                counts = gpu.ctx.gs_get_counts()
+                break
+            except b.GsError as e:
+                if e.code != -5 or attempt == 2:
+                    raise
+        got = dict(features=gpu.ctx.gs_get_features(), binning=gpu.ctx.gs_get_binning(), counts=counts)
+        info = check_features(oracle, sc, ref, got, cam)
+        info["instances"] = check_binning(oracle, got, cam)
+        assert info["instances"] > 1_000_000 and info["visible"] > 100_000
+        b.backward(gpu.ctx, out, torch.from_numpy(gC).cuda(), torch.from_numpy(gD).cuda(), None,
+                   flags=(b.GS_ACCUMULATE if j > 0 else 0), pose=True)
+        torch.cuda.synchronize()
+        gpu.ctx.gs_poll()
+        img = {k: out[k].cpu().numpy() for k in ("rgb", "depth", "alpha")}
+        info["flagged"], info["img_err"] = check_image(ref, img)
+        acc = {k: ref[k].copy() for k in names} if acc is None else {k: acc[k] + ref[k] for k in names}
+        print(sc.name, "view", v, info)
+        del ref, got
+    errs = check_grads(acc, {k: out[k].cpu().numpy() for k in names})
+    print(sc.name, "accumulated", errs)
+
+
 def test_edge_cases(oracle, gpu):
     b, torch = gpu.binding, gpu.torch
     base = scenes.tiny_scene()
@@ -255,6 +309,17 @@ def test_edge_cases(oracle, gpu):
     ties.means[:, :2] += np.random.default_rng(4).uniform(-0.3, 0.3, (N, 2)).astype(np.float32)
     info = full_check(oracle, gpu, ties, 5)
     assert info["instances"] == N * 5 * 3
+    # the same pile with IDENTICAL isotropic Gaussians (scales 2.0, identity quaternions): Sigma does not depend on the
+    # rotation, so dL/dq is exactly zero in the oracle and relative L2 is undefined -- bounded absolutely instead
+    # (|dL/dq| ~ |dL/ds| s for a generic Gaussian; here only rounding residue of that size times 2^-24 may remain)
+    iso = copy.copy(ties)
+    iso.scales = np.full((N, 3), 2.0, np.float32)
+    iso.quats = np.tile(np.array([[1.0, 0.0, 0.0, 0.0]], np.float32), (N, 1))
+    iso.name = "ties_isotropic"
+    info = full_check(oracle, gpu, iso, 5, grad_names=("g_means", "g_scales", "g_opacities", "g_sh", "g_twist"))
+    assert info["instances"] == N * 5 * 3
+    assert not np.any(info["ref"]["g_quats"])
+    assert np.linalg.norm(info["got"]["g_quats"]) <= 1e-4 * 2.0 * np.linalg.norm(info["ref"]["g_scales"])
 
 
 @pytest.mark.parametrize("N,spread", [(1500, 0.02), (3000, 0.02), (6000, 0.02), (12000, 0.02)])

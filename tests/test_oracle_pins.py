@@ -283,10 +283,11 @@ def test_transmittance_monotone_and_colour_in_hull(oracle):
 # ------------------------------------------------------------------------------------------------------------------
 # hand-built one-pixel stacks: termination rule Q3(b), clamp gradient Q2, alpha threshold Q1
 # ------------------------------------------------------------------------------------------------------------------
-def _stack(oracle, alphas, cols, zs, opt=None, gC=(1.0, 0.0, 0.0), gD=0.0, bg=(0, 0, 0)):
-    """Gaussians centred on the single pixel (0,0) of a 1x1 image with G = 1 there, so alpha_i = min(.99, o_i)."""
+def _stack(oracle, alphas, cols, zs, opt=None, gC=(1.0, 0.0, 0.0), gD=0.0, bg=(0, 0, 0), mean2d=None):
+    """Gaussians centred on the single pixel (0,0) of a 1x1 image with G = 1 there, so alpha_i = min(.99, o_i)
+    (`mean2d` moves the centres: unit conic, so G = exp(-|mean|^2 / 2) at the pixel)."""
     n = len(alphas)
-    feat = dict(visible=np.ones(n, np.uint8), mean2d=np.zeros((n, 2)), cov2d=np.tile([[1.0, 0, 1.0]], (n, 1)),
+    feat = dict(visible=np.ones(n, np.uint8), mean2d=np.zeros((n, 2)) if mean2d is None else np.asarray(mean2d, float).reshape(n, 2), cov2d=np.tile([[1.0, 0, 1.0]], (n, 1)),
                 conic=np.tile([[1.0, 0, 1.0]], (n, 1)), color=np.asarray(cols, float).reshape(n, 3),
                 z=np.asarray(zs, float), z32=np.asarray(zs, np.float32))
     cam = types.SimpleNamespace(width=1, height=1, fx=1.0, fy=1.0, cx=0.0, cy=0.0, near_z=0.2,
@@ -339,6 +340,48 @@ def test_alpha_threshold_and_clamp_gradient(oracle):
     assert np.isclose(r["g_opac"][0], w1 - w2 * 0.6) and np.isclose(r["g_opac"][1], w2 * 0.7)
 
 
+def test_margin_values_by_hand(oracle):
+    """`margin` (C6) decides which pixels the GPU parity tests hold to 1e-5 and which to 1e-2, so its value
+    is pinned on one-pixel stacks where it can be computed by hand:
+    margin = min( min_i |alpha_i / (1/255) - 1| over evaluated Gaussians, |T / 1e-4 - 1| at every exit test )."""
+    # one Gaussian just above the alpha threshold: alpha = (1 + 3e-5)/255 -> 3e-5 (the exit test gives |1/1e-4 - 1|)
+    r = _stack(oracle, [(1 + 3e-5) / 255], [[1, 1, 1]], [1])
+    assert r["n_blended"][0, 0] == 1 and np.isclose(r["margin"][0, 0], 3e-5, rtol=1e-9, atol=0)
+    # just below (opacity 0.5, pixel at the distance where o G = (1 - 3e-5)/255, inside the oracle's padded box):
+    # skipped, and the margin is the same distance on the other side
+    d = np.sqrt(-2.0 * np.log((1 - 3e-5) / 255 / 0.5))
+    r = _stack(oracle, [0.5], [[1, 1, 1]], [1], mean2d=[[d, 0.0]])
+    assert r["n_blended"][0, 0] == 0 and np.isclose(r["margin"][0, 0], 3e-5, rtol=1e-6, atol=0)
+    r = _stack(oracle, [0.5], [[1, 1, 1]], [1], mean2d=[[0.0, -np.sqrt(-2.0 * np.log((1 + 3e-5) / 255 / 0.5))]])
+    assert r["n_blended"][0, 0] == 1 and np.isclose(r["margin"][0, 0], 3e-5, rtol=1e-6, atol=0)
+    # a far-from-threshold Gaussian: alpha = 0.5 -> |127.5 - 1| from the alpha test, |1e4 - 1| from the exit test
+    r = _stack(oracle, [0.5], [[1, 1, 1]], [1])
+    assert np.isclose(r["margin"][0, 0], 126.5, rtol=1e-12)
+    # transmittance in front of the third entry = 1e-4 (1 +- delta): margin = delta; + side blends it, - side exits
+    opt = oracle.Options(alpha_max=0.99999)
+    for delta, blended in ((+1e-3, 3), (-1e-3, 2), (+2.5e-5, 3), (-2.5e-5, 2)):
+        a2 = 1.0 - 1e-3 * (1.0 + delta)      # (1 - 0.9)(1 - a2) = 1e-4 (1 + delta)
+        r = _stack(oracle, [0.9, a2, 0.5], [[1, 0, 0], [0, 1, 0], [0, 0, 1]], [1, 2, 3], opt=opt)
+        T3 = (1.0 - 0.9) * (1.0 - a2)
+        assert r["n_blended"][0, 0] == blended
+        assert np.isclose(r["margin"][0, 0], abs(T3 / 1e-4 - 1.0), rtol=1e-9) and np.isclose(r["margin"][0, 0], abs(delta), rtol=1e-6)
+    # the exit test is only taken for Gaussians that pass the alpha test: a sub-threshold Gaussian at T ~ 1e-4 adds
+    # its alpha distance, not its T distance
+    d = np.sqrt(-2.0 * np.log(0.0039 / 0.5))   # third Gaussian: opacity 0.5, alpha = 0.0039 < 1/255 at the pixel
+    r = _stack(oracle, [0.9, 1.0 - 1e-3 * (1 + 1e-3), 0.5], [[1, 0, 0]] * 3, [1, 2, 3], opt=opt, mean2d=[[0, 0], [0, 0], [d, 0]])
+    assert r["n_blended"][0, 0] == 2 and np.isclose(r["margin"][0, 0], abs(0.0039 * 255 - 1.0), rtol=1e-6)
+    # a pixel that no Gaussian reaches: +inf (empty list), and >= 1 - tiny when the only Gaussian is far away
+    r = _stack(oracle, [], np.zeros((0, 3)), [])
+    assert np.isinf(r["margin"][0, 0]) and r["margin"][0, 0] > 0
+    n = 1
+    feat = dict(visible=np.ones(n, np.uint8), mean2d=np.full((n, 2), 40.0), cov2d=np.tile([[1.0, 0, 1.0]], (n, 1)),
+                conic=np.tile([[1.0, 0, 1.0]], (n, 1)), color=np.ones((n, 3)), z=np.ones(n), z32=np.ones(n, np.float32))
+    cam = types.SimpleNamespace(width=1, height=1, fx=1.0, fy=1.0, cx=0.0, cy=0.0, near_z=0.2, T_cw=scenes.identity_pose())
+    for brute in (False, True):
+        r = oracle.render(feat, np.array([0.9]), cam, np.zeros(3), oracle.Options(brute_force=brute))
+        assert r["n_blended"][0, 0] == 0 and r["margin"][0, 0] >= 1.0 - 1e-12
+
+
 # ------------------------------------------------------------------------------------------------------------------
 # analytic gradients vs central finite differences (pin 4), incl. the pose; pose <-> means consistency
 # ------------------------------------------------------------------------------------------------------------------
@@ -371,8 +414,8 @@ def test_gradients_match_central_finite_differences(oracle, cutoffs):
     feat = oracle.preprocess(sc, opt)
     img = oracle.render(feat, sc.opacities, sc.camera, sc.bg, opt, gC, gD, gA)
     g = oracle.preprocess_bwd(sc, img, opt)
-    if cutoffs:
-        assert (img["n_blended"] < feat["visible"].sum()).any() or True
+    if cutoffs:  # the cut-offs are live in this scene: some pixel blends fewer Gaussians than are visible
+        assert (img["n_blended"] < feat["visible"].sum()).any()
     names = dict(means="g_means", scales="g_scales", quats="g_quats", opacities="g_opacities", sh="g_sh")
     for pname, gname in names.items():
         base = getattr(sc, pname)
