@@ -81,7 +81,7 @@ GS_API int gs_destroy(gs_ctx* ctx);
 GS_API const char* gs_last_error(const gs_ctx* ctx);
 
 /* Step a1 -- EWA projection, conic, screen extent, colour (oracle reading C1 steps 1-6, 8).
- *   N            number of Gaussians (0 <= N < 2^24: sorted list entries carry index << 8 | region mask)
+ *   N            number of Gaussians (0 <= N < 2^24: sorted list entries carry slot << 8 | region mask)
  *   sh_degree    0..3; K = (sh_degree+1)^2 coefficients per channel
  *   means        [N,3]  world-space centres mu
  *   scales       [N,3]  ACTIVATED scales s > 0  (Sigma = R diag(s)^2 R^T)
@@ -97,10 +97,15 @@ GS_API int gs_preprocess(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, co
                   const float* quats, const float* opacities, const float* sh, const gs_camera* cam,
                   const float* T_cw_dev);
 
-/* Steps a2-a5 -- prefix sum of tiles touched, duplication into (tile id << 32 | depth bits, Gaussian index)
- * instances, stable radix sort, per-tile ranges.  Order inside a tile: depth key, then Gaussian index (Q13).
+/* Steps a2-a5 -- per-tile instance lists ordered by (depth key, Gaussian index)  (Q13).  The sort on (tile id, depth
+ * bits, index) keys is split MSD-first: counting pass on the tile digit (per-tile counts by gs_preprocess, multi-CTA
+ * prefix sum = the per-tile ranges, duplication into tile buckets with an 8-bit mask of the 8x4-pixel regions of the
+ * tile the Gaussian can reach), then a register-resident bitonic sort of every bucket on its unique 64-bit keys: the
+ * result is THE (tile, depth, index) order, bit for bit (DESIGN.md section 6 records the measured radix alternatives).
  * The first call after gs_create (or after N / the image size changed) synchronises once to size the instance
- * buffers; later calls are asynchronous and report an overflow through GS_E_OVERFLOW on a later call. */
+ * buffers; later calls are asynchronous and report an overflow through GS_E_OVERFLOW on a later call.
+ * The prefix-sum kernel exchanges per-CTA totals through flags its CTAs spin on: it is launched cooperatively
+ * (all of its <= 128 CTAs are guaranteed co-resident; GS_E_CUDA if the device cannot hold them, e.g. under MPS limits). */
 GS_API int gs_bin_tiles(gs_ctx* ctx, void* stream);
 
 /* Step a6 -- per-tile front-to-back compositing (oracle reading C1 step 7).
@@ -108,7 +113,8 @@ GS_API int gs_bin_tiles(gs_ctx* ctx, void* stream);
  *   rgb    [3,H,W]; depth [H,W] = sum z_c alpha T (un-normalised, Q8); alpha [H,W] = 1 - T_final.  Any may be NULL. */
 GS_API int gs_rasterize_fwd(gs_ctx* ctx, void* stream, const float* bg, float* rgb, float* depth, float* alpha);
 
-/* Steps a8-a9 -- back-to-front per-pixel backward (warp-reduced, then global atomics into per-Gaussian 2-D
+/* Steps a8-a9 -- back-to-front per-pixel backward (per-Gaussian sums reduced over the 32 pixels of a warp's region
+ * through shared memory, then one coalesced set of global RED.ADD per (region, Gaussian) into per-Gaussian 2-D
  * gradients), then the per-Gaussian chain rule (oracle readings C2, C3).
  *   d_rgb [3,H,W], d_depth [H,W] (NULL = 0), d_alpha [H,W] (NULL = 0): upstream gradients of the three outputs
  *   flags: GS_ACCUMULATE, GS_POSE_ONLY
@@ -145,8 +151,11 @@ GS_API int gs_profile_enable(gs_ctx* ctx, int on);
 GS_API int gs_profile_read(gs_ctx* ctx, float* ms);
 /* Number of CUDA kernels this context has launched so far (HOST counter). */
 GS_API int gs_get_launch_count(gs_ctx* ctx, uint64_t* n);
-/* Workload of the last forward (SYNCHRONISES): HOST uint64[4] = { evaluated (pixel, Gaussian) pairs with per-pixel
- * exit, blended pairs, sum over pixels of the last blended list position, sum over tiles of list length * pixels }. */
+/* Workload of the last forward (SYNCHRONISES; re-walks the lists with the forward's own decisions): HOST
+ * uint64[GS_NUM_WORKLOAD] = { E: (pixel, Gaussian) pairs evaluated while the pixel was still alive, over the (region,
+ * Gaussian) entries the region masks keep; C: blended pairs; L: sum over pixels of the last blended list position;
+ * sum over pixels of their tile's list length; R: relevant (8x4 region, Gaussian) entries walked by the forward }. */
+#define GS_NUM_WORKLOAD 5
 GS_API int gs_get_workload(gs_ctx* ctx, void* stream, uint64_t* out);
 
 /* ---- auxiliary kernels outside the five-call contract (losses of configs 2 and 4, on-device pose step) ---------- */
@@ -178,6 +187,29 @@ GS_API int gs_loss_iso(void* stream, int64_t N, const float* scales, float lambd
  * Asynchronous on `stream`.  GS_E_INVALID on null pointers, s <= 0 or misaligned quaternions. */
 GS_API int gs_sim3_apply(void* stream, int64_t N, float s, const float* R, const float* t, const float* means,
                          const float* scales, const float* quats, float* means_out, float* scales_out, float* quats_out);
+
+/* ---- measured machine peaks: the denominators of bench.py's roofline entries -------- */
+/* Runs small synthetic kernels on `device` (allocates and frees ~2 GiB, synchronises; ~0.2 s) and fills HOST double
+ * out[GS_NUM_PEAKS]:  FP32 FMA lane rate (T lane-FMA/s; x2 = TFLOP/s), mixed FFMA+integer issue rate (T warp
+ * instructions/s), MUFU.EX2 rate (T lanes/s), shared-memory load rates in T warp-level LDS/s (128-bit broadcast = how the
+ * compositing kernels read a Gaussian record; 128-bit conflict-free; 32- and 64-bit broadcast), L2 RED.ADD.F32 rate
+ * (G lane-adds/s on 128-byte rows), HBM read / write / copy (GB/s, 1 GiB streams), SM count and maximum SM clock (MHz).
+ * None of the method's arithmetic is involved.  GS_E_NOMEM if the buffers cannot be allocated. */
+#define GS_PEAK_FMA_TLANES 0
+#define GS_PEAK_ISSUE_TWARP 1
+#define GS_PEAK_EX2_TLANES 2
+#define GS_PEAK_LDS128_BCAST_TWARP 3
+#define GS_PEAK_LDS128_TWARP 4
+#define GS_PEAK_LDS32_BCAST_TWARP 5
+#define GS_PEAK_LDS64_BCAST_TWARP 6
+#define GS_PEAK_RED_GLANES 7
+#define GS_PEAK_HBM_READ_GBS 8
+#define GS_PEAK_HBM_WRITE_GBS 9
+#define GS_PEAK_HBM_COPY_GBS 10
+#define GS_PEAK_SM_COUNT 11
+#define GS_PEAK_SM_MHZ_MAX 12
+#define GS_NUM_PEAKS 13
+GS_API int gs_measure_peaks(int device, void* stream, double* out);
 
 /* ---- host-buffer convenience (bench.py "e2e"): one whole fwd+bwd iteration with HOST arrays -------------------- */
 /* Copies the parameters host->device, runs the five steps with the given upstream gradients (HOST), copies the image

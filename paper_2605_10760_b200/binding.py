@@ -22,7 +22,9 @@ STATUS = {0: "GS_OK", -1: "GS_E_INVALID", -2: "GS_E_ORDER", -3: "GS_E_CUDA", -4:
 EXPORTS = ["gs_create", "gs_destroy", "gs_last_error", "gs_preprocess", "gs_bin_tiles", "gs_rasterize_fwd",
            "gs_rasterize_bwd", "gs_pose_grad", "gs_get_counts", "gs_get_binning", "gs_get_features", "gs_poll",
            "gs_aux_l1_grad", "gs_aux_pose_step", "gs_fwd_bwd_host", "gs_profile_enable", "gs_profile_read",
-           "gs_get_launch_count", "gs_get_workload", "gs_loss_map", "gs_loss_iso", "gs_sim3_apply"]
+           "gs_get_launch_count", "gs_get_workload", "gs_loss_map", "gs_loss_iso", "gs_sim3_apply", "gs_measure_peaks"]
+PEAKS = ["fma_tlanes", "issue_twarp", "ex2_tlanes", "lds128_bcast_twarp", "lds128_twarp", "lds32_bcast_twarp",
+         "lds64_bcast_twarp", "red_glanes", "hbm_read_gbs", "hbm_write_gbs", "hbm_copy_gbs", "sm_count", "sm_mhz_max"]
 STAGES = ["preprocess", "tile_scan", "emit", "tile_sort", "raster_fwd", "raster_bwd", "gauss_bwd", "pose_grad"]
 
 
@@ -68,7 +70,8 @@ def load_library():
     lib.gs_profile_enable.argtypes = [vp, C.c_int]
     lib.gs_profile_read.argtypes = [vp, C.POINTER(f * 8)]
     lib.gs_get_launch_count.argtypes = [vp, C.POINTER(C.c_uint64)]
-    lib.gs_get_workload.argtypes = [vp, vp, C.POINTER(C.c_uint64 * 4)]
+    lib.gs_get_workload.argtypes = [vp, vp, C.POINTER(C.c_uint64 * 5)]
+    lib.gs_measure_peaks.argtypes = [C.c_int, vp, C.POINTER(C.c_double * len(PEAKS))]
     lib.gs_fwd_bwd_host.argtypes = [vp, vp, i64, C.c_int, vp, vp, vp, vp, vp, C.POINTER(gs_camera), C.POINTER(f * 3)] + [vp] * 11
     for name in EXPORTS:
         if name != "gs_last_error":
@@ -228,9 +231,10 @@ class Context:
         return int(n.value)
 
     def gs_get_workload(self, stream=None) -> dict:
-        w = (C.c_uint64 * 4)()
+        w = (C.c_uint64 * 5)()
         self._check(self.lib.gs_get_workload(self._h, _stream(stream), C.byref(w)))
-        return dict(evaluated=int(w[0]), blended=int(w[1]), last_pos_sum=int(w[2]), list_len_x_pixels=int(w[3]))
+        return dict(evaluated=int(w[0]), blended=int(w[1]), last_pos_sum=int(w[2]), list_len_x_pixels=int(w[3]),
+                    region_entries=int(w[4]))
 
     # -- host-buffer path (numpy arrays in / out; copies inside) ---------------------------------------------------
     def gs_fwd_bwd_host(self, scene_arrays, sh_degree, cam, bg, d_rgb, d_depth, out, stream=None):
@@ -294,6 +298,15 @@ def gs_sim3_apply(s, R, t, means, scales, quats, means_out=None, scales_out=None
                                       _ptr(scales, f32), _ptr(quats, f32), _ptr(mo, f32), _ptr(so, f32), _ptr(qo, f32))
     if rc != 0:
         raise GsError(rc, "gs_sim3_apply")
+
+
+def gs_measure_peaks(device: int = 0, stream=None) -> dict:
+    """Measured machine peaks (include/gs.h): the roofline denominators.  Synchronous, ~0.2 s."""
+    out = (C.c_double * len(PEAKS))()
+    rc = load_library().gs_measure_peaks(int(device), _stream(stream), C.byref(out))
+    if rc != 0:
+        raise GsError(rc, "gs_measure_peaks")
+    return {k: float(out[i]) for i, k in enumerate(PEAKS)}
 
 
 def gs_aux_pose_step(T_cw_dev, g_twist, step, stream=None):

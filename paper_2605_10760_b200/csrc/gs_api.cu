@@ -35,10 +35,11 @@ __global__ void features_export_kernel(int64_t N, const float4* __restrict__ fea
     mean2d[2 * i] = vis ? (double)((pk << 16) >> 16) + (double)f0.x : 0.0;
     mean2d[2 * i + 1] = vis ? (double)(pk >> 16) + (double)f0.y : 0.0;
   }
-  if (conic) {
-    conic[3 * i] = (float)(-2.0 * ln2 * (double)f1.x);
-    conic[3 * i + 1] = (float)(-ln2 * (double)f1.y);
-    conic[3 * i + 2] = (float)(-2.0 * ln2 * (double)f1.z);
+  if (conic) {  // 0.5 log2(e) Q = L L^T  (gs_internal.cuh)
+    const double l11 = f1.x, l21 = f1.y, l22 = f1.z;
+    conic[3 * i] = (float)(2.0 * ln2 * l11 * l11);
+    conic[3 * i + 1] = (float)(2.0 * ln2 * l11 * l21);
+    conic[3 * i + 2] = (float)(2.0 * ln2 * (l21 * l21 + l22 * l22));
   }
   if (color) { color[3 * i] = f2.x; color[3 * i + 1] = f2.y; color[3 * i + 2] = f2.z; }
   if (depth) depth[i] = f2.w;
@@ -153,7 +154,6 @@ int gs_create(gs_ctx** out, int device) {
   gs_ctx* ctx = new (std::nothrow) gs_ctx();
   if (!ctx) return GS_E_NOMEM;
   ctx->device = device;
-  if (const char* e = getenv("GS_RASTER_FWD")) ctx->shape_fwd = atoi(e);
   bool ok = cudaSetDevice(device) == cudaSuccess;
   ok = ok && alloc_header(ctx, 0) == GS_OK;
   ok = ok && cudaHostAlloc((void**)&ctx->mailbox, sizeof(Counts), cudaHostAllocMapped) == cudaSuccess;

@@ -4,14 +4,16 @@
 // keys plus a serial per-thread duplication cost 112 + 40 us of a 614 us iteration): the sort on (tile, depth, index)
 // keys is split MSD-first.
 //   1. gs_preprocess counts the instances of every tile (atomics on tile_count) while it computes the rects.
-//   2. tile_scan_kernel (one CTA): exclusive prefix sum over the tile counts = the per-tile ranges (step a5 comes for
-//      free), the instance total / overflow flag, and the tile order by descending list length.
-//   3. emit_kernel: every visible Gaussian appends (depth bits << 32 | index) to the bucket of each tile of its rect
-//      (atomic cursor per tile) -- a counting-sort pass on the tile digit; the order inside a bucket is arbitrary.
-//   4. tile_sort_kernel: every bucket is sorted by its 64-bit key in shared memory (bitonic network).  The keys are
-//      unique (the index is part of the key), so the result is THE (tile, depth bits, index) order, bit for bit,
-//      whatever the arrival order was.  Buckets beyond the shared-memory capacity are sorted in global memory.
-// Integer work only.  Bytes: 8 I (emit) + 8 I (sort read) + 12 I (sorted keys + ids) vs (8 + 24 * 6) I before.
+//   2. tile_scan_kernel (multi-CTA, single pass, cooperative launch): exclusive prefix sum over the tile counts = the
+//      per-tile ranges (step a5 comes for free), the instance total / overflow flag, and the tile order by descending
+//      list-length class.
+//   3. emit_kernel: every visible Gaussian appends (depth bits << 32 | index << 8 | region mask) to the bucket of each
+//      tile of its rect (atomic cursor per tile) -- a counting-sort pass on the tile digit; the order inside a bucket is
+//      arbitrary at this point.
+//   4. tile_sort_kernel / tile_sort_large_kernel: every bucket is sorted on its 64-bit keys by a register-resident
+//      bitonic network.  The keys are unique (the index is part of the key), so the result is THE (tile, depth bits,
+//      index) order, bit for bit, whatever the arrival order was.  Buckets beyond 8192 keys are sorted in global memory.
+// Integer work only.  Bytes: 8 I (emit) + 8 I (sort read) + 12 I (sorted keys + list entries) vs (8 + 24 * 6) I before.
 #include "gs_internal.cuh"
 #include "gs_raster.cuh"
 
@@ -19,12 +21,12 @@ namespace gs {
 
 constexpr int kSmallSortMax = 255;  // buckets up to this size are sorted by one warp (whole length/8 classes of the tile order)
 constexpr int kMidSortMax = 2047;   // buckets up to this size are sorted by one CTA of 4 warps; beyond: the large kernel
-constexpr int kLargeSort = 8192;
-// tile_count / tile_cursor are strided by 32 words: one counter per 128-byte line, so that the atomics of different
-// tiles are served by different L2 lines (3225 adjacent counters would share ~100 lines and serialise there)   // up to this size: 512-thread CTA, 64 KB dynamic shared memory; beyond: global memory
+constexpr int kLargeSort = 8192;    // up to this size: 512-thread CTA, 64 KB dynamic shared memory; beyond: global memory
+// tile_count / tile_cursor are strided by 32 words (kCtrStride): one counter per 128-byte line, so that the atomics of
+// different tiles are served by different L2 lines (3225 adjacent counters would share ~100 lines and serialise there)
 
 // ---------------------------------------------------------------------------------------------------------------
-// a2 + a5: prefix sum over the tile counts, ranges, totals, overflow flag, LPT tile order.  One CTA of 1024 threads.
+// a2 + a5: prefix sum over the tile counts, ranges, totals, overflow flag, LPT tile order.
 // ---------------------------------------------------------------------------------------------------------------
 // Multi-CTA single-pass scan.  (Measured with clock64 on the one-CTA versions: ~20 k cycles whatever the algorithm --
 // shared-memory atomics, L2 atomics or none -- because the 3225 strided counter loads and the ~3 x 3225 scattered
@@ -32,7 +34,8 @@ constexpr int kLargeSort = 8192;
 // tiles per thread.  The block scan carries 9 words per thread: the instance count and 16 length-class counters packed
 // as 16-bit fields, so one scan yields the per-tile ranges AND a stable counting sort of the tiles by length class
 // (= the tile order); no atomics.  Every CTA publishes its 17 unpacked totals with an epoch flag and reads those of
-// all the others (at most 128 CTAs, all co-resident), i.e. one L2 round trip instead of a second kernel.
+// all the others (at most 128 CTAs; the launch is COOPERATIVE, so the runtime guarantees they are all co-resident and a
+// CTA spinning on a sibling's flag cannot starve it), i.e. one L2 round trip instead of a second kernel.
 constexpr int kScanT = 256;      // threads per CTA
 constexpr int kScanWords = 9;    // [0] instances, [1..8] 16 class counters, two per word
 constexpr int kScanCls = 16;
@@ -180,37 +183,6 @@ tile_scan_kernel(int tiles, const uint32_t* __restrict__ tile_count, uint32_t* _
 constexpr int kEmitG = 32;    // visible Gaussians per CTA
 constexpr int kEmitT = 128;   // threads per CTA
 
-// Which of the eight 8x4-pixel regions of tile (tx, ty) can the ellipse {alpha >= 1/255} of this Gaussian reach?  The
-// test is the one the compositing kernels used to repeat per (region, batch) in their phase 1 (exact maximum of the
-// concave power over the region rectangle, gs_raster.cuh), done ONCE per instance here: profiles/r1_v4 -- phase 1 was
-// 27 % of the forward's instructions and its staging of never-relevant records 2/3 of the cp.async traffic.
-__device__ __forceinline__ uint32_t region_mask(const float4& f0, const float4& f1, int tx, int ty) {
-  GaussReg g;  // decoded once, relative to the tile origin; the reciprocals are shared by the eight rectangles
-  decode_gauss(f0, f1, tx * GS_TILE, ty * GS_TILE, g);
-  const float nbc = -g.B * rcp_approx(2.f * g.C), nba = -g.B * rcp_approx(2.f * g.A);
-  const float thr = g.thr - 1e-3f;
-  uint32_t m = 0;
-#pragma unroll
-  for (int sub = 0; sub < 8; ++sub) {
-    const float x0 = (float)((sub % 2) * 8) - g.mx, x1 = x0 + 7.f, y0 = (float)((sub / 2) * 4) - g.my, y1 = y0 + 3.f;
-    float best = 0.f;
-    if (!(x0 <= 0.f && x1 >= 0.f && y0 <= 0.f && y1 >= 0.f)) {
-      best = -INFINITY;
-#pragma unroll
-      for (int e = 0; e < 2; ++e) {
-        const float dxe = e ? x1 : x0;
-        const float dys = fminf(fmaxf(nbc * dxe, y0), y1);
-        best = fmaxf(best, g.A * dxe * dxe + g.B * dxe * dys + g.C * dys * dys);
-        const float dye = e ? y1 : y0;
-        const float dxs = fminf(fmaxf(nba * dye, x0), x1);
-        best = fmaxf(best, g.A * dxs * dxs + g.B * dxs * dye + g.C * dye * dye);
-      }
-    }
-    m |= (best >= thr) ? (1u << sub) : 0u;
-  }
-  return m;
-}
-
 __global__ void __launch_bounds__(kEmitT)
 emit_kernel(const uint4* __restrict__ vis_rec, const float4* __restrict__ feat, int tiles_x,
             uint32_t* __restrict__ tile_cursor, const Counts* __restrict__ counts, uint64_t* __restrict__ keys) {
@@ -267,7 +239,13 @@ emit_kernel(const uint4* __restrict__ vis_rec, const float4* __restrict__ feat, 
         const uint32_t local = item - s_excl[owner], w = s_w[owner], xy = s_xy[owner];
         const uint32_t ty = (xy >> 16) + local / w, tx = (xy & 0xffffu) + local % w;
         cur[u] = &tile_cursor[(size_t)(ty * tiles_x + tx) * kCtrStride];
-        kk[u] = s_key[owner] | (uint64_t)region_mask(s_f0[owner], s_f1[owner], (int)tx, (int)ty);
+        // 8-bit mask of the tile's 8x4-pixel regions the ellipse {alpha >= 1/255} can reach (gs_raster.cuh), decided
+        // ONCE per instance here instead of per (region, batch) in both compositing kernels
+        const float4 f0 = s_f0[owner], f1 = s_f1[owner];
+        const int pk = __float_as_int(f0.z);
+        const float mx = (float)(((pk << 16) >> 16) - (int)tx * GS_TILE) + f0.x;
+        const float my = (float)((pk >> 16) - (int)ty * GS_TILE) + f0.y;
+        kk[u] = s_key[owner] | (uint64_t)region_mask(f1.x, f1.y, f1.z, f0.w, mx, my);
       }
     }
 #pragma unroll
@@ -532,15 +510,19 @@ static int run_tile_scan(gs_ctx* ctx, cudaStream_t s) {
   uint32_t* flags = ctx->scan_ws + kScanMaxCta * kScanAgg;
   const uint32_t epoch = ++ctx->scan_epoch;
   const int nb1 = (int)div_up(tiles, kScanT);
-  if (nb1 <= kScanMaxCta) {
-    tile_scan_kernel<1><<<nb1, kScanT, 0, s>>>(tiles, ctx->tile_count, ctx->tile_cursor, ctx->ranges, ctx->tile_order, agg,
-                                               flags, epoch, ctx->cap_I, ctx->counts, ctx->mailbox_dev, ctx->seq);
-  } else {
-    const int nb8 = (int)div_up(tiles, kScanT * 8);
-    if (nb8 > kScanMaxCta) return fail(ctx, GS_E_INVALID, "gs_bin_tiles: more than 262144 tiles");
-    tile_scan_kernel<8><<<nb8, kScanT, 0, s>>>(tiles, ctx->tile_count, ctx->tile_cursor, ctx->ranges, ctx->tile_order, agg,
-                                               flags, epoch, ctx->cap_I, ctx->counts, ctx->mailbox_dev, ctx->seq);
-  }
+  const int nb8 = (int)div_up(tiles, kScanT * 8);
+  if (nb8 > kScanMaxCta) return fail(ctx, GS_E_INVALID, "gs_bin_tiles: more than 262144 tiles");
+  int tiles_arg = tiles;
+  const uint32_t* count_arg = ctx->tile_count;
+  int64_t cap_arg = ctx->cap_I;
+  uint32_t seq_arg = ctx->seq, epoch_arg = epoch;
+  void* args[] = {&tiles_arg, &count_arg, &ctx->tile_cursor, &ctx->ranges, &ctx->tile_order, &agg, &flags, &epoch_arg,
+                  &cap_arg, &ctx->counts, &ctx->mailbox_dev, &seq_arg};
+  // cooperative launch: co-residency of the CTAs that wait on each other's flags is guaranteed by the runtime
+  if (nb1 <= kScanMaxCta)
+    GS_CUDA(cudaLaunchCooperativeKernel((const void*)tile_scan_kernel<1>, dim3(nb1), dim3(kScanT), args, 0, s));
+  else
+    GS_CUDA(cudaLaunchCooperativeKernel((const void*)tile_scan_kernel<8>, dim3(nb8), dim3(kScanT), args, 0, s));
   GS_LAUNCH_CHECK("tile_scan_kernel");
   return GS_OK;
 }

@@ -54,11 +54,12 @@ gauss_bwd_kernel(int64_t N, const float* __restrict__ means, const float* __rest
     Proj<R> P;
     project_gaussian<R, false>(cam, T, mu0, mu1, mu2, s0, s1, s2, q.x, q.y, q.z, q.w, o, P);
     {
-      // The conic is taken from the forward's feature record (computed in fp64 by gs_preprocess, stored pre-scaled by
-      // -0.5 log2(e) / -log2(e)): the fp32 determinant cxx cyy - cxy^2 loses all digits for long thin footprints.
+      // The conic is taken from the forward's feature record (whitened Cholesky factor computed in fp64 by
+      // gs_preprocess: 0.5 log2(e) Q = L L^T): the fp32 determinant cxx cyy - cxy^2 loses all digits for long thin
+      // footprints.
       const float4 f1 = __ldg(feat + 3 * (size_t)kk + 1);
-      const R ln2 = (R)0.69314718055994531;
-      P.a = -(R)2 * ln2 * (R)f1.x; P.b = -ln2 * (R)f1.y; P.c = -(R)2 * ln2 * (R)f1.z;
+      const R ik = (R)(2.0 * 0.69314718055994531);  // 1 / (0.5 log2 e)
+      P.a = ik * (R)f1.x * (R)f1.x; P.b = ik * (R)f1.x * (R)f1.y; P.c = ik * ((R)f1.y * (R)f1.y + (R)f1.z * (R)f1.z);
     }
     const R W[9] = {T[0], T[1], T[2], T[4], T[5], T[6], T[8], T[9], T[10]};
     // ga.x, ga.y = sum gp dx, sum gp dy (moments about the mean); d power / d mean = -(Q d), ln2 * log2(e) = 1

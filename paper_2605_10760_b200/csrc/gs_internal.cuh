@@ -32,10 +32,11 @@ __device__ __forceinline__ void load_pose(const DevCam& cam, float* T) {
 
 // ---------------------------------------------------------------------------------------------------------------
 // Per-Gaussian feature record written by gs_preprocess and gathered by the rasteriser: 3 x float4 = 48 B.
-//   f0 = { mfx, mfy, bits(miy << 16 | mix & 0xffff), thr }  2-D mean = integer pixel (mix,miy) + fraction in [-0.5,0.5];
-//                               thr = -log2(255 opacity): alpha >= 1/255  <=>  power2 >= thr
-//   f1 = { A, B, C, opacity }   power2 = A dx^2 + B dx dy + C dy^2  (conic pre-scaled: A = -0.5 log2(e) a, B = -log2(e) b,
-//                               C = -0.5 log2(e) c), alpha = min(0.99, opacity * 2^power2)
+//   f0 = { mfx, mfy, bits(miy << 16 | mix & 0xffff), lo }  2-D mean = integer pixel (mix,miy) + fraction in [-0.5,0.5];
+//                               lo = log2(opacity)
+//   f1 = { l11, l21, l22, opacity }   L = sqrt(0.5 log2 e) chol(conic) (lower triangular, fp64 in gs_preprocess):
+//                               p2(d) = lo - (l11 dx + l21 dy)^2 - (l22 dy)^2,  alpha = min(0.99, 2^p2),
+//                               alpha >= 1/255  <=>  p2 >= -log2(255)            (gs_raster.cuh)
 //   f2 = { r, g, b, z_c }
 // ---------------------------------------------------------------------------------------------------------------
 constexpr int kFeatVec = 3;
@@ -55,7 +56,7 @@ struct alignas(16) Counts {
   uint32_t n_instances;  // total tile instances of the last scan (even if it overflowed)
   uint32_t overflow;     // 1 if n_instances > capacity: nothing was emitted and downstream kernels see 0 instances
   uint32_t seq;          // iteration number of the writer
-  uint32_t n_large;      // number of tiles whose list is longer than one 4-warp CTA sorts in registers (> 1023)
+  uint32_t n_large;      // number of tiles whose list is longer than one 4-warp CTA sorts in registers (> 2047)
   uint32_t n_mid;        // number of tiles whose list is longer than one warp sorts in registers (> 255; includes n_large)
 };
 
@@ -120,8 +121,6 @@ struct gs_ctx {
   gs::Counts* mailbox = nullptr;      // pinned host, mapped
   gs::Counts* mailbox_dev = nullptr;  // device alias of the mailbox
 
-  // region shape of the compositing kernels; tuning knobs GS_RASTER_FWD / GS_RASTER_BWD read by gs_create.
-  int shape_fwd = 0;  // 0: the branch-free 8 x 4 kernel; else the generic forward "NXNY": region per warp = (8 NX) x (4 NY) pixels (the backward is fixed at 8 x 4)
   uint32_t* tile_order = nullptr;      // [tiles] tile ids by descending list length (longest lists are scheduled first)
 
   // side stream: the zero fill of the dense gradient arrays overlaps the (ALU-bound) pixel backward

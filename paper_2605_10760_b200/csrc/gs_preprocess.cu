@@ -79,12 +79,15 @@ preprocess_kernel(int64_t N, const float* __restrict__ means, const float* __res
   // mean = integer pixel (two int16, clamped: a centre that far off-screen needs no sub-pixel precision) + fraction
   const double rmx = fmin(fmax(rint(P.mx), -32000.0), 32000.0);
   const double rmy = fmin(fmax(rint(P.my), -32000.0), 32000.0);
-  const double kl = 1.4426950408889634;  // log2(e)
+  // whitened conic (gs_raster.cuh): 0.5 log2(e) d^T Q d = u^2 + v^2, u = l11 dx + l21 dy, v = l22 dy; fp64 Cholesky,
+  // k c - l21^2 = k det(Q) / a > 0 for the positive-definite Q that passed the cull
+  const double kh = 0.5 * 1.4426950408889634;  // 0.5 log2(e)
+  const double l11 = sqrt(kh * P.a), l21 = kh * P.b / l11, l22 = sqrt(kh * (P.c - P.b * P.b / P.a));
   float4 f0, f1, f2;
   f0.x = (float)(P.mx - rmx); f0.y = (float)(P.my - rmy);
   f0.z = __int_as_float(((int)rmy << 16) | ((int)rmx & 0xffff));
-  f0.w = -log2f(255.f * o);  // alpha >= 1/255  <=>  power2 >= thr
-  f1.x = (float)(-0.5 * kl * P.a); f1.y = (float)(-kl * P.b); f1.z = (float)(-0.5 * kl * P.c); f1.w = o;
+  f0.w = (float)log2((double)o);
+  f1.x = (float)l11; f1.y = (float)l21; f1.z = (float)l22; f1.w = o;
   f2.x = fmaxf(col[0] + 0.5f, 0.f); f2.y = fmaxf(col[1] + 0.5f, 0.f); f2.z = fmaxf(col[2] + 0.5f, 0.f);
   f2.w = (float)P.z;
   const uint32_t dk = __float_as_uint(depth_key_f32(T, mu0, mu1, mu2));

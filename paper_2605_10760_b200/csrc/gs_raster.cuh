@@ -1,18 +1,35 @@
-// gs_raster.cuh -- pieces shared by the forward and backward compositing kernels (v2: one warp per tile region,
-// several interleaved pixels per lane).  The power evaluation MUST be the same instruction sequence in both kernels
-// (the backward re-takes the forward's alpha >= 1/255 decisions), so it is written with explicit rounding intrinsics
-// that the compiler cannot contract or re-associate differently per kernel.
+// gs_raster.cuh -- pieces shared by the binning masks and the forward / backward compositing kernels.
+//
+// The power of a Gaussian at a pixel is evaluated in WHITENED, REGION-LOCAL form ("precision"):
+//     p2 = lo - u^2 - v^2,   u = l11 x + l21 y + u0,   v = l22 y + v0,      alpha = min(0.99, 2^p2)
+// with (x, y) the pixel's coordinates inside the warp's 8x4 region (0..7, 0..3), L = sqrt(0.5 log2 e) chol(conic) from
+// gs_preprocess (fp64 there), lo = log2(opacity), and (u0, v0) = -L^T (mean - region origin) formed in fp64 when the
+// record is staged.  Every fp32 operand of the per-pixel arithmetic is then O(10) whatever the footprint's size or
+// anisotropy (the direct form A dx^2 + B dx dy + C dy^2 cancels terms of size |A| dx^2 -- measured 1e-3 image error on
+// config 5).  alpha >= 1/255 <=> p2 >= -log2(255): a constant, so neither the opacity nor a per-Gaussian threshold is
+// read in the pixel loop.  The sequence below MUST be the same instructions in the forward and in the backward (the
+// backward re-takes the forward's decisions), hence the explicit rounding intrinsics.
 #pragma once
 
 #include "gs_internal.cuh"
 
 namespace gs {
 
-constexpr int kWarpBatch = 32;  // Gaussians staged per round by one warp (one per lane)
+constexpr int kWarpBatch = 32;  // list entries examined per round by one warp (one per lane)
+constexpr unsigned kFull = 0xffffffffu;
+constexpr int kGroup = 4;       // relevant entries evaluated together in phase 2
+
+// -log2(255): alpha >= 1/255  <=>  p2 >= kPowerMin
+#define GS_POWER_MIN (-7.994353436858858f)
 
 __device__ __forceinline__ float ex2_approx(float x) {
   float y;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ float rcp_approx(float x) {
+  float y;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
 
@@ -26,83 +43,54 @@ __device__ __forceinline__ void cp_async_wait() {
   asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
 }
 
-// Pixel slots of a lane.  Lanes form an 8 (x) by 4 (y) grid; slot (kx, ky) of lane (lx, ly) is the pixel
-// (lx + 8 kx, ly + 4 ky) of the warp's region, kx < NX, ky < NY: the region is (8 NX) x (4 NY) pixels and a lane's
-// pixels are INTERLEAVED over it, so that the footprint of one Gaussian falls on few slots of many lanes (SIMT
-// efficiency) rather than on all slots of few lanes.  Slot index k = ky * NX + kx.
-
-// One staged Gaussian, decoded for a region with origin (ox, oy).
-struct GaussReg {
-  float mx, my;       // mean, region-local
-  float A, B, C, o;   // pre-scaled conic, opacity
-  float thr;          // power threshold: alpha >= 1/255 <=> power2 >= thr
-};
-
-__device__ __forceinline__ void decode_gauss(const float4& f0, const float4& f1, int ox, int oy, GaussReg& g) {
+// Staged record -> whitened record relative to the origin (ox, oy), in fp64 (exact integer part of the mean, exact
+// products with the fp32-rounded L; one rounding of u0, v0 at the end).  Also returns the origin-relative mean (fp32).
+__device__ __forceinline__ void decode_whitened(const float4& f0, const float4& f1, int ox, int oy, float& u0, float& v0,
+                                                float& mx, float& my) {
   const int pk = __float_as_int(f0.z);
-  g.mx = (float)(((pk << 16) >> 16) - ox) + f0.x;  // integer part minus origin is exact; fraction added in fp32
-  g.my = (float)((pk >> 16) - oy) + f0.y;
-  g.A = f1.x; g.B = f1.y; g.C = f1.z; g.o = f1.w;
-  g.thr = f0.w;
+  const double mxd = (double)(((pk << 16) >> 16) - ox) + (double)f0.x;
+  const double myd = (double)((pk >> 16) - oy) + (double)f0.y;
+  u0 = (float)(-((double)f1.x * mxd + (double)f1.y * myd));
+  v0 = (float)(-((double)f1.z * myd));
+  mx = (float)mxd;
+  my = (float)myd;
 }
 
-// power2 of every slot: p[ky*NX+kx] = dx (A dx + B dy) + C dy^2, with the products shared across rows / columns.
-// Explicit rounding intrinsics: the sequence is the same in every kernel that includes this header.
-template <int NX, int NY>
-__device__ __forceinline__ void eval_power(const GaussReg& g, float fx0, float fy0, float (&dx)[NX], float (&dy)[NY],
-                                           float (&p)[NX * NY]) {
-  float ax[NX], cy[NY];
+// p2 at the lane's pixel (fx0, fy0) of the region: five FFMA, no subtraction of large numbers
+__device__ __forceinline__ float eval_power(float u0, float v0, float l11, float l21, float l22, float lo, float fx0,
+                                            float fy0) {
+  const float u = __fmaf_rn(l11, fx0, __fmaf_rn(l21, fy0, u0));
+  const float v = __fmaf_rn(l22, fy0, v0);
+  return __fmaf_rn(-u, u, __fmaf_rn(-v, v, lo));
+}
+
+// Which of the eight 8x4-pixel regions of a 16x16 tile can the ellipse {p2 >= -log2(255)} reach?  Exact up to an
+// outward slack: per band of four pixel rows the ellipse's x-extent over the band is [xl, xr] (a convex set projects
+// to an interval, attained at the band-clamped extreme points), and a region is hit iff the interval meets the
+// region's columns.  (mx, my): mean relative to the tile origin.  ~120 instructions per (Gaussian, tile) instance;
+// the previous per-rectangle maximisation of the quadratic was ~500 and made the duplication kernel issue-bound.
+__device__ __forceinline__ uint32_t region_mask(float l11, float l21, float l22, float lo, float mx, float my) {
+  const float R2 = lo - GS_POWER_MIN + 0.02f;   // outward slack: 0.02 in the exponent, >> the fp32 error of this test
+  if (!(R2 > 0.f)) return 0u;
+  const float R = sqrtf(R2);
+  const float il22 = 1.f / l22, il11 = 1.f / l11;
+  const float hy = R * il22;                                       // half height of the ellipse
+  const float dyR = -l21 * R * rsqrtf(l21 * l21 + l22 * l22) * il22;  // row (relative to the mean) of the rightmost point
+  const float eps = 1e-3f + 1e-6f * fabsf(mx);
+  uint32_t m = 0;
 #pragma unroll
-  for (int kx = 0; kx < NX; ++kx) {
-    dx[kx] = __fsub_rn(fx0 + 8.f * kx, g.mx);
-    ax[kx] = __fmul_rn(g.A, dx[kx]);
+  for (int band = 0; band < 4; ++band) {
+    const float ya = (float)(4 * band) - my, yb = ya + 3.f;
+    const float lo_y = fmaxf(ya, -hy), hi_y = fminf(yb, hy);
+    if (lo_y > hi_y) continue;
+    const float dyr = fminf(fmaxf(dyR, lo_y), hi_y), dyl = fminf(fmaxf(-dyR, lo_y), hi_y);
+    const float vr = l22 * dyr, vl = l22 * dyl;
+    const float sr = sqrtf(fmaxf(R2 - vr * vr, 0.f)), sl = sqrtf(fmaxf(R2 - vl * vl, 0.f));
+    const float xr = mx + (sr - l21 * dyr) * il11 + eps, xl = mx - (sl + l21 * dyl) * il11 - eps;
+    if (xl <= 7.f && xr >= 0.f) m |= 1u << (2 * band);
+    if (xl <= 15.f && xr >= 8.f) m |= 2u << (2 * band);
   }
-#pragma unroll
-  for (int ky = 0; ky < NY; ++ky) {
-    dy[ky] = __fsub_rn(fy0 + 4.f * ky, g.my);
-    cy[ky] = __fmul_rn(__fmul_rn(g.C, dy[ky]), dy[ky]);
-  }
-#pragma unroll
-  for (int ky = 0; ky < NY; ++ky)
-#pragma unroll
-    for (int kx = 0; kx < NX; ++kx)
-      p[ky * NX + kx] = __fmaf_rn(dx[kx], __fmaf_rn(g.B, dy[ky], ax[kx]), cy[ky]);
-}
-
-// the same sequence for one pixel per lane (8x4 regions)
-__device__ __forceinline__ float eval_power1(float mx, float my, float A, float B, float C, float fx0, float fy0,
-                                             float& dx, float& dy) {
-  dx = __fsub_rn(fx0, mx);
-  dy = __fsub_rn(fy0, my);
-  return __fmaf_rn(dx, __fmaf_rn(B, dy, __fmul_rn(A, dx)), __fmul_rn(__fmul_rn(C, dy), dy));
-}
-
-__device__ __forceinline__ float rcp_approx(float x) {
-  float y;
-  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-  return y;
-}
-
-constexpr unsigned kFull = 0xffffffffu;
-constexpr int kGroup = 4;                    // Gaussians evaluated together in phase 2
-
-// Maximum of power2 over the continuous rectangle [0,xmax] x [0,ymax] (region-local), exact for the concave quadratic:
-// 0 if the centre is inside, else the largest of the four clamped edge maxima.
-__device__ __forceinline__ float region_max_power(const GaussReg& g, float xmax, float ymax) {
-  const float x0 = -g.mx, x1 = xmax - g.mx, y0 = -g.my, y1 = ymax - g.my;  // rectangle in centre-relative coordinates
-  if (x0 <= 0.f && x1 >= 0.f && y0 <= 0.f && y1 >= 0.f) return 0.f;
-  const float i2C = rcp_approx(2.f * g.C), i2A = rcp_approx(2.f * g.A);  // the test has 1e-3 of slack
-  float best = -INFINITY;
-#pragma unroll
-  for (int e = 0; e < 2; ++e) {
-    const float dxe = e ? x1 : x0;
-    const float dys = fminf(fmaxf(-g.B * dxe * i2C, y0), y1);
-    best = fmaxf(best, g.A * dxe * dxe + g.B * dxe * dys + g.C * dys * dys);
-    const float dye = e ? y1 : y0;
-    const float dxs = fminf(fmaxf(-g.B * dye * i2A, x0), x1);
-    best = fmaxf(best, g.A * dxs * dxs + g.B * dxs * dye + g.C * dye * dye);
-  }
-  return best;
+  return m;
 }
 
 }  // namespace gs

@@ -99,6 +99,7 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
   constexpr int RPT = 8;  // 8x4-pixel regions per 16x16 tile
   __shared__ __align__(16) float4 s_feat[2][(kWarpBatch + kGroup) * 3];  // records of the relevant entries, decoded in place
   __shared__ uint32_t s_tag[2][kWarpBatch];
+  __shared__ float2 s_mean[kWarpBatch + kGroup];  // region-local means of the current batch's entries (Gaussian phase)
   __shared__ __align__(16) float2 s_pair[kSlots * kPairRow];
   __shared__ __align__(16) float4 s_pix[32];
   const int lane = threadIdx.x;
@@ -167,15 +168,17 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
     if (nrel == 0) continue;
     const int lastb = (int)last - b * kWarpBatch;  // entries of this batch at positions < lastb were blended by this pixel
     float4* sf = s_feat[b & 1];
-    if (lane < nrel) {  // decode once per (region, Gaussian), in place: region-local mean
-      GaussReg g;
-      decode_gauss(sf[3 * lane], sf[3 * lane + 1], ox, oy, g);
-      sf[3 * lane] = make_float4(g.mx, g.my, g.A, g.B);
-      sf[3 * lane + 1] = make_float4(g.C, g.o, g.thr, __uint_as_float(s_tag[b & 1][lane]));
+    if (lane < nrel) {  // decode once per (region, Gaussian), in place: whitened region-local record (gs_raster.cuh)
+      const float4 f0 = sf[3 * lane], f1 = sf[3 * lane + 1];
+      float u0, v0, mx, my;
+      decode_whitened(f0, f1, ox, oy, u0, v0, mx, my);
+      sf[3 * lane] = make_float4(u0, v0, f1.x, f1.y);
+      sf[3 * lane + 1] = make_float4(f1.z, f0.w, __uint_as_float(s_tag[b & 1][lane]), 0.f);
+      s_mean[lane] = make_float2(mx, my);
     }
-    if (lane < kGroup) {  // padding records never pass: p >= NaN is false
+    if (lane < kGroup) {  // padding records never pass: lo = -inf  =>  p2 = -inf
       sf[3 * (nrel + lane)] = make_float4(0.f, 0.f, 0.f, 0.f);
-      sf[3 * (nrel + lane) + 1] = make_float4(0.f, 0.f, __int_as_float(0x7fc00000), 0.f);
+      sf[3 * (nrel + lane) + 1] = make_float4(0.f, -INFINITY, 0.f, 0.f);
     }
     __syncwarp();
     for (int r0 = 0; r0 < nrel; r0 += kGroup) {  // back to front, four list entries at a time
@@ -185,12 +188,11 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
       unsigned bal[kGroup];
 #pragma unroll
       for (int q = 0; q < kGroup; ++q) {
-        a0[q] = sf[3 * (r0 + q)];      // mx, my, A, B
-        a1[q] = sf[3 * (r0 + q) + 1];  // C, opacity, thr, tag
-        float dx, dy;
-        p[q] = eval_power1(a0[q].x, a0[q].y, a0[q].z, a0[q].w, a1[q].x, fx0, fy0, dx, dy);
+        a0[q] = sf[3 * (r0 + q)];      // u0, v0, l11, l21
+        a1[q] = sf[3 * (r0 + q) + 1];  // l22, lo, tag
+        p[q] = eval_power(a0[q].x, a0[q].y, a0[q].z, a0[q].w, a1[q].x, a1[q].y, fx0, fy0);
         // blended by the forward: alpha >= 1/255 and in front of the pixel's last contributor
-        hit[q] = p[q] >= a1[q].z && (int)(__float_as_uint(a1[q].w) & 31u) < lastb;
+        hit[q] = p[q] >= GS_POWER_MIN && (int)(__float_as_uint(a1[q].z) & 31u) < lastb;
         bal[q] = __ballot_sync(kFull, hit[q]);
       }
 #pragma unroll
@@ -199,7 +201,7 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
         float gp = 0.f, w = 0.f;
         if (hit[q]) {
           const float4 f2 = sf[3 * (r0 + q) + 2];
-          const float og = __fmul_rn(a1[q].y, ex2_approx(p[q]));
+          const float og = ex2_approx(p[q]);  // opacity * G: log2(opacity) is folded into the exponent
           const float a = fminf(GS_ALPHA_MAX, og);
           const float ioma = rcp_approx(1.f - a);
           T *= ioma;  // transmittance in front of this Gaussian
@@ -213,7 +215,8 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
         *pair_ptr = make_float2(gp, w);
         pair_ptr += kPairRow;
         if ((lane & (kSlots - 1)) == nslot) {
-          slot_mx = a0[q].x; slot_my = a0[q].y; slot_id = __float_as_uint(a1[q].w) >> 5;
+          const float2 m = s_mean[r0 + q];
+          slot_mx = m.x; slot_my = m.y; slot_id = __float_as_uint(a1[q].z) >> 5;
         }
         if (++nslot == kSlots) {
           gaussian_phase<2>(s_pair, s_pix, kSlots, lane, slot_mx, slot_my, slot_id, g2d);
