@@ -154,8 +154,10 @@ GS_API int gs_get_launch_count(gs_ctx* ctx, uint64_t* n);
 /* Workload of the last forward (SYNCHRONISES; re-walks the lists with the forward's own decisions): HOST
  * uint64[GS_NUM_WORKLOAD] = { E: (pixel, Gaussian) pairs evaluated while the pixel was still alive, over the (region,
  * Gaussian) entries the region masks keep; C: blended pairs; L: sum over pixels of the last blended list position;
- * sum over pixels of their tile's list length; R: relevant (8x4 region, Gaussian) entries walked by the forward }. */
-#define GS_NUM_WORKLOAD 5
+ * sum over pixels of their tile's list length; R: relevant (8x4 region, Gaussian) entries walked by the forward;
+ * Eb: pairs the backward must evaluate (relevant entries up to each pixel's last blended one); Rb: relevant entries the
+ * backward walks (up to each region's last blended one) }. */
+#define GS_NUM_WORKLOAD 7
 GS_API int gs_get_workload(gs_ctx* ctx, void* stream, uint64_t* out);
 
 /* ---- auxiliary kernels outside the five-call contract (losses of configs 2 and 4, on-device pose step) ---------- */

@@ -70,7 +70,7 @@ def load_library():
     lib.gs_profile_enable.argtypes = [vp, C.c_int]
     lib.gs_profile_read.argtypes = [vp, C.POINTER(f * 8)]
     lib.gs_get_launch_count.argtypes = [vp, C.POINTER(C.c_uint64)]
-    lib.gs_get_workload.argtypes = [vp, vp, C.POINTER(C.c_uint64 * 5)]
+    lib.gs_get_workload.argtypes = [vp, vp, C.POINTER(C.c_uint64 * 7)]
     lib.gs_measure_peaks.argtypes = [C.c_int, vp, C.POINTER(C.c_double * len(PEAKS))]
     lib.gs_fwd_bwd_host.argtypes = [vp, vp, i64, C.c_int, vp, vp, vp, vp, vp, C.POINTER(gs_camera), C.POINTER(f * 3)] + [vp] * 11
     for name in EXPORTS:
@@ -231,10 +231,10 @@ class Context:
         return int(n.value)
 
     def gs_get_workload(self, stream=None) -> dict:
-        w = (C.c_uint64 * 5)()
+        w = (C.c_uint64 * 7)()
         self._check(self.lib.gs_get_workload(self._h, _stream(stream), C.byref(w)))
         return dict(evaluated=int(w[0]), blended=int(w[1]), last_pos_sum=int(w[2]), list_len_x_pixels=int(w[3]),
-                    region_entries=int(w[4]))
+                    region_entries=int(w[4]), evaluated_bwd=int(w[5]), region_entries_bwd=int(w[6]))
 
     # -- host-buffer path (numpy arrays in / out; copies inside) ---------------------------------------------------
     def gs_fwd_bwd_host(self, scene_arrays, sh_degree, cam, bg, d_rgb, d_depth, out, stream=None):

@@ -53,28 +53,22 @@ gauss_bwd_kernel(int64_t N, const float* __restrict__ means, const float* __rest
     const float s0 = pb.x, s1 = pb.y, s2 = pb.z;
     Proj<R> P;
     project_gaussian<R, false>(cam, T, mu0, mu1, mu2, s0, s1, s2, q.x, q.y, q.z, q.w, o, P);
-    {
-      // The conic is taken from the forward's feature record (whitened Cholesky factor computed in fp64 by
-      // gs_preprocess: 0.5 log2(e) Q = L L^T): the fp32 determinant cxx cyy - cxy^2 loses all digits for long thin
-      // footprints.
-      const float4 f1 = __ldg(feat + 3 * (size_t)kk + 1);
-      const R ik = (R)(2.0 * 0.69314718055994531);  // 1 / (0.5 log2 e)
-      P.a = ik * (R)f1.x * (R)f1.x; P.b = ik * (R)f1.x * (R)f1.y; P.c = ik * ((R)f1.y * (R)f1.y + (R)f1.z * (R)f1.z);
-    }
+    // 2-D gradients from the whitened moments (gs_internal.cuh): with k Q = L L^T and w = L^T d,
+    //   dL/dmean = sum gp Q d = L M1 / k,      dL/dSigma' = sum gp (Q d)(Q d)^T / 2 = L M2 L^T / (2 k^2);
+    // L comes from the forward's feature record (fp64 Cholesky in gs_preprocess), so neither the fp32 determinant of
+    // Sigma' nor the product -Q gQ Q (which cancels for long thin footprints) is ever formed here.
     const R W[9] = {T[0], T[1], T[2], T[4], T[5], T[6], T[8], T[9], T[10]};
-    // ga.x, ga.y = sum gp dx, sum gp dy (moments about the mean); d power / d mean = -(Q d), ln2 * log2(e) = 1
-    const R g_mx = P.a * (R)ga.x + P.b * (R)ga.y, g_my = P.b * (R)ga.x + P.c * (R)ga.y;
-    const R g_a = -(R)0.5 * (R)ga.z, g_b = -(R)ga.w, g_c = -(R)0.5 * (R)gb.x;
+    const float4 f1 = __ldg(feat + 3 * (size_t)kk + 1);
+    const R l11 = f1.x, l21 = f1.y, l22 = f1.z;
+    const R ik = (R)(2.0 * 0.69314718055994531);  // 1 / k, k = 0.5 log2(e)
+    const R g_mx = ik * l11 * (R)ga.x, g_my = ik * (l21 * (R)ga.x + l22 * (R)ga.y);
     const R g_o = (R)gb.y / (R)o;
     const float gcol[3] = {gb.z, gb.w, gc.x};
     const R g_z = gc.y;
-    // conic -> Sigma': gS = -Q gQ Q
-    const R q00 = P.a, q01 = P.b, q11 = P.c;
-    const R h = (R)0.5 * g_b;
-    const R t00 = q00 * g_a + q01 * h, t01 = q00 * h + q01 * g_c;
-    const R t10 = q01 * g_a + q11 * h, t11 = q01 * h + q11 * g_c;
-    const R gS00 = -(t00 * q00 + t01 * q01), gS01 = -(t00 * q01 + t01 * q11);
-    const R gS10 = -(t10 * q00 + t11 * q01), gS11 = -(t10 * q01 + t11 * q11);
+    const R hk = (R)0.5 * ik * ik;
+    const R n00 = l11 * (R)ga.z, n01 = l11 * (R)ga.w;
+    const R n10 = l21 * (R)ga.z + l22 * (R)ga.w, n11 = l21 * (R)ga.w + l22 * (R)gb.x;
+    const R gS00 = hk * n00 * l11, gS01 = hk * (n00 * l21 + n01 * l22), gS10 = gS01, gS11 = hk * (n10 * l21 + n11 * l22);
     // gM = 2 gS M
     R gM[6];
 #pragma unroll

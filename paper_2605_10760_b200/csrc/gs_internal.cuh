@@ -41,10 +41,11 @@ __device__ __forceinline__ void load_pose(const DevCam& cam, float* T) {
 // ---------------------------------------------------------------------------------------------------------------
 constexpr int kFeatVec = 3;
 
-// 2-D gradient record accumulated by the pixel backward (global atomics), 12 floats = 48 B per Gaussian:
-//   [0] sum gp dx               [1] sum gp dy               [2] sum gp dx^2   [3] sum gp dx dy   [4] sum gp dy^2
-//   [5] sum gp                  [6..8] sum w gC             [9] sum w gD      [10],[11] unused
-// with gp = alpha * dL/dalpha on unclamped contributions and w = alpha T.
+// 2-D gradient record accumulated by the pixel backward (global atomics), 12 floats = 48 B per Gaussian: moments of
+// gp = alpha * dL/dalpha (unclamped contributions) in the WHITENED offsets (u, v) = L^T (pixel - mean) of gs_raster.cuh
+//   [0] sum gp u                [1] sum gp v                [2] sum gp u^2    [3] sum gp u v     [4] sum gp v^2
+//   [5] sum gp                  [6..8] sum w gC             [9] sum w gD      [10],[11] unused          (w = alpha T)
+// from which dL/dmean = L M1 / k and dL/dSigma' = L M2 L^T / (2 k^2), k = 0.5 log2(e)  (gs_gauss_bwd.cu).
 constexpr int kG2D = 12;
 
 constexpr int kHdrBytes = 256;  // Counts (128 B) + 16 pose accumulators, in front of the per-tile counters (gs_api.cu)

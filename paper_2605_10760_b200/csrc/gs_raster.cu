@@ -39,7 +39,8 @@ raster_fwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
   // T starts at 0 for a lane outside the image, so such a lane never blends (and writes nothing)
   float T = inside ? 1.f : 0.f, C0 = 0.f, C1 = 0.f, C2 = 0.f, D = 0.f;
   uint32_t last = 0;
-  unsigned long long n_eval = 0, n_blend = 0, n_entries = 0;
+  unsigned long long n_eval = 0, n_blend = 0;
+  uint32_t rank = 0, last_rank = 0;   // STATS: relevant entries walked so far; rank of the pixel's last blended one
 
   auto issue = [&](int b, uint32_t v) -> int {
     const bool relevant = (b * kWarpBatch + lane < n) && ((v >> sub) & 1u);
@@ -104,9 +105,10 @@ raster_fwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
         T = fmaf(-a, T, T);
         last = hit ? __float_as_uint(a1.z) : last;
         if (STATS && r0 + q < nrel) {
+          ++rank;
           n_eval += alive ? 1 : 0;
           n_blend += hit ? 1 : 0;
-          n_entries += lane == 0 ? 1 : 0;
+          last_rank = hit ? rank : last_rank;
         }
       }
       if (!__any_sync(kFull, T >= GS_T_MIN)) { stop = true; break; }
@@ -115,10 +117,11 @@ raster_fwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
   }
   cp_async_wait<0>();
   if (STATS) {
-    // [0] pixel-pairs evaluated while the pixel was alive, [1] blended pairs, [2] sum of the last blended list positions,
-    // [3] list length x pixels, [4] relevant (region, entry) pairs walked by the forward
+    // gs.h gs_get_workload: E, C, L, list length x pixels, R (forward), Eb, Rb (what the backward must walk: the
+    // relevant entries up to the pixel's / the region's last blended one)
+    const uint32_t max_rank = __reduce_max_sync(kFull, last_rank);
     unsigned long long v[GS_NUM_WORKLOAD] = {n_eval, n_blend, inside ? last : 0ull, inside ? (unsigned long long)n : 0ull,
-                                            n_entries};
+                                            lane == 0 ? rank : 0ull, last_rank, lane == 0 ? max_rank : 0ull};
 #pragma unroll
     for (int q = 0; q < GS_NUM_WORKLOAD; ++q) {
 #pragma unroll

@@ -9,9 +9,12 @@
 //     reaches at least one pixel hands over just TWO numbers per lane -- gp = alpha dL/dalpha (0 where clamped or not
 //     blended) and w = alpha T -- with one STS.64 into a [slot][pixel] table;
 //   * GAUSSIAN phase (lane = Gaussian slot x half of the region), run when 16 slots are full: every lane walks 16
-//     pixels of ITS Gaussian, re-forms dx, dy from the slot's mean and accumulates the 10 sums (moments of gp about the
-//     mean; w-weighted upstream colour / depth gradients) in registers -- no cross-lane reduction except one SHFL per
-//     sum to join the two halves -- and the 16 x 10 totals leave through shared memory as coalesced RED.ADD.F32.
+//     pixels of ITS Gaussian, re-forms the WHITENED offsets (u, v) = L^T (pixel - mean) from the slot's record
+//     (gs_raster.cuh: |u|, |v| <= ~4 wherever gp != 0) and accumulates the 10 sums (moments of gp in (u, v); w-weighted
+//     upstream colour / depth gradients) in registers -- no cross-lane reduction except one SHFL per sum to join the
+//     two halves -- and the 16 x 10 totals leave through shared memory as coalesced RED.ADD.F32.  Moments in the
+//     whitened frame are well conditioned for any footprint: dL/dSigma' = L M2 L^T / (2 k^2) needs no cancellation
+//     (moments of dx, dy lost 3 digits on 1000:1 footprints through -Q gQ Q).
 //   ~15 instructions and ~5 shared-memory wavefronts per (region, Gaussian) for the whole reduction.
 #include "gs_internal.cuh"
 #include "gs_raster.cuh"
@@ -27,20 +30,34 @@ constexpr int kOutVals = 10;   // sums per Gaussian (gs_internal.cuh kG2D, first
 
 // Gaussian phase.  SPLIT = 2: lane = (slot = lane & 15, half = lane >> 4), 2 pixel rows per lane;
 //                  SPLIT = 4: lane = (slot = lane & 7, quarter = lane >> 3), 1 pixel row per lane (tail flush, <= 8 slots).
+// Record of the Gaussian in slot (lane & 15), kept in registers between the pixel phase and the flush: the whitened
+// offset of the region origin and the visible slot; L is re-read from the feature record at the flush (one LDG.128 per
+// lane per 16 Gaussians) instead of being carried in three more registers (80 registers is the occupancy limit here).
+struct SlotRec { float u0, v0; };
+
 template <int SPLIT>
-__device__ __forceinline__ void gaussian_phase(float2* s_pair, const float4* s_pix, int nslot, int lane, float slot_mx,
-                                               float slot_my, uint32_t slot_id, float* __restrict__ g2d) {
+__device__ __forceinline__ void gaussian_phase(float2* s_pair, const float4* s_pix, int nslot, int lane, const SlotRec& sr,
+                                               uint32_t slot_id, const float4* __restrict__ feat, float* __restrict__ g2d) {
   constexpr int LS = 32 / SPLIT, R = 4 / SPLIT;  // slots per pass, pixel rows per lane
   __syncwarp();
   const int slot = lane & (LS - 1), part = lane / LS;
   // the slot records live in registers: lane s (and lane s + 16) holds the record of slot s
-  const float mx = SPLIT == 2 ? slot_mx : __shfl_sync(kFull, slot_mx, slot);
-  const float my = SPLIT == 2 ? slot_my : __shfl_sync(kFull, slot_my, slot);
-  float dxs[8], dys[R];
+  float u0 = sr.u0, v0 = sr.v0;
+  uint32_t id = slot_id;
+  if (SPLIT == 4) {
+    u0 = __shfl_sync(kFull, sr.u0, slot); v0 = __shfl_sync(kFull, sr.v0, slot);
+    id = __shfl_sync(kFull, slot_id, slot);
+  }
+  float4 L = make_float4(0.f, 0.f, 0.f, 0.f);
+  if (slot < nslot) L = __ldg(feat + 3 * (size_t)id + 1);  // l11, l21, l22
+  struct { float u0, v0, l11, l21, l22; } g = {u0, v0, L.x, L.y, L.z};
+  float ub[R], vs[R];
 #pragma unroll
-  for (int c = 0; c < 8; ++c) dxs[c] = (float)c - mx;
-#pragma unroll
-  for (int r = 0; r < R; ++r) dys[r] = (float)(part * R + r) - my;
+  for (int r = 0; r < R; ++r) {
+    const float y = (float)(part * R + r);
+    ub[r] = fmaf(g.l21, y, g.u0);
+    vs[r] = fmaf(g.l22, y, g.v0);
+  }
   const float2* pr = s_pair + slot * kPairRow + part * (R * 8);
   const float4* px = s_pix + part * (R * 8);
   float acc[kOutVals];
@@ -52,12 +69,13 @@ __device__ __forceinline__ void gaussian_phase(float2* s_pair, const float4* s_p
     for (int c = 0; c < 8; ++c) {
       const float2 pw = pr[r * 8 + c];  // gp, w of (this Gaussian, pixel)
       const float4 gu = px[r * 8 + c];  // upstream dL/dRGB, dL/dDepth of the pixel
-      const float gx = pw.x * dxs[c], gy = pw.x * dys[r];
+      const float uu = fmaf(g.l11, (float)c, ub[r]);
+      const float gx = pw.x * uu, gy = pw.x * vs[r];
       acc[0] += gx;
       acc[1] += gy;
-      acc[2] = fmaf(gx, dxs[c], acc[2]);
-      acc[3] = fmaf(gx, dys[r], acc[3]);
-      acc[4] = fmaf(gy, dys[r], acc[4]);
+      acc[2] = fmaf(gx, uu, acc[2]);
+      acc[3] = fmaf(gx, vs[r], acc[3]);
+      acc[4] = fmaf(gy, vs[r], acc[4]);
       acc[5] += pw.x;
       acc[6] = fmaf(pw.y, gu.x, acc[6]);
       acc[7] = fmaf(pw.y, gu.y, acc[7]);
@@ -99,7 +117,6 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
   constexpr int RPT = 8;  // 8x4-pixel regions per 16x16 tile
   __shared__ __align__(16) float4 s_feat[2][(kWarpBatch + kGroup) * 3];  // records of the relevant entries, decoded in place
   __shared__ uint32_t s_tag[2][kWarpBatch];
-  __shared__ float2 s_mean[kWarpBatch + kGroup];  // region-local means of the current batch's entries (Gaussian phase)
   __shared__ __align__(16) float2 s_pair[kSlots * kPairRow];
   __shared__ __align__(16) float4 s_pix[32];
   const int lane = threadIdx.x;
@@ -128,7 +145,7 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
   const int nb = (n + kWarpBatch - 1) / kWarpBatch;
   int nslot = 0;
   float2* pair_ptr = s_pair + lane;     // where this lane's (gp, w) of the next slot goes
-  float slot_mx = 0.f, slot_my = 0.f;  // record of slot (lane & 15), kept in registers
+  SlotRec slot = {0.f, 0.f};  // record of slot (lane & 15), kept in registers
   uint32_t slot_id = 0;
 
   // phase 1: the list entries are (index << 8 | region mask) -- gs_bin_tiles already decided which regions of the tile
@@ -174,7 +191,6 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
       decode_whitened(f0, f1, ox, oy, u0, v0, mx, my);
       sf[3 * lane] = make_float4(u0, v0, f1.x, f1.y);
       sf[3 * lane + 1] = make_float4(f1.z, f0.w, __uint_as_float(s_tag[b & 1][lane]), 0.f);
-      s_mean[lane] = make_float2(mx, my);
     }
     if (lane < kGroup) {  // padding records never pass: lo = -inf  =>  p2 = -inf
       sf[3 * (nrel + lane)] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -215,11 +231,11 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
         *pair_ptr = make_float2(gp, w);
         pair_ptr += kPairRow;
         if ((lane & (kSlots - 1)) == nslot) {
-          const float2 m = s_mean[r0 + q];
-          slot_mx = m.x; slot_my = m.y; slot_id = __float_as_uint(a1[q].z) >> 5;
+          slot.u0 = a0[q].x; slot.v0 = a0[q].y;
+          slot_id = __float_as_uint(a1[q].z) >> 5;
         }
         if (++nslot == kSlots) {
-          gaussian_phase<2>(s_pair, s_pix, kSlots, lane, slot_mx, slot_my, slot_id, g2d);
+          gaussian_phase<2>(s_pair, s_pix, kSlots, lane, slot, slot_id, feat, g2d);
           nslot = 0;
           pair_ptr = s_pair + lane;
         }
@@ -227,8 +243,8 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
     }
     __syncwarp();
   }
-  if (nslot > 8) gaussian_phase<2>(s_pair, s_pix, nslot, lane, slot_mx, slot_my, slot_id, g2d);
-  else if (nslot > 0) gaussian_phase<4>(s_pair, s_pix, nslot, lane, slot_mx, slot_my, slot_id, g2d);
+  if (nslot > 8) gaussian_phase<2>(s_pair, s_pix, nslot, lane, slot, slot_id, feat, g2d);
+  else if (nslot > 0) gaussian_phase<4>(s_pair, s_pix, nslot, lane, slot, slot_id, feat, g2d);
 }
 
 int launch_raster_bwd(gs_ctx* ctx, cudaStream_t s, const float* d_rgb, const float* d_depth, const float* d_alpha) {

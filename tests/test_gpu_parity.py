@@ -390,9 +390,15 @@ def test_growing_instance_count_is_reported_and_recovered(oracle, gpu):
     assert n1 > 1.5 * n0
     ref = oracle.forward(big)
     torch.cuda.synchronize()
+    # ~150 blended layers per pixel and footprints six times larger (quadratic-form terms up to 6e3): the whitened
+    # region-local power evaluation keeps the north_star tolerance here too (measured 7e-7 / 3e-7 / 1e-7)
     flagged = ref["margin"] < MARGIN
-    # ~150 blended layers per pixel (scales x 6): a stress scene, not a parity config -- fp32 error grows with depth
-    assert np.abs(out["alpha"].cpu().numpy() - ref["alpha"])[~flagged].max() <= 2e-4
+    assert flagged.mean() <= 5e-3           # deep lists: more pairs near a threshold than in the parity configs
+    for k in ("rgb", "depth", "alpha"):
+        err = np.abs(out[k].cpu().numpy().astype(np.float64) - ref[k])
+        err = err if err.ndim == 2 else err.max(axis=0)
+        assert err[~flagged].max() <= TOL_IMG, (k, err[~flagged].max())
+        assert err[flagged].max() <= TOL_FLAGGED, (k, err[flagged].max())
     ctx.close()
 
 
