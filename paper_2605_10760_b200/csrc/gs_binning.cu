@@ -245,7 +245,7 @@ emit_kernel(const uint4* __restrict__ vis_rec, const float4* __restrict__ feat, 
         const int pk = __float_as_int(f0.z);
         const float mx = (float)(((pk << 16) >> 16) - (int)tx * GS_TILE) + f0.x;
         const float my = (float)((pk >> 16) - (int)ty * GS_TILE) + f0.y;
-        kk[u] = s_key[owner] | (uint64_t)region_mask(f1.x, f1.y, f1.z, f0.w, mx, my);
+        kk[u] = s_key[owner] | (uint64_t)region_mask(f1.x, f1.y, f1.z, f1.w, mx, my);
       }
     }
 #pragma unroll
@@ -350,15 +350,28 @@ __device__ __forceinline__ void smem_step(uint64_t (&k)[E], uint64_t* s, int tid
   __syncthreads();
 }
 
-// what the compositing kernels read: (visible slot << 8 | region mask) for a sorted key (.. | index << 8 | mask)
-__device__ __forceinline__ uint32_t list_entry(uint64_t key, const uint32_t* __restrict__ slot_of) {
+// What the compositing kernels read for a sorted key (.. | index << 8 | mask): the list entry (visible slot << 8 | region
+// mask) and the instance's whitened tile-local offset (u0, v0) = -L^T (mean - tile origin), in fp64 (gs_raster.cuh).
+struct SortOut {
+  uint32_t* ids;
+  float2* uv;
+  const uint32_t* slot_of;
+  const float4* feat;
+  int ox, oy;  // pixel origin of the bucket's tile
+};
+
+__device__ __forceinline__ void write_entry(const SortOut& o, int i, uint64_t key) {
   const uint32_t lo = (uint32_t)key;
-  return (__ldg(slot_of + (lo >> 8)) << 8) | (lo & 0xffu);
+  const uint32_t slot = __ldg(o.slot_of + (lo >> 8));
+  o.ids[i] = (slot << 8) | (lo & 0xffu);
+  const float4 f0 = __ldg(o.feat + 3 * (size_t)slot), f1 = __ldg(o.feat + 3 * (size_t)slot + 1);
+  float u0, v0, mx, my;
+  decode_whitened(f0, f1, o.ox, o.oy, u0, v0, mx, my);
+  o.uv[i] = make_float2(u0, v0);
 }
 
 template <int E, int NW>
-__device__ __forceinline__ void bucket_sort(uint64_t* __restrict__ g, uint32_t* __restrict__ ids, int n, uint64_t* s, int tid,
-                                            const uint32_t* __restrict__ slot_of) {
+__device__ __forceinline__ void bucket_sort(uint64_t* __restrict__ g, const SortOut& out, int n, uint64_t* s, int tid) {
   constexpr int T = 32 * NW;
   uint64_t k[E];
 #pragma unroll
@@ -380,20 +393,42 @@ __device__ __forceinline__ void bucket_sort(uint64_t* __restrict__ g, uint32_t* 
       else reg_step_dyn<E, false>(k, j);
     }
   }
+  // epilogue in phases of up to four keys, so that the dependent gather chains (key -> slot -> feature record) of a
+  // thread overlap without holding E feature records in registers
+  constexpr int C = E < 4 ? E : 4;
 #pragma unroll
-  for (int e = 0; e < E; ++e) {
-    const int i = tid * E + e;
-    if (i < n) { g[i] = k[e]; ids[i] = list_entry(k[e], slot_of); }
+  for (int c = 0; c < E; c += C) {
+    uint32_t slot[C];
+    float4 f0[C], f1[C];
+#pragma unroll
+    for (int e = 0; e < C; ++e) slot[e] = (tid * E + c + e < n) ? __ldg(out.slot_of + ((uint32_t)k[c + e] >> 8)) : 0u;
+#pragma unroll
+    for (int e = 0; e < C; ++e) {
+      f0[e] = __ldg(out.feat + 3 * (size_t)slot[e]);
+      f1[e] = __ldg(out.feat + 3 * (size_t)slot[e] + 1);
+    }
+#pragma unroll
+    for (int e = 0; e < C; ++e) {
+      const int i = tid * E + c + e;
+      if (i < n) {
+        g[i] = k[c + e];
+        out.ids[i] = (slot[e] << 8) | ((uint32_t)k[c + e] & 0xffu);
+        float u0, v0, mx, my;
+        decode_whitened(f0[e], f1[e], out.ox, out.oy, u0, v0, mx, my);
+        out.uv[i] = make_float2(u0, v0);
+      }
+    }
   }
 }
+
 
 // Buckets of 2048 .. kLargeSort keys (the first n_large entries of `order`): one CTA of 512 threads per bucket, 16 keys
 // per thread; beyond kLargeSort the shared-memory-free network above runs in place in global memory (slow; degenerate
 // scenes only).
 __global__ void __launch_bounds__(512)
-tile_sort_large_kernel(const uint32_t* __restrict__ order, const uint2* __restrict__ ranges,
+tile_sort_large_kernel(int tiles_x, const uint32_t* __restrict__ order, const uint2* __restrict__ ranges,
                        const Counts* __restrict__ counts, uint64_t* __restrict__ keys, uint32_t* __restrict__ ids,
-                       const uint32_t* __restrict__ slot_of) {
+                       float2* __restrict__ uv, const uint32_t* __restrict__ slot_of, const float4* __restrict__ feat) {
   extern __shared__ uint64_t s_dyn[];
   const int tid = threadIdx.x, nth = blockDim.x;
   const int limit = (int)counts->n_large;
@@ -403,14 +438,15 @@ tile_sort_large_kernel(const uint32_t* __restrict__ order, const uint2* __restri
     const int n = (int)(r.y - r.x);
     if (n <= kMidSortMax) continue;
     uint64_t* g = keys + r.x;
+    const SortOut out = {ids + r.x, uv + r.x, slot_of, feat, (tile % tiles_x) * GS_TILE, (tile / tiles_x) * GS_TILE};
     if (n > kLargeSort) {
       bitonic_sort(g, n, tid, nth);  // __syncthreads orders the CTA's own global writes
-      for (int t = tid; t < n; t += nth) ids[r.x + t] = list_entry(g[t], slot_of);
+      for (int t = tid; t < n; t += nth) write_entry(out, t, g[t]);
       __syncthreads();
       continue;
     }
-    if (n <= 4096) bucket_sort<8, 16>(g, ids + r.x, n, s_dyn, tid, slot_of);
-    else bucket_sort<16, 16>(g, ids + r.x, n, s_dyn, tid, slot_of);
+    if (n <= 4096) bucket_sort<8, 16>(g, out, n, s_dyn, tid);
+    else bucket_sort<16, 16>(g, out, n, s_dyn, tid);
     __syncthreads();
   }
 }
@@ -419,30 +455,34 @@ tile_sort_large_kernel(const uint32_t* __restrict__ order, const uint2* __restri
 // large kernel are skipped) take a whole CTA each, 8 keys per thread; the remaining buckets (< 256 keys) take one warp
 // each, four buckets per CTA, no barrier at all.
 __global__ void __launch_bounds__(128)
-tile_sort_kernel(int tiles, const uint32_t* __restrict__ order, const uint2* __restrict__ ranges,
+tile_sort_kernel(int tiles, int tiles_x, const uint32_t* __restrict__ order, const uint2* __restrict__ ranges,
                  const Counts* __restrict__ counts, uint64_t* __restrict__ keys, uint32_t* __restrict__ ids,
-                 const uint32_t* __restrict__ slot_of) {
+                 float2* __restrict__ uv, const uint32_t* __restrict__ slot_of, const float4* __restrict__ feat) {
   __shared__ uint64_t s_x[2048];
   const int tid = threadIdx.x;
   const int n_mid = (int)counts->n_mid;
   if ((int)blockIdx.x < n_mid) {
-    const uint2 r = ranges[order[blockIdx.x]];
+    const int tile = (int)order[blockIdx.x];
+    const uint2 r = ranges[tile];
     const int n = (int)(r.y - r.x);
     if (n > kMidSortMax) return;
+    const SortOut out = {ids + r.x, uv + r.x, slot_of, feat, (tile % tiles_x) * GS_TILE, (tile / tiles_x) * GS_TILE};
     // keys per thread matched to the bucket: the network runs over 128 E slots whatever n is
-    if (n <= 512) bucket_sort<4, 4>(keys + r.x, ids + r.x, n, s_x, tid, slot_of);
-    else if (n <= 1024) bucket_sort<8, 4>(keys + r.x, ids + r.x, n, s_x, tid, slot_of);
-    else bucket_sort<16, 4>(keys + r.x, ids + r.x, n, s_x, tid, slot_of);
+    if (n <= 512) bucket_sort<4, 4>(keys + r.x, out, n, s_x, tid);
+    else if (n <= 1024) bucket_sort<8, 4>(keys + r.x, out, n, s_x, tid);
+    else bucket_sort<16, 4>(keys + r.x, out, n, s_x, tid);
     return;
   }
   const int idx = n_mid + ((int)blockIdx.x - n_mid) * 4 + (tid >> 5);
   if (idx >= tiles) return;
-  const uint2 r = ranges[order[idx]];
+  const int tile = (int)order[idx];
+  const uint2 r = ranges[tile];
   const int n = (int)(r.y - r.x), lane = tid & 31;
   if (n == 0) return;
-  if (n <= 64) bucket_sort<2, 1>(keys + r.x, ids + r.x, n, nullptr, lane, slot_of);
-  else if (n <= 128) bucket_sort<4, 1>(keys + r.x, ids + r.x, n, nullptr, lane, slot_of);
-  else bucket_sort<8, 1>(keys + r.x, ids + r.x, n, nullptr, lane, slot_of);
+  const SortOut out = {ids + r.x, uv + r.x, slot_of, feat, (tile % tiles_x) * GS_TILE, (tile / tiles_x) * GS_TILE};
+  if (n <= 64) bucket_sort<2, 1>(keys + r.x, out, n, nullptr, lane);
+  else if (n <= 128) bucket_sort<4, 1>(keys + r.x, out, n, nullptr, lane);
+  else bucket_sort<8, 1>(keys + r.x, out, n, nullptr, lane);
 }
 
 // export for gs_get_binning: keys_sorted[k] = tile << 32 | depth bits
@@ -483,6 +523,7 @@ int ensure_instance_capacity(gs_ctx* ctx, int64_t need) {
   int rc;
   if ((rc = grow(ctx, ctx->keys[0], cap)) != GS_OK) return rc;
   if ((rc = grow(ctx, ctx->vals[0], cap)) != GS_OK) return rc;
+  if ((rc = grow(ctx, ctx->inst_uv, cap)) != GS_OK) return rc;
   ctx->cap_I = cap;
   return GS_OK;
 }
@@ -574,12 +615,13 @@ int launch_binning(gs_ctx* ctx, cudaStream_t s) {
       GS_CUDA(cudaEventRecord(ctx->ev_fork2, s));
       GS_CUDA(cudaStreamWaitEvent(sl, ctx->ev_fork2, 0));
     }
-    tile_sort_large_kernel<<<min(tiles, 296), 512, kLargeSort * sizeof(uint64_t), sl>>>(ctx->tile_order, ctx->ranges, ctx->counts,
-                                                                                        ctx->keys[0], ctx->vals[0], ctx->slot_of);
+    tile_sort_large_kernel<<<min(tiles, 296), 512, kLargeSort * sizeof(uint64_t), sl>>>(
+        ctx->cam.tiles_x, ctx->tile_order, ctx->ranges, ctx->counts, ctx->keys[0], ctx->vals[0], ctx->inst_uv, ctx->slot_of,
+        ctx->feat);
     GS_LAUNCH_CHECK("tile_sort_large_kernel");
     if (fork) GS_CUDA(cudaEventRecord(ctx->ev_join2, sl));
-    tile_sort_kernel<<<tiles, 128, 0, s>>>(tiles, ctx->tile_order, ctx->ranges, ctx->counts, ctx->keys[0], ctx->vals[0],
-                                           ctx->slot_of);
+    tile_sort_kernel<<<tiles, 128, 0, s>>>(tiles, ctx->cam.tiles_x, ctx->tile_order, ctx->ranges, ctx->counts, ctx->keys[0],
+                                           ctx->vals[0], ctx->inst_uv, ctx->slot_of, ctx->feat);
     GS_LAUNCH_CHECK("tile_sort_kernel");
     if (fork) GS_CUDA(cudaStreamWaitEvent(s, ctx->ev_join2, 0));
   }

@@ -31,13 +31,16 @@ __device__ __forceinline__ void load_pose(const DevCam& cam, float* T) {
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// Per-Gaussian feature record written by gs_preprocess and gathered by the rasteriser: 3 x float4 = 48 B.
-//   f0 = { mfx, mfy, bits(miy << 16 | mix & 0xffff), lo }  2-D mean = integer pixel (mix,miy) + fraction in [-0.5,0.5];
-//                               lo = log2(opacity)
-//   f1 = { l11, l21, l22, opacity }   L = sqrt(0.5 log2 e) chol(conic) (lower triangular, fp64 in gs_preprocess):
+// Per-Gaussian feature record written by gs_preprocess, indexed by visible slot: 3 x float4 = 48 B.
+//   f0 = { mfx, mfy, bits(miy << 16 | mix & 0xffff), opacity }  2-D mean = integer pixel (mix,miy) + fraction in [-0.5,0.5]
+//   f1 = { l11, l21, l22, lo }  L = sqrt(0.5 log2 e) chol(conic) (lower triangular, fp64 in gs_preprocess), lo = log2(opacity):
 //                               p2(d) = lo - (l11 dx + l21 dy)^2 - (l22 dy)^2,  alpha = min(0.99, 2^p2),
 //                               alpha >= 1/255  <=>  p2 >= -log2(255)            (gs_raster.cuh)
 //   f2 = { r, g, b, z_c }
+// f1, f2 (32 contiguous bytes) are what the compositing kernels gather; f0 is read by the binning kernels only.
+// Per tile INSTANCE (sorted list position) gs_bin_tiles also writes uv = (u0, v0) = -L^T (mean - tile origin), formed in
+// fp64: with it the per-pixel arithmetic of the compositing kernels is u = l11 X + l21 Y + u0, v = l22 Y + v0 on
+// tile-local pixel coordinates (X, Y) in 0..15 -- every operand O(10), whatever the footprint.
 // ---------------------------------------------------------------------------------------------------------------
 constexpr int kFeatVec = 3;
 
@@ -97,7 +100,8 @@ struct gs_ctx {
   int64_t cal_N = -1;
   int32_t cal_W = -1, cal_H = -1;
   uint64_t* keys[2] = {nullptr, nullptr};  // [0]: (depth bits << 32 | id) bucketed by tile, sorted in place
-  uint32_t* vals[2] = {nullptr, nullptr};  // [0]: sorted (Gaussian id << 8 | region mask): what the compositing kernels read
+  uint32_t* vals[2] = {nullptr, nullptr};  // [0]: sorted (visible slot << 8 | region mask): what the compositing kernels read
+  float2* inst_uv = nullptr;               // [cap_I] whitened tile-local offset (u0, v0) of every sorted instance
   int sorted_buf = 0;
   bool sort_attr_set = false;
 

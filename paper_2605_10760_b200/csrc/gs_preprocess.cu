@@ -86,8 +86,8 @@ preprocess_kernel(int64_t N, const float* __restrict__ means, const float* __res
   float4 f0, f1, f2;
   f0.x = (float)(P.mx - rmx); f0.y = (float)(P.my - rmy);
   f0.z = __int_as_float(((int)rmy << 16) | ((int)rmx & 0xffff));
-  f0.w = (float)log2((double)o);
-  f1.x = (float)l11; f1.y = (float)l21; f1.z = (float)l22; f1.w = o;
+  f0.w = o;
+  f1.x = (float)l11; f1.y = (float)l21; f1.z = (float)l22; f1.w = (float)log2((double)o);
   f2.x = fmaxf(col[0] + 0.5f, 0.f); f2.y = fmaxf(col[1] + 0.5f, 0.f); f2.z = fmaxf(col[2] + 0.5f, 0.f);
   f2.w = (float)P.z;
   const uint32_t dk = __float_as_uint(depth_key_f32(T, mu0, mu1, mu2));

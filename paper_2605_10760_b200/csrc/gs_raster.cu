@@ -1,99 +1,125 @@
 // gs_raster.cu -- step a6: per-tile front-to-back compositing (oracle reading C1 step 7).
 //
-// Design (evidence: profiles/r1_v1_baseline.md, r1_v3_regions.md, r1_v5_masks.md, r2_*.md):
-//   * one WARP per 8x4-pixel region of a tile, one pixel per lane, single-warp CTAs: no block barrier, early exit per
-//     region, the hardware CTA scheduler balances the very uneven lists (regions are launched longest tile first);
-//   * the list entries are (visible slot << 8 | region mask): gs_bin_tiles already decided which regions of the tile a
-//     Gaussian can reach.  Lane g looks at entry g of a batch of 32; the relevant ones are compacted (ballot rank) and
-//     only their 48-byte records are gathered by cp.async (LDGSTS), one batch ahead of the compute;
-//   * every staged record is turned ONCE per (region, Gaussian) into the whitened region-local form of gs_raster.cuh
-//     (fp64, lane-parallel, in place); the pixel loop reads it back as three broadcast LDS.128;
-//   * the pixel loop is branch-free: every relevant entry is evaluated and blended under a per-lane predicate
-//     (alpha_eff = 0 where the pixel is not hit or has terminated), four entries unrolled, one vote per four entries
-//     for the early exit; alpha >= 1/255 is tested in the exponent domain against a constant, so rejected pairs cost
-//     no MUFU and the opacity never enters the loop: ~20 instructions per relevant (region, Gaussian) entry.
+// Design (evidence: profiles/r1_*.md for the history; profiles/r2_v7_tile_cta.md for this version).  Up to round-2 v6 every
+// 8x4 region was an autonomous single-warp CTA that gathered, decoded and compacted its own records: per relevant
+// (region, Gaussian) entry the forward then spent 47 warp instructions and 13.8 shared-memory wavefronts, of which only
+// ~22 / 7.4 were the blend itself (R = 1.24 M entries, 58.6 M instructions, 17.1 M wavefronts on config 3) -- staging
+// cost as much as compositing, and the kernel sat on the shared-memory pipe (l1tex 85-88 %).  Now:
+//   * one CTA per 16x16 TILE, eight warps = its eight 8x4-pixel regions, one pixel per lane;
+//   * the tile's list is staged ONCE per tile, 64 entries per round, into a three-stage ring: 64 threads each gather the
+//     32 contiguous bytes {l11, l21, l22, lo}{r, g, b, z} of one Gaussian by visible slot (2 x cp.async 16 B) plus the
+//     8-byte tile-local whitened offset (u0, v0) of the instance (written in fp64 by gs_bin_tiles) -- nothing is decoded
+//     here any more; one block barrier per round, which also carries the "is any pixel of the tile still alive" vote;
+//   * every warp turns the round's 64 region masks into a byte list of the entries relevant to ITS region (two ballots,
+//     ranks by popc, byte stores) and walks that list front to back, four entries per step: the records are read as
+//     broadcast LDS.128 x 2 + LDS.64;
+//   * the pixel loop is branch-free: every relevant entry is evaluated and blended under a per-lane predicate (alpha_eff
+//     = 0 where the pixel is not hit or has terminated); alpha >= 1/255 is tested in the exponent domain against a
+//     constant, so rejected pairs cost no MUFU and the opacity never enters the loop.
 #include "gs_internal.cuh"
 #include "gs_raster.cuh"
 
 namespace gs {
 
+// NW: warps (= regions) per CTA.  8: one CTA per tile; 4 / 2: half / quarter tiles -- the list is then staged 2 / 4 times
+// per tile, but fewer warps wait for each other at the per-round barrier (profiles/r2_v7_tile_cta.md).
+#ifndef GS_FWD_WARPS
+#define GS_FWD_WARPS 4
+#endif
+
 // STATS = true: the same walk with the same decisions, counting the workload instead of writing the image
 // (gs_get_workload; never on the timed path).
-template <bool STATS>
-__global__ void __launch_bounds__(32)
+template <int NW, bool STATS>
+__global__ void __launch_bounds__(NW * 32)
 raster_fwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order, const uint2* __restrict__ ranges,
-                  const uint32_t* __restrict__ ids, const float4* __restrict__ feat, float bg0, float bg1, float bg2,
-                  float* __restrict__ rgb, float* __restrict__ depth, float* __restrict__ alpha_out,
-                  float* __restrict__ final_T, uint32_t* __restrict__ n_contrib, unsigned long long* __restrict__ stats) {
-  __shared__ __align__(16) float4 s_feat[2][(kWarpBatch + kGroup) * 3];  // records of the relevant entries (cp.async),
-  __shared__ uint32_t s_pos[2][kWarpBatch];                               // decoded in place; their list positions + 1
-  const int lane = threadIdx.x;
-  const int tile = (int)__ldg(order + blockIdx.x / 8), sub = blockIdx.x % 8;
-  const int ox = (tile % tiles_x) * GS_TILE + (sub % 2) * 8, oy = (tile / tiles_x) * GS_TILE + (sub / 2) * 4;
-  const int lx = lane & 7, ly = lane >> 3;
-  const float fx0 = (float)lx, fy0 = (float)ly;
-  const bool inside = ox + lx < W && oy + ly < H;
+                  const uint32_t* __restrict__ ids, const float2* __restrict__ inst_uv, const float4* __restrict__ feat,
+                  float bg0, float bg1, float bg2, float* __restrict__ rgb, float* __restrict__ depth,
+                  float* __restrict__ alpha_out, float* __restrict__ final_T, uint32_t* __restrict__ n_contrib,
+                  unsigned long long* __restrict__ stats) {
+  static_assert(NW == 2 || NW == 4 || NW == 8, "64 producer threads are needed");
+  constexpr int CPT = 8 / NW;  // CTAs per tile
+  __shared__ StageBuf s_st[kStages];
+  // per warp: byte offsets (into the stage) of the round's relevant entries, in list order
+  __shared__ __align__(8) uint16_t s_idx[NW][kTileBatch + kGroup];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int tile = (int)__ldg(order + blockIdx.x / CPT), sub = (blockIdx.x % CPT) * NW + warp;
+  const int tx0 = (tile % tiles_x) * GS_TILE, ty0 = (tile / tiles_x) * GS_TILE;
+  const int X = (sub % 2) * 8 + (lane & 7), Y = (sub / 2) * 4 + (lane >> 3);  // tile-local pixel of this lane
+  const float fx0 = (float)X, fy0 = (float)Y;
+  const bool inside = tx0 + X < W && ty0 + Y < H;
   const uint2 range = ranges[tile];
   const int n = (int)(range.y - range.x);
-  const int nb = (n + kWarpBatch - 1) / kWarpBatch;
+  const int nb = (n + kTileBatch - 1) / kTileBatch;
   // T starts at 0 for a lane outside the image, so such a lane never blends (and writes nothing)
   float T = inside ? 1.f : 0.f, C0 = 0.f, C1 = 0.f, C2 = 0.f, D = 0.f;
-  uint32_t last = 0;
+  uint32_t last48 = 0;                // 48 x (list position + 1) of the last blended entry
   unsigned long long n_eval = 0, n_blend = 0;
   uint32_t rank = 0, last_rank = 0;   // STATS: relevant entries walked so far; rank of the pixel's last blended one
 
-  auto issue = [&](int b, uint32_t v) -> int {
-    const bool relevant = (b * kWarpBatch + lane < n) && ((v >> sub) & 1u);
-    const unsigned rel = __ballot_sync(kFull, relevant);
-    if (relevant) {
-      const int r = __popc(rel & ((1u << lane) - 1u));
-      const float4* src = feat + 3 * (size_t)(v >> 8);
-      float4* dst = &s_feat[b & 1][r * 3];
-      cp_async16(dst, src); cp_async16(dst + 1, src + 1); cp_async16(dst + 2, src + 2);
-      s_pos[b & 1][r] = (uint32_t)(b * kWarpBatch + lane + 1);
+  if (tid < kStages) {  // padding records never pass: lo = -inf  =>  p2 = -inf
+    StageRec& pr = s_st[tid].rec[kPadIdx];
+    pr.g = make_float4(0.f, 0.f, 0.f, -INFINITY);
+    pr.c = make_float4(0.f, 0.f, 0.f, 0.f);
+    pr.uv = make_float2(0.f, 0.f);
+  }
+  // producer: thread t < 64 stages list entry 64 j + t of round j (the list entry itself is fetched one round earlier)
+  uint32_t v_pre = 0;
+  int i_pre = tid;  // list index of the entry this thread fetches next
+  auto prefetch = [&]() {
+    v_pre = (tid < kTileBatch && i_pre < n) ? __ldg(ids + range.x + i_pre) : 0u;
+  };
+  int i_pro = tid, st_pro = 0;
+  auto produce = [&]() {
+    if (tid < kTileBatch) {
+      StageRec& r = s_st[st_pro].rec[tid];
+      r.ent = v_pre;
+      if (i_pro < n) {
+        const float4* src = feat + 3 * (size_t)(v_pre >> 8) + 1;
+        cp_async16(&r.g, src);
+        cp_async16(&r.c, src + 1);
+        cp_async8(&r.uv, inst_uv + range.x + i_pro);
+      }
     }
     cp_async_commit();
-    return __popc(rel);
+    i_pro += kTileBatch;
+    st_pro = st_pro + 1 == kStages ? 0 : st_pro + 1;
   };
-  uint32_t v_next = 0;
-  int nrel = 0, nrel_next = 0;
-  if (nb > 0) {
-    nrel_next = issue(0, lane < n ? __ldg(ids + range.x + lane) : 0u);
-    if (nb > 1) v_next = (kWarpBatch + lane < n) ? __ldg(ids + range.x + kWarpBatch + lane) : 0u;
-  }
-  bool stop = !__any_sync(kFull, inside);
-  for (int b = 0; b < nb && !stop; ++b) {
-    nrel = nrel_next;
-    if (b + 1 < nb) {
-      nrel_next = issue(b + 1, v_next);
-      const int i2 = (b + 2) * kWarpBatch + lane;
-      if (b + 2 < nb) v_next = (i2 < n) ? __ldg(ids + range.x + i2) : 0u;
-      cp_async_wait<1>();
-    } else {
-      cp_async_wait<0>();
-    }
-    __syncwarp();
+  prefetch(); i_pre += kTileBatch; produce();
+  prefetch(); i_pre += kTileBatch; produce();
+  prefetch(); i_pre += kTileBatch;
+  bool alive_warp = __any_sync(kFull, inside);
+  int st_con = 0;
+  uint32_t base48 = 48u;  // 48 x (list position + 1) of entry 0 of the round
+  for (int j = 0; j < nb; ++j, base48 += 48u * kTileBatch) {
+    cp_async_wait<1>();  // this thread's copies of round j have landed ...
+    // ... and after the barrier everybody's have; every warp has also finished round j - 1, whose stage is refilled next
+    if (!__syncthreads_or(alive_warp)) break;
+    produce();
+    prefetch(); i_pre += kTileBatch;
+    const StageBuf& sb = s_st[st_con];
+    st_con = st_con + 1 == kStages ? 0 : st_con + 1;
+    if (!alive_warp) continue;
+    // the entries of this round that can reach this warp's region, as a list of byte offsets in list order
+    const bool r0 = (sb.rec[lane].ent >> sub) & 1u, r1 = (sb.rec[lane + 32].ent >> sub) & 1u;
+    const unsigned b0 = __ballot_sync(kFull, r0), b1 = __ballot_sync(kFull, r1);
+    const int n0 = __popc(b0), nrel = n0 + __popc(b1);
     if (nrel == 0) continue;
-    float4* sf = s_feat[b & 1];
-    if (lane < nrel) {  // decode once per (region, Gaussian), in place: whitened region-local record
-      const float4 f0 = sf[3 * lane], f1 = sf[3 * lane + 1];
-      float u0, v0, mx, my;
-      decode_whitened(f0, f1, ox, oy, u0, v0, mx, my);
-      sf[3 * lane] = make_float4(u0, v0, f1.x, f1.y);
-      sf[3 * lane + 1] = make_float4(f1.z, f0.w, __uint_as_float(s_pos[b & 1][lane]), 0.f);
-    }
-    if (lane < kGroup) {  // padding records never pass: lo = -inf  =>  p2 = -inf
-      sf[3 * (nrel + lane)] = make_float4(0.f, 0.f, 0.f, 0.f);
-      sf[3 * (nrel + lane) + 1] = make_float4(0.f, -INFINITY, 0.f, 0.f);
-      sf[3 * (nrel + lane) + 2] = make_float4(0.f, 0.f, 0.f, 0.f);
-    }
+    const unsigned lt = (1u << lane) - 1u;
+    uint16_t* idx = s_idx[warp];
+    if (r0) idx[__popc(b0 & lt)] = (uint16_t)(lane * 48);
+    if (r1) idx[n0 + __popc(b1 & lt)] = (uint16_t)((32 + lane) * 48);
+    if (lane < kGroup) idx[nrel + lane] = (uint16_t)(kPadIdx * 48);
     __syncwarp();
-    // phase 2: front to back, branch-free
-    for (int r0 = 0; r0 < nrel; r0 += kGroup) {
+    const char* recs = reinterpret_cast<const char*>(sb.rec);
+    for (int r = 0; r < nrel; r += kGroup) {
+      const uint2 o4 = *reinterpret_cast<const uint2*>(idx + r);
+      const uint32_t off[kGroup] = {o4.x & 0xffffu, o4.x >> 16, o4.y & 0xffffu, o4.y >> 16};
 #pragma unroll
       for (int q = 0; q < kGroup; ++q) {
-        const float4 a0 = sf[3 * (r0 + q)], a1 = sf[3 * (r0 + q) + 1], f2 = sf[3 * (r0 + q) + 2];
-        const float p = eval_power(a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, fx0, fy0);
+        const StageRec& e = *reinterpret_cast<const StageRec*>(recs + off[q]);
+        const float4 a0 = e.g, f2 = e.c;
+        const float2 uv = e.uv;
+        const float p = eval_power(uv.x, uv.y, a0.x, a0.y, a0.z, a0.w, fx0, fy0);
         const bool alive = T >= GS_T_MIN;
         const bool hit = (p >= GS_POWER_MIN) && alive;   // alpha >= 1/255 and the pixel has not terminated
         const float a = hit ? fminf(GS_ALPHA_MAX, ex2_approx(p)) : 0.f;
@@ -103,19 +129,19 @@ raster_fwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
         C2 = fmaf(f2.z, w, C2);
         D = fmaf(f2.w, w, D);
         T = fmaf(-a, T, T);
-        last = hit ? __float_as_uint(a1.z) : last;
-        if (STATS && r0 + q < nrel) {
+        last48 = hit ? base48 + off[q] : last48;
+        if (STATS && r + q < nrel) {
           ++rank;
           n_eval += alive ? 1 : 0;
           n_blend += hit ? 1 : 0;
           last_rank = hit ? rank : last_rank;
         }
       }
-      if (!__any_sync(kFull, T >= GS_T_MIN)) { stop = true; break; }
+      if (!__any_sync(kFull, T >= GS_T_MIN)) { alive_warp = false; break; }
     }
-    __syncwarp();
   }
   cp_async_wait<0>();
+  const uint32_t last = last48 / 48u;
   if (STATS) {
     // gs.h gs_get_workload: E, C, L, list length x pixels, R (forward), Eb, Rb (what the backward must walk: the
     // relevant entries up to the pixel's / the region's last blended one)
@@ -132,7 +158,7 @@ raster_fwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
   }
   if (inside) {
     const size_t HW = (size_t)W * H;
-    const size_t p = (size_t)(oy + ly) * W + (ox + lx);
+    const size_t p = (size_t)(ty0 + Y) * W + (tx0 + X);
     if (rgb) {
       rgb[p] = fmaf(T, bg0, C0);
       rgb[HW + p] = fmaf(T, bg1, C1);
@@ -146,25 +172,26 @@ raster_fwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
 }
 
 int launch_raster_fwd(gs_ctx* ctx, cudaStream_t s, float* rgb, float* depth, float* alpha) {
-  const int units = ctx->cam.tiles_x * ctx->cam.tiles_y * 8;
-  if (units == 0) return GS_OK;
-  raster_fwd_kernel<false><<<units, 32, 0, s>>>(ctx->cam.W, ctx->cam.H, ctx->cam.tiles_x, ctx->tile_order, ctx->ranges,
-                                                ctx->vals[ctx->sorted_buf], ctx->feat, ctx->bg[0], ctx->bg[1], ctx->bg[2],
-                                                rgb, depth, alpha, ctx->final_T, ctx->n_contrib, nullptr);
+  const int tiles = ctx->cam.tiles_x * ctx->cam.tiles_y;
+  if (tiles == 0) return GS_OK;
+  constexpr int NW = GS_FWD_WARPS;
+  raster_fwd_kernel<NW, false><<<tiles * (8 / NW), NW * 32, 0, s>>>(
+      ctx->cam.W, ctx->cam.H, ctx->cam.tiles_x, ctx->tile_order, ctx->ranges, ctx->vals[ctx->sorted_buf], ctx->inst_uv,
+      ctx->feat, ctx->bg[0], ctx->bg[1], ctx->bg[2], rgb, depth, alpha, ctx->final_T, ctx->n_contrib, nullptr);
   GS_LAUNCH_CHECK("raster_fwd_kernel");
   return GS_OK;
 }
 
-// Workload statistics of the forward (introspection only): re-walks every region's list with the forward's decisions.
+// Workload statistics of the forward (introspection only): re-walks every tile's list with the forward's decisions.
 int launch_workload_stats(gs_ctx* ctx, cudaStream_t s, uint64_t* out_host) {
-  const int units = ctx->cam.tiles_x * ctx->cam.tiles_y * 8;
+  const int tiles = ctx->cam.tiles_x * ctx->cam.tiles_y;
   if (!ctx->stats_ws) GS_CUDA(cudaMalloc((void**)&ctx->stats_ws, 8 * sizeof(unsigned long long)));
   unsigned long long* d = ctx->stats_ws;
   GS_CUDA(cudaMemsetAsync(d, 0, 8 * sizeof(unsigned long long), s));
-  if (units > 0) {
-    raster_fwd_kernel<true><<<units, 32, 0, s>>>(ctx->cam.W, ctx->cam.H, ctx->cam.tiles_x, ctx->tile_order, ctx->ranges,
-                                                 ctx->vals[ctx->sorted_buf], ctx->feat, 0.f, 0.f, 0.f, nullptr, nullptr,
-                                                 nullptr, nullptr, nullptr, d);
+  if (tiles > 0) {
+    raster_fwd_kernel<8, true><<<tiles, 256, 0, s>>>(ctx->cam.W, ctx->cam.H, ctx->cam.tiles_x, ctx->tile_order, ctx->ranges,
+                                                     ctx->vals[ctx->sorted_buf], ctx->inst_uv, ctx->feat, 0.f, 0.f, 0.f,
+                                                     nullptr, nullptr, nullptr, nullptr, nullptr, d);
     GS_LAUNCH_CHECK("raster_fwd_kernel<stats>");
   }
   GS_CUDA(cudaMemcpyAsync(out_host, d, GS_NUM_WORKLOAD * sizeof(unsigned long long), cudaMemcpyDeviceToHost, s));

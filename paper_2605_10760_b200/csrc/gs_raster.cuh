@@ -1,10 +1,10 @@
 // gs_raster.cuh -- pieces shared by the binning masks and the forward / backward compositing kernels.
 //
-// The power of a Gaussian at a pixel is evaluated in WHITENED, REGION-LOCAL form ("precision"):
-//     p2 = lo - u^2 - v^2,   u = l11 x + l21 y + u0,   v = l22 y + v0,      alpha = min(0.99, 2^p2)
-// with (x, y) the pixel's coordinates inside the warp's 8x4 region (0..7, 0..3), L = sqrt(0.5 log2 e) chol(conic) from
-// gs_preprocess (fp64 there), lo = log2(opacity), and (u0, v0) = -L^T (mean - region origin) formed in fp64 when the
-// record is staged.  Every fp32 operand of the per-pixel arithmetic is then O(10) whatever the footprint's size or
+// The power of a Gaussian at a pixel is evaluated in WHITENED, TILE-LOCAL form ("precision"):
+//     p2 = lo - u^2 - v^2,   u = l11 X + l21 Y + u0,   v = l22 Y + v0,      alpha = min(0.99, 2^p2)
+// with (X, Y) the pixel's coordinates inside its 16x16 tile (0..15), L = sqrt(0.5 log2 e) chol(conic) from gs_preprocess
+// (fp64 there), lo = log2(opacity), and (u0, v0) = -L^T (mean - tile origin) formed in fp64 once per tile instance by
+// gs_bin_tiles.  Every fp32 operand of the per-pixel arithmetic is then O(10) whatever the footprint's size or
 // anisotropy (the direct form A dx^2 + B dx dy + C dy^2 cancels terms of size |A| dx^2 -- measured 1e-3 image error on
 // config 5).  alpha >= 1/255 <=> p2 >= -log2(255): a constant, so neither the opacity nor a per-Gaussian threshold is
 // read in the pixel loop.  The sequence below MUST be the same instructions in the forward and in the backward (the
@@ -15,9 +15,26 @@
 
 namespace gs {
 
-constexpr int kWarpBatch = 32;  // list entries examined per round by one warp (one per lane)
 constexpr unsigned kFull = 0xffffffffu;
-constexpr int kGroup = 4;       // relevant entries evaluated together in phase 2
+constexpr int kGroup = 4;        // relevant entries evaluated together in the pixel loop
+constexpr int kTileBatch = 64;   // list entries staged per round by a CTA
+constexpr int kStages = 3;       // staging ring depth
+constexpr int kPadIdx = kTileBatch;  // index of the stage's padding record (never passes: lo = -inf)
+
+// One staged list entry (48 B): what the pixel loops read as broadcast LDS.128 x 2 + LDS.64.
+//   g  = { l11, l21, l22, lo }, c = { r, g, b, z }   gathered by visible slot (cp.async, 2 x 16 B)
+//   uv = { u0, v0 }                                   the instance's tile-local whitened offset (cp.async 8 B)
+//   ent = visible slot << 8 | region mask             (0 beyond the end of the list)
+struct __align__(16) StageRec {
+  float4 g, c;
+  float2 uv;
+  uint32_t ent, pad;
+};
+static_assert(sizeof(StageRec) == 48, "StageRec layout");
+// One stage of a CTA's staging ring: 64 consecutive list entries of the tile + the padding record.
+struct __align__(16) StageBuf {
+  StageRec rec[kTileBatch + 1];
+};
 
 // -log2(255): alpha >= 1/255  <=>  p2 >= kPowerMin
 #define GS_POWER_MIN (-7.994353436858858f)
@@ -37,13 +54,17 @@ __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
   const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
   asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
 }
+__device__ __forceinline__ void cp_async8(void* smem_dst, const void* gmem_src) {
+  const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gmem_src) : "memory");
+}
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_async_wait() {
   asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
 }
 
-// Staged record -> whitened record relative to the origin (ox, oy), in fp64 (exact integer part of the mean, exact
+// Feature record -> whitened offset relative to the origin (ox, oy), in fp64 (exact integer part of the mean, exact
 // products with the fp32-rounded L; one rounding of u0, v0 at the end).  Also returns the origin-relative mean (fp32).
 __device__ __forceinline__ void decode_whitened(const float4& f0, const float4& f1, int ox, int oy, float& u0, float& v0,
                                                 float& mx, float& my) {
@@ -56,7 +77,7 @@ __device__ __forceinline__ void decode_whitened(const float4& f0, const float4& 
   my = (float)myd;
 }
 
-// p2 at the lane's pixel (fx0, fy0) of the region: five FFMA, no subtraction of large numbers
+// p2 at the lane's pixel (fx0, fy0) of the tile: five FFMA, no subtraction of large numbers
 __device__ __forceinline__ float eval_power(float u0, float v0, float l11, float l21, float l22, float lo, float fx0,
                                             float fy0) {
   const float u = __fmaf_rn(l11, fx0, __fmaf_rn(l21, fy0, u0));

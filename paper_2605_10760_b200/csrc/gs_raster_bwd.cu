@@ -1,12 +1,13 @@
 // gs_raster_bwd.cu -- step a8: back-to-front per-pixel backward of the compositing, reduced per (region, Gaussian)
 // before global atomics.
 //
-// v4 design (evidence: profiles/r1_v3_regions.md -- one warp per 8x4-pixel region, one pixel per lane; the register
-// butterfly that reduced the 10 per-Gaussian sums over the lanes was 42 % of the instructions, and parking the 10
-// values per lane in shared memory instead made the kernel LSU-bound: 20 wavefronts per (region, Gaussian)):
-//   * PIXEL phase (lane = pixel): walks the region's list back to front exactly like the forward walks it front to
-//     back (cp.async staging, phase-1 rectangle culling, groups of four), rebuilds T, and for every Gaussian that
-//     reaches at least one pixel hands over just TWO numbers per lane -- gp = alpha dL/dalpha (0 where clamped or not
+// Same tile-CTA structure as the forward (gs_raster.cu): one CTA per 16x16 tile, eight warps = its eight 8x4-pixel
+// regions, the tile's list staged once per tile through a three-stage cp.async ring, walked from the deepest blended
+// position of the tile back to the front.  Per warp (evidence: profiles/r1_v3_regions.md -- a register butterfly that
+// reduced the 10 per-Gaussian sums over the lanes was 42 % of the instructions, and parking the 10 values per lane in
+// shared memory made the kernel LSU-bound at 20 wavefronts per (region, Gaussian)):
+//   * PIXEL phase (lane = pixel): walks the region's relevant entries back to front, rebuilds T, and for every Gaussian
+//     that reaches at least one pixel hands over just TWO numbers per lane -- gp = alpha dL/dalpha (0 where clamped or not
 //     blended) and w = alpha T -- with one STS.64 into a [slot][pixel] table;
 //   * GAUSSIAN phase (lane = Gaussian slot x half of the region), run when 16 slots are full: every lane walks 16
 //     pixels of ITS Gaussian, re-forms the WHITENED offsets (u, v) = L^T (pixel - mean) from the slot's record
@@ -15,29 +16,30 @@
 //     two halves -- and the 16 x 10 totals leave through shared memory as coalesced RED.ADD.F32.  Moments in the
 //     whitened frame are well conditioned for any footprint: dL/dSigma' = L M2 L^T / (2 k^2) needs no cancellation
 //     (moments of dx, dy lost 3 digits on 1000:1 footprints through -Q gQ Q).
-//   ~15 instructions and ~5 shared-memory wavefronts per (region, Gaussian) for the whole reduction.
 #include "gs_internal.cuh"
 #include "gs_raster.cuh"
 
 namespace gs {
 
-#ifndef GS_BWD_MIN_BLOCKS
-#define GS_BWD_MIN_BLOCKS 22
+#ifndef GS_BWD_MIN_CTAS
+#define GS_BWD_MIN_CTAS 3
 #endif
 constexpr int kSlots = 16;     // Gaussians per flush of the Gaussian phase
 constexpr int kPairRow = 33;   // float2 per slot row (32 pixels + 1: conflict-free transposed LDS.64)
 constexpr int kOutVals = 10;   // sums per Gaussian (gs_internal.cuh kG2D, first 10)
 
-// Gaussian phase.  SPLIT = 2: lane = (slot = lane & 15, half = lane >> 4), 2 pixel rows per lane;
-//                  SPLIT = 4: lane = (slot = lane & 7, quarter = lane >> 3), 1 pixel row per lane (tail flush, <= 8 slots).
 // Record of the Gaussian in slot (lane & 15), kept in registers between the pixel phase and the flush: the whitened
-// offset of the region origin and the visible slot; L is re-read from the feature record at the flush (one LDG.128 per
+// offset of the tile origin and the visible slot; L is re-read from the feature record at the flush (one LDG.128 per
 // lane per 16 Gaussians) instead of being carried in three more registers (80 registers is the occupancy limit here).
 struct SlotRec { float u0, v0; };
 
+// Gaussian phase.  SPLIT = 2: lane = (slot = lane & 15, half = lane >> 4), 2 pixel rows per lane;
+//                  SPLIT = 4: lane = (slot = lane & 7, quarter = lane >> 3), 1 pixel row per lane (tail flush, <= 8 slots).
+// (xo, yo): tile-local coordinates of the region's first pixel.
 template <int SPLIT>
 __device__ __forceinline__ void gaussian_phase(float2* s_pair, const float4* s_pix, int nslot, int lane, const SlotRec& sr,
-                                               uint32_t slot_id, const float4* __restrict__ feat, float* __restrict__ g2d) {
+                                               uint32_t slot_id, float xo, float yo, const float4* __restrict__ feat,
+                                               float* __restrict__ g2d) {
   constexpr int LS = 32 / SPLIT, R = 4 / SPLIT;  // slots per pass, pixel rows per lane
   __syncwarp();
   const int slot = lane & (LS - 1), part = lane / LS;
@@ -50,13 +52,12 @@ __device__ __forceinline__ void gaussian_phase(float2* s_pair, const float4* s_p
   }
   float4 L = make_float4(0.f, 0.f, 0.f, 0.f);
   if (slot < nslot) L = __ldg(feat + 3 * (size_t)id + 1);  // l11, l21, l22
-  struct { float u0, v0, l11, l21, l22; } g = {u0, v0, L.x, L.y, L.z};
   float ub[R], vs[R];
 #pragma unroll
   for (int r = 0; r < R; ++r) {
-    const float y = (float)(part * R + r);
-    ub[r] = fmaf(g.l21, y, g.u0);
-    vs[r] = fmaf(g.l22, y, g.v0);
+    const float y = yo + (float)(part * R + r);
+    ub[r] = fmaf(L.y, y, fmaf(L.x, xo, u0));
+    vs[r] = fmaf(L.z, y, v0);
   }
   const float2* pr = s_pair + slot * kPairRow + part * (R * 8);
   const float4* px = s_pix + part * (R * 8);
@@ -69,7 +70,7 @@ __device__ __forceinline__ void gaussian_phase(float2* s_pair, const float4* s_p
     for (int c = 0; c < 8; ++c) {
       const float2 pw = pr[r * 8 + c];  // gp, w of (this Gaussian, pixel)
       const float4 gu = px[r * 8 + c];  // upstream dL/dRGB, dL/dDepth of the pixel
-      const float uu = fmaf(g.l11, (float)c, ub[r]);
+      const float uu = fmaf(L.x, (float)c, ub[r]);
       const float gx = pw.x * uu, gy = pw.x * vs[r];
       acc[0] += gx;
       acc[1] += gy;
@@ -101,160 +102,184 @@ __device__ __forceinline__ void gaussian_phase(float2* s_pair, const float4* s_p
   for (int t = 0; t < (LS * kOutVals + 31) / 32; ++t) {
     const int idx = t * 32 + lane;
     const int sl_i = min(idx / kOutVals, LS - 1), val = idx - sl_i * kOutVals;
-    const uint32_t id = __shfl_sync(kFull, slot_id, sl_i);
-    if (idx < total) atomicAdd(g2d + (size_t)id * kG2D + val, s_out[idx]);
+    const uint32_t gid = __shfl_sync(kFull, slot_id, sl_i);
+    if (idx < total) atomicAdd(g2d + (size_t)gid * kG2D + val, s_out[idx]);
   }
   __syncwarp();
 }
 
-template <bool HAS_GA>
-__global__ void __launch_bounds__(32, GS_BWD_MIN_BLOCKS)
+// NW: warps (= regions) per CTA, as in the forward (gs_raster.cu).
+#ifndef GS_BWD_WARPS
+#define GS_BWD_WARPS 4
+#endif
+
+template <int NW, bool HAS_GA>
+__global__ void __launch_bounds__(NW * 32, (GS_BWD_MIN_CTAS * 8) / NW)
 raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order, const uint2* __restrict__ ranges,
-                  const uint32_t* __restrict__ ids, const float4* __restrict__ feat, float bg0, float bg1, float bg2,
-                  const float* __restrict__ final_T, const uint32_t* __restrict__ n_contrib,
-                  const float* __restrict__ d_rgb, const float* __restrict__ d_depth, const float* __restrict__ d_alpha,
-                  float* __restrict__ g2d) {
-  constexpr int RPT = 8;  // 8x4-pixel regions per 16x16 tile
-  __shared__ __align__(16) float4 s_feat[2][(kWarpBatch + kGroup) * 3];  // records of the relevant entries, decoded in place
-  __shared__ uint32_t s_tag[2][kWarpBatch];
-  __shared__ __align__(16) float2 s_pair[kSlots * kPairRow];
-  __shared__ __align__(16) float4 s_pix[32];
-  const int lane = threadIdx.x;
-  const int tile = (int)__ldg(order + blockIdx.x / RPT), sub = blockIdx.x % RPT;
-  const int ox = (tile % tiles_x) * GS_TILE + (sub % 2) * 8, oy = (tile / tiles_x) * GS_TILE + (sub / 2) * 4;
-  const int lx = lane & 7, ly = lane >> 3;
-  const float fx0 = (float)lx, fy0 = (float)ly;
+                  const uint32_t* __restrict__ ids, const float2* __restrict__ inst_uv, const float4* __restrict__ feat,
+                  float bg0, float bg1, float bg2, const float* __restrict__ final_T,
+                  const uint32_t* __restrict__ n_contrib, const float* __restrict__ d_rgb,
+                  const float* __restrict__ d_depth, const float* __restrict__ d_alpha, float* __restrict__ g2d) {
+  static_assert(NW == 2 || NW == 4 || NW == 8, "64 producer threads are needed");
+  constexpr int CPT = 8 / NW;  // CTAs per tile
+  __shared__ StageBuf s_st[kStages];
+  // per warp: byte offsets (into the stage) of the round's relevant entries, back to front
+  __shared__ __align__(8) uint16_t s_idx[NW][kTileBatch + kGroup];
+  __shared__ __align__(16) float2 s_pair_all[NW][kSlots * kPairRow];
+  __shared__ __align__(16) float4 s_pix_all[NW][32];
+  __shared__ int s_nmax[NW];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int tile = (int)__ldg(order + blockIdx.x / CPT), sub = (blockIdx.x % CPT) * NW + warp;
+  const int tx0 = (tile % tiles_x) * GS_TILE, ty0 = (tile / tiles_x) * GS_TILE;
+  const int xo = (sub % 2) * 8, yo = (sub / 2) * 4;
+  const int X = xo + (lane & 7), Y = yo + (lane >> 3);  // tile-local pixel of this lane
+  const float fx0 = (float)X, fy0 = (float)Y;
   const uint2 range = ranges[tile];
   const size_t HW = (size_t)W * H;
+  float2* s_pair = s_pair_all[warp];
+  float4* s_pix = s_pix_all[warp];
   float T = 1.f, gC0 = 0.f, gC1 = 0.f, gC2 = 0.f, gD = 0.f, gA = 0.f;
   uint32_t last = 0;
-  {
-    const int X = ox + lx, Y = oy + ly;
-    if (X < W && Y < H) {
-      const size_t p = (size_t)Y * W + X;
-      T = final_T[p];
-      last = n_contrib[p];
-      gC0 = d_rgb[p]; gC1 = d_rgb[HW + p]; gC2 = d_rgb[2 * HW + p];
-      if (d_depth) gD = d_depth[p];
-      if (HAS_GA) gA = d_alpha[p];
-    }
+  if (tx0 + X < W && ty0 + Y < H) {
+    const size_t p = (size_t)(ty0 + Y) * W + (tx0 + X);
+    T = final_T[p];
+    last = n_contrib[p];
+    gC0 = d_rgb[p]; gC1 = d_rgb[HW + p]; gC2 = d_rgb[2 * HW + p];
+    if (d_depth) gD = d_depth[p];
+    if (HAS_GA) gA = d_alpha[p];
   }
   s_pix[lane] = make_float4(gC0, gC1, gC2, gD);
   float S = T * (gC0 * bg0 + gC1 * bg1 + gC2 * bg2);
-  const int n = (int)__reduce_max_sync(kFull, last);  // deepest blended list position of the region
-  const int nb = (n + kWarpBatch - 1) / kWarpBatch;
+  const int n_w = (int)__reduce_max_sync(kFull, last);  // deepest blended list position of the region
+  if (lane == 0) s_nmax[warp] = n_w;
+  if (tid < kStages) {  // padding records never pass: lo = -inf  =>  p2 = -inf
+    StageRec& pr = s_st[tid].rec[kPadIdx];
+    pr.g = make_float4(0.f, 0.f, 0.f, -INFINITY);
+    pr.c = make_float4(0.f, 0.f, 0.f, 0.f);
+    pr.uv = make_float2(0.f, 0.f);
+    pr.ent = 0u;
+  }
+  __syncthreads();
+  int n = 0;
+#pragma unroll
+  for (int k = 0; k < NW; ++k) n = max(n, s_nmax[k]);  // ... and of the CTA: entries beyond it are never staged
+  const int nb = (n + kTileBatch - 1) / kTileBatch;
   int nslot = 0;
   float2* pair_ptr = s_pair + lane;     // where this lane's (gp, w) of the next slot goes
-  SlotRec slot = {0.f, 0.f};  // record of slot (lane & 15), kept in registers
+  SlotRec slot = {0.f, 0.f};            // record of slot (lane & 15), kept in registers
   uint32_t slot_id = 0;
 
-  // phase 1: the list entries are (index << 8 | region mask) -- gs_bin_tiles already decided which regions of the tile
-  // a Gaussian can reach.  Lane g looks at entry g of the batch; the relevant ones are compacted in REVERSE list order
-  // (ballot rank) and only their records are staged, one batch ahead; tag = index << 5 | position in the batch.
-  auto issue = [&](int b, uint32_t v) -> int {
-    const bool relevant = (b * kWarpBatch + lane < n) && ((v >> sub) & 1u);
-    const unsigned rel = __ballot_sync(kFull, relevant);
-    const int cnt = __popc(rel);
-    if (relevant) {
-      const int r = cnt - 1 - __popc(rel & ((1u << lane) - 1u));
-      const float4* src = feat + 3 * (size_t)(v >> 8);
-      float4* dst = &s_feat[b & 1][r * 3];
-      cp_async16(dst, src); cp_async16(dst + 1, src + 1); cp_async16(dst + 2, src + 2);
-      s_tag[b & 1][r] = ((v >> 8) << 5) | (uint32_t)lane;
+  // producer: rounds are staged back to front (list round nb - 1 first); thread t < 64 stages its entry t
+  uint32_t v_pre = 0;
+  int i_pre = (nb - 1) * kTileBatch + tid;  // list index of the entry this thread fetches next
+  auto prefetch = [&]() {
+    v_pre = (tid < kTileBatch && i_pre >= 0 && i_pre < n) ? __ldg(ids + range.x + i_pre) : 0u;
+    i_pre -= kTileBatch;
+  };
+  int i_pro = (nb - 1) * kTileBatch + tid, st_pro = 0;
+  auto produce = [&]() {
+    if (tid < kTileBatch && i_pro >= 0) {
+      StageRec& r = s_st[st_pro].rec[tid];
+      r.ent = v_pre;
+      if (i_pro < n) {
+        const float4* src = feat + 3 * (size_t)(v_pre >> 8) + 1;
+        cp_async16(&r.g, src);
+        cp_async16(&r.c, src + 1);
+        cp_async8(&r.uv, inst_uv + range.x + i_pro);
+      }
     }
     cp_async_commit();
-    return cnt;
+    i_pro -= kTileBatch;
+    st_pro = st_pro + 1 == kStages ? 0 : st_pro + 1;
   };
-  uint32_t v_next = 0;
-  int nrel = 0, nrel_next = 0;
-  if (nb > 0) {
-    const int i0 = (nb - 1) * kWarpBatch + lane;
-    nrel_next = issue(nb - 1, i0 < n ? __ldg(ids + range.x + i0) : 0u);
-    if (nb > 1) v_next = __ldg(ids + range.x + (nb - 2) * kWarpBatch + lane);
-  }
-  for (int b = nb - 1; b >= 0; --b) {
-    nrel = nrel_next;
-    if (b >= 1) {
-      nrel_next = issue(b - 1, v_next);
-      if (b >= 2) v_next = __ldg(ids + range.x + (b - 2) * kWarpBatch + lane);
-      cp_async_wait<1>();
-    } else {
-      cp_async_wait<0>();
-    }
-    __syncwarp();
+  prefetch(); produce();
+  prefetch(); produce();
+  prefetch();
+  int st_con = 0;
+  for (int j = nb - 1; j >= 0; --j) {  // list rounds, back to front
+    cp_async_wait<1>();  // this thread's copies of this round have landed ...
+    __syncthreads();     // ... everybody's have, and every warp has finished the previous round, whose stage is refilled next
+    produce();
+    prefetch();
+    const StageBuf& sb = s_st[st_con];
+    st_con = st_con + 1 == kStages ? 0 : st_con + 1;
+    const int pbase = j * kTileBatch;
+    if (pbase >= n_w) continue;      // nothing of this round was blended in this region
+    // the entries of this round that can reach this warp's region and lie in front of its deepest blended position, as
+    // a list of byte offsets in REVERSE list order
+    const bool r0 = ((sb.rec[lane].ent >> sub) & 1u) && pbase + lane < n_w;
+    const bool r1 = ((sb.rec[lane + 32].ent >> sub) & 1u) && pbase + 32 + lane < n_w;
+    const unsigned b0 = __ballot_sync(kFull, r0), b1 = __ballot_sync(kFull, r1);
+    const int n1 = __popc(b1), nrel = n1 + __popc(b0);
     if (nrel == 0) continue;
-    const int lastb = (int)last - b * kWarpBatch;  // entries of this batch at positions < lastb were blended by this pixel
-    float4* sf = s_feat[b & 1];
-    if (lane < nrel) {  // decode once per (region, Gaussian), in place: whitened region-local record (gs_raster.cuh)
-      const float4 f0 = sf[3 * lane], f1 = sf[3 * lane + 1];
-      float u0, v0, mx, my;
-      decode_whitened(f0, f1, ox, oy, u0, v0, mx, my);
-      sf[3 * lane] = make_float4(u0, v0, f1.x, f1.y);
-      sf[3 * lane + 1] = make_float4(f1.z, f0.w, __uint_as_float(s_tag[b & 1][lane]), 0.f);
-    }
-    if (lane < kGroup) {  // padding records never pass: lo = -inf  =>  p2 = -inf
-      sf[3 * (nrel + lane)] = make_float4(0.f, 0.f, 0.f, 0.f);
-      sf[3 * (nrel + lane) + 1] = make_float4(0.f, -INFINITY, 0.f, 0.f);
-    }
+    const unsigned gt = ~((2u << lane) - 1u);  // lanes above this one
+    uint16_t* idx = s_idx[warp];
+    if (r1) idx[__popc(b1 & gt)] = (uint16_t)((32 + lane) * 48);
+    if (r0) idx[n1 + __popc(b0 & gt)] = (uint16_t)(lane * 48);
+    if (lane < kGroup) idx[nrel + lane] = (uint16_t)(kPadIdx * 48);
     __syncwarp();
-    for (int r0 = 0; r0 < nrel; r0 += kGroup) {  // back to front, four list entries at a time
-      float4 a0[kGroup], a1[kGroup];
+    const int lastb48 = ((int)last - pbase) * 48;  // entries of this round at offsets < lastb48 were blended by this pixel
+    const char* recs = reinterpret_cast<const char*>(sb.rec);
+    for (int r = 0; r < nrel; r += kGroup) {  // back to front, four list entries at a time
+      const uint2 o4 = *reinterpret_cast<const uint2*>(idx + r);
+      const uint32_t off[kGroup] = {o4.x & 0xffffu, o4.x >> 16, o4.y & 0xffffu, o4.y >> 16};
+      float2 uv[kGroup];
       float p[kGroup];
       bool hit[kGroup];
       unsigned bal[kGroup];
 #pragma unroll
       for (int q = 0; q < kGroup; ++q) {
-        a0[q] = sf[3 * (r0 + q)];      // u0, v0, l11, l21
-        a1[q] = sf[3 * (r0 + q) + 1];  // l22, lo, tag
-        p[q] = eval_power(a0[q].x, a0[q].y, a0[q].z, a0[q].w, a1[q].x, a1[q].y, fx0, fy0);
+        const StageRec& e = *reinterpret_cast<const StageRec*>(recs + off[q]);
+        const float4 a0 = e.g;  // l11, l21, l22, lo
+        uv[q] = e.uv;
+        p[q] = eval_power(uv[q].x, uv[q].y, a0.x, a0.y, a0.z, a0.w, fx0, fy0);
         // blended by the forward: alpha >= 1/255 and in front of the pixel's last contributor
-        hit[q] = p[q] >= GS_POWER_MIN && (int)(__float_as_uint(a1[q].z) & 31u) < lastb;
+        hit[q] = p[q] >= GS_POWER_MIN && (int)off[q] < lastb48;
         bal[q] = __ballot_sync(kFull, hit[q]);
       }
 #pragma unroll
       for (int q = 0; q < kGroup; ++q) {
         if (bal[q] == 0) continue;  // the Gaussian reaches no pixel of the region
-        float gp = 0.f, w = 0.f;
-        if (hit[q]) {
-          const float4 f2 = sf[3 * (r0 + q) + 2];
-          const float og = ex2_approx(p[q]);  // opacity * G: log2(opacity) is folded into the exponent
-          const float a = fminf(GS_ALPHA_MAX, og);
-          const float ioma = rcp_approx(1.f - a);
-          T *= ioma;  // transmittance in front of this Gaussian
-          w = a * T;
-          float wi = fmaf(gC0, f2.x, fmaf(gC1, f2.y, fmaf(gC2, f2.z, gD * f2.w)));
-          if (HAS_GA) wi += gA;
-          const float dalpha = fmaf(T, wi, -S * ioma);
-          S = fmaf(wi, w, S);
-          gp = (og <= GS_ALPHA_MAX) ? a * dalpha : 0.f;  // no gradient through the clamp (Q2)
-        }
+        const StageRec& e = *reinterpret_cast<const StageRec*>(recs + off[q]);
+        // branch-free: a lane that is not hit runs the same instructions with alpha = 0 (T, S unchanged, gp = w = 0)
+        const float4 f2 = e.c;
+        const float og = ex2_approx(p[q]);  // opacity * G: log2(opacity) is folded into the exponent
+        const float a = hit[q] ? fminf(GS_ALPHA_MAX, og) : 0.f;
+        const float ioma = rcp_approx(1.f - a);
+        T *= ioma;  // transmittance in front of this Gaussian
+        const float w = a * T;
+        float wi = fmaf(gC0, f2.x, fmaf(gC1, f2.y, fmaf(gC2, f2.z, gD * f2.w)));
+        if (HAS_GA) wi += gA;
+        const float dalpha = fmaf(T, wi, -S * ioma);
+        S = fmaf(wi, w, S);
+        const float gp = (og <= GS_ALPHA_MAX) ? a * dalpha : 0.f;  // no gradient through the clamp (Q2)
         *pair_ptr = make_float2(gp, w);
         pair_ptr += kPairRow;
         if ((lane & (kSlots - 1)) == nslot) {
-          slot.u0 = a0[q].x; slot.v0 = a0[q].y;
-          slot_id = __float_as_uint(a1[q].z) >> 5;
+          slot.u0 = uv[q].x; slot.v0 = uv[q].y;
+          slot_id = e.ent >> 8;
         }
         if (++nslot == kSlots) {
-          gaussian_phase<2>(s_pair, s_pix, kSlots, lane, slot, slot_id, feat, g2d);
+          gaussian_phase<2>(s_pair, s_pix, kSlots, lane, slot, slot_id, (float)xo, (float)yo, feat, g2d);
           nslot = 0;
           pair_ptr = s_pair + lane;
         }
       }
     }
-    __syncwarp();
   }
-  if (nslot > 8) gaussian_phase<2>(s_pair, s_pix, nslot, lane, slot, slot_id, feat, g2d);
-  else if (nslot > 0) gaussian_phase<4>(s_pair, s_pix, nslot, lane, slot, slot_id, feat, g2d);
+  cp_async_wait<0>();
+  if (nslot > 8) gaussian_phase<2>(s_pair, s_pix, nslot, lane, slot, slot_id, (float)xo, (float)yo, feat, g2d);
+  else if (nslot > 0) gaussian_phase<4>(s_pair, s_pix, nslot, lane, slot, slot_id, (float)xo, (float)yo, feat, g2d);
 }
 
 int launch_raster_bwd(gs_ctx* ctx, cudaStream_t s, const float* d_rgb, const float* d_depth, const float* d_alpha) {
-  const int units = ctx->cam.tiles_x * ctx->cam.tiles_y * 8;
-  if (units == 0) return GS_OK;
+  const int tiles = ctx->cam.tiles_x * ctx->cam.tiles_y;
+  if (tiles == 0) return GS_OK;
+  constexpr int NW = GS_BWD_WARPS;
 #define GS_BWD(GA)                                                                                                  \
-  raster_bwd_kernel<GA><<<units, 32, 0, s>>>(ctx->cam.W, ctx->cam.H, ctx->cam.tiles_x, ctx->tile_order, ctx->ranges, \
-                                             ctx->vals[ctx->sorted_buf], ctx->feat, ctx->bg[0], ctx->bg[1],         \
-                                             ctx->bg[2], ctx->final_T, ctx->n_contrib, d_rgb, d_depth, d_alpha,     \
-                                             ctx->g2d)
+  raster_bwd_kernel<NW, GA><<<tiles * (8 / NW), NW * 32, 0, s>>>(                                                   \
+      ctx->cam.W, ctx->cam.H, ctx->cam.tiles_x, ctx->tile_order, ctx->ranges, ctx->vals[ctx->sorted_buf], ctx->inst_uv, \
+      ctx->feat, ctx->bg[0], ctx->bg[1], ctx->bg[2], ctx->final_T, ctx->n_contrib, d_rgb, d_depth, d_alpha, ctx->g2d)
   if (d_alpha) GS_BWD(true); else GS_BWD(false);
 #undef GS_BWD
   GS_LAUNCH_CHECK("raster_bwd_kernel");
