@@ -53,3 +53,70 @@ def iso_loss(scales, lambda_s=10.0):
         loss += np.abs(s[i] - sbar).sum()
         g[i] = sg - sg.sum() / 3.0            # d/ds_ij sum_k |s_ik - sbar| with dsbar/ds_ij = 1/3
     return lambda_s * loss, lambda_s * g
+
+
+# ----------------------------------------------------------------------------------------------------------------------
+# Eq. 23: the refinement loss of the fused map on the exposure-compensated render
+#     I~(u) = e^{a_k} I^(u) + b_k,     L_rf = alpha' L1(I~, I) + lambda (1 - SSIM(I~, I)) + beta L1(D^, D-)  [+ lambda'_n L_normal]
+# with alpha' = (1 - lambda) + alpha = 1.75, lambda = 0.2 (lambda_n is garbled there -- reading Q16 -- and the
+# normal term is oracle/normals.py).  The paper does not define SSIM beyond its name.  Reading Q19: the
+# standard structural similarity index with an 11 x 11 Gaussian window of sigma 1.5 (normalised to sum 1), constants
+# C1 = 0.01^2, C2 = 0.03^2 (dynamic range 1), windowed moments by correlation with ZERO padding outside the image
+# (window always 11 x 11, so border pixels see zeros), computed per colour channel; SSIM(I~, I) = mean of the SSIM map
+# over all pixels and channels.
+# ----------------------------------------------------------------------------------------------------------------------
+SSIM_C1, SSIM_C2 = 0.01 ** 2, 0.03 ** 2
+
+
+def ssim_window(size=11, sigma=1.5):
+    g = np.exp(-((np.arange(size) - size // 2) ** 2) / (2.0 * sigma * sigma))
+    g /= g.sum()
+    return np.outer(g, g)
+
+
+def _win(img, w):
+    from scipy.signal import correlate2d
+    return correlate2d(img, w, mode="same", boundary="fill", fillvalue=0.0)
+
+
+def ssim_terms(x, y):
+    """SSIM map of one channel pair [H,W] and the partial derivatives of the map w.r.t. the windowed moments of x:
+    returns (s, ds/dm1, ds/de11, ds/de12) with m1 = W*x, e11 = W*x^2, e12 = W*(x y)."""
+    w = ssim_window()
+    m1, m2 = _win(x, w), _win(y, w)
+    e11, e22, e12 = _win(x * x, w), _win(y * y, w), _win(x * y, w)
+    n1, n2 = 2 * m1 * m2 + SSIM_C1, 2 * (e12 - m1 * m2) + SSIM_C2
+    d1, d2 = m1 * m1 + m2 * m2 + SSIM_C1, (e11 - m1 * m1) + (e22 - m2 * m2) + SSIM_C2
+    s = n1 * n2 / (d1 * d2)
+    ds_dm1 = (2 * m2 * n2 - 2 * m2 * n1) / (d1 * d2) - s * (2 * m1 / d1 - 2 * m1 / d2)
+    ds_de11 = -s / d2
+    ds_de12 = 2 * n1 / (d1 * d2)
+    return s, ds_dm1, ds_de11, ds_de12
+
+
+def ssim_mean(x, y):
+    """Mean SSIM over pixels and channels of [3,H,W] images, and its gradient w.r.t. x (plain chain rule: every moment is
+    a correlation with the symmetric window, whose adjoint under zero padding is the same correlation)."""
+    x = np.asarray(x, np.float64); y = np.asarray(y, np.float64)
+    C, H, W = x.shape
+    w = ssim_window()
+    total, g = 0.0, np.zeros_like(x)
+    for c in range(C):
+        s, a, b11, b12 = ssim_terms(x[c], y[c])
+        total += s.sum()
+        g[c] = _win(a, w) + 2.0 * x[c] * _win(b11, w) + y[c] * _win(b12, w)
+    n = C * H * W
+    return total / n, g / n
+
+
+def refine_loss(rgb, depth, target_rgb, target_depth, a, b, alpha_p=1.75, lam=0.2, beta=0.25):
+    """Eq. 23 without the normal term.  Returns a dict: the terms, the total, dL/dI^ [3,H,W], dL/dD^ [H,W], dL/da, dL/db."""
+    rgb = np.asarray(rgb, np.float64)
+    ea = float(np.exp(a))
+    it = ea * rgb + float(b)                                   # I~ = e^a I^ + b
+    l1, ld, g1, gd = l1_terms(it, depth, target_rgb, target_depth)
+    sm, gs = ssim_mean(it, np.asarray(target_rgb, np.float64))
+    g_it = alpha_p * g1 - lam * gs                             # dL / dI~
+    total = alpha_p * l1 + lam * (1.0 - sm) + beta * ld
+    return dict(l1_rgb=l1, ssim=sm, l1_depth=ld, total=total, d_rgb=ea * g_it, d_depth=beta * gd,
+                g_a=float((g_it * ea * rgb).sum()), g_b=float(g_it.sum()))
