@@ -182,6 +182,19 @@ GS_API int gs_loss_map(void* stream, int32_t width, int32_t height, const float*
  * DEVICE double loss[2]: loss[0] = the weighted loss (loss[1] is scratch). */
 GS_API int gs_loss_iso(void* stream, int64_t N, const float* scales, float lambda_s, float* g_scales, double* loss);
 
+/* ---- refinement loss of the fused map, Eq. 23, without its normal term (gs_loss_normal) ---------- */
+/* On the exposure-compensated render I~ = e^a I^ + b (per-keyframe log-gain a and bias b):
+ *     L = alpha' L1(I~, I) + lambda (1 - SSIM(I~, I)) + beta L1(D^, D-)       (paper: alpha' = 1.75, lambda = 0.2, beta = 0.25).
+ * Readings: Q19 SSIM = 11 x 11 Gaussian window of sigma 1.5, C1 = 0.01^2, C2 = 0.03^2, zero padding, per channel,
+ * mean over pixels and channels; Q18 mean reductions, depth term where target_depth > 0, sign(0) = 0.
+ * Inputs DEVICE: rgb, target_rgb [3,H,W]; depth, target_depth [H,W]; ab float[2] = (a, b).  Outputs DEVICE: d_rgb [3,H,W] =
+ * dL/dI^ and d_depth [H,W] = dL/dD^ (directly the upstream gradients of gs_rasterize_bwd); g_ab float[2] = (dL/da, dL/db);
+ * loss double[8] = { L1(I~,I), SSIM(I~,I), L1(D^,D-), L, dL/da, dL/db, scratch, scratch }.  work: DEVICE scratch of 9 H W floats.
+ * Asynchronous on `stream` (three launches); all arrays caller-owned.  GS_E_INVALID on a null pointer or an empty image. */
+GS_API int gs_loss_refine(void* stream, int32_t width, int32_t height, const float* rgb, const float* depth,
+                          const float* target_rgb, const float* target_depth, const float* ab, float alpha_p, float lambda,
+                          float beta, float* d_rgb, float* d_depth, float* g_ab, float* work, double* loss);
+
 /* ---- Eq. 19: a submap's Sim(3) correction applied to its Gaussians --------------------------------- */
 /* mu' = s R mu + t, s_i' = s s_i, q' = q_R (x) q (so that Sigma' = s^2 R Sigma R^T); opacity and colour are unchanged
  * and are not arguments.  s > 0, R row-major float[9] (a rotation), t float[3]: HOST.  means, scales

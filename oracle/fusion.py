@@ -54,3 +54,126 @@ def sim3_apply(means, scales, quats, s, R, t):
 def covariance(scales_i, quat_i):
     Rq = rotation_of_quat(quat_i)
     return Rq @ np.diag(np.asarray(scales_i, np.float64) ** 2) @ Rq.T
+
+
+# ----------------------------------------------------------------------------------------------------------------------
+# Eqs. 20-22: occupancy-aware fusion on "a frustum-aware occupancy grid of voxel size v"
+#   O_occ  = U_i   { kappa(x) : x in [mu_i - k s_i, mu_i + k s_i] }                      (Eq. 20, target Gaussians)
+#   O_free = U_u,k { kappa(c_k + t (r_k(u) - c_k)) : t in [0, 1) }                       (Eq. 21, keyframe depth maps)
+#   a borrowed Gaussian j is retained iff kappa(mu_j) not in O_occ and not in O_free       (Eq. 22)
+# "We pack each voxel index kappa(.) into a 64-bit spatial-hash key".
+# Readings (Q21): kappa(x) = floor(x / v) per axis (fp64 division of the fp32 inputs); key = three 21-bit
+# fields (index + 2^20) packed x | y << 21 | z << 42; the box of Eq. 20 is axis-aligned in world coordinates with half
+# extents k s_i component-wise (the paper's interval notation; the Gaussian's rotation is ignored); r_k(u) is the
+# back-projection of pixel u (integer-centred, Q7) at its depth D_k(u) (camera-space z), c_k the camera centre; pixels with
+# depth <= 0 cast no ray; v and k are arguments (unpublished).  The voxel set of a ray is computed by the 3-D DDA
+# (Amanatides & Woo) written out below in fp64, one IEEE operation at a time -- the CUDA path follows the same sequence, so
+# the sets agree bit for bit; `ray_voxels_by_definition` is the independent plain definition used to pin it.
+# ----------------------------------------------------------------------------------------------------------------------
+KEY_BIAS = 1 << 20
+
+
+def pack_key(ix, iy, iz):
+    ix = np.asarray(ix, np.int64) + KEY_BIAS; iy = np.asarray(iy, np.int64) + KEY_BIAS; iz = np.asarray(iz, np.int64) + KEY_BIAS
+    assert ((ix >= 0) & (ix < (1 << 21)) & (iy >= 0) & (iy < (1 << 21)) & (iz >= 0) & (iz < (1 << 21))).all()
+    return (ix | (iy << 21) | (iz << 42)).astype(np.uint64)
+
+
+def kappa(x, v):
+    """Voxel index of points x [...,3]: floor(x / v) in fp64."""
+    return np.floor(np.asarray(x, np.float64) / np.float64(v)).astype(np.int64)
+
+
+def occupied_set(means, scales, v, k):
+    """Eq. 20 as a Python set of packed keys: every voxel meeting the closed box [mu - k s, mu + k s]."""
+    means = np.asarray(means, np.float64); scales = np.asarray(scales, np.float64)
+    out = set()
+    for i in range(means.shape[0]):
+        lo = kappa(means[i] - np.float64(k) * scales[i], v)
+        hi = kappa(means[i] + np.float64(k) * scales[i], v)
+        for iz in range(lo[2], hi[2] + 1):
+            for iy in range(lo[1], hi[1] + 1):
+                for ix in range(lo[0], hi[0] + 1):
+                    out.add(int(pack_key(ix, iy, iz)))
+    return out
+
+
+def ray_voxels(c, r, v):
+    """Voxels met by the half-open segment c + t (r - c), t in [0, 1): 3-D DDA in fp64.  Returns a list of (ix,iy,iz)."""
+    c = np.asarray(c, np.float64); r = np.asarray(r, np.float64); v = np.float64(v)
+    d = r - c
+    idx = np.floor(c / v).astype(np.int64)
+    step = np.zeros(3, np.int64); t_max = np.full(3, np.inf); t_delta = np.full(3, np.inf)
+    for a in range(3):
+        if d[a] > 0:
+            step[a] = 1
+            t_max[a] = ((np.float64(idx[a]) + 1.0) * v - c[a]) / d[a]
+            t_delta[a] = v / d[a]
+        elif d[a] < 0:
+            step[a] = -1
+            t_max[a] = (np.float64(idx[a]) * v - c[a]) / d[a]
+            t_delta[a] = -v / d[a]
+    out = [tuple(int(q) for q in idx)]
+    while True:
+        a = 0                                  # axis of the nearest boundary; ties -> lowest axis
+        if t_max[1] < t_max[a]:
+            a = 1
+        if t_max[2] < t_max[a]:
+            a = 2
+        if not (t_max[a] < 1.0):               # the next boundary lies at t >= 1: outside the half-open segment
+            break
+        idx[a] += step[a]
+        t_max[a] = t_max[a] + t_delta[a]
+        out.append(tuple(int(q) for q in idx))
+    return out
+
+
+def ray_voxels_by_definition(c, r, v):
+    """The plain definition of Eq. 21 for one ray: kappa at the midpoints between consecutive boundary crossings of the
+    open parameter interval (0, 1) (and at t -> 0+).  Equals ray_voxels except on measure-zero ties."""
+    c = np.asarray(c, np.float64); r = np.asarray(r, np.float64); d = r - c
+    ts = [0.0, 1.0]
+    for a in range(3):
+        if d[a] != 0:
+            lo, hi = sorted((c[a], r[a]))
+            for m in range(int(np.floor(lo / v)) - 1, int(np.floor(hi / v)) + 2):
+                t = (m * v - c[a]) / d[a]
+                if 0.0 < t < 1.0:
+                    ts.append(t)
+    ts = sorted(set(ts))
+    return {tuple(int(q) for q in np.floor((c + 0.5 * (t0 + t1) * d) / v)) for t0, t1 in zip(ts[:-1], ts[1:])}
+
+
+def backproject(depth, fx, fy, cx, cy, T_cw, stride=1):
+    """Camera centre c_k and world-space surface points r_k(u) of the pixels (every `stride`-th in x and y) with depth > 0:
+    p_c = ((u - cx) z / fx, (v - cy) z / fy, z), r = R^T (p_c - t)   (world-to-camera pose)."""
+    depth = np.asarray(depth, np.float64)
+    T = np.asarray(T_cw, np.float64).reshape(3, 4)
+    R, t = T[:, :3], T[:, 3]
+    c = -(R.T @ t)
+    H, W = depth.shape
+    pts = []
+    for y in range(0, H, stride):
+        for x in range(0, W, stride):
+            z = depth[y, x]
+            if z > 0.0:
+                pc = np.array([(x - np.float64(cx)) * z / np.float64(fx), (y - np.float64(cy)) * z / np.float64(fy), z])
+                pts.append(R.T @ (pc - t))
+    return c, np.asarray(pts).reshape(-1, 3)
+
+
+def free_set(depth, fx, fy, cx, cy, T_cw, v, stride=1):
+    """Eq. 21 for one keyframe as a Python set of packed keys."""
+    c, pts = backproject(depth, fx, fy, cx, cy, T_cw, stride)
+    out = set()
+    for r in pts:
+        for (ix, iy, iz) in ray_voxels(c, r, v):
+            out.add(int(pack_key(ix, iy, iz)))
+    return out
+
+
+def retain_mask(means, occ, free, v):
+    """Eq. 22: True where kappa(mu_j) is in neither set."""
+    idx = kappa(means, v)
+    keys = pack_key(idx[:, 0], idx[:, 1], idx[:, 2])
+    return np.array([(int(q) not in occ) and (int(q) not in free) for q in keys], dtype=bool)

@@ -22,7 +22,7 @@ STATUS = {0: "GS_OK", -1: "GS_E_INVALID", -2: "GS_E_ORDER", -3: "GS_E_CUDA", -4:
 EXPORTS = ["gs_create", "gs_destroy", "gs_last_error", "gs_preprocess", "gs_bin_tiles", "gs_rasterize_fwd",
            "gs_rasterize_bwd", "gs_pose_grad", "gs_get_counts", "gs_get_binning", "gs_get_features", "gs_poll",
            "gs_aux_l1_grad", "gs_aux_pose_step", "gs_fwd_bwd_host", "gs_profile_enable", "gs_profile_read",
-           "gs_get_launch_count", "gs_get_workload", "gs_loss_map", "gs_loss_iso", "gs_sim3_apply", "gs_measure_peaks"]
+           "gs_get_launch_count", "gs_get_workload", "gs_loss_map", "gs_loss_iso", "gs_sim3_apply", "gs_measure_peaks", "gs_loss_refine"]
 PEAKS = ["fma_tlanes", "issue_twarp", "ex2_tlanes", "lds128_bcast_twarp", "lds128_twarp", "lds32_bcast_twarp",
          "lds64_bcast_twarp", "red_glanes", "hbm_read_gbs", "hbm_write_gbs", "hbm_copy_gbs", "sm_count", "sm_mhz_max"]
 STAGES = ["preprocess", "tile_scan", "emit", "tile_sort", "raster_fwd", "raster_bwd", "gauss_bwd", "pose_grad"]
@@ -66,6 +66,7 @@ def load_library():
     lib.gs_aux_pose_step.argtypes = [vp, vp, vp, f]
     lib.gs_loss_map.argtypes = [vp, C.c_int32, C.c_int32, vp, vp, vp, vp, f, f, vp, vp, vp]
     lib.gs_loss_iso.argtypes = [vp, i64, vp, f, vp, vp]
+    lib.gs_loss_refine.argtypes = [vp, C.c_int32, C.c_int32, vp, vp, vp, vp, vp, f, f, f, vp, vp, vp, vp, vp]
     lib.gs_sim3_apply.argtypes = [vp, i64, f, C.POINTER(f * 9), C.POINTER(f * 3), vp, vp, vp, vp, vp, vp]
     lib.gs_profile_enable.argtypes = [vp, C.c_int]
     lib.gs_profile_read.argtypes = [vp, C.POINTER(f * 8)]
@@ -273,6 +274,21 @@ def gs_loss_map(rgb, depth, target_rgb, target_depth, alpha, beta, d_rgb, d_dept
                                     _ptr(loss, torch.float64))
     if rc != 0:
         raise GsError(rc, "gs_loss_map")
+
+
+def gs_loss_refine(rgb, depth, target_rgb, target_depth, ab, alpha_p, lam, beta, d_rgb, d_depth, g_ab, work, loss, stream=None):
+    """Eq. 23 (without the normal term) on the exposure-compensated render: writes the upstream gradients, (dL/da, dL/db)
+    and double loss[8] (device).  work: float scratch of 9 H W elements."""
+    import torch
+    f32 = torch.float32
+    H, W = depth.shape
+    assert work.numel() >= 9 * H * W
+    rc = load_library().gs_loss_refine(_stream(stream), int(W), int(H), _ptr(rgb, f32), _ptr(depth, f32), _ptr(target_rgb, f32),
+                                       _ptr(target_depth, f32), _ptr(ab, f32), float(alpha_p), float(lam), float(beta),
+                                       _ptr(d_rgb, f32), _ptr(d_depth, f32), _ptr(g_ab, f32), _ptr(work, f32),
+                                       _ptr(loss, torch.float64))
+    if rc != 0:
+        raise GsError(rc, "gs_loss_refine")
 
 
 def gs_loss_iso(scales, lambda_s, g_scales, loss, stream=None):

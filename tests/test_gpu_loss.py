@@ -66,3 +66,37 @@ def test_loss_iso_matches_oracle_and_accumulates():
     b.gs_loss_iso(torch.zeros(0, 3, device="cuda"), 10.0, torch.zeros(0, 3, device="cuda"), loss)
     torch.cuda.synchronize()
     assert float(loss[0]) == 0.0
+
+
+@pytest.mark.parametrize("shape", [(680, 1200), (33, 47), (5, 7), (16, 16)])   # full size, ragged tiles, smaller than the window
+def test_loss_refine_matches_oracle(shape):
+    """Eq. 23 on the exposure-compensated render: sums within 1e-6 relative, image gradients within
+    1e-4 relative L2 and 1e-5 / (3 H W) absolute (fp32 window sums against the fp64 oracle), (dL/da, dL/db) within 1e-5."""
+    import torch
+    from oracle import loss as ol
+    from paper_2605_10760_b200 import binding as b
+    H, W = shape
+    rgb, d, trgb, td = _images(11 + H, H, W)
+    a, bb = 0.11, -0.03
+    ref = ol.refine_loss(rgb, d, trgb, td, np.float32(a), np.float32(bb), 1.75, 0.2, 0.25)
+    t = lambda x: torch.from_numpy(np.ascontiguousarray(x, np.float32)).cuda()
+    o_rgb = torch.empty(3, H, W, device="cuda"); o_d = torch.empty(H, W, device="cuda")
+    g_ab = torch.zeros(2, device="cuda"); work = torch.empty(9 * H * W, device="cuda")
+    loss = torch.full((8,), -1.0, dtype=torch.float64, device="cuda")
+    b.gs_loss_refine(t(rgb), t(d), t(trgb), t(td), t(np.array([a, bb])), 1.75, 0.2, 0.25, o_rgb, o_d, g_ab, work, loss)
+    torch.cuda.synchronize()
+    got = loss.cpu().numpy()
+    for k, name in enumerate(("l1_rgb", "ssim", "l1_depth", "total")):
+        assert abs(got[k] - ref[name]) <= 2e-6 * abs(ref[name]) + 1e-12, (name, got[k], ref[name])
+    gr = o_rgb.cpu().numpy().astype(np.float64)
+    # pixels where I~ - I is a rounding-level tie may take the other sign of the L1 sub-gradient: compare off those
+    it = np.exp(np.float64(np.float32(a))) * rgb.astype(np.float64) + np.float64(np.float32(bb))
+    tie = np.abs(it - trgb) < 1e-6
+    diff = np.where(tie, 0.0, gr - ref["d_rgb"])
+    assert np.linalg.norm(diff) <= 1e-4 * np.linalg.norm(ref["d_rgb"])
+    assert np.abs(diff).max() <= 1e-5 / (3 * H * W) * 50
+    assert np.allclose(o_d.cpu().numpy(), ref["d_depth"], rtol=2e-7, atol=0)
+    ga, gb = g_ab.cpu().numpy()
+    scale = max(abs(ref["g_a"]), abs(ref["g_b"]), 1e-3)
+    assert abs(ga - ref["g_a"]) <= 2e-5 * scale and abs(gb - ref["g_b"]) <= 2e-5 * scale, (ga, gb, ref["g_a"], ref["g_b"])
+    assert abs(got[4] - ref["g_a"]) <= 2e-5 * scale and abs(got[5] - ref["g_b"]) <= 2e-5 * scale
