@@ -203,6 +203,53 @@ GS_API int gs_loss_refine(void* stream, int32_t width, int32_t height, const flo
 GS_API int gs_sim3_apply(void* stream, int64_t N, float s, const float* R, const float* t, const float* means,
                          const float* scales, const float* quats, float* means_out, float* scales_out, float* quats_out);
 
+/* ---- Eqs. 20-22: occupancy-aware fusion ---------------------------------------------------- */
+/* Voxel sets are open-addressing hash tables of 64-bit spatial-hash keys in CALLER-provided DEVICE memory: uint64
+ * table[capacity], capacity a power of two, empty slot = 0xFFFFFFFFFFFFFFFF.  Readings (Q21): kappa(x) = floor(x / v)
+ * per axis (fp64), key = (ix + 2^20) | (iy + 2^20) << 21 | (iz + 2^20) << 42; the box of Eq. 20 is axis-aligned in world
+ * coordinates with half extents k s_i; r_k(u) = back-projection of integer-centred pixel u at its camera-space depth; pixels
+ * with depth <= 0 cast no ray; the voxels of a ray are those of the 3-D DDA in fp64 (bit-identical to the plain definition
+ * of Eq. 21).  v (voxel) and k are unpublished: arguments.  `overflow` (DEVICE uint32, caller-zeroed) counts keys that
+ * could not be stored (table full, index beyond 21 bits, non-finite input): the sets are exact iff it stays 0.
+ * All calls are asynchronous on `stream`; GS_E_INVALID on null pointers, non-power-of-two capacities, voxel <= 0. */
+GS_API int gs_voxel_set_clear(void* stream, uint64_t* table, int64_t capacity);
+/* O_occ (Eq. 20) of target Gaussians: DEVICE means, scales [N,3] (activated scales). */
+GS_API int gs_voxel_insert_boxes(void* stream, uint64_t* table, int64_t capacity, float voxel, float k, int64_t N,
+                                 const float* means, const float* scales, uint32_t* overflow);
+/* O_free (Eq. 21) of one keyframe: cam HOST (intrinsics, world-to-camera pose), DEVICE depth [H,W]; every `stride`-th pixel
+ * in x and y casts a ray (stride 1 = every pixel, as in the paper). */
+GS_API int gs_voxel_insert_rays(void* stream, uint64_t* table, int64_t capacity, float voxel, const gs_camera* cam,
+                                const float* depth, int32_t stride, uint32_t* overflow);
+/* Eq. 22: retain[j] = 1 iff kappa(mu_j) is in neither set (either table may be NULL = empty set).  DEVICE uint8 retain[N]. */
+GS_API int gs_voxel_retain(void* stream, const uint64_t* occ, int64_t occ_capacity, const uint64_t* free_set,
+                           int64_t free_capacity, float voxel, int64_t N, const float* means, uint8_t* retain);
+
+/* ---- optimiser step and pruning of the refinement ------------------------------------------------ */
+/* The five parameter arrays of a Gaussian set (DEVICE pointers; shapes as in gs_preprocess: [N,3], [N,3], [N,4], [N], [N,K,3]). */
+typedef struct { float* means; float* scales; float* quats; float* opacities; float* sh; } gs_gaussians;
+typedef struct {
+  float lr_means, lr_scales, lr_quats, lr_opacities, lr_sh; /* learning rate per parameter group */
+  float beta1, beta2, eps;                                  /* Adam constants (0.9, 0.999, 1e-15) */
+  int32_t step;                                             /* 1-based iteration number t of the bias correction */
+} gs_adam_config;
+/* One fused Adam step (reading Q20: the paper says only "gradient descent" and "learning rate"): Kingma & Ba
+ * Algorithm 1 with bias correction; centres, raw quaternions and SH directly, scales through log s and opacities through
+ * logit o, so the ACTIVATED values of this ABI stay in (0, inf) / (0, 1).  grads = gradients w.r.t. the activated values
+ * (the outputs of gs_rasterize_bwd); m, v = first / second moments, same shapes as the parameters, caller-zeroed at start.
+ * visible: NULL, or DEVICE uint32[N]: only Gaussians with a non-zero entry are touched (parameters and moments).
+ * cfg HOST.  In place, asynchronous (five launches).  GS_E_INVALID on null pointers, degree outside 0..3, step < 1. */
+GS_API int gs_adam_step(void* stream, int64_t N, int sh_degree, const gs_adam_config* cfg, const gs_gaussians* params,
+                        const gs_gaussians* grads, const gs_gaussians* m, const gs_gaussians* v, const uint32_t* visible);
+/* keep[i] = opacities[i] >= min_opacity  ("prunes Gaussians with opacity below 0.005").  DEVICE uint8 keep[N]. */
+GS_API int gs_prune_mask(void* stream, int64_t N, const float* opacities, float min_opacity, uint8_t* keep);
+/* Order-preserving stream compaction, shared by pruning and by the retain test of Eq. 22.  gs_compact_plan turns a keep
+ * mask into index[i] = destination row of Gaussian i (0xFFFFFFFF if dropped) and the DEVICE count n_kept; work = DEVICE
+ * scratch of gs_compact_work_bytes(N) bytes.  gs_compact_rows gathers the kept rows of one [N,width] float array into
+ * `out` (must not alias `in`; rows beyond n_kept are untouched).  N < 2^32. */
+GS_API int64_t gs_compact_work_bytes(int64_t N);
+GS_API int gs_compact_plan(void* stream, int64_t N, const uint8_t* keep, uint32_t* index, int64_t* n_kept, void* work);
+GS_API int gs_compact_rows(void* stream, int64_t N, int32_t width, const uint32_t* index, const float* in, float* out);
+
 /* ---- measured machine peaks: the denominators of bench.py's roofline entries -------- */
 /* Runs small synthetic kernels on `device` (allocates and frees ~2 GiB, synchronises; ~0.2 s) and fills HOST double
  * out[GS_NUM_PEAKS]:  FP32 FMA lane rate (T lane-FMA/s; x2 = TFLOP/s), mixed FFMA+integer issue rate (T warp

@@ -150,16 +150,20 @@ def backproject(depth, fx, fy, cx, cy, T_cw, stride=1):
     depth = np.asarray(depth, np.float64)
     T = np.asarray(T_cw, np.float64).reshape(3, 4)
     R, t = T[:, :3], T[:, 3]
-    c = -(R.T @ t)
+    fx, fy, cx, cy = np.float64(fx), np.float64(fy), np.float64(cx), np.float64(cy)
+    # every sum is written out left to right, one IEEE operation at a time (no library matrix product: its summation order
+    # and use of fused multiply-adds are not defined), so that the CUDA path can follow the same sequence bit for bit
+    c = np.array([-((R[0, a] * t[0] + R[1, a] * t[1]) + R[2, a] * t[2]) for a in range(3)])
     H, W = depth.shape
     pts = []
     for y in range(0, H, stride):
         for x in range(0, W, stride):
             z = depth[y, x]
             if z > 0.0:
-                pc = np.array([(x - np.float64(cx)) * z / np.float64(fx), (y - np.float64(cy)) * z / np.float64(fy), z])
-                pts.append(R.T @ (pc - t))
-    return c, np.asarray(pts).reshape(-1, 3)
+                pc = ((np.float64(x) - cx) * z / fx, (np.float64(y) - cy) * z / fy, z)
+                q = (pc[0] - t[0], pc[1] - t[1], pc[2] - t[2])
+                pts.append([(R[0, a] * q[0] + R[1, a] * q[1]) + R[2, a] * q[2] for a in range(3)])
+    return c, np.asarray(pts, np.float64).reshape(-1, 3)
 
 
 def free_set(depth, fx, fy, cx, cy, T_cw, v, stride=1):

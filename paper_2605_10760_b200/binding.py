@@ -22,7 +22,9 @@ STATUS = {0: "GS_OK", -1: "GS_E_INVALID", -2: "GS_E_ORDER", -3: "GS_E_CUDA", -4:
 EXPORTS = ["gs_create", "gs_destroy", "gs_last_error", "gs_preprocess", "gs_bin_tiles", "gs_rasterize_fwd",
            "gs_rasterize_bwd", "gs_pose_grad", "gs_get_counts", "gs_get_binning", "gs_get_features", "gs_poll",
            "gs_aux_l1_grad", "gs_aux_pose_step", "gs_fwd_bwd_host", "gs_profile_enable", "gs_profile_read",
-           "gs_get_launch_count", "gs_get_workload", "gs_loss_map", "gs_loss_iso", "gs_sim3_apply", "gs_measure_peaks", "gs_loss_refine"]
+           "gs_get_launch_count", "gs_get_workload", "gs_loss_map", "gs_loss_iso", "gs_sim3_apply", "gs_measure_peaks", "gs_loss_refine", "gs_voxel_set_clear", "gs_voxel_insert_boxes",
+           "gs_voxel_insert_rays", "gs_voxel_retain", "gs_adam_step", "gs_prune_mask", "gs_compact_work_bytes",
+           "gs_compact_plan", "gs_compact_rows"]
 PEAKS = ["fma_tlanes", "issue_twarp", "ex2_tlanes", "lds128_bcast_twarp", "lds128_twarp", "lds32_bcast_twarp",
          "lds64_bcast_twarp", "red_glanes", "hbm_read_gbs", "hbm_write_gbs", "hbm_copy_gbs", "sm_count", "sm_mhz_max"]
 STAGES = ["preprocess", "tile_scan", "emit", "tile_sort", "raster_fwd", "raster_bwd", "gauss_bwd", "pose_grad"]
@@ -37,6 +39,15 @@ class GsError(RuntimeError):
 class gs_camera(C.Structure):
     _fields_ = [("width", C.c_int32), ("height", C.c_int32), ("fx", C.c_float), ("fy", C.c_float), ("cx", C.c_float),
                 ("cy", C.c_float), ("near_z", C.c_float), ("T_cw", C.c_float * 12)]
+
+
+class gs_gaussians(C.Structure):
+    _fields_ = [(k, C.c_void_p) for k in ("means", "scales", "quats", "opacities", "sh")]
+
+
+class gs_adam_config(C.Structure):
+    _fields_ = [("lr_means", C.c_float), ("lr_scales", C.c_float), ("lr_quats", C.c_float), ("lr_opacities", C.c_float),
+                ("lr_sh", C.c_float), ("beta1", C.c_float), ("beta2", C.c_float), ("eps", C.c_float), ("step", C.c_int32)]
 
 
 def load_library():
@@ -72,11 +83,22 @@ def load_library():
     lib.gs_profile_read.argtypes = [vp, C.POINTER(f * 8)]
     lib.gs_get_launch_count.argtypes = [vp, C.POINTER(C.c_uint64)]
     lib.gs_get_workload.argtypes = [vp, vp, C.POINTER(C.c_uint64 * 7)]
+    lib.gs_voxel_set_clear.argtypes = [vp, vp, i64]
+    lib.gs_voxel_insert_boxes.argtypes = [vp, vp, i64, f, f, i64, vp, vp, vp]
+    lib.gs_voxel_insert_rays.argtypes = [vp, vp, i64, f, C.POINTER(gs_camera), vp, C.c_int32, vp]
+    lib.gs_voxel_retain.argtypes = [vp, vp, i64, vp, i64, f, i64, vp, vp]
+    lib.gs_adam_step.argtypes = [vp, i64, C.c_int, C.POINTER(gs_adam_config), C.POINTER(gs_gaussians), C.POINTER(gs_gaussians),
+                                 C.POINTER(gs_gaussians), C.POINTER(gs_gaussians), vp]
+    lib.gs_prune_mask.argtypes = [vp, i64, vp, f, vp]
+    lib.gs_compact_work_bytes.argtypes = [i64]
+    lib.gs_compact_plan.argtypes = [vp, i64, vp, vp, vp, vp]
+    lib.gs_compact_rows.argtypes = [vp, i64, C.c_int32, vp, vp, vp]
     lib.gs_measure_peaks.argtypes = [C.c_int, vp, C.POINTER(C.c_double * len(PEAKS))]
     lib.gs_fwd_bwd_host.argtypes = [vp, vp, i64, C.c_int, vp, vp, vp, vp, vp, C.POINTER(gs_camera), C.POINTER(f * 3)] + [vp] * 11
     for name in EXPORTS:
-        if name != "gs_last_error":
+        if name not in ("gs_last_error", "gs_compact_work_bytes"):
             getattr(lib, name).restype = C.c_int
+    lib.gs_compact_work_bytes.restype = C.c_int64
     _lib = lib
     return lib
 
@@ -314,6 +336,118 @@ def gs_sim3_apply(s, R, t, means, scales, quats, means_out=None, scales_out=None
                                       _ptr(scales, f32), _ptr(quats, f32), _ptr(mo, f32), _ptr(so, f32), _ptr(qo, f32))
     if rc != 0:
         raise GsError(rc, "gs_sim3_apply")
+
+
+PARAM_KEYS = ("means", "scales", "quats", "opacities", "sh")
+
+
+def _gaussians(d) -> gs_gaussians:
+    import torch
+    g = gs_gaussians()
+    for k in PARAM_KEYS:
+        t = d[k]
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous() and t.dtype == torch.float32):
+            raise TypeError(f"{k}: expected a contiguous float32 CUDA tensor")
+        setattr(g, k, t.data_ptr())
+    return g
+
+
+def gs_adam_step(params, grads, m, v, lrs, step, visible=None, beta1=0.9, beta2=0.999, eps=1e-15, stream=None):
+    """One fused Adam step in place (include/gs.h).  params / grads / m / v: dicts of CUDA tensors keyed means, scales, quats,
+    opacities, sh; lrs: dict of learning rates; visible: optional int32/uint32 CUDA tensor [N]."""
+    import torch
+    N = int(params["means"].shape[0])
+    K = int(params["sh"].shape[1])
+    deg = int(round(K ** 0.5)) - 1
+    cfg = gs_adam_config(float(lrs["means"]), float(lrs["scales"]), float(lrs["quats"]), float(lrs["opacities"]), float(lrs["sh"]),
+                         float(beta1), float(beta2), float(eps), int(step))
+    gp, gg, gm, gv = _gaussians(params), _gaussians(grads), _gaussians(m), _gaussians(v)
+    vis = None if visible is None else C.c_void_p(visible.data_ptr())
+    rc = load_library().gs_adam_step(_stream(stream), N, deg, C.byref(cfg), C.byref(gp), C.byref(gg), C.byref(gm), C.byref(gv), vis)
+    if rc != 0:
+        raise GsError(rc, "gs_adam_step")
+
+
+def gs_prune_mask(opacities, min_opacity, keep, stream=None):
+    import torch
+    rc = load_library().gs_prune_mask(_stream(stream), int(opacities.numel()), _ptr(opacities, torch.float32), float(min_opacity),
+                                      _ptr(keep, torch.uint8))
+    if rc != 0:
+        raise GsError(rc, "gs_prune_mask")
+
+
+def gs_compact(keep, arrays, stream=None):
+    """Order-preserving compaction of a dict of [N,...] float32 CUDA tensors by the uint8 mask `keep`.  Returns (dict of
+    compacted tensors [n_kept,...], index tensor [N] (destination row or 0xFFFFFFFF))."""
+    import torch
+    lib = load_library()
+    N = int(keep.numel())
+    dev = keep.device
+    index = torch.empty(N, dtype=torch.int32, device=dev)
+    n_kept = torch.zeros(1, dtype=torch.int64, device=dev)
+    work = torch.empty(max(1, int(lib.gs_compact_work_bytes(N))), dtype=torch.uint8, device=dev)
+    rc = lib.gs_compact_plan(_stream(stream), N, _ptr(keep, torch.uint8), _ptr(index), _ptr(n_kept), _ptr(work))
+    if rc != 0:
+        raise GsError(rc, "gs_compact_plan")
+    n = int(n_kept.item())                                # the one host read: sizes the outputs
+    out = {}
+    for k, a in arrays.items():
+        width = int(a.numel() // max(N, 1)) if N else 1
+        o = torch.empty((n,) + tuple(a.shape[1:]), dtype=torch.float32, device=dev)
+        rc = lib.gs_compact_rows(_stream(stream), N, width, _ptr(index), _ptr(a, torch.float32), _ptr(o, torch.float32))
+        if rc != 0:
+            raise GsError(rc, "gs_compact_rows")
+        out[k] = o
+    return out, index
+
+
+class VoxelSet:
+    """Hash set of 64-bit voxel keys in device memory (include/gs.h, Eqs. 20-22)."""
+
+    def __init__(self, capacity: int, device: int = 0):
+        import torch
+        assert capacity >= 2 and capacity & (capacity - 1) == 0
+        dev = torch.device("cuda", device)
+        self.capacity = capacity
+        self.table = torch.empty(capacity, dtype=torch.int64, device=dev)
+        self.overflow = torch.zeros(1, dtype=torch.int32, device=dev)
+        self.clear()
+
+    def clear(self, stream=None):
+        rc = load_library().gs_voxel_set_clear(_stream(stream), _ptr(self.table), self.capacity)
+        if rc != 0:
+            raise GsError(rc, "gs_voxel_set_clear")
+        self.overflow.zero_()
+
+    def insert_boxes(self, means, scales, voxel, k, stream=None):
+        import torch
+        rc = load_library().gs_voxel_insert_boxes(_stream(stream), _ptr(self.table), self.capacity, float(voxel), float(k),
+                                                  int(means.shape[0]), _ptr(means, torch.float32), _ptr(scales, torch.float32),
+                                                  _ptr(self.overflow))
+        if rc != 0:
+            raise GsError(rc, "gs_voxel_insert_boxes")
+
+    def insert_rays(self, cam, depth, voxel, stride=1, stream=None):
+        import torch
+        c = cam if isinstance(cam, gs_camera) else camera_struct(cam)
+        rc = load_library().gs_voxel_insert_rays(_stream(stream), _ptr(self.table), self.capacity, float(voxel), C.byref(c),
+                                                 _ptr(depth, torch.float32), int(stride), _ptr(self.overflow))
+        if rc != 0:
+            raise GsError(rc, "gs_voxel_insert_rays")
+
+    def keys(self):
+        """Sorted numpy uint64 array of the stored keys (test / inspection helper; synchronises)."""
+        t = self.table.cpu().numpy().view(np.uint64)
+        return np.sort(t[t != np.uint64(0xFFFFFFFFFFFFFFFF)])
+
+
+def gs_voxel_retain(occ, free, voxel, means, retain, stream=None):
+    import torch
+    rc = load_library().gs_voxel_retain(_stream(stream), _ptr(occ.table) if occ else None, occ.capacity if occ else 0,
+                                        _ptr(free.table) if free else None, free.capacity if free else 0, float(voxel),
+                                        int(means.shape[0]), _ptr(means, torch.float32), _ptr(retain, torch.uint8))
+    if rc != 0:
+        raise GsError(rc, "gs_voxel_retain")
 
 
 def gs_measure_peaks(device: int = 0, stream=None) -> dict:

@@ -85,3 +85,211 @@ extern "C" int gs_sim3_apply(void* stream, int64_t N, float s, const float* R, c
   sim3_kernel<<<(unsigned)grid, 256, 0, (cudaStream_t)stream>>>(N, C, means, scales, quats, means_out, scales_out, quats_out);
   return cudaGetLastError() == cudaSuccess ? GS_OK : GS_E_CUDA;
 }
+
+// ---------------------------------------------------------------------------------------------------------------
+// Eqs. 20-22: occupancy-aware fusion on a voxel grid of size v, voxel indices packed into 64-bit
+// spatial-hash keys.  Sets are open-addressing hash tables (linear probing, 64-bit atomicCAS) in caller-provided device
+// memory.  Every coordinate computation is fp64 with explicitly rounded single operations (no FMA contraction), in the
+// sequence DESIGN.md Q21 fixes, so that the sets are bit-identical to the plain definition's.
+// ---------------------------------------------------------------------------------------------------------------
+namespace gs {
+
+constexpr unsigned long long kVoxEmpty = 0xFFFFFFFFFFFFFFFFull;
+constexpr long long kKeyBias = 1ll << 20;
+
+__device__ __forceinline__ unsigned long long vox_key(long long ix, long long iy, long long iz) {
+  return (unsigned long long)(ix + kKeyBias) | ((unsigned long long)(iy + kKeyBias) << 21) |
+         ((unsigned long long)(iz + kKeyBias) << 42);
+}
+__device__ __forceinline__ bool vox_in_range(long long i) { return i >= -kKeyBias && i < kKeyBias; }
+__device__ __forceinline__ unsigned long long vox_hash(unsigned long long k) {  // splitmix64 finaliser
+  k ^= k >> 30; k *= 0xbf58476d1ce4e5b9ull; k ^= k >> 27; k *= 0x94d049bb133111ebull; k ^= k >> 31;
+  return k;
+}
+__device__ __forceinline__ long long vox_floor_div(double x, double v) { return (long long)floor(__ddiv_rn(x, v)); }
+
+__device__ __forceinline__ void vox_insert(unsigned long long* table, unsigned long long mask, unsigned long long key,
+                                           uint32_t* overflow) {
+  unsigned long long slot = vox_hash(key) & mask;
+  for (unsigned long long probe = 0; probe <= mask; ++probe) {
+    const unsigned long long cur = table[slot];   // most insertions are duplicates: read before the atomic
+    if (cur == key) return;
+    if (cur == kVoxEmpty) {
+      const unsigned long long old = atomicCAS(table + slot, kVoxEmpty, key);
+      if (old == kVoxEmpty || old == key) return;
+    }
+    slot = (slot + 1) & mask;
+  }
+  atomicAdd(overflow, 1u);  // table full
+}
+
+__device__ __forceinline__ bool vox_contains(const unsigned long long* table, unsigned long long mask, unsigned long long key) {
+  unsigned long long slot = vox_hash(key) & mask;
+  for (unsigned long long probe = 0; probe <= mask; ++probe) {
+    const unsigned long long cur = __ldg(table + slot);
+    if (cur == key) return true;
+    if (cur == kVoxEmpty) return false;
+    slot = (slot + 1) & mask;
+  }
+  return false;
+}
+
+__global__ void __launch_bounds__(256) vox_clear_kernel(unsigned long long* table, int64_t cap) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < cap; i += stride) table[i] = kVoxEmpty;
+}
+
+// Eq. 20: every voxel meeting the closed axis-aligned box [mu - k s, mu + k s]
+__global__ void __launch_bounds__(128)
+vox_boxes_kernel(unsigned long long* table, unsigned long long mask, double v, double k, int64_t N,
+                 const float* __restrict__ means, const float* __restrict__ scales, uint32_t* overflow) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  long long lo[3], hi[3];
+  bool ok = true;
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    const double mu = (double)means[3 * i + a], h = __dmul_rn(k, (double)scales[3 * i + a]);
+    lo[a] = vox_floor_div(__dsub_rn(mu, h), v);
+    hi[a] = vox_floor_div(__dadd_rn(mu, h), v);
+    ok = ok && vox_in_range(lo[a]) && vox_in_range(hi[a]);
+  }
+  if (!ok) { atomicAdd(overflow, 1u); return; }   // outside the 21-bit index range (or non-finite)
+  for (long long iz = lo[2]; iz <= hi[2]; ++iz)
+    for (long long iy = lo[1]; iy <= hi[1]; ++iy)
+      for (long long ix = lo[0]; ix <= hi[0]; ++ix) vox_insert(table, mask, vox_key(ix, iy, iz), overflow);
+}
+
+struct RayCam { double fx, fy, cx, cy, R[9], t[3]; int W, H, stride; };
+
+// Eq. 21: 3-D DDA along c + t (r - c), t in [0, 1), one thread per (sub-sampled) pixel with depth > 0
+__global__ void __launch_bounds__(128)
+vox_rays_kernel(unsigned long long* table, unsigned long long mask, double v, RayCam cam, const float* __restrict__ depth,
+                uint32_t* overflow) {
+  const int nx = (cam.W + cam.stride - 1) / cam.stride, ny = (cam.H + cam.stride - 1) / cam.stride;
+  const int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (q >= (int64_t)nx * ny) return;
+  const int X = (int)(q % nx) * cam.stride, Y = (int)(q / nx) * cam.stride;
+  const double z = (double)depth[(size_t)Y * cam.W + X];
+  if (!(z > 0.0)) return;
+  // camera centre c = -R^T t and surface point r = R^T (p_c - t), sums left to right, one rounding per operation
+  double pc[3] = {__ddiv_rn(__dmul_rn(__dsub_rn((double)X, cam.cx), z), cam.fx),
+                  __ddiv_rn(__dmul_rn(__dsub_rn((double)Y, cam.cy), z), cam.fy), z};
+  double c[3], d[3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    c[a] = -__dadd_rn(__dadd_rn(__dmul_rn(cam.R[a], cam.t[0]), __dmul_rn(cam.R[3 + a], cam.t[1])), __dmul_rn(cam.R[6 + a], cam.t[2]));
+    const double q0 = __dsub_rn(pc[0], cam.t[0]), q1 = __dsub_rn(pc[1], cam.t[1]), q2 = __dsub_rn(pc[2], cam.t[2]);
+    const double r = __dadd_rn(__dadd_rn(__dmul_rn(cam.R[a], q0), __dmul_rn(cam.R[3 + a], q1)), __dmul_rn(cam.R[6 + a], q2));
+    d[a] = __dsub_rn(r, c[a]);
+  }
+  long long idx[3], step[3];
+  double t_max[3], t_delta[3];
+  bool ok = true;
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    idx[a] = vox_floor_div(c[a], v);
+    ok = ok && vox_in_range(idx[a]) && isfinite(d[a]);
+    step[a] = 0; t_max[a] = INFINITY; t_delta[a] = INFINITY;
+    if (d[a] > 0.0) {
+      step[a] = 1;
+      t_max[a] = __ddiv_rn(__dsub_rn(__dmul_rn(__dadd_rn((double)idx[a], 1.0), v), c[a]), d[a]);
+      t_delta[a] = __ddiv_rn(v, d[a]);
+    } else if (d[a] < 0.0) {
+      step[a] = -1;
+      t_max[a] = __ddiv_rn(__dsub_rn(__dmul_rn((double)idx[a], v), c[a]), d[a]);
+      t_delta[a] = __ddiv_rn(-v, d[a]);
+    }
+  }
+  if (!ok) { atomicAdd(overflow, 1u); return; }
+  vox_insert(table, mask, vox_key(idx[0], idx[1], idx[2]), overflow);
+  for (int guard = 0; guard < (1 << 22); ++guard) {
+    int a = 0;                                   // axis of the nearest boundary; ties -> lowest axis
+    if (t_max[1] < t_max[a]) a = 1;
+    if (t_max[2] < t_max[a]) a = 2;
+    const double tm = a == 0 ? t_max[0] : (a == 1 ? t_max[1] : t_max[2]);
+    if (!(tm < 1.0)) break;                      // the next boundary lies at t >= 1
+    if (a == 0) { idx[0] += step[0]; t_max[0] = __dadd_rn(t_max[0], t_delta[0]); }
+    else if (a == 1) { idx[1] += step[1]; t_max[1] = __dadd_rn(t_max[1], t_delta[1]); }
+    else { idx[2] += step[2]; t_max[2] = __dadd_rn(t_max[2], t_delta[2]); }
+    if (!(vox_in_range(idx[0]) && vox_in_range(idx[1]) && vox_in_range(idx[2]))) { atomicAdd(overflow, 1u); return; }
+    vox_insert(table, mask, vox_key(idx[0], idx[1], idx[2]), overflow);
+  }
+}
+
+// Eq. 22: retained iff kappa(mu) is in neither set
+__global__ void __launch_bounds__(256)
+vox_retain_kernel(const unsigned long long* occ, unsigned long long occ_mask, const unsigned long long* fre,
+                  unsigned long long free_mask, double v, int64_t N, const float* __restrict__ means, uint8_t* __restrict__ retain) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  const long long ix = vox_floor_div((double)means[3 * i], v), iy = vox_floor_div((double)means[3 * i + 1], v),
+                  iz = vox_floor_div((double)means[3 * i + 2], v);
+  bool keep = true;
+  if (vox_in_range(ix) && vox_in_range(iy) && vox_in_range(iz)) {
+    const unsigned long long key = vox_key(ix, iy, iz);
+    if (occ && vox_contains(occ, occ_mask, key)) keep = false;
+    if (keep && fre && vox_contains(fre, free_mask, key)) keep = false;
+  }
+  retain[i] = keep ? 1 : 0;
+}
+
+static bool pow2(int64_t c) { return c >= 2 && (c & (c - 1)) == 0; }
+
+}  // namespace gs
+
+using namespace gs;
+
+extern "C" {
+
+int gs_voxel_set_clear(void* stream, uint64_t* table, int64_t capacity) {
+  if (!table || !pow2(capacity)) return GS_E_INVALID;
+  int64_t g = div_up(capacity, 256);
+  if (g > 148 * 16) g = 148 * 16;
+  vox_clear_kernel<<<(int)g, 256, 0, (cudaStream_t)stream>>>(reinterpret_cast<unsigned long long*>(table), capacity);
+  return cudaGetLastError() == cudaSuccess ? GS_OK : GS_E_CUDA;
+}
+
+int gs_voxel_insert_boxes(void* stream, uint64_t* table, int64_t capacity, float voxel, float k, int64_t N,
+                          const float* means, const float* scales, uint32_t* overflow) {
+  if (!table || !pow2(capacity) || !(voxel > 0.f) || !(k >= 0.f) || N < 0 || !overflow || (N > 0 && (!means || !scales)))
+    return GS_E_INVALID;
+  if (N == 0) return GS_OK;
+  vox_boxes_kernel<<<(unsigned)div_up(N, 128), 128, 0, (cudaStream_t)stream>>>(
+      reinterpret_cast<unsigned long long*>(table), (unsigned long long)capacity - 1ull, (double)voxel, (double)k, N, means,
+      scales, overflow);
+  return cudaGetLastError() == cudaSuccess ? GS_OK : GS_E_CUDA;
+}
+
+int gs_voxel_insert_rays(void* stream, uint64_t* table, int64_t capacity, float voxel, const gs_camera* cam,
+                         const float* depth, int32_t stride, uint32_t* overflow) {
+  if (!table || !pow2(capacity) || !(voxel > 0.f) || !cam || !depth || stride < 1 || !overflow || cam->width <= 0 ||
+      cam->height <= 0)
+    return GS_E_INVALID;
+  RayCam rc;
+  rc.fx = cam->fx; rc.fy = cam->fy; rc.cx = cam->cx; rc.cy = cam->cy;
+  for (int r = 0; r < 3; ++r) {
+    for (int c = 0; c < 3; ++c) rc.R[3 * r + c] = cam->T_cw[4 * r + c];
+    rc.t[r] = cam->T_cw[4 * r + 3];
+  }
+  rc.W = cam->width; rc.H = cam->height; rc.stride = stride;
+  const int64_t n = (int64_t)((cam->width + stride - 1) / stride) * ((cam->height + stride - 1) / stride);
+  vox_rays_kernel<<<(unsigned)div_up(n, 128), 128, 0, (cudaStream_t)stream>>>(
+      reinterpret_cast<unsigned long long*>(table), (unsigned long long)capacity - 1ull, (double)voxel, rc, depth, overflow);
+  return cudaGetLastError() == cudaSuccess ? GS_OK : GS_E_CUDA;
+}
+
+int gs_voxel_retain(void* stream, const uint64_t* occ, int64_t occ_capacity, const uint64_t* free_set, int64_t free_capacity,
+                    float voxel, int64_t N, const float* means, uint8_t* retain) {
+  if ((occ && !pow2(occ_capacity)) || (free_set && !pow2(free_capacity)) || !(voxel > 0.f) || N < 0 ||
+      (N > 0 && (!means || !retain)))
+    return GS_E_INVALID;
+  if (N == 0) return GS_OK;
+  vox_retain_kernel<<<(unsigned)div_up(N, 256), 256, 0, (cudaStream_t)stream>>>(
+      reinterpret_cast<const unsigned long long*>(occ), occ ? (unsigned long long)occ_capacity - 1ull : 0ull,
+      reinterpret_cast<const unsigned long long*>(free_set), free_set ? (unsigned long long)free_capacity - 1ull : 0ull,
+      (double)voxel, N, means, retain);
+  return cudaGetLastError() == cudaSuccess ? GS_OK : GS_E_CUDA;
+}
+
+}  // extern "C"

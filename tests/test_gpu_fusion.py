@@ -45,3 +45,100 @@ def test_sim3_apply_matches_oracle(case):
     assert torch.equal(dm, om) and torch.equal(dsc, os_) and torch.equal(dq, oq)
     if case == "identity":
         assert np.array_equal(gm, means) and np.array_equal(gs_, scales) and np.array_equal(gq, quats)
+
+
+# ----------------------------------------------------------------------------------------------------------------------
+# Eqs. 20-22: occupancy sets and the retain test -- BIT-EXACT against oracle/fusion.py (set contents as sorted key lists,
+# retain masks, order-preserving compaction)
+# ----------------------------------------------------------------------------------------------------------------------
+def _f32(x):
+    return np.ascontiguousarray(x, np.float32)
+
+
+def test_occupied_set_matches_oracle_bit_exact():
+    import torch
+    from oracle import fusion as of
+    from paper_2605_10760_b200 import binding as b, scenes
+    sc = scenes.replica_scene(seed=61, N=3000, width=64, height=48, f=32.0, sh_degree=0)
+    v, k = np.float32(0.02), np.float32(1.5)
+    want = np.array(sorted(of.occupied_set(sc.means, sc.scales, float(v), float(k))), np.uint64)
+    vs = b.VoxelSet(1 << 17)
+    vs.insert_boxes(torch.from_numpy(sc.means).cuda(), torch.from_numpy(sc.scales).cuda(), v, k)
+    torch.cuda.synchronize()
+    assert int(vs.overflow.item()) == 0
+    assert np.array_equal(vs.keys(), want) and len(want) > 3000
+    # inserting the same Gaussians again changes nothing; a table that is too small reports the overflow
+    vs.insert_boxes(torch.from_numpy(sc.means).cuda(), torch.from_numpy(sc.scales).cuda(), v, k)
+    torch.cuda.synchronize()
+    assert np.array_equal(vs.keys(), want)
+    small = b.VoxelSet(1 << 10)
+    small.insert_boxes(torch.from_numpy(sc.means).cuda(), torch.from_numpy(sc.scales).cuda(), v, k)
+    torch.cuda.synchronize()
+    assert int(small.overflow.item()) > 0 and len(small.keys()) == 1 << 10
+
+
+@pytest.mark.parametrize("stride", [1, 3])
+def test_free_set_matches_oracle_bit_exact(stride):
+    import torch
+    from oracle import fusion as of
+    from paper_2605_10760_b200 import binding as b, scenes
+    r = np.random.Generator(np.random.PCG64(62 + stride))
+    W, H = 37, 23          # ragged against the stride and the CTA size
+    cam = scenes.Camera(W, H, 30.0, 31.0, 18.25, 11.0, scenes.perturb_pose(scenes.look_at([1.0, 2.0, 1.2], [4.0, 3.0, 1.0]),
+                                                                               r.normal(0, 0.05, 6)))
+    depth = _f32(r.uniform(0.4, 3.0, (H, W)))
+    depth[r.uniform(size=(H, W)) < 0.15] = 0.0       # invalid pixels cast no ray
+    v = np.float32(0.05)
+    want = np.array(sorted(of.free_set(depth, np.float32(cam.fx), np.float32(cam.fy), np.float32(cam.cx), np.float32(cam.cy),
+                                       _f32(cam.T_cw), float(v), stride)), np.uint64)
+    vs = b.VoxelSet(1 << 18)
+    vs.insert_rays(cam, torch.from_numpy(depth).cuda(), v, stride)
+    torch.cuda.synchronize()
+    assert int(vs.overflow.item()) == 0
+    got = vs.keys()
+    assert len(got) == len(want) and np.array_equal(got, want)
+
+
+def test_retain_and_compaction_config5_shaped():
+    """Config-5 shape: a target submap and three borrowed submaps mapped by Eq. 19 into its frame (reduced to 4 x 20k
+    Gaussians so that the pure-Python oracle finishes in seconds); Eq. 22 retain masks bit-exact, retained Gaussians compacted
+    in their original order."""
+    import torch
+    from oracle import fusion as of
+    from paper_2605_10760_b200 import binding as b, scenes
+    sc, cams = scenes.fused_scene(seed=63, N_sub=20_000, submaps=4, views=2, width=48, height=32, f=24.0, sh_degree=0)
+    n = 20_000
+    tgt_m, tgt_s = sc.means[:n], sc.scales[:n]
+    src_m = sc.means[n:]
+    v, k = np.float32(0.04), np.float32(1.0)
+    occ_o = of.occupied_set(tgt_m, tgt_s, float(v), float(k))
+    depth = _f32(np.random.Generator(np.random.PCG64(64)).uniform(1.0, 4.0, (32, 48)))
+    free_o = set()
+    for cam in cams:
+        free_o |= of.free_set(depth, np.float32(cam.fx), np.float32(cam.fy), np.float32(cam.cx), np.float32(cam.cy),
+                              _f32(cam.T_cw), float(v), 1)
+    want = of.retain_mask(src_m, occ_o, free_o, float(v))
+    occ, free = b.VoxelSet(1 << 19), b.VoxelSet(1 << 19)
+    occ.insert_boxes(torch.from_numpy(tgt_m).cuda(), torch.from_numpy(tgt_s).cuda(), v, k)
+    for cam in cams:
+        free.insert_rays(cam, torch.from_numpy(depth).cuda(), v, 1)
+    src = torch.from_numpy(np.ascontiguousarray(src_m)).cuda()
+    retain = torch.empty(src.shape[0], dtype=torch.uint8, device="cuda")
+    b.gs_voxel_retain(occ, free, v, src, retain)
+    torch.cuda.synchronize()
+    assert int(occ.overflow.item()) == 0 and int(free.overflow.item()) == 0
+    assert np.array_equal(occ.keys(), np.array(sorted(occ_o), np.uint64))
+    assert np.array_equal(free.keys(), np.array(sorted(free_o), np.uint64))
+    got = retain.cpu().numpy().astype(bool)
+    assert np.array_equal(got, want) and 0 < want.sum() < len(want)
+    # one-set variants (either table may be NULL)
+    b.gs_voxel_retain(occ, None, v, src, retain)
+    torch.cuda.synchronize()
+    assert np.array_equal(retain.cpu().numpy().astype(bool), of.retain_mask(src_m, occ_o, set(), float(v)))
+    # compaction keeps the original order: fused set = target + retained borrowed Gaussians
+    b.gs_voxel_retain(occ, free, v, src, retain)
+    out, index = b.gs_compact(retain, dict(means=src, quats=torch.from_numpy(np.ascontiguousarray(sc.quats[n:])).cuda()))
+    torch.cuda.synchronize()
+    assert np.array_equal(out["means"].cpu().numpy(), src_m[want]) and np.array_equal(out["quats"].cpu().numpy(), sc.quats[n:][want])
+    idx = index.cpu().numpy().view(np.uint32)
+    assert np.array_equal(idx[want], np.arange(want.sum(), dtype=np.uint32)) and (idx[~want] == 0xFFFFFFFF).all()
