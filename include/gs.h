@@ -80,6 +80,17 @@ GS_API int gs_destroy(gs_ctx* ctx);
 /* Message of the last failing call on this context (never NULL; owned by the context). */
 GS_API const char* gs_last_error(const gs_ctx* ctx);
 
+/* Options of a context (take effect from the next gs_preprocess).
+ *   GS_OPT_EXACT_TILE_CULL (default 0): gs_bin_tiles drops the (Gaussian, tile) instances whose ellipse {alpha >= 1/255}
+ *   reaches no pixel region of the tile although the tile lies in the ellipse's bounding rectangle (the corner tiles of
+ *   large footprints).  Images and gradients are unchanged (such instances never pass the alpha test); the per-tile lists
+ *   become the (tile, depth, index)-ordered SUBSET of the default lists, so the mode sits outside the bit-exact binning
+ *   contract: gs_get_counts still reports the rectangle-based instance total (the capacity the lists are laid out in),
+ *   gs_get_binning's tile_ranges delimit the shorter lists and the entries between a list's end and the next list's
+ *   start are unspecified. */
+#define GS_OPT_EXACT_TILE_CULL 1
+GS_API int gs_set_option(gs_ctx* ctx, int option, int value);
+
 /* Step a1 -- EWA projection, conic, screen extent, colour (oracle reading C1 steps 1-6, 8).
  *   N            number of Gaussians (0 <= N < 2^24: sorted list entries carry slot << 8 | region mask)
  *   sh_degree    0..3; K = (sh_degree+1)^2 coefficients per channel
@@ -194,6 +205,20 @@ GS_API int gs_loss_iso(void* stream, int64_t N, const float* scales, float lambd
 GS_API int gs_loss_refine(void* stream, int32_t width, int32_t height, const float* rgb, const float* depth,
                           const float* target_rgb, const float* target_depth, const float* ab, float alpha_p, float lambda,
                           float beta, float* d_rgb, float* d_depth, float* g_ab, float* work, double* loss);
+
+/* ---- depth-induced normals and the normal term of Eqs. 4 / 23 -------------------------------- */
+/* N^ = depth-induced normal of the rendered depth (reading Q22: pinhole back-projection, forward differences,
+ * N^ = (t_y x t_x) / |.|, facing the camera; defined off the last column / row where the three depths are > 0), and
+ * lambda_n L_normal, L_normal = (1 / H W) sum |1 - N^ . N-| over pixels that have a normal and a non-zero prior N-.
+ *   depth         DEVICE [H,W]   rendered depth (gs_rasterize_fwd)
+ *   normal_prior  DEVICE [3,H,W] unit normals in camera coordinates, zero vector = no prior; NULL = normals only
+ *   normals_out   DEVICE [3,H,W] or NULL: the depth-induced normal map (zeros where undefined)
+ *   d_depth       DEVICE [H,W]: lambda_n dL_normal/dD^ is ADDED (call after gs_loss_map / gs_loss_refine wrote it)
+ *   loss          DEVICE double[2]: loss[0] = lambda_n L_normal (loss[1] scratch)
+ * Asynchronous on `stream`.  GS_E_INVALID on null / inconsistent pointers or an empty image. */
+GS_API int gs_loss_normal(void* stream, int32_t width, int32_t height, float fx, float fy, float cx, float cy,
+                          const float* depth, const float* normal_prior, float lambda_n, float* normals_out, float* d_depth,
+                          double* loss);
 
 /* ---- Eq. 19: a submap's Sim(3) correction applied to its Gaussians --------------------------------- */
 /* mu' = s R mu + t, s_i' = s s_i, q' = q_R (x) q (so that Sigma' = s^2 R Sigma R^T); opacity and colour are unchanged

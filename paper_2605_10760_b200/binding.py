@@ -24,7 +24,8 @@ EXPORTS = ["gs_create", "gs_destroy", "gs_last_error", "gs_preprocess", "gs_bin_
            "gs_aux_l1_grad", "gs_aux_pose_step", "gs_fwd_bwd_host", "gs_profile_enable", "gs_profile_read",
            "gs_get_launch_count", "gs_get_workload", "gs_loss_map", "gs_loss_iso", "gs_sim3_apply", "gs_measure_peaks", "gs_loss_refine", "gs_voxel_set_clear", "gs_voxel_insert_boxes",
            "gs_voxel_insert_rays", "gs_voxel_retain", "gs_adam_step", "gs_prune_mask", "gs_compact_work_bytes",
-           "gs_compact_plan", "gs_compact_rows"]
+           "gs_compact_plan", "gs_compact_rows", "gs_loss_normal", "gs_set_option"]
+GS_OPT_EXACT_TILE_CULL = 1
 PEAKS = ["fma_tlanes", "issue_twarp", "ex2_tlanes", "lds128_bcast_twarp", "lds128_twarp", "lds32_bcast_twarp",
          "lds64_bcast_twarp", "red_glanes", "hbm_read_gbs", "hbm_write_gbs", "hbm_copy_gbs", "sm_count", "sm_mhz_max"]
 STAGES = ["preprocess", "tile_scan", "emit", "tile_sort", "raster_fwd", "raster_bwd", "gauss_bwd", "pose_grad"]
@@ -73,6 +74,7 @@ def load_library():
     lib.gs_get_binning.argtypes = [vp, vp, vp, vp, vp]
     lib.gs_get_features.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
     lib.gs_poll.argtypes = [vp]
+    lib.gs_set_option.argtypes = [vp, C.c_int, C.c_int]
     lib.gs_aux_l1_grad.argtypes = [vp, i64, vp, vp, f, vp]
     lib.gs_aux_pose_step.argtypes = [vp, vp, vp, f]
     lib.gs_loss_map.argtypes = [vp, C.c_int32, C.c_int32, vp, vp, vp, vp, f, f, vp, vp, vp]
@@ -93,6 +95,7 @@ def load_library():
     lib.gs_compact_work_bytes.argtypes = [i64]
     lib.gs_compact_plan.argtypes = [vp, i64, vp, vp, vp, vp]
     lib.gs_compact_rows.argtypes = [vp, i64, C.c_int32, vp, vp, vp]
+    lib.gs_loss_normal.argtypes = [vp, C.c_int32, C.c_int32, f, f, f, f, vp, vp, f, vp, vp, vp]
     lib.gs_measure_peaks.argtypes = [C.c_int, vp, C.POINTER(C.c_double * len(PEAKS))]
     lib.gs_fwd_bwd_host.argtypes = [vp, vp, i64, C.c_int, vp, vp, vp, vp, vp, C.POINTER(gs_camera), C.POINTER(f * 3)] + [vp] * 11
     for name in EXPORTS:
@@ -237,6 +240,9 @@ class Context:
         res["depth_key"] = res["depth_key"].view(np.uint32)
         return res
 
+    def gs_set_option(self, option: int, value: int):
+        self._check(self.lib.gs_set_option(self._h, int(option), int(value)))
+
     def gs_poll(self):
         self._check(self.lib.gs_poll(self._h))
 
@@ -311,6 +317,18 @@ def gs_loss_refine(rgb, depth, target_rgb, target_depth, ab, alpha_p, lam, beta,
                                        _ptr(loss, torch.float64))
     if rc != 0:
         raise GsError(rc, "gs_loss_refine")
+
+
+def gs_loss_normal(cam, depth, normal_prior, lambda_n, normals_out, d_depth, loss, stream=None):
+    """Depth-induced normals (normals_out, optional) and lambda_n L_normal; its depth gradient is ADDED into d_depth."""
+    import torch
+    f32 = torch.float32
+    H, W = depth.shape
+    rc = load_library().gs_loss_normal(_stream(stream), int(W), int(H), float(cam.fx), float(cam.fy), float(cam.cx), float(cam.cy),
+                                       _ptr(depth, f32), _ptr(normal_prior, f32), float(lambda_n), _ptr(normals_out, f32),
+                                       _ptr(d_depth, f32), _ptr(loss, torch.float64))
+    if rc != 0:
+        raise GsError(rc, "gs_loss_normal")
 
 
 def gs_loss_iso(scales, lambda_s, g_scales, loss, stream=None):

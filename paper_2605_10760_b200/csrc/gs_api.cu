@@ -196,6 +196,12 @@ int gs_destroy(gs_ctx* ctx) {
 
 const char* gs_last_error(const gs_ctx* ctx) { return ctx ? ctx->err : "null context"; }
 
+int gs_set_option(gs_ctx* ctx, int option, int value) {
+  if (!ctx) return GS_E_INVALID;
+  if (option == GS_OPT_EXACT_TILE_CULL) { ctx->opt_exact_cull = value != 0; return GS_OK; }
+  return fail(ctx, GS_E_INVALID, "gs_set_option: unknown option");
+}
+
 int gs_poll(gs_ctx* ctx) {
   if (!ctx) return GS_E_INVALID;
   return handle_overflow(ctx);

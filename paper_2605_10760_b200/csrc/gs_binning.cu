@@ -185,7 +185,8 @@ constexpr int kEmitT = 128;   // threads per CTA
 
 __global__ void __launch_bounds__(kEmitT)
 emit_kernel(const uint4* __restrict__ vis_rec, const float4* __restrict__ feat, int tiles_x,
-            uint32_t* __restrict__ tile_cursor, const Counts* __restrict__ counts, uint64_t* __restrict__ keys) {
+            uint32_t* __restrict__ tile_cursor, const Counts* __restrict__ counts, uint64_t* __restrict__ keys,
+            bool exact_cull) {
   // Block-cooperative: the instances of the CTA's 32 Gaussians form one work list (prefix sum of the per-Gaussian tile
   // counts); every round the 128 threads take consecutive work items, whatever Gaussian they belong to, so a Gaussian
   // covering hundreds of tiles is emitted by the whole CTA; four independent atomics per thread are put in flight
@@ -245,7 +246,11 @@ emit_kernel(const uint4* __restrict__ vis_rec, const float4* __restrict__ feat, 
         const int pk = __float_as_int(f0.z);
         const float mx = (float)(((pk << 16) >> 16) - (int)tx * GS_TILE) + f0.x;
         const float my = (float)((pk >> 16) - (int)ty * GS_TILE) + f0.y;
-        kk[u] = s_key[owner] | (uint64_t)region_mask(f1.x, f1.y, f1.z, f1.w, mx, my);
+        const uint32_t mask = region_mask(f1.x, f1.y, f1.z, f1.w, mx, my);
+        kk[u] = s_key[owner] | (uint64_t)mask;
+        // GS_OPT_EXACT_TILE_CULL: a tile of the rect that the ellipse itself does not reach (empty region mask) gets no
+        // list entry at all; range_fix_kernel then shortens the tile's range to what was emitted
+        if (exact_cull && mask == 0u) cur[u] = nullptr;
       }
     }
 #pragma unroll
@@ -254,6 +259,15 @@ emit_kernel(const uint4* __restrict__ vis_rec, const float4* __restrict__ feat, 
     for (int u = 0; u < 4; ++u)
       if (cur[u]) keys[pos[u]] = kk[u];
   }
+}
+
+// exact-cull mode only: the tile ranges were sized by the rect-based counts; shrink them to the emitted entries
+__global__ void __launch_bounds__(256)
+range_fix_kernel(int tiles, const uint32_t* __restrict__ tile_cursor, uint2* __restrict__ ranges) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= tiles) return;
+  uint2 r = ranges[t];
+  if (r.y > r.x) { r.y = min(r.y, tile_cursor[(size_t)t * kCtrStride]); if (r.y == r.x) r = make_uint2(0u, 0u); ranges[t] = r; }
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -494,15 +508,18 @@ __global__ void export_keys_kernel(int tiles, const uint2* __restrict__ ranges, 
   for (uint32_t k = r.x + threadIdx.x; k < r.y; k += blockDim.x) out[k] = ((uint64_t)tile << 32) | (keys[k] >> 32);
 }
 
-__global__ void export_ids_kernel(int64_t I, const uint32_t* __restrict__ vals, const uint32_t* __restrict__ vis_ids,
-                                  uint32_t* __restrict__ out) {
-  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (k < I) out[k] = vis_ids[vals[k] >> 8];  // strip the region mask, visible slot -> Gaussian index
+__global__ void export_ids_kernel(int tiles, const uint2* __restrict__ ranges, const uint32_t* __restrict__ vals,
+                                  const uint32_t* __restrict__ vis_ids, uint32_t* __restrict__ out) {
+  const int tile = blockIdx.x;
+  if (tile >= tiles) return;
+  const uint2 r = ranges[tile];  // per tile range: in exact-cull mode the entries between two lists are unspecified
+  for (uint32_t k = r.x + threadIdx.x; k < r.y; k += blockDim.x) out[k] = vis_ids[vals[k] >> 8];  // slot -> Gaussian index
 }
 
 int export_sorted_ids(gs_ctx* ctx, cudaStream_t s, int64_t I, uint32_t* out) {
-  if (I <= 0) return GS_OK;
-  export_ids_kernel<<<(unsigned)div_up(I, 256), 256, 0, s>>>(I, ctx->vals[ctx->sorted_buf], ctx->vis_ids, out);
+  const int tiles = ctx->cam.tiles_x * ctx->cam.tiles_y;
+  if (I <= 0 || tiles == 0) return GS_OK;
+  export_ids_kernel<<<tiles, 128, 0, s>>>(tiles, ctx->ranges, ctx->vals[ctx->sorted_buf], ctx->vis_ids, out);
   GS_LAUNCH_CHECK("export_ids_kernel");
   return GS_OK;
 }
@@ -598,8 +615,13 @@ int launch_binning(gs_ctx* ctx, cudaStream_t s) {
   GS_PROF(3, s);
   if (ctx->N > 0) {
     emit_kernel<<<(unsigned)div_up(ctx->N, kEmitG), kEmitT, 0, s>>>(ctx->vis_rec, ctx->feat, ctx->cam.tiles_x,
-                                                                    ctx->tile_cursor, ctx->counts, ctx->keys[0]);
+                                                                    ctx->tile_cursor, ctx->counts, ctx->keys[0],
+                                                                    ctx->opt_exact_cull);
     GS_LAUNCH_CHECK("emit_kernel");
+    if (ctx->opt_exact_cull && tiles > 0) {
+      range_fix_kernel<<<(unsigned)div_up(tiles, 256), 256, 0, s>>>(tiles, ctx->tile_cursor, ctx->ranges);
+      GS_LAUNCH_CHECK("range_fix_kernel");
+    }
   }
   GS_PROF(4, s);
   if (ctx->N > 0 && tiles > 0) {

@@ -127,6 +127,7 @@ struct gs_ctx {
   gs::Counts* mailbox_dev = nullptr;  // device alias of the mailbox
 
   uint32_t* tile_order = nullptr;      // [tiles] tile ids by descending list length (longest lists are scheduled first)
+  bool opt_exact_cull = false;         // GS_OPT_EXACT_TILE_CULL (gs_set_option)
 
   // side stream: the zero fill of the dense gradient arrays overlaps the (ALU-bound) pixel backward
   cudaStream_t side_stream = nullptr;

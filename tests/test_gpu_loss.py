@@ -100,3 +100,52 @@ def test_loss_refine_matches_oracle(shape):
     scale = max(abs(ref["g_a"]), abs(ref["g_b"]), 1e-3)
     assert abs(ga - ref["g_a"]) <= 2e-5 * scale and abs(gb - ref["g_b"]) <= 2e-5 * scale, (ga, gb, ref["g_a"], ref["g_b"])
     assert abs(got[4] - ref["g_a"]) <= 2e-5 * scale and abs(got[5] - ref["g_b"]) <= 2e-5 * scale
+
+
+@pytest.mark.parametrize("shape", [(680, 1200), (33, 47), (2, 2), (1, 5)])
+def test_loss_normal_matches_oracle(shape):
+    """Depth-induced normals and lambda_n L_normal against oracle/normals.py: normals within 2e-6, loss within
+    1e-6 relative, depth gradient within 1e-4 relative L2 (added into d_depth)."""
+    import torch
+    import types
+    from oracle import normals as on
+    from paper_2605_10760_b200 import binding as b
+    H, W = shape
+    r = np.random.Generator(np.random.PCG64(21 + H))
+    cam = types.SimpleNamespace(fx=np.float32(600.0 * W / 1200), fy=np.float32(610.0 * W / 1200), cx=np.float32((W - 1) / 2), cy=np.float32((H - 1) / 2))
+    ys, xs = np.mgrid[0:H, 0:W]
+    depth = (2.0 + 0.002 * xs + 0.003 * ys + 0.01 * r.normal(size=(H, W))).astype(np.float32)
+    depth[r.uniform(size=(H, W)) < 0.05] = 0.0
+    prior = r.normal(size=(3, H, W)); prior[2] = -np.abs(prior[2]) - 1.0
+    prior = (prior / np.linalg.norm(prior, axis=0)).astype(np.float32)
+    prior[:, r.uniform(size=(H, W)) < 0.05] = 0.0
+    small = H * W > 100_000
+    if small:   # the pure-Python oracle on a 120 x 100 crop of the full-size image (same pixels: the crop's own borders differ)
+        y0, x0, hh, ww = 300, 500, 100, 120
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    dd0 = (1e-6 * r.normal(size=(H, W))).astype(np.float32)   # what an earlier loss term left in d_depth: the call ADDS to it
+    nout = torch.empty(3, H, W, device="cuda"); dd = t(dd0) if False else torch.from_numpy(dd0).cuda()
+    loss = torch.zeros(2, dtype=torch.float64, device="cuda")
+    b.gs_loss_normal(cam, t(depth), t(prior), 0.01, nout, dd, loss)
+    torch.cuda.synchronize()
+    got_n = nout.cpu().numpy(); got_g = dd.cpu().numpy().astype(np.float64) - dd0.astype(np.float64)
+    if small:
+        # interior of the crop: shift the principal point so that crop pixel (x, y) is image pixel (x0 + x, y0 + y)
+        ref_n, ok = on.normals(depth[y0:y0 + hh, x0:x0 + ww], cam.fx, cam.fy, cam.cx - x0, cam.cy - y0)
+        assert np.abs(got_n[:, y0:y0 + hh - 1, x0:x0 + ww - 1] - ref_n[:, :-1, :-1]).max() <= 2e-6
+        _, g = on.normal_loss(depth[y0:y0 + hh, x0:x0 + ww], prior[:, y0:y0 + hh, x0:x0 + ww], cam.fx, cam.fy, cam.cx - x0, cam.cy - y0)
+        g = g * (hh * ww) / (H * W) * 0.01          # crop mean -> full-image mean, times lambda_n
+        inner = (slice(1, hh - 1), slice(1, ww - 1))  # pixels whose three normals all lie inside the crop
+        sub = got_g[y0:y0 + hh, x0:x0 + ww]
+        assert np.linalg.norm(sub[inner] - g[inner]) <= 1e-4 * np.linalg.norm(g[inner]) + 1e-7 * np.linalg.norm(dd0)
+        return
+    ref_n, ok = on.normals(depth, cam.fx, cam.fy, cam.cx, cam.cy)
+    assert np.abs(got_n - ref_n).max() <= 2e-6
+    l, g = on.normal_loss(depth, prior, cam.fx, cam.fy, cam.cx, cam.cy)
+    assert abs(loss.cpu().numpy()[0] - 0.01 * l) <= 2e-6 * 0.01 * l + 1e-15
+    assert np.linalg.norm(got_g - 0.01 * g) <= 1e-4 * np.linalg.norm(0.01 * g) + 1e-7 * np.linalg.norm(dd0) + 1e-12
+    # normals only (no prior): same map, d_depth untouched
+    n2 = torch.empty(3, H, W, device="cuda")
+    b.gs_loss_normal(cam, t(depth), None, 0.0, n2, None, None)
+    torch.cuda.synchronize()
+    assert np.array_equal(n2.cpu().numpy(), got_n)

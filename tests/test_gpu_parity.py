@@ -417,3 +417,33 @@ def test_host_buffer_entry_point(oracle, gpu):
     check_image(ref, out)
     check_grads(ref, out)
     ctx.close()
+
+
+def test_exact_tile_cull_mode_gives_the_same_image_and_gradients_with_shorter_lists(oracle, gpu):
+    """GS_OPT_EXACT_TILE_CULL: corner tiles of a footprint's rectangle that the ellipse does not
+    reach get no list entry.  Outside the bit-exact binning contract: the lists must be ordered subsets of the default
+    lists; image and gradients keep the north_star tolerances."""
+    b, torch = gpu.binding, gpu.torch
+    sc = scenes.replica_scene(seed=38, N=30000, width=400, height=230, f=200.0, sh_degree=1)
+    sc.scales = (sc.scales * 3.0).astype(np.float32)      # footprints of several tiles, so that corner tiles exist
+    cam = sc.camera
+    gC, gD = scenes.upstream_gradients(38, cam.width, cam.height)
+    ref = oracle.forward_backward(sc, gC, gD)
+    base = run_gpu(gpu, sc, gC, gD)
+    ctx = b.Context(0)
+    ctx.gs_set_option(b.GS_OPT_EXACT_TILE_CULL, 1)
+    g2 = types.SimpleNamespace(ctx=ctx, binding=b, torch=torch)
+    got = run_gpu(g2, sc, gC, gD)
+    ctx.close()
+    check_image(ref, got)
+    check_grads(ref, got)
+    k0, i0, r0 = base["binning"]
+    k1, i1, r1 = got["binning"]
+    n0 = int((r0[:, 1] - r0[:, 0]).sum()); n1 = int((r1[:, 1] - r1[:, 0]).sum())
+    assert n1 < 0.97 * n0, (n0, n1)                      # a visible share of the instances is gone
+    for t in range(r0.shape[0]):
+        a0, e0 = r0[t]; a1, e1 = r1[t]
+        full = list(zip(k0[a0:e0].tolist(), i0[a0:e0].tolist()))
+        sub = list(zip(k1[a1:e1].tolist(), i1[a1:e1].tolist()))
+        it = iter(full)
+        assert all(x in it for x in sub), t             # ordered subsequence
