@@ -275,6 +275,33 @@ GS_API int64_t gs_compact_work_bytes(int64_t N);
 GS_API int gs_compact_plan(void* stream, int64_t N, const uint8_t* keep, uint32_t* index, int64_t* n_kept, void* work);
 GS_API int gs_compact_rows(void* stream, int64_t N, int32_t width, const uint32_t* index, const float* in, float* out);
 
+/* ---- one whole iteration of the joint refinement (Eq. 23) over a batch of keyframe views ----------- */
+/* For every view k: gs_preprocess -> gs_bin_tiles -> gs_rasterize_fwd -> gs_loss_refine on I~ = e^{a_k} I^ + b_k (+ gs_loss_normal
+ * if normal priors are given) -> gs_rasterize_bwd with the parameter gradients ACCUMULATED over the views -> gs_pose_grad:
+ * everything the refinement differentiates (the fused Gaussians, the per-keyframe pose deltas and the per-keyframe log-gain
+ * and bias) in one call, no framework op and no host synchronisation in between.  All views share one image size.
+ *   batch (HOST struct): cams HOST [n_views]; T_cw_dev NULL or DEVICE [n_views,12] poses that override the cams' (pose
+ *     deltas applied on the device); target_rgb DEVICE [n_views,3,H,W]; target_depth DEVICE [n_views,H,W]; normal_prior NULL
+ *     or DEVICE [n_views,3,H,W]; ab DEVICE [n_views,2]; the weights of Eq. 23 (paper: 1.75, 0.2, 0.25; lambda_n garbled, Q16).
+ *   grads      DEVICE arrays of the parameter shapes: sum over the views of dL_k/dparam (written by view 0, accumulated after)
+ *   g_twist    DEVICE [n_views,6]; g_ab DEVICE [n_views,2]
+ *   loss       DEVICE double [n_views,10]: the eight entries of gs_loss_refine, then lambda_n L_normal and a scratch word
+ *   visible    NULL or DEVICE uint32[N]: 1 where the Gaussian was on screen in at least one view (the mask of gs_adam_step)
+ * The rendered images live in context-owned scratch.  Same asynchrony and overflow protocol as the five calls. */
+typedef struct {
+  int32_t n_views;
+  const gs_camera* cams;
+  const float* T_cw_dev;
+  const float* target_rgb;
+  const float* target_depth;
+  const float* normal_prior;
+  const float* ab;
+  float alpha_p, lambda, beta, lambda_n;
+} gs_refine_batch;
+GS_API int gs_refine_views(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, const gs_gaussians* params,
+                           const gs_refine_batch* batch, const float* bg, const gs_gaussians* grads, float* g_twist, float* g_ab,
+                           double* loss, uint32_t* visible);
+
 /* ---- measured machine peaks: the denominators of bench.py's roofline entries -------- */
 /* Runs small synthetic kernels on `device` (allocates and frees ~2 GiB, synchronises; ~0.2 s) and fills HOST double
  * out[GS_NUM_PEAKS]:  FP32 FMA lane rate (T lane-FMA/s; x2 = TFLOP/s), mixed FFMA+integer issue rate (T warp

@@ -24,7 +24,7 @@ EXPORTS = ["gs_create", "gs_destroy", "gs_last_error", "gs_preprocess", "gs_bin_
            "gs_aux_l1_grad", "gs_aux_pose_step", "gs_fwd_bwd_host", "gs_profile_enable", "gs_profile_read",
            "gs_get_launch_count", "gs_get_workload", "gs_loss_map", "gs_loss_iso", "gs_sim3_apply", "gs_measure_peaks", "gs_loss_refine", "gs_voxel_set_clear", "gs_voxel_insert_boxes",
            "gs_voxel_insert_rays", "gs_voxel_retain", "gs_adam_step", "gs_prune_mask", "gs_compact_work_bytes",
-           "gs_compact_plan", "gs_compact_rows", "gs_loss_normal", "gs_set_option"]
+           "gs_compact_plan", "gs_compact_rows", "gs_loss_normal", "gs_set_option", "gs_refine_views"]
 GS_OPT_EXACT_TILE_CULL = 1
 PEAKS = ["fma_tlanes", "issue_twarp", "ex2_tlanes", "lds128_bcast_twarp", "lds128_twarp", "lds32_bcast_twarp",
          "lds64_bcast_twarp", "red_glanes", "hbm_read_gbs", "hbm_write_gbs", "hbm_copy_gbs", "sm_count", "sm_mhz_max"]
@@ -44,6 +44,12 @@ class gs_camera(C.Structure):
 
 class gs_gaussians(C.Structure):
     _fields_ = [(k, C.c_void_p) for k in ("means", "scales", "quats", "opacities", "sh")]
+
+
+class gs_refine_batch(C.Structure):
+    _fields_ = [("n_views", C.c_int32), ("cams", C.POINTER(gs_camera)), ("T_cw_dev", C.c_void_p), ("target_rgb", C.c_void_p),
+                ("target_depth", C.c_void_p), ("normal_prior", C.c_void_p), ("ab", C.c_void_p), ("alpha_p", C.c_float),
+                ("lambda_", C.c_float), ("beta", C.c_float), ("lambda_n", C.c_float)]
 
 
 class gs_adam_config(C.Structure):
@@ -96,6 +102,8 @@ def load_library():
     lib.gs_compact_plan.argtypes = [vp, i64, vp, vp, vp, vp]
     lib.gs_compact_rows.argtypes = [vp, i64, C.c_int32, vp, vp, vp]
     lib.gs_loss_normal.argtypes = [vp, C.c_int32, C.c_int32, f, f, f, f, vp, vp, f, vp, vp, vp]
+    lib.gs_refine_views.argtypes = [vp, vp, i64, C.c_int, C.POINTER(gs_gaussians), C.POINTER(gs_refine_batch), C.POINTER(f * 3),
+                                    C.POINTER(gs_gaussians), vp, vp, vp, vp]
     lib.gs_measure_peaks.argtypes = [C.c_int, vp, C.POINTER(C.c_double * len(PEAKS))]
     lib.gs_fwd_bwd_host.argtypes = [vp, vp, i64, C.c_int, vp, vp, vp, vp, vp, C.POINTER(gs_camera), C.POINTER(f * 3)] + [vp] * 11
     for name in EXPORTS:
@@ -202,6 +210,23 @@ class Context:
     def gs_pose_grad(self, flags, g_twist, stream=None):
         import torch
         self._check(self.lib.gs_pose_grad(self._h, _stream(stream), int(flags), _ptr(g_twist, torch.float32)))
+
+    def gs_refine_views(self, params, sh_degree, cams, target_rgb, target_depth, ab, weights, bg, grads, g_twist, g_ab, loss,
+                        normal_prior=None, T_cw_dev=None, visible=None, stream=None):
+        """One Eq. 23 iteration over the views (include/gs.h).  params / grads: dicts of CUDA tensors; cams: list of cameras;
+        target_rgb [V,3,H,W], target_depth [V,H,W], ab [V,2]; weights = (alpha', lambda, beta, lambda_n)."""
+        import torch
+        V = len(cams)
+        arr = (gs_camera * V)(*[c if isinstance(c, gs_camera) else camera_struct(c) for c in cams])
+        p = lambda t: None if t is None else t.data_ptr()
+        batch = gs_refine_batch(V, arr, p(T_cw_dev), p(target_rgb), p(target_depth), p(normal_prior), p(ab), float(weights[0]),
+                                float(weights[1]), float(weights[2]), float(weights[3]))
+        gp, gg = _gaussians(params), _gaussians(grads)
+        self._keep = (params, grads, target_rgb, target_depth, ab, normal_prior, T_cw_dev, arr)
+        self._check(self.lib.gs_refine_views(self._h, _stream(stream), int(params["means"].shape[0]), int(sh_degree), C.byref(gp),
+                                             C.byref(batch), _bg(bg), C.byref(gg), _ptr(g_twist, torch.float32),
+                                             _ptr(g_ab, torch.float32), _ptr(loss, torch.float64),
+                                             None if visible is None else C.c_void_p(visible.data_ptr())))
 
     # -- introspection -------------------------------------------------------------------------------------------
     def gs_get_counts(self, stream=None):

@@ -123,6 +123,12 @@ static int alloc_header(gs_ctx* ctx, int64_t tiles) {
   return GS_OK;
 }
 
+// visible[i] = (first ? 0 : visible[i]) | (tiles_touched[i] > 0): which Gaussians were on screen in any view so far
+__global__ void visible_or_kernel(int64_t N, const uint32_t* __restrict__ tiles_touched, uint32_t* __restrict__ visible, bool first) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < N) visible[i] = (first ? 0u : visible[i]) | (tiles_touched[i] > 0u ? 1u : 0u);
+}
+
 static int ensure_image_capacity(gs_ctx* ctx, int64_t tiles, int64_t pix) {
   int rc;
   if (tiles > ctx->cap_tiles) {
@@ -181,7 +187,7 @@ int gs_destroy(gs_ctx* ctx) {
   cudaFree(ctx->inst_uv);
   cudaFree(ctx->hdr); cudaFree(ctx->tile_cursor); cudaFree(ctx->scan_ws);
   cudaFree(ctx->ranges); cudaFree(ctx->tile_order); cudaFree(ctx->final_T); cudaFree(ctx->n_contrib);
-  cudaFree(ctx->hb); cudaFree(ctx->stats_ws);
+  cudaFree(ctx->hb); cudaFree(ctx->stats_ws); cudaFree(ctx->rv);
   if (ctx->mailbox) cudaFreeHost(ctx->mailbox);
   if (ctx->side_stream) cudaStreamDestroy(ctx->side_stream);
   if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
@@ -418,6 +424,56 @@ int gs_aux_pose_step(void* stream, float* T_cw_dev, const float* g_twist, float 
   if (!T_cw_dev || !g_twist) return GS_E_INVALID;
   pose_step_kernel<<<1, 32, 0, (cudaStream_t)stream>>>(T_cw_dev, g_twist, step);
   return cudaGetLastError() == cudaSuccess ? GS_OK : GS_E_CUDA;
+}
+
+int gs_refine_views(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, const gs_gaussians* params,
+                    const gs_refine_batch* batch, const float* bg, const gs_gaussians* grads, float* g_twist, float* g_ab,
+                    double* loss, uint32_t* visible) {
+  if (!ctx) return GS_E_INVALID;
+  if (!params || !batch || !grads || !g_twist || !g_ab || !loss || batch->n_views < 1 || !batch->cams || !batch->target_rgb ||
+      !batch->target_depth || !batch->ab)
+    return fail(ctx, GS_E_INVALID, "gs_refine_views: null argument or no view");
+  const int32_t W = batch->cams[0].width, H = batch->cams[0].height;
+  for (int v = 0; v < batch->n_views; ++v)
+    if (batch->cams[v].width != W || batch->cams[v].height != H) return fail(ctx, GS_E_INVALID, "gs_refine_views: views differ in size");
+  if (W <= 0 || H <= 0) return fail(ctx, GS_E_INVALID, "gs_refine_views: empty image");
+  cudaStream_t s = (cudaStream_t)stream;
+  GS_CUDA(cudaSetDevice(ctx->device));
+  const int64_t P = (int64_t)W * H;
+  if (18 * P > ctx->rv_floats) {   // rendered rgb (3), depth, alpha, d_rgb (3), d_depth, SSIM scratch (9)
+    GS_CUDA(cudaDeviceSynchronize());
+    int rc = grow(ctx, ctx->rv, 18 * P);
+    if (rc != GS_OK) { ctx->rv_floats = 0; return rc; }
+    ctx->rv_floats = 18 * P;
+  }
+  float *rgb = ctx->rv, *depth = rgb + 3 * P, *alpha = depth + P, *d_rgb = alpha + P, *d_depth = d_rgb + 3 * P, *work = d_depth + P;
+  for (int v = 0; v < batch->n_views; ++v) {
+    int rc;
+    const float* T_dev = batch->T_cw_dev ? batch->T_cw_dev + 12 * v : nullptr;
+    if ((rc = gs_preprocess(ctx, stream, N, sh_degree, params->means, params->scales, params->quats, params->opacities,
+                            params->sh, &batch->cams[v], T_dev)) != GS_OK) return rc;
+    if ((rc = gs_bin_tiles(ctx, stream)) != GS_OK) return rc;
+    if ((rc = gs_rasterize_fwd(ctx, stream, bg, rgb, depth, alpha)) != GS_OK) return rc;
+    double* lv = loss + 10 * v;
+    if ((rc = gs_loss_refine(stream, W, H, rgb, depth, batch->target_rgb + 3 * P * v, batch->target_depth + P * v,
+                             batch->ab + 2 * v, batch->alpha_p, batch->lambda, batch->beta, d_rgb, d_depth, g_ab + 2 * v, work,
+                             lv)) != GS_OK) return fail(ctx, rc, "gs_refine_views: gs_loss_refine failed");
+    if (batch->normal_prior) {
+      const gs_camera& c = batch->cams[v];
+      if ((rc = gs_loss_normal(stream, W, H, c.fx, c.fy, c.cx, c.cy, depth, batch->normal_prior + 3 * P * v, batch->lambda_n,
+                               nullptr, d_depth, lv + 8)) != GS_OK) return fail(ctx, rc, "gs_refine_views: gs_loss_normal failed");
+    } else {
+      GS_CUDA(cudaMemsetAsync(lv + 8, 0, 2 * sizeof(double), s));
+    }
+    if ((rc = gs_rasterize_bwd(ctx, stream, d_rgb, d_depth, nullptr, v > 0 ? GS_ACCUMULATE : 0u, grads->means, grads->scales,
+                               grads->quats, grads->opacities, grads->sh)) != GS_OK) return rc;
+    if ((rc = gs_pose_grad(ctx, stream, 0u, g_twist + 6 * v)) != GS_OK) return rc;
+    if (visible && N > 0) {
+      visible_or_kernel<<<(unsigned)div_up(N, 256), 256, 0, s>>>(N, ctx->tiles_touched, visible, v == 0);
+      GS_LAUNCH_CHECK("visible_or_kernel");
+    }
+  }
+  return GS_OK;
 }
 
 int gs_fwd_bwd_host(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, const float* means, const float* scales,

@@ -140,6 +140,10 @@ struct gs_ctx {
   bool ev_made = false;
   uint64_t launches = 0;  // kernels launched by this context (gs_get_launch_count)
 
+  // gs_refine_views: rendered images, upstream gradients and SSIM scratch of one view (18 H W floats), grown on demand
+  float* rv = nullptr;
+  int64_t rv_floats = 0;
+
   // host-buffer path (gs_fwd_bwd_host): device staging, grown on demand
   float* hb = nullptr;
   int64_t hb_floats = 0;
