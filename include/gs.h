@@ -66,6 +66,10 @@ typedef struct gs_ctx gs_ctx; /* opaque */
 /* flags of gs_rasterize_bwd / gs_pose_grad */
 #define GS_ACCUMULATE 1u /* parameter gradients are added to the output arrays instead of overwriting them (config 5) */
 #define GS_POSE_ONLY 2u  /* Gaussians frozen: no parameter gradients are written; output pointers may be NULL (config 4) */
+#define GS_SPARSE_GRADS 4u /* parameter gradients are written COMPACT: row r of every g_* array belongs to the Gaussian
+                            gs_visible_ids()[r], r < n_visible (arrays need n_visible <= N rows); rows of culled Gaussians do
+                            not exist (their gradient is zero), nothing is zero-filled.  What gs_adam_step_sparse consumes: the
+                            dense (11 + 3K) N gradient write is 1/3 of the iteration's HBM bytes.  Not with GS_ACCUMULATE. */
 
 /* Compile-time semantics of the rasteriser (DESIGN.md readings; north_star of BASELINE.json) */
 #define GS_TILE 16               /* binning tiles are 16x16 pixels */
@@ -150,6 +154,13 @@ GS_API int gs_get_binning(gs_ctx* ctx, void* stream, uint64_t* keys_sorted, uint
  * depth), rect int32[N,4] tile rectangle tx0,ty0,tx1,ty1 (half-open; all zero = culled).  Any may be NULL. */
 GS_API int gs_get_features(gs_ctx* ctx, void* stream, double* mean2d, float* conic, float* color, float* depth,
                     uint32_t* depth_key, int32_t* rect);
+/* DEVICE pointers (context-owned, valid until the next gs_preprocess) to the compacted indices of the visible Gaussians of
+ * the last gs_preprocess, uint32[n_visible] in visible-slot order (arbitrary but fixed for the iteration), and to the count
+ * itself: the row order of GS_SPARSE_GRADS gradients.  No synchronisation. */
+GS_API int gs_visible_ids(gs_ctx* ctx, const uint32_t** ids, const uint32_t** n_visible);
+/* Copies that index list into caller-owned DEVICE memory ids_out uint32[N] (entries beyond n_visible are unspecified);
+ * asynchronous on `stream`. */
+GS_API int gs_get_visible_ids(gs_ctx* ctx, void* stream, uint32_t* ids_out);
 /* Non-blocking: GS_E_OVERFLOW if an earlier asynchronous iteration overflowed the instance capacity, else GS_OK. */
 GS_API int gs_poll(gs_ctx* ctx);
 
@@ -265,6 +276,12 @@ typedef struct {
  * cfg HOST.  In place, asynchronous (five launches).  GS_E_INVALID on null pointers, degree outside 0..3, step < 1. */
 GS_API int gs_adam_step(void* stream, int64_t N, int sh_degree, const gs_adam_config* cfg, const gs_gaussians* params,
                         const gs_gaussians* grads, const gs_gaussians* m, const gs_gaussians* v, const uint32_t* visible);
+/* The same step on GS_SPARSE_GRADS gradients: grads arrays hold one row per visible Gaussian, row r -> Gaussian ids[r],
+ * r < *n_rows (DEVICE count, e.g. from gs_visible_ids); max_rows >= *n_rows bounds the launch (N is always enough).
+ * Touches exactly the Gaussians listed (parameters and moments), like gs_adam_step with a visibility mask. */
+GS_API int gs_adam_step_sparse(void* stream, int64_t N, int sh_degree, const gs_adam_config* cfg, const gs_gaussians* params,
+                               const gs_gaussians* grads, const gs_gaussians* m, const gs_gaussians* v, const uint32_t* ids,
+                               const uint32_t* n_rows, int64_t max_rows);
 /* keep[i] = opacities[i] >= min_opacity  ("prunes Gaussians with opacity below 0.005").  DEVICE uint8 keep[N]. */
 GS_API int gs_prune_mask(void* stream, int64_t N, const float* opacities, float min_opacity, uint8_t* keep);
 /* Order-preserving stream compaction, shared by pruning and by the retain test of Eq. 22.  gs_compact_plan turns a keep

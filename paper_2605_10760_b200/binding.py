@@ -11,6 +11,7 @@ import numpy as np
 
 GS_ACCUMULATE = 1
 GS_POSE_ONLY = 2
+GS_SPARSE_GRADS = 4
 GS_TILE = 16
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -24,7 +25,7 @@ EXPORTS = ["gs_create", "gs_destroy", "gs_last_error", "gs_preprocess", "gs_bin_
            "gs_aux_l1_grad", "gs_aux_pose_step", "gs_fwd_bwd_host", "gs_profile_enable", "gs_profile_read",
            "gs_get_launch_count", "gs_get_workload", "gs_loss_map", "gs_loss_iso", "gs_sim3_apply", "gs_measure_peaks", "gs_loss_refine", "gs_voxel_set_clear", "gs_voxel_insert_boxes",
            "gs_voxel_insert_rays", "gs_voxel_retain", "gs_adam_step", "gs_prune_mask", "gs_compact_work_bytes",
-           "gs_compact_plan", "gs_compact_rows", "gs_loss_normal", "gs_set_option", "gs_refine_views"]
+           "gs_compact_plan", "gs_compact_rows", "gs_loss_normal", "gs_set_option", "gs_refine_views", "gs_visible_ids", "gs_adam_step_sparse", "gs_get_visible_ids"]
 GS_OPT_EXACT_TILE_CULL = 1
 PEAKS = ["fma_tlanes", "issue_twarp", "ex2_tlanes", "lds128_bcast_twarp", "lds128_twarp", "lds32_bcast_twarp",
          "lds64_bcast_twarp", "red_glanes", "hbm_read_gbs", "hbm_write_gbs", "hbm_copy_gbs", "sm_count", "sm_mhz_max"]
@@ -102,6 +103,10 @@ def load_library():
     lib.gs_compact_plan.argtypes = [vp, i64, vp, vp, vp, vp]
     lib.gs_compact_rows.argtypes = [vp, i64, C.c_int32, vp, vp, vp]
     lib.gs_loss_normal.argtypes = [vp, C.c_int32, C.c_int32, f, f, f, f, vp, vp, f, vp, vp, vp]
+    lib.gs_visible_ids.argtypes = [vp, C.POINTER(vp), C.POINTER(vp)]
+    lib.gs_get_visible_ids.argtypes = [vp, vp, vp]
+    lib.gs_adam_step_sparse.argtypes = [vp, i64, C.c_int, C.POINTER(gs_adam_config), C.POINTER(gs_gaussians), C.POINTER(gs_gaussians),
+                                        C.POINTER(gs_gaussians), C.POINTER(gs_gaussians), vp, vp, i64]
     lib.gs_refine_views.argtypes = [vp, vp, i64, C.c_int, C.POINTER(gs_gaussians), C.POINTER(gs_refine_batch), C.POINTER(f * 3),
                                     C.POINTER(gs_gaussians), vp, vp, vp, vp]
     lib.gs_measure_peaks.argtypes = [C.c_int, vp, C.POINTER(C.c_double * len(PEAKS))]
@@ -265,6 +270,19 @@ class Context:
         res["depth_key"] = res["depth_key"].view(np.uint32)
         return res
 
+    def gs_visible_ids(self):
+        """(ids_ptr, n_visible_ptr): raw DEVICE addresses (ints) of the visible-Gaussian index list and its count."""
+        a, b = C.c_void_p(), C.c_void_p()
+        self._check(self.lib.gs_visible_ids(self._h, C.byref(a), C.byref(b)))
+        return int(a.value), int(b.value)
+
+    def gs_get_visible_ids(self, stream=None):
+        """int32 CUDA tensor [N] holding the visible-Gaussian indices in slot order (first n_visible entries valid)."""
+        import torch
+        out = torch.empty(max(self.N, 1), dtype=torch.int32, device=torch.device("cuda", self.device))
+        self._check(self.lib.gs_get_visible_ids(self._h, _stream(stream), _ptr(out)))
+        return out[:self.N]
+
     def gs_set_option(self, option: int, value: int):
         self._check(self.lib.gs_set_option(self._h, int(option), int(value)))
 
@@ -409,6 +427,21 @@ def gs_adam_step(params, grads, m, v, lrs, step, visible=None, beta1=0.9, beta2=
     rc = load_library().gs_adam_step(_stream(stream), N, deg, C.byref(cfg), C.byref(gp), C.byref(gg), C.byref(gm), C.byref(gv), vis)
     if rc != 0:
         raise GsError(rc, "gs_adam_step")
+
+
+def gs_adam_step_sparse(params, grads, m, v, lrs, step, ids_ptr, n_rows_ptr, max_rows, beta1=0.9, beta2=0.999, eps=1e-15,
+                        stream=None):
+    """gs_adam_step on GS_SPARSE_GRADS gradients; ids_ptr / n_rows_ptr: device addresses from Context.gs_visible_ids()."""
+    N = int(params["means"].shape[0])
+    K = int(params["sh"].shape[1])
+    deg = int(round(K ** 0.5)) - 1
+    cfg = gs_adam_config(float(lrs["means"]), float(lrs["scales"]), float(lrs["quats"]), float(lrs["opacities"]), float(lrs["sh"]),
+                         float(beta1), float(beta2), float(eps), int(step))
+    gp, gg, gm, gv = _gaussians(params), _gaussians(grads), _gaussians(m), _gaussians(v)
+    rc = load_library().gs_adam_step_sparse(_stream(stream), N, deg, C.byref(cfg), C.byref(gp), C.byref(gg), C.byref(gm),
+                                            C.byref(gv), C.c_void_p(ids_ptr), C.c_void_p(n_rows_ptr), int(max_rows))
+    if rc != 0:
+        raise GsError(rc, "gs_adam_step_sparse")
 
 
 def gs_prune_mask(opacities, min_opacity, keep, stream=None):

@@ -202,6 +202,23 @@ int gs_destroy(gs_ctx* ctx) {
 
 const char* gs_last_error(const gs_ctx* ctx) { return ctx ? ctx->err : "null context"; }
 
+int gs_visible_ids(gs_ctx* ctx, const uint32_t** ids, const uint32_t** n_visible) {
+  if (!ctx || !ids || !n_visible) return GS_E_INVALID;
+  if (ctx->stage < 1) return fail(ctx, GS_E_ORDER, "gs_visible_ids before gs_preprocess");
+  *ids = ctx->vis_ids;
+  *n_visible = &ctx->counts->n_visible;
+  return GS_OK;
+}
+
+int gs_get_visible_ids(gs_ctx* ctx, void* stream, uint32_t* ids_out) {
+  if (!ctx || !ids_out) return GS_E_INVALID;
+  if (ctx->stage < 1) return fail(ctx, GS_E_ORDER, "gs_get_visible_ids before gs_preprocess");
+  GS_CUDA(cudaSetDevice(ctx->device));
+  if (ctx->N > 0)
+    GS_CUDA(cudaMemcpyAsync(ids_out, ctx->vis_ids, (size_t)ctx->N * sizeof(uint32_t), cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+  return GS_OK;
+}
+
 int gs_set_option(gs_ctx* ctx, int option, int value) {
   if (!ctx) return GS_E_INVALID;
   if (option == GS_OPT_EXACT_TILE_CULL) { ctx->opt_exact_cull = value != 0; return GS_OK; }
@@ -280,6 +297,8 @@ int gs_rasterize_bwd(gs_ctx* ctx, void* stream, const float* d_rgb, const float*
   if (ctx->stage < 3) return fail(ctx, GS_E_ORDER, "gs_rasterize_bwd before gs_rasterize_fwd");
   if (!d_rgb) return fail(ctx, GS_E_INVALID, "gs_rasterize_bwd: d_rgb is null");
   const bool write = !(flags & GS_POSE_ONLY);
+  if ((flags & GS_SPARSE_GRADS) && (flags & GS_ACCUMULATE))
+    return fail(ctx, GS_E_INVALID, "gs_rasterize_bwd: GS_SPARSE_GRADS cannot be combined with GS_ACCUMULATE (the rows of two views differ)");
   if (write && ctx->N > 0 && (!g_means || !g_scales || !g_quats || !g_opacities || !g_sh))
     return fail(ctx, GS_E_INVALID, "gs_rasterize_bwd: null gradient array without GS_POSE_ONLY");
   if (write && ((uintptr_t)g_quats & 15) != 0) return fail(ctx, GS_E_INVALID, "gs_rasterize_bwd: g_quats must be 16-byte aligned");
@@ -292,7 +311,7 @@ int gs_rasterize_bwd(gs_ctx* ctx, void* stream, const float* d_rgb, const float*
   ctx->pose_acc_valid = false;
   GS_PROF(8, s);
   int rc;
-  const bool fork = write && !(flags & GS_ACCUMULATE) && ctx->N > 0 && ctx->side_stream;
+  const bool fork = write && !(flags & (GS_ACCUMULATE | GS_SPARSE_GRADS)) && ctx->N > 0 && ctx->side_stream;
   if (fork) {  // zero fill of the dense gradient arrays on the side stream, overlapping the pixel backward
     GS_CUDA(cudaEventRecord(ctx->ev_fork, s));
     GS_CUDA(cudaStreamWaitEvent(ctx->side_stream, ctx->ev_fork, 0));

@@ -195,7 +195,8 @@ emit_kernel(const uint4* __restrict__ vis_rec, const float4* __restrict__ feat, 
   // key = depth bits << 32 | index << 8 | region mask (the mask is a function of (index, tile): the order is unchanged)
   __shared__ uint32_t s_excl[kEmitG + 1], s_w[kEmitG], s_xy[kEmitG];
   __shared__ uint64_t s_key[kEmitG];
-  __shared__ float4 s_f0[kEmitG], s_f1[kEmitG];
+  __shared__ float4 s_f0[kEmitG];
+  __shared__ MaskSetup s_ms[kEmitG];
   const int tid = threadIdx.x;
   const uint32_t V = counts->n_visible;
   const uint32_t k0 = blockIdx.x * kEmitG;
@@ -206,7 +207,8 @@ emit_kernel(const uint4* __restrict__ vis_rec, const float4* __restrict__ feat, 
     if (k < V) {
       rec = __ldg(vis_rec + k);
       s_f0[tid] = __ldg(feat + 3 * (size_t)k);  // the feature records are stored by visible slot
-      s_f1[tid] = __ldg(feat + 3 * (size_t)k + 1);
+      const float4 f1 = __ldg(feat + 3 * (size_t)k + 1);
+      s_ms[tid] = region_mask_setup(f1.x, f1.y, f1.z, f1.w);
     }
     const uint32_t w = (rec.y & 0xffffu) - (rec.x & 0xffffu), h = (rec.y >> 16) - (rec.x >> 16);
     const uint32_t n = w * h;
@@ -242,11 +244,11 @@ emit_kernel(const uint4* __restrict__ vis_rec, const float4* __restrict__ feat, 
         cur[u] = &tile_cursor[(size_t)(ty * tiles_x + tx) * kCtrStride];
         // 8-bit mask of the tile's 8x4-pixel regions the ellipse {alpha >= 1/255} can reach (gs_raster.cuh), decided
         // ONCE per instance here instead of per (region, batch) in both compositing kernels
-        const float4 f0 = s_f0[owner], f1 = s_f1[owner];
+        const float4 f0 = s_f0[owner];
         const int pk = __float_as_int(f0.z);
         const float mx = (float)(((pk << 16) >> 16) - (int)tx * GS_TILE) + f0.x;
         const float my = (float)((pk >> 16) - (int)ty * GS_TILE) + f0.y;
-        const uint32_t mask = region_mask(f1.x, f1.y, f1.z, f1.w, mx, my);
+        const uint32_t mask = region_mask(s_ms[owner], mx, my);
         kk[u] = s_key[owner] | (uint64_t)mask;
         // GS_OPT_EXACT_TILE_CULL: a tile of the rect that the ellipse itself does not reach (empty region mask) gets no
         // list entry at all; range_fix_kernel then shortens the tile's range to what was emitted

@@ -25,7 +25,7 @@ gauss_bwd_kernel(int64_t N, const float* __restrict__ means, const float* __rest
                  const float* __restrict__ quats, const float* __restrict__ opacities, const float* __restrict__ sh,
                  DevCam cam, const uint32_t* __restrict__ vis_ids, const float4* __restrict__ vis_par,
                  const float4* __restrict__ feat, const Counts* __restrict__ counts,
-                 float* __restrict__ g2d, bool accumulate,
+                 float* __restrict__ g2d, bool accumulate, bool sparse,
                  float* __restrict__ g_means, float* __restrict__ g_scales, float* __restrict__ g_quats,
                  float* __restrict__ g_opac, float* __restrict__ g_sh, double* __restrict__ pose_acc) {
   constexpr int K = (DEG + 1) * (DEG + 1);
@@ -35,6 +35,7 @@ gauss_bwd_kernel(int64_t N, const float* __restrict__ means, const float* __rest
   if ((int64_t)blockIdx.x * blockDim.x >= (int64_t)V) return;
   const bool vis = kk < (int64_t)V;
   const int64_t i = vis ? (int64_t)vis_ids[kk] : 0;
+  const int64_t orow = sparse ? kk : i;  // output row: GS_SPARSE_GRADS writes one row per VISIBLE Gaussian, in slot order
   (void)N;
   float T[12];
   load_pose(cam, T);
@@ -163,15 +164,15 @@ gauss_bwd_kernel(int64_t N, const float* __restrict__ means, const float* __rest
                              W[2] * gpc[0] + W[5] * gpc[1] + W[8] * gpc[2] + gv[2]};
 #pragma unroll
       for (int k = 0; k < 3; ++k) {
-        store_or_add(g_means + 3 * i + k, (float)gmu[k], accumulate);
-        store_or_add(g_scales + 3 * i + k, (float)gs_[k], accumulate);
+        store_or_add(g_means + 3 * orow + k, (float)gmu[k], accumulate);
+        store_or_add(g_scales + 3 * orow + k, (float)gs_[k], accumulate);
       }
-      float4* gq4 = reinterpret_cast<float4*>(g_quats + 4 * i);
+      float4* gq4 = reinterpret_cast<float4*>(g_quats + 4 * orow);
       float4 qo = make_float4((float)gq[0], (float)gq[1], (float)gq[2], (float)gq[3]);
       if (accumulate) { const float4 old = *gq4; qo.x += old.x; qo.y += old.y; qo.z += old.z; qo.w += old.w; }
       *gq4 = qo;
-      store_or_add(g_opac + i, (float)g_o, accumulate);
-      float* gsh = g_sh + (int64_t)3 * K * i;
+      store_or_add(g_opac + orow, (float)g_o, accumulate);
+      float* gsh = g_sh + (int64_t)3 * K * orow;
       if constexpr ((3 * K) % 4 == 0) {
 #pragma unroll
         for (int v = 0; v < 3 * K / 4; ++v) {
@@ -254,7 +255,8 @@ int launch_gauss_bwd(gs_ctx* ctx, cudaStream_t s, uint32_t flags, float* g_means
   if (ctx->N == 0) return GS_OK;
   const bool write = !(flags & GS_POSE_ONLY);
   const bool accum = (flags & GS_ACCUMULATE) != 0;
-  if (write && !accum && !ctx->zero_filled) {
+  const bool sparse = (flags & GS_SPARSE_GRADS) != 0;
+  if (write && !accum && !sparse && !ctx->zero_filled) {
     int rc = launch_zero_fill(ctx, s, g_means, g_scales, g_quats, g_opac, g_sh);
     if (rc != GS_OK) return rc;
   }
@@ -263,7 +265,7 @@ int launch_gauss_bwd(gs_ctx* ctx, cudaStream_t s, uint32_t flags, float* g_means
   const unsigned blocks = (unsigned)div_up(ctx->N, threads);
 #define GS_GB(D, Wr)                                                                                                 \
   gauss_bwd_kernel<D, Wr><<<blocks, threads, 0, s>>>(ctx->N, ctx->means, ctx->scales, ctx->quats, ctx->opacities,   \
-                                                      ctx->sh, ctx->cam, ctx->vis_ids, ctx->vis_par, ctx->feat, ctx->counts, ctx->g2d, accum, \
+                                                      ctx->sh, ctx->cam, ctx->vis_ids, ctx->vis_par, ctx->feat, ctx->counts, ctx->g2d, accum, sparse, \
                                                       g_means, g_scales, g_quats, g_opac, g_sh, ctx->pose_acc)
   if (write) {
     switch (ctx->sh_degree) {

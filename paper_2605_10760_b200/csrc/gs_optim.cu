@@ -40,6 +40,33 @@ adam_kernel(int64_t n, int32_t width, float* __restrict__ p, const float* __rest
   }
 }
 
+// the same step on compact gradient rows (GS_SPARSE_GRADS): row r belongs to Gaussian ids[r], r < *n_rows
+template <int MODE>
+__global__ void __launch_bounds__(256)
+adam_sparse_kernel(int64_t max_n, int32_t width, float* __restrict__ p, const float* __restrict__ g, float* __restrict__ m,
+                   float* __restrict__ v, const uint32_t* __restrict__ ids, const uint32_t* __restrict__ n_rows, float lr,
+                   float beta1, float beta2, float eps, float ibc1, float ibc2) {
+  const int64_t n = min(max_n, (int64_t)__ldg(n_rows) * width);
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; r < n; r += stride) {
+    const int64_t row = r / width;
+    const int64_t e = (int64_t)__ldg(ids + row) * width + (r - row * width);
+    const float x = p[e];
+    float gr = g[r];
+    if (MODE == kLog) gr *= x;
+    if (MODE == kLogit) gr *= x * (1.f - x);
+    const float mn = fmaf(beta1, m[e], (1.f - beta1) * gr);
+    const float vn = fmaf(beta2, v[e], (1.f - beta2) * gr * gr);
+    m[e] = mn; v[e] = vn;
+    const float d = -lr * (mn * ibc1) / (sqrtf(vn * ibc2) + eps);
+    float xn;
+    if (MODE == kDirect) xn = x + d;
+    else if (MODE == kLog) xn = x * expf(d);
+    else { const float t = x * expf(d); xn = t / ((1.f - x) + t); }
+    p[e] = xn;
+  }
+}
+
 __global__ void __launch_bounds__(256)
 prune_mask_kernel(int64_t N, const float* __restrict__ opac, float min_opacity, uint8_t* __restrict__ keep) {
   const int64_t stride = (int64_t)gridDim.x * blockDim.x;
@@ -181,6 +208,35 @@ int gs_adam_step(void* stream, int64_t N, int sh_degree, const gs_adam_config* c
     const int grid = grid_for(n);
 #define GS_ADAM(MODE) adam_kernel<MODE><<<grid, 256, 0, s>>>(n, width[k], P[k], G[k], M[k], V[k], visible, lr[k], cfg->beta1, \
                                                             cfg->beta2, cfg->eps, ibc1, ibc2)
+    if (k == 1) GS_ADAM(kLog); else if (k == 3) GS_ADAM(kLogit); else GS_ADAM(kDirect);
+#undef GS_ADAM
+  }
+  return cudaGetLastError() == cudaSuccess ? GS_OK : GS_E_CUDA;
+}
+
+int gs_adam_step_sparse(void* stream, int64_t N, int sh_degree, const gs_adam_config* cfg, const gs_gaussians* params,
+                        const gs_gaussians* grads, const gs_gaussians* m, const gs_gaussians* v, const uint32_t* ids,
+                        const uint32_t* n_rows, int64_t max_rows) {
+  if (N < 0 || sh_degree < 0 || sh_degree > 3 || !cfg || !params || !grads || !m || !v || cfg->step < 1 || max_rows < 0 ||
+      max_rows > N || (max_rows > 0 && (!ids || !n_rows)))
+    return GS_E_INVALID;
+  if (max_rows == 0) return GS_OK;
+  const int K3 = 3 * (sh_degree + 1) * (sh_degree + 1);
+  float* P[5] = {params->means, params->scales, params->quats, params->opacities, params->sh};
+  const float* G[5] = {grads->means, grads->scales, grads->quats, grads->opacities, grads->sh};
+  float* M[5] = {m->means, m->scales, m->quats, m->opacities, m->sh};
+  float* V[5] = {v->means, v->scales, v->quats, v->opacities, v->sh};
+  const int width[5] = {3, 3, 4, 1, K3};
+  const float lr[5] = {cfg->lr_means, cfg->lr_scales, cfg->lr_quats, cfg->lr_opacities, cfg->lr_sh};
+  for (int k = 0; k < 5; ++k)
+    if (!P[k] || !G[k] || !M[k] || !V[k]) return GS_E_INVALID;
+  cudaStream_t s = (cudaStream_t)stream;
+  const float ibc1 = (float)(1.0 / (1.0 - pow((double)cfg->beta1, (double)cfg->step)));
+  const float ibc2 = (float)(1.0 / (1.0 - pow((double)cfg->beta2, (double)cfg->step)));
+  for (int k = 0; k < 5; ++k) {
+    const int64_t n = max_rows * width[k];
+    const int grid = grid_for(n);
+#define GS_ADAM(MODE) adam_sparse_kernel<MODE><<<grid, 256, 0, s>>>(n, width[k], P[k], G[k], M[k], V[k], ids, n_rows, lr[k],                                                                    cfg->beta1, cfg->beta2, cfg->eps, ibc1, ibc2)
     if (k == 1) GS_ADAM(kLog); else if (k == 3) GS_ADAM(kLogit); else GS_ADAM(kDirect);
 #undef GS_ADAM
   }

@@ -28,6 +28,21 @@ preprocess_kernel(int64_t N, const float* __restrict__ means, const float* __res
     sc0 = scales[3 * i]; sc1 = scales[3 * i + 1]; sc2 = scales[3 * i + 2];
     o = opacities[i];
     q = *reinterpret_cast<const float4*>(quats + 4 * i);
+    {
+      // The SH row (12 K bytes) is only read if the Gaussian turns out visible, i.e. after the whole fp64 chain: a cheap
+      // fp32 guess (in front of the near plane, centre within the image grown by ~4 sigma_max) starts it on its way to L2
+      // now (measured A/B on one box: preprocess 32.3 -> 31.9 us; the same prefetch in gauss_bwd cost +1.7 us and a
+      // warp-cooperative tile-count loop gained nothing here and cost emit_kernel 4 us: both reverted, profiles/r2_stages.md).
+      const float zc = depth_key_f32(T, mu0, mu1, mu2);
+      const float xc = fmaf(T[0], mu0, fmaf(T[1], mu1, fmaf(T[2], mu2, T[3]))), yc = fmaf(T[4], mu0, fmaf(T[5], mu1, fmaf(T[6], mu2, T[7])));
+      const float iz = 1.f / fmaxf(zc, 1e-6f), m = 4.f * fmaxf(sc0, fmaxf(sc1, sc2)) * fmaxf(cam.fx, cam.fy) * iz + 8.f;
+      const float u = cam.fx * xc * iz + cam.cx, v = cam.fy * yc * iz + cam.cy;
+      if (zc > cam.near_z && u > -m && u < (float)cam.W + m && v > -m && v < (float)cam.H + m) {
+        const char* row = reinterpret_cast<const char*>(sh + (int64_t)3 * K * i);
+#pragma unroll
+        for (int b = 0; b < 12 * K; b += 128) asm volatile("prefetch.global.L2 [%0];" ::"l"(row + b));
+      }
+    }
     vis = project_gaussian<double>(cam, T, mu0, mu1, mu2, sc0, sc1, sc2, q.x, q.y, q.z, q.w, o, P);
     if (vis) vis = tile_rect(cam, P, o, tx0, ty0, tx1, ty1);
     tiles_touched[i] = vis ? (uint32_t)((tx1 - tx0) * (ty1 - ty0)) : 0u;

@@ -88,26 +88,41 @@ __device__ __forceinline__ float eval_power(float u0, float v0, float l11, float
 // Which of the eight 8x4-pixel regions of a 16x16 tile can the ellipse {p2 >= -log2(255)} reach?  Exact up to an
 // outward slack: per band of four pixel rows the ellipse's x-extent over the band is [xl, xr] (a convex set projects
 // to an interval, attained at the band-clamped extreme points), and a region is hit iff the interval meets the
-// region's columns.  (mx, my): mean relative to the tile origin.  ~120 instructions per (Gaussian, tile) instance;
-// the previous per-rectangle maximisation of the quadratic was ~500 and made the duplication kernel issue-bound.
-__device__ __forceinline__ uint32_t region_mask(float l11, float l21, float l22, float lo, float mx, float my) {
-  const float R2 = lo - GS_POWER_MIN + 0.02f;   // outward slack: 0.02 in the exponent, >> the fp32 error of this test
-  if (!(R2 > 0.f)) return 0u;
-  const float R = sqrtf(R2);
-  const float il22 = 1.f / l22, il11 = 1.f / l11;
-  const float hy = R * il22;                                       // half height of the ellipse
-  const float dyR = -l21 * R * rsqrtf(l21 * l21 + l22 * l22) * il22;  // row (relative to the mean) of the rightmost point
-  const float eps = 1e-3f + 1e-6f * fabsf(mx);
+// region's columns.  (mx, my): mean relative to the tile origin.  Square roots and reciprocals are the 1-instruction
+// approximations (2 ulp): the test has 0.02 of slack in the exponent.  ~70 instructions per (Gaussian, tile) instance after a
+// per-Gaussian setup; the previous per-rectangle maximisation of the quadratic was ~500 and made the duplication kernel
+// issue-bound.
+__device__ __forceinline__ float sqrt_approx(float x) {
+  float y;
+  asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+
+// Per-Gaussian part of the region test (the same for every tile of the Gaussian's rectangle).
+struct MaskSetup { float R2, hy, dyR, il11, l21, l22; };
+__device__ __forceinline__ MaskSetup region_mask_setup(float l11, float l21, float l22, float lo) {
+  MaskSetup m;
+  m.R2 = lo - GS_POWER_MIN + 0.02f;   // outward slack: 0.02 in the exponent, >> the error of the approximate ops below
+  const float R = sqrt_approx(fmaxf(m.R2, 0.f)), il22 = rcp_approx(l22);
+  m.hy = R * il22;                                                    // half height of the ellipse
+  m.dyR = -l21 * R * rsqrtf(l21 * l21 + l22 * l22) * il22;            // row (relative to the mean) of the rightmost point
+  m.il11 = rcp_approx(l11); m.l21 = l21; m.l22 = l22;
+  return m;
+}
+
+__device__ __forceinline__ uint32_t region_mask(const MaskSetup& g, float mx, float my) {
+  if (!(g.R2 > 0.f)) return 0u;
+  const float eps = 2e-3f + 2e-6f * fabsf(mx);
   uint32_t m = 0;
 #pragma unroll
   for (int band = 0; band < 4; ++band) {
     const float ya = (float)(4 * band) - my, yb = ya + 3.f;
-    const float lo_y = fmaxf(ya, -hy), hi_y = fminf(yb, hy);
+    const float lo_y = fmaxf(ya, -g.hy), hi_y = fminf(yb, g.hy);
     if (lo_y > hi_y) continue;
-    const float dyr = fminf(fmaxf(dyR, lo_y), hi_y), dyl = fminf(fmaxf(-dyR, lo_y), hi_y);
-    const float vr = l22 * dyr, vl = l22 * dyl;
-    const float sr = sqrtf(fmaxf(R2 - vr * vr, 0.f)), sl = sqrtf(fmaxf(R2 - vl * vl, 0.f));
-    const float xr = mx + (sr - l21 * dyr) * il11 + eps, xl = mx - (sl + l21 * dyl) * il11 - eps;
+    const float dyr = fminf(fmaxf(g.dyR, lo_y), hi_y), dyl = fminf(fmaxf(-g.dyR, lo_y), hi_y);
+    const float vr = g.l22 * dyr, vl = g.l22 * dyl;
+    const float sr = sqrt_approx(fmaxf(g.R2 - vr * vr, 0.f)), sl = sqrt_approx(fmaxf(g.R2 - vl * vl, 0.f));
+    const float xr = mx + (sr - g.l21 * dyr) * g.il11 + eps, xl = mx - (sl + g.l21 * dyl) * g.il11 - eps;
     if (xl <= 7.f && xr >= 0.f) m |= 1u << (2 * band);
     if (xl <= 15.f && xr >= 8.f) m |= 2u << (2 * band);
   }

@@ -83,3 +83,55 @@ def test_prune_and_compaction_bit_exact(N):
         assert np.array_equal(out[k].cpu().numpy(), kept[k]), k
     ix = index.cpu().numpy().view(np.uint32)
     assert np.array_equal(ix[want_keep], np.arange(len(idx), dtype=np.uint32)) and (ix[~want_keep] == 0xFFFFFFFF).all()
+
+
+def test_sparse_gradients_and_sparse_adam(oracle):
+    """GS_SPARSE_GRADS: one gradient row per visible Gaussian, in the order of gs_visible_ids -- against the oracle's dense
+    gradients gathered at those indices; gs_adam_step_sparse on them == gs_adam_step with the visibility mask, bit for bit."""
+    import torch
+    from paper_2605_10760_b200 import binding as b, scenes
+    sc = scenes.replica_scene(seed=39, N=20000, width=300, height=170, f=150.0, sh_degree=2)
+    gC, gD = scenes.upstream_gradients(39, 300, 170)
+    ref = oracle.forward_backward(sc, gC, gD)
+    ctx = b.Context(0)
+    ds = b.DeviceScene(sc)
+    out = ds.alloc_outputs(300, 170)
+    b.forward(ctx, ds, sc.camera, out)
+    nv, _ = ctx.gs_get_counts()
+    for k in ("g_means", "g_scales", "g_quats", "g_opacities", "g_sh"):
+        out[k].fill_(123.0)                       # rows beyond n_visible must stay untouched
+    b.backward(ctx, out, torch.from_numpy(gC).cuda(), torch.from_numpy(gD).cuda(), None, flags=b.GS_SPARSE_GRADS)
+    torch.cuda.synchronize()
+    ids_ptr, n_ptr = ctx.gs_visible_ids()
+    holder = ctx.gs_get_visible_ids()[:nv].clone()
+    ids_h = holder.cpu().numpy().astype(np.int64)
+    assert len(set(ids_h.tolist())) == nv and (ref["visible"][ids_h] == 1).all()
+    for gk, rk in (("g_means", "g_means"), ("g_scales", "g_scales"), ("g_quats", "g_quats"), ("g_opacities", "g_opacities"), ("g_sh", "g_sh")):
+        got = out[gk].cpu().numpy()
+        want = ref[rk][ids_h]
+        rel = np.linalg.norm(got[:nv].astype(np.float64) - want) / np.linalg.norm(want)
+        assert rel <= 1e-3, (gk, rel)
+        assert (got[nv:] == 123.0).all(), gk
+    assert np.linalg.norm(out["g_twist"].cpu().numpy() - ref["g_twist"]) <= 1e-3 * np.linalg.norm(ref["g_twist"])
+    with pytest.raises(b.GsError, match="GS_E_INVALID"):
+        b.backward(ctx, out, torch.from_numpy(gC).cuda(), torch.from_numpy(gD).cuda(), None, flags=b.GS_SPARSE_GRADS | b.GS_ACCUMULATE)
+    # sparse Adam == masked dense Adam, bit for bit
+    keys = ("means", "scales", "quats", "opacities", "sh")
+    pa = dict(means=ds.means.clone(), scales=ds.scales.clone(), quats=ds.quats.clone(), opacities=ds.opacities.clone(), sh=ds.sh.clone())
+    pb = {k: t.clone() for k, t in pa.items()}
+    ma = {k: torch.zeros_like(t) for k, t in pa.items()}; va = {k: torch.zeros_like(t) for k, t in pa.items()}
+    mb = {k: torch.zeros_like(t) for k, t in pa.items()}; vb = {k: torch.zeros_like(t) for k, t in pa.items()}
+    sparse = dict(means=out["g_means"], scales=out["g_scales"], quats=out["g_quats"], opacities=out["g_opacities"], sh=out["g_sh"])
+    dense = {k: torch.zeros_like(t) for k, t in pa.items()}
+    idt = holder.long()
+    for k in keys:
+        dense[k][idt] = sparse[k][:nv]
+    mask = torch.zeros(sc.N, dtype=torch.int32, device="cuda"); mask[idt] = 1
+    lrs = dict(means=1.6e-4, scales=5e-3, quats=1e-3, opacities=5e-2, sh=2.5e-3)
+    b.gs_adam_step_sparse(pa, sparse, ma, va, lrs, 1, ids_ptr, n_ptr, sc.N)
+    b.gs_adam_step(pb, dense, mb, vb, lrs, 1, mask)
+    torch.cuda.synchronize()
+    for k in keys:
+        assert torch.equal(pa[k], pb[k]) and torch.equal(ma[k], mb[k]) and torch.equal(va[k], vb[k]), k
+        assert not torch.equal(pa[k], getattr(ds, k))
+    ctx.close()
