@@ -211,11 +211,12 @@ def replica_throughput(world: int, steps: int, ms_total: float) -> float:
     return world * steps / (ms_total / 1e3)
 
 
-def stage_models(N, K3, V, I, P, tiles, E, C, Eb, R, Rb, pose_only):
+def stage_models(N, K3, V, I, P, tiles, E, C, Eb, R, Rb, pose_only, dense_fill=True):
     """Algorithmic work per launch of every stage: HBM bytes, or FP32 flops + broadcast LDS for the
     two compositing kernels.  V visible Gaussians, I tile instances, P pixels, E / Eb (pixel, Gaussian) pairs evaluated
     by the forward / backward, C blended pairs, R / Rb relevant (region, Gaussian) entries of the forward / backward."""
     gp = 0 if pose_only else (44 + 4 * K3)
+    fill = gp if dense_fill else 0
     return {
         "preprocess": {"bound": "hbm", "bytes": 48 * N + (4 * K3 + 120) * V},
         "tile_scan": {"bound": "hbm", "bytes": 16.0 * tiles, "note": "latency-bound: one L2 round trip between its CTAs"},
@@ -225,11 +226,10 @@ def stage_models(N, K3, V, I, P, tiles, E, C, Eb, R, Rb, pose_only):
                        "bytes": 4 * I + 48 * V + 24 * P},
         "raster_bwd": {"bound": "alu", "flops": Eb * FLOP_EVAL + C * FLOP_BLEND_BWD, "lds": Rb * LDS_PER_ENTRY,
                        "bytes": 4 * I + 48 * V + 28 * P + 48 * V},
-        "gauss_bwd": {"bound": "hbm", "bytes": (48 + 48 + 48 + 16 + 4 + 4 * K3) * V + gp * V,
-                      "note": "its own traffic; the dense zero fill of the culled Gaussians' gradients runs as memsets "
-                              "on a side stream under raster_bwd and is listed as zero_fill"},
+        "gauss_bwd": {"bound": "hbm", "bytes": (48 + 48 + 48 + 16 + 4 + 4 * K3) * V + gp * V + (fill * (N - V) + 4 * N if fill else 0),
+                      "note": "reads g2d, parameters, SH of the V visible Gaussians, writes their gradient rows; dense mode: "
+                              "+ the zero rows of the N - V culled Gaussians, cleared by the same kernel"},
         "pose_grad": {"bound": "hbm", "bytes": 120.0, "note": "latency-bound: one thread"},
-        "zero_fill": {"bound": "hbm", "bytes": gp * N, "note": "cudaMemsetAsync on the side stream, overlapped"},
     }
 
 
@@ -270,6 +270,9 @@ def run_ours(args):
             ups.append([tuple(to_dev(a) for a in scenes.upstream_gradients(wl.up_seeds[k] + v, W, H))
                         for v in range(wl.views)])
 
+    # --grads sparse: GS_SPARSE_GRADS (one gradient row per visible Gaussian, no dense zero fill); single-view workloads
+    grad_flag = B.GS_SPARSE_GRADS if (args.grads == "sparse" and wl.views == 1) else 0
+
     def step(k):
         s = k % len(dss)
         if wl.pose_only:
@@ -282,7 +285,7 @@ def run_ours(args):
             return
         for v, cam in enumerate(wl.cams[s]):
             B.forward(ctx, dss[s], cam, out)
-            B.backward(ctx, out, ups[s][v][0], ups[s][v][1], None, flags=(B.GS_ACCUMULATE if v > 0 else 0), pose=True)
+            B.backward(ctx, out, ups[s][v][0], ups[s][v][1], None, flags=(B.GS_ACCUMULATE if v > 0 else grad_flag), pose=True)
 
     def barrier():
         torch.cuda.synchronize()
@@ -351,7 +354,8 @@ def run_ours(args):
     P, tiles = W * H, ((W + 15) // 16) * ((H + 15) // 16)
     V, I = mean("visible"), mean("instances")
     models = stage_models(N, K3, V, I, P, tiles, mean("evaluated"), mean("blended"), mean("evaluated_bwd"),
-                          mean("region_entries"), mean("region_entries_bwd"), wl.pose_only)
+                          mean("region_entries"), mean("region_entries_bwd"), wl.pose_only,
+                          dense_fill=(grad_flag == 0 and wl.views == 1))
     roof_stages = {}
     for s in B.STAGES:
         m, t = models[s], stage_ms[s] * 1e-3
@@ -368,7 +372,6 @@ def run_ours(args):
         if "note" in m:
             e["note"] = m["note"]
         roof_stages[s] = e
-    roof_stages["zero_fill"] = {"bound": "hbm", "bytes": models["zero_fill"]["bytes"], "note": models["zero_fill"]["note"]}
     dominant = max(stage_ms, key=stage_ms.get)
     kernel_name = {"raster_fwd": "raster_fwd_kernel", "raster_bwd": "raster_bwd_kernel"}.get(dominant, dominant + "_kernel")
     d = roof_stages[dominant]
@@ -403,7 +406,7 @@ def run_ours(args):
                 "value": value, "unit": "iter/s", "n_gpus": world, "steps": K, "warmup": warm,
                 "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f32", "data": "synthetic", "config": config_dict(wl, world),
-                "views_per_iter": wl.views, "mpix_iter_per_s": value * wl.views * W * H / 1e6,
+                "views_per_iter": wl.views, "grads": "sparse" if grad_flag else "dense", "mpix_iter_per_s": value * wl.views * W * H / 1e6,
                 "clocks": clk.summary(), "e2e": e2e, "gpu_launches": launches, "roofline": roof,
                 "roofline_stages": roof_stages, "cpu_baseline": cpu,
                 "hbm_frac_whole_iteration": hbm_frac_iter, "algorithmic_bytes_per_iter": bytes_iter,
@@ -535,6 +538,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="replica300k")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--grads", default="dense", choices=["dense", "sparse"],
+                    help="dense (default, the headline): (11 + 3K) N gradient arrays; sparse: GS_SPARSE_GRADS rows of the visible Gaussians")
     args = ap.parse_args()
     if args.workload == "fused2m" and args.steps == 2000:
         args.steps = 50   # 8 views per step: the default still finishes within a minute

@@ -164,8 +164,6 @@ int gs_create(gs_ctx** out, int device) {
   ok = ok && alloc_header(ctx, 0) == GS_OK;
   ok = ok && cudaHostAlloc((void**)&ctx->mailbox, sizeof(Counts), cudaHostAllocMapped) == cudaSuccess;
   ok = ok && cudaStreamCreateWithFlags(&ctx->side_stream, cudaStreamNonBlocking) == cudaSuccess;
-  ok = ok && cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming) == cudaSuccess;
-  ok = ok && cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming) == cudaSuccess;
   ok = ok && cudaEventCreateWithFlags(&ctx->ev_fork2, cudaEventDisableTiming) == cudaSuccess;
   ok = ok && cudaEventCreateWithFlags(&ctx->ev_join2, cudaEventDisableTiming) == cudaSuccess;
   if (ok) {
@@ -190,8 +188,6 @@ int gs_destroy(gs_ctx* ctx) {
   cudaFree(ctx->hb); cudaFree(ctx->stats_ws); cudaFree(ctx->rv);
   if (ctx->mailbox) cudaFreeHost(ctx->mailbox);
   if (ctx->side_stream) cudaStreamDestroy(ctx->side_stream);
-  if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
-  if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
   if (ctx->ev_fork2) cudaEventDestroy(ctx->ev_fork2);
   if (ctx->ev_join2) cudaEventDestroy(ctx->ev_join2);
   if (ctx->ev_made) for (int k = 0; k < 13; ++k) cudaEventDestroy(ctx->ev[k]);
@@ -310,20 +306,8 @@ int gs_rasterize_bwd(gs_ctx* ctx, void* stream, const float* d_rgb, const float*
   ctx->g2d_dirty = true;
   ctx->pose_acc_valid = false;
   GS_PROF(8, s);
-  int rc;
-  const bool fork = write && !(flags & (GS_ACCUMULATE | GS_SPARSE_GRADS)) && ctx->N > 0 && ctx->side_stream;
-  if (fork) {  // zero fill of the dense gradient arrays on the side stream, overlapping the pixel backward
-    GS_CUDA(cudaEventRecord(ctx->ev_fork, s));
-    GS_CUDA(cudaStreamWaitEvent(ctx->side_stream, ctx->ev_fork, 0));
-    if ((rc = launch_zero_fill(ctx, ctx->side_stream, g_means, g_scales, g_quats, g_opacities, g_sh)) != GS_OK) return rc;
-    GS_CUDA(cudaEventRecord(ctx->ev_join, ctx->side_stream));
-  }
-  rc = launch_raster_bwd(ctx, s, d_rgb, d_depth, d_alpha);
+  int rc = launch_raster_bwd(ctx, s, d_rgb, d_depth, d_alpha);
   if (rc != GS_OK) return rc;
-  if (fork) {
-    GS_CUDA(cudaStreamWaitEvent(s, ctx->ev_join, 0));
-    ctx->zero_filled = true;
-  }
   GS_PROF(9, s);
   if (write) {
     if ((rc = launch_gauss_bwd(ctx, s, flags, g_means, g_scales, g_quats, g_opacities, g_sh)) != GS_OK) return rc;

@@ -25,18 +25,57 @@ gauss_bwd_kernel(int64_t N, const float* __restrict__ means, const float* __rest
                  const float* __restrict__ quats, const float* __restrict__ opacities, const float* __restrict__ sh,
                  DevCam cam, const uint32_t* __restrict__ vis_ids, const float4* __restrict__ vis_par,
                  const float4* __restrict__ feat, const Counts* __restrict__ counts,
-                 float* __restrict__ g2d, bool accumulate, bool sparse,
+                 const uint32_t* __restrict__ tiles_touched, float* __restrict__ g2d, bool accumulate, bool sparse, bool fill,
                  float* __restrict__ g_means, float* __restrict__ g_scales, float* __restrict__ g_quats,
                  float* __restrict__ g_opac, float* __restrict__ g_sh, double* __restrict__ pose_acc) {
   constexpr int K = (DEG + 1) * (DEG + 1);
   // one thread per VISIBLE Gaussian (compacted list of gs_preprocess); culled Gaussians were zero-filled by memset
   const int64_t kk = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const uint32_t V = counts->n_visible;
+  if (WRITE && fill) {
+    // Dense outputs: exact zeros for the culled Gaussians.  Block b clears the culled rows among the Gaussians
+    // [128 b, 128 b + 128) -- N - V rows in total instead of a memset of all N (the five cudaMemsetAsync on a side stream
+    // cost raster_bwd 23 us of the SMs they ran on, profiles/r2_stages.md); the rows of the visible Gaussians are written
+    // below by the blocks that own their visible slots.  Rows are cleared by consecutive threads in 16-byte pieces.
+    __shared__ uint32_t s_rows[128];
+    __shared__ uint32_t s_wcnt[4];
+    const bool culled = kk < N && tiles_touched[kk] == 0u;
+    const unsigned bal = __ballot_sync(0xffffffffu, culled);
+    const int wl = threadIdx.x >> 5, ln = threadIdx.x & 31;
+    if (ln == 0) s_wcnt[wl] = __popc(bal);
+    __syncthreads();
+    uint32_t before = 0, cnt = 0;
+#pragma unroll
+    for (int w = 0; w < 4; ++w) { before += w < wl ? s_wcnt[w] : 0u; cnt += s_wcnt[w]; }
+    if (culled) s_rows[before + __popc(bal & ((1u << ln) - 1u))] = (uint32_t)kk;
+    __syncthreads();
+    const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
+    if constexpr ((3 * K) % 4 == 0) {
+      constexpr int Q = 3 * K / 4;  // float4 per SH row
+      for (uint32_t t = threadIdx.x; t < cnt * Q; t += blockDim.x) {
+        const uint32_t r = t / Q, c = t - r * Q;
+        reinterpret_cast<float4*>(g_sh + (int64_t)3 * K * s_rows[r])[c] = z4;
+      }
+    } else {
+      for (uint32_t t = threadIdx.x; t < cnt * (3 * K); t += blockDim.x) {
+        const uint32_t r = t / (3 * K), c = t - r * (3 * K);
+        g_sh[(int64_t)3 * K * s_rows[r] + c] = 0.f;
+      }
+    }
+    for (uint32_t t = threadIdx.x; t < cnt * 3; t += blockDim.x) {
+      const uint32_t r = t / 3, c = t - r * 3;
+      g_means[(int64_t)3 * s_rows[r] + c] = 0.f;
+      g_scales[(int64_t)3 * s_rows[r] + c] = 0.f;
+    }
+    for (uint32_t t = threadIdx.x; t < cnt; t += blockDim.x) {
+      reinterpret_cast<float4*>(g_quats)[s_rows[t]] = z4;
+      g_opac[s_rows[t]] = 0.f;
+    }
+  }
   if ((int64_t)blockIdx.x * blockDim.x >= (int64_t)V) return;
   const bool vis = kk < (int64_t)V;
   const int64_t i = vis ? (int64_t)vis_ids[kk] : 0;
   const int64_t orow = sparse ? kk : i;  // output row: GS_SPARSE_GRADS writes one row per VISIBLE Gaussian, in slot order
-  (void)N;
   float T[12];
   load_pose(cam, T);
   R acc[15];
@@ -256,16 +295,12 @@ int launch_gauss_bwd(gs_ctx* ctx, cudaStream_t s, uint32_t flags, float* g_means
   const bool write = !(flags & GS_POSE_ONLY);
   const bool accum = (flags & GS_ACCUMULATE) != 0;
   const bool sparse = (flags & GS_SPARSE_GRADS) != 0;
-  if (write && !accum && !sparse && !ctx->zero_filled) {
-    int rc = launch_zero_fill(ctx, s, g_means, g_scales, g_quats, g_opac, g_sh);
-    if (rc != GS_OK) return rc;
-  }
-  ctx->zero_filled = false;
+  const bool fill = write && !accum && !sparse;  // dense outputs: the kernel clears the rows of the culled Gaussians itself
   const int threads = 128;
   const unsigned blocks = (unsigned)div_up(ctx->N, threads);
 #define GS_GB(D, Wr)                                                                                                 \
   gauss_bwd_kernel<D, Wr><<<blocks, threads, 0, s>>>(ctx->N, ctx->means, ctx->scales, ctx->quats, ctx->opacities,   \
-                                                      ctx->sh, ctx->cam, ctx->vis_ids, ctx->vis_par, ctx->feat, ctx->counts, ctx->g2d, accum, sparse, \
+                                                      ctx->sh, ctx->cam, ctx->vis_ids, ctx->vis_par, ctx->feat, ctx->counts, ctx->tiles_touched, ctx->g2d, accum, sparse, fill, \
                                                       g_means, g_scales, g_quats, g_opac, g_sh, ctx->pose_acc)
   if (write) {
     switch (ctx->sh_degree) {
@@ -284,19 +319,6 @@ int launch_gauss_bwd(gs_ctx* ctx, cudaStream_t s, uint32_t flags, float* g_means
   }
 #undef GS_GB
   GS_LAUNCH_CHECK("gauss_bwd_kernel");
-  return GS_OK;
-}
-
-// Dense outputs: exact zeros for the culled Gaussians (the visible ones are overwritten by gauss_bwd_kernel).
-int launch_zero_fill(gs_ctx* ctx, cudaStream_t s, float* g_means, float* g_scales, float* g_quats, float* g_opac,
-                     float* g_sh) {
-  const size_t f = sizeof(float), Nn = (size_t)ctx->N, K3 = 3 * (size_t)(ctx->sh_degree + 1) * (ctx->sh_degree + 1);
-  if (Nn == 0) return GS_OK;
-  GS_CUDA(cudaMemsetAsync(g_sh, 0, Nn * K3 * f, s));
-  GS_CUDA(cudaMemsetAsync(g_means, 0, Nn * 3 * f, s));
-  GS_CUDA(cudaMemsetAsync(g_scales, 0, Nn * 3 * f, s));
-  GS_CUDA(cudaMemsetAsync(g_quats, 0, Nn * 4 * f, s));
-  GS_CUDA(cudaMemsetAsync(g_opac, 0, Nn * f, s));
   return GS_OK;
 }
 

@@ -129,10 +129,9 @@ struct gs_ctx {
   uint32_t* tile_order = nullptr;      // [tiles] tile ids by descending list length (longest lists are scheduled first)
   bool opt_exact_cull = false;         // GS_OPT_EXACT_TILE_CULL (gs_set_option)
 
-  // side stream: the zero fill of the dense gradient arrays overlaps the (ALU-bound) pixel backward
+  // side stream: the block-wide sort of the few long tile lists runs beside the warp-level sort of the rest
   cudaStream_t side_stream = nullptr;
-  cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_fork2 = nullptr, ev_join2 = nullptr;
-  bool zero_filled = false;  // set by gs_rasterize_bwd when the fill was issued on the side stream
+  cudaEvent_t ev_fork2 = nullptr, ev_join2 = nullptr;
 
   // stage timing (gs_profile_*): events recorded around the kernel groups when enabled
   bool prof_on = false;
@@ -220,7 +219,6 @@ int launch_raster_fwd(gs_ctx* ctx, cudaStream_t s, float* rgb, float* depth, flo
 int launch_raster_bwd(gs_ctx* ctx, cudaStream_t s, const float* d_rgb, const float* d_depth, const float* d_alpha);
 int launch_gauss_bwd(gs_ctx* ctx, cudaStream_t s, uint32_t flags, float* g_means, float* g_scales, float* g_quats,
                      float* g_opac, float* g_sh);
-int launch_zero_fill(gs_ctx* ctx, cudaStream_t s, float* g_means, float* g_scales, float* g_quats, float* g_opac, float* g_sh);
 int launch_pose_final(gs_ctx* ctx, cudaStream_t s, uint32_t flags, float* g_twist);
 int ensure_instance_capacity(gs_ctx* ctx, int64_t need);
 int handle_overflow(gs_ctx* ctx);

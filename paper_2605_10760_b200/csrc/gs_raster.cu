@@ -22,7 +22,7 @@
 namespace gs {
 
 // NW: warps (= regions) per CTA.  8: one CTA per tile; 4 / 2: half / quarter tiles -- the list is then staged 2 / 4 times
-// per tile, but fewer warps wait for each other at the per-round barrier (profiles/r2_v7_tile_cta.md).
+// per tile (profiles/r2_v7_tile_cta.md, r2_v9_ring.md).
 #ifndef GS_FWD_WARPS
 #define GS_FWD_WARPS 4
 #endif
@@ -36,11 +36,12 @@ raster_fwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
                   float bg0, float bg1, float bg2, float* __restrict__ rgb, float* __restrict__ depth,
                   float* __restrict__ alpha_out, float* __restrict__ final_T, uint32_t* __restrict__ n_contrib,
                   unsigned long long* __restrict__ stats) {
-  static_assert(NW == 2 || NW == 4 || NW == 8, "64 producer threads are needed");
   constexpr int CPT = 8 / NW;  // CTAs per tile
-  __shared__ StageBuf s_st[kStages];
+  constexpr int TPE = Ring<NW>::TPE;
+  __shared__ __align__(16) Ring<NW> ring;
   // per warp: byte offsets (into the stage) of the round's relevant entries, in list order
   __shared__ __align__(8) uint16_t s_idx[NW][kTileBatch + kGroup];
+  __shared__ int s_live;  // warps of the CTA that still have a live pixel: staging stops when it reaches zero
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int tile = (int)__ldg(order + blockIdx.x / CPT), sub = (blockIdx.x % CPT) * NW + warp;
   const int tx0 = (tile % tiles_x) * GS_TILE, ty0 = (tile / tiles_x) * GS_TILE;
@@ -56,91 +57,94 @@ raster_fwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
   unsigned long long n_eval = 0, n_blend = 0;
   uint32_t rank = 0, last_rank = 0;   // STATS: relevant entries walked so far; rank of the pixel's last blended one
 
-  if (tid < kStages) {  // padding records never pass: lo = -inf  =>  p2 = -inf
-    StageRec& pr = s_st[tid].rec[kPadIdx];
-    pr.g = make_float4(0.f, 0.f, 0.f, -INFINITY);
-    pr.c = make_float4(0.f, 0.f, 0.f, 0.f);
-    pr.uv = make_float2(0.f, 0.f);
-  }
-  // producer: thread t < 64 stages list entry 64 j + t of round j (the list entry itself is fetched one round earlier)
-  uint32_t v_pre = 0;
-  int i_pre = tid;  // list index of the entry this thread fetches next
-  auto prefetch = [&]() {
-    v_pre = (tid < kTileBatch && i_pre < n) ? __ldg(ids + range.x + i_pre) : 0u;
-  };
-  int i_pro = tid, st_pro = 0;
-  auto produce = [&]() {
-    if (tid < kTileBatch) {
-      StageRec& r = s_st[st_pro].rec[tid];
-      r.ent = v_pre;
-      if (i_pro < n) {
-        const float4* src = feat + 3 * (size_t)(v_pre >> 8) + 1;
-        cp_async16(&r.g, src);
-        cp_async16(&r.c, src + 1);
-        cp_async8(&r.uv, inst_uv + range.x + i_pro);
-      }
-    }
-    cp_async_commit();
-    i_pro += kTileBatch;
-    st_pro = st_pro + 1 == kStages ? 0 : st_pro + 1;
-  };
-  prefetch(); i_pre += kTileBatch; produce();
-  prefetch(); i_pre += kTileBatch; produce();
-  prefetch(); i_pre += kTileBatch;
   bool alive_warp = __any_sync(kFull, inside);
-  int st_con = 0;
+  ring.init(tid);
+  if (tid == 0) s_live = 0;
+  __syncthreads();
+  if (lane == 0 && alive_warp) atomicAdd(&s_live, 1);
+  // producer state: this thread stages entry e_pro of every round; the list word is fetched one step ahead
+  const int e_pro = tid / TPE;
+  uint32_t v_pre = 0;
+  auto fetch = [&](int k) {
+    const int i = k * kTileBatch + e_pro;
+    v_pre = i < n ? __ldg(ids + range.x + i) : 0u;
+  };
+  fetch(0);
+#pragma unroll
+  for (int k = 0; k < kAhead; ++k) {
+    if (k < nb) ring.produce(k, k * kTileBatch + e_pro, n, range.x, v_pre, tid, ids, inst_uv, feat);
+    fetch(k + 1);
+  }
+  __syncthreads();  // s_live is complete
+  const volatile int* live = &s_live;
   uint32_t base48 = 48u;  // 48 x (list position + 1) of entry 0 of the round
   for (int j = 0; j < nb; ++j, base48 += 48u * kTileBatch) {
-    cp_async_wait<1>();  // this thread's copies of round j have landed ...
-    // ... and after the barrier everybody's have; every warp has also finished round j - 1, whose stage is refilled next
-    if (!__syncthreads_or(alive_warp)) break;
-    produce();
-    prefetch(); i_pre += kTileBatch;
-    const StageBuf& sb = s_st[st_con];
-    st_con = st_con + 1 == kStages ? 0 : st_con + 1;
-    if (!alive_warp) continue;
-    // the entries of this round that can reach this warp's region, as a list of byte offsets in list order
-    const bool r0 = (sb.rec[lane].ent >> sub) & 1u, r1 = (sb.rec[lane + 32].ent >> sub) & 1u;
-    const unsigned b0 = __ballot_sync(kFull, r0), b1 = __ballot_sync(kFull, r1);
-    const int n0 = __popc(b0), nrel = n0 + __popc(b1);
-    if (nrel == 0) continue;
-    const unsigned lt = (1u << lane) - 1u;
-    uint16_t* idx = s_idx[warp];
-    if (r0) idx[__popc(b0 & lt)] = (uint16_t)(lane * 48);
-    if (r1) idx[n0 + __popc(b1 & lt)] = (uint16_t)((32 + lane) * 48);
-    if (lane < kGroup) idx[nrel + lane] = (uint16_t)(kPadIdx * 48);
-    __syncwarp();
-    const char* recs = reinterpret_cast<const char*>(sb.rec);
-    for (int r = 0; r < nrel; r += kGroup) {
-      const uint2 o4 = *reinterpret_cast<const uint2*>(idx + r);
-      const uint32_t off[kGroup] = {o4.x & 0xffffu, o4.x >> 16, o4.y & 0xffffu, o4.y >> 16};
+    const int stage = j & (kStages - 1);
+    if (alive_warp) {
+      mbar_wait(&ring.full[stage], (uint32_t)(j / kStages) & 1u);
+      const StageBuf& sb = ring.st[stage];
+      // the entries of this round that can reach this warp's region, as a list of byte offsets in list order
+      const int left = n - j * kTileBatch;  // entries of the round that exist (what lies beyond is stale)
+      const bool r0 = ((sb.rec[lane].ent >> sub) & 1u) && lane < left, r1 = ((sb.rec[lane + 32].ent >> sub) & 1u) && lane + 32 < left;
+      const unsigned b0 = __ballot_sync(kFull, r0), b1 = __ballot_sync(kFull, r1);
+      const int n0 = __popc(b0), nrel = n0 + __popc(b1);
+      if (nrel) {
+        const unsigned lt = (1u << lane) - 1u;
+        uint16_t* idx = s_idx[warp];
+        if (r0) idx[__popc(b0 & lt)] = (uint16_t)(lane * 48);
+        if (r1) idx[n0 + __popc(b1 & lt)] = (uint16_t)((32 + lane) * 48);
+        if (lane < kGroup) idx[nrel + lane] = (uint16_t)(kPadIdx * 48);
+        __syncwarp();
+        const char* recs = reinterpret_cast<const char*>(sb.rec);
+        for (int r = 0; r < nrel; r += kGroup) {
+          const uint2 o4 = *reinterpret_cast<const uint2*>(idx + r);
+          const uint32_t off[kGroup] = {o4.x & 0xffffu, o4.x >> 16, o4.y & 0xffffu, o4.y >> 16};
 #pragma unroll
-      for (int q = 0; q < kGroup; ++q) {
-        const StageRec& e = *reinterpret_cast<const StageRec*>(recs + off[q]);
-        const float4 a0 = e.g, f2 = e.c;
-        const float2 uv = e.uv;
-        const float p = eval_power(uv.x, uv.y, a0.x, a0.y, a0.z, a0.w, fx0, fy0);
-        const bool alive = T >= GS_T_MIN;
-        const bool hit = (p >= GS_POWER_MIN) && alive;   // alpha >= 1/255 and the pixel has not terminated
-        const float a = hit ? fminf(GS_ALPHA_MAX, ex2_approx(p)) : 0.f;
-        const float w = a * T;
-        C0 = fmaf(f2.x, w, C0);
-        C1 = fmaf(f2.y, w, C1);
-        C2 = fmaf(f2.z, w, C2);
-        D = fmaf(f2.w, w, D);
-        T = fmaf(-a, T, T);
-        last48 = hit ? base48 + off[q] : last48;
-        if (STATS && r + q < nrel) {
-          ++rank;
-          n_eval += alive ? 1 : 0;
-          n_blend += hit ? 1 : 0;
-          last_rank = hit ? rank : last_rank;
+          for (int q = 0; q < kGroup; ++q) {
+            const StageRec& e = *reinterpret_cast<const StageRec*>(recs + off[q]);
+            const float4 a0 = e.g, f2 = e.c;
+            const float2 uv = e.uv;
+            const float p = eval_power(uv.x, uv.y, a0.x, a0.y, a0.z, a0.w, fx0, fy0);
+            const bool alive = T >= GS_T_MIN;
+            const bool hit = (p >= GS_POWER_MIN) && alive;   // alpha >= 1/255 and the pixel has not terminated
+            const float a = hit ? fminf(GS_ALPHA_MAX, ex2_approx(p)) : 0.f;
+            const float w = a * T;
+            C0 = fmaf(f2.x, w, C0);
+            C1 = fmaf(f2.y, w, C1);
+            C2 = fmaf(f2.z, w, C2);
+            D = fmaf(f2.w, w, D);
+            T = fmaf(-a, T, T);
+            last48 = hit ? base48 + off[q] : last48;
+            if (STATS && r + q < nrel) {
+              ++rank;
+              n_eval += alive ? 1 : 0;
+              n_blend += hit ? 1 : 0;
+              last_rank = hit ? rank : last_rank;
+            }
+          }
+          if (!__any_sync(kFull, T >= GS_T_MIN)) { alive_warp = false; break; }
         }
+        if (!alive_warp && lane == 0) atomicSub(&s_live, 1);
       }
-      if (!__any_sync(kFull, T >= GS_T_MIN)) { alive_warp = false; break; }
     }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&ring.empty[stage]);  // this warp is done with the stage (a dead warp: at once)
+    // refill: the stage of round j - kDelay takes round j + kAhead once every warp has released it
+    const int k = j + kAhead;
+    if (k < nb) {
+      bool stop = false;
+      if (j >= kDelay) {
+        const uint32_t par = (uint32_t)((j - kDelay) / kStages) & 1u;
+        while (!mbar_try_wait(&ring.empty[k & (kStages - 1)], par))
+          if (*live == 0) { stop = true; break; }   // the warps this one waits for have left
+      }
+      if (stop) break;
+      ring.produce(k, k * kTileBatch + e_pro, n, range.x, v_pre, tid, ids, inst_uv, feat);
+      fetch(k + 1);
+    }
+    if (*live == 0) break;  // no pixel of the CTA is alive any more
   }
-  cp_async_wait<0>();
+  cp_async_wait_all();
   const uint32_t last = last48 / 48u;
   if (STATS) {
     // gs.h gs_get_workload: E, C, L, list length x pixels, R (forward), Eb, Rb (what the backward must walk: the

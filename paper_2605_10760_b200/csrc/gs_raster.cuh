@@ -18,7 +18,18 @@ namespace gs {
 constexpr unsigned kFull = 0xffffffffu;
 constexpr int kGroup = 4;        // relevant entries evaluated together in the pixel loop
 constexpr int kTileBatch = 64;   // list entries staged per round by a CTA
-constexpr int kStages = 3;       // staging ring depth
+#ifndef GS_RING_STAGES
+#define GS_RING_STAGES 4
+#endif
+#ifndef GS_RING_DELAY
+#define GS_RING_DELAY 2
+#endif
+constexpr int kStages = GS_RING_STAGES;  // staging ring depth (power of two)
+// A warp that has finished round j refills the stage of round j - kDelay (with round j - kDelay + kStages): the warps of a
+// CTA may be up to kDelay + 1 rounds apart before one waits for another, and kStages - kDelay rounds are in flight.
+constexpr int kDelay = GS_RING_DELAY;
+constexpr int kAhead = kStages - kDelay;
+static_assert((kStages & (kStages - 1)) == 0 && kDelay >= 0 && kAhead >= 2, "ring shape");
 constexpr int kPadIdx = kTileBatch;  // index of the stage's padding record (never passes: lo = -inf)
 
 // One staged list entry (48 B): what the pixel loops read as broadcast LDS.128 x 2 + LDS.64.
@@ -58,11 +69,75 @@ __device__ __forceinline__ void cp_async8(void* smem_dst, const void* gmem_src) 
   const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gmem_src) : "memory");
 }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() {
-  asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
+__device__ __forceinline__ void cp_async4(void* smem_dst, const void* gmem_src) {
+  const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(gmem_src) : "memory");
 }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+// mbarrier (shared::cta) helpers of the staging ring.  full[s]: every thread of the CTA arrives through
+// cp.async.mbarrier.arrive.noinc, i.e. when ITS cp.async copies into stage s have landed (count = threads of the CTA);
+// empty[s]: one arrival per warp that has finished reading stage s (count = warps of the CTA).
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("{\n.reg .b64 st;\nmbarrier.arrive.shared::cta.b64 st, [%0];\n}" ::"r"((uint32_t)__cvta_generic_to_shared(bar)) : "memory");
+}
+__device__ __forceinline__ void cp_async_mbar_arrive(uint64_t* bar) {
+  asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"((uint32_t)__cvta_generic_to_shared(bar)) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
+               : "=r"(ok) : "r"((uint32_t)__cvta_generic_to_shared(bar)), "r"(parity) : "memory");
+  return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  while (!mbar_try_wait(bar, parity)) {}
+}
+
+// The staging ring shared by the forward and the backward kernels.  Every thread of the CTA is a producer: entry e of a
+// round is staged by T / 64 consecutive threads (record halves g, c by 16-byte cp.async, the instance's (u0, v0) by an
+// 8-byte and its list word by a 4-byte cp.async), each of which then lets full[stage] count its copies
+// (cp.async.mbarrier.arrive.noinc).  Consumers (the same warps) wait on full[stage] and release the stage through
+// empty[stage]; there is NO block-wide barrier in the loop: warps of different regions, which find different numbers of
+// relevant entries per round, drift up to kDelay + 1 rounds apart (the per-round __syncthreads of v7 held 19-25 % of the
+// stall samples of both kernels).
+template <int NW>
+struct Ring {
+  static constexpr int T = NW * 32, TPE = T / kTileBatch;  // threads per staged entry: 1, 2 or 4
+  static_assert(TPE == 1 || TPE == 2 || TPE == 4, "2, 4 or 8 warps");
+  StageBuf st[kStages];
+  uint64_t full[kStages], empty[kStages];
+
+  __device__ __forceinline__ void init(int tid) {
+    if (tid < kStages) {  // padding records never pass: lo = -inf  =>  p2 = -inf
+      StageRec& pr = st[tid].rec[kPadIdx];
+      pr.g = make_float4(0.f, 0.f, 0.f, -INFINITY);
+      pr.c = make_float4(0.f, 0.f, 0.f, 0.f);
+      pr.uv = make_float2(0.f, 0.f);
+      pr.ent = 0u;
+      mbar_init(&full[tid], T);
+      mbar_init(&empty[tid], NW);
+    }
+  }
+  // stages list entry i (valid if i < n) of the tile whose list starts at `first`, for staged round k; v = ids[first + i]
+  __device__ __forceinline__ void produce(int k, int i, int n, uint32_t first, uint32_t v, int tid,
+                                          const uint32_t* __restrict__ ids, const float2* __restrict__ inst_uv,
+                                          const float4* __restrict__ feat) {
+    const int stage = k & (kStages - 1), part = tid & (TPE - 1);
+    StageRec& r = st[stage].rec[tid / TPE];
+    if (i >= 0 && i < n) {
+      const float4* src = feat + 3 * (size_t)(v >> 8) + 1;
+      if (part == 0) cp_async16(&r.g, src);
+      if (part == (1 & (TPE - 1))) cp_async16(&r.c, src + 1);
+      if (part == (2 & (TPE - 1))) cp_async8(&r.uv, inst_uv + first + i);
+      if (part == (3 & (TPE - 1))) cp_async4(&r.ent, ids + first + i);
+    }
+    cp_async_mbar_arrive(&full[stage]);
+  }
+};
 
 // Feature record -> whitened offset relative to the origin (ox, oy), in fp64 (exact integer part of the mean, exact
 // products with the fp32-rounded L; one rounding of u0, v0 at the end).  Also returns the origin-relative mean (fp32).

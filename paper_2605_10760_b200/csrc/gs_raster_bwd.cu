@@ -28,66 +28,77 @@ constexpr int kSlots = 16;     // Gaussians per flush of the Gaussian phase
 constexpr int kPairRow = 33;   // float2 per slot row (32 pixels + 1: conflict-free transposed LDS.64)
 constexpr int kOutVals = 10;   // sums per Gaussian (gs_internal.cuh kG2D, first 10)
 
-// Record of the Gaussian in slot (lane & 15), kept in registers between the pixel phase and the flush: the whitened
-// offset of the tile origin and the visible slot; L is re-read from the feature record at the flush (one LDG.128 per
-// lane per 16 Gaussians) instead of being carried in three more registers (80 registers is the occupancy limit here).
-struct SlotRec { float u0, v0; };
+// Record of the Gaussian in slot s, parked in shared memory by lane 0 of the pixel phase (one STS.128; up to round-2 v8
+// the records were kept in registers of lane s through selects: 9 instructions per entry and 10 % of the stall samples,
+// profiles/r2_v9_ring.md): the tile-local whitened offset of the instance and its list word (visible slot << 8 | mask).
+// L is re-read from the feature record at the flush (one LDG.128 per lane per 16 Gaussians).
+struct __align__(16) SlotRec { float u0, v0; uint32_t ent, pad; };
 
 // Gaussian phase.  SPLIT = 2: lane = (slot = lane & 15, half = lane >> 4), 2 pixel rows per lane;
 //                  SPLIT = 4: lane = (slot = lane & 7, quarter = lane >> 3), 1 pixel row per lane (tail flush, <= 8 slots).
 // (xo, yo): tile-local coordinates of the region's first pixel.
+// The moments of gp are accumulated in the REGION-CENTRED PIXEL coordinates (x, y) = (c - 3.5, row - 1.5): per pixel that
+// is three operations with immediates (sum gp, sum gp x, sum gp x^2 per row; y enters once per row) instead of nine on
+// per-Gaussian whitened offsets, and the six raw moments are mapped to the whitened frame once per Gaussian:
+//   u = l11 x + l21 y + uc,  v = l22 y + vc     (uc, vc: whitened offset of the region's centre)
+// |l| <= sqrt(0.5 log2(e) / 0.3) = 1.55 (the 0.3-pixel dilation bounds the conic) and |u|, |v| <= 2.9 wherever gp != 0, so
+// |uc|, |vc| <= ~11 and the expansion of sum gp u^2 cancels at most ~1e2 x: 1e-5 relative, against the 1e-3 gradient bound.
 template <int SPLIT>
-__device__ __forceinline__ void gaussian_phase(float2* s_pair, const float4* s_pix, int nslot, int lane, const SlotRec& sr,
-                                               uint32_t slot_id, float xo, float yo, const float4* __restrict__ feat,
+__device__ __forceinline__ void gaussian_phase(float2* s_pair, const float4* s_pix, const SlotRec* s_slot, int nslot,
+                                               int lane, float xo, float yo, const float4* __restrict__ feat,
                                                float* __restrict__ g2d) {
   constexpr int LS = 32 / SPLIT, R = 4 / SPLIT;  // slots per pass, pixel rows per lane
   __syncwarp();
   const int slot = lane & (LS - 1), part = lane / LS;
-  // the slot records live in registers: lane s (and lane s + 16) holds the record of slot s
-  float u0 = sr.u0, v0 = sr.v0;
-  uint32_t id = slot_id;
-  if (SPLIT == 4) {
-    u0 = __shfl_sync(kFull, sr.u0, slot); v0 = __shfl_sync(kFull, sr.v0, slot);
-    id = __shfl_sync(kFull, slot_id, slot);
-  }
+  const SlotRec sr = s_slot[slot];
+  const uint32_t id = sr.ent >> 8;
   float4 L = make_float4(0.f, 0.f, 0.f, 0.f);
   if (slot < nslot) L = __ldg(feat + 3 * (size_t)id + 1);  // l11, l21, l22
-  float ub[R], vs[R];
-#pragma unroll
-  for (int r = 0; r < R; ++r) {
-    const float y = yo + (float)(part * R + r);
-    ub[r] = fmaf(L.y, y, fmaf(L.x, xo, u0));
-    vs[r] = fmaf(L.z, y, v0);
-  }
   const float2* pr = s_pair + slot * kPairRow + part * (R * 8);
   const float4* px = s_pix + part * (R * 8);
-  float acc[kOutVals];
-#pragma unroll
-  for (int u = 0; u < kOutVals; ++u) acc[u] = 0.f;
+  float m00 = 0.f, m10 = 0.f, m20 = 0.f, m01 = 0.f, m11 = 0.f, m02 = 0.f, c0 = 0.f, c1 = 0.f, c2 = 0.f, c3 = 0.f;
 #pragma unroll
   for (int r = 0; r < R; ++r) {
+    float s0 = 0.f, s1 = 0.f, s2 = 0.f;
 #pragma unroll
     for (int c = 0; c < 8; ++c) {
       const float2 pw = pr[r * 8 + c];  // gp, w of (this Gaussian, pixel)
       const float4 gu = px[r * 8 + c];  // upstream dL/dRGB, dL/dDepth of the pixel
-      const float uu = fmaf(L.x, (float)c, ub[r]);
-      const float gx = pw.x * uu, gy = pw.x * vs[r];
-      acc[0] += gx;
-      acc[1] += gy;
-      acc[2] = fmaf(gx, uu, acc[2]);
-      acc[3] = fmaf(gx, vs[r], acc[3]);
-      acc[4] = fmaf(gy, vs[r], acc[4]);
-      acc[5] += pw.x;
-      acc[6] = fmaf(pw.y, gu.x, acc[6]);
-      acc[7] = fmaf(pw.y, gu.y, acc[7]);
-      acc[8] = fmaf(pw.y, gu.z, acc[8]);
-      acc[9] = fmaf(pw.y, gu.w, acc[9]);
+      constexpr float kHalf = 3.5f;
+      const float x = (float)c - kHalf;
+      s0 += pw.x;
+      s1 = fmaf(pw.x, x, s1);
+      s2 = fmaf(pw.x, x * x, s2);
+      c0 = fmaf(pw.y, gu.x, c0);
+      c1 = fmaf(pw.y, gu.y, c1);
+      c2 = fmaf(pw.y, gu.z, c2);
+      c3 = fmaf(pw.y, gu.w, c3);
     }
+    const float y = (float)(part * R + r) - 1.5f;
+    m00 += s0; m10 += s1; m20 += s2;
+    m01 = fmaf(y, s0, m01); m11 = fmaf(y, s1, m11); m02 = fmaf(y * y, s0, m02);
   }
+  float acc[kOutVals] = {m10, m01, m20, m11, m02, m00, c0, c1, c2, c3};
 #pragma unroll
   for (int u = 0; u < kOutVals; ++u) {
     acc[u] += __shfl_xor_sync(kFull, acc[u], 16);
     if (SPLIT == 4) acc[u] += __shfl_xor_sync(kFull, acc[u], 8);
+  }
+  // raw moments -> whitened moments
+  {
+    const float M10 = acc[0], M01 = acc[1], M20 = acc[2], M11 = acc[3], M02 = acc[4], M00 = acc[5];
+    const float xc = xo + 3.5f, yc = yo + 1.5f;
+    const float uc = fmaf(L.x, xc, fmaf(L.y, yc, sr.u0)), vc = fmaf(L.z, yc, sr.v0);
+    const float a1 = fmaf(L.x, M10, L.y * M01);                 // sum gp (l11 x + l21 y)
+    const float b1 = L.z * M01;                                 // sum gp l22 y
+    const float a2 = fmaf(L.x * L.x, M20, fmaf(2.f * L.x * L.y, M11, L.y * L.y * M02));
+    const float ab = L.z * fmaf(L.x, M11, L.y * M02);
+    const float b2 = L.z * L.z * M02;
+    acc[0] = fmaf(uc, M00, a1);
+    acc[1] = fmaf(vc, M00, b1);
+    acc[2] = fmaf(uc, fmaf(uc, M00, 2.f * a1), a2);
+    acc[3] = fmaf(vc, a1, fmaf(uc, fmaf(vc, M00, b1), ab));
+    acc[4] = fmaf(vc, fmaf(vc, M00, 2.f * b1), b2);
   }
   // the totals leave through shared memory (the pair table is consumed: the shuffles above converged the warp) so that
   // consecutive lanes carry consecutive values of consecutive slots: coalesced RED
@@ -102,8 +113,7 @@ __device__ __forceinline__ void gaussian_phase(float2* s_pair, const float4* s_p
   for (int t = 0; t < (LS * kOutVals + 31) / 32; ++t) {
     const int idx = t * 32 + lane;
     const int sl_i = min(idx / kOutVals, LS - 1), val = idx - sl_i * kOutVals;
-    const uint32_t gid = __shfl_sync(kFull, slot_id, sl_i);
-    if (idx < total) atomicAdd(g2d + (size_t)gid * kG2D + val, s_out[idx]);
+    if (idx < total) atomicAdd(g2d + (size_t)(s_slot[sl_i].ent >> 8) * kG2D + val, s_out[idx]);
   }
   __syncwarp();
 }
@@ -120,13 +130,14 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
                   float bg0, float bg1, float bg2, const float* __restrict__ final_T,
                   const uint32_t* __restrict__ n_contrib, const float* __restrict__ d_rgb,
                   const float* __restrict__ d_depth, const float* __restrict__ d_alpha, float* __restrict__ g2d) {
-  static_assert(NW == 2 || NW == 4 || NW == 8, "64 producer threads are needed");
   constexpr int CPT = 8 / NW;  // CTAs per tile
-  __shared__ StageBuf s_st[kStages];
+  constexpr int TPE = Ring<NW>::TPE;
+  __shared__ __align__(16) Ring<NW> ring;  // staging ring (gs_raster.cuh): no block-wide barrier in the loop
   // per warp: byte offsets (into the stage) of the round's relevant entries, back to front
   __shared__ __align__(8) uint16_t s_idx[NW][kTileBatch + kGroup];
   __shared__ __align__(16) float2 s_pair_all[NW][kSlots * kPairRow];
   __shared__ __align__(16) float4 s_pix_all[NW][32];
+  __shared__ SlotRec s_slot_all[NW][kSlots];
   __shared__ int s_nmax[NW];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int tile = (int)__ldg(order + blockIdx.x / CPT), sub = (blockIdx.x % CPT) * NW + warp;
@@ -138,6 +149,7 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
   const size_t HW = (size_t)W * H;
   float2* s_pair = s_pair_all[warp];
   float4* s_pix = s_pix_all[warp];
+  SlotRec* s_slot = s_slot_all[warp];
   float T = 1.f, gC0 = 0.f, gC1 = 0.f, gC2 = 0.f, gD = 0.f, gA = 0.f;
   uint32_t last = 0;
   if (tx0 + X < W && ty0 + Y < H) {
@@ -152,13 +164,7 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
   float S = T * (gC0 * bg0 + gC1 * bg1 + gC2 * bg2);
   const int n_w = (int)__reduce_max_sync(kFull, last);  // deepest blended list position of the region
   if (lane == 0) s_nmax[warp] = n_w;
-  if (tid < kStages) {  // padding records never pass: lo = -inf  =>  p2 = -inf
-    StageRec& pr = s_st[tid].rec[kPadIdx];
-    pr.g = make_float4(0.f, 0.f, 0.f, -INFINITY);
-    pr.c = make_float4(0.f, 0.f, 0.f, 0.f);
-    pr.uv = make_float2(0.f, 0.f);
-    pr.ent = 0u;
-  }
+  ring.init(tid);
   __syncthreads();
   int n = 0;
 #pragma unroll
@@ -166,110 +172,100 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
   const int nb = (n + kTileBatch - 1) / kTileBatch;
   int nslot = 0;
   float2* pair_ptr = s_pair + lane;     // where this lane's (gp, w) of the next slot goes
-  SlotRec slot = {0.f, 0.f};            // record of slot (lane & 15), kept in registers
-  uint32_t slot_id = 0;
 
-  // producer: rounds are staged back to front (list round nb - 1 first); thread t < 64 stages its entry t
+  // producer state: rounds are staged back to front (staged round k = list round nb - 1 - k); this thread stages entry
+  // e_pro of every round and fetches its list word one step ahead
+  const int e_pro = tid / TPE;
   uint32_t v_pre = 0;
-  int i_pre = (nb - 1) * kTileBatch + tid;  // list index of the entry this thread fetches next
-  auto prefetch = [&]() {
-    v_pre = (tid < kTileBatch && i_pre >= 0 && i_pre < n) ? __ldg(ids + range.x + i_pre) : 0u;
-    i_pre -= kTileBatch;
+  auto fetch = [&](int k) {
+    const int i = (nb - 1 - k) * kTileBatch + e_pro;
+    v_pre = (i >= 0 && i < n) ? __ldg(ids + range.x + i) : 0u;
   };
-  int i_pro = (nb - 1) * kTileBatch + tid, st_pro = 0;
-  auto produce = [&]() {
-    if (tid < kTileBatch && i_pro >= 0) {
-      StageRec& r = s_st[st_pro].rec[tid];
-      r.ent = v_pre;
-      if (i_pro < n) {
-        const float4* src = feat + 3 * (size_t)(v_pre >> 8) + 1;
-        cp_async16(&r.g, src);
-        cp_async16(&r.c, src + 1);
-        cp_async8(&r.uv, inst_uv + range.x + i_pro);
+  fetch(0);
+#pragma unroll
+  for (int k = 0; k < kAhead; ++k) {
+    if (k < nb) ring.produce(k, (nb - 1 - k) * kTileBatch + e_pro, n, range.x, v_pre, tid, ids, inst_uv, feat);
+    fetch(k + 1);
+  }
+  for (int k = 0; k < nb; ++k) {  // list rounds, back to front
+    const int stage = k & (kStages - 1);
+    const int pbase = (nb - 1 - k) * kTileBatch;
+    if (pbase < n_w) {  // else nothing of this round was blended in this region
+      mbar_wait(&ring.full[stage], (uint32_t)(k / kStages) & 1u);
+      const StageBuf& sb = ring.st[stage];
+      // the entries of this round that can reach this warp's region and lie in front of its deepest blended position, as
+      // a list of byte offsets in REVERSE list order
+      const bool r0 = ((sb.rec[lane].ent >> sub) & 1u) && pbase + lane < n_w;
+      const bool r1 = ((sb.rec[lane + 32].ent >> sub) & 1u) && pbase + 32 + lane < n_w;
+      const unsigned b0 = __ballot_sync(kFull, r0), b1 = __ballot_sync(kFull, r1);
+      const int n1 = __popc(b1), nrel = n1 + __popc(b0);
+      if (nrel) {
+        const unsigned gt = ~((2u << lane) - 1u);  // lanes above this one
+        uint16_t* idx = s_idx[warp];
+        if (r1) idx[__popc(b1 & gt)] = (uint16_t)((32 + lane) * 48);
+        if (r0) idx[n1 + __popc(b0 & gt)] = (uint16_t)(lane * 48);
+        if (lane < kGroup) idx[nrel + lane] = (uint16_t)(kPadIdx * 48);
+        __syncwarp();
+        const int lastb48 = ((int)last - pbase) * 48;  // entries of this round at offsets < lastb48 were blended by this pixel
+        const char* recs = reinterpret_cast<const char*>(sb.rec);
+        for (int r = 0; r < nrel; r += kGroup) {  // back to front, four list entries at a time
+          const uint2 o4 = *reinterpret_cast<const uint2*>(idx + r);
+          const uint32_t off[kGroup] = {o4.x & 0xffffu, o4.x >> 16, o4.y & 0xffffu, o4.y >> 16};
+          float4 uv[kGroup];  // u0, v0, bits(list word), -
+          float p[kGroup];
+          bool hit[kGroup];
+          unsigned bal[kGroup];
+#pragma unroll
+          for (int q = 0; q < kGroup; ++q) {
+            const StageRec& e = *reinterpret_cast<const StageRec*>(recs + off[q]);
+            const float4 a0 = e.g;  // l11, l21, l22, lo
+            uv[q] = *reinterpret_cast<const float4*>(&e.uv);  // one LDS.128 brings the list word along
+            p[q] = eval_power(uv[q].x, uv[q].y, a0.x, a0.y, a0.z, a0.w, fx0, fy0);
+            // blended by the forward: alpha >= 1/255 and in front of the pixel's last contributor
+            hit[q] = p[q] >= GS_POWER_MIN && (int)off[q] < lastb48;
+            bal[q] = __ballot_sync(kFull, hit[q]);
+          }
+#pragma unroll
+          for (int q = 0; q < kGroup; ++q) {
+            if (bal[q] == 0) continue;  // the Gaussian reaches no pixel of the region
+            const StageRec& e = *reinterpret_cast<const StageRec*>(recs + off[q]);
+            // branch-free: a lane that is not hit runs the same instructions with alpha = 0 (T, S unchanged, gp = w = 0)
+            const float4 f2 = e.c;
+            const float og = ex2_approx(p[q]);  // opacity * G: log2(opacity) is folded into the exponent
+            const float a = hit[q] ? fminf(GS_ALPHA_MAX, og) : 0.f;
+            const float ioma = rcp_approx(1.f - a);
+            T *= ioma;  // transmittance in front of this Gaussian
+            const float w = a * T;
+            float wi = fmaf(gC0, f2.x, fmaf(gC1, f2.y, fmaf(gC2, f2.z, gD * f2.w)));
+            if (HAS_GA) wi += gA;
+            const float dalpha = fmaf(T, wi, -S * ioma);
+            S = fmaf(wi, w, S);
+            const float gp = (og <= GS_ALPHA_MAX) ? a * dalpha : 0.f;  // no gradient through the clamp (Q2)
+            *pair_ptr = make_float2(gp, w);
+            pair_ptr += kPairRow;
+            if (lane == 0) *reinterpret_cast<float4*>(s_slot + nslot) = uv[q];
+            if (++nslot == kSlots) {
+              gaussian_phase<2>(s_pair, s_pix, s_slot, kSlots, lane, (float)xo, (float)yo, feat, g2d);
+              nslot = 0;
+              pair_ptr = s_pair + lane;
+            }
+          }
+        }
       }
     }
-    cp_async_commit();
-    i_pro -= kTileBatch;
-    st_pro = st_pro + 1 == kStages ? 0 : st_pro + 1;
-  };
-  prefetch(); produce();
-  prefetch(); produce();
-  prefetch();
-  int st_con = 0;
-  for (int j = nb - 1; j >= 0; --j) {  // list rounds, back to front
-    cp_async_wait<1>();  // this thread's copies of this round have landed ...
-    __syncthreads();     // ... everybody's have, and every warp has finished the previous round, whose stage is refilled next
-    produce();
-    prefetch();
-    const StageBuf& sb = s_st[st_con];
-    st_con = st_con + 1 == kStages ? 0 : st_con + 1;
-    const int pbase = j * kTileBatch;
-    if (pbase >= n_w) continue;      // nothing of this round was blended in this region
-    // the entries of this round that can reach this warp's region and lie in front of its deepest blended position, as
-    // a list of byte offsets in REVERSE list order
-    const bool r0 = ((sb.rec[lane].ent >> sub) & 1u) && pbase + lane < n_w;
-    const bool r1 = ((sb.rec[lane + 32].ent >> sub) & 1u) && pbase + 32 + lane < n_w;
-    const unsigned b0 = __ballot_sync(kFull, r0), b1 = __ballot_sync(kFull, r1);
-    const int n1 = __popc(b1), nrel = n1 + __popc(b0);
-    if (nrel == 0) continue;
-    const unsigned gt = ~((2u << lane) - 1u);  // lanes above this one
-    uint16_t* idx = s_idx[warp];
-    if (r1) idx[__popc(b1 & gt)] = (uint16_t)((32 + lane) * 48);
-    if (r0) idx[n1 + __popc(b0 & gt)] = (uint16_t)(lane * 48);
-    if (lane < kGroup) idx[nrel + lane] = (uint16_t)(kPadIdx * 48);
     __syncwarp();
-    const int lastb48 = ((int)last - pbase) * 48;  // entries of this round at offsets < lastb48 were blended by this pixel
-    const char* recs = reinterpret_cast<const char*>(sb.rec);
-    for (int r = 0; r < nrel; r += kGroup) {  // back to front, four list entries at a time
-      const uint2 o4 = *reinterpret_cast<const uint2*>(idx + r);
-      const uint32_t off[kGroup] = {o4.x & 0xffffu, o4.x >> 16, o4.y & 0xffffu, o4.y >> 16};
-      float2 uv[kGroup];
-      float p[kGroup];
-      bool hit[kGroup];
-      unsigned bal[kGroup];
-#pragma unroll
-      for (int q = 0; q < kGroup; ++q) {
-        const StageRec& e = *reinterpret_cast<const StageRec*>(recs + off[q]);
-        const float4 a0 = e.g;  // l11, l21, l22, lo
-        uv[q] = e.uv;
-        p[q] = eval_power(uv[q].x, uv[q].y, a0.x, a0.y, a0.z, a0.w, fx0, fy0);
-        // blended by the forward: alpha >= 1/255 and in front of the pixel's last contributor
-        hit[q] = p[q] >= GS_POWER_MIN && (int)off[q] < lastb48;
-        bal[q] = __ballot_sync(kFull, hit[q]);
-      }
-#pragma unroll
-      for (int q = 0; q < kGroup; ++q) {
-        if (bal[q] == 0) continue;  // the Gaussian reaches no pixel of the region
-        const StageRec& e = *reinterpret_cast<const StageRec*>(recs + off[q]);
-        // branch-free: a lane that is not hit runs the same instructions with alpha = 0 (T, S unchanged, gp = w = 0)
-        const float4 f2 = e.c;
-        const float og = ex2_approx(p[q]);  // opacity * G: log2(opacity) is folded into the exponent
-        const float a = hit[q] ? fminf(GS_ALPHA_MAX, og) : 0.f;
-        const float ioma = rcp_approx(1.f - a);
-        T *= ioma;  // transmittance in front of this Gaussian
-        const float w = a * T;
-        float wi = fmaf(gC0, f2.x, fmaf(gC1, f2.y, fmaf(gC2, f2.z, gD * f2.w)));
-        if (HAS_GA) wi += gA;
-        const float dalpha = fmaf(T, wi, -S * ioma);
-        S = fmaf(wi, w, S);
-        const float gp = (og <= GS_ALPHA_MAX) ? a * dalpha : 0.f;  // no gradient through the clamp (Q2)
-        *pair_ptr = make_float2(gp, w);
-        pair_ptr += kPairRow;
-        if ((lane & (kSlots - 1)) == nslot) {
-          slot.u0 = uv[q].x; slot.v0 = uv[q].y;
-          slot_id = e.ent >> 8;
-        }
-        if (++nslot == kSlots) {
-          gaussian_phase<2>(s_pair, s_pix, kSlots, lane, slot, slot_id, (float)xo, (float)yo, feat, g2d);
-          nslot = 0;
-          pair_ptr = s_pair + lane;
-        }
-      }
+    if (lane == 0) mbar_arrive(&ring.empty[stage]);  // this warp is done with the stage
+    // refill: the stage of staged round k - kDelay takes round k + kAhead once every warp has released it
+    const int kn = k + kAhead;
+    if (kn < nb) {
+      if (k >= kDelay) mbar_wait(&ring.empty[kn & (kStages - 1)], (uint32_t)((k - kDelay) / kStages) & 1u);
+      ring.produce(kn, (nb - 1 - kn) * kTileBatch + e_pro, n, range.x, v_pre, tid, ids, inst_uv, feat);
+      fetch(kn + 1);
     }
   }
-  cp_async_wait<0>();
-  if (nslot > 8) gaussian_phase<2>(s_pair, s_pix, nslot, lane, slot, slot_id, (float)xo, (float)yo, feat, g2d);
-  else if (nslot > 0) gaussian_phase<4>(s_pair, s_pix, nslot, lane, slot, slot_id, (float)xo, (float)yo, feat, g2d);
+  cp_async_wait_all();
+  if (nslot > 8) gaussian_phase<2>(s_pair, s_pix, s_slot, nslot, lane, (float)xo, (float)yo, feat, g2d);
+  else if (nslot > 0) gaussian_phase<4>(s_pair, s_pix, s_slot, nslot, lane, (float)xo, (float)yo, feat, g2d);
 }
 
 int launch_raster_bwd(gs_ctx* ctx, cudaStream_t s, const float* d_rgb, const float* d_depth, const float* d_alpha) {
