@@ -383,11 +383,12 @@ def run_ours(args):
     if "lds_bcast" in d:
         roof["lds_bcast"] = d["lds_bcast"]
     try:  # DRAM traffic per launch of the dominant kernel, from the committed ncu capture of this round (profiles/)
-        with open(os.path.join(ROOT, "profiles", "r2_traffic.json")) as f:
-            tr = json.load(f)
-        if tr.get("workload") == args.workload and kernel_name in tr["kernels"]:
-            roof["traffic"] = tr["kernels"][kernel_name]["dram_bytes_per_launch"]
-            roof["traffic_source"] = tr["source"]
+        import csv
+        with open(os.path.join(ROOT, "profiles", "r2_traffic.csv")) as f:
+            for row in csv.DictReader(f):
+                if row["workload"] == args.workload and row["kernel"] == kernel_name:
+                    roof["traffic"] = int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
+                    roof["traffic_source"] = row["source"]
     except Exception:
         pass
     # whole-iteration HBM figure (BASELINE.json "% HBM roofline"): algorithmic bytes of all stages / step time
