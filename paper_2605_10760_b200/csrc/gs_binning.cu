@@ -96,6 +96,7 @@ tile_scan_kernel(int tiles, const uint32_t* __restrict__ tile_count, uint32_t* _
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int b = blockIdx.x, nb = gridDim.x;
   const int t0 = (b * kScanT + tid) * IT;
+  pdl_enter();
   if (tid < kScanAgg) { s_pre[tid] = 0; s_tot[tid] = 0; }
   uint32_t c[IT];
   int cls[IT];
@@ -198,6 +199,7 @@ emit_kernel(const uint4* __restrict__ vis_rec, const float4* __restrict__ feat, 
   __shared__ float4 s_f0[kEmitG];
   __shared__ MaskSetup s_ms[kEmitG];
   const int tid = threadIdx.x;
+  pdl_enter();
   const uint32_t V = counts->n_visible;
   const uint32_t k0 = blockIdx.x * kEmitG;
   if (k0 >= V || counts->overflow) return;
@@ -267,6 +269,7 @@ emit_kernel(const uint4* __restrict__ vis_rec, const float4* __restrict__ feat, 
 __global__ void __launch_bounds__(256)
 range_fix_kernel(int tiles, const uint32_t* __restrict__ tile_cursor, uint2* __restrict__ ranges) {
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  pdl_enter();
   if (t >= tiles) return;
   uint2 r = ranges[t];
   if (r.y > r.x) { r.y = min(r.y, tile_cursor[(size_t)t * kCtrStride]); if (r.y == r.x) r = make_uint2(0u, 0u); ranges[t] = r; }
@@ -476,6 +479,7 @@ tile_sort_kernel(int tiles, int tiles_x, const uint32_t* __restrict__ order, con
                  float2* __restrict__ uv, const uint32_t* __restrict__ slot_of, const float4* __restrict__ feat) {
   __shared__ uint64_t s_x[2048];
   const int tid = threadIdx.x;
+  pdl_enter();
   const int n_mid = (int)counts->n_mid;
   if ((int)blockIdx.x < n_mid) {
     const int tile = (int)order[blockIdx.x];
@@ -578,11 +582,24 @@ static int run_tile_scan(gs_ctx* ctx, cudaStream_t s) {
   uint32_t seq_arg = ctx->seq, epoch_arg = epoch;
   void* args[] = {&tiles_arg, &count_arg, &ctx->tile_cursor, &ctx->ranges, &ctx->tile_order, &agg, &flags, &epoch_arg,
                   &cap_arg, &ctx->counts, &ctx->mailbox_dev, &seq_arg};
-  // cooperative launch: co-residency of the CTAs that wait on each other's flags is guaranteed by the runtime
-  if (nb1 <= kScanMaxCta)
-    GS_CUDA(cudaLaunchCooperativeKernel((const void*)tile_scan_kernel<1>, dim3(nb1), dim3(kScanT), args, 0, s));
-  else
-    GS_CUDA(cudaLaunchCooperativeKernel((const void*)tile_scan_kernel<8>, dim3(nb8), dim3(kScanT), args, 0, s));
+  // cooperative launch: co-residency of the CTAs that wait on each other's flags is guaranteed by the runtime; the
+  // programmatic-serialization attribute (pdl_enter) is added when the driver accepts the combination
+  const void* fn = nb1 <= kScanMaxCta ? (const void*)tile_scan_kernel<1> : (const void*)tile_scan_kernel<8>;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(nb1 <= kScanMaxCta ? nb1 : nb8); cfg.blockDim = dim3(kScanT); cfg.stream = s;
+  cudaLaunchAttribute at[2];
+  at[0].id = cudaLaunchAttributeCooperative; at[0].val.cooperative = 1;
+  at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[1].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = ctx->scan_pdl ? 2 : 1;
+  cudaError_t e = cudaLaunchKernelExC(&cfg, fn, args);
+  if (e != cudaSuccess && ctx->scan_pdl) {
+    cudaGetLastError();
+    ctx->scan_pdl = false;
+    cfg.numAttrs = 1;
+    e = cudaLaunchKernelExC(&cfg, fn, args);
+  }
+  GS_CUDA(e);
   GS_LAUNCH_CHECK("tile_scan_kernel");
   return GS_OK;
 }
@@ -616,12 +633,12 @@ int launch_binning(gs_ctx* ctx, cudaStream_t s) {
   }
   GS_PROF(3, s);
   if (ctx->N > 0) {
-    emit_kernel<<<(unsigned)div_up(ctx->N, kEmitG), kEmitT, 0, s>>>(ctx->vis_rec, ctx->feat, ctx->cam.tiles_x,
-                                                                    ctx->tile_cursor, ctx->counts, ctx->keys[0],
-                                                                    ctx->opt_exact_cull);
+    GS_LAUNCH_PDL(emit_kernel, (unsigned)div_up(ctx->N, kEmitG), kEmitT, 0, s, (const uint4*)ctx->vis_rec,
+                  (const float4*)ctx->feat, ctx->cam.tiles_x, ctx->tile_cursor, (const Counts*)ctx->counts, ctx->keys[0],
+                  ctx->opt_exact_cull);
     GS_LAUNCH_CHECK("emit_kernel");
     if (ctx->opt_exact_cull && tiles > 0) {
-      range_fix_kernel<<<(unsigned)div_up(tiles, 256), 256, 0, s>>>(tiles, ctx->tile_cursor, ctx->ranges);
+      GS_LAUNCH_PDL(range_fix_kernel, (unsigned)div_up(tiles, 256), 256, 0, s, tiles, (const uint32_t*)ctx->tile_cursor, ctx->ranges);
       GS_LAUNCH_CHECK("range_fix_kernel");
     }
   }
@@ -644,8 +661,9 @@ int launch_binning(gs_ctx* ctx, cudaStream_t s) {
         ctx->feat);
     GS_LAUNCH_CHECK("tile_sort_large_kernel");
     if (fork) GS_CUDA(cudaEventRecord(ctx->ev_join2, sl));
-    tile_sort_kernel<<<tiles, 128, 0, s>>>(tiles, ctx->cam.tiles_x, ctx->tile_order, ctx->ranges, ctx->counts, ctx->keys[0],
-                                           ctx->vals[0], ctx->inst_uv, ctx->slot_of, ctx->feat);
+    GS_LAUNCH_PDL(tile_sort_kernel, tiles, 128, 0, s, tiles, ctx->cam.tiles_x, (const uint32_t*)ctx->tile_order,
+                  (const uint2*)ctx->ranges, (const Counts*)ctx->counts, ctx->keys[0], ctx->vals[0], ctx->inst_uv,
+                  (const uint32_t*)ctx->slot_of, (const float4*)ctx->feat);
     GS_LAUNCH_CHECK("tile_sort_kernel");
     if (fork) GS_CUDA(cudaStreamWaitEvent(s, ctx->ev_join2, 0));
   }

@@ -38,6 +38,7 @@ gauss_bwd_kernel(int64_t N, const float* __restrict__ means, const float* __rest
   constexpr int K = (DEG + 1) * (DEG + 1);
   // one thread per VISIBLE Gaussian (compacted list of gs_preprocess)
   const int64_t kk = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  pdl_enter();
   const uint32_t V = counts->n_visible;
   if (WRITE && fill) {
     // Dense outputs: exact zeros for the culled Gaussians.  Block b clears the culled rows among the Gaussians
@@ -321,6 +322,7 @@ gauss_bwd_kernel(int64_t N, const float* __restrict__ means, const float* __rest
 // g_rho = sum g_pc + W sum g_v ; g_phi_k = <g_W, [e_k]x W> + (sum g_pc) . (e_k x t)      (C4)
 __global__ void pose_final_kernel(DevCam cam, const double* __restrict__ pose_acc, bool accumulate,
                                   float* __restrict__ g_twist) {
+  pdl_enter();
   if (threadIdx.x != 0 || blockIdx.x != 0) return;
   float T[12];
   load_pose(cam, T);
@@ -356,9 +358,10 @@ int launch_gauss_bwd(gs_ctx* ctx, cudaStream_t s, uint32_t flags, float* g_means
   const int threads = 128;
   const unsigned blocks = (unsigned)div_up(ctx->N, threads);
 #define GS_GB(D, Wr)                                                                                                 \
-  gauss_bwd_kernel<D, Wr><<<blocks, threads, 0, s>>>(ctx->N, ctx->means, ctx->scales, ctx->quats, ctx->opacities,   \
-                                                      ctx->sh, ctx->cam, ctx->vis_ids, ctx->vis_par, ctx->feat, ctx->counts, ctx->tiles_touched, ctx->g2d, accum, sparse, fill, \
-                                                      g_means, g_scales, g_quats, g_opac, g_sh, ctx->pose_acc)
+  GS_LAUNCH_PDL((gauss_bwd_kernel<D, Wr>), blocks, threads, 0, s, ctx->N, ctx->means, ctx->scales, ctx->quats,      \
+                ctx->opacities, ctx->sh, ctx->cam, (const uint32_t*)ctx->vis_ids, (const float4*)ctx->vis_par,        \
+                (const float4*)ctx->feat, (const Counts*)ctx->counts, (const uint32_t*)ctx->tiles_touched, ctx->g2d,  \
+                accum, sparse, fill, g_means, g_scales, g_quats, g_opac, g_sh, ctx->pose_acc)
   if (write) {
     switch (ctx->sh_degree) {
       case 0: GS_GB(0, true); break;
@@ -380,7 +383,7 @@ int launch_gauss_bwd(gs_ctx* ctx, cudaStream_t s, uint32_t flags, float* g_means
 }
 
 int launch_pose_final(gs_ctx* ctx, cudaStream_t s, uint32_t flags, float* g_twist) {
-  pose_final_kernel<<<1, 32, 0, s>>>(ctx->cam, ctx->pose_acc, (flags & GS_ACCUMULATE) != 0, g_twist);
+  GS_LAUNCH_PDL(pose_final_kernel, 1, 32, 0, s, ctx->cam, (const double*)ctx->pose_acc, (flags & GS_ACCUMULATE) != 0, g_twist);
   GS_LAUNCH_CHECK("pose_final_kernel");
   return GS_OK;
 }

@@ -51,6 +51,17 @@ constexpr int kFeatVec = 3;
 // from which dL/dmean = L M1 / k and dL/dSigma' = L M2 L^T / (2 k^2), k = 0.5 log2(e)  (gs_gauss_bwd.cu).
 constexpr int kG2D = 12;
 
+// Programmatic dependent launch (sm_90+): every kernel of the iteration is launched with
+// cudaLaunchAttributeProgrammaticStreamSerialization and starts with pdl_enter(): griddepcontrol.wait returns once the
+// kernel in front of it in the stream has completed and its writes are visible (every CTA of every kernel calls it
+// unconditionally, so completion is transitive along the chain), launch_dependents then lets the CTAs of the NEXT kernel
+// become resident while this one drains: launch latency and the ramp of each kernel hide under the tail of the one
+// before.  Without the launch attribute both instructions are no-ops.
+__device__ __forceinline__ void pdl_enter() {
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
+
 constexpr int kHdrBytes = 256;  // Counts (128 B) + 16 pose accumulators, in front of the per-tile counters (gs_api.cu)
 constexpr int kCtrStride = 32;  // per-tile counters are one per 128-byte line (gs_binning.cu)
 
@@ -112,6 +123,7 @@ struct gs_ctx {
   uint32_t* tile_cursor = nullptr;  // [tiles] write cursors of the duplication
   uint32_t* scan_ws = nullptr;      // tile scan: per-CTA totals [128][17] + epoch flags [128]
   uint32_t scan_epoch = 0;
+  bool scan_pdl = true;             // the cooperative tile scan also takes the programmatic-serialization attribute
   float* final_T = nullptr;         // [H*W]
   uint32_t* n_contrib = nullptr;    // [H*W]
 
@@ -171,6 +183,19 @@ inline int fail_cuda(gs_ctx* ctx, cudaError_t e, const char* where) {
     cudaError_t e__ = cudaGetLastError();                              \
     if (e__ != cudaSuccess) return gs::fail_cuda(ctx, e__, name);      \
     ctx->launches++;                                                   \
+  } while (0)
+
+// Launch with the programmatic-stream-serialization attribute (see pdl_enter above).
+#define GS_LAUNCH_PDL(kernel, grid__, block__, smem__, stream__, ...)                                         \
+  do {                                                                                                 \
+    cudaLaunchConfig_t cfg__ = {};                                                                     \
+    cfg__.gridDim = dim3(grid__); cfg__.blockDim = dim3(block__);                                          \
+    cfg__.dynamicSmemBytes = (smem__); cfg__.stream = (stream__);                                          \
+    cudaLaunchAttribute at__[1];                                                                       \
+    at__[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;                                   \
+    at__[0].val.programmaticStreamSerializationAllowed = 1;                                            \
+    cfg__.attrs = at__; cfg__.numAttrs = 1;                                                            \
+    GS_CUDA(cudaLaunchKernelEx(&cfg__, kernel, __VA_ARGS__));                                          \
   } while (0)
 
 // stage-timing event k on stream s (no-op unless gs_profile_enable(ctx, 1))

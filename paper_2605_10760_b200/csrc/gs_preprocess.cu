@@ -16,6 +16,7 @@ preprocess_kernel(int64_t N, const float* __restrict__ means, const float* __res
                   uint32_t* __restrict__ slot_of, Counts* __restrict__ counts) {
   constexpr int K = (DEG + 1) * (DEG + 1);
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  pdl_enter();
   float T[12];
   load_pose(cam, T);
   bool vis = false;
@@ -125,9 +126,9 @@ int launch_preprocess(gs_ctx* ctx, cudaStream_t s) {
   const int threads = 128;  // 64 registers, 8 CTAs / SM: the kernel is latency-bound (measured 256x3: 34.0, 256x4: 31.6, 128x8: 30.9, 128x10: 34.5 us)
   const unsigned blocks = (unsigned)div_up(N, threads);
 #define GS_PRE(D)                                                                                                    \
-  preprocess_kernel<D><<<blocks, threads, 0, s>>>(N, ctx->means, ctx->scales, ctx->quats, ctx->opacities, ctx->sh,  \
-                                                   ctx->cam, ctx->feat,                  \
-                                                   ctx->tiles_touched, ctx->tile_count, ctx->vis_ids, ctx->vis_rec, ctx->vis_par, ctx->slot_of, ctx->counts)
+  GS_LAUNCH_PDL(preprocess_kernel<D>, blocks, threads, 0, s, N, ctx->means, ctx->scales, ctx->quats, ctx->opacities, \
+                ctx->sh, ctx->cam, ctx->feat, ctx->tiles_touched, ctx->tile_count, ctx->vis_ids, ctx->vis_rec,        \
+                ctx->vis_par, ctx->slot_of, ctx->counts)
   switch (ctx->sh_degree) {
     case 0: GS_PRE(0); break;
     case 1: GS_PRE(1); break;

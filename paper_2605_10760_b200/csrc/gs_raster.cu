@@ -43,6 +43,7 @@ raster_fwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
   __shared__ __align__(8) uint16_t s_idx[NW][kTileBatch + kGroup];
   __shared__ int s_live;  // warps of the CTA that still have a live pixel: staging stops when it reaches zero
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  pdl_enter();
   const int tile = (int)__ldg(order + blockIdx.x / CPT), sub = (blockIdx.x % CPT) * NW + warp;
   const int tx0 = (tile % tiles_x) * GS_TILE, ty0 = (tile / tiles_x) * GS_TILE;
   const int X = (sub % 2) * 8 + (lane & 7), Y = (sub / 2) * 4 + (lane >> 3);  // tile-local pixel of this lane
@@ -179,9 +180,10 @@ int launch_raster_fwd(gs_ctx* ctx, cudaStream_t s, float* rgb, float* depth, flo
   const int tiles = ctx->cam.tiles_x * ctx->cam.tiles_y;
   if (tiles == 0) return GS_OK;
   constexpr int NW = GS_FWD_WARPS;
-  raster_fwd_kernel<NW, false><<<tiles * (8 / NW), NW * 32, 0, s>>>(
-      ctx->cam.W, ctx->cam.H, ctx->cam.tiles_x, ctx->tile_order, ctx->ranges, ctx->vals[ctx->sorted_buf], ctx->inst_uv,
-      ctx->feat, ctx->bg[0], ctx->bg[1], ctx->bg[2], rgb, depth, alpha, ctx->final_T, ctx->n_contrib, nullptr);
+  GS_LAUNCH_PDL((raster_fwd_kernel<NW, false>), tiles * (8 / NW), NW * 32, 0, s, ctx->cam.W, ctx->cam.H, ctx->cam.tiles_x,
+                (const uint32_t*)ctx->tile_order, (const uint2*)ctx->ranges, (const uint32_t*)ctx->vals[ctx->sorted_buf],
+                (const float2*)ctx->inst_uv, (const float4*)ctx->feat, ctx->bg[0], ctx->bg[1], ctx->bg[2], rgb, depth, alpha,
+                ctx->final_T, ctx->n_contrib, (unsigned long long*)nullptr);
   GS_LAUNCH_CHECK("raster_fwd_kernel");
   return GS_OK;
 }

@@ -140,6 +140,7 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
   __shared__ SlotRec s_slot_all[NW][kSlots];
   __shared__ int s_nmax[NW];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  pdl_enter();
   const int tile = (int)__ldg(order + blockIdx.x / CPT), sub = (blockIdx.x % CPT) * NW + warp;
   const int tx0 = (tile % tiles_x) * GS_TILE, ty0 = (tile / tiles_x) * GS_TILE;
   const int xo = (sub % 2) * 8, yo = (sub / 2) * 4;
@@ -273,9 +274,10 @@ int launch_raster_bwd(gs_ctx* ctx, cudaStream_t s, const float* d_rgb, const flo
   if (tiles == 0) return GS_OK;
   constexpr int NW = GS_BWD_WARPS;
 #define GS_BWD(GA)                                                                                                  \
-  raster_bwd_kernel<NW, GA><<<tiles * (8 / NW), NW * 32, 0, s>>>(                                                   \
-      ctx->cam.W, ctx->cam.H, ctx->cam.tiles_x, ctx->tile_order, ctx->ranges, ctx->vals[ctx->sorted_buf], ctx->inst_uv, \
-      ctx->feat, ctx->bg[0], ctx->bg[1], ctx->bg[2], ctx->final_T, ctx->n_contrib, d_rgb, d_depth, d_alpha, ctx->g2d)
+  GS_LAUNCH_PDL((raster_bwd_kernel<NW, GA>), tiles * (8 / NW), NW * 32, 0, s, ctx->cam.W, ctx->cam.H, ctx->cam.tiles_x, \
+                (const uint32_t*)ctx->tile_order, (const uint2*)ctx->ranges, (const uint32_t*)ctx->vals[ctx->sorted_buf], \
+                (const float2*)ctx->inst_uv, (const float4*)ctx->feat, ctx->bg[0], ctx->bg[1], ctx->bg[2],               \
+                (const float*)ctx->final_T, (const uint32_t*)ctx->n_contrib, d_rgb, d_depth, d_alpha, ctx->g2d)
   if (d_alpha) GS_BWD(true); else GS_BWD(false);
 #undef GS_BWD
   GS_LAUNCH_CHECK("raster_bwd_kernel");
