@@ -120,6 +120,7 @@ static int alloc_header(gs_ctx* ctx, int64_t tiles) {
   ctx->counts = reinterpret_cast<Counts*>(ctx->hdr);
   ctx->pose_acc = reinterpret_cast<double*>(ctx->hdr + 128);
   ctx->tile_count = reinterpret_cast<uint32_t*>(ctx->hdr + kHdrBytes);
+  ctx->hdr_clean = true;
   return GS_OK;
 }
 
@@ -253,9 +254,13 @@ int gs_preprocess(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, const flo
   ctx->N = N; ctx->sh_degree = sh_degree;
   ctx->means = means; ctx->scales = scales; ctx->quats = quats; ctx->opacities = opacities; ctx->sh = sh;
   ctx->seq++;
+  ctx->counts = reinterpret_cast<Counts*>(ctx->hdr + 64 * (ctx->seq & 1u));
   GS_PROF(0, s);
-  // counters, pose accumulators and per-tile instance counters: one memset (alloc_header)
-  GS_CUDA(cudaMemsetAsync(ctx->hdr, 0, kHdrBytes + (size_t)c.tiles_x * c.tiles_y * kCtrStride * sizeof(uint32_t), s));
+  // counters, pose accumulators and per-tile instance counters: in the steady state the previous iteration left them
+  // zero (gs_internal.cuh kHdrBytes); otherwise (first call, gs_preprocess twice in a row, a calibration pass, N = 0) one memset
+  if (!ctx->hdr_clean || N == 0)
+    GS_CUDA(cudaMemsetAsync(ctx->hdr, 0, kHdrBytes + (size_t)c.tiles_x * c.tiles_y * kCtrStride * sizeof(uint32_t), s));
+  ctx->hdr_clean = false;
   ctx->pose_acc_clean = true;
   if ((rc = launch_preprocess(ctx, s)) != GS_OK) return rc;
   GS_PROF(1, s);

@@ -88,9 +88,9 @@ __device__ __forceinline__ ScanVec block_excl_scan_vec(const ScanVec& v, uint32_
 
 template <int IT>
 __global__ void __launch_bounds__(kScanT)
-tile_scan_kernel(int tiles, const uint32_t* __restrict__ tile_count, uint32_t* __restrict__ tile_cursor,
+tile_scan_kernel(int tiles, uint32_t* __restrict__ tile_count, uint32_t* __restrict__ tile_cursor,
                  uint2* __restrict__ ranges, uint32_t* __restrict__ order, uint32_t* agg, uint32_t* flags,
-                 uint32_t epoch, int64_t capacity, Counts* counts, Counts* mailbox, uint32_t seq) {
+                 uint32_t epoch, int64_t capacity, Counts* counts, Counts* mailbox, uint32_t seq, Counts* counts_next) {
   __shared__ uint32_t wsum[kScanT / 32][kScanWords];
   __shared__ uint32_t s_pre[kScanAgg], s_tot[kScanAgg], s_base[kScanCls];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -104,7 +104,14 @@ tile_scan_kernel(int tiles, const uint32_t* __restrict__ tile_count, uint32_t* _
 #pragma unroll
   for (int k = 0; k < kScanWords; ++k) v.w[k] = 0;
 #pragma unroll
-  for (int u = 0; u < IT; ++u) c[u] = (t0 + u < tiles) ? __ldg(tile_count + (size_t)(t0 + u) * kCtrStride) : 0u;
+  for (int u = 0; u < IT; ++u) c[u] = (t0 + u < tiles) ? tile_count[(size_t)(t0 + u) * kCtrStride] : 0u;
+  // counts_next != null: leave the counters this scan consumed, and the Counts record of the next iteration, zero
+  if (counts_next) {
+#pragma unroll
+    for (int u = 0; u < IT; ++u)
+      if (t0 + u < tiles) tile_count[(size_t)(t0 + u) * kCtrStride] = 0u;
+    if (b == 0 && tid == 0) counts_next->n_visible = 0u;
+  }
 #pragma unroll
   for (int u = 0; u < IT; ++u) {
     cls[u] = length_class(c[u]);
@@ -153,6 +160,7 @@ tile_scan_kernel(int tiles, const uint32_t* __restrict__ tile_count, uint32_t* _
       // one 16-byte store to the mapped host mailbox {n_visible, n_instances, overflow, seq}: a single posted write,
       // so no system-scope fence is needed to order the fields
       *reinterpret_cast<uint4*>(mailbox) = make_uint4(counts->n_visible, I, ovf ? 1u : 0u, seq);
+      mailbox->n_large = nl;  // a hint for the next launch_binning (is the block-wide sort kernel needed at all?)
     }
   }
   __syncthreads();
@@ -476,7 +484,8 @@ tile_sort_large_kernel(int tiles_x, const uint32_t* __restrict__ order, const ui
 __global__ void __launch_bounds__(128)
 tile_sort_kernel(int tiles, int tiles_x, const uint32_t* __restrict__ order, const uint2* __restrict__ ranges,
                  const Counts* __restrict__ counts, uint64_t* __restrict__ keys, uint32_t* __restrict__ ids,
-                 float2* __restrict__ uv, const uint32_t* __restrict__ slot_of, const float4* __restrict__ feat) {
+                 float2* __restrict__ uv, const uint32_t* __restrict__ slot_of, const float4* __restrict__ feat,
+                 bool do_large) {
   __shared__ uint64_t s_x[2048];
   const int tid = threadIdx.x;
   pdl_enter();
@@ -485,8 +494,17 @@ tile_sort_kernel(int tiles, int tiles_x, const uint32_t* __restrict__ order, con
     const int tile = (int)order[blockIdx.x];
     const uint2 r = ranges[tile];
     const int n = (int)(r.y - r.x);
-    if (n > kMidSortMax) return;
     const SortOut out = {ids + r.x, uv + r.x, slot_of, feat, (tile % tiles_x) * GS_TILE, (tile / tiles_x) * GS_TILE};
+    if (n > kMidSortMax) {
+      // a long bucket: tile_sort_large_kernel's, unless the host did not launch it (do_large: the last finished iteration
+      // had no long bucket, so the side-stream launch was skipped) -- then sorted here in global memory: slow, correct, and
+      // the next iteration launches the large kernel again
+      if (do_large) {
+        bitonic_sort(keys + r.x, n, tid, 128);
+        for (int t = tid; t < n; t += 128) write_entry(out, t, keys[r.x + t]);
+      }
+      return;
+    }
     // keys per thread matched to the bucket: the network runs over 128 E slots whatever n is
     if (n <= 512) bucket_sort<4, 4>(keys + r.x, out, n, s_x, tid);
     else if (n <= 1024) bucket_sort<8, 4>(keys + r.x, out, n, s_x, tid);
@@ -563,7 +581,7 @@ int handle_overflow(gs_ctx* ctx) {
   return fail(ctx, GS_E_OVERFLOW, "tile-instance capacity exceeded in an earlier iteration; scratch has grown, re-issue");
 }
 
-static int run_tile_scan(gs_ctx* ctx, cudaStream_t s) {
+static int run_tile_scan(gs_ctx* ctx, cudaStream_t s, bool clear) {
   const int tiles = ctx->cam.tiles_x * ctx->cam.tiles_y;
   if (tiles == 0) return GS_OK;
   if (!ctx->scan_ws) {
@@ -577,11 +595,12 @@ static int run_tile_scan(gs_ctx* ctx, cudaStream_t s) {
   const int nb8 = (int)div_up(tiles, kScanT * 8);
   if (nb8 > kScanMaxCta) return fail(ctx, GS_E_INVALID, "gs_bin_tiles: more than 262144 tiles");
   int tiles_arg = tiles;
-  const uint32_t* count_arg = ctx->tile_count;
+  uint32_t* count_arg = ctx->tile_count;
+  Counts* next_arg = clear ? reinterpret_cast<Counts*>(ctx->hdr + 64 * ((ctx->seq + 1u) & 1u)) : nullptr;
   int64_t cap_arg = ctx->cap_I;
   uint32_t seq_arg = ctx->seq, epoch_arg = epoch;
   void* args[] = {&tiles_arg, &count_arg, &ctx->tile_cursor, &ctx->ranges, &ctx->tile_order, &agg, &flags, &epoch_arg,
-                  &cap_arg, &ctx->counts, &ctx->mailbox_dev, &seq_arg};
+                  &cap_arg, &ctx->counts, &ctx->mailbox_dev, &seq_arg, &next_arg};
   // cooperative launch: co-residency of the CTAs that wait on each other's flags is guaranteed by the runtime; the
   // programmatic-serialization attribute (pdl_enter) is added when the driver accepts the combination
   const void* fn = nb1 <= kScanMaxCta ? (const void*)tile_scan_kernel<1> : (const void*)tile_scan_kernel<8>;
@@ -600,6 +619,7 @@ static int run_tile_scan(gs_ctx* ctx, cudaStream_t s) {
     e = cudaLaunchKernelExC(&cfg, fn, args);
   }
   GS_CUDA(e);
+  if (clear) ctx->hdr_clean = true;
   GS_LAUNCH_CHECK("tile_scan_kernel");
   return GS_OK;
 }
@@ -612,12 +632,12 @@ int launch_binning(gs_ctx* ctx, cudaStream_t s) {
   if (!same_shape) {
     // calibration: scan the tile counts, read the instance total, size the buffers, scan again if it was short.
     // This is the only synchronising path of the iteration.
-    if ((rc = run_tile_scan(ctx, s)) != GS_OK) return rc;
+    if ((rc = run_tile_scan(ctx, s, false)) != GS_OK) return rc;
     GS_CUDA(cudaStreamSynchronize(s));
     const int64_t I = ctx->mailbox->n_instances;
     if (I > ctx->cap_I) {
       if ((rc = ensure_instance_capacity(ctx, I)) != GS_OK) return rc;
-      if ((rc = run_tile_scan(ctx, s)) != GS_OK) return rc;
+      if ((rc = run_tile_scan(ctx, s, false)) != GS_OK) return rc;
     }
     ctx->mailbox->overflow = 0;
     ctx->calibrated = true;
@@ -629,7 +649,7 @@ int launch_binning(gs_ctx* ctx, cudaStream_t s) {
     const Counts mb = read_mailbox(ctx);
     if ((int64_t)mb.n_instances + (int64_t)mb.n_instances / 8 > ctx->cap_I)
       if ((rc = ensure_instance_capacity(ctx, (int64_t)mb.n_instances + (int64_t)mb.n_instances / 4)) != GS_OK) return rc;
-    if ((rc = run_tile_scan(ctx, s)) != GS_OK) return rc;
+    if ((rc = run_tile_scan(ctx, s, true)) != GS_OK) return rc;
   }
   GS_PROF(3, s);
   if (ctx->N > 0) {
@@ -649,23 +669,26 @@ int launch_binning(gs_ctx* ctx, cudaStream_t s) {
                                    kLargeSort * (int)sizeof(uint64_t)));
       ctx->sort_attr_set = true;
     }
-    // the few long buckets (block-wide network) sort on the side stream while the warp kernel sorts the rest
-    const bool fork = ctx->side_stream != nullptr;
-    cudaStream_t sl = fork ? ctx->side_stream : s;
-    if (fork) {
+    // The few long buckets (block-wide network) sort on the side stream while the warp kernel sorts the rest -- when there
+    // are any: the number of long buckets of the last finished iteration (mailbox; exact after a calibration pass) decides
+    // whether the side-stream kernel is launched at all.  Without it the main stream is one chain of programmatically
+    // dependent kernels; a long bucket that shows up unannounced is sorted by tile_sort_kernel itself (slow path).
+    const bool large = ctx->side_stream != nullptr && read_mailbox(ctx).n_large > 0;
+    if (large) {
+      cudaStream_t sl = ctx->side_stream;
       GS_CUDA(cudaEventRecord(ctx->ev_fork2, s));
       GS_CUDA(cudaStreamWaitEvent(sl, ctx->ev_fork2, 0));
+      tile_sort_large_kernel<<<min(tiles, 296), 512, kLargeSort * sizeof(uint64_t), sl>>>(
+          ctx->cam.tiles_x, ctx->tile_order, ctx->ranges, ctx->counts, ctx->keys[0], ctx->vals[0], ctx->inst_uv, ctx->slot_of,
+          ctx->feat);
+      GS_LAUNCH_CHECK("tile_sort_large_kernel");
+      GS_CUDA(cudaEventRecord(ctx->ev_join2, sl));
     }
-    tile_sort_large_kernel<<<min(tiles, 296), 512, kLargeSort * sizeof(uint64_t), sl>>>(
-        ctx->cam.tiles_x, ctx->tile_order, ctx->ranges, ctx->counts, ctx->keys[0], ctx->vals[0], ctx->inst_uv, ctx->slot_of,
-        ctx->feat);
-    GS_LAUNCH_CHECK("tile_sort_large_kernel");
-    if (fork) GS_CUDA(cudaEventRecord(ctx->ev_join2, sl));
     GS_LAUNCH_PDL(tile_sort_kernel, tiles, 128, 0, s, tiles, ctx->cam.tiles_x, (const uint32_t*)ctx->tile_order,
                   (const uint2*)ctx->ranges, (const Counts*)ctx->counts, ctx->keys[0], ctx->vals[0], ctx->inst_uv,
-                  (const uint32_t*)ctx->slot_of, (const float4*)ctx->feat);
+                  (const uint32_t*)ctx->slot_of, (const float4*)ctx->feat, !large);
     GS_LAUNCH_CHECK("tile_sort_kernel");
-    if (fork) GS_CUDA(cudaStreamWaitEvent(s, ctx->ev_join2, 0));
+    if (large) GS_CUDA(cudaStreamWaitEvent(s, ctx->ev_join2, 0));
   }
   ctx->sorted_buf = 0;
   GS_PROF(5, s);

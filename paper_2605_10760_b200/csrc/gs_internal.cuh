@@ -62,7 +62,11 @@ __device__ __forceinline__ void pdl_enter() {
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 }
 
-constexpr int kHdrBytes = 256;  // Counts (128 B) + 16 pose accumulators, in front of the per-tile counters (gs_api.cu)
+// Header allocation: two Counts records (64 B apart; iteration seq uses record seq & 1, so the count of visible Gaussians
+// of one iteration stays readable until the next gs_preprocess while the other record is already cleared for it) + 16 pose
+// accumulators, in front of the per-tile counters (gs_api.cu).  Steady state needs no memset: tile_scan_kernel clears the
+// tile counters it has read and the other Counts record, preprocess_kernel clears the pose accumulators.
+constexpr int kHdrBytes = 256;
 constexpr int kCtrStride = 32;  // per-tile counters are one per 128-byte line (gs_binning.cu)
 
 // Device counters (one per context) + pinned-host mirror ("mailbox") the host may poll without synchronising.
@@ -132,7 +136,8 @@ struct gs_ctx {
   bool pose_acc_valid = false;
   bool pose_acc_clean = false;  // zeroed by gs_preprocess and not yet accumulated into
   unsigned long long* stats_ws = nullptr;  // gs_get_workload: its own 8 counters (never the pose accumulators)
-  char* hdr = nullptr;          // one allocation: counts, pose_acc, tile_count (zeroed by one memset per iteration)
+  char* hdr = nullptr;          // one allocation: counts x 2, pose_acc, tile_count
+  bool hdr_clean = false;       // the tile counters and the Counts record of the NEXT iteration are zero (else: one memset)
 
   gs::Counts* counts = nullptr;       // device
   gs::Counts* mailbox = nullptr;      // pinned host, mapped
@@ -233,7 +238,8 @@ inline Counts read_mailbox(const gs_ctx* ctx) {
     c.n_visible = m->n_visible; c.n_instances = m->n_instances; c.overflow = m->overflow;
     if (m->seq == c.seq) break;
   }
-  c.n_large = 0; c.n_mid = 0;
+  c.n_large = m->n_large;  // a hint only (written by a second store)
+  c.n_mid = 0;
   return c;
 }
 

@@ -13,10 +13,11 @@ preprocess_kernel(int64_t N, const float* __restrict__ means, const float* __res
                   DevCam cam, float4* __restrict__ feat,
                   uint32_t* __restrict__ tiles_touched, uint32_t* __restrict__ tile_count,
                   uint32_t* __restrict__ vis_ids, uint4* __restrict__ vis_rec, float4* __restrict__ vis_par,
-                  uint32_t* __restrict__ slot_of, Counts* __restrict__ counts) {
+                  uint32_t* __restrict__ slot_of, Counts* __restrict__ counts, double* __restrict__ pose_acc) {
   constexpr int K = (DEG + 1) * (DEG + 1);
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   pdl_enter();
+  if (blockIdx.x == 0 && threadIdx.x < 16) pose_acc[threadIdx.x] = 0.0;  // accumulated by gauss_bwd_kernel of this iteration
   float T[12];
   load_pose(cam, T);
   bool vis = false;
@@ -128,7 +129,7 @@ int launch_preprocess(gs_ctx* ctx, cudaStream_t s) {
 #define GS_PRE(D)                                                                                                    \
   GS_LAUNCH_PDL(preprocess_kernel<D>, blocks, threads, 0, s, N, ctx->means, ctx->scales, ctx->quats, ctx->opacities, \
                 ctx->sh, ctx->cam, ctx->feat, ctx->tiles_touched, ctx->tile_count, ctx->vis_ids, ctx->vis_rec,        \
-                ctx->vis_par, ctx->slot_of, ctx->counts)
+                ctx->vis_par, ctx->slot_of, ctx->counts, ctx->pose_acc)
   switch (ctx->sh_degree) {
     case 0: GS_PRE(0); break;
     case 1: GS_PRE(1); break;

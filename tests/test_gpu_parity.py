@@ -340,6 +340,27 @@ def test_long_buckets_all_sort_paths(oracle, gpu, N, spread):
     assert info["instances"] >= 2 * N   # most Gaussians touch the four tiles around pixel (32, 32)
 
 
+def test_unannounced_long_buckets_take_the_fallback_sort(oracle, gpu):
+    """gs_bin_tiles launches the block-wide sort of the long buckets only if the last finished iteration had any (no
+    host synchronisation).  Same (N, W, H) twice on one context: a spread-out scene first (no long bucket), then the pile:
+    its buckets of ~6000 keys arrive unannounced and are sorted by tile_sort_kernel's global-memory fallback; the third
+    iteration (announced) takes the side-stream kernel again.  Binning bit-exact, image and gradients vs the oracle."""
+    N = 6000
+    def scene(spread, seed):
+        r = np.random.Generator(np.random.PCG64(seed))
+        means = np.stack([r.normal(0.0, spread, N), r.normal(0.0, spread, N), r.uniform(2.0, 4.0, N)], axis=1).astype(np.float32)
+        return scenes.Scene(means=means, scales=np.exp(r.normal(-6.0, 0.3, (N, 3))).astype(np.float32),
+                            quats=r.normal(size=(N, 4)).astype(np.float32),
+                            opacities=(1.0 / (1.0 + np.exp(-r.normal(-2.0, 1.0, N)))).astype(np.float32),
+                            sh=r.normal(0.0, 0.5, (N, 1, 3)).astype(np.float32), sh_degree=0, camera=scenes.tiny_scene().camera,
+                            bg=np.zeros(3, np.float32), name=f"spread{spread}")
+    a = full_check(oracle, gpu, scene(1.0, 77), 9, uniform_edges=False)
+    assert a["instances"] < 4 * N
+    for _ in range(2):
+        b = full_check(oracle, gpu, scene(0.02, 78), 9, uniform_edges=False)
+        assert b["instances"] >= 2 * N
+
+
 def test_call_order_and_argument_errors(gpu):
     b, torch = gpu.binding, gpu.torch
     ctx = b.Context(0)
