@@ -67,7 +67,10 @@ __device__ __forceinline__ void pdl_enter() {
 // accumulators, in front of the per-tile counters (gs_api.cu).  Steady state needs no memset: tile_scan_kernel clears the
 // tile counters it has read and the other Counts record, preprocess_kernel clears the pose accumulators.
 constexpr int kHdrBytes = 256;
-constexpr int kCtrStride = 32;  // per-tile counters are one per 128-byte line (gs_binning.cu)
+#ifndef GS_CTR_STRIDE
+#define GS_CTR_STRIDE 32
+#endif
+constexpr int kCtrStride = GS_CTR_STRIDE;  // per-tile counters are one per 128-byte line (gs_binning.cu)
 
 // Device counters (one per context) + pinned-host mirror ("mailbox") the host may poll without synchronising.
 struct alignas(16) Counts {
