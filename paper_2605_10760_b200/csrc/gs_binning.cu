@@ -14,6 +14,8 @@
 //      bitonic network.  The keys are unique (the index is part of the key), so the result is THE (tile, depth bits,
 //      index) order, bit for bit, whatever the arrival order was.  Buckets beyond 8192 keys are sorted in global memory.
 // Integer work only.  Bytes: 8 I (emit) + 8 I (sort read) + 12 I (sorted keys + list entries) vs (8 + 24 * 6) I before.
+#include <algorithm>
+
 #include "gs_internal.cuh"
 #include "gs_raster.cuh"
 
@@ -209,8 +211,10 @@ emit_kernel(const uint4* __restrict__ vis_rec, const float4* __restrict__ feat, 
   const int tid = threadIdx.x;
   pdl_enter();
   const uint32_t V = counts->n_visible;
-  const uint32_t k0 = blockIdx.x * kEmitG;
-  if (k0 >= V || counts->overflow) return;
+  if (counts->overflow) return;
+  // grid-stride over groups of 32 visible Gaussians: the host sizes the grid from the visible count of the last finished
+  // iteration (two thirds of the N / 32 CTAs a worst-case grid needs would find nothing to do)
+  for (uint32_t k0 = blockIdx.x * kEmitG; k0 < V; k0 += gridDim.x * kEmitG) {
   if (tid < 32) {
     const uint32_t k = k0 + tid;
     uint4 rec = make_uint4(0u, 0u, 0u, 0u);
@@ -270,6 +274,8 @@ emit_kernel(const uint4* __restrict__ vis_rec, const float4* __restrict__ feat, 
 #pragma unroll
     for (int u = 0; u < 4; ++u)
       if (cur[u]) keys[pos[u]] = kk[u];
+  }
+  __syncthreads();  // the shared records are rewritten by the next group
   }
 }
 
@@ -656,7 +662,10 @@ int launch_binning(gs_ctx* ctx, cudaStream_t s) {
   }
   GS_PROF(3, s);
   if (ctx->N > 0) {
-    GS_LAUNCH_PDL(emit_kernel, (unsigned)div_up(ctx->N, kEmitG), kEmitT, 0, s, (const uint4*)ctx->vis_rec,
+    // grid: enough CTAs for 1.5 x the visible count of the last finished iteration (the kernel strides over the rest)
+    const int64_t v_hint = (int64_t)read_mailbox(ctx).n_visible;
+    const int64_t emit_ctas = std::min<int64_t>(div_up(ctx->N, kEmitG), std::max<int64_t>(div_up(v_hint + v_hint / 2, kEmitG), 148 * 8));
+    GS_LAUNCH_PDL(emit_kernel, (unsigned)emit_ctas, kEmitT, 0, s, (const uint4*)ctx->vis_rec,
                   (const float4*)ctx->feat, ctx->cam.tiles_x, ctx->tile_cursor, (const Counts*)ctx->counts, ctx->keys[0],
                   ctx->opt_exact_cull);
     GS_LAUNCH_CHECK("emit_kernel");
