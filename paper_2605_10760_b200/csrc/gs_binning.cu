@@ -124,19 +124,23 @@ tile_scan_kernel(int tiles, uint32_t* __restrict__ tile_count, uint32_t* __restr
     }
   }
   ScanVec pref = block_excl_scan_vec(v, wsum, lane, warp, total);
-  // publish this CTA's totals, then gather everybody's
+  // publish this CTA's totals, then gather everybody's.  Every total travels as ONE 64-bit word {epoch, value}: the reader
+  // spins on the word itself, so neither a flag nor a fence is needed (two L2 round trips less than flag-after-data)
+  unsigned long long* agg64 = reinterpret_cast<unsigned long long*>(agg);
   if (tid < kScanAgg) {
     const uint32_t x = tid == 0 ? total.w[0] : (total.w[1 + ((tid - 1) >> 1)] >> (((tid - 1) & 1) * 16)) & 0xffffu;
-    __stcg(agg + b * kScanAgg + tid, x);
-    __threadfence();
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(agg64 + b * kScanAgg + tid), "l"(((unsigned long long)epoch << 32) | x) : "memory");
   }
-  __syncthreads();
-  if (tid == 0) { __threadfence(); *reinterpret_cast<volatile uint32_t*>(flags + b) = epoch; }
+  const uint32_t nvis = counts->n_visible;  // for the mailbox (off the critical path)
   for (int i = tid; i < nb * kScanAgg; i += kScanT) {
     const int j = i / kScanAgg, k = i - j * kScanAgg;
-    while (*reinterpret_cast<volatile uint32_t*>(flags + j) != epoch) {}
-    __threadfence();
-    const uint32_t x = __ldcg(agg + j * kScanAgg + k);
+    unsigned long long w;
+    // one 64-bit load per poll, in asm: left to the compiler (__ldcg) the word was split into a hoisted load of the value
+    // half and a polled load of the epoch half -- stale totals whenever the scene changed
+    do {
+      asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(w) : "l"(agg64 + i) : "memory");
+    } while ((uint32_t)(w >> 32) != epoch);
+    const uint32_t x = (uint32_t)w;
     if (x) {
       atomicAdd(&s_tot[k], x);
       if (j < b) atomicAdd(&s_pre[k], x);
@@ -161,7 +165,7 @@ tile_scan_kernel(int tiles, uint32_t* __restrict__ tile_count, uint32_t* __restr
       counts->seq = seq;
       // one 16-byte store to the mapped host mailbox {n_visible, n_instances, overflow, seq}: a single posted write,
       // so no system-scope fence is needed to order the fields
-      *reinterpret_cast<uint4*>(mailbox) = make_uint4(counts->n_visible, I, ovf ? 1u : 0u, seq);
+      *reinterpret_cast<uint4*>(mailbox) = make_uint4(nvis, I, ovf ? 1u : 0u, seq);
       mailbox->n_large = nl;  // a hint for the next launch_binning (is the block-wide sort kernel needed at all?)
     }
   }
@@ -594,11 +598,11 @@ static int run_tile_scan(gs_ctx* ctx, cudaStream_t s, bool clear) {
   const int tiles = ctx->cam.tiles_x * ctx->cam.tiles_y;
   if (tiles == 0) return GS_OK;
   if (!ctx->scan_ws) {
-    GS_CUDA(cudaMalloc((void**)&ctx->scan_ws, (size_t)kScanMaxCta * (kScanAgg + 1) * sizeof(uint32_t)));
-    GS_CUDA(cudaMemset(ctx->scan_ws, 0, (size_t)kScanMaxCta * (kScanAgg + 1) * sizeof(uint32_t)));
+    GS_CUDA(cudaMalloc((void**)&ctx->scan_ws, (size_t)kScanMaxCta * kScanAgg * sizeof(unsigned long long)));
+    GS_CUDA(cudaMemset(ctx->scan_ws, 0, (size_t)kScanMaxCta * kScanAgg * sizeof(unsigned long long)));
   }
   uint32_t* agg = ctx->scan_ws;
-  uint32_t* flags = ctx->scan_ws + kScanMaxCta * kScanAgg;
+  uint32_t* flags = nullptr;  // (unused: the epoch travels inside the totals)
   const uint32_t epoch = ++ctx->scan_epoch;
   const int nb1 = (int)div_up(tiles, kScanT);
   const int nb8 = (int)div_up(tiles, kScanT * 8);

@@ -128,7 +128,7 @@ struct gs_ctx {
   uint2* ranges = nullptr;          // [tiles]
   uint32_t* tile_count = nullptr;   // [tiles] instances per tile (atomics in gs_preprocess)
   uint32_t* tile_cursor = nullptr;  // [tiles] write cursors of the duplication
-  uint32_t* scan_ws = nullptr;      // tile scan: per-CTA totals [128][17] + epoch flags [128]
+  uint32_t* scan_ws = nullptr;      // tile scan: per-CTA totals [128][17] as 64-bit words {epoch, value}
   uint32_t scan_epoch = 0;
   bool scan_pdl = true;             // the cooperative tile scan also takes the programmatic-serialization attribute
   float* final_T = nullptr;         // [H*W]

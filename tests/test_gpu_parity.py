@@ -361,6 +361,16 @@ def test_unannounced_long_buckets_take_the_fallback_sort(oracle, gpu):
         assert b["instances"] >= 2 * N
 
 
+def test_scene_change_on_a_calibrated_context_multi_cta_scan(oracle, gpu):
+    """Same (N, W, H) with different scenes back to back on one context: the asynchronous path of gs_bin_tiles (no
+    calibration pass), with a tile scan of several CTAs (1500 tiles) whose totals travel through re-used global words --
+    a stale total would shift every range.  Binning bit-exact, image and gradients vs the oracle, each time."""
+    for seed in (36, 37, 36):
+        sc = scenes.replica_scene(seed=seed, N=30000, width=800, height=480, f=400.0, sh_degree=1)
+        info = full_check(oracle, gpu, sc, seed)
+        assert info["instances"] > 5_000
+
+
 def test_call_order_and_argument_errors(gpu):
     b, torch = gpu.binding, gpu.torch
     ctx = b.Context(0)
