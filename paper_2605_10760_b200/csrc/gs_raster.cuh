@@ -74,6 +74,14 @@ __device__ __forceinline__ void cp_async4(void* smem_dst, const void* gmem_src) 
   asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(gmem_src) : "memory");
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+// TMA (bulk-copy engine) variant of the record gather, -DGS_RING_BULK: one cp.async.bulk of the 32 contiguous bytes
+// {l11,l21,l22,lo}{r,g,b,z} per staged entry, completing on the stage's mbarrier through its transaction count, instead of
+// two 16-byte cp.async.  Measured against the default in profiles/r2_v10_chain.md ("TMA where it pays").
+__device__ __forceinline__ void bulk_copy32(void* smem_dst, const void* gmem_src, uint64_t* bar) {
+  const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst), b = (uint32_t)__cvta_generic_to_shared(bar);
+  asm volatile("mbarrier.expect_tx.relaxed.cta.shared::cta.b64 [%0], 32;" ::"r"(b) : "memory");
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], 32, [%2];" ::"r"(d), "l"(gmem_src), "r"(b) : "memory");
+}
 
 // mbarrier (shared::cta) helpers of the staging ring.  full[s]: every thread of the CTA arrives through
 // cp.async.mbarrier.arrive.noinc, i.e. when ITS cp.async copies into stage s have landed (count = threads of the CTA);
@@ -130,8 +138,12 @@ struct Ring {
     StageRec& r = st[stage].rec[tid / TPE];
     if (i >= 0 && i < n) {
       const float4* src = feat + 3 * (size_t)(v >> 8) + 1;
+#ifdef GS_RING_BULK
+      if (part == 0) bulk_copy32(&r.g, src, &full[stage]);
+#else
       if (part == 0) cp_async16(&r.g, src);
       if (part == (1 & (TPE - 1))) cp_async16(&r.c, src + 1);
+#endif
       if (part == (2 & (TPE - 1))) cp_async8(&r.uv, inst_uv + first + i);
       if (part == (3 & (TPE - 1))) cp_async4(&r.ent, ids + first + i);
     }
