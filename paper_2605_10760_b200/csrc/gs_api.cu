@@ -164,7 +164,12 @@ int gs_create(gs_ctx** out, int device) {
   bool ok = cudaSetDevice(device) == cudaSuccess;
   ok = ok && alloc_header(ctx, 0) == GS_OK;
   ok = ok && cudaHostAlloc((void**)&ctx->mailbox, sizeof(Counts), cudaHostAllocMapped) == cudaSuccess;
-  ok = ok && cudaStreamCreateWithFlags(&ctx->side_stream, cudaStreamNonBlocking) == cudaSuccess;
+  // the side stream sorts the few long buckets beside tile_sort_kernel: highest priority, so that its 512-thread CTAs are
+  // placed first (launched behind the programmatically pre-launched tile_sort_kernel they otherwise queued until all 3225
+  // of its CTAs had been dispatched: the two kernels ran one after the other, config 4: 105 us for 57 || 53)
+  int prio_lo = 0, prio_hi = 0;
+  ok = ok && cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi) == cudaSuccess;
+  ok = ok && cudaStreamCreateWithPriority(&ctx->side_stream, cudaStreamNonBlocking, prio_hi) == cudaSuccess;
   ok = ok && cudaEventCreateWithFlags(&ctx->ev_fork2, cudaEventDisableTiming) == cudaSuccess;
   ok = ok && cudaEventCreateWithFlags(&ctx->ev_join2, cudaEventDisableTiming) == cudaSuccess;
   if (ok) {

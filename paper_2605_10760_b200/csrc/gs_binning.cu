@@ -491,10 +491,13 @@ tile_sort_large_kernel(int tiles_x, const uint32_t* __restrict__ order, const ui
 // Buckets up to kMidSortMax keys.  CTAs of 4 warps: the first n_mid entries of `order` (256 .. 2047 keys; those of the
 // large kernel are skipped) take a whole CTA each, 8 keys per thread; the remaining buckets (< 256 keys) take one warp
 // each, four buckets per CTA, no barrier at all.
-#ifndef GS_SORT_MIN_CTAS
-#define GS_SORT_MIN_CTAS 1
-#endif
+// (an explicit minimum of 1 CTA per SM lets ptxas take 110 registers instead of 92: four of these CTAs then no longer fit
+// beside the 512-thread CTA of tile_sort_large_kernel, and the two kernels of a scene with long buckets ran one after the other)
+#ifdef GS_SORT_MIN_CTAS
 __global__ void __launch_bounds__(128, GS_SORT_MIN_CTAS)
+#else
+__global__ void __launch_bounds__(128)
+#endif
 tile_sort_kernel(int tiles, int tiles_x, const uint32_t* __restrict__ order, const uint2* __restrict__ ranges,
                  const Counts* __restrict__ counts, uint64_t* __restrict__ keys, uint32_t* __restrict__ ids,
                  float2* __restrict__ uv, const uint32_t* __restrict__ slot_of, const float4* __restrict__ feat,

@@ -24,12 +24,9 @@ namespace gs {
 //          consecutive 16 bytes of a row); the colour is then evaluated from the thread's row (row stride 52 floats:
 //          conflict-free LDS.128).
 constexpr int kPreT = 128;
-#ifndef GS_PRE_U
-#define GS_PRE_U 4
-#endif
-constexpr int kPreU = GS_PRE_U;  // Gaussians per thread and round of the cull phase
+constexpr int kPreUMax = 4;  // Gaussians per thread and round of the cull phase (template parameter U: 1, 2 or 4)
 
-template <int DEG>
+template <int DEG, int kPreU>
 __global__ void __launch_bounds__(kPreT, 5)
 preprocess_kernel(int64_t N, const float* __restrict__ means, const float* __restrict__ scales,
                   const float* __restrict__ quats, const float* __restrict__ opacities, const float* __restrict__ sh,
@@ -43,7 +40,7 @@ preprocess_kernel(int64_t N, const float* __restrict__ means, const float* __res
   constexpr int RS = V4 ? ((K3 / 4) % 2 ? K3 : K3 + 4) : K3;  // row stride in floats (gs_gauss_bwd.cu uses the same layout)
   constexpr int EW = V4 ? 4 : 1, EPR = K3 / EW;
   __shared__ __align__(16) float s_sh[kPreT * RS];
-  __shared__ uint32_t s_q[(kPreU + 1) * kPreT];  // candidate queue (Gaussian indices)
+  __shared__ uint32_t s_q[(kPreUMax + 1) * kPreT];  // candidate queue (Gaussian indices)
   __shared__ uint32_t s_wcnt[kPreT / 32];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   pdl_enter();
@@ -216,11 +213,19 @@ int launch_preprocess(gs_ctx* ctx, cudaStream_t s) {
   const int threads = kPreT;
   int sms = 148;
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, ctx->device);
-  const unsigned blocks = (unsigned)min((int64_t)sms * GS_PRE_CTAS_PER_SM, div_up(N, threads * kPreU));  // persistent CTAs
-#define GS_PRE(D)                                                                                                    \
-  GS_LAUNCH_PDL(preprocess_kernel<D>, blocks, threads, 0, s, N, ctx->means, ctx->scales, ctx->quats, ctx->opacities, \
+  // Gaussians per thread and round of the cull phase: 4 when that still gives every resident CTA a round (measured on
+  // config 3: 1 / 2 / 4 / 8 -> 29.3 / 29.0 / 27.5 / 36.2 us), fewer for small scenes (config 2: 50 k Gaussians)
+  const int64_t resident = (int64_t)sms * GS_PRE_CTAS_PER_SM;
+  const int U = N >= 3 * resident * threads ? 4 : (N >= 2 * resident * threads ? 2 : 1);
+  const unsigned blocks = (unsigned)min(resident, div_up(N, threads * U));  // persistent CTAs
+#define GS_PRE_U(D, UU)                                                                                              \
+  GS_LAUNCH_PDL((preprocess_kernel<D, UU>), blocks, threads, 0, s, N, ctx->means, ctx->scales, ctx->quats, ctx->opacities, \
                 ctx->sh, ctx->cam, ctx->feat, ctx->tiles_touched, ctx->tile_count, ctx->vis_ids, ctx->vis_rec,        \
                 ctx->vis_par, ctx->slot_of, ctx->counts, ctx->pose_acc)
+#define GS_PRE(D)                                                                                                    \
+  do {                                                                                                               \
+    if (U == 4) GS_PRE_U(D, 4); else if (U == 2) GS_PRE_U(D, 2); else GS_PRE_U(D, 1);                                \
+  } while (0)
   switch (ctx->sh_degree) {
     case 0: GS_PRE(0); break;
     case 1: GS_PRE(1); break;
@@ -228,6 +233,7 @@ int launch_preprocess(gs_ctx* ctx, cudaStream_t s) {
     default: GS_PRE(3); break;
   }
 #undef GS_PRE
+#undef GS_PRE_U
   GS_LAUNCH_CHECK("preprocess_kernel");
   return GS_OK;
 }
