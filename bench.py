@@ -41,6 +41,11 @@ SEEDS = (30, 31, 32, 33, 34)
 #       pixels of the region): u (2), gp u, gp v (2), 2 adds (2), 3 FFMA (6), sum gp (1), 4 FFMA (8) = 21     -> 41
 FLOP_EVAL, FLOP_BLEND_FWD, FLOP_BLEND_BWD = 12.0, 12.0, 41.0
 LDS_PER_ENTRY = 3.0   # broadcast LDS.128 per relevant (region, Gaussian) entry in the pixel loops (48-byte record)
+# Warp instructions the kernels execute per relevant entry, from the committed ncu captures (profiles/r2_v9_ring.md,
+# r2_v10_chain.md: smsp__inst_executed / relevant entries of the captured scene).  NOT an algorithmic count: it says how
+# close the kernels run to the issue rate that actually binds them (roofline_stages[...]["issue"]), next to the
+# algorithmic FLOP fraction.
+WINST_PER_ENTRY_FWD, WINST_PER_ENTRY_BWD = 33.0, 67.0
 
 
 def load_measured_peaks_file():
@@ -223,9 +228,9 @@ def stage_models(N, K3, V, I, P, tiles, E, C, Eb, R, Rb, pose_only, dense_fill=T
         "emit": {"bound": "hbm", "bytes": 48 * V + 8 * I},
         "tile_sort": {"bound": "hbm", "bytes": 24 * I, "note": "compare-exchange network in registers: integer-ALU work"},
         "raster_fwd": {"bound": "alu", "flops": E * FLOP_EVAL + C * FLOP_BLEND_FWD, "lds": R * LDS_PER_ENTRY,
-                       "bytes": 4 * I + 48 * V + 24 * P},
+                       "winst": R * WINST_PER_ENTRY_FWD, "bytes": 4 * I + 48 * V + 24 * P},
         "raster_bwd": {"bound": "alu", "flops": Eb * FLOP_EVAL + C * FLOP_BLEND_BWD, "lds": Rb * LDS_PER_ENTRY,
-                       "bytes": 4 * I + 48 * V + 28 * P + 48 * V},
+                       "winst": Rb * WINST_PER_ENTRY_BWD, "bytes": 4 * I + 48 * V + 28 * P + 48 * V},
         "gauss_bwd": {"bound": "hbm", "bytes": (48 + 48 + 48 + 16 + 4 + 4 * K3) * V + gp * V + (fill * (N - V) + 4 * N if fill else 0),
                       "note": "reads g2d, parameters, SH of the V visible Gaussians, writes their gradient rows; dense mode: "
                               "+ the zero rows of the N - V culled Gaussians, cleared by the same kernel"},
@@ -367,7 +372,10 @@ def run_ours(args):
         else:
             e.update(flops=m["flops"], achieved=m["flops"] / t / 1e12, peak=alu_peak, unit="TFLOP/s",
                      lds_bcast={"warp_lds": m["lds"], "achieved": m["lds"] / t / 1e12, "peak": peaks["lds128_bcast_twarp"],
-                                "unit": "T warp-level LDS.128/s", "frac": m["lds"] / t / 1e12 / peaks["lds128_bcast_twarp"]})
+                                "unit": "T warp-level LDS.128/s", "frac": m["lds"] / t / 1e12 / peaks["lds128_bcast_twarp"]},
+                     issue={"warp_inst": m["winst"], "achieved": m["winst"] / t / 1e12, "peak": peaks["issue_twarp"],
+                            "unit": "T warp instructions/s", "frac": m["winst"] / t / 1e12 / peaks["issue_twarp"],
+                            "note": "executed (not algorithmic) instructions per relevant entry from the committed ncu capture"})
         e["frac"] = e["achieved"] / e["peak"]
         if "note" in m:
             e["note"] = m["note"]
@@ -382,6 +390,7 @@ def run_ours(args):
             "stage_share": stage_ms[dominant] / sum(stage_ms.values())}
     if "lds_bcast" in d:
         roof["lds_bcast"] = d["lds_bcast"]
+        roof["issue"] = d["issue"]
     try:  # DRAM traffic per launch of the dominant kernel, from the committed ncu capture of this round (profiles/)
         import csv
         with open(os.path.join(ROOT, "profiles", "r2_traffic.csv")) as f:
