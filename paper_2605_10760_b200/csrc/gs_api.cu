@@ -5,6 +5,8 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <algorithm>
+
 #include "gs_internal.cuh"
 
 using namespace gs;
@@ -121,6 +123,7 @@ static int alloc_header(gs_ctx* ctx, int64_t tiles) {
   ctx->pose_acc = reinterpret_cast<double*>(ctx->hdr + 128);
   ctx->tile_count = reinterpret_cast<uint32_t*>(ctx->hdr + kHdrBytes);
   ctx->hdr_clean = true;
+  ctx->ctr_dirty = 0;
   return GS_OK;
 }
 
@@ -263,9 +266,14 @@ int gs_preprocess(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, const flo
   GS_PROF(0, s);
   // counters, pose accumulators and per-tile instance counters: in the steady state the previous iteration left them
   // zero (gs_internal.cuh kHdrBytes); otherwise (first call, gs_preprocess twice in a row, a calibration pass, N = 0) one memset
-  if (!ctx->hdr_clean || N == 0)
-    GS_CUDA(cudaMemsetAsync(ctx->hdr, 0, kHdrBytes + (size_t)c.tiles_x * c.tiles_y * kCtrStride * sizeof(uint32_t), s));
+  const int64_t tiles_now = (int64_t)c.tiles_x * c.tiles_y;
+  if (!ctx->hdr_clean || N == 0 || ctx->ctr_dirty > tiles_now) {
+    // (also the counters a LARGER image of an earlier call may have left behind: a scan clears only the tiles it reads)
+    GS_CUDA(cudaMemsetAsync(ctx->hdr, 0, kHdrBytes + (size_t)std::max(tiles_now, ctx->ctr_dirty) * kCtrStride * sizeof(uint32_t), s));
+    ctx->ctr_dirty = 0;
+  }
   ctx->hdr_clean = false;
+  ctx->ctr_dirty = std::max(ctx->ctr_dirty, tiles_now);
   ctx->pose_acc_clean = true;
   if ((rc = launch_preprocess(ctx, s)) != GS_OK) return rc;
   GS_PROF(1, s);

@@ -635,7 +635,10 @@ static int run_tile_scan(gs_ctx* ctx, cudaStream_t s, bool clear) {
     e = cudaLaunchKernelExC(&cfg, fn, args);
   }
   GS_CUDA(e);
-  if (clear) ctx->hdr_clean = true;
+  if (clear) {  // the scan leaves the counters of THIS image size zero
+    ctx->hdr_clean = true;
+    if (ctx->ctr_dirty <= (int64_t)tiles) ctx->ctr_dirty = 0;
+  }
   GS_LAUNCH_CHECK("tile_scan_kernel");
   return GS_OK;
 }

@@ -141,6 +141,7 @@ struct gs_ctx {
   unsigned long long* stats_ws = nullptr;  // gs_get_workload: its own 8 counters (never the pose accumulators)
   char* hdr = nullptr;          // one allocation: counts x 2, pose_acc, tile_count
   bool hdr_clean = false;       // the tile counters and the Counts record of the NEXT iteration are zero (else: one memset)
+  int64_t ctr_dirty = 0;        // number of leading tile counters that may be non-zero (image sizes may change between calls)
 
   gs::Counts* counts = nullptr;       // device
   gs::Counts* mailbox = nullptr;      // pinned host, mapped

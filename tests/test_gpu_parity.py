@@ -371,6 +371,21 @@ def test_scene_change_on_a_calibrated_context_multi_cta_scan(oracle, gpu):
         assert info["instances"] > 5_000
 
 
+def test_tile_counters_survive_changes_of_image_size(oracle, gpu):
+    """The steady state has no memset: the tile scan zeroes the counters it consumed.  A gs_preprocess on a LARGE image
+    that is never binned leaves counters behind which a later pass on a SMALL image does not reach; the next large pass
+    must still start from zero counters (the library tracks how far the counters may be dirty)."""
+    b = gpu.binding
+    big = scenes.replica_scene(seed=38, N=20000, width=640, height=400, f=320.0, sh_degree=0)
+    small = scenes.replica_scene(seed=38, N=20000, width=160, height=96, f=80.0, sh_degree=0)
+    full_check(oracle, gpu, big, 38)       # calibrates the big shape
+    full_check(oracle, gpu, small, 38)     # calibrates the small shape
+    ds = b.DeviceScene(big)
+    gpu.ctx.gs_preprocess(ds.means, ds.scales, ds.quats, ds.opacities, ds.sh, 0, big.camera)   # counted, never binned
+    for sc in (small, small, big, big):
+        full_check(oracle, gpu, sc, 38)
+
+
 def test_call_order_and_argument_errors(gpu):
     b, torch = gpu.binding, gpu.torch
     ctx = b.Context(0)
