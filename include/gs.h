@@ -64,7 +64,8 @@ typedef struct {
 typedef struct gs_ctx gs_ctx; /* opaque */
 
 /* flags of gs_rasterize_bwd / gs_pose_grad */
-#define GS_ACCUMULATE 1u /* parameter gradients are added to the output arrays instead of overwriting them (config 5) */
+#define GS_ACCUMULATE 1u /* parameter gradients are added to the output arrays instead of overwriting them (config 5);
+                            the addition is one fp32 RED.ADD per element at L2 (a denormal sum is flushed to zero) */
 #define GS_POSE_ONLY 2u  /* Gaussians frozen: no parameter gradients are written; output pointers may be NULL (config 4) */
 #define GS_SPARSE_GRADS 4u /* parameter gradients are written COMPACT: row r of every g_* array belongs to the Gaussian
                             gs_visible_ids()[r], r < n_visible (arrays need n_visible <= N rows); rows of culled Gaussians do
@@ -119,8 +120,13 @@ GS_API int gs_preprocess(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, co
  * result is THE (tile, depth, index) order, bit for bit (DESIGN.md section 6 records the measured radix alternatives).
  * The first call after gs_create (or after N / the image size changed) synchronises once to size the instance
  * buffers; later calls are asynchronous and report an overflow through GS_E_OVERFLOW on a later call.
- * The prefix-sum kernel exchanges per-CTA totals through flags its CTAs spin on: it is launched cooperatively
- * (all of its <= 128 CTAs are guaranteed co-resident; GS_E_CUDA if the device cannot hold them, e.g. under MPS limits). */
+ * The prefix-sum kernel exchanges per-CTA totals through {epoch, value} words its CTAs poll: it is launched cooperatively
+ * (all of its <= 128 CTAs are guaranteed co-resident; GS_E_CUDA if the device cannot hold them, e.g. under MPS limits).
+ * Stream behaviour of the five calls: every kernel is launched on `stream` with the programmatic-stream-serialization
+ * attribute and begins with griddepcontrol.wait, i.e. it consumes nothing before the work in front of it on the stream
+ * (the caller's own kernels included) has completed; work the caller enqueues behind a call is ordered as usual.  Only
+ * buckets beyond 2047 keys are sorted on a context-owned side stream (forked from and joined to `stream` by events), and
+ * only in iterations that follow one that had such buckets. */
 GS_API int gs_bin_tiles(gs_ctx* ctx, void* stream);
 
 /* Step a6 -- per-tile front-to-back compositing (oracle reading C1 step 7).
