@@ -190,8 +190,8 @@ int gs_destroy(gs_ctx* ctx) {
   cudaDeviceSynchronize();
   cudaFree(ctx->feat); cudaFree(ctx->tiles_touched); cudaFree(ctx->vis_ids); cudaFree(ctx->vis_rec); cudaFree(ctx->vis_par); cudaFree(ctx->slot_of);
   cudaFree(ctx->g2d);
-  for (int b = 0; b < 2; ++b) { cudaFree(ctx->keys[b]); cudaFree(ctx->vals[b]); }
-  cudaFree(ctx->inst_uv);
+  for (int b = 0; b < 2; ++b) cudaFree(ctx->keys[b]);
+  cudaFree(ctx->inst_rec);
   cudaFree(ctx->hdr); cudaFree(ctx->tile_cursor); cudaFree(ctx->scan_ws);
   cudaFree(ctx->ranges); cudaFree(ctx->tile_order); cudaFree(ctx->final_T); cudaFree(ctx->n_contrib);
   cudaFree(ctx->hb); cudaFree(ctx->stats_ws); cudaFree(ctx->rv);

@@ -390,8 +390,7 @@ __device__ __forceinline__ void smem_step(uint64_t (&k)[E], uint64_t* s, int tid
 // What the compositing kernels read for a sorted key (.. | index << 8 | mask): the list entry (visible slot << 8 | region
 // mask) and the instance's whitened tile-local offset (u0, v0) = -L^T (mean - tile origin), in fp64 (gs_raster.cuh).
 struct SortOut {
-  uint32_t* ids;
-  float2* uv;
+  float4* rec;   // {u0, v0, bits(slot << 8 | mask), -} per sorted instance
   const uint32_t* slot_of;
   const float4* feat;
   int ox, oy;  // pixel origin of the bucket's tile
@@ -400,11 +399,10 @@ struct SortOut {
 __device__ __forceinline__ void write_entry(const SortOut& o, int i, uint64_t key) {
   const uint32_t lo = (uint32_t)key;
   const uint32_t slot = __ldg(o.slot_of + (lo >> 8));
-  o.ids[i] = (slot << 8) | (lo & 0xffu);
   const float4 f0 = __ldg(o.feat + 3 * (size_t)slot), f1 = __ldg(o.feat + 3 * (size_t)slot + 1);
   float u0, v0, mx, my;
   decode_whitened(f0, f1, o.ox, o.oy, u0, v0, mx, my);
-  o.uv[i] = make_float2(u0, v0);
+  o.rec[i] = make_float4(u0, v0, __uint_as_float((slot << 8) | (lo & 0xffu)), 0.f);
 }
 
 template <int E, int NW>
@@ -449,10 +447,9 @@ __device__ __forceinline__ void bucket_sort(uint64_t* __restrict__ g, const Sort
       const int i = tid * E + c + e;
       if (i < n) {
         g[i] = k[c + e];
-        out.ids[i] = (slot[e] << 8) | ((uint32_t)k[c + e] & 0xffu);
         float u0, v0, mx, my;
         decode_whitened(f0[e], f1[e], out.ox, out.oy, u0, v0, mx, my);
-        out.uv[i] = make_float2(u0, v0);
+        out.rec[i] = make_float4(u0, v0, __uint_as_float((slot[e] << 8) | ((uint32_t)k[c + e] & 0xffu)), 0.f);
       }
     }
   }
@@ -464,8 +461,8 @@ __device__ __forceinline__ void bucket_sort(uint64_t* __restrict__ g, const Sort
 // scenes only).
 __global__ void __launch_bounds__(512)
 tile_sort_large_kernel(int tiles_x, const uint32_t* __restrict__ order, const uint2* __restrict__ ranges,
-                       const Counts* __restrict__ counts, uint64_t* __restrict__ keys, uint32_t* __restrict__ ids,
-                       float2* __restrict__ uv, const uint32_t* __restrict__ slot_of, const float4* __restrict__ feat) {
+                       const Counts* __restrict__ counts, uint64_t* __restrict__ keys,
+                       float4* __restrict__ rec, const uint32_t* __restrict__ slot_of, const float4* __restrict__ feat) {
   extern __shared__ uint64_t s_dyn[];
   const int tid = threadIdx.x, nth = blockDim.x;
   const int limit = (int)counts->n_large;
@@ -475,7 +472,7 @@ tile_sort_large_kernel(int tiles_x, const uint32_t* __restrict__ order, const ui
     const int n = (int)(r.y - r.x);
     if (n <= kMidSortMax) continue;
     uint64_t* g = keys + r.x;
-    const SortOut out = {ids + r.x, uv + r.x, slot_of, feat, (tile % tiles_x) * GS_TILE, (tile / tiles_x) * GS_TILE};
+    const SortOut out = {rec + r.x, slot_of, feat, (tile % tiles_x) * GS_TILE, (tile / tiles_x) * GS_TILE};
     if (n > kLargeSort) {
       bitonic_sort(g, n, tid, nth);  // __syncthreads orders the CTA's own global writes
       for (int t = tid; t < n; t += nth) write_entry(out, t, g[t]);
@@ -499,8 +496,8 @@ __global__ void __launch_bounds__(128, GS_SORT_MIN_CTAS)
 __global__ void __launch_bounds__(128)
 #endif
 tile_sort_kernel(int tiles, int tiles_x, const uint32_t* __restrict__ order, const uint2* __restrict__ ranges,
-                 const Counts* __restrict__ counts, uint64_t* __restrict__ keys, uint32_t* __restrict__ ids,
-                 float2* __restrict__ uv, const uint32_t* __restrict__ slot_of, const float4* __restrict__ feat,
+                 const Counts* __restrict__ counts, uint64_t* __restrict__ keys,
+                 float4* __restrict__ rec, const uint32_t* __restrict__ slot_of, const float4* __restrict__ feat,
                  bool do_large) {
   __shared__ uint64_t s_x[2048];
   const int tid = threadIdx.x;
@@ -510,7 +507,7 @@ tile_sort_kernel(int tiles, int tiles_x, const uint32_t* __restrict__ order, con
     const int tile = (int)order[blockIdx.x];
     const uint2 r = ranges[tile];
     const int n = (int)(r.y - r.x);
-    const SortOut out = {ids + r.x, uv + r.x, slot_of, feat, (tile % tiles_x) * GS_TILE, (tile / tiles_x) * GS_TILE};
+    const SortOut out = {rec + r.x, slot_of, feat, (tile % tiles_x) * GS_TILE, (tile / tiles_x) * GS_TILE};
     if (n > kMidSortMax) {
       // a long bucket: tile_sort_large_kernel's, unless the host did not launch it (do_large: the last finished iteration
       // had no long bucket, so the side-stream launch was skipped) -- then sorted here in global memory: slow, correct, and
@@ -533,7 +530,7 @@ tile_sort_kernel(int tiles, int tiles_x, const uint32_t* __restrict__ order, con
   const uint2 r = ranges[tile];
   const int n = (int)(r.y - r.x), lane = tid & 31;
   if (n == 0) return;
-  const SortOut out = {ids + r.x, uv + r.x, slot_of, feat, (tile % tiles_x) * GS_TILE, (tile / tiles_x) * GS_TILE};
+  const SortOut out = {rec + r.x, slot_of, feat, (tile % tiles_x) * GS_TILE, (tile / tiles_x) * GS_TILE};
   if (n <= 64) bucket_sort<2, 1>(keys + r.x, out, n, nullptr, lane);
   else if (n <= 128) bucket_sort<4, 1>(keys + r.x, out, n, nullptr, lane);
   else bucket_sort<8, 1>(keys + r.x, out, n, nullptr, lane);
@@ -548,18 +545,18 @@ __global__ void export_keys_kernel(int tiles, const uint2* __restrict__ ranges, 
   for (uint32_t k = r.x + threadIdx.x; k < r.y; k += blockDim.x) out[k] = ((uint64_t)tile << 32) | (keys[k] >> 32);
 }
 
-__global__ void export_ids_kernel(int tiles, const uint2* __restrict__ ranges, const uint32_t* __restrict__ vals,
+__global__ void export_ids_kernel(int tiles, const uint2* __restrict__ ranges, const float4* __restrict__ rec,
                                   const uint32_t* __restrict__ vis_ids, uint32_t* __restrict__ out) {
   const int tile = blockIdx.x;
   if (tile >= tiles) return;
   const uint2 r = ranges[tile];  // per tile range: in exact-cull mode the entries between two lists are unspecified
-  for (uint32_t k = r.x + threadIdx.x; k < r.y; k += blockDim.x) out[k] = vis_ids[vals[k] >> 8];  // slot -> Gaussian index
+  for (uint32_t k = r.x + threadIdx.x; k < r.y; k += blockDim.x) out[k] = vis_ids[__float_as_uint(rec[k].z) >> 8];  // slot -> Gaussian index
 }
 
 int export_sorted_ids(gs_ctx* ctx, cudaStream_t s, int64_t I, uint32_t* out) {
   const int tiles = ctx->cam.tiles_x * ctx->cam.tiles_y;
   if (I <= 0 || tiles == 0) return GS_OK;
-  export_ids_kernel<<<tiles, 128, 0, s>>>(tiles, ctx->ranges, ctx->vals[ctx->sorted_buf], ctx->vis_ids, out);
+  export_ids_kernel<<<tiles, 128, 0, s>>>(tiles, ctx->ranges, ctx->inst_rec, ctx->vis_ids, out);
   GS_LAUNCH_CHECK("export_ids_kernel");
   return GS_OK;
 }
@@ -579,8 +576,7 @@ int ensure_instance_capacity(gs_ctx* ctx, int64_t need) {
   if (cap >= (1ll << 31)) return fail(ctx, GS_E_NOMEM, "more than 2^31 tile instances");
   int rc;
   if ((rc = grow(ctx, ctx->keys[0], cap)) != GS_OK) return rc;
-  if ((rc = grow(ctx, ctx->vals[0], cap)) != GS_OK) return rc;
-  if ((rc = grow(ctx, ctx->inst_uv, cap)) != GS_OK) return rc;
+  if ((rc = grow(ctx, ctx->inst_rec, cap)) != GS_OK) return rc;
   ctx->cap_I = cap;
   return GS_OK;
 }
@@ -701,13 +697,13 @@ int launch_binning(gs_ctx* ctx, cudaStream_t s) {
       GS_CUDA(cudaEventRecord(ctx->ev_fork2, s));
       GS_CUDA(cudaStreamWaitEvent(sl, ctx->ev_fork2, 0));
       tile_sort_large_kernel<<<min(tiles, 296), 512, kLargeSort * sizeof(uint64_t), sl>>>(
-          ctx->cam.tiles_x, ctx->tile_order, ctx->ranges, ctx->counts, ctx->keys[0], ctx->vals[0], ctx->inst_uv, ctx->slot_of,
+          ctx->cam.tiles_x, ctx->tile_order, ctx->ranges, ctx->counts, ctx->keys[0], ctx->inst_rec, ctx->slot_of,
           ctx->feat);
       GS_LAUNCH_CHECK("tile_sort_large_kernel");
       GS_CUDA(cudaEventRecord(ctx->ev_join2, sl));
     }
     GS_LAUNCH_PDL(tile_sort_kernel, tiles, 128, 0, s, tiles, ctx->cam.tiles_x, (const uint32_t*)ctx->tile_order,
-                  (const uint2*)ctx->ranges, (const Counts*)ctx->counts, ctx->keys[0], ctx->vals[0], ctx->inst_uv,
+                  (const uint2*)ctx->ranges, (const Counts*)ctx->counts, ctx->keys[0], ctx->inst_rec,
                   (const uint32_t*)ctx->slot_of, (const float4*)ctx->feat, !large);
     GS_LAUNCH_CHECK("tile_sort_kernel");
     if (large) GS_CUDA(cudaStreamWaitEvent(s, ctx->ev_join2, 0));

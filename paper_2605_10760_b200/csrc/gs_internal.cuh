@@ -118,8 +118,9 @@ struct gs_ctx {
   int64_t cal_N = -1;
   int32_t cal_W = -1, cal_H = -1;
   uint64_t* keys[2] = {nullptr, nullptr};  // [0]: (depth bits << 32 | id) bucketed by tile, sorted in place
-  uint32_t* vals[2] = {nullptr, nullptr};  // [0]: sorted (visible slot << 8 | region mask): what the compositing kernels read
-  float2* inst_uv = nullptr;               // [cap_I] whitened tile-local offset (u0, v0) of every sorted instance
+  // [cap_I] one 16-byte record per sorted instance, what the compositing kernels stage with a single cp.async:
+  // {u0, v0, bits(visible slot << 8 | region mask), -}: the whitened tile-local offset of the instance and its list word
+  float4* inst_rec = nullptr;
   int sorted_buf = 0;
   bool sort_attr_set = false;
 

@@ -32,7 +32,7 @@ namespace gs {
 template <int NW, bool STATS>
 __global__ void __launch_bounds__(NW * 32)
 raster_fwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order, const uint2* __restrict__ ranges,
-                  const uint32_t* __restrict__ ids, const float2* __restrict__ inst_uv, const float4* __restrict__ feat,
+                  const float4* __restrict__ inst, const float4* __restrict__ feat,
                   float bg0, float bg1, float bg2, float* __restrict__ rgb, float* __restrict__ depth,
                   float* __restrict__ alpha_out, float* __restrict__ final_T, uint32_t* __restrict__ n_contrib,
                   unsigned long long* __restrict__ stats) {
@@ -68,12 +68,12 @@ raster_fwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
   uint32_t v_pre = 0;
   auto fetch = [&](int k) {
     const int i = k * kTileBatch + e_pro;
-    v_pre = i < n ? __ldg(ids + range.x + i) : 0u;
+    v_pre = i < n ? __float_as_uint(__ldg(&inst[range.x + i].z)) : 0u;
   };
   fetch(0);
 #pragma unroll
   for (int k = 0; k < kAhead; ++k) {
-    if (k < nb) ring.produce(k, k * kTileBatch + e_pro, n, range.x, v_pre, tid, ids, inst_uv, feat);
+    if (k < nb) ring.produce(k, k * kTileBatch + e_pro, n, range.x, v_pre, tid, inst, feat);
     fetch(k + 1);
   }
   __syncthreads();  // s_live is complete
@@ -140,7 +140,7 @@ raster_fwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
           if (*live == 0) { stop = true; break; }   // the warps this one waits for have left
       }
       if (stop) break;
-      ring.produce(k, k * kTileBatch + e_pro, n, range.x, v_pre, tid, ids, inst_uv, feat);
+      ring.produce(k, k * kTileBatch + e_pro, n, range.x, v_pre, tid, inst, feat);
       fetch(k + 1);
     }
     if (*live == 0) break;  // no pixel of the CTA is alive any more
@@ -181,8 +181,7 @@ int launch_raster_fwd(gs_ctx* ctx, cudaStream_t s, float* rgb, float* depth, flo
   if (tiles == 0) return GS_OK;
   constexpr int NW = GS_FWD_WARPS;
   GS_LAUNCH_PDL((raster_fwd_kernel<NW, false>), tiles * (8 / NW), NW * 32, 0, s, ctx->cam.W, ctx->cam.H, ctx->cam.tiles_x,
-                (const uint32_t*)ctx->tile_order, (const uint2*)ctx->ranges, (const uint32_t*)ctx->vals[ctx->sorted_buf],
-                (const float2*)ctx->inst_uv, (const float4*)ctx->feat, ctx->bg[0], ctx->bg[1], ctx->bg[2], rgb, depth, alpha,
+                (const uint32_t*)ctx->tile_order, (const uint2*)ctx->ranges, (const float4*)ctx->inst_rec, (const float4*)ctx->feat, ctx->bg[0], ctx->bg[1], ctx->bg[2], rgb, depth, alpha,
                 ctx->final_T, ctx->n_contrib, (unsigned long long*)nullptr);
   GS_LAUNCH_CHECK("raster_fwd_kernel");
   return GS_OK;
@@ -196,7 +195,7 @@ int launch_workload_stats(gs_ctx* ctx, cudaStream_t s, uint64_t* out_host) {
   GS_CUDA(cudaMemsetAsync(d, 0, 8 * sizeof(unsigned long long), s));
   if (tiles > 0) {
     raster_fwd_kernel<8, true><<<tiles, 256, 0, s>>>(ctx->cam.W, ctx->cam.H, ctx->cam.tiles_x, ctx->tile_order, ctx->ranges,
-                                                     ctx->vals[ctx->sorted_buf], ctx->inst_uv, ctx->feat, 0.f, 0.f, 0.f,
+                                                     ctx->inst_rec, ctx->feat, 0.f, 0.f, 0.f,
                                                      nullptr, nullptr, nullptr, nullptr, nullptr, d);
     GS_LAUNCH_CHECK("raster_fwd_kernel<stats>");
   }

@@ -138,8 +138,7 @@ struct Ring {
   }
   // stages list entry i (valid if i < n) of the tile whose list starts at `first`, for staged round k; v = ids[first + i]
   __device__ __forceinline__ void produce(int k, int i, int n, uint32_t first, uint32_t v, int tid,
-                                          const uint32_t* __restrict__ ids, const float2* __restrict__ inst_uv,
-                                          const float4* __restrict__ feat) {
+                                          const float4* __restrict__ inst, const float4* __restrict__ feat) {
     const int stage = k & (kStages - 1), part = tid & (TPE - 1);
     StageRec& r = st[stage].rec[tid / TPE];
     if (i >= 0 && i < n) {
@@ -150,8 +149,7 @@ struct Ring {
       if (part == 0) cp_async16(&r.g, src);
       if (part == (1 & (TPE - 1))) cp_async16(&r.c, src + 1);
 #endif
-      if (part == (2 & (TPE - 1))) cp_async8(&r.uv, inst_uv + first + i);
-      if (part == (3 & (TPE - 1))) cp_async4(&r.ent, ids + first + i);
+      if (part == (2 & (TPE - 1))) cp_async16(&r.uv, inst + first + i);  // {u0, v0, list word, -}: the record's last 16 bytes
     }
     cp_async_mbar_arrive(&full[stage]);
   }

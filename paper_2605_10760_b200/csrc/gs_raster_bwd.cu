@@ -126,7 +126,7 @@ __device__ __forceinline__ void gaussian_phase(float2* s_pair, const float4* s_p
 template <int NW, bool HAS_GA>
 __global__ void __launch_bounds__(NW * 32, (GS_BWD_MIN_CTAS * 8) / NW)
 raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order, const uint2* __restrict__ ranges,
-                  const uint32_t* __restrict__ ids, const float2* __restrict__ inst_uv, const float4* __restrict__ feat,
+                  const float4* __restrict__ inst, const float4* __restrict__ feat,
                   float bg0, float bg1, float bg2, const float* __restrict__ final_T,
                   const uint32_t* __restrict__ n_contrib, const float* __restrict__ d_rgb,
                   const float* __restrict__ d_depth, const float* __restrict__ d_alpha, float* __restrict__ g2d) {
@@ -180,12 +180,12 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
   uint32_t v_pre = 0;
   auto fetch = [&](int k) {
     const int i = (nb - 1 - k) * kTileBatch + e_pro;
-    v_pre = (i >= 0 && i < n) ? __ldg(ids + range.x + i) : 0u;
+    v_pre = (i >= 0 && i < n) ? __float_as_uint(__ldg(&inst[range.x + i].z)) : 0u;
   };
   fetch(0);
 #pragma unroll
   for (int k = 0; k < kAhead; ++k) {
-    if (k < nb) ring.produce(k, (nb - 1 - k) * kTileBatch + e_pro, n, range.x, v_pre, tid, ids, inst_uv, feat);
+    if (k < nb) ring.produce(k, (nb - 1 - k) * kTileBatch + e_pro, n, range.x, v_pre, tid, inst, feat);
     fetch(k + 1);
   }
   for (int k = 0; k < nb; ++k) {  // list rounds, back to front
@@ -260,7 +260,7 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
     const int kn = k + kAhead;
     if (kn < nb) {
       if (k >= kDelay) mbar_wait(&ring.empty[kn & (kStages - 1)], (uint32_t)((k - kDelay) / kStages) & 1u);
-      ring.produce(kn, (nb - 1 - kn) * kTileBatch + e_pro, n, range.x, v_pre, tid, ids, inst_uv, feat);
+      ring.produce(kn, (nb - 1 - kn) * kTileBatch + e_pro, n, range.x, v_pre, tid, inst, feat);
       fetch(kn + 1);
     }
   }
@@ -275,8 +275,8 @@ int launch_raster_bwd(gs_ctx* ctx, cudaStream_t s, const float* d_rgb, const flo
   constexpr int NW = GS_BWD_WARPS;
 #define GS_BWD(GA)                                                                                                  \
   GS_LAUNCH_PDL((raster_bwd_kernel<NW, GA>), tiles * (8 / NW), NW * 32, 0, s, ctx->cam.W, ctx->cam.H, ctx->cam.tiles_x, \
-                (const uint32_t*)ctx->tile_order, (const uint2*)ctx->ranges, (const uint32_t*)ctx->vals[ctx->sorted_buf], \
-                (const float2*)ctx->inst_uv, (const float4*)ctx->feat, ctx->bg[0], ctx->bg[1], ctx->bg[2],               \
+                (const uint32_t*)ctx->tile_order, (const uint2*)ctx->ranges, (const float4*)ctx->inst_rec, (const float4*)ctx->feat,    \
+                ctx->bg[0], ctx->bg[1], ctx->bg[2],                                                                       \
                 (const float*)ctx->final_T, (const uint32_t*)ctx->n_contrib, d_rgb, d_depth, d_alpha, ctx->g2d)
   if (d_alpha) GS_BWD(true); else GS_BWD(false);
 #undef GS_BWD
