@@ -245,11 +245,14 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
             *pair_ptr = make_float2(gp, w);
             pair_ptr += kPairRow;
             if (lane == 0) *reinterpret_cast<float4*>(s_slot + nslot) = uv[q];
-            if (++nslot == kSlots) {
-              gaussian_phase<2>(s_pair, s_pix, s_slot, kSlots, lane, (float)xo, (float)yo, feat, g2d);
-              nslot = 0;
-              pair_ptr = s_pair + lane;
-            }
+            ++nslot;
+          }
+          // flush once per group of four entries, as soon as another group might not fit (one copy of the Gaussian phase
+          // in the instruction stream instead of four)
+          if (nslot > kSlots - kGroup) {
+            gaussian_phase<2>(s_pair, s_pix, s_slot, nslot, lane, (float)xo, (float)yo, feat, g2d);
+            nslot = 0;
+            pair_ptr = s_pair + lane;
           }
         }
       }
