@@ -226,11 +226,11 @@ def stage_models(N, K3, V, I, P, tiles, E, C, Eb, R, Rb, pose_only, dense_fill=T
         "preprocess": {"bound": "hbm", "bytes": 48 * N + (4 * K3 + 120) * V},
         "tile_scan": {"bound": "hbm", "bytes": 16.0 * tiles, "note": "latency-bound: one L2 round trip between its CTAs"},
         "emit": {"bound": "hbm", "bytes": 48 * V + 8 * I},
-        "tile_sort": {"bound": "hbm", "bytes": 24 * I, "note": "compare-exchange network in registers: integer-ALU work"},
+        "tile_sort": {"bound": "hbm", "bytes": 32 * I, "note": "compare-exchange network in registers: integer-ALU work"},
         "raster_fwd": {"bound": "alu", "flops": E * FLOP_EVAL + C * FLOP_BLEND_FWD, "lds": R * LDS_PER_ENTRY,
-                       "winst": R * WINST_PER_ENTRY_FWD, "bytes": 4 * I + 48 * V + 24 * P},
+                       "winst": R * WINST_PER_ENTRY_FWD, "bytes": 16 * I + 32 * V + 24 * P},
         "raster_bwd": {"bound": "alu", "flops": Eb * FLOP_EVAL + C * FLOP_BLEND_BWD, "lds": Rb * LDS_PER_ENTRY,
-                       "winst": Rb * WINST_PER_ENTRY_BWD, "bytes": 4 * I + 48 * V + 28 * P + 48 * V},
+                       "winst": Rb * WINST_PER_ENTRY_BWD, "bytes": 16 * I + 32 * V + 28 * P + 48 * V},
         "gauss_bwd": {"bound": "hbm", "bytes": (48 + 48 + 48 + 16 + 4 + 4 * K3) * V + gp * V + (fill * (N - V) + 4 * N if fill else 0),
                       "note": "reads g2d, parameters, SH of the V visible Gaussians, writes their gradient rows; dense mode: "
                               "+ the zero rows of the N - V culled Gaussians, cleared by the same kernel"},
