@@ -278,6 +278,19 @@ def run_ours(args):
     # --grads sparse: GS_SPARSE_GRADS (one gradient row per visible Gaussian, no dense zero fill); single-view workloads
     grad_flag = B.GS_SPARSE_GRADS if (args.grads == "sparse" and wl.views == 1) else 0
 
+    # multi-view workloads: extra (context, stream, output) sets; the gradient arrays are shared
+    n_vs = max(1, args.view_streams) if wl.views > 1 else 1
+    prof_seq = [False]  # the stage-profile loop runs the views one after the other on `ctx`
+    vctx, vstreams, vout = [ctx], [], [out]
+    if n_vs > 1:
+        vctx += [B.Context(local) for _ in range(n_vs - 1)]
+        vstreams = [torch.cuda.Stream(device=dev) for _ in range(n_vs)]
+        for _ in range(n_vs - 1):
+            o = dss[0].alloc_outputs(W, H)
+            for name in ("g_means", "g_scales", "g_quats", "g_opacities", "g_sh"):
+                o[name] = out[name]
+            vout.append(o)
+
     def step(k):
         s = k % len(dss)
         if wl.pose_only:
@@ -287,6 +300,23 @@ def run_ours(args):
             B.gs_aux_l1_grad(out["rgb"], target, 1.0 / (3 * W * H), gC_track)
             B.backward(ctx, out, gC_track, None, None, flags=B.GS_POSE_ONLY, pose=True)
             B.gs_aux_pose_step(T_dev, out["g_twist"], 1e-3)
+            return
+        if n_vs > 1 and not prof_seq[0]:
+            # views round-robin on n_vs (context, stream) pairs: the latency-bound per-Gaussian and binning kernels of one
+            # view overlap the compositing kernels of another.  All views ACCUMULATE into the zeroed gradient arrays.
+            for name in ("g_means", "g_scales", "g_quats", "g_opacities", "g_sh"):
+                out[name].zero_()
+            main = torch.cuda.current_stream()
+            fork = torch.cuda.Event(); fork.record(main)
+            for st in vstreams:
+                st.wait_event(fork)
+            for v, cam in enumerate(wl.cams[s]):
+                j = v % n_vs
+                with torch.cuda.stream(vstreams[j]):
+                    B.forward(vctx[j], dss[s], cam, vout[j])
+                    B.backward(vctx[j], vout[j], ups[s][v][0], ups[s][v][1], None, flags=B.GS_ACCUMULATE, pose=True)
+            for st in vstreams:
+                join = torch.cuda.Event(); join.record(st); main.wait_event(join)
             return
         for v, cam in enumerate(wl.cams[s]):
             B.forward(ctx, dss[s], cam, out)
@@ -305,13 +335,15 @@ def run_ours(args):
         try:
             step(k)
             torch.cuda.synchronize()
-            ctx.gs_poll()
+            for c in vctx:
+                c.gs_poll()
             k += 1
         except B.GsError as e:
             if e.code != -5:
                 raise
     # workload statistics per scene (last view of the step): V, I and the pair counts of the compositing kernels
     stats = []
+    prof_seq[0] = True
     for k in range(len(dss)):
         step(k)
         nv, ni = ctx.gs_get_counts()
@@ -319,11 +351,12 @@ def run_ours(args):
         stats.append(dict(visible=nv, instances=ni, **wlst))
     if wl.pose_only:
         T_dev.copy_(to_dev(np.asarray(wl.scenes[0].camera.T_cw, np.float32).reshape(-1)))
+    prof_seq[0] = False
     barrier()
 
     # ---- timed region: exactly K steps, device time, max over ranks ----
     K = args.steps
-    l0 = ctx.gs_get_launch_count()
+    l0 = sum(c.gs_get_launch_count() for c in vctx)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     with ClockSampler(local) as clk:
         barrier()
@@ -333,12 +366,14 @@ def run_ours(args):
         e1.record()
         barrier()
     ms_total = e0.elapsed_time(e1)
-    ctx.gs_poll()
-    launches = ctx.gs_get_launch_count() - l0
+    for c in vctx:
+        c.gs_poll()
+    launches = sum(c.gs_get_launch_count() for c in vctx) - l0
     ms_total = max_over_ranks(ms_total, dist, dev)
     value = replica_throughput(world, K, ms_total)
 
     # ---- per-stage device times (second loop, stage events on; same steps; last view of each step) ----
+    prof_seq[0] = True
     ctx.gs_profile_enable(True)
     stage_ms = {s: 0.0 for s in B.STAGES}
     for k in range(K):
@@ -416,7 +451,7 @@ def run_ours(args):
                 "value": value, "unit": "iter/s", "n_gpus": world, "steps": K, "warmup": warm,
                 "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f32", "data": "synthetic", "config": config_dict(wl, world),
-                "views_per_iter": wl.views, "grads": "sparse" if grad_flag else "dense", "mpix_iter_per_s": value * wl.views * W * H / 1e6,
+                "views_per_iter": wl.views, "view_streams": n_vs, "grads": "sparse" if grad_flag else "dense", "mpix_iter_per_s": value * wl.views * W * H / 1e6,
                 "clocks": clk.summary(), "e2e": e2e, "gpu_launches": launches, "roofline": roof,
                 "roofline_stages": roof_stages, "cpu_baseline": cpu,
                 "hbm_frac_whole_iteration": hbm_frac_iter, "algorithmic_bytes_per_iter": bytes_iter,
@@ -548,6 +583,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="replica300k")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--view-streams", type=int, default=4,
+                    help="multi-view workloads (fused2m): views of one iteration are issued round-robin on this many "
+                         "context + stream pairs; GS_ACCUMULATE adds with L2 reductions, so concurrent views are safe")
     ap.add_argument("--grads", default="dense", choices=["dense", "sparse"],
                     help="dense (default, the headline): (11 + 3K) N gradient arrays; sparse: GS_SPARSE_GRADS rows of the visible Gaussians")
     args = ap.parse_args()

@@ -65,7 +65,8 @@ typedef struct gs_ctx gs_ctx; /* opaque */
 
 /* flags of gs_rasterize_bwd / gs_pose_grad */
 #define GS_ACCUMULATE 1u /* parameter gradients are added to the output arrays instead of overwriting them (config 5);
-                            the addition is one fp32 RED.ADD per element at L2 (a denormal sum is flushed to zero) */
+                            the addition is one fp32 RED.ADD per element at L2 (a denormal sum is flushed to zero), so
+                            several contexts on different streams may accumulate into the same arrays concurrently */
 #define GS_POSE_ONLY 2u  /* Gaussians frozen: no parameter gradients are written; output pointers may be NULL (config 4) */
 #define GS_SPARSE_GRADS 4u /* parameter gradients are written COMPACT: row r of every g_* array belongs to the Gaussian
                             gs_visible_ids()[r], r < n_visible (arrays need n_visible <= N rows); rows of culled Gaussians do

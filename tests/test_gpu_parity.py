@@ -238,6 +238,48 @@ def test_config5_fused_two_views_accumulate(oracle, gpu):
         assert rel_l2(out[k].cpu().numpy(), acc[k]) <= TOL_GRAD, k
 
 
+def test_config5_views_accumulate_concurrently_on_two_contexts(oracle, gpu):
+    """GS_ACCUMULATE adds with one fp32 reduction per element at L2, so the views of one refinement iteration may run
+    CONCURRENTLY on separate (context, stream) pairs into the same zeroed gradient arrays (bench.py --view-streams): four
+    views round-robin on two contexts / streams, sum compared with the oracle's."""
+    sc, cams = scenes.fused_scene(seed=50, N_sub=40_000, views=4, width=400, height=230, f=200.0)
+    b, torch = gpu.binding, gpu.torch
+    ds = b.DeviceScene(sc)
+    names = ("g_means", "g_scales", "g_quats", "g_opacities", "g_sh")
+    ctxs = [gpu.ctx, b.Context(0)]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    outs = [ds.alloc_outputs(400, 230), ds.alloc_outputs(400, 230)]
+    for k in names:
+        outs[1][k] = outs[0][k]
+    acc, ups = None, []
+    for v, cam in enumerate(cams):
+        gC, gD = scenes.upstream_gradients(50 + v, 400, 230)
+        r = oracle.forward_backward(sc, gC, gD, camera=cam)
+        acc = {k: r[k].copy() for k in names} if acc is None else {k: acc[k] + r[k] for k in acc}
+        ups.append((torch.from_numpy(gC).cuda(), torch.from_numpy(gD).cuda()))
+    for attempt in range(4):   # a view that outgrows its context's instance capacity is reported once and re-issued
+        try:
+            for k in names:
+                outs[0][k].zero_()
+            torch.cuda.synchronize()
+            for v, cam in enumerate(cams):
+                j = v % 2
+                with torch.cuda.stream(streams[j]):
+                    b.forward(ctxs[j], ds, cam, outs[j])
+                    b.backward(ctxs[j], outs[j], ups[v][0], ups[v][1], None, flags=b.GS_ACCUMULATE, pose=False)
+            torch.cuda.synchronize()
+            for c in ctxs:
+                c.gs_poll()
+            break
+        except b.GsError as e:
+            torch.cuda.synchronize()
+            if e.code != -5 or attempt == 3:
+                raise
+    ctxs[1].close()
+    for k in acc:
+        assert rel_l2(outs[0][k].cpu().numpy(), acc[k]) <= TOL_GRAD, k
+
+
 def test_config5_fused_full_size_two_views(oracle, gpu):
     """Config 5 at FULL size (2 M Gaussians = 4 Sim(3)-mapped submaps, 1200x680, SH3), two of the eight views: features,
     bit-exact binning, image, and the gradients -- including the twist -- accumulated over the views with GS_ACCUMULATE
