@@ -95,6 +95,12 @@ GS_API const char* gs_last_error(const gs_ctx* ctx);
  *   gs_get_binning's tile_ranges delimit the shorter lists and the entries between a list's end and the next list's
  *   start are unspecified. */
 #define GS_OPT_EXACT_TILE_CULL 1
+/*   GS_OPT_VIEW_STREAMS (default 1, 1..8): gs_refine_views issues its views round-robin on this context and on
+ *     value - 1 context-owned sub-contexts with their own streams (forked from and joined to the caller's stream by
+ *     events); every view then ACCUMULATES into gradient arrays zeroed up front.  The latency-bound per-Gaussian and
+ *     binning kernels of one view overlap the compositing kernels of another (config 5: 164 -> 195 eight-view it/s at 4).
+ *     Each sub-context holds its own scratch (about 250 bytes per Gaussian + 50 bytes per tile instance). */
+#define GS_OPT_VIEW_STREAMS 2
 GS_API int gs_set_option(gs_ctx* ctx, int option, int value);
 
 /* Step a1 -- EWA projection, conic, screen extent, colour (oracle reading C1 steps 1-6, 8).
@@ -307,7 +313,8 @@ GS_API int gs_compact_rows(void* stream, int64_t N, int32_t width, const uint32_
  *   batch (HOST struct): cams HOST [n_views]; T_cw_dev NULL or DEVICE [n_views,12] poses that override the cams' (pose
  *     deltas applied on the device); target_rgb DEVICE [n_views,3,H,W]; target_depth DEVICE [n_views,H,W]; normal_prior NULL
  *     or DEVICE [n_views,3,H,W]; ab DEVICE [n_views,2]; the weights of Eq. 23 (paper: 1.75, 0.2, 0.25; lambda_n garbled, Q16).
- *   grads      DEVICE arrays of the parameter shapes: sum over the views of dL_k/dparam (written by view 0, accumulated after)
+ *   grads      DEVICE arrays of the parameter shapes: sum over the views of dL_k/dparam (written by view 0, accumulated after;
+ *              with GS_OPT_VIEW_STREAMS > 1: zeroed first, accumulated by all views in whatever order they finish)
  *   g_twist    DEVICE [n_views,6]; g_ab DEVICE [n_views,2]
  *   loss       DEVICE double [n_views,10]: the eight entries of gs_loss_refine, then lambda_n L_normal and a scratch word
  *   visible    NULL or DEVICE uint32[N]: 1 where the Gaussian was on screen in at least one view (the mask of gs_adam_step)

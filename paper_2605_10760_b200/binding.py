@@ -27,6 +27,7 @@ EXPORTS = ["gs_create", "gs_destroy", "gs_last_error", "gs_preprocess", "gs_bin_
            "gs_voxel_insert_rays", "gs_voxel_retain", "gs_adam_step", "gs_prune_mask", "gs_compact_work_bytes",
            "gs_compact_plan", "gs_compact_rows", "gs_loss_normal", "gs_set_option", "gs_refine_views", "gs_visible_ids", "gs_adam_step_sparse", "gs_get_visible_ids"]
 GS_OPT_EXACT_TILE_CULL = 1
+GS_OPT_VIEW_STREAMS = 2
 PEAKS = ["fma_tlanes", "issue_twarp", "ex2_tlanes", "lds128_bcast_twarp", "lds128_twarp", "lds32_bcast_twarp",
          "lds64_bcast_twarp", "red_glanes", "hbm_read_gbs", "hbm_write_gbs", "hbm_copy_gbs", "sm_count", "sm_mhz_max"]
 STAGES = ["preprocess", "tile_scan", "emit", "tile_sort", "raster_fwd", "raster_bwd", "gauss_bwd", "pose_grad"]

@@ -127,10 +127,11 @@ static int alloc_header(gs_ctx* ctx, int64_t tiles) {
   return GS_OK;
 }
 
-// visible[i] = (first ? 0 : visible[i]) | (tiles_touched[i] > 0): which Gaussians were on screen in any view so far
-__global__ void visible_or_kernel(int64_t N, const uint32_t* __restrict__ tiles_touched, uint32_t* __restrict__ visible, bool first) {
+// visible[i] = 1 where the Gaussian was on screen in this view (the mask is zeroed before the first view; every writer
+// writes the same 1, so views on different streams may run this at the same time)
+__global__ void visible_or_kernel(int64_t N, const uint32_t* __restrict__ tiles_touched, uint32_t* __restrict__ visible) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < N) visible[i] = (first ? 0u : visible[i]) | (tiles_touched[i] > 0u ? 1u : 0u);
+  if (i < N && tiles_touched[i] > 0u) visible[i] = 1u;
 }
 
 static int ensure_image_capacity(gs_ctx* ctx, int64_t tiles, int64_t pix) {
@@ -188,6 +189,12 @@ int gs_destroy(gs_ctx* ctx) {
   if (!ctx) return GS_E_INVALID;
   cudaSetDevice(ctx->device);
   cudaDeviceSynchronize();
+  for (int k = 0; k < 7; ++k) {
+    if (ctx->sub[k]) gs_destroy(ctx->sub[k]);
+    if (ctx->sub_stream[k]) cudaStreamDestroy(ctx->sub_stream[k]);
+    if (ctx->ev_view_join[k]) cudaEventDestroy(ctx->ev_view_join[k]);
+  }
+  if (ctx->ev_view_fork) cudaEventDestroy(ctx->ev_view_fork);
   cudaFree(ctx->feat); cudaFree(ctx->tiles_touched); cudaFree(ctx->vis_ids); cudaFree(ctx->vis_rec); cudaFree(ctx->vis_par); cudaFree(ctx->slot_of);
   cudaFree(ctx->g2d);
   for (int b = 0; b < 2; ++b) cudaFree(ctx->keys[b]);
@@ -226,7 +233,16 @@ int gs_get_visible_ids(gs_ctx* ctx, void* stream, uint32_t* ids_out) {
 
 int gs_set_option(gs_ctx* ctx, int option, int value) {
   if (!ctx) return GS_E_INVALID;
-  if (option == GS_OPT_EXACT_TILE_CULL) { ctx->opt_exact_cull = value != 0; return GS_OK; }
+  if (option == GS_OPT_EXACT_TILE_CULL) {
+    ctx->opt_exact_cull = value != 0;
+    for (gs_ctx* c : ctx->sub) if (c) c->opt_exact_cull = value != 0;
+    return GS_OK;
+  }
+  if (option == GS_OPT_VIEW_STREAMS) {
+    if (value < 1 || value > 8) return fail(ctx, GS_E_INVALID, "gs_set_option: GS_OPT_VIEW_STREAMS takes 1..8");
+    ctx->opt_view_streams = value;
+    return GS_OK;
+  }
   return fail(ctx, GS_E_INVALID, "gs_set_option: unknown option");
 }
 
@@ -461,40 +477,86 @@ int gs_refine_views(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, const g
   cudaStream_t s = (cudaStream_t)stream;
   GS_CUDA(cudaSetDevice(ctx->device));
   const int64_t P = (int64_t)W * H;
-  if (18 * P > ctx->rv_floats) {   // rendered rgb (3), depth, alpha, d_rgb (3), d_depth, SSIM scratch (9)
-    GS_CUDA(cudaDeviceSynchronize());
-    int rc = grow(ctx, ctx->rv, 18 * P);
-    if (rc != GS_OK) { ctx->rv_floats = 0; return rc; }
-    ctx->rv_floats = 18 * P;
+  // GS_OPT_VIEW_STREAMS > 1: the views run round-robin on this context (caller's stream) and on S - 1 sub-contexts with
+  // their own streams; every view ACCUMULATES (one L2 reduction per element) into gradient arrays zeroed up front, so the
+  // order in which the views finish does not matter.  S == 1: view 0 writes, the others accumulate, all on `stream`.
+  const int S = std::min(ctx->opt_view_streams, batch->n_views);
+  for (int k = 0; k + 1 < S; ++k) {
+    if (!ctx->sub[k]) {
+      int rc = gs_create(&ctx->sub[k], ctx->device);
+      if (rc != GS_OK) return fail(ctx, rc, "gs_refine_views: could not create a sub-context");
+      ctx->sub[k]->opt_exact_cull = ctx->opt_exact_cull;
+      GS_CUDA(cudaStreamCreateWithFlags(&ctx->sub_stream[k], cudaStreamNonBlocking));
+      GS_CUDA(cudaEventCreateWithFlags(&ctx->ev_view_join[k], cudaEventDisableTiming));
+    }
   }
-  float *rgb = ctx->rv, *depth = rgb + 3 * P, *alpha = depth + P, *d_rgb = alpha + P, *d_depth = d_rgb + 3 * P, *work = d_depth + P;
-  for (int v = 0; v < batch->n_views; ++v) {
+  if (S > 1 && !ctx->ev_view_fork) GS_CUDA(cudaEventCreateWithFlags(&ctx->ev_view_fork, cudaEventDisableTiming));
+  for (int k = 0; k < S; ++k) {
+    gs_ctx* c = k == 0 ? ctx : ctx->sub[k - 1];
+    if (18 * P > c->rv_floats) {   // rendered rgb (3), depth, alpha, d_rgb (3), d_depth, SSIM scratch (9)
+      GS_CUDA(cudaDeviceSynchronize());
+      int rc = grow(c, c->rv, 18 * P);
+      if (rc != GS_OK) { c->rv_floats = 0; return fail(ctx, rc, "gs_refine_views: out of memory"); }
+      c->rv_floats = 18 * P;
+    }
+  }
+  if (visible && N > 0) GS_CUDA(cudaMemsetAsync(visible, 0, (size_t)N * sizeof(uint32_t), s));
+  if (S > 1) {
+    const int64_t K3 = 3 * (int64_t)(sh_degree + 1) * (sh_degree + 1);
+    if (N > 0) {
+      GS_CUDA(cudaMemsetAsync(grads->means, 0, (size_t)N * 3 * sizeof(float), s));
+      GS_CUDA(cudaMemsetAsync(grads->scales, 0, (size_t)N * 3 * sizeof(float), s));
+      GS_CUDA(cudaMemsetAsync(grads->quats, 0, (size_t)N * 4 * sizeof(float), s));
+      GS_CUDA(cudaMemsetAsync(grads->opacities, 0, (size_t)N * sizeof(float), s));
+      GS_CUDA(cudaMemsetAsync(grads->sh, 0, (size_t)N * K3 * sizeof(float), s));
+    }
+    GS_CUDA(cudaEventRecord(ctx->ev_view_fork, s));
+    for (int k = 0; k + 1 < S; ++k) GS_CUDA(cudaStreamWaitEvent(ctx->sub_stream[k], ctx->ev_view_fork, 0));
+  }
+  int rc_all = GS_OK;
+  for (int v = 0; v < batch->n_views && rc_all == GS_OK; ++v) {
+    const int k = v % S;
+    gs_ctx* c = k == 0 ? ctx : ctx->sub[k - 1];
+    cudaStream_t vs = k == 0 ? s : ctx->sub_stream[k - 1];
+    void* vstream = (void*)vs;
+    float *rgb = c->rv, *depth = rgb + 3 * P, *alpha = depth + P, *d_rgb = alpha + P, *d_depth = d_rgb + 3 * P, *work = d_depth + P;
     int rc;
-    const float* T_dev = batch->T_cw_dev ? batch->T_cw_dev + 12 * v : nullptr;
-    if ((rc = gs_preprocess(ctx, stream, N, sh_degree, params->means, params->scales, params->quats, params->opacities,
-                            params->sh, &batch->cams[v], T_dev)) != GS_OK) return rc;
-    if ((rc = gs_bin_tiles(ctx, stream)) != GS_OK) return rc;
-    if ((rc = gs_rasterize_fwd(ctx, stream, bg, rgb, depth, alpha)) != GS_OK) return rc;
-    double* lv = loss + 10 * v;
-    if ((rc = gs_loss_refine(stream, W, H, rgb, depth, batch->target_rgb + 3 * P * v, batch->target_depth + P * v,
-                             batch->ab + 2 * v, batch->alpha_p, batch->lambda, batch->beta, d_rgb, d_depth, g_ab + 2 * v, work,
-                             lv)) != GS_OK) return fail(ctx, rc, "gs_refine_views: gs_loss_refine failed");
-    if (batch->normal_prior) {
-      const gs_camera& c = batch->cams[v];
-      if ((rc = gs_loss_normal(stream, W, H, c.fx, c.fy, c.cx, c.cy, depth, batch->normal_prior + 3 * P * v, batch->lambda_n,
-                               nullptr, d_depth, lv + 8)) != GS_OK) return fail(ctx, rc, "gs_refine_views: gs_loss_normal failed");
-    } else {
-      GS_CUDA(cudaMemsetAsync(lv + 8, 0, 2 * sizeof(double), s));
-    }
-    if ((rc = gs_rasterize_bwd(ctx, stream, d_rgb, d_depth, nullptr, v > 0 ? GS_ACCUMULATE : 0u, grads->means, grads->scales,
-                               grads->quats, grads->opacities, grads->sh)) != GS_OK) return rc;
-    if ((rc = gs_pose_grad(ctx, stream, 0u, g_twist + 6 * v)) != GS_OK) return rc;
-    if (visible && N > 0) {
-      visible_or_kernel<<<(unsigned)div_up(N, 256), 256, 0, s>>>(N, ctx->tiles_touched, visible, v == 0);
-      GS_LAUNCH_CHECK("visible_or_kernel");
-    }
+    auto view = [&]() -> int {
+      const float* T_dev = batch->T_cw_dev ? batch->T_cw_dev + 12 * v : nullptr;
+      if ((rc = gs_preprocess(c, vstream, N, sh_degree, params->means, params->scales, params->quats, params->opacities,
+                              params->sh, &batch->cams[v], T_dev)) != GS_OK) return rc;
+      if ((rc = gs_bin_tiles(c, vstream)) != GS_OK) return rc;
+      if ((rc = gs_rasterize_fwd(c, vstream, bg, rgb, depth, alpha)) != GS_OK) return rc;
+      double* lv = loss + 10 * v;
+      if ((rc = gs_loss_refine(vstream, W, H, rgb, depth, batch->target_rgb + 3 * P * v, batch->target_depth + P * v,
+                               batch->ab + 2 * v, batch->alpha_p, batch->lambda, batch->beta, d_rgb, d_depth, g_ab + 2 * v, work,
+                               lv)) != GS_OK) return fail(c, rc, "gs_refine_views: gs_loss_refine failed");
+      if (batch->normal_prior) {
+        const gs_camera& cm = batch->cams[v];
+        if ((rc = gs_loss_normal(vstream, W, H, cm.fx, cm.fy, cm.cx, cm.cy, depth, batch->normal_prior + 3 * P * v, batch->lambda_n,
+                                 nullptr, d_depth, lv + 8)) != GS_OK) return fail(c, rc, "gs_refine_views: gs_loss_normal failed");
+      } else {
+        if (cudaMemsetAsync(lv + 8, 0, 2 * sizeof(double), vs) != cudaSuccess) return GS_E_CUDA;
+      }
+      if ((rc = gs_rasterize_bwd(c, vstream, d_rgb, d_depth, nullptr, (S > 1 || v > 0) ? GS_ACCUMULATE : 0u, grads->means,
+                                 grads->scales, grads->quats, grads->opacities, grads->sh)) != GS_OK) return rc;
+      if ((rc = gs_pose_grad(c, vstream, 0u, g_twist + 6 * v)) != GS_OK) return rc;
+      if (visible && N > 0) {
+        visible_or_kernel<<<(unsigned)div_up(N, 256), 256, 0, vs>>>(N, c->tiles_touched, visible);
+        if (cudaGetLastError() != cudaSuccess) return GS_E_CUDA;
+        c->launches++;
+      }
+      return GS_OK;
+    };
+    rc_all = view();
+    if (rc_all != GS_OK && c != ctx) snprintf(ctx->err, sizeof(ctx->err), "%s", c->err);
   }
-  return GS_OK;
+  // join: the caller's stream waits for the sub-streams (also after an error, so that nothing is left running unordered)
+  for (int k = 0; k + 1 < S; ++k) {
+    GS_CUDA(cudaEventRecord(ctx->ev_view_join[k], ctx->sub_stream[k]));
+    GS_CUDA(cudaStreamWaitEvent(s, ctx->ev_view_join[k], 0));
+  }
+  return rc_all;
 }
 
 int gs_fwd_bwd_host(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, const float* means, const float* scales,

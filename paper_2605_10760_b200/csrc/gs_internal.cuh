@@ -150,6 +150,12 @@ struct gs_ctx {
 
   uint32_t* tile_order = nullptr;      // [tiles] tile ids by descending list length (longest lists are scheduled first)
   bool opt_exact_cull = false;         // GS_OPT_EXACT_TILE_CULL (gs_set_option)
+  // GS_OPT_VIEW_STREAMS (gs_set_option): gs_refine_views issues its views round-robin on this context and on
+  // opt_view_streams - 1 context-owned sub-contexts with their own streams (created on first use)
+  int opt_view_streams = 1;
+  gs_ctx* sub[7] = {};
+  cudaStream_t sub_stream[7] = {};
+  cudaEvent_t ev_view_fork = nullptr, ev_view_join[7] = {};
 
   // side stream: the block-wide sort of the few long tile lists runs beside the warp-level sort of the rest
   cudaStream_t side_stream = nullptr;

@@ -15,8 +15,8 @@ def _rel(a, b):
     return np.linalg.norm(a - b) / n if n > 0 else np.linalg.norm(a - b)
 
 
-@pytest.mark.parametrize("with_normals", [False, True])
-def test_refine_views_matches_the_composed_oracles(oracle, with_normals):
+@pytest.mark.parametrize("with_normals,view_streams", [(False, 1), (True, 1), (True, 2), (False, 3)])
+def test_refine_views_matches_the_composed_oracles(oracle, with_normals, view_streams):
     import torch
     from oracle import loss as ol, normals as on
     from paper_2605_10760_b200 import binding as b
@@ -46,6 +46,8 @@ def test_refine_views_matches_the_composed_oracles(oracle, with_normals):
         tw.append(g["g_twist"]); gab.append([lo["g_a"], lo["g_b"]]); losses.append([lo["l1_rgb"], lo["ssim"], lo["l1_depth"], lo["total"], wts[3] * ln])
     # GPU: one call
     ctx = b.Context(0)
+    # view_streams > 1: the views run concurrently on sub-contexts / streams and all ACCUMULATE into zeroed arrays
+    ctx.gs_set_option(b.GS_OPT_VIEW_STREAMS, view_streams)
     ds = b.DeviceScene(sc)
     params = dict(means=ds.means, scales=ds.scales, quats=ds.quats, opacities=ds.opacities, sh=ds.sh)
     grads = {k: torch.full_like(t, 3.0) for k, t in params.items()}      # view 0 overwrites whatever is there
