@@ -280,6 +280,10 @@ def run_ours(args):
 
     # multi-view workloads: extra (context, stream, output) sets; the gradient arrays are shared
     n_vs = max(1, args.view_streams) if wl.views > 1 else 1
+    n_is = max(1, args.iter_streams) if (wl.views == 1 and not wl.pose_only) else 1
+    ictx = [ctx] + [B.Context(local) for _ in range(n_is - 1)]
+    istreams = [torch.cuda.Stream(device=dev) for _ in range(n_is)] if n_is > 1 else []
+    iout = [out] + [dss[0].alloc_outputs(W, H) for _ in range(n_is - 1)]
     prof_seq = [False]  # the stage-profile loop runs the views one after the other on `ctx`
     vctx, vstreams, vout = [ctx], [], [out]
     if n_vs > 1:
@@ -300,6 +304,12 @@ def run_ours(args):
             B.gs_aux_l1_grad(out["rgb"], target, 1.0 / (3 * W * H), gC_track)
             B.backward(ctx, out, gC_track, None, None, flags=B.GS_POSE_ONLY, pose=True)
             B.gs_aux_pose_step(T_dev, out["g_twist"], 1e-3)
+            return
+        if n_is > 1 and not prof_seq[0]:
+            j = k % n_is
+            with torch.cuda.stream(istreams[j]):
+                B.forward(ictx[j], dss[s], wl.cams[s][0], iout[j])
+                B.backward(ictx[j], iout[j], ups[s][0][0], ups[s][0][1], None, flags=grad_flag, pose=True)
             return
         if n_vs > 1 and not prof_seq[0]:
             # views round-robin on n_vs (context, stream) pairs: the latency-bound per-Gaussian and binning kernels of one
@@ -335,7 +345,7 @@ def run_ours(args):
         try:
             step(k)
             torch.cuda.synchronize()
-            for c in vctx:
+            for c in vctx + ictx[1:]:
                 c.gs_poll()
             k += 1
         except B.GsError as e:
@@ -356,19 +366,26 @@ def run_ours(args):
 
     # ---- timed region: exactly K steps, device time, max over ranks ----
     K = args.steps
-    l0 = sum(c.gs_get_launch_count() for c in vctx)
+    l0 = sum(c.gs_get_launch_count() for c in vctx + ictx[1:])
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     with ClockSampler(local) as clk:
         barrier()
         e0.record()
+        if n_is > 1:   # the iteration streams start behind e0 and are joined in front of e1
+            fk = torch.cuda.Event(); fk.record()
+            for st in istreams:
+                st.wait_event(fk)
         for k in range(K):
             step(k)
+        if n_is > 1:
+            for st in istreams:
+                jn = torch.cuda.Event(); jn.record(st); torch.cuda.current_stream().wait_event(jn)
         e1.record()
         barrier()
     ms_total = e0.elapsed_time(e1)
-    for c in vctx:
+    for c in vctx + ictx[1:]:
         c.gs_poll()
-    launches = sum(c.gs_get_launch_count() for c in vctx) - l0
+    launches = sum(c.gs_get_launch_count() for c in vctx + ictx[1:]) - l0
     ms_total = max_over_ranks(ms_total, dist, dev)
     value = replica_throughput(world, K, ms_total)
 
@@ -451,7 +468,7 @@ def run_ours(args):
                 "value": value, "unit": "iter/s", "n_gpus": world, "steps": K, "warmup": warm,
                 "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f32", "data": "synthetic", "config": config_dict(wl, world),
-                "views_per_iter": wl.views, "view_streams": n_vs, "grads": "sparse" if grad_flag else "dense", "mpix_iter_per_s": value * wl.views * W * H / 1e6,
+                "views_per_iter": wl.views, "view_streams": n_vs, "iter_streams": n_is, "grads": "sparse" if grad_flag else "dense", "mpix_iter_per_s": value * wl.views * W * H / 1e6,
                 "clocks": clk.summary(), "e2e": e2e, "gpu_launches": launches, "roofline": roof,
                 "roofline_stages": roof_stages, "cpu_baseline": cpu,
                 "hbm_frac_whole_iteration": hbm_frac_iter, "algorithmic_bytes_per_iter": bytes_iter,
@@ -583,6 +600,10 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="replica300k")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--iter-streams", type=int, default=1,
+                    help="single-view workloads: issue consecutive (independent) iterations round-robin on this many "
+                         "context + stream pairs, e.g. the maps of several agents optimised on one GPU; default 1 = the "
+                         "headline number, one iteration after the other")
     ap.add_argument("--view-streams", type=int, default=4,
                     help="multi-view workloads (fused2m): views of one iteration are issued round-robin on this many "
                          "context + stream pairs; GS_ACCUMULATE adds with L2 reductions, so concurrent views are safe")
