@@ -14,7 +14,7 @@ namespace gs {
 // Persistent CTAs of 128 threads.  Two phases (evidence: profiles/r2_stages.md -- with one thread per Gaussian doing
 // everything, the third of the Gaussians that is visible was spread evenly over every warp: the fp64 projection chain, the
 // SH evaluation and the record writes ran at 18 of 32 lanes, and every thread walked its own 192-byte SH row):
-//   CULL   one thread per Gaussian of a 128-chunk: a cheap fp32 test that can only err on the side of keeping (behind the
+//   CULL   U (1, 2 or 4) Gaussians per thread and round, all their loads in flight at once: a cheap fp32 test that can only err on the side of keeping (behind the
 //          near plane with a rounding margin; opacity < 1/255, exact; a bound of the footprint -- rho sqrt(s_max^2 |J|_F^2
 //          + 0.3), which dominates both half widths of the exact extent -- that misses the image).  Survivors are appended
 //          to a queue in shared memory; the rest get tiles_touched = 0 and are done.
