@@ -26,6 +26,14 @@ namespace gs {
 #ifndef GS_FWD_WARPS
 #define GS_FWD_WARPS 4
 #endif
+#ifndef GS_FWD_RING_STAGES
+#define GS_FWD_RING_STAGES 8
+#endif
+#ifndef GS_FWD_RING_DELAY
+#define GS_FWD_RING_DELAY 5
+#endif
+constexpr int kStages = GS_FWD_RING_STAGES, kDelay = GS_FWD_RING_DELAY, kAhead = kStages - kDelay;  // gs_raster.cuh
+static_assert(kDelay >= 0 && kAhead >= 2, "ring shape");
 
 // STATS = true: the same walk with the same decisions, counting the workload instead of writing the image
 // (gs_get_workload; never on the timed path).
@@ -37,8 +45,8 @@ raster_fwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
                   float* __restrict__ alpha_out, float* __restrict__ final_T, uint32_t* __restrict__ n_contrib,
                   unsigned long long* __restrict__ stats) {
   constexpr int CPT = 8 / NW;  // CTAs per tile
-  constexpr int TPE = Ring<NW>::TPE;
-  __shared__ __align__(16) Ring<NW> ring;
+  constexpr int TPE = Ring<NW, kStages>::TPE;
+  __shared__ __align__(16) Ring<NW, kStages> ring;
   // per warp: byte offsets (into the stage) of the round's relevant entries, in list order
   __shared__ __align__(8) uint16_t s_idx[NW][kTileBatch + kGroup];
   __shared__ int s_live;  // warps of the CTA that still have a live pixel: staging stops when it reaches zero

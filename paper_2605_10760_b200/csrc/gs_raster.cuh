@@ -18,18 +18,12 @@ namespace gs {
 constexpr unsigned kFull = 0xffffffffu;
 constexpr int kGroup = 4;        // relevant entries evaluated together in the pixel loop
 constexpr int kTileBatch = 64;   // list entries staged per round by a CTA
-#ifndef GS_RING_STAGES
-#define GS_RING_STAGES 4
-#endif
-#ifndef GS_RING_DELAY
-#define GS_RING_DELAY 2
-#endif
-constexpr int kStages = GS_RING_STAGES;  // staging ring depth (power of two)
-// A warp that has finished round j refills the stage of round j - kDelay (with round j - kDelay + kStages): the warps of a
-// CTA may be up to kDelay + 1 rounds apart before one waits for another, and kStages - kDelay rounds are in flight.
-constexpr int kDelay = GS_RING_DELAY;
-constexpr int kAhead = kStages - kDelay;
-static_assert((kStages & (kStages - 1)) == 0 && kDelay >= 0 && kAhead >= 2, "ring shape");
+// Staging ring shape: STAGES stages (a power of two) of 64 entries.  A warp that has finished round j refills the stage of
+// round j - DELAY (with round j - DELAY + STAGES): the warps of a CTA may be up to DELAY + 1 rounds apart before one waits
+// for another, and STAGES - DELAY rounds are in flight.  The two compositing kernels choose differently (each defines
+// kStages / kDelay / kAhead in its own translation unit): the forward is short of nothing but issue slots and takes 8
+// stages with 5 rounds of slack between its warps (4 / 2 -> 8 / 5: 61.9 -> 57.7 us); the backward pays for shared memory
+// with a CTA of occupancy and stays at 4 / 2 (8 / 2: 141.5 -> 154.3 us, profiles/r2_v9_ring.md).
 constexpr int kPadIdx = kTileBatch;  // index of the stage's padding record (never passes: lo = -inf)
 
 // One staged list entry (48 B): what the pixel loops read as broadcast LDS.128 x 2 + LDS.64.
@@ -118,8 +112,9 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
 // empty[stage]; there is NO block-wide barrier in the loop: warps of different regions, which find different numbers of
 // relevant entries per round, drift up to kDelay + 1 rounds apart (the per-round __syncthreads of v7 held 19-25 % of the
 // stall samples of both kernels).
-template <int NW>
+template <int NW, int kStages>
 struct Ring {
+  static_assert((kStages & (kStages - 1)) == 0, "ring depth must be a power of two");
   static constexpr int T = NW * 32, TPE = T / kTileBatch;  // threads per staged entry: 1, 2 or 4
   static_assert(TPE == 1 || TPE == 2 || TPE == 4, "2, 4 or 8 warps");
   StageBuf st[kStages];

@@ -21,6 +21,14 @@
 
 namespace gs {
 
+#ifndef GS_BWD_RING_STAGES
+#define GS_BWD_RING_STAGES 4
+#endif
+#ifndef GS_BWD_RING_DELAY
+#define GS_BWD_RING_DELAY 2
+#endif
+constexpr int kStages = GS_BWD_RING_STAGES, kDelay = GS_BWD_RING_DELAY, kAhead = kStages - kDelay;  // gs_raster.cuh
+static_assert(kDelay >= 0 && kAhead >= 2, "ring shape");
 #ifndef GS_BWD_MIN_CTAS
 #define GS_BWD_MIN_CTAS 3
 #endif
@@ -131,8 +139,8 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
                   const uint32_t* __restrict__ n_contrib, const float* __restrict__ d_rgb,
                   const float* __restrict__ d_depth, const float* __restrict__ d_alpha, float* __restrict__ g2d) {
   constexpr int CPT = 8 / NW;  // CTAs per tile
-  constexpr int TPE = Ring<NW>::TPE;
-  __shared__ __align__(16) Ring<NW> ring;  // staging ring (gs_raster.cuh): no block-wide barrier in the loop
+  constexpr int TPE = Ring<NW, kStages>::TPE;
+  __shared__ __align__(16) Ring<NW, kStages> ring;  // staging ring (gs_raster.cuh): no block-wide barrier in the loop
   // per warp: byte offsets (into the stage) of the round's relevant entries, back to front
   __shared__ __align__(8) uint16_t s_idx[NW][kTileBatch + kGroup];
   __shared__ __align__(16) float2 s_pair_all[NW][kSlots * kPairRow];
