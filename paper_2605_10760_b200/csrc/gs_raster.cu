@@ -27,11 +27,15 @@ namespace gs {
 #define GS_FWD_WARPS 4
 #endif
 #ifndef GS_FWD_RING_STAGES
-#define GS_FWD_RING_STAGES 8
+#define GS_FWD_RING_STAGES 4
 #endif
 #ifndef GS_FWD_RING_DELAY
-#define GS_FWD_RING_DELAY 5
+#define GS_FWD_RING_DELAY 2
 #endif
+#ifndef GS_FWD_BATCH
+#define GS_FWD_BATCH 128
+#endif
+constexpr int kTileBatch = GS_FWD_BATCH, kPadIdx = kTileBatch;  // list entries staged per round by a CTA; padding record
 constexpr int kStages = GS_FWD_RING_STAGES, kDelay = GS_FWD_RING_DELAY, kAhead = kStages - kDelay;  // gs_raster.cuh
 static_assert(kDelay >= 0 && kAhead >= 2, "ring shape");
 
@@ -45,8 +49,8 @@ raster_fwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
                   float* __restrict__ alpha_out, float* __restrict__ final_T, uint32_t* __restrict__ n_contrib,
                   unsigned long long* __restrict__ stats) {
   constexpr int CPT = 8 / NW;  // CTAs per tile
-  constexpr int TPE = Ring<NW, kStages>::TPE;
-  __shared__ __align__(16) Ring<NW, kStages> ring;
+  constexpr int TPE = Ring<NW, kStages, kTileBatch>::TPE;
+  __shared__ __align__(16) Ring<NW, kStages, kTileBatch> ring;
   // per warp: byte offsets (into the stage) of the round's relevant entries, in list order
   __shared__ __align__(8) uint16_t s_idx[NW][kTileBatch + kGroup];
   __shared__ int s_live;  // warps of the CTA that still have a live pixel: staging stops when it reaches zero
@@ -91,17 +95,28 @@ raster_fwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
     const int stage = j & (kStages - 1);
     if (alive_warp) {
       mbar_wait(&ring.full[stage], (uint32_t)(j / kStages) & 1u);
-      const StageBuf& sb = ring.st[stage];
+      const StageBuf<kTileBatch>& sb = ring.st[stage];
       // the entries of this round that can reach this warp's region, as a list of byte offsets in list order
       const int left = n - j * kTileBatch;  // entries of the round that exist (what lies beyond is stale)
-      const bool r0 = ((sb.rec[lane].ent >> sub) & 1u) && lane < left, r1 = ((sb.rec[lane + 32].ent >> sub) & 1u) && lane + 32 < left;
-      const unsigned b0 = __ballot_sync(kFull, r0), b1 = __ballot_sync(kFull, r1);
-      const int n0 = __popc(b0), nrel = n0 + __popc(b1);
+      constexpr int NCH = kTileBatch / 32;
+      bool rr[NCH];
+      unsigned bb[NCH];
+      int nrel = 0;
+#pragma unroll
+      for (int c = 0; c < NCH; ++c) {
+        rr[c] = ((sb.rec[lane + 32 * c].ent >> sub) & 1u) && lane + 32 * c < left;
+        bb[c] = __ballot_sync(kFull, rr[c]);
+        nrel += __popc(bb[c]);
+      }
       if (nrel) {
         const unsigned lt = (1u << lane) - 1u;
         uint16_t* idx = s_idx[warp];
-        if (r0) idx[__popc(b0 & lt)] = (uint16_t)(lane * 48);
-        if (r1) idx[n0 + __popc(b1 & lt)] = (uint16_t)((32 + lane) * 48);
+        int at = 0;
+#pragma unroll
+        for (int c = 0; c < NCH; ++c) {
+          if (rr[c]) idx[at + __popc(bb[c] & lt)] = (uint16_t)((lane + 32 * c) * 48);
+          at += __popc(bb[c]);
+        }
         if (lane < kGroup) idx[nrel + lane] = (uint16_t)(kPadIdx * 48);
         __syncwarp();
         const char* recs = reinterpret_cast<const char*>(sb.rec);

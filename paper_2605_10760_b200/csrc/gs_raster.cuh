@@ -17,15 +17,14 @@ namespace gs {
 
 constexpr unsigned kFull = 0xffffffffu;
 constexpr int kGroup = 4;        // relevant entries evaluated together in the pixel loop
-constexpr int kTileBatch = 64;   // list entries staged per round by a CTA
-// Staging ring shape: STAGES stages (a power of two) of 64 entries.  A warp that has finished round j refills the stage of
-// round j - DELAY (with round j - DELAY + STAGES): the warps of a CTA may be up to DELAY + 1 rounds apart before one waits
-// for another, and STAGES - DELAY rounds are in flight.  The two compositing kernels choose differently (each defines
-// kStages / kDelay / kAhead in its own translation unit): the forward is short of nothing but issue slots and takes 8
-// stages with 5 rounds of slack between its warps (4 / 2 -> 8 / 5: 61.9 -> 57.7 us); the backward pays for shared memory
-// with a CTA of occupancy and stays at 4 / 2 (8 / 2: 141.5 -> 154.3 us, profiles/r2_v9_ring.md).
-constexpr int kPadIdx = kTileBatch;  // index of the stage's padding record (never passes: lo = -inf)
-
+// Staging ring shape: STAGES stages (a power of two) of BATCH list entries.  A warp that has finished round j refills the
+// stage of round j - DELAY (with round j - DELAY + STAGES): the warps of a CTA may be up to DELAY + 1 rounds apart before
+// one waits for another, and STAGES - DELAY rounds are in flight.  The two compositing kernels choose differently (each
+// defines kTileBatch / kStages / kDelay / kAhead in its own translation unit).  The forward is short of nothing but issue
+// slots: rounds of 128 entries halve its per-round work (ballots, list building, barrier traffic, refill: 10 of its 34
+// instructions per relevant entry), 4 stages / 2 rounds of slack (64 x 4 / 2 -> 64 x 8 / 5 -> 128 x 4 / 2: 61.9 -> 57.7 ->
+// 55.0 us).  The backward pays for shared memory with a CTA of occupancy and stays at 64 x 4 / 2 (64 x 8 / 2: 141.5 ->
+// 154.3 us, profiles/r2_v9_ring.md).
 // One staged list entry (48 B): what the pixel loops read as broadcast LDS.128 x 2 + LDS.64.
 //   g  = { l11, l21, l22, lo }, c = { r, g, b, z }   gathered by visible slot (cp.async, 2 x 16 B)
 //   uv = { u0, v0 }                                   the instance's tile-local whitened offset (cp.async 8 B)
@@ -37,8 +36,10 @@ struct __align__(16) StageRec {
 };
 static_assert(sizeof(StageRec) == 48, "StageRec layout");
 // One stage of a CTA's staging ring: 64 consecutive list entries of the tile + the padding record.
+// (kTileBatch list entries per round: 64 in the backward, 128 in the forward; each kernel defines kTileBatch and kPadIdx)
+template <int kTileBatch>
 struct __align__(16) StageBuf {
-  StageRec rec[kTileBatch + 1];
+  StageRec rec[kTileBatch + 1];  // [kTileBatch] = the padding record (never passes: lo = -inf)
 };
 
 // -log2(255): alpha >= 1/255  <=>  p2 >= kPowerMin
@@ -112,12 +113,13 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
 // empty[stage]; there is NO block-wide barrier in the loop: warps of different regions, which find different numbers of
 // relevant entries per round, drift up to kDelay + 1 rounds apart (the per-round __syncthreads of v7 held 19-25 % of the
 // stall samples of both kernels).
-template <int NW, int kStages>
+template <int NW, int kStages, int kTileBatch>
 struct Ring {
+  static constexpr int kPadIdx = kTileBatch;
   static_assert((kStages & (kStages - 1)) == 0, "ring depth must be a power of two");
   static constexpr int T = NW * 32, TPE = T / kTileBatch;  // threads per staged entry: 1, 2 or 4
   static_assert(TPE == 1 || TPE == 2 || TPE == 4, "2, 4 or 8 warps");
-  StageBuf st[kStages];
+  StageBuf<kTileBatch> st[kStages];
   uint64_t full[kStages], empty[kStages];
 
   __device__ __forceinline__ void init(int tid) {

@@ -27,6 +27,7 @@ namespace gs {
 #ifndef GS_BWD_RING_DELAY
 #define GS_BWD_RING_DELAY 2
 #endif
+constexpr int kTileBatch = 64, kPadIdx = kTileBatch;  // list entries staged per round by a CTA; padding record
 constexpr int kStages = GS_BWD_RING_STAGES, kDelay = GS_BWD_RING_DELAY, kAhead = kStages - kDelay;  // gs_raster.cuh
 static_assert(kDelay >= 0 && kAhead >= 2, "ring shape");
 #ifndef GS_BWD_MIN_CTAS
@@ -139,8 +140,8 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
                   const uint32_t* __restrict__ n_contrib, const float* __restrict__ d_rgb,
                   const float* __restrict__ d_depth, const float* __restrict__ d_alpha, float* __restrict__ g2d) {
   constexpr int CPT = 8 / NW;  // CTAs per tile
-  constexpr int TPE = Ring<NW, kStages>::TPE;
-  __shared__ __align__(16) Ring<NW, kStages> ring;  // staging ring (gs_raster.cuh): no block-wide barrier in the loop
+  constexpr int TPE = Ring<NW, kStages, kTileBatch>::TPE;
+  __shared__ __align__(16) Ring<NW, kStages, kTileBatch> ring;  // staging ring (gs_raster.cuh): no block-wide barrier in the loop
   // per warp: byte offsets (into the stage) of the round's relevant entries, back to front
   __shared__ __align__(8) uint16_t s_idx[NW][kTileBatch + kGroup];
   __shared__ __align__(16) float2 s_pair_all[NW][kSlots * kPairRow];
@@ -201,7 +202,7 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
     const int pbase = (nb - 1 - k) * kTileBatch;
     if (pbase < n_w) {  // else nothing of this round was blended in this region
       mbar_wait(&ring.full[stage], (uint32_t)(k / kStages) & 1u);
-      const StageBuf& sb = ring.st[stage];
+      const StageBuf<kTileBatch>& sb = ring.st[stage];
       // the entries of this round that can reach this warp's region and lie in front of its deepest blended position, as
       // a list of byte offsets in REVERSE list order
       const bool r0 = ((sb.rec[lane].ent >> sub) & 1u) && pbase + lane < n_w;
