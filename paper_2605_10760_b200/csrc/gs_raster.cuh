@@ -23,8 +23,9 @@ constexpr int kGroup = 4;        // relevant entries evaluated together in the p
 // defines kTileBatch / kStages / kDelay / kAhead in its own translation unit).  The forward is short of nothing but issue
 // slots: rounds of 128 entries halve its per-round work (ballots, list building, barrier traffic, refill: 10 of its 34
 // instructions per relevant entry), 4 stages / 2 rounds of slack (64 x 4 / 2 -> 64 x 8 / 5 -> 128 x 4 / 2: 61.9 -> 57.7 ->
-// 55.0 us).  The backward pays for shared memory with a CTA of occupancy and stays at 64 x 4 / 2 (64 x 8 / 2: 141.5 ->
-// 154.3 us, profiles/r2_v9_ring.md).
+// 55.0 us).  The backward pays for shared memory with a CTA of occupancy (64 x 8 / 2: 141.5 -> 154.3 us, 128 x 4 / 2: 115.1 ->
+// 127.6 us) and spends its 12 KB on two stages of 128 entries, no slack (64 x 4 / 2 -> 128 x 2 / 0: 115.1 -> 112.3 us): the
+// halved per-round work outweighs the tighter coupling of its four warps.
 // One staged list entry (48 B): what the pixel loops read as broadcast LDS.128 x 2 + LDS.64.
 //   g  = { l11, l21, l22, lo }, c = { r, g, b, z }   gathered by visible slot (cp.async, 2 x 16 B)
 //   uv = { u0, v0 }                                   the instance's tile-local whitened offset (cp.async 8 B)

@@ -22,12 +22,15 @@
 namespace gs {
 
 #ifndef GS_BWD_RING_STAGES
-#define GS_BWD_RING_STAGES 4
+#define GS_BWD_RING_STAGES 2
 #endif
 #ifndef GS_BWD_RING_DELAY
-#define GS_BWD_RING_DELAY 2
+#define GS_BWD_RING_DELAY 0
 #endif
-constexpr int kTileBatch = 64, kPadIdx = kTileBatch;  // list entries staged per round by a CTA; padding record
+#ifndef GS_BWD_BATCH
+#define GS_BWD_BATCH 128
+#endif
+constexpr int kTileBatch = GS_BWD_BATCH, kPadIdx = kTileBatch;  // list entries staged per round by a CTA; padding record
 constexpr int kStages = GS_BWD_RING_STAGES, kDelay = GS_BWD_RING_DELAY, kAhead = kStages - kDelay;  // gs_raster.cuh
 static_assert(kDelay >= 0 && kAhead >= 2, "ring shape");
 #ifndef GS_BWD_MIN_CTAS
@@ -205,15 +208,25 @@ raster_bwd_kernel(int W, int H, int tiles_x, const uint32_t* __restrict__ order,
       const StageBuf<kTileBatch>& sb = ring.st[stage];
       // the entries of this round that can reach this warp's region and lie in front of its deepest blended position, as
       // a list of byte offsets in REVERSE list order
-      const bool r0 = ((sb.rec[lane].ent >> sub) & 1u) && pbase + lane < n_w;
-      const bool r1 = ((sb.rec[lane + 32].ent >> sub) & 1u) && pbase + 32 + lane < n_w;
-      const unsigned b0 = __ballot_sync(kFull, r0), b1 = __ballot_sync(kFull, r1);
-      const int n1 = __popc(b1), nrel = n1 + __popc(b0);
+      constexpr int NCH = kTileBatch / 32;
+      bool rr[NCH];
+      unsigned bb[NCH];
+      int nrel = 0;
+#pragma unroll
+      for (int c = 0; c < NCH; ++c) {
+        rr[c] = ((sb.rec[lane + 32 * c].ent >> sub) & 1u) && pbase + 32 * c + lane < n_w;
+        bb[c] = __ballot_sync(kFull, rr[c]);
+        nrel += __popc(bb[c]);
+      }
       if (nrel) {
         const unsigned gt = ~((2u << lane) - 1u);  // lanes above this one
         uint16_t* idx = s_idx[warp];
-        if (r1) idx[__popc(b1 & gt)] = (uint16_t)((32 + lane) * 48);
-        if (r0) idx[n1 + __popc(b0 & gt)] = (uint16_t)(lane * 48);
+        int at = 0;
+#pragma unroll
+        for (int c = NCH - 1; c >= 0; --c) {
+          if (rr[c]) idx[at + __popc(bb[c] & gt)] = (uint16_t)((32 * c + lane) * 48);
+          at += __popc(bb[c]);
+        }
         if (lane < kGroup) idx[nrel + lane] = (uint16_t)(kPadIdx * 48);
         __syncwarp();
         const int lastb48 = ((int)last - pbase) * 48;  // entries of this round at offsets < lastb48 were blended by this pixel
