@@ -41,11 +41,11 @@ SEEDS = (30, 31, 32, 33, 34)
 #       pixels of the region): u (2), gp u, gp v (2), 2 adds (2), 3 FFMA (6), sum gp (1), 4 FFMA (8) = 21     -> 41
 FLOP_EVAL, FLOP_BLEND_FWD, FLOP_BLEND_BWD = 12.0, 12.0, 41.0
 LDS_PER_ENTRY = 3.0   # broadcast LDS.128 per relevant (region, Gaussian) entry in the pixel loops (48-byte record)
-# Warp instructions the kernels execute per relevant entry, from the committed ncu captures (profiles/r2_v9_ring.md,
+# Warp instructions the kernels execute per relevant entry, from the committed ncu capture (profiles/r2_v10_ncu_full.txt,
 # r2_v10_chain.md: smsp__inst_executed / relevant entries of the captured scene).  NOT an algorithmic count: it says how
 # close the kernels run to the issue rate that actually binds them (roofline_stages[...]["issue"]), next to the
 # algorithmic FLOP fraction.
-WINST_PER_ENTRY_FWD, WINST_PER_ENTRY_BWD = 33.0, 67.0
+WINST_PER_ENTRY_FWD, WINST_PER_ENTRY_BWD = 34.0, 67.6   # scene seed 30: 47.78 M / 1.4055 M, 94.26 M / 1.3947 M
 
 
 def load_measured_peaks_file():
