@@ -6,7 +6,7 @@
 #include "gs_sh.cuh"
 
 #ifndef GS_PRE_CTAS_PER_SM
-#define GS_PRE_CTAS_PER_SM 5
+#define GS_PRE_CTAS_PER_SM 4
 #endif
 
 namespace gs {
@@ -27,7 +27,7 @@ constexpr int kPreT = 128;
 constexpr int kPreUMax = 4;  // Gaussians per thread and round of the cull phase (template parameter U: 1, 2 or 4)
 
 template <int DEG, int kPreU>
-__global__ void __launch_bounds__(kPreT, 5)
+__global__ void __launch_bounds__(kPreT, GS_PRE_CTAS_PER_SM)
 preprocess_kernel(int64_t N, const float* __restrict__ means, const float* __restrict__ scales,
                   const float* __restrict__ quats, const float* __restrict__ opacities, const float* __restrict__ sh,
                   DevCam cam, float4* __restrict__ feat,
