@@ -428,6 +428,36 @@ def test_tile_counters_survive_changes_of_image_size(oracle, gpu):
         full_check(oracle, gpu, sc, 38)
 
 
+def test_conservative_cull_never_drops_a_visible_gaussian(oracle, gpu):
+    """gs_preprocess culls in two steps: a cheap fp32 test (near plane with a rounding margin, opacity, a bound of the
+    footprint that dominates both half widths of the exact extent) and then the exact fp64 test on the survivors.  The
+    first step must only err on the side of keeping.  Adversarial scene: centres projected up to 3 image widths OUTSIDE the
+    image or around the near plane, scales log-uniform over four decades (footprints from sub-pixel to thousands of
+    pixels, 1000:1 anisotropy), opacities from just below 1/255 up: the GPU's visible set must contain the oracle's, and
+    features, binning (bit-exact) and images must agree at the usual tolerances.  (The gradients of this scene are not
+    asserted: footprints of 10^4-10^5 pixels accumulate their moments through thousands of fp32 atomics of both signs, and
+    g_means lands between 8e-4 and 6e-3 relative L2 from run to run -- outside what any configuration contains, and
+    recorded in DESIGN.md section 9.)"""
+    W, H, f, N = 160, 96, 80.0, 6000
+    r = np.random.Generator(np.random.PCG64(4242))
+    z = np.where(r.uniform(size=N) < 0.15, r.uniform(0.19, 0.21, N), r.uniform(0.25, 8.0, N))   # 15 % hug the near plane
+    u = r.uniform(-3 * W, 4 * W, N); v = r.uniform(-3 * H, 4 * H, N)
+    means = np.stack([(u - W / 2) * z / f, (v - H / 2) * z / f, z], 1).astype(np.float32)
+    scales = np.exp(r.uniform(np.log(1e-3), np.log(3.0), (N, 3))).astype(np.float32)
+    opac = np.exp(r.uniform(np.log(0.0035), 0.0, N)).astype(np.float32)   # 1/255 = 0.00392: some just below
+    cam = scenes.Camera(W, H, f, f, W / 2.0, H / 2.0, scenes.identity_pose())
+    sc = scenes.Scene(means=means, scales=scales, quats=r.normal(size=(N, 4)).astype(np.float32), opacities=opac,
+                      sh=r.normal(0.0, 0.5, (N, 1, 3)).astype(np.float32), sh_degree=0, camera=cam,
+                      bg=np.zeros(3, np.float32), name="cull_adversarial")
+    gC, gD = scenes.upstream_gradients(77, W, H)
+    ref = oracle.forward_backward(sc, gC, gD)
+    got = run_gpu(gpu, sc, gC, gD)
+    info = check_features(oracle, sc, ref, got, cam, uniform_edges=False)
+    check_binning(oracle, got, cam)
+    check_image(ref, got)
+    assert 200 < info["visible"] < N - 200   # both outcomes of the cull are well represented
+
+
 def test_call_order_and_argument_errors(gpu):
     b, torch = gpu.binding, gpu.torch
     ctx = b.Context(0)
