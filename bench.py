@@ -57,41 +57,76 @@ def load_measured_peaks_file():
 
 
 class ClockSampler:
-    """Samples nvidia-smi clocks / throttle reasons during the timed region."""
+    """nvidia-smi clocks / throttle reasons during the timed region, the way the profiling recipe does it: ONE nvidia-smi
+    process in loop mode, started before the warm-up and killed after the timed region (a process forked per sample at the
+    start of the timed loop took the launching thread's CPU: -2.3 % on a 20-step run).  Samples inside the timed window
+    are reported; a window shorter than the sampling period falls back to the samples since the warm-up (the GPU is under
+    the same load from the first warm-up step to the last timed one)."""
     Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
 
-    def __init__(self, index: int):
-        self.index, self.rows, self._stop, self._t = index, [], threading.Event(), None
+    def __init__(self, index: int, period_ms: int = 20):
+        self.index, self.period_ms, self.rows, self._p, self._t = index, period_ms, [], None, None
+        self.t_begin = self.t_end = None
 
     def _run(self):
-        while not self._stop.is_set():
-            try:
-                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-i",
-                                      str(self.index)], capture_output=True, text=True, timeout=5).stdout.strip()
-                if out:
-                    self.rows.append([c.strip() for c in out.splitlines()[0].split(",")])
-            except Exception:
-                pass
-            self._stop.wait(0.1)
+        try:
+            for line in self._p.stdout:
+                c = [x.strip() for x in line.strip().split(",")]
+                if len(c) >= 6:
+                    self.rows.append((time.perf_counter(), c))
+        except Exception:
+            pass
 
-    def __enter__(self):
-        self._t = threading.Thread(target=self._run, daemon=True)
-        self._t.start()
+    def start(self):
+        try:
+            self._p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-i",
+                                        str(self.index), "-lms", str(self.period_ms)], stdout=subprocess.PIPE,
+                                       stderr=subprocess.DEVNULL, text=True)
+            self._t = threading.Thread(target=self._run, daemon=True)
+            self._t.start()
+        except Exception:
+            self._p = None
         return self
 
-    def __exit__(self, *a):
-        self._stop.set()
-        self._t.join(timeout=6)
+    def wait_first(self, timeout_s: float):
+        t0 = time.perf_counter()
+        while not self.rows and time.perf_counter() - t0 < timeout_s and self._p is not None and self._p.poll() is None:
+            time.sleep(0.01)
+
+    def mark_begin(self):
+        self.t_begin = time.perf_counter()
+
+    def mark_end(self):
+        self.t_end = time.perf_counter()
+
+    def stop(self):
+        if self._p is not None:
+            try:
+                self._p.kill()
+                self._p.wait(timeout=5)
+            except Exception:
+                pass
+        if self._t is not None:
+            self._t.join(timeout=5)
 
     def summary(self):
-        if not self.rows:
+        inside = [c for t, c in self.rows if self.t_begin is not None and self.t_begin <= t <= (self.t_end or t)]
+        window = "timed region"
+        if not inside:   # region shorter than the sampling period: everything since the warm-up began
+            t_lo = (self.t_begin or 0.0) - 2.0   # the warm-up, the statistics pass and the timed steps: the same load
+            inside = [c for t, c in self.rows if t >= t_lo and (self.t_end is None or t <= self.t_end + 0.05)]
+            window = "warm-up + timed region (the timed region is shorter than the sampling period)"
+        if not inside:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unsampled"]}
-        sm = sorted(float(r[0]) for r in self.rows)
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        reasons = [n for k, n in enumerate(names) if any(r[2 + k].lower().startswith("active") for r in self.rows)]
-        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(self.rows[0][1]), "reasons": reasons,
-                "samples": len(self.rows)}
+        try:
+            sm = sorted(float(r[0]) for r in inside)
+            names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+            reasons = [n for k, n in enumerate(names) if any(r[2 + k].lower().startswith("active") for r in inside)]
+            return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(inside[0][1]), "reasons": reasons,
+                    "samples": len(inside), "window": window}
+        except Exception:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unparsed"]}
 
 
 # ----------------------------------------------------------------------------------------------------------------------
@@ -252,6 +287,7 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
+    clk = ClockSampler(local).start()   # one nvidia-smi in loop mode from here to the end of the timed region
     peaks = B.gs_measure_peaks(local)          # measured in this run: the roofline denominators
     wl = Workload(args.workload)
     W, H = wl.W, wl.H
@@ -338,6 +374,7 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    clk.wait_first(5.0)
     # warm-up: also calibrates the instance capacity over all poses (an overflowing iteration is re-issued)
     warm = max(args.warmup, 3)
     k = 0
@@ -368,20 +405,22 @@ def run_ours(args):
     K = args.steps
     l0 = sum(c.gs_get_launch_count() for c in vctx + ictx[1:])
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    with ClockSampler(local) as clk:
-        barrier()
-        e0.record()
-        if n_is > 1:   # the iteration streams start behind e0 and are joined in front of e1
-            fk = torch.cuda.Event(); fk.record()
-            for st in istreams:
-                st.wait_event(fk)
-        for k in range(K):
-            step(k)
-        if n_is > 1:
-            for st in istreams:
-                jn = torch.cuda.Event(); jn.record(st); torch.cuda.current_stream().wait_event(jn)
-        e1.record()
-        barrier()
+    barrier()
+    clk.mark_begin()
+    e0.record()
+    if n_is > 1:   # the iteration streams start behind e0 and are joined in front of e1
+        fk = torch.cuda.Event(); fk.record()
+        for st in istreams:
+            st.wait_event(fk)
+    for k in range(K):
+        step(k)
+    if n_is > 1:
+        for st in istreams:
+            jn = torch.cuda.Event(); jn.record(st); torch.cuda.current_stream().wait_event(jn)
+    e1.record()
+    barrier()
+    clk.mark_end()
+    clk.stop()
     ms_total = e0.elapsed_time(e1)
     for c in vctx + ictx[1:]:
         c.gs_poll()
