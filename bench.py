@@ -531,6 +531,7 @@ def run_e2e(args, wl, B, torch, local, world, K):
     """The same metric end to end: HOST (pinned) buffers in and out, copies inside the timed region."""
     dev = torch.device("cuda", local)
     W, H = wl.W, wl.H
+    extra_close = []
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, np.float32)).pin_memory()
     steps = max(3, min(K, 10))
     if args.workload in ("replica300k", "mono50k", "replica_small"):
@@ -540,17 +541,29 @@ def run_e2e(args, wl, B, torch, local, world, K):
         hsc = [tuple(pin(x).numpy() for x in (sc.means, sc.scales, sc.quats, sc.opacities, sc.sh)) for sc in scs]
         hup = [tuple(pin(x).numpy() for x in scenes.upstream_gradients(wl.up_seeds[k], W, H)) for k in range(len(scs))]
         Kc, Ng = (scs[0].sh_degree + 1) ** 2, scs[0].N
-        hout = {k: torch.zeros(s, dtype=torch.float32).pin_memory().numpy() for k, s in
-                dict(rgb=(3, H, W), depth=(H, W), alpha=(H, W), g_means=(Ng, 3), g_scales=(Ng, 3), g_quats=(Ng, 4),
-                     g_opacities=(Ng,), g_sh=(Ng, Kc, 3), g_twist=(6,)).items()}
+        # two (context, stream, pinned output set) pairs fed alternately through gs_fwd_bwd_host_async: the device->host
+        # copies of one step overlap the host->device copies and kernels of the next (PCIe is full duplex); every step
+        # still copies all of its inputs in and all of its results out, and a pair is synchronised before it is reused
+        mk = lambda: {k: torch.zeros(s, dtype=torch.float32).pin_memory().numpy() for k, s in
+                      dict(rgb=(3, H, W), depth=(H, W), alpha=(H, W), g_means=(Ng, 3), g_scales=(Ng, 3), g_quats=(Ng, 4),
+                           g_opacities=(Ng,), g_sh=(Ng, Kc, 3), g_twist=(6,)).items()}
+        houts = [mk(), mk()]
+        hout = houts[0]
         ctx2 = B.Context(local)
+        ctx3 = B.Context(local)
+        pair_ctx, pair_stream = [ctx2, ctx3], [torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)]
+        extra_close = [ctx3]
 
         def e2e_step(k):
-            j = k % len(scs)
-            ctx2.gs_fwd_bwd_host(hsc[j], scs[0].sh_degree, scs[j].camera, scs[j].bg, hup[j][0], hup[j][1], hout)
+            j, p = k % len(scs), k % 2
+            pair_stream[p].synchronize()   # the results of step k - 2 are in this pair's host buffers
+            pair_ctx[p].gs_poll()
+            pair_ctx[p].gs_fwd_bwd_host(hsc[j], scs[0].sh_degree, scs[j].camera, scs[j].bg, hup[j][0], hup[j][1], houts[p],
+                                        stream=pair_stream[p], sync=False)
         h2d = sum(x.nbytes for x in hsc[0]) + sum(x.nbytes for x in hup[0])
         d2h = sum(x.nbytes for x in hout.values())
-        what = "gs_fwd_bwd_host: parameters + upstream gradients in, images + all gradients out"
+        what = ("gs_fwd_bwd_host_async on two alternating (context, stream) pairs: parameters + upstream gradients in, images "
+                "+ all gradients out, every step")
     else:
         # configs 4 / 5: the Gaussians stay resident (they are frozen, or updated by the on-device optimiser); per step the
         # host sends the pose (tracking) or the per-view upstream gradients (refinement) from pinned memory and reads
@@ -609,6 +622,8 @@ def run_e2e(args, wl, B, torch, local, world, K):
     torch.cuda.synchronize()
     dt = time.perf_counter() - t0
     ctx2.close()
+    for c in extra_close:
+        c.close()
     return {"value": world * steps / dt, "unit": "iter/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
             "steps": steps, "what": what}
 

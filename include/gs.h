@@ -363,6 +363,15 @@ GS_API int gs_fwd_bwd_host(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, 
                     const float* quats, const float* opacities, const float* sh, const gs_camera* cam, const float* bg,
                     const float* d_rgb, const float* d_depth, float* rgb, float* depth, float* alpha, float* g_means,
                     float* g_scales, float* g_quats, float* g_opacities, float* g_sh, float* g_twist);
+/* The same without the final synchronisation: everything is enqueued on `stream` and the call returns.  The host arrays
+ * must be page-locked and must not be touched until the caller has synchronised the stream (then gs_poll reports an
+ * overflow of that iteration).  Two contexts on two streams fed alternately overlap one iteration's device->host copies
+ * with the next one's host->device copies and kernels (PCIe is full duplex): bench.py "e2e". */
+GS_API int gs_fwd_bwd_host_async(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, const float* means,
+                          const float* scales, const float* quats, const float* opacities, const float* sh,
+                          const gs_camera* cam, const float* bg, const float* d_rgb, const float* d_depth, float* rgb,
+                          float* depth, float* alpha, float* g_means, float* g_scales, float* g_quats, float* g_opacities,
+                          float* g_sh, float* g_twist);
 
 #ifdef __cplusplus
 }

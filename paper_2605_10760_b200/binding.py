@@ -22,7 +22,7 @@ STATUS = {0: "GS_OK", -1: "GS_E_INVALID", -2: "GS_E_ORDER", -3: "GS_E_CUDA", -4:
 
 EXPORTS = ["gs_create", "gs_destroy", "gs_last_error", "gs_preprocess", "gs_bin_tiles", "gs_rasterize_fwd",
            "gs_rasterize_bwd", "gs_pose_grad", "gs_get_counts", "gs_get_binning", "gs_get_features", "gs_poll",
-           "gs_aux_l1_grad", "gs_aux_pose_step", "gs_fwd_bwd_host", "gs_profile_enable", "gs_profile_read",
+           "gs_aux_l1_grad", "gs_aux_pose_step", "gs_fwd_bwd_host", "gs_fwd_bwd_host_async", "gs_profile_enable", "gs_profile_read",
            "gs_get_launch_count", "gs_get_workload", "gs_loss_map", "gs_loss_iso", "gs_sim3_apply", "gs_measure_peaks", "gs_loss_refine", "gs_voxel_set_clear", "gs_voxel_insert_boxes",
            "gs_voxel_insert_rays", "gs_voxel_retain", "gs_adam_step", "gs_prune_mask", "gs_compact_work_bytes",
            "gs_compact_plan", "gs_compact_rows", "gs_loss_normal", "gs_set_option", "gs_refine_views", "gs_visible_ids", "gs_adam_step_sparse", "gs_get_visible_ids"]
@@ -112,6 +112,7 @@ def load_library():
                                     C.POINTER(gs_gaussians), vp, vp, vp, vp]
     lib.gs_measure_peaks.argtypes = [C.c_int, vp, C.POINTER(C.c_double * len(PEAKS))]
     lib.gs_fwd_bwd_host.argtypes = [vp, vp, i64, C.c_int, vp, vp, vp, vp, vp, C.POINTER(gs_camera), C.POINTER(f * 3)] + [vp] * 11
+    lib.gs_fwd_bwd_host_async.argtypes = lib.gs_fwd_bwd_host.argtypes
     for name in EXPORTS:
         if name not in ("gs_last_error", "gs_compact_work_bytes"):
             getattr(lib, name).restype = C.c_int
@@ -310,7 +311,7 @@ class Context:
                     region_entries=int(w[4]), evaluated_bwd=int(w[5]), region_entries_bwd=int(w[6]))
 
     # -- host-buffer path (numpy arrays in / out; copies inside) ---------------------------------------------------
-    def gs_fwd_bwd_host(self, scene_arrays, sh_degree, cam, bg, d_rgb, d_depth, out, stream=None):
+    def gs_fwd_bwd_host(self, scene_arrays, sh_degree, cam, bg, d_rgb, d_depth, out, stream=None, sync=True):
         """scene_arrays = (means, scales, quats, opacities, sh) float32 numpy (ideally pinned); out = dict of float32
         numpy arrays rgb, depth, alpha, g_means, g_scales, g_quats, g_opacities, g_sh, g_twist (any may be absent)."""
         def hp(a):
@@ -320,7 +321,8 @@ class Context:
             return C.c_void_p(a.ctypes.data)
         means, scales, quats, opac, sh = scene_arrays
         c = cam if isinstance(cam, gs_camera) else camera_struct(cam)
-        self._check(self.lib.gs_fwd_bwd_host(
+        fn = self.lib.gs_fwd_bwd_host if sync else self.lib.gs_fwd_bwd_host_async   # async: the caller synchronises
+        self._check(fn(
             self._h, _stream(stream), int(means.shape[0]), int(sh_degree), hp(means), hp(scales), hp(quats), hp(opac),
             hp(sh), C.byref(c), _bg(bg), hp(d_rgb), hp(d_depth), hp(out.get("rgb")), hp(out.get("depth")),
             hp(out.get("alpha")), hp(out.get("g_means")), hp(out.get("g_scales")), hp(out.get("g_quats")),

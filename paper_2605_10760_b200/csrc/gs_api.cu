@@ -559,10 +559,10 @@ int gs_refine_views(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, const g
   return rc_all;
 }
 
-int gs_fwd_bwd_host(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, const float* means, const float* scales,
-                    const float* quats, const float* opacities, const float* sh, const gs_camera* cam, const float* bg,
-                    const float* d_rgb, const float* d_depth, float* rgb, float* depth, float* alpha, float* g_means,
-                    float* g_scales, float* g_quats, float* g_opacities, float* g_sh, float* g_twist) {
+static int fwd_bwd_host(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, const float* means, const float* scales,
+                        const float* quats, const float* opacities, const float* sh, const gs_camera* cam, const float* bg,
+                        const float* d_rgb, const float* d_depth, float* rgb, float* depth, float* alpha, float* g_means,
+                        float* g_scales, float* g_quats, float* g_opacities, float* g_sh, float* g_twist, bool sync) {
   if (!ctx || !cam || sh_degree < 0 || sh_degree > 3 || N < 0) return GS_E_INVALID;
   if (!d_rgb) return fail(ctx, GS_E_INVALID, "gs_fwd_bwd_host: d_rgb is null");
   cudaStream_t s = (cudaStream_t)stream;
@@ -611,8 +611,25 @@ int gs_fwd_bwd_host(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, const f
     if (g_sh) GS_CUDA(cudaMemcpyAsync(g_sh, dg_sh, N * K3 * f, cudaMemcpyDeviceToHost, s));
   }
   if (g_twist) GS_CUDA(cudaMemcpyAsync(g_twist, d_twist, 6 * f, cudaMemcpyDeviceToHost, s));
+  if (!sync) return GS_OK;
   GS_CUDA(cudaStreamSynchronize(s));
   return gs_poll(ctx);
+}
+
+int gs_fwd_bwd_host(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, const float* means, const float* scales,
+                    const float* quats, const float* opacities, const float* sh, const gs_camera* cam, const float* bg,
+                    const float* d_rgb, const float* d_depth, float* rgb, float* depth, float* alpha, float* g_means,
+                    float* g_scales, float* g_quats, float* g_opacities, float* g_sh, float* g_twist) {
+  return fwd_bwd_host(ctx, stream, N, sh_degree, means, scales, quats, opacities, sh, cam, bg, d_rgb, d_depth, rgb, depth,
+                      alpha, g_means, g_scales, g_quats, g_opacities, g_sh, g_twist, true);
+}
+
+int gs_fwd_bwd_host_async(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, const float* means, const float* scales,
+                          const float* quats, const float* opacities, const float* sh, const gs_camera* cam,
+                          const float* bg, const float* d_rgb, const float* d_depth, float* rgb, float* depth, float* alpha,
+                          float* g_means, float* g_scales, float* g_quats, float* g_opacities, float* g_sh, float* g_twist) {
+  return fwd_bwd_host(ctx, stream, N, sh_degree, means, scales, quats, opacities, sh, cam, bg, d_rgb, d_depth, rgb, depth,
+                      alpha, g_means, g_scales, g_quats, g_opacities, g_sh, g_twist, false);
 }
 
 }  // extern "C"

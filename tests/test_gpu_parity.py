@@ -534,6 +534,20 @@ def test_host_buffer_entry_point(oracle, gpu):
     ctx.gs_fwd_bwd_host((sc.means, sc.scales, sc.quats, sc.opacities, sc.sh), 3, sc.camera, sc.bg, gC, gD, out)
     check_image(ref, out)
     check_grads(ref, out)
+    # gs_fwd_bwd_host_async: pinned host arrays, a side stream, the caller synchronises (bench.py "e2e" feeds two such
+    # pairs alternately); twice on the same pair, as the double-buffered loop does
+    torch = gpu.torch
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, np.float32)).pin_memory().numpy()
+    arrays = tuple(pin(a) for a in (sc.means, sc.scales, sc.quats, sc.opacities, sc.sh))
+    hC, hD = pin(gC), pin(gD)
+    out2 = {k: pin(np.full_like(v, np.nan)) for k, v in out.items()}
+    st = torch.cuda.Stream()
+    for _ in range(2):
+        ctx.gs_fwd_bwd_host(arrays, 3, sc.camera, sc.bg, hC, hD, out2, stream=st, sync=False)
+    st.synchronize()
+    ctx.gs_poll()
+    check_image(ref, out2)
+    check_grads(ref, out2)
     ctx.close()
 
 
