@@ -47,10 +47,12 @@ typedef enum {
   GS_E_ORDER = -2,    /* call sequence violated (e.g. gs_rasterize_bwd before gs_rasterize_fwd) */
   GS_E_CUDA = -3,     /* a CUDA runtime call failed; text in gs_last_error */
   GS_E_NOMEM = -4,    /* growing the scratch failed */
-  GS_E_OVERFLOW = -5  /* the tile-instance capacity was exceeded by an asynchronous iteration: that iteration's outputs
+  GS_E_OVERFLOW = -5, /* the tile-instance capacity was exceeded by an asynchronous iteration: that iteration's outputs
                          are invalid (image = background, gradients = 0).  Reported once, by the first of
                          gs_preprocess / gs_bin_tiles / gs_poll / gs_get_counts to notice; the context has already
                          grown when it is returned: re-issue the iteration from gs_preprocess. */
+  GS_E_TOO_LARGE = -6 /* a size beyond the fixed capacity of an entry point that owns no growable memory
+                         (gs_compact_plan_static: N > gs_compact_plan_static_max()); nothing was launched */
 } gs_status;
 
 /* Pinhole camera + world-to-camera pose, p_c = R p_w + t.  HOST struct. */
@@ -304,6 +306,26 @@ GS_API int gs_prune_mask(void* stream, int64_t N, const float* opacities, float 
 GS_API int64_t gs_compact_work_bytes(int64_t N);
 GS_API int gs_compact_plan(void* stream, int64_t N, const uint8_t* keep, uint32_t* index, int64_t* n_kept, void* work);
 GS_API int gs_compact_rows(void* stream, int64_t N, int32_t width, const uint32_t* index, const float* in, float* out);
+/* gs_compact_plan for callers that must not allocate device memory where they compact.  Two kinds of caller are meant:
+ * a long-running agent that sized all of its device buffers at start-up and handed the rest of HBM to its own pool, so a
+ * cudaMalloc in the middle of a mission can fail (or fragment the pool it does not know about); and a loop that prunes or
+ * fuses (Eq. 22) while tracking and mapping kernels run on other streams, where cudaMalloc / cudaFree would
+ * stall all of them, because both synchronise the whole device.  Such callers already own keep / index / n_kept; the one
+ * thing gs_compact_plan still asks them to find room for is its scratch.  Here that scratch is a fixed array inside the
+ * library image (64 KiB, one uint32 per 1024 Gaussians): every GPU that loads libgs.so holds it until the process exits.
+ *   - Same arguments (minus `work`), same outputs, bit for bit, as gs_compact_plan.  Asynchronous on `stream`, which must
+ *     belong to the CURRENT device (the scratch used is the current device's copy).
+ *   - Limit: N <= gs_compact_plan_static_max() = 16 777 216 Gaussians.  A larger N returns GS_E_TOO_LARGE and launches
+ *     nothing; use gs_compact_plan with caller scratch for such maps.
+ *   - The call never calls cudaMalloc, cudaFree or any routine that allocates.  The FIRST call on each device looks up
+ *     the array's device address (cudaGetSymbolAddress, once per device, mutex-guarded); make that first call during
+ *     set-up, before any stream capture; a call with N = 0 (it only clears *n_kept) is enough.
+ *   - All calls on one device share the one array and it keeps whatever the last call left.  That is harmless for calls
+ *     that follow one another on a stream (every word read is written earlier in the same call; nothing needs zeroing),
+ *     but two calls whose kernels can overlap on the GPU (different streams, no dependency between them) RACE on it and
+ *     both results are garbage.  Order them with an event, or give one of them gs_compact_plan with its own scratch. */
+GS_API int64_t gs_compact_plan_static_max(void);
+GS_API int gs_compact_plan_static(void* stream, int64_t N, const uint8_t* keep, uint32_t* index, int64_t* n_kept);
 
 /* ---- one whole iteration of the joint refinement (Eq. 23) over a batch of keyframe views ----------- */
 /* For every view k: gs_preprocess -> gs_bin_tiles -> gs_rasterize_fwd -> gs_loss_refine on I~ = e^{a_k} I^ + b_k (+ gs_loss_normal

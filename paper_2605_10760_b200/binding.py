@@ -18,14 +18,16 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libgs.so")
 _lib = None
 
-STATUS = {0: "GS_OK", -1: "GS_E_INVALID", -2: "GS_E_ORDER", -3: "GS_E_CUDA", -4: "GS_E_NOMEM", -5: "GS_E_OVERFLOW"}
+STATUS = {0: "GS_OK", -1: "GS_E_INVALID", -2: "GS_E_ORDER", -3: "GS_E_CUDA", -4: "GS_E_NOMEM", -5: "GS_E_OVERFLOW",
+          -6: "GS_E_TOO_LARGE"}
 
 EXPORTS = ["gs_create", "gs_destroy", "gs_last_error", "gs_preprocess", "gs_bin_tiles", "gs_rasterize_fwd",
            "gs_rasterize_bwd", "gs_pose_grad", "gs_get_counts", "gs_get_binning", "gs_get_features", "gs_poll",
            "gs_aux_l1_grad", "gs_aux_pose_step", "gs_fwd_bwd_host", "gs_fwd_bwd_host_async", "gs_profile_enable", "gs_profile_read",
            "gs_get_launch_count", "gs_get_workload", "gs_loss_map", "gs_loss_iso", "gs_sim3_apply", "gs_measure_peaks", "gs_loss_refine", "gs_voxel_set_clear", "gs_voxel_insert_boxes",
            "gs_voxel_insert_rays", "gs_voxel_retain", "gs_adam_step", "gs_prune_mask", "gs_compact_work_bytes",
-           "gs_compact_plan", "gs_compact_rows", "gs_loss_normal", "gs_set_option", "gs_refine_views", "gs_visible_ids", "gs_adam_step_sparse", "gs_get_visible_ids"]
+           "gs_compact_plan", "gs_compact_rows", "gs_loss_normal", "gs_set_option", "gs_refine_views", "gs_visible_ids", "gs_adam_step_sparse", "gs_get_visible_ids",
+           "gs_compact_plan_static", "gs_compact_plan_static_max"]
 GS_OPT_EXACT_TILE_CULL = 1
 GS_OPT_VIEW_STREAMS = 2
 PEAKS = ["fma_tlanes", "issue_twarp", "ex2_tlanes", "lds128_bcast_twarp", "lds128_twarp", "lds32_bcast_twarp",
@@ -103,6 +105,8 @@ def load_library():
     lib.gs_compact_work_bytes.argtypes = [i64]
     lib.gs_compact_plan.argtypes = [vp, i64, vp, vp, vp, vp]
     lib.gs_compact_rows.argtypes = [vp, i64, C.c_int32, vp, vp, vp]
+    lib.gs_compact_plan_static.argtypes = [vp, i64, vp, vp, vp]
+    lib.gs_compact_plan_static_max.argtypes = []
     lib.gs_loss_normal.argtypes = [vp, C.c_int32, C.c_int32, f, f, f, f, vp, vp, f, vp, vp, vp]
     lib.gs_visible_ids.argtypes = [vp, C.POINTER(vp), C.POINTER(vp)]
     lib.gs_get_visible_ids.argtypes = [vp, vp, vp]
@@ -114,9 +118,10 @@ def load_library():
     lib.gs_fwd_bwd_host.argtypes = [vp, vp, i64, C.c_int, vp, vp, vp, vp, vp, C.POINTER(gs_camera), C.POINTER(f * 3)] + [vp] * 11
     lib.gs_fwd_bwd_host_async.argtypes = lib.gs_fwd_bwd_host.argtypes
     for name in EXPORTS:
-        if name not in ("gs_last_error", "gs_compact_work_bytes"):
+        if name not in ("gs_last_error", "gs_compact_work_bytes", "gs_compact_plan_static_max"):
             getattr(lib, name).restype = C.c_int
     lib.gs_compact_work_bytes.restype = C.c_int64
+    lib.gs_compact_plan_static_max.restype = C.c_int64
     _lib = lib
     return lib
 
@@ -478,6 +483,26 @@ def gs_compact(keep, arrays, stream=None):
             raise GsError(rc, "gs_compact_rows")
         out[k] = o
     return out, index
+
+
+def gs_compact_plan_static(keep, index, n_kept, stream=None):
+    """gs_compact_plan_static of include/gs.h: the compaction plan of the uint8 mask `keep` written into the caller's
+    `index` (int32/uint32 [N]) and `n_kept` (int64 [1]) CUDA tensors, with the scratch taken from a fixed 64 KiB array
+    inside libgs.so instead of a fresh device allocation.  It is meant for code that cannot allocate where it compacts: an
+    agent whose device memory was all handed out at start-up, or a pruning / fusion step running beside tracking streams
+    that a cudaMalloc would stall.  Nothing is allocated here either (the caller brings every tensor), and N above
+    gs_compact_plan_static_max() (16 Mi Gaussians) raises GS_E_TOO_LARGE.  Calls on one device share the scratch, so two
+    calls that may overlap on the GPU race; make the first call on a device during set-up."""
+    import torch
+    lib = load_library()
+    N = int(keep.numel())
+    if N > int(lib.gs_compact_plan_static_max()):
+        raise GsError(-6, f"gs_compact_plan_static: N = {N} exceeds the fixed scratch of {int(lib.gs_compact_plan_static_max())} "
+                          "Gaussians; use gs_compact_plan with caller scratch")
+    assert index.numel() == N and index.element_size() == 4 and n_kept.dtype == torch.int64 and n_kept.numel() == 1
+    rc = lib.gs_compact_plan_static(_stream(stream), N, _ptr(keep, torch.uint8), _ptr(index), _ptr(n_kept))
+    if rc != 0:
+        raise GsError(rc, "gs_compact_plan_static")
 
 
 class VoxelSet:

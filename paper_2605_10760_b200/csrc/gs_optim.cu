@@ -10,6 +10,8 @@
 //   gs_compact_plan / gs_compact_rows : exclusive scan of a keep mask -> destination row of every kept Gaussian (original
 //                     order preserved), then a row gather per parameter array.
 // HBM-streaming kernels, one element per thread, grid-stride.  Product code: nothing here includes, links or calls oracle/.
+#include <mutex>
+
 #include "gs_internal.cuh"
 
 namespace gs {
@@ -181,6 +183,34 @@ static int grid_for(int64_t n) {
   return (int)(g < 1 ? 1 : g);
 }
 
+// ---- scratch of gs_compact_plan_static: lives in the library image, not on the heap -------------------------------------
+// One word per block of kPlanBlock Gaussians, for at most kStaticPlanMaxN Gaussians: 64 KiB that every GPU loading libgs.so
+// holds from module load to process exit.  gs_compact_plan_static exists for callers that may not allocate device memory
+// at the point where they compact (see include/gs.h); it is the only user of this array.
+constexpr int64_t kStaticPlanMaxN = 1ll << 24;                      // 16 Mi Gaussians
+constexpr int kStaticPlanWords = (int)(kStaticPlanMaxN / kPlanBlock);  // 16384 block counters
+static __device__ __align__(256) uint32_t g_static_plan_counts[kStaticPlanWords];
+
+// In host code the name g_static_plan_counts is only a handle for the runtime, never a device address: handing it to a
+// kernel would fault (or, on a GPU that can reach host memory, quietly work on the wrong bytes).  The device address is
+// asked for once per device, with that device current, and kept here.
+constexpr int kStaticPlanMaxDevices = 64;
+static uint32_t* s_static_plan_ptr[kStaticPlanMaxDevices];
+static std::mutex s_static_plan_mutex;
+
+static int static_plan_scratch(uint32_t** out) {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kStaticPlanMaxDevices) { cudaGetLastError(); return GS_E_CUDA; }
+  std::lock_guard<std::mutex> lock(s_static_plan_mutex);
+  if (!s_static_plan_ptr[dev]) {
+    void* p = nullptr;
+    if (cudaGetSymbolAddress(&p, g_static_plan_counts) != cudaSuccess || !p) { cudaGetLastError(); return GS_E_CUDA; }
+    s_static_plan_ptr[dev] = static_cast<uint32_t*>(p);
+  }
+  *out = s_static_plan_ptr[dev];
+  return GS_OK;
+}
+
 }  // namespace gs
 
 using namespace gs;
@@ -258,6 +288,27 @@ int gs_compact_plan(void* stream, int64_t N, const uint8_t* keep, uint32_t* inde
   if (N == 0) return cudaMemsetAsync(n_kept, 0, sizeof(int64_t), s) == cudaSuccess ? GS_OK : GS_E_CUDA;
   const int nblocks = (int)div_up(N, kPlanBlock);
   uint32_t* bc = reinterpret_cast<uint32_t*>(work);
+  plan_count_kernel<<<nblocks, 256, 0, s>>>(N, keep, bc);
+  plan_scan_kernel<<<1, 1024, 0, s>>>(nblocks, bc, n_kept);
+  plan_index_kernel<<<nblocks, 256, 0, s>>>(N, keep, bc, index);
+  return cudaGetLastError() == cudaSuccess ? GS_OK : GS_E_CUDA;
+}
+
+int64_t gs_compact_plan_static_max(void) { return kStaticPlanMaxN; }
+
+// gs_compact_plan with its scratch in g_static_plan_counts instead of a caller-provided buffer: same three kernels, same
+// results.  Nothing in the array has to be zero when the call starts: plan_count_kernel writes every one of the `nblocks`
+// counters before plan_scan_kernel and plan_index_kernel read them, and no word beyond `nblocks` is read, so what an
+// earlier call (of any size) left behind is harmless.  No cudaMalloc / cudaFree / allocating routine on this path.
+int gs_compact_plan_static(void* stream, int64_t N, const uint8_t* keep, uint32_t* index, int64_t* n_kept) {
+  if (N < 0 || !n_kept || (N > 0 && (!keep || !index))) return GS_E_INVALID;
+  if (N > kStaticPlanMaxN) return GS_E_TOO_LARGE;
+  cudaStream_t s = (cudaStream_t)stream;
+  uint32_t* bc = nullptr;
+  const int rc = static_plan_scratch(&bc);  // first call on this device: cudaGetSymbolAddress (may load the module)
+  if (rc != GS_OK) return rc;
+  if (N == 0) return cudaMemsetAsync(n_kept, 0, sizeof(int64_t), s) == cudaSuccess ? GS_OK : GS_E_CUDA;
+  const int nblocks = (int)div_up(N, kPlanBlock);
   plan_count_kernel<<<nblocks, 256, 0, s>>>(N, keep, bc);
   plan_scan_kernel<<<1, 1024, 0, s>>>(nblocks, bc, n_kept);
   plan_index_kernel<<<nblocks, 256, 0, s>>>(N, keep, bc, index);
