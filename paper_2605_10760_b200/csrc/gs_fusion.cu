@@ -108,24 +108,31 @@ __device__ __forceinline__ unsigned long long vox_hash(unsigned long long k) {  
 }
 __device__ __forceinline__ long long vox_floor_div(double x, double v) { return (long long)floor(__ddiv_rn(x, v)); }
 
-__device__ __forceinline__ void vox_insert(unsigned long long* table, unsigned long long mask, unsigned long long key,
+// Probe sequences are cut at kVoxMaxProbe slots: a key that finds neither itself nor an empty slot within that window is
+// counted in `overflow` (the table is too full for it).  vox_contains walks the same window, so a stored key is always
+// found.  At the load factors the sets are sized for (<= 0.5) linear probing essentially never reaches 128; an undersized
+// table now costs at most 128 reads per key instead of `capacity`.
+constexpr unsigned long long kVoxMaxProbe = 128;
+
+__device__ __forceinline__ bool vox_insert(unsigned long long* table, unsigned long long mask, unsigned long long key,
                                            uint32_t* overflow) {
   unsigned long long slot = vox_hash(key) & mask;
-  for (unsigned long long probe = 0; probe <= mask; ++probe) {
+  for (unsigned long long probe = 0; probe <= mask && probe < kVoxMaxProbe; ++probe) {
     const unsigned long long cur = table[slot];   // most insertions are duplicates: read before the atomic
-    if (cur == key) return;
+    if (cur == key) return true;
     if (cur == kVoxEmpty) {
       const unsigned long long old = atomicCAS(table + slot, kVoxEmpty, key);
-      if (old == kVoxEmpty || old == key) return;
+      if (old == kVoxEmpty || old == key) return true;
     }
     slot = (slot + 1) & mask;
   }
-  atomicAdd(overflow, 1u);  // table full
+  atomicAdd(overflow, 1u);  // no room within the probe window
+  return false;
 }
 
 __device__ __forceinline__ bool vox_contains(const unsigned long long* table, unsigned long long mask, unsigned long long key) {
   unsigned long long slot = vox_hash(key) & mask;
-  for (unsigned long long probe = 0; probe <= mask; ++probe) {
+  for (unsigned long long probe = 0; probe <= mask && probe < kVoxMaxProbe; ++probe) {
     const unsigned long long cur = __ldg(table + slot);
     if (cur == key) return true;
     if (cur == kVoxEmpty) return false;
@@ -139,25 +146,58 @@ __global__ void __launch_bounds__(256) vox_clear_kernel(unsigned long long* tabl
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < cap; i += stride) table[i] = kVoxEmpty;
 }
 
-// Eq. 20: every voxel meeting the closed axis-aligned box [mu - k s, mu + k s]
+// Eq. 20: every voxel meeting the closed axis-aligned box [mu - k s, mu + k s].  One thread per Gaussian; a box of up to
+// kBoxInline voxels is inserted by its own thread, a larger one by the whole warp (lanes stride over the linearised box),
+// so that one background Gaussian costs count / 32 inserts per lane instead of `count` in a single thread.  A box of more
+// than kBoxMaxVoxels voxels is not inserted at all and counted in `overflow` (no table a caller would pass holds it).  On
+// the warp path a lane stops at its first key that finds no room: the set is inexact from there on anyway (gs.h), and a
+// full table then costs one failed probe window per lane and box instead of one per voxel.
+constexpr unsigned long long kBoxInline = 64;
+constexpr unsigned long long kBoxMaxVoxels = 1ull << 24;
+
 __global__ void __launch_bounds__(128)
 vox_boxes_kernel(unsigned long long* table, unsigned long long mask, double v, double k, int64_t N,
                  const float* __restrict__ means, const float* __restrict__ scales, uint32_t* overflow) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= N) return;
-  long long lo[3], hi[3];
-  bool ok = true;
+  long long lo[3] = {0, 0, 0};
+  unsigned long long n[3] = {0, 0, 0}, count = 0;
+  if (i < N) {
+    long long hi[3];
+    bool ok = true;
 #pragma unroll
-  for (int a = 0; a < 3; ++a) {
-    const double mu = (double)means[3 * i + a], h = __dmul_rn(k, (double)scales[3 * i + a]);
-    lo[a] = vox_floor_div(__dsub_rn(mu, h), v);
-    hi[a] = vox_floor_div(__dadd_rn(mu, h), v);
-    ok = ok && vox_in_range(lo[a]) && vox_in_range(hi[a]);
+    for (int a = 0; a < 3; ++a) {
+      const double mu = (double)means[3 * i + a], h = __dmul_rn(k, (double)scales[3 * i + a]);
+      ok = ok && isfinite(mu) && isfinite(h);        // floor(NaN) converts to 0: caught here, not by the range test
+      lo[a] = vox_floor_div(__dsub_rn(mu, h), v);
+      hi[a] = vox_floor_div(__dadd_rn(mu, h), v);
+      ok = ok && vox_in_range(lo[a]) && vox_in_range(hi[a]) && hi[a] >= lo[a];
+      n[a] = ok ? (unsigned long long)(hi[a] - lo[a] + 1) : 0ull;
+    }
+    count = n[0] * n[1] * n[2];                      // each factor <= 2^21
+    if (!ok || count > kBoxMaxVoxels) { atomicAdd(overflow, 1u); count = 0; }
+    if (count <= kBoxInline) {
+      for (unsigned long long j = 0; j < count; ++j) {
+        const unsigned long long ix = j % n[0], r = j / n[0];
+        vox_insert(table, mask, vox_key(lo[0] + (long long)ix, lo[1] + (long long)(r % n[1]), lo[2] + (long long)(r / n[1])), overflow);
+      }
+      count = 0;
+    }
   }
-  if (!ok) { atomicAdd(overflow, 1u); return; }   // outside the 21-bit index range (or non-finite)
-  for (long long iz = lo[2]; iz <= hi[2]; ++iz)
-    for (long long iy = lo[1]; iy <= hi[1]; ++iy)
-      for (long long ix = lo[0]; ix <= hi[0]; ++ix) vox_insert(table, mask, vox_key(ix, iy, iz), overflow);
+  // boxes left over: one at a time, spread over the warp
+  const unsigned lane = threadIdx.x & 31;
+  unsigned pending = __ballot_sync(0xffffffffu, count != 0);
+  while (pending) {
+    const int src = __ffs(pending) - 1;
+    pending &= pending - 1;
+    const long long l0 = __shfl_sync(0xffffffffu, lo[0], src), l1 = __shfl_sync(0xffffffffu, lo[1], src),
+                    l2 = __shfl_sync(0xffffffffu, lo[2], src);
+    const uint32_t n0 = (uint32_t)__shfl_sync(0xffffffffu, n[0], src), n1 = (uint32_t)__shfl_sync(0xffffffffu, n[1], src);
+    const uint32_t cnt = (uint32_t)__shfl_sync(0xffffffffu, count, src);   // <= 2^24
+    for (uint32_t j = lane; j < cnt; j += 32) {
+      const uint32_t ix = j % n0, r = j / n0;
+      if (!vox_insert(table, mask, vox_key(l0 + ix, l1 + (r % n1), l2 + (r / n1)), overflow)) break;
+    }
+  }
 }
 
 struct RayCam { double fx, fy, cx, cy, R[9], t[3]; int W, H, stride; };
@@ -202,7 +242,7 @@ vox_rays_kernel(unsigned long long* table, unsigned long long mask, double v, Ra
     }
   }
   if (!ok) { atomicAdd(overflow, 1u); return; }
-  vox_insert(table, mask, vox_key(idx[0], idx[1], idx[2]), overflow);
+  if (!vox_insert(table, mask, vox_key(idx[0], idx[1], idx[2]), overflow)) return;   // table full: give the ray up
   for (int guard = 0; guard < (1 << 22); ++guard) {
     int a = 0;                                   // axis of the nearest boundary; ties -> lowest axis
     if (t_max[1] < t_max[a]) a = 1;
@@ -213,7 +253,7 @@ vox_rays_kernel(unsigned long long* table, unsigned long long mask, double v, Ra
     else if (a == 1) { idx[1] += step[1]; t_max[1] = __dadd_rn(t_max[1], t_delta[1]); }
     else { idx[2] += step[2]; t_max[2] = __dadd_rn(t_max[2], t_delta[2]); }
     if (!(vox_in_range(idx[0]) && vox_in_range(idx[1]) && vox_in_range(idx[2]))) { atomicAdd(overflow, 1u); return; }
-    vox_insert(table, mask, vox_key(idx[0], idx[1], idx[2]), overflow);
+    if (!vox_insert(table, mask, vox_key(idx[0], idx[1], idx[2]), overflow)) return;
   }
 }
 
@@ -223,10 +263,10 @@ vox_retain_kernel(const unsigned long long* occ, unsigned long long occ_mask, co
                   unsigned long long free_mask, double v, int64_t N, const float* __restrict__ means, uint8_t* __restrict__ retain) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= N) return;
-  const long long ix = vox_floor_div((double)means[3 * i], v), iy = vox_floor_div((double)means[3 * i + 1], v),
-                  iz = vox_floor_div((double)means[3 * i + 2], v);
-  bool keep = true;
-  if (vox_in_range(ix) && vox_in_range(iy) && vox_in_range(iz)) {
+  const float m0 = means[3 * i], m1 = means[3 * i + 1], m2 = means[3 * i + 2];
+  const long long ix = vox_floor_div((double)m0, v), iy = vox_floor_div((double)m1, v), iz = vox_floor_div((double)m2, v);
+  bool keep = isfinite(m0) && isfinite(m1) && isfinite(m2);   // a Gaussian without a position is never retained (gs.h)
+  if (keep && vox_in_range(ix) && vox_in_range(iy) && vox_in_range(iz)) {
     const unsigned long long key = vox_key(ix, iy, iz);
     if (occ && vox_contains(occ, occ_mask, key)) keep = false;
     if (keep && fre && vox_contains(fre, free_mask, key)) keep = false;
@@ -252,7 +292,7 @@ int gs_voxel_set_clear(void* stream, uint64_t* table, int64_t capacity) {
 
 int gs_voxel_insert_boxes(void* stream, uint64_t* table, int64_t capacity, float voxel, float k, int64_t N,
                           const float* means, const float* scales, uint32_t* overflow) {
-  if (!table || !pow2(capacity) || !(voxel > 0.f) || !(k >= 0.f) || N < 0 || !overflow || (N > 0 && (!means || !scales)))
+  if (!table || !pow2(capacity) || !(voxel > 0.f) || !isfinite(voxel) || !(k >= 0.f) || !isfinite(k) || N < 0 || !overflow || (N > 0 && (!means || !scales)))
     return GS_E_INVALID;
   if (N == 0) return GS_OK;
   vox_boxes_kernel<<<(unsigned)div_up(N, 128), 128, 0, (cudaStream_t)stream>>>(
@@ -263,7 +303,7 @@ int gs_voxel_insert_boxes(void* stream, uint64_t* table, int64_t capacity, float
 
 int gs_voxel_insert_rays(void* stream, uint64_t* table, int64_t capacity, float voxel, const gs_camera* cam,
                          const float* depth, int32_t stride, uint32_t* overflow) {
-  if (!table || !pow2(capacity) || !(voxel > 0.f) || !cam || !depth || stride < 1 || !overflow || cam->width <= 0 ||
+  if (!table || !pow2(capacity) || !(voxel > 0.f) || !isfinite(voxel) || !cam || !depth || stride < 1 || !overflow || cam->width <= 0 ||
       cam->height <= 0)
     return GS_E_INVALID;
   RayCam rc;
@@ -281,7 +321,7 @@ int gs_voxel_insert_rays(void* stream, uint64_t* table, int64_t capacity, float 
 
 int gs_voxel_retain(void* stream, const uint64_t* occ, int64_t occ_capacity, const uint64_t* free_set, int64_t free_capacity,
                     float voxel, int64_t N, const float* means, uint8_t* retain) {
-  if ((occ && !pow2(occ_capacity)) || (free_set && !pow2(free_capacity)) || !(voxel > 0.f) || N < 0 ||
+  if ((occ && !pow2(occ_capacity)) || (free_set && !pow2(free_capacity)) || !(voxel > 0.f) || !isfinite(voxel) || N < 0 ||
       (N > 0 && (!means || !retain)))
     return GS_E_INVALID;
   if (N == 0) return GS_OK;

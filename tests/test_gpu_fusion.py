@@ -142,3 +142,94 @@ def test_retain_and_compaction_config5_shaped():
     assert np.array_equal(out["means"].cpu().numpy(), src_m[want]) and np.array_equal(out["quats"].cpu().numpy(), sc.quats[n:][want])
     idx = index.cpu().numpy().view(np.uint32)
     assert np.array_equal(idx[want], np.arange(want.sum(), dtype=np.uint32)) and (idx[~want] == 0xFFFFFFFF).all()
+
+
+def _box_keys(of, means, scales, v, k):
+    """Eq. 20 by its definition, vectorised: per Gaussian every voxel index between kappa(mu - k s) and kappa(mu + k s)."""
+    out = []
+    for m, s in zip(np.asarray(means, np.float64), np.asarray(scales, np.float64)):
+        lo, hi = of.kappa(m - np.float64(k) * s, v), of.kappa(m + np.float64(k) * s, v)
+        gx, gy, gz = np.meshgrid(*(np.arange(lo[a], hi[a] + 1) for a in range(3)), indexing="ij")
+        out.append(of.pack_key(gx.ravel(), gy.ravel(), gz.ravel()))
+    return np.unique(np.concatenate(out))
+
+
+def test_large_boxes_are_inserted_completely():
+    """Background-sized Gaussians (10^4..10^5 voxels per box: the warp-cooperative path of vox_boxes_kernel) mixed with
+    ordinary ones: the set is the definition's, bit for bit."""
+    import torch
+    from oracle import fusion as of
+    from paper_2605_10760_b200 import binding as b
+    r = np.random.Generator(np.random.PCG64(66))
+    N = 300
+    means = _f32(r.uniform(-2, 2, (N, 3)))
+    scales = _f32(np.exp(r.normal(-4.0, 0.5, (N, 3))))
+    big = [3, 64, 65, 131, 299]            # two of them in one warp, one in the last (ragged) warp
+    scales[big] = _f32([[0.3, 0.2, 0.1], [0.05, 0.4, 0.05], [0.2, 0.2, 0.2], [0.011, 0.013, 0.6], [0.25, 0.1, 0.3]])
+    v, k = np.float32(0.02), np.float32(3.0)
+    want = _box_keys(of, means, scales, float(v), float(k))
+    assert np.array_equal(_box_keys(of, means[:40], scales[:40], float(v), float(k)),
+                          np.array(sorted(of.occupied_set(means[:40], scales[:40], float(v), float(k))), np.uint64))
+    vs = b.VoxelSet(1 << 21)
+    vs.insert_boxes(torch.from_numpy(means).cuda(), torch.from_numpy(scales).cuda(), v, k)
+    torch.cuda.synchronize()
+    assert int(vs.overflow.item()) == 0
+    got = vs.keys()
+    assert len(want) > 400_000 and np.array_equal(got, want)
+
+
+def test_full_table_and_runaway_scales_end_promptly_with_overflow():
+    """An undersized table and Gaussians with metre-sized scales must end in an overflow report, not in a kernel that
+    probes the whole table per key or walks 10^8 voxels in one thread."""
+    import torch
+    from paper_2605_10760_b200 import binding as b, scenes
+    r = np.random.Generator(np.random.PCG64(67))
+    v, k = np.float32(0.02), np.float32(3.0)
+    N = 5_000
+    means = _f32(r.uniform(-3, 3, (N, 3)))
+    scales = _f32(np.exp(r.normal(-3.5, 0.4, (N, 3))))
+    scales[::500] = 2.0                     # (2 * 3 * 2 m / 2 cm)^3 = 2e8 voxels each: beyond the per-box limit
+    scales[7::500] = 0.5                    # 3.4e6 voxels each: warp path, abandoned once the overflow is known
+    small = b.VoxelSet(1 << 12)
+    dm, dsc = torch.from_numpy(means).cuda(), torch.from_numpy(scales).cuda()
+    depth = torch.from_numpy(_f32(r.uniform(1.0, 5.0, (480, 640)))).cuda()
+    cam = scenes.Camera(640, 480, 300.0, 300.0, 320.0, 240.0, scenes.look_at([0.0, 0.0, 0.0], [1.0, 0.2, 0.1]))
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0.record()
+    small.insert_boxes(dm, dsc, v, k)
+    small.insert_rays(cam, depth, v, 1)     # 307 200 rays of ~100 steps each into the full table
+    t1.record()
+    torch.cuda.synchronize()
+    assert int(small.overflow.item()) >= 10 and len(small.keys()) == 1 << 12
+    assert t0.elapsed_time(t1) < 2000.0, t0.elapsed_time(t1)
+    # a roomy table still refuses the 2e8-voxel boxes (counted once each) and stores everything else
+    roomy = b.VoxelSet(1 << 24)
+    keep = np.ones(N, bool); keep[7::500] = False          # leave the 3.4e6-voxel boxes out of this part
+    roomy.insert_boxes(torch.from_numpy(means[keep]).cuda(), torch.from_numpy(scales[keep]).cuda(), v, k)
+    torch.cuda.synchronize()
+    assert int(roomy.overflow.item()) == len(range(0, N, 500)) and 100_000 < len(roomy.keys()) < 1 << 23
+
+
+def test_non_finite_gaussians_are_counted_and_never_retained():
+    import torch
+    from oracle import fusion as of
+    from paper_2605_10760_b200 import binding as b
+    r = np.random.Generator(np.random.PCG64(68))
+    N = 1000
+    means = _f32(r.uniform(-1, 1, (N, 3)))
+    scales = _f32(np.exp(r.normal(-4.0, 0.3, (N, 3))))
+    v, k = np.float32(0.05), np.float32(1.0)
+    bad = np.zeros(N, bool); bad[[0, 17, 500, 999]] = True
+    m2, s2 = means.copy(), scales.copy()
+    m2[0, 1] = np.nan; m2[17, 0] = np.inf; s2[500, 2] = np.nan; m2[999] = -np.inf
+    want = _box_keys(of, means[~bad], scales[~bad], float(v), float(k))
+    vs = b.VoxelSet(1 << 16)
+    vs.insert_boxes(torch.from_numpy(m2).cuda(), torch.from_numpy(s2).cuda(), v, k)
+    torch.cuda.synchronize()
+    assert int(vs.overflow.item()) == 4 and np.array_equal(vs.keys(), want)     # voxel 0 was not invented for the NaNs
+    # retain against an EMPTY pair of sets: everything finite is retained, nothing non-finite is
+    retain = torch.empty(N, dtype=torch.uint8, device="cuda")
+    b.gs_voxel_retain(b.VoxelSet(1 << 4), None, v, torch.from_numpy(m2).cuda(), retain)
+    torch.cuda.synchronize()
+    finite = np.isfinite(m2).all(1)
+    assert np.array_equal(retain.cpu().numpy().astype(bool), finite) and (~finite).sum() == 3
