@@ -176,7 +176,9 @@ GS_API int gs_visible_ids(gs_ctx* ctx, const uint32_t** ids, const uint32_t** n_
 /* Copies that index list into caller-owned DEVICE memory ids_out uint32[N] (entries beyond n_visible are unspecified);
  * asynchronous on `stream`. */
 GS_API int gs_get_visible_ids(gs_ctx* ctx, void* stream, uint32_t* ids_out);
-/* Non-blocking: GS_E_OVERFLOW if an earlier asynchronous iteration overflowed the instance capacity, else GS_OK. */
+/* Non-blocking: GS_E_OVERFLOW if an earlier asynchronous iteration overflowed the instance capacity, else GS_OK.  Covers
+ * the context and the view sub-contexts of gs_refine_views (GS_OPT_VIEW_STREAMS > 1): a view that overflowed on any of
+ * them is reported here after the stream has been synchronised, and at the entry of the next gs_refine_views. */
 GS_API int gs_poll(gs_ctx* ctx);
 
 /* Stage timing.  gs_profile_enable(ctx, 1) makes the five calls record CUDA events on their stream around each kernel

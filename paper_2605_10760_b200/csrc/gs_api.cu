@@ -246,9 +246,26 @@ int gs_set_option(gs_ctx* ctx, int option, int value) {
   return fail(ctx, GS_E_INVALID, "gs_set_option: unknown option");
 }
 
+// Overflow check of a context AND of the view sub-contexts gs_refine_views runs some of its views on
+// (GS_OPT_VIEW_STREAMS > 1): every one that overflowed grows and clears its flag; the first failure is the one reported,
+// with the sub-context's message copied into the parent's.
+static int handle_overflow_all(gs_ctx* ctx) {
+  int rc_all = handle_overflow(ctx);
+  for (int k = 0; k < (int)(sizeof(ctx->sub) / sizeof(ctx->sub[0])); ++k) {
+    gs_ctx* c = ctx->sub[k];
+    if (!c) continue;
+    const int rc = handle_overflow(c);
+    if (rc != GS_OK && rc_all == GS_OK) {
+      rc_all = rc;
+      snprintf(ctx->err, sizeof(ctx->err), "view stream %d: %.200s", k + 1, c->err);
+    }
+  }
+  return rc_all;
+}
+
 int gs_poll(gs_ctx* ctx) {
   if (!ctx) return GS_E_INVALID;
-  return handle_overflow(ctx);
+  return handle_overflow_all(ctx);
 }
 
 int gs_preprocess(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, const float* means, const float* scales,
@@ -476,6 +493,8 @@ int gs_refine_views(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, const g
   if (W <= 0 || H <= 0) return fail(ctx, GS_E_INVALID, "gs_refine_views: empty image");
   cudaStream_t s = (cudaStream_t)stream;
   GS_CUDA(cudaSetDevice(ctx->device));
+  // an overflow left by an earlier call on ANY of the contexts involved is reported before anything is enqueued
+  { const int rc = handle_overflow_all(ctx); if (rc != GS_OK) return rc; }
   const int64_t P = (int64_t)W * H;
   // GS_OPT_VIEW_STREAMS > 1: the views run round-robin on this context (caller's stream) and on S - 1 sub-contexts with
   // their own streams; every view ACCUMULATES (one L2 reduction per element) into gradient arrays zeroed up front, so the

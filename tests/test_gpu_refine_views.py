@@ -76,3 +76,60 @@ def test_refine_views_matches_the_composed_oracles(oracle, with_normals, view_st
     gv = vis.cpu().numpy()
     assert set(np.unique(gv)) <= {0, 1} and (gv[seen] == 1).all() and gv.sum() <= seen.sum() * 1.01 + 2
     ctx.close()
+
+
+def test_overflow_on_a_view_sub_context_is_reported_by_gs_poll():
+    """GS_OPT_VIEW_STREAMS = 2: view 1 runs on a context-owned sub-context.  If only THAT context's instance capacity
+    overflows (its calibration view saw almost nothing, the next call's view sees the whole scene), gs_poll on the parent
+    after the stream sync must say so -- the accumulated gradients are missing a view -- and the re-issued call must agree
+    with a single-stream context."""
+    import torch
+    from paper_2605_10760_b200 import binding as b
+    W, H = 300, 170
+    sc = scenes.replica_scene(seed=36, N=20000, width=W, height=H, f=150.0, sh_degree=1)
+    near = sc.camera
+    away = near.copy()
+    away.T_cw = near.T_cw.copy()
+    away.T_cw[2, 3] -= 1000.0                         # the whole scene lies far behind this camera: no instances at all
+    r = np.random.Generator(np.random.PCG64(95))
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    trgb = t(r.uniform(0, 1, (2, 3, H, W)).astype(np.float32)); tdep = t(r.uniform(0.5, 5, (2, H, W)).astype(np.float32))
+    ab = t(np.zeros((2, 2), np.float32))
+    ds = b.DeviceScene(sc)
+    params = dict(means=ds.means, scales=ds.scales, quats=ds.quats, opacities=ds.opacities, sh=ds.sh)
+    wts = (1.75, 0.2, 0.25, 0.0)
+
+    def run(ctx, cams):
+        grads = {k: torch.zeros_like(v) for k, v in params.items()}
+        g_twist = torch.zeros(2, 6, device="cuda"); g_ab = torch.zeros(2, 2, device="cuda")
+        loss = torch.zeros(2, 10, dtype=torch.float64, device="cuda")
+        ctx.gs_refine_views(params, 1, cams, trgb, tdep, ab, wts, sc.bg, grads, g_twist, g_ab, loss)
+        torch.cuda.synchronize()
+        return grads, g_twist
+
+    ctx = b.Context(0)
+    ctx.gs_set_option(b.GS_OPT_VIEW_STREAMS, 2)
+    run(ctx, [near, away])                 # calibration: the sub-context (view 1) sizes itself for an almost empty view
+    ctx.gs_poll()
+    run(ctx, [near, near])                 # view 1 overflows the sub-context; the parent (same view as before) does not
+    with pytest.raises(b.GsError, match="GS_E_OVERFLOW") as e:
+        ctx.gs_poll()
+    assert "view stream 1" in str(e.value)
+    ctx.gs_poll()                          # reported once; both contexts are clean (and the sub-context has grown)
+    grads, g_twist = run(ctx, [near, near])
+    ctx.gs_poll()
+    # left unpolled, the same overflow is caught at the ENTRY of the next gs_refine_views, before anything is enqueued
+    ctx2 = b.Context(0)
+    ctx2.gs_set_option(b.GS_OPT_VIEW_STREAMS, 2)
+    run(ctx2, [near, away]); run(ctx2, [near, near])
+    with pytest.raises(b.GsError, match="GS_E_OVERFLOW"):
+        run(ctx2, [near, near])
+    ctx2.close()
+    one = b.Context(0)
+    want, want_twist = run(one, [near, near])
+    one.gs_poll()
+    for k in params:
+        assert _rel(grads[k].cpu().numpy(), want[k].cpu().numpy()) <= 1e-5, k
+        assert float(want[k].abs().max()) > 0
+    assert _rel(g_twist.cpu().numpy(), want_twist.cpu().numpy()) <= 1e-5
+    ctx.close(); one.close()
