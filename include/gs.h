@@ -135,7 +135,8 @@ GS_API int gs_preprocess(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, co
  * attribute and begins with griddepcontrol.wait, i.e. it consumes nothing before the work in front of it on the stream
  * (the caller's own kernels included) has completed; work the caller enqueues behind a call is ordered as usual.  Only
  * buckets beyond 2047 keys are sorted on a context-owned side stream (forked from and joined to `stream` by events), and
- * only in iterations that follow one that had such buckets. */
+ * only in iterations that follow one that had such buckets.
+ * Once per gs_preprocess: the scan consumes (and clears) the per-tile counters, a second call returns GS_E_ORDER. */
 GS_API int gs_bin_tiles(gs_ctx* ctx, void* stream);
 
 /* Step a6 -- per-tile front-to-back compositing (oracle reading C1 step 7).

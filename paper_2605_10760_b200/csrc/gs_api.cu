@@ -318,6 +318,9 @@ int gs_preprocess(gs_ctx* ctx, void* stream, int64_t N, int sh_degree, const flo
 int gs_bin_tiles(gs_ctx* ctx, void* stream) {
   if (!ctx) return GS_E_INVALID;
   if (ctx->stage < 1) return fail(ctx, GS_E_ORDER, "gs_bin_tiles before gs_preprocess");
+  // the scan clears the per-tile counters it consumes (no memset in the steady state): a second pass over the same
+  // preprocess would read zeros and bin nothing
+  if (ctx->stage >= 2) return fail(ctx, GS_E_ORDER, "gs_bin_tiles called twice for one gs_preprocess (its tile counters are consumed)");
   GS_CUDA(cudaSetDevice(ctx->device));
   int rc = launch_binning(ctx, (cudaStream_t)stream);
   if (rc != GS_OK) return rc;
