@@ -508,7 +508,7 @@ def run_ours(args):
                 "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f32", "data": "synthetic", "config": config_dict(wl, world),
                 "views_per_iter": wl.views, "view_streams": n_vs, "iter_streams": n_is, "grads": "sparse" if grad_flag else "dense", "mpix_iter_per_s": value * wl.views * W * H / 1e6,
-                "clocks": clk.summary(), "e2e": e2e, "gpu_launches": launches, "roofline": roof,
+                "clocks": clk.summary(), "e2e": e2e, "e2e_sequential": e2e.get("sequential"), "gpu_launches": launches, "roofline": roof,
                 "roofline_stages": roof_stages, "cpu_baseline": cpu,
                 "hbm_frac_whole_iteration": hbm_frac_iter, "algorithmic_bytes_per_iter": bytes_iter,
                 "stages_ms": stage_ms, "stages_note": "device time per stage of the LAST view of a step (CUDA events in the library)",
@@ -534,6 +534,7 @@ def run_e2e(args, wl, B, torch, local, world, K):
     extra_close = []
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, np.float32)).pin_memory()
     steps = max(3, min(K, 10))
+    seq_step = None
     if args.workload in ("replica300k", "mono50k", "replica_small"):
         # through the C-ABI host-buffer entry point gs_fwd_bwd_host: H2D of all parameters and upstream gradients, D2H
         # of the images and all gradients, every step
@@ -565,6 +566,12 @@ def run_e2e(args, wl, B, torch, local, world, K):
         d2h = sum(x.nbytes for x in hout.values())
         what = ("gs_fwd_bwd_host_async on two alternating (context, stream) pairs: parameters + upstream gradients in, images "
                 "+ all gradients out, every step")
+
+        def seq_step(k):
+            # one iteration at a time (a loop whose host-side optimiser needs step k's gradients before step k + 1)
+            j = k % len(scs)
+            pair_ctx[0].gs_fwd_bwd_host(hsc[j], scs[0].sh_degree, scs[j].camera, scs[j].bg, hup[j][0], hup[j][1], houts[0],
+                                        stream=pair_stream[0], sync=True)
     else:
         # configs 4 / 5: the Gaussians stay resident (they are frozen, or updated by the on-device optimiser); per step the
         # host sends the pose (tracking) or the per-view upstream gradients (refinement) from pinned memory and reads
@@ -622,11 +629,24 @@ def run_e2e(args, wl, B, torch, local, world, K):
         e2e_step(k)
     torch.cuda.synchronize()
     dt = time.perf_counter() - t0
+    res = {"value": world * steps / dt, "unit": "iter/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+           "steps": steps, "what": what}
+    if seq_step is not None:
+        # the pipelined figure above overlaps two INDEPENDENT iterations; the sequential one is the figure to compare from
+        # round to round (round 1's e2e was sequential) and the one a host-side optimiser loop sees
+        for k in range(2):
+            seq_step(k)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for k in range(steps):
+            seq_step(k)
+        torch.cuda.synchronize()
+        res["sequential"] = {"value": world * steps / (time.perf_counter() - t0), "unit": "iter/s", "steps": steps,
+                             "what": "gs_fwd_bwd_host, one context, each step synchronised before the next starts; same copies"}
     ctx2.close()
     for c in extra_close:
         c.close()
-    return {"value": world * steps / dt, "unit": "iter/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-            "steps": steps, "what": what}
+    return res
 
 
 def run_peaks(args):
