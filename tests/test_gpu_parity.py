@@ -217,6 +217,59 @@ def test_config4_tracking_pose_only(oracle, gpu):
     assert rel_l2(out["g_means"].cpu().numpy(), ref["g_means"]) <= TOL_GRAD
 
 
+def test_config4_tracking_loop_five_steps(oracle, gpu):
+    """The loop bench.py times for config 4 ("per-keyframe pose deltas"): pose held on the device ->
+    forward -> L1 gradient -> pose-only backward -> on-device normalised twist step, five times, against the same loop
+    written with the oracle (gso.forward / forward_backward / pose_apply).  The C-ABI keeps the pose as float32[12], so the
+    oracle's pose is rounded to float32 after every step as well.  Tolerance on the pose after n steps: each step moves
+    the pose by `step` along g/|g|, and the twist gradient is held to TOL_GRAD, so the two poses can drift apart by
+    n * step * TOL_GRAD (+ float32 rounding of O(1) entries); measured drift is printed."""
+    b, torch = gpu.binding, gpu.torch
+    W, H, n_steps, step = 400, 230, 5, 2e-3
+    sc = scenes.replica_scene(seed=41, N=60_000, width=W, height=H, f=200.0)
+    cam_t = sc.camera.copy()
+    cam_t.T_cw = scenes.perturb_pose(sc.camera.T_cw, scenes.tracking_perturbation(41))
+    target = oracle.forward(sc, camera=cam_t)["rgb"].astype(np.float32)
+    P = W * H
+    # oracle loop
+    T = np.ascontiguousarray(sc.camera.T_cw, np.float32)
+    poses, twists, losses = [], [], []
+    for _ in range(n_steps):
+        cam = sc.camera.copy(); cam.T_cw = T
+        img = oracle.forward(sc, camera=cam)["rgb"]
+        losses.append(float(np.abs(img - target).mean()))
+        gC = (np.sign(img.astype(np.float32) - target) / np.float32(3 * P)).astype(np.float32)
+        g = oracle.forward_backward(sc, gC, None, camera=cam)["g_twist"]
+        T = oracle.pose_apply(-step * g / np.linalg.norm(g), T).astype(np.float32)
+        poses.append(T.copy()); twists.append(g)
+    # GPU loop, no host read in between
+    ds = b.DeviceScene(sc)
+    out = ds.alloc_outputs(W, H)
+    T_dev = torch.from_numpy(np.ascontiguousarray(sc.camera.T_cw, np.float32).reshape(-1).copy()).cuda()
+    tgt = torch.from_numpy(target).cuda()
+    gCd = torch.empty_like(out["rgb"])
+    cam_bad = sc.camera.copy(); cam_bad.T_cw = scenes.identity_pose()    # must be ignored: the device pose overrides it
+    got_T, got_g = [], []
+    for it in range(n_steps):
+        b.forward(gpu.ctx, ds, cam_bad, out, T_cw_dev=T_dev)
+        b.gs_aux_l1_grad(out["rgb"], tgt, 1.0 / (3 * P), gCd)
+        b.backward(gpu.ctx, out, gCd, None, None, flags=b.GS_POSE_ONLY, pose=True)
+        got_g.append(out["g_twist"].clone())
+        b.gs_aux_pose_step(T_dev, out["g_twist"], step)
+        got_T.append(T_dev.clone())
+    torch.cuda.synchronize(); gpu.ctx.gs_poll()
+    drift = [float(np.abs(got_T[i].cpu().numpy().reshape(3, 4) - poses[i]).max()) for i in range(n_steps)]
+    print("config-4 loop: pose drift per step", drift)
+    for i in range(n_steps):
+        assert rel_l2(got_g[i].cpu().numpy(), twists[i]) <= TOL_GRAD, (i, rel_l2(got_g[i].cpu().numpy(), twists[i]))
+        assert drift[i] <= (i + 1) * step * TOL_GRAD + 1e-6, (i, drift)
+    # the loop went somewhere: a twist of norm `step` moves the pose entries by up to step * (1 + |t|) per step
+    moved = float(np.abs(poses[-1] - np.asarray(sc.camera.T_cw)).max())
+    reach = float(1 + np.abs(np.asarray(sc.camera.T_cw)[:, 3]).max())
+    print("config-4 loop: pose moved", moved, "L1 per step", losses)
+    assert 0.5 * step < moved <= n_steps * step * reach * 1.01
+
+
 def test_config5_fused_two_views_accumulate(oracle, gpu):
     """Config-5 shape at reduced size: union of 4 Sim(3)-mapped submaps, gradients accumulated over views with
     GS_ACCUMULATE."""
@@ -475,7 +528,13 @@ def test_call_order_and_argument_errors(gpu):
     with pytest.raises(b.GsError, match="GS_E_ORDER"):
         ctx.gs_rasterize_bwd(out["rgb"], None, None, 0, out["g_means"], out["g_scales"], out["g_quats"],
                              out["g_opacities"], out["g_sh"])
+    with pytest.raises(b.GsError, match="GS_E_ORDER"):
+        ctx.gs_bin_tiles()      # the counters of this preprocess are consumed: refused, not silently empty
     ctx.gs_rasterize_fwd(None, out["rgb"], out["depth"], out["alpha"])
+    torch.cuda.synchronize()
+    assert float(out["alpha"].max()) > 0.5     # the refused call left the binning of the first one intact
+    with pytest.raises(b.GsError, match="GS_E_ORDER"):
+        ctx.gs_bin_tiles()
     with pytest.raises(b.GsError, match="GS_E_INVALID"):
         ctx.gs_rasterize_bwd(out["rgb"], None, None, 0, None, None, None, None, None)
     with pytest.raises(b.GsError, match="GS_E_ORDER"):
