@@ -110,7 +110,13 @@ class ClockSampler:
         if self._t is not None:
             self._t.join(timeout=5)
 
-    def summary(self):
+    def summary(self, t_begin=None, t_end=None):
+        if t_begin is not None:     # an explicit window (the sustained leg)
+            inside = [c for t, c in self.rows if t_begin <= t <= t_end]
+            window = "sustained leg"
+            if not inside:
+                return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unsampled"]}
+            return self._fmt(inside, window)
         inside = [c for t, c in self.rows if self.t_begin is not None and self.t_begin <= t <= (self.t_end or t)]
         window = "timed region"
         if not inside:   # region shorter than the sampling period: everything since the warm-up began
@@ -119,6 +125,10 @@ class ClockSampler:
             window = "warm-up + timed region (the timed region is shorter than the sampling period)"
         if not inside:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unsampled"]}
+        return self._fmt(inside, window)
+
+    @staticmethod
+    def _fmt(inside, window):
         try:
             sm = sorted(float(r[0]) for r in inside)
             names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
@@ -420,13 +430,36 @@ def run_ours(args):
     e1.record()
     barrier()
     clk.mark_end()
-    clk.stop()
     ms_total = e0.elapsed_time(e1)
     for c in vctx + ictx[1:]:
         c.gs_poll()
     launches = sum(c.gs_get_launch_count() for c in vctx + ictx[1:]) - l0
     ms_total = max_over_ranks(ms_total, dist, dev)
     value = replica_throughput(world, K, ms_total)
+
+    # ---- sustained leg: a timed region under 0.25 s (e.g. the driver's --steps 20: 5 ms) is too short for the clock
+    # sampler and for an outside clock to see; the same loop is then timed again over about half a second.  `value`,
+    # `steps` and `ms_per_step` stay those of the K requested steps; this is reported beside them.
+    sustained = None
+    if ms_total < 250.0 and n_is == 1:
+        K2 = int(min(50_000, max(K, np.ceil(500.0 / max(ms_total / K, 1e-3)))))
+        if dist is not None:   # every rank must run the same number of steps
+            t = torch.tensor([K2], device=dev); dist.all_reduce(t, op=dist.ReduceOp.MAX); K2 = int(t.item())
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        tb = time.perf_counter()
+        s0.record()
+        for k in range(K2):
+            step(k)
+        s1.record()
+        barrier()
+        te = time.perf_counter()
+        ms2 = max_over_ranks(s0.elapsed_time(s1), dist, dev)
+        for c in vctx + ictx[1:]:
+            c.gs_poll()
+        sustained = {"value": replica_throughput(world, K2, ms2), "unit": "iter/s", "steps": K2, "ms_per_step": ms2 / K2,
+                     "clocks": clk.summary(tb, te)}
+    clk.stop()
 
     # ---- per-stage device times (second loop, stage events on; same steps; last view of each step) ----
     prof_seq[0] = True
@@ -489,6 +522,9 @@ def run_ours(args):
                 if row["workload"] == args.workload and row["kernel"] == kernel_name:
                     roof["traffic"] = int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
                     roof["traffic_source"] = row["source"]
+                    roof["traffic_note"] = ("ncu dram read+write of ONE launch on ONE scene (seed 30), while the other fields "
+                                            "average the five scenes; writes that stay resident in the 126 MB L2 (images, "
+                                            "gradient rows) are not in it, so it is a lower bound of the bytes moved")
     except Exception:
         pass
     # whole-iteration HBM figure (BASELINE.json "% HBM roofline"): algorithmic bytes of all stages / step time
@@ -508,7 +544,7 @@ def run_ours(args):
                 "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f32", "data": "synthetic", "config": config_dict(wl, world),
                 "views_per_iter": wl.views, "view_streams": n_vs, "iter_streams": n_is, "grads": "sparse" if grad_flag else "dense", "mpix_iter_per_s": value * wl.views * W * H / 1e6,
-                "clocks": clk.summary(), "e2e": e2e, "e2e_sequential": e2e.get("sequential"), "gpu_launches": launches, "roofline": roof,
+                "clocks": clk.summary(), "value_sustained": sustained, "e2e": e2e, "e2e_sequential": e2e.get("sequential"), "gpu_launches": launches, "roofline": roof,
                 "roofline_stages": roof_stages, "cpu_baseline": cpu,
                 "hbm_frac_whole_iteration": hbm_frac_iter, "algorithmic_bytes_per_iter": bytes_iter,
                 "stages_ms": stage_ms, "stages_note": "device time per stage of the LAST view of a step (CUDA events in the library)",

@@ -1,18 +1,20 @@
 // gs_raster.cu -- step a6: per-tile front-to-back compositing (oracle reading C1 step 7).
 //
-// Design (evidence: profiles/r1_*.md for the history; profiles/r2_v7_tile_cta.md for this version).  Up to round-2 v6 every
-// 8x4 region was an autonomous single-warp CTA that gathered, decoded and compacted its own records: per relevant
-// (region, Gaussian) entry the forward then spent 47 warp instructions and 13.8 shared-memory wavefronts, of which only
-// ~22 / 7.4 were the blend itself (R = 1.24 M entries, 58.6 M instructions, 17.1 M wavefronts on config 3) -- staging
-// cost as much as compositing, and the kernel sat on the shared-memory pipe (l1tex 85-88 %).  Now:
-//   * one CTA per 16x16 TILE, eight warps = its eight 8x4-pixel regions, one pixel per lane;
-//   * the tile's list is staged ONCE per tile, 64 entries per round, into a three-stage ring: 64 threads each gather the
-//     32 contiguous bytes {l11, l21, l22, lo}{r, g, b, z} of one Gaussian by visible slot (2 x cp.async 16 B) plus the
-//     8-byte tile-local whitened offset (u0, v0) of the instance (written in fp64 by gs_bin_tiles) -- nothing is decoded
-//     here any more; one block barrier per round, which also carries the "is any pixel of the tile still alive" vote;
-//   * every warp turns the round's 64 region masks into a byte list of the entries relevant to ITS region (two ballots,
-//     ranks by popc, byte stores) and walks that list front to back, four entries per step: the records are read as
-//     broadcast LDS.128 x 2 + LDS.64;
+// Design as built (v10; history and evidence: profiles/r1_*.md, r2_v7_tile_cta.md, r2_v9_ring.md, r2_v10_chain.md).  Up to
+// round-2 v6 every 8x4 region was an autonomous single-warp CTA that gathered, decoded and compacted its own records: per
+// relevant (region, Gaussian) entry the forward spent 47 warp instructions and 13.8 shared-memory wavefronts, of which
+// only ~22 / 7.4 were the blend itself.  Now:
+//   * one CTA of FOUR warps per HALF tile (GS_FWD_WARPS = 4; two CTAs per 16x16 tile), a warp = one 8x4-pixel region, one
+//     pixel per lane; tiles are visited in the longest-list-first order gs_bin_tiles wrote (`order`);
+//   * the tile's list is staged in rounds of 128 entries (GS_FWD_BATCH) into a ring of 4 stages with 2 rounds of slack
+//     (GS_FWD_RING_STAGES / _DELAY, Ring<> in gs_raster.cuh): every thread is a producer -- one 16-byte cp.async.cg for
+//     the instance record {u0, v0, list word} and two for the 32 contiguous bytes {l11, l21, l22, lo}{r, g, b, z} of the
+//     Gaussian, gathered by visible slot -- and signals the stage's `full` mbarrier through cp.async.mbarrier.arrive;
+//     a warp releases a stage through its `empty` mbarrier.  There is NO block-wide barrier in the loop: the four warps
+//     drift up to kDelay + 1 rounds apart; staging stops when no warp of the CTA has a live pixel (s_live);
+//   * every warp turns the round's 128 region masks into a list of byte offsets of the entries relevant to ITS region
+//     (ballots, ranks by popc, 16-bit stores into s_idx) and walks that list front to back, four entries per step
+//     (kGroup): the records are read as broadcast LDS.128 x 2 + LDS.64;
 //   * the pixel loop is branch-free: every relevant entry is evaluated and blended under a per-lane predicate (alpha_eff
 //     = 0 where the pixel is not hit or has terminated); alpha >= 1/255 is tested in the exponent domain against a
 //     constant, so rejected pairs cost no MUFU and the opacity never enters the loop.

@@ -27,8 +27,9 @@ constexpr int kGroup = 4;        // relevant entries evaluated together in the p
 // 127.6 us) and spends its 12 KB on two stages of 128 entries, no slack (64 x 4 / 2 -> 128 x 2 / 0: 115.1 -> 112.3 us): the
 // halved per-round work outweighs the tighter coupling of its four warps.
 // One staged list entry (48 B): what the pixel loops read as broadcast LDS.128 x 2 + LDS.64.
-//   g  = { l11, l21, l22, lo }, c = { r, g, b, z }   gathered by visible slot (cp.async, 2 x 16 B)
-//   uv = { u0, v0 }                                   the instance's tile-local whitened offset (cp.async 8 B)
+//   g  = { l11, l21, l22, lo }, c = { r, g, b, z }   gathered by visible slot (cp.async.cg, 2 x 16 B)
+//   { uv = { u0, v0 }, ent, pad }                     the 16-byte instance record written by the sort epilogue, one
+//                                                     cp.async.cg: tile-local whitened offset + list word
 //   ent = visible slot << 8 | region mask             (0 beyond the end of the list)
 struct __align__(16) StageRec {
   float4 g, c;
@@ -36,8 +37,8 @@ struct __align__(16) StageRec {
   uint32_t ent, pad;
 };
 static_assert(sizeof(StageRec) == 48, "StageRec layout");
-// One stage of a CTA's staging ring: 64 consecutive list entries of the tile + the padding record.
-// (kTileBatch list entries per round: 64 in the backward, 128 in the forward; each kernel defines kTileBatch and kPadIdx)
+// One stage of a CTA's staging ring: kTileBatch consecutive list entries of the tile + the padding record
+// (128 per round in both compositing kernels since v10; each kernel defines kTileBatch and kPadIdx).
 template <int kTileBatch>
 struct __align__(16) StageBuf {
   StageRec rec[kTileBatch + 1];  // [kTileBatch] = the padding record (never passes: lo = -inf)
@@ -107,9 +108,9 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   while (!mbar_try_wait(bar, parity)) {}
 }
 
-// The staging ring shared by the forward and the backward kernels.  Every thread of the CTA is a producer: entry e of a
-// round is staged by T / 64 consecutive threads (record halves g, c by 16-byte cp.async, the instance's (u0, v0) by an
-// 8-byte and its list word by a 4-byte cp.async), each of which then lets full[stage] count its copies
+// The staging ring shared by the forward and the backward kernels.  Every thread of the CTA is a producer: the entries
+// of a round are dealt to the threads of the CTA (record halves g, c and the 16-byte instance record {u0, v0, list word}
+// by one 16-byte cp.async.cg each), and every thread then lets full[stage] count its copies
 // (cp.async.mbarrier.arrive.noinc).  Consumers (the same warps) wait on full[stage] and release the stage through
 // empty[stage]; there is NO block-wide barrier in the loop: warps of different regions, which find different numbers of
 // relevant entries per round, drift up to kDelay + 1 rounds apart (the per-round __syncthreads of v7 held 19-25 % of the

@@ -1,9 +1,10 @@
 // gs_raster_bwd.cu -- step a8: back-to-front per-pixel backward of the compositing, reduced per (region, Gaussian)
 // before global atomics.
 //
-// Same tile-CTA structure as the forward (gs_raster.cu): one CTA per 16x16 tile, eight warps = its eight 8x4-pixel
-// regions, the tile's list staged once per tile through a three-stage cp.async ring, walked from the deepest blended
-// position of the tile back to the front.  Per warp (evidence: profiles/r1_v3_regions.md -- a register butterfly that
+// Same structure as the forward (gs_raster.cu): one CTA of four warps per HALF tile, a warp = one 8x4-pixel region, the
+// list staged in rounds of 128 entries (GS_BWD_BATCH) through the mbarrier / cp.async ring of gs_raster.cuh -- here two
+// stages and no slack (GS_BWD_RING_STAGES = 2, _DELAY = 0: 12 KB; a deeper ring costs a CTA of occupancy), no block-wide
+// barrier in the loop -- walked from the deepest blended position of the half tile back to the front.  Per warp (evidence: profiles/r1_v3_regions.md -- a register butterfly that
 // reduced the 10 per-Gaussian sums over the lanes was 42 % of the instructions, and parking the 10 values per lane in
 // shared memory made the kernel LSU-bound at 20 wavefronts per (region, Gaussian)):
 //   * PIXEL phase (lane = pixel): walks the region's relevant entries back to front, rebuilds T, and for every Gaussian
