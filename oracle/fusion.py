@@ -67,8 +67,10 @@ def covariance(scales_i, quat_i):
 # extents k s_i component-wise (the paper's interval notation; the Gaussian's rotation is ignored); r_k(u) is the
 # back-projection of pixel u (integer-centred, Q7) at its depth D_k(u) (camera-space z), c_k the camera centre; pixels with
 # depth <= 0 cast no ray; v and k are arguments (unpublished).  The voxel set of a ray is computed by the 3-D DDA
-# (Amanatides & Woo) written out below in fp64, one IEEE operation at a time -- the CUDA path follows the same sequence, so
-# the sets agree bit for bit; `ray_voxels_by_definition` is the independent plain definition used to pin it.
+# (Amanatides & Woo) in fp64; `ray_voxels_by_definition` is the independent plain definition used to pin it.  Which voxels
+# a ray meets is decided by comparisons of crossing parameters; where two crossings coincide to within rounding (a ray
+# through a voxel edge, a surface point on a voxel face) the set is not determined by the mathematics: `free_keys`
+# reports those voxels separately (`ambiguous`), and a second implementation is compared with this one up to them.
 # ----------------------------------------------------------------------------------------------------------------------
 KEY_BIAS = 1 << 20
 
@@ -145,25 +147,20 @@ def ray_voxels_by_definition(c, r, v):
 
 
 def backproject(depth, fx, fy, cx, cy, T_cw, stride=1):
-    """Camera centre c_k and world-space surface points r_k(u) of the pixels (every `stride`-th in x and y) with depth > 0:
-    p_c = ((u - cx) z / fx, (v - cy) z / fy, z), r = R^T (p_c - t)   (world-to-camera pose)."""
+    """Camera centre c_k = -R^T t and world-space surface points r_k(u) = R^T (p_c - t) of the pixels (every `stride`-th in
+    x and y, row by row) with depth > 0, p_c = ((u - cx) z / fx, (v - cy) z / fy, z)   (world-to-camera pose)."""
     depth = np.asarray(depth, np.float64)
     T = np.asarray(T_cw, np.float64).reshape(3, 4)
     R, t = T[:, :3], T[:, 3]
     fx, fy, cx, cy = np.float64(fx), np.float64(fy), np.float64(cx), np.float64(cy)
-    # every sum is written out left to right, one IEEE operation at a time (no library matrix product: its summation order
-    # and use of fused multiply-adds are not defined), so that the CUDA path can follow the same sequence bit for bit
-    c = np.array([-((R[0, a] * t[0] + R[1, a] * t[1]) + R[2, a] * t[2]) for a in range(3)])
+    c = -(R.T @ t)
     H, W = depth.shape
-    pts = []
-    for y in range(0, H, stride):
-        for x in range(0, W, stride):
-            z = depth[y, x]
-            if z > 0.0:
-                pc = ((np.float64(x) - cx) * z / fx, (np.float64(y) - cy) * z / fy, z)
-                q = (pc[0] - t[0], pc[1] - t[1], pc[2] - t[2])
-                pts.append([(R[0, a] * q[0] + R[1, a] * q[1]) + R[2, a] * q[2] for a in range(3)])
-    return c, np.asarray(pts, np.float64).reshape(-1, 3)
+    ys, xs = np.meshgrid(np.arange(0, H, stride), np.arange(0, W, stride), indexing="ij")
+    z = depth[ys, xs]
+    ok = z > 0.0
+    xs, ys, z = xs[ok].astype(np.float64), ys[ok].astype(np.float64), z[ok]
+    pc = np.stack([(xs - cx) * z / fx, (ys - cy) * z / fy, z], axis=1)
+    return c, (pc - t) @ R          # row i: R^T (p_c,i - t)
 
 
 def free_set(depth, fx, fy, cx, cy, T_cw, v, stride=1):
@@ -181,3 +178,99 @@ def retain_mask(means, occ, free, v):
     idx = kappa(means, v)
     keys = pack_key(idx[:, 0], idx[:, 1], idx[:, 2])
     return np.array([(int(q) not in occ) and (int(q) not in free) for q in keys], dtype=bool)
+
+
+
+# ----------------------------------------------------------------------------------------------------------------------
+# The same sets for inputs of the paper's size (a 1200 x 680 depth map, 5 x 10^5 Gaussians): identical definitions, written
+# over arrays of rays / Gaussians instead of Python loops over them.  Pinned against the per-item functions above
+# (tests/test_oracle_fusion_occupancy_pins.py).
+# ----------------------------------------------------------------------------------------------------------------------
+def occupied_keys(means, scales, v, k):
+    """Eq. 20 as a sorted array of unique packed keys: offsets (dx, dy, dz) >= 0 from the lowest voxel of every box, kept
+    where they stay inside that Gaussian's box."""
+    means = np.asarray(means, np.float64); scales = np.asarray(scales, np.float64)
+    if means.shape[0] == 0:
+        return np.zeros(0, np.uint64)
+    lo = kappa(means - np.float64(k) * scales, v)
+    hi = kappa(means + np.float64(k) * scales, v)
+    n = hi - lo + 1
+    out = []
+    small = (n <= 8).all(axis=1)                      # the bulk: one pass per offset; the few large boxes one by one
+    ls, ns = lo[small], n[small]
+    if ls.shape[0]:
+        m = ns.max(axis=0)
+        for dz in range(m[2]):
+            for dy in range(m[1]):
+                for dx in range(m[0]):
+                    w = (dx < ns[:, 0]) & (dy < ns[:, 1]) & (dz < ns[:, 2])
+                    if w.any():
+                        out.append(np.unique(pack_key(ls[w, 0] + dx, ls[w, 1] + dy, ls[w, 2] + dz)))
+    for l, h in zip(lo[~small], hi[~small]):
+        gx, gy, gz = np.meshgrid(*(np.arange(l[a], h[a] + 1) for a in range(3)), indexing="ij")
+        out.append(pack_key(gx.ravel(), gy.ravel(), gz.ravel()))
+    return np.unique(np.concatenate(out))
+
+
+_EPS = np.finfo(np.float64).eps
+
+
+def free_keys(c, pts, v):
+    """Eq. 21 for rays c -> pts[i]: the 3-D DDA of `ray_voxels`, all rays stepped together.  Returns (keys, ambiguous):
+    sorted unique packed keys of the voxels met, and the keys whose membership hinges on a comparison that rounding can
+    turn -- two boundary crossings closer than the crossing parameters are known (either order is a valid walk and the
+    voxel in between differs), or a crossing that close to t = 1 (the end voxel is entered or not).  A crossing parameter
+    t = (boundary - c_a) / d_a computed from c, r that are themselves a few ulp uncertain is known to about
+    tol_a = 64 eps ((|c_a| + |r_a| + v) / |d_a| + 1) + 4 eps n after n steps of accumulation."""
+    c = np.asarray(c, np.float64); r = np.asarray(pts, np.float64).reshape(-1, 3); v = np.float64(v)
+    M = r.shape[0]
+    if M == 0:
+        return np.zeros(0, np.uint64), np.zeros(0, np.uint64)
+    d = r - c
+    idx = np.repeat(np.floor(c / v).astype(np.int64)[None, :], M, axis=0)
+    step = np.sign(d).astype(np.int64)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        nxt = np.where(d > 0, (idx + 1).astype(np.float64) * v, idx.astype(np.float64) * v)
+        t_max = np.where(d != 0, (nxt - c) / d, np.inf)
+        t_delta = np.where(d != 0, v / np.abs(d), np.inf)
+        tol = np.where(d != 0, 64 * _EPS * ((np.abs(c) + np.abs(r) + v) / np.abs(d) + 1.0), 0.0)
+    frac = c / v - np.floor(c / v)
+    start_fragile = bool(((frac < 64 * _EPS * (1 + np.abs(c / v))) | (1 - frac < 64 * _EPS * (1 + np.abs(c / v)))).any())
+    keys = [np.unique(pack_key(idx[:1, 0], idx[:1, 1], idx[:1, 2]))]
+    amb = []
+    alive = np.arange(M)
+    n = 0
+    rows = None
+    while alive.size:
+        tm = t_max[alive]
+        a = np.argmin(tm, axis=1)                    # ties -> lowest axis
+        rows = np.arange(alive.size)
+        t_a = tm[rows, a]
+        slack = tol[alive] + 4 * _EPS * n
+        go = t_a < 1.0
+        # crossings that rounding could reorder or move across t = 1
+        near_end = np.abs(t_a - 1.0) <= slack[rows, a]
+        tm2 = tm.copy(); tm2[rows, a] = np.inf
+        b = np.argmin(tm2, axis=1)
+        t_b = tm2[rows, b]
+        near_tie = go & np.isfinite(t_b) & (t_b - t_a <= slack[rows, a] + slack[rows, b])
+        for sel, ax in ((near_end, a), (near_tie, a), (near_tie, b)):
+            if sel.any():
+                q = idx[alive[sel]].copy()
+                q[np.arange(q.shape[0]), ax[sel]] += step[alive[sel], ax[sel]]
+                amb.append(pack_key(q[:, 0], q[:, 1], q[:, 2]))
+        alive, a = alive[go], a[go]
+        if not alive.size:
+            break
+        rows = np.arange(alive.size)
+        idx[alive, a] += step[alive, a]
+        t_max[alive, a] = t_max[alive, a] + t_delta[alive, a]
+        keys.append(np.unique(pack_key(idx[alive, 0], idx[alive, 1], idx[alive, 2])))
+        n += 1
+        if len(keys) >= 16:
+            keys = [np.unique(np.concatenate(keys))]
+    keys = np.unique(np.concatenate(keys))
+    amb = np.unique(np.concatenate(amb)) if amb else np.zeros(0, np.uint64)
+    if start_fragile:      # the camera centre sits on a voxel face: every ray's first voxel is undetermined
+        amb = keys
+    return keys, amb

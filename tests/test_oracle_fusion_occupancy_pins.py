@@ -92,3 +92,70 @@ def test_backprojection_inverts_the_pinhole_model():
     uu = 7.0 * pc[:, 0] / pc[:, 2] + 2.0; vv = 8.0 * pc[:, 1] / pc[:, 2] + 1.5
     assert np.allclose(uu.reshape(4, 5), np.arange(5)[None, :], atol=1e-10) and np.allclose(vv.reshape(4, 5), np.arange(4)[:, None], atol=1e-10)
     assert np.allclose(pc[:, 2].reshape(4, 5), depth)
+
+
+# ----------------------------------------------------------------------------------------------------------------------
+# The array forms used at the paper's sizes (occupied_keys, free_keys) against the per-item definitions, and the tie
+# analysis of free_keys on rays built to be degenerate.
+# ----------------------------------------------------------------------------------------------------------------------
+def test_occupied_keys_equals_the_per_gaussian_definition():
+    r = np.random.Generator(np.random.PCG64(11))
+    m = r.uniform(-1, 1, (400, 3)); s = np.exp(r.normal(-4, 0.6, (400, 3)))
+    s[3] = [0.3, 0.2, 0.1]; s[77] = [0.001, 0.5, 0.001]                    # large boxes take the one-by-one branch
+    for v, k in ((0.02, 1.5), (0.05, 3.0), (1.0, 0.0)):
+        want = np.array(sorted(of.occupied_set(m, s, v, k)), np.uint64)
+        assert np.array_equal(of.occupied_keys(m, s, v, k), want)
+    assert of.occupied_keys(np.zeros((0, 3)), np.zeros((0, 3)), 0.02, 1.0).size == 0
+
+
+def test_free_keys_equals_the_per_ray_dda_and_the_plain_definition():
+    from scipy.spatial.transform import Rotation
+    r = np.random.Generator(np.random.PCG64(12))
+    R = Rotation.random(random_state=13).as_matrix(); t = r.normal(size=3)
+    depth = r.uniform(0.4, 3.0, (19, 31)); depth[r.uniform(size=depth.shape) < 0.2] = 0.0
+    for stride, v in ((1, 0.05), (3, 0.11)):
+        c, pts = of.backproject(depth, 30.0, 31.0, 15.25, 9.0, np.concatenate([R, t[:, None]], 1), stride)
+        keys, amb = of.free_keys(c, pts, v)
+        per_ray, by_def = set(), set()
+        for p in pts:
+            per_ray |= {int(of.pack_key(*q)) for q in of.ray_voxels(c, p, v)}
+            by_def |= {int(of.pack_key(*q)) for q in of.ray_voxels_by_definition(c, p, v)}
+        assert set(map(int, keys)) == per_ray == by_def and amb.size == 0      # generic rays: nothing hinges on rounding
+    k0, a0 = of.free_keys(np.zeros(3), np.zeros((0, 3)), 0.1)
+    assert k0.size == 0 and a0.size == 0
+
+
+def test_free_keys_reports_the_voxels_that_hinge_on_a_tie():
+    key = lambda *q: int(of.pack_key(*q))
+    # through the voxel edge x = 1, y = 1 (both crossings at t = 0.25): the walk goes (0,0,0) -> (1,0,0) -> (1,1,0) -> ...
+    # but (0,1,0) instead of (1,0,0) is as valid; both are reported, the unambiguous voxels are not
+    keys, amb = of.free_keys([0.5, 0.5, 0.5], [[2.5, 2.5, 0.5]], 1.0)
+    assert {key(0, 0, 0), key(1, 1, 0), key(2, 2, 0)} <= set(map(int, keys))
+    assert {key(1, 0, 0), key(0, 1, 0)} <= set(map(int, amb)) and key(0, 0, 0) not in set(map(int, amb))
+    # surface point exactly on the face x = 3 (t = 1 there): the end voxel (3,0,0) is not entered, and is reported
+    keys, amb = of.free_keys([0.5, 0.5, 0.5], [[3.0, 0.5, 0.5]], 1.0)
+    assert set(map(int, keys)) == {key(0, 0, 0), key(1, 0, 0), key(2, 0, 0)} and set(map(int, amb)) == {key(3, 0, 0)}
+    # the same two rays moved off the degenerate position by 1e-6: nothing is reported
+    keys, amb = of.free_keys([0.5, 0.5, 0.5], [[2.5, 2.5 + 1e-6, 0.5], [3.0 - 1e-6, 0.5, 0.5]], 1.0)
+    assert amb.size == 0
+    # a camera centre on a voxel face makes every first voxel undetermined
+    keys, amb = of.free_keys([1.0, 0.5, 0.5], [[2.5, 0.7, 0.5]], 1.0)
+    assert np.array_equal(keys, amb)
+
+
+def test_backprojection_is_the_matrix_form():
+    """c = -R^T t and r = R^T (p_c - t) written with matrix products equal the component sums (to rounding)."""
+    from scipy.spatial.transform import Rotation
+    r = np.random.Generator(np.random.PCG64(14))
+    R = Rotation.random(random_state=15).as_matrix(); t = r.normal(size=3)
+    depth = r.uniform(0.5, 3, (6, 7)); depth[2, 3] = 0.0; depth[5, 6] = -1.0
+    c, pts = of.backproject(depth, 7.0, 8.0, 2.0, 1.5, np.concatenate([R, t[:, None]], 1), 2)
+    want = []
+    for y in range(0, 6, 2):
+        for x in range(0, 7, 2):
+            z = depth[y, x]
+            if z > 0:
+                pc = np.array([(x - 2.0) * z / 7.0, (y - 1.5) * z / 8.0, z])
+                want.append([sum(R[b, a] * (pc[b] - t[b]) for b in range(3)) for a in range(3)])
+    assert pts.shape == (len(want), 3) and np.allclose(pts, want, rtol=0, atol=1e-14)
+    assert np.allclose(c, [-sum(R[b, a] * t[b] for b in range(3)) for a in range(3)], rtol=0, atol=1e-15)
