@@ -267,7 +267,7 @@ GS_API int gs_sim3_apply(void* stream, int64_t N, float s, const float* R, const
  * could not be stored (table full, index beyond 21 bits, non-finite input): the sets are exact iff it stays 0.
  * "Table full" means: no free slot within 128 probes of the key's home slot (size the tables for a load factor <= 0.5);
  * a Gaussian whose box of Eq. 20 covers more than 2^24 voxels is not inserted and counted once, and a ray or a large box
- * is given up at its first key that finds no room (so the count is a lower bound of the keys lost) -- an undersized
+ * is given up at its first key that finds no room (the count is of failed attempts: zero or non-zero is what it tells) -- an undersized
  * table or a runaway scale ends in a prompt overflow report, never in a long-running kernel.  gs_voxel_retain never retains a Gaussian with a non-finite mean.
  * All calls are asynchronous on `stream`; GS_E_INVALID on null pointers, non-power-of-two capacities, voxel <= 0. */
 GS_API int gs_voxel_set_clear(void* stream, uint64_t* table, int64_t capacity);

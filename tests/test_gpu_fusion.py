@@ -48,11 +48,23 @@ def test_sim3_apply_matches_oracle(case):
 
 
 # ----------------------------------------------------------------------------------------------------------------------
-# Eqs. 20-22: occupancy sets and the retain test -- BIT-EXACT against oracle/fusion.py (set contents as sorted key lists,
-# retain masks, order-preserving compaction)
+# Eqs. 20-22: occupancy sets and the retain test against oracle/fusion.py (set contents as sorted key lists, retain
+# masks, order-preserving compaction).  O_occ, retain masks and index lists are bit-exact.  O_free is compared up to the
+# voxels the oracle reports as undetermined by the mathematics (two boundary crossings, or a crossing and t = 1, closer
+# than rounding resolves: free_keys' `ambiguous`): the symmetric difference must lie inside that set, and the set must be
+# tiny -- on generic inputs it is empty, so the comparison is exact in practice and says so when it is not.
 # ----------------------------------------------------------------------------------------------------------------------
 def _f32(x):
     return np.ascontiguousarray(x, np.float32)
+
+
+def _assert_equal_up_to_ties(got, keys, amb, rays):
+    diff = np.setxor1d(got, keys)
+    print(f"free set: {len(keys)} keys, {len(amb)} ambiguous, {len(diff)} differ")
+    assert np.isin(diff, amb).all(), (len(diff), len(amb))
+    # a ray steps ~10^2 times and a step is ambiguous with probability ~10^-12 (tolerance / spread of the crossing
+    # parameters): anything beyond a handful means the tolerance or one of the two walks is wrong
+    assert len(amb) <= 8 + rays // 100_000
 
 
 def test_occupied_set_matches_oracle_bit_exact():
@@ -89,14 +101,14 @@ def test_free_set_matches_oracle_bit_exact(stride):
     depth = _f32(r.uniform(0.4, 3.0, (H, W)))
     depth[r.uniform(size=(H, W)) < 0.15] = 0.0       # invalid pixels cast no ray
     v = np.float32(0.05)
-    want = np.array(sorted(of.free_set(depth, np.float32(cam.fx), np.float32(cam.fy), np.float32(cam.cx), np.float32(cam.cy),
-                                       _f32(cam.T_cw), float(v), stride)), np.uint64)
+    c, pts = of.backproject(depth, np.float32(cam.fx), np.float32(cam.fy), np.float32(cam.cx), np.float32(cam.cy),
+                            _f32(cam.T_cw), stride)
+    keys, amb = of.free_keys(c, pts, float(v))
     vs = b.VoxelSet(1 << 18)
     vs.insert_rays(cam, torch.from_numpy(depth).cuda(), v, stride)
     torch.cuda.synchronize()
     assert int(vs.overflow.item()) == 0
-    got = vs.keys()
-    assert len(got) == len(want) and np.array_equal(got, want)
+    _assert_equal_up_to_ties(vs.keys(), keys, amb, len(pts))
 
 
 def test_retain_and_compaction_config5_shaped():
@@ -233,3 +245,62 @@ def test_non_finite_gaussians_are_counted_and_never_retained():
     torch.cuda.synchronize()
     finite = np.isfinite(m2).all(1)
     assert np.array_equal(retain.cpu().numpy().astype(bool), finite) and (~finite).sum() == 3
+
+
+def test_free_set_of_a_full_size_depth_map():
+    """Eq. 21 at the paper's keyframe size: every pixel of a 1200 x 680 depth map casts a ray (stride 1)."""
+    import torch
+    from oracle import fusion as of
+    from paper_2605_10760_b200 import binding as b, scenes
+    r = np.random.Generator(np.random.PCG64(71))
+    W, H = 1200, 680
+    cam = scenes.Camera(W, H, 600.0, 600.0, 599.5, 339.5,
+                        scenes.perturb_pose(scenes.look_at([0.3, -0.2, 1.4], [4.0, 1.0, 1.1]), r.normal(0, 0.05, 6)))
+    # a room-like depth: smooth walls 2..6 m away, objects in front of them, pixel noise, 5 % invalid pixels
+    yy, xx = np.meshgrid(np.linspace(-1, 1, H), np.linspace(-1, 1, W), indexing="ij")
+    depth = 4.0 + 1.5 * np.sin(2.1 * xx + 0.3) * np.cos(1.3 * yy) + 0.4 * xx * yy
+    depth[(np.abs(xx - 0.2) < 0.25) & (np.abs(yy + 0.1) < 0.4)] = 1.3
+    depth = _f32(depth + r.normal(0, 0.01, depth.shape))
+    depth[r.uniform(size=depth.shape) < 0.05] = 0.0
+    v = np.float32(0.08)
+    c, pts = of.backproject(depth, np.float32(cam.fx), np.float32(cam.fy), np.float32(cam.cx), np.float32(cam.cy), _f32(cam.T_cw), 1)
+    keys, amb = of.free_keys(c, pts, float(v))
+    assert len(pts) > 0.9 * W * H and len(keys) > 50_000
+    vs = b.VoxelSet(1 << 21)
+    vs.insert_rays(cam, torch.from_numpy(depth).cuda(), v, 1)
+    torch.cuda.synchronize()
+    assert int(vs.overflow.item()) == 0
+    _assert_equal_up_to_ties(vs.keys(), keys, amb, len(pts))
+
+
+def test_occupied_set_of_half_a_million_gaussians_and_a_nearly_full_table():
+    """Eq. 20 for a config-4-sized map (500 k Gaussians, Replica-shaped scales), bit-exact; then the same keys into a table
+    only ~1.2 x their number: either everything fits within the probe window (exact set, no overflow) or the overflow is
+    reported and nothing foreign was stored."""
+    import torch
+    from oracle import fusion as of
+    from paper_2605_10760_b200 import binding as b, scenes
+    sc = scenes.replica_scene(seed=69, N=500_000)
+    v, k = np.float32(0.04), np.float32(2.0)
+    want = of.occupied_keys(sc.means, sc.scales, float(v), float(k))
+    dm, dsc = torch.from_numpy(sc.means).cuda(), torch.from_numpy(sc.scales).cuda()
+    vs = b.VoxelSet(1 << 20)                         # load factor ~0.4
+    vs.insert_boxes(dm, dsc, v, k)
+    torch.cuda.synchronize()
+    assert 300_000 < len(want) < 500_000
+    assert int(vs.overflow.item()) == 0 and np.array_equal(vs.keys(), want)
+    tight = b.VoxelSet(1 << 19)                      # load factor ~0.8: probe windows of 128 slots start to fill up
+    tight.insert_boxes(dm, dsc, v, k)
+    torch.cuda.synchronize()
+    got, ov = tight.keys(), int(tight.overflow.item())
+    print(f"nearly full table: {len(got)} of {len(want)} keys stored, overflow {ov}")
+    assert np.isin(got, want).all()
+    assert (ov == 0 and np.array_equal(got, want)) or (ov > 0 and len(got) < len(want))
+    # the retain test against the roomy set: bit-exact for 500 k borrowed Gaussians (vectorised form of Eq. 22)
+    src = _f32(sc.means + np.random.Generator(np.random.PCG64(70)).normal(0, 0.05, sc.means.shape))
+    idx = of.kappa(src, float(v))
+    want_retain = ~np.isin(of.pack_key(idx[:, 0], idx[:, 1], idx[:, 2]), want)
+    retain = torch.empty(src.shape[0], dtype=torch.uint8, device="cuda")
+    b.gs_voxel_retain(vs, None, v, torch.from_numpy(src).cuda(), retain)
+    torch.cuda.synchronize()
+    assert np.array_equal(retain.cpu().numpy().astype(bool), want_retain) and 0.05 < want_retain.mean() < 0.95
