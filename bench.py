@@ -611,6 +611,21 @@ def run_config_subrecords(args, budget_s: float = 150.0):
             out[name] = rec
         except Exception as e:   # a sub-record must never cost the headline line
             out[name] = {"error": f"{type(e).__name__}: {str(e)[:200]}"}
+    # the kernels of SURVEY.md section 8(f), each alone (bench.py --workload next), compact: time and HBM fraction
+    left = budget_s - (time.perf_counter() - t_start)
+    if left < 20.0:
+        out["next"] = {"skipped": "time budget of the sub-records used up"}
+    else:
+        try:
+            r = subprocess.run([sys.executable, os.path.abspath(__file__), "--workload", "next", "--steps", "10"],
+                               capture_output=True, text=True, timeout=left)
+            d = json.loads(r.stdout.strip().splitlines()[-1])
+            out["next"] = {"what": "SURVEY.md 8(f) kernels, each alone, L2 flushed between launches; ms = median device time per call",
+                           "hbm_peak_gbs": d["hbm_peak_gbs"],
+                           "kernels": {k: {kk: v[kk] for kk in ("ms", "algorithmic_bytes", "frac_hbm", "mrays_per_s") if kk in v}
+                                       for k, v in d["kernels"].items()}}
+        except Exception as e:
+            out["next"] = {"error": f"{type(e).__name__}: {str(e)[:200]}"}
     return out
 
 
@@ -754,6 +769,95 @@ def run_peaks(args):
                       "driver_file": load_measured_peaks_file()}))
 
 
+def run_next(args):
+    """bench.py --workload next: device time of the kernels of SURVEY.md section 8(f) (losses, optimiser, compaction, ray
+    casting) at the sizes of configs 3 / 5, each alone, CUDA events on the launching stream, L2 flushed between launches
+    (a 256 MB fill), against the HBM copy peak where the kernel streams (algorithmic bytes stated per entry)."""
+    import torch
+    from paper_2605_10760_b200 import binding as B
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    pf = load_measured_peaks_file()
+    hbm = float(pf["hbm_gbs"]) if pf else B.gs_measure_peaks(0)["hbm_copy_gbs"]
+    flush = torch.empty(64 * 1024 * 1024, dtype=torch.float32, device=dev)
+    r = np.random.Generator(np.random.PCG64(123))
+    rep = max(3, min(args.steps, 10))
+    out = {}
+
+    def timed(name, fn, nbytes, note, reset=None):
+        ms = []
+        for it in range(rep + 2):
+            if reset is not None:
+                reset()
+            flush.fill_(1.0)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); fn(); e1.record()
+            torch.cuda.synchronize()
+            if it >= 2:
+                ms.append(e0.elapsed_time(e1))
+        t = float(np.median(ms))
+        rec = {"ms": t, "launches_timed": rep, "note": note}
+        if nbytes:
+            rec.update({"algorithmic_bytes": int(nbytes), "gbs": nbytes / t / 1e6, "frac_hbm": nbytes / t / 1e6 / hbm})
+        out[name] = rec
+
+    W, H = 1200, 680
+    P = W * H
+    f = lambda *shape: torch.from_numpy(r.uniform(0, 1, shape).astype(np.float32)).to(dev)
+    rgb, trgb, depth, tdep = f(3, H, W), f(3, H, W), f(H, W) * 5, f(H, W) * 5
+    d_rgb, d_depth = torch.empty_like(rgb), torch.empty_like(depth)
+    loss = torch.zeros(10, dtype=torch.float64, device=dev)
+    timed("gs_loss_map", lambda: B.gs_loss_map(rgb, depth, trgb, tdep, 0.9, 0.1, d_rgb, d_depth, loss), 48 * P,
+          "Eq. 4 L1 terms at 1200x680: 32 B read + 16 B written per pixel")
+    ab, g_ab, work = torch.zeros(2, device=dev), torch.zeros(2, device=dev), torch.empty(9 * P, device=dev)
+    timed("gs_loss_refine", lambda: B.gs_loss_refine(rgb, depth, trgb, tdep, ab, 1.75, 0.2, 0.25, d_rgb, d_depth, g_ab, work, loss),
+          48 * P, "Eq. 23 exposure + L1 + SSIM (11x11 separable) + depth at 1200x680, three launches; bytes = images in + "
+                  "gradients out only (the SSIM planes in `work` are extra traffic, so frac_hbm understates the bytes moved)")
+    # optimiser at the fused map's size (config 5: 2 M Gaussians, SH3)
+    N, K = 2_000_000, 16
+    shapes = dict(means=(N, 3), scales=(N, 3), quats=(N, 4), opacities=(N,), sh=(N, K, 3))
+    mk = lambda lo, hi: {k: torch.empty(sh, device=dev).uniform_(lo, hi) for k, sh in shapes.items()}
+    params, grads = mk(0.1, 0.9), mk(-1.0, 1.0)
+    m, v = {k: torch.zeros_like(t) for k, t in params.items()}, {k: torch.zeros_like(t) for k, t in params.items()}
+    lrs = dict(means=1.6e-4, scales=5e-3, quats=1e-3, opacities=5e-2, sh=2.5e-3)
+    floats = 11 + 3 * K
+    timed("gs_adam_step_dense_2m", lambda: B.gs_adam_step(params, grads, m, v, lrs, 3, None), 28 * floats * N,
+          "fused Adam on all 2 M Gaussians (SH3): 28 B per parameter float (p, m, v read + written, g read); five launches")
+    vis = (torch.rand(N, device=dev) < 0.3).to(torch.int32)
+    nv = int(vis.sum().item())
+    timed("gs_adam_step_masked_2m", lambda: B.gs_adam_step(params, grads, m, v, lrs, 3, vis), 28 * floats * nv + 4 * N,
+          f"the same with a visibility mask ({nv} of {N} visible, scattered): bytes of the visible rows + the mask")
+    ids = torch.nonzero(vis).flatten().to(torch.int32)
+    n_rows = torch.tensor([nv], dtype=torch.int32, device=dev)
+    sgrads = {k: torch.empty((nv,) + tuple(sh[1:]), device=dev).uniform_(-1, 1) for k, sh in shapes.items()}
+    timed("gs_adam_step_sparse_2m", lambda: B.gs_adam_step_sparse(params, sgrads, m, v, lrs, 3, ids.data_ptr(), n_rows.data_ptr(), nv),
+          28 * floats * nv + 4 * nv, "GS_SPARSE_GRADS rows (compact gradient rows, id list): bytes of the visible rows + ids")
+    # pruning: mask, plan, gather of the SH array
+    keep = torch.empty(N, dtype=torch.uint8, device=dev)
+    timed("gs_prune_mask_2m", lambda: B.gs_prune_mask(params["opacities"], 0.3, keep), 5 * N, "4 B read + 1 B written per Gaussian")
+    index, n_kept = torch.empty(N, dtype=torch.int32, device=dev), torch.zeros(1, dtype=torch.int64, device=dev)
+    timed("gs_compact_plan_static_2m", lambda: B.gs_compact_plan_static(keep, index, n_kept), 6 * N,
+          "keep mask read twice (count, index) + 4 B index written per Gaussian; three launches, scratch inside the library")
+    kept = int(n_kept.item())
+    dst = torch.empty((kept, K, 3), device=dev)
+    lib = B.load_library()
+    timed("gs_compact_rows_sh_2m", lambda: lib.gs_compact_rows(B._stream(), N, 3 * K, B._ptr(index), B._ptr(params["sh"]), B._ptr(dst)),
+          4 * N + 4 * 3 * K * (N + kept), f"SH rows (192 B) of {kept} kept Gaussians gathered in order: all rows read, kept rows written")
+    # Eq. 21 on one keyframe depth map
+    cam = scenes.Camera(W, H, 600.0, 600.0, 599.5, 339.5, scenes.look_at([0.3, -0.2, 1.4], [4.0, 1.0, 1.1]))
+    yy, xx = np.meshgrid(np.linspace(-1, 1, H), np.linspace(-1, 1, W), indexing="ij")
+    dm = torch.from_numpy((4.0 + 1.5 * np.sin(2.1 * xx + 0.3) * np.cos(1.3 * yy)).astype(np.float32)).to(dev)
+    vs = B.VoxelSet(1 << 22)
+    steps_per_ray = float((dm / 0.05).mean().item()) * 1.5
+    timed("gs_voxel_insert_rays_1200x680", lambda: vs.insert_rays(cam, dm, 0.05, 1), 0,
+          f"Eq. 21, every pixel casts a ray, v = 5 cm, ~{steps_per_ray:.0f} DDA steps per ray into a 4 Mi-slot set: latency / "
+          "atomics bound, not HBM", reset=vs.clear)
+    out["gs_voxel_insert_rays_1200x680"]["mrays_per_s"] = P / out["gs_voxel_insert_rays_1200x680"]["ms"] / 1e3
+    out["gs_voxel_insert_rays_1200x680"]["keys_stored"] = int(len(vs.keys()))
+    print(json.dumps({"workload": "next", "unit": "ms per call (median)", "hbm_peak_gbs": hbm, "l2": "flushed between launches (256 MB fill)",
+                      "kernels": out}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -781,6 +885,8 @@ def main():
         run_reference(args)
     elif args.workload == "peaks":
         run_peaks(args)
+    elif args.workload == "next":
+        run_next(args)
     else:
         run_ours(args)
 
